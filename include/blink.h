@@ -1,0 +1,170 @@
+/*
+ * blink.h -- C ABI of libblink: the data-parallel hot path of the BLINK high-time-resolution
+ * imager (arxiv 2405.13478; citations are /root/reference/PAPER.md line numbers), hand-written
+ * for NVIDIA B200 (sm_100a).
+ *
+ *   for every (time step t, channel ch) snapshot:
+ *     grid the complex visibilities of all baselines on an N x N uv grid (nearest cell, V and its
+ *     Hermitian conjugate, per-cell weight count)            PAPER.md:348-370 (sec 5.2.1), :211
+ *     -> natural / uniform weighting                           PAPER.md:209-213 (sec 4.4.2), :360
+ *     -> 2-D inverse DFT, fftshift, normalise, real part       PAPER.md:160-176 (Eq. 4-6), :372-376
+ *
+ * Conventions
+ *   - plain C linkage, no exceptions cross the boundary, no torch / C++ types in signatures;
+ *   - every pointer argument says HOST or DEVICE; device pointers are raw CUDA device addresses
+ *     on the current device; `stream` is a cudaStream_t passed as void* (NULL = legacy default);
+ *   - all functions return 0 (BLINK_OK) or a negative blink_status; on error outputs are
+ *     untouched unless stated;
+ *   - complex64 = interleaved float (re, im) pairs, i.e. float2 / cufftComplex layout
+ *     ("gpufftComplex");
+ *   - there is NO CPU fallback: without a CUDA device every call except blink_version,
+ *     blink_strerror and the blink_host_* table helpers returns BLINK_ECUDA.
+ *
+ * Baseline order (cross-correlations only):
+ *   bl(i,j) = i (2 n_ant - i - 1) / 2 + (j - i - 1)  for 0 <= i < j < n_ant,  b_ij = r_j - r_i.
+ *
+ * Cell rule (bit-exact, identical to the oracle; DESIGN.md "Readings" c5-c7):
+ *   sc = freq_hz / 299792458.0;  u = (E_j - E_i) * sc;  v = (N_j - N_i) * sc   (fp64, no FMA)
+ *   G  = (double)n_pix * pixscale            (= 1/du, Eq. 9)
+ *   kx = llround(u * G), ky = llround(v * G) (nearest, ties away from zero)
+ *   kept iff |kx| <= N/2-1 and |ky| <= N/2-1, else the baseline AND its conjugate are dropped
+ *   cell = (ky mod N) * N + (kx mod N)       (FFT-native order, DC at [0][0])
+ *   conjugate cell = ((-ky) mod N) * N + ((-kx) mod N)
+ */
+#ifndef BLINK_H_
+#define BLINK_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BLINK_VERSION 100 /* 0.1.0 */
+
+typedef enum blink_status {
+  BLINK_OK = 0,
+  BLINK_EINVAL = -1, /* bad argument (NULL, odd / unsupported n_pix, n_ant < 2, ...) */
+  BLINK_ENOMEM = -2, /* host or device allocation failed */
+  BLINK_ECUDA = -3,  /* CUDA runtime error or no device (see blink_last_cuda_error) */
+  BLINK_EUNSUPPORTED = -4 /* valid request outside what this build implements */
+} blink_status;
+
+typedef enum blink_weighting {
+  BLINK_NATURAL = 0, /* plain sum per cell; image norm = sum of counts */
+  BLINK_UNIFORM = 1  /* cell sum / cell count; image norm = occupied cells */
+} blink_weighting;
+
+/* `what` selectors of blink_plan_query.  [ch] forms take the channel in the low 16 bits of
+ * `index`.  Device-pointer queries return pointers that stay valid until blink_plan_destroy. */
+typedef enum blink_query {
+  BLINK_Q_N_ANT = 0,      /* out: int32                                            */
+  BLINK_Q_N_BL = 1,       /* out: int32   n_ant (n_ant-1)/2                        */
+  BLINK_Q_N_CH = 2,       /* out: int32                                            */
+  BLINK_Q_N_PIX = 3,      /* out: int32                                            */
+  BLINK_Q_N_DROPPED = 4,  /* out: int64   [ch] baselines outside the grid          */
+  BLINK_Q_WSUM = 5,       /* out: int64   [ch] sum of counts = 2 (n_bl - n_dropped) */
+  BLINK_Q_N_OCC = 6,      /* out: int64   [ch] number of cells with count > 0      */
+  BLINK_Q_BBOX = 7,       /* out: int32[2] [ch] kx_max, ky_max over kept baselines */
+  BLINK_Q_NORM = 8,       /* out: double  [ch] image normalisation (WSUM or N_OCC) */
+  BLINK_Q_CELL_IDX = 9,   /* out: const int32* DEVICE [n_ch][n_bl], cell of V, -1 = dropped */
+  BLINK_Q_COUNTS = 10,    /* out: const uint32* DEVICE [n_ch][N][N] weight counts  */
+  BLINK_Q_IMAGE_PATH = 11,/* out: int32   0 = shared-memory single pass, 1 = two-pass */
+  BLINK_Q_SCRATCH_BYTES = 12 /* out: int64 device scratch currently held by the plan */
+} blink_query;
+
+typedef struct blink_plan blink_plan; /* opaque */
+
+int blink_version(void);
+const char *blink_strerror(int status);
+/* text of the last CUDA error seen by this thread's last failing call ("" if none) */
+const char *blink_last_cuda_error(void);
+
+/*
+ * blink_plan_create -- step a0: uv-index precompute (the paper recomputes
+ * frequency and wavelength per thread per launch; here the fixed array geometry
+ * is exploited once).  Runs the fp64 index kernel on the device, builds the per-channel count grid
+ * (PAPER.md:354), normalisation constants, bounding box and the cell-sorted gather tables used
+ * by blink_grid.
+ *   out         HOST  receives the plan; untouched on error
+ *   ant_enu_m   HOST  [n_ant][3] East, North, Up in metres (Up ignored: coplanar)
+ *   freq_hz     HOST  [n_ch] channel centre frequencies in Hz
+ *   n_pix       grid = image side N; power of two, 32 <= N <= 4096 in this build
+ *   pixscale    pixel size dx in direction-cosine units (all-sky: 2.0 / n_pix; small field:
+ *               radians per pixel); du = 1 / (n_pix * pixscale), Eq. 9
+ *   weighting   blink_weighting
+ *   stream      cudaStream_t for the plan-time kernels / copies; the call synchronises it
+ * Inputs are copied; the caller may free them on return.  The plan owns its device tables.
+ */
+int blink_plan_create(blink_plan **out, const double *ant_enu_m, int n_ant, const double *freq_hz,
+                      int n_ch, int n_pix, double pixscale, int weighting, void *stream);
+
+/* frees the plan and its device memory; NULL is a no-op */
+int blink_plan_destroy(blink_plan *plan);
+
+/* read-only view of plan facts; `out` HOST, sized per blink_query */
+int blink_plan_query(const blink_plan *plan, int what, int index, void *out);
+
+/*
+ * blink_grid -- steps a1/a2: gridding.  For each snapshot s = t*n_ch + ch:
+ *   uv_grid[s][cell(bl)] += vis[s][bl];  uv_grid[s][cell*(bl)] += conj(vis[s][bl])
+ * over all kept baselines, every other cell = 0.  Unweighted sums regardless of the plan's
+ * weighting.  The per-cell summation order is fixed (ascending baseline index), so the result is
+ * bit-reproducible run to run -- the deterministic reduction the paper plans.
+ *   vis      DEVICE complex64 [n_t][n_ch][n_bl], baseline fastest; 16-byte aligned base
+ *   uv_grid  DEVICE complex64 [n_t][n_ch][N][N] row-major [ky][kx], FFT-native order (DC at
+ *            [0][0]); COMPLETELY overwritten, zeros included (no memset needed); 16-byte aligned
+ *   n_t      number of time steps in this call (any >= 0; 0 is a no-op)
+ * Asynchronous on `stream`; no allocation, no host synchronisation.  Caller owns both buffers.
+ */
+int blink_grid(const blink_plan *plan, const void *vis, int n_t, void *uv_grid, void *stream);
+
+/*
+ * blink_image -- steps a3-a5:
+ *   G'  = uv_grid (natural) or uv_grid / count where count > 0 (uniform)
+ *   img[s][y][x] = Re sum_{ky,kx} G'[ky][kx] exp(+2 pi i (kx (x-N/2) + ky (y-N/2)) / N) / norm[ch]
+ * i.e. unnormalised inverse DFT, fftshift so pixel (N/2, N/2) is the phase centre
+ * (l = (x-N/2) dx East, m = (y-N/2) dx North), 1/norm, real part.
+ *   uv_grid  DEVICE complex64 [n_t][n_ch][N][N], const (never used as scratch).  CONTRACT: cells
+ *            outside the plan's bounding box (|kx| > kx_max or |ky| > ky_max, BLINK_Q_BBOX) must be
+ *            zero -- true of every blink_grid output -- and are not read.  Inside the box any
+ *            values are accepted; the real part of the transform is formed exactly, i.e. a
+ *            non-Hermitian grid is symmetrised, (G[k] + conj(G[-k])) / 2.
+ *   images   DEVICE float32 [n_t][n_ch][N][N] row-major [y][x]; completely overwritten
+ * Asynchronous on `stream`.  May grow the plan's internal device scratch on first use with a
+ * larger n_t (the only allocation; query BLINK_Q_SCRATCH_BYTES) -- call blink_plan_reserve first
+ * to keep the hot call allocation-free.
+ */
+int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *images, void *stream);
+
+/*
+ * blink_plan_read -- copies one channel's slice of a plan table to HOST memory (synchronous):
+ *   what = BLINK_Q_CELL_IDX -> int32 [n_bl];  what = BLINK_Q_COUNTS -> uint32 [N*N].
+ * `bytes` must equal the slice size.  This is how a harness checks indices and counts bit-exactly.
+ */
+int blink_plan_read(const blink_plan *plan, int what, int ch, void *dst_host, size_t bytes);
+
+/* pre-allocates whatever scratch blink_image needs for up to n_t time steps per call */
+int blink_plan_reserve(blink_plan *plan, int n_t);
+
+/*
+ * Host-side table helper, exported so the host logic is testable without a GPU.
+ * Builds the cell-sorted gather tables blink_grid uses from per-baseline cell indices of ONE
+ * channel (as returned by BLINK_Q_CELL_IDX): every kept baseline contributes once to its
+ * canonical cell (the member of {cell, cell*} in the half-plane ky > 0 or ky == 0, kx >= 0), as V
+ * or as conj(V).  Entries are sorted by (canonical cell, baseline).
+ *   cell        HOST int32 [n_bl], -1 = dropped
+ *   n_can_out   HOST number of distinct canonical cells
+ *   can_cell    HOST int32 [n_bl]   out: canonical cell index per segment (first n_can valid)
+ *   seg_start   HOST int32 [n_bl+1] out: CSR offsets into src (first n_can+1 valid)
+ *   src         HOST int32 [n_bl]   out: (baseline << 1) | conj_flag, n_kept entries
+ * Returns the number of kept baselines or a negative blink_status.
+ */
+int blink_host_build_gather(const int32_t *cell, int n_bl, int n_pix, int32_t *n_can_out,
+                            int32_t *can_cell, int32_t *seg_start, int32_t *src);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BLINK_H_ */

@@ -1,0 +1,203 @@
+"""Thin Python binding over the C-ABI library libblink.so (include/blink.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels behind the C ABI.
+PyTorch is used for device memory and streams, nothing else.  There is no fallback of any kind: if
+libblink.so is missing or was not built, importing/using this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libblink.so")
+
+NATURAL, UNIFORM = 0, 1
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
+(Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
+ Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES) = range(13)
+
+EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create",
+           "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
+           "blink_grid",
+           "blink_image", "blink_host_build_gather"]
+
+_lib = None
+
+
+class BlinkError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        lib = load()
+        msg = lib.blink_strerror(status).decode()
+        cuda = lib.blink_last_cuda_error().decode()
+        super().__init__(f"{what}: {msg} ({status})" + (f" [{cuda}]" if cuda else ""))
+        self.status = status
+
+
+def load() -> ctypes.CDLL:
+    """dlopen libblink.so (raises if it has not been built; there is no other path)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: run `python -m paper_2405_13478_b200.build` "
+                          "(nvcc, sm_100a); there is no CPU or PyTorch fallback")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    lib.blink_version.restype = ci
+    lib.blink_strerror.restype = ctypes.c_char_p
+    lib.blink_strerror.argtypes = [ci]
+    lib.blink_last_cuda_error.restype = ctypes.c_char_p
+    lib.blink_plan_create.restype = ci
+    lib.blink_plan_create.argtypes = [ctypes.POINTER(vp), vp, ci, vp, ci, ci, cd, ci, vp]
+    lib.blink_plan_destroy.restype = ci
+    lib.blink_plan_destroy.argtypes = [vp]
+    lib.blink_plan_query.restype = ci
+    lib.blink_plan_query.argtypes = [vp, ci, ci, vp]
+    lib.blink_plan_read.restype = ci
+    lib.blink_plan_read.argtypes = [vp, ci, ci, vp, ctypes.c_size_t]
+    lib.blink_plan_reserve.restype = ci
+    lib.blink_plan_reserve.argtypes = [vp, ci]
+    lib.blink_grid.restype = ci
+    lib.blink_grid.argtypes = [vp, vp, ci, vp, vp]
+    lib.blink_image.restype = ci
+    lib.blink_image.argtypes = [vp, vp, ci, vp, vp]
+    lib.blink_host_build_gather.restype = ci
+    lib.blink_host_build_gather.argtypes = [vp, ci, ci, vp, vp, vp, vp]
+    _lib = lib
+    return lib
+
+
+def _check(status: int, what: str):
+    if status != OK:
+        raise BlinkError(status, what)
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def host_build_gather(cell: np.ndarray, n_pix: int):
+    """blink_host_build_gather: cell-sorted gather tables of one channel (host logic, no GPU)."""
+    lib = load()
+    cell = np.ascontiguousarray(cell, np.int32)
+    n_bl = cell.shape[0]
+    n_can = ctypes.c_int32(0)
+    can_cell = np.zeros(max(n_bl, 1), np.int32)
+    seg = np.zeros(n_bl + 1, np.int32)
+    src = np.zeros(max(n_bl, 1), np.int32)
+    rc = lib.blink_host_build_gather(cell.ctypes.data, n_bl, int(n_pix), ctypes.byref(n_can),
+                                     can_cell.ctypes.data, seg.ctypes.data, src.ctypes.data)
+    if rc < 0:
+        raise BlinkError(rc, "blink_host_build_gather")
+    n = n_can.value
+    return dict(n_kept=rc, n_can=n, can_cell=can_cell[:n], seg_start=seg[:n + 1], src=src[:rc])
+
+
+class Plan:
+    """blink_plan_create / blink_plan_destroy and the calls that take a plan."""
+
+    def __init__(self, ant_enu_m, freq_hz, n_pix: int, pixscale: float, weighting: int = NATURAL,
+                 stream=None):
+        lib = load()
+        ant = np.ascontiguousarray(ant_enu_m, np.float64)
+        fr = np.ascontiguousarray(freq_hz, np.float64).reshape(-1)
+        if ant.ndim != 2 or ant.shape[1] != 3:
+            raise ValueError("ant_enu_m must be [n_ant, 3]")
+        self._h = ctypes.c_void_p(None)
+        self._lib = lib
+        _check(lib.blink_plan_create(ctypes.byref(self._h), ant.ctypes.data, ant.shape[0],
+                                     fr.ctypes.data, fr.shape[0], int(n_pix), float(pixscale),
+                                     int(weighting), _stream_ptr(stream)), "blink_plan_create")
+        self.n_ant, self.n_ch, self.n_pix = ant.shape[0], fr.shape[0], int(n_pix)
+        self.n_bl = self.query_i32(Q_N_BL)
+        self.weighting = int(weighting)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.blink_plan_destroy(self._h)
+            self._h = ctypes.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- queries
+    def _query(self, what, index, ctype, n=1):
+        buf = (ctype * n)()
+        _check(self._lib.blink_plan_query(self._h, what, index, ctypes.byref(buf)), "blink_plan_query")
+        return buf[0] if n == 1 else list(buf)
+
+    def query_i32(self, what, index=0):
+        return int(self._query(what, index, ctypes.c_int32))
+
+    def query_i64(self, what, index=0):
+        return int(self._query(what, index, ctypes.c_int64))
+
+    def n_dropped(self, ch):
+        return self.query_i64(Q_N_DROPPED, ch)
+
+    def wsum(self, ch):
+        return self.query_i64(Q_WSUM, ch)
+
+    def n_occ(self, ch):
+        return self.query_i64(Q_N_OCC, ch)
+
+    def bbox(self, ch):
+        return tuple(self._query(Q_BBOX, ch, ctypes.c_int32, 2))
+
+    def norm(self, ch):
+        return float(self._query(Q_NORM, ch, ctypes.c_double))
+
+    def _read(self, what, ch, n, dtype):
+        out = np.empty(n, dtype)
+        _check(self._lib.blink_plan_read(self._h, what, int(ch), out.ctypes.data, out.nbytes),
+               "blink_plan_read")
+        return out
+
+    def cell_idx(self, ch):
+        """int32 [n_bl] cell of V per baseline of channel ch (-1 dropped), host copy."""
+        return self._read(Q_CELL_IDX, ch, self.n_bl, np.int32)
+
+    def counts(self, ch):
+        """uint32 [N, N] weight counts of channel ch, host copy."""
+        return self._read(Q_COUNTS, ch, self.n_pix * self.n_pix, np.uint32).reshape(self.n_pix, self.n_pix)
+
+    # ---- hot path
+    def reserve(self, n_t: int):
+        _check(self._lib.blink_plan_reserve(self._h, int(n_t)), "blink_plan_reserve")
+
+    def grid(self, vis, uv_grid=None, stream=None):
+        """blink_grid: vis complex64 cuda [n_t, n_ch, n_bl] -> uv_grid complex64 [n_t, n_ch, N, N]."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        n_t = vis.shape[0]
+        assert tuple(vis.shape[1:]) == (self.n_ch, self.n_bl)
+        if uv_grid is None:
+            uv_grid = torch.empty((n_t, self.n_ch, self.n_pix, self.n_pix), dtype=torch.complex64,
+                                  device=vis.device)
+        assert uv_grid.is_cuda and uv_grid.dtype == torch.complex64 and uv_grid.is_contiguous()
+        assert tuple(uv_grid.shape) == (n_t, self.n_ch, self.n_pix, self.n_pix)
+        _check(self._lib.blink_grid(self._h, vis.data_ptr(), n_t, uv_grid.data_ptr(),
+                                    _stream_ptr(stream)), "blink_grid")
+        return uv_grid
+
+    def image(self, uv_grid, images=None, stream=None):
+        """blink_image: uv_grid complex64 [n_t, n_ch, N, N] -> images float32 [n_t, n_ch, N, N]."""
+        import torch
+        assert uv_grid.is_cuda and uv_grid.dtype == torch.complex64 and uv_grid.is_contiguous()
+        n_t = uv_grid.shape[0]
+        assert tuple(uv_grid.shape[1:]) == (self.n_ch, self.n_pix, self.n_pix)
+        if images is None:
+            images = torch.empty((n_t, self.n_ch, self.n_pix, self.n_pix), dtype=torch.float32,
+                                 device=uv_grid.device)
+        assert images.is_cuda and images.dtype == torch.float32 and images.is_contiguous()
+        _check(self._lib.blink_image(self._h, uv_grid.data_ptr(), n_t, images.data_ptr(),
+                                     _stream_ptr(stream)), "blink_image")
+        return images

@@ -1,0 +1,225 @@
+// blink_image.cu -- steps a3-a5: weighting, batched 2-D inverse FFT, fftshift, normalisation, real
+// part (the paper calls cufftPlanMany / ExecC2C, then takes the real part
+// and shifts in separate steps).  Hand-written Stockham transforms (fft_core.cuh), fused with
+// everything around them:
+//
+//   pass A (columns, along ky): reads only the half-plane kx = 0..kx_max of the plan's bounding box
+//     and its mirror, forms H = (G[k] + conj(G[-k])) / 2 -- so the REAL PART of the transform is
+//     produced by a Hermitian (half-size) transform --, applies the uniform weight 1/count, the
+//     normalisation 1/norm and the fftshift as the sign (-1)^(kx+ky) ON LOAD, then U[y][kx] =
+//     sum_ky H[ky][kx] w^(ky y).
+//   pass B (rows, along kx): two real rows per complex transform: Z = U[y] + i U[y'] extended by
+//     Hermitian symmetry, z = IFFT(Z), image[y] = Re z, image[y'] = Im z, stored coalesced straight
+//     from the last butterfly stage.
+//
+// U lives in a small plan-owned scratch (two-pass path) sized to stay L2-resident between the two
+// launches of a chunk of snapshots.
+#include <algorithm>
+
+#include "blink_internal.h"
+#include "fft_core.cuh"
+
+namespace blink {
+using namespace blinkfft;
+
+template <int N> struct ImgCfg {
+  static constexpr int T = N / 16;                                   // threads per transform
+  static constexpr int CT = (N <= 1024) ? 16 : (N == 2048 ? 8 : 4);  // columns per CTA, pass A
+  static constexpr int RP0 = (N <= 256) ? (256 / T) : (512 / T);
+  static constexpr int RP = RP0 < N / 2 ? RP0 : N / 2;                // row pairs per CTA, pass B
+  static constexpr int LS = ((LineSize<N>::value + 15) / 16) * 16 + 1;  // line stride, = 1 mod 16
+  static constexpr int THREADS_A = CT * T;
+  static constexpr int THREADS_B = RP * T;
+};
+
+struct ImgParams {
+  const float2 *uv;
+  float *img;
+  float2 *U;
+  const ChannelInfo *chinfo;
+  const uint32_t *counts;
+  const float2 *tw;
+  int n_ch, wu, uniform, snap_base;
+};
+
+// run stages 1.. of the transform; stage 0's load is done by the caller
+template <int N, class Store>
+__device__ __forceinline__ void fft_tail(cf32 *v, int t, cf32 *line, const cf32 *__restrict__ tw, Store st) {
+  using F = Fft<N>;
+  auto lds = [&](int idx) { return line[pad16(idx)]; };
+  auto sts = [&](int idx, cf32 x) { line[pad16(idx)] = x; };
+  F::template compute<0>(v, t, tw);
+  F::template store<0>(v, t, sts);
+  __syncthreads();
+  F::template load<1>(v, t, lds);
+  F::template compute<1>(v, t, tw);
+  if constexpr (F::NSTAGE == 2) {
+    F::template store<1>(v, t, st);
+  } else {
+    __syncthreads();
+    F::template store<1>(v, t, sts);
+    __syncthreads();
+    F::template load<2>(v, t, lds);
+    F::template compute<2>(v, t, tw);
+    F::template store<2>(v, t, st);
+  }
+}
+
+template <int N>
+__global__ void __launch_bounds__(ImgCfg<N>::THREADS_A) k_image_cols(const ImgParams p) {
+  using C = ImgCfg<N>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cf32 *lines = reinterpret_cast<cf32 *>(smem_raw);
+  const int tid = threadIdx.x;
+  const int sl = blockIdx.y, s = p.snap_base + sl, ch = s % p.n_ch;
+  const ChannelInfo ci = p.chinfo[ch];
+  const int kx0 = blockIdx.x * C::CT;
+  const float2 *__restrict__ G = p.uv + (size_t)s * N * N;
+
+  for (int i = tid; i < C::CT * C::LS; i += C::THREADS_A) lines[i] = mk(0.f, 0.f);
+  __syncthreads();
+  const int nrow = 2 * ci.ky_max + 1;
+  const uint32_t *__restrict__ cnt = p.counts + (size_t)ch * N * N;
+  for (int e = tid; e < nrow * C::CT; e += C::THREADS_A) {
+    const int c = e % C::CT, ky = e / C::CT - ci.ky_max, kx = kx0 + c;
+    if (kx > ci.kx_max) continue;
+    const int iy = (ky + N) & (N - 1);
+    const float2 a = __ldg(G + (size_t)iy * N + kx);
+    const float2 b = __ldg(G + (size_t)((N - iy) & (N - 1)) * N + ((N - kx) & (N - 1)));
+    float w = 0.5f * ci.inv_norm;
+    if (p.uniform) {
+      const uint32_t n = __ldg(cnt + (size_t)iy * N + kx);
+      w = n ? w / (float)n : 0.f;
+    }
+    if ((kx + ky) & 1) w = -w;
+    lines[c * C::LS + pad16(iy)] = mk((a.x + b.x) * w, (a.y - b.y) * w);
+  }
+  __syncthreads();
+
+  const int c = tid % C::CT, t = tid / C::CT;
+  cf32 *line = lines + c * C::LS;
+  cf32 v[16];
+  Fft<N>::template load<0>(v, t, [&](int idx) { return line[pad16(idx)]; });
+  __syncthreads();
+  float2 *__restrict__ U = p.U + (size_t)sl * N * p.wu + kx0 + c;
+  fft_tail<N>(v, t, line, p.tw, [&](int y, cf32 x) { U[(size_t)y * p.wu] = x; });
+}
+
+template <int N>
+__global__ void __launch_bounds__(ImgCfg<N>::THREADS_B) k_image_rows(const ImgParams p) {
+  using C = ImgCfg<N>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cf32 *lines = reinterpret_cast<cf32 *>(smem_raw);
+  const int tid = threadIdx.x;
+  const int sl = blockIdx.y, s = p.snap_base + sl, ch = s % p.n_ch;
+  const int kxm = p.chinfo[ch].kx_max;
+  const int pr = tid / C::T, t = tid % C::T;
+  const int y0 = blockIdx.x * C::RP + pr, y1 = y0 + N / 2;
+  const float2 *__restrict__ U0 = p.U + ((size_t)sl * N + y0) * p.wu;
+  const float2 *__restrict__ U1 = p.U + ((size_t)sl * N + y1) * p.wu;
+  cf32 *line = lines + pr * C::LS;
+  cf32 v[16];
+  Fft<N>::template load<0>(v, t, [&](int idx) {
+    if (idx <= kxm) {
+      const float2 a = U0[idx], b = U1[idx];
+      return mk(a.x - b.y, a.y + b.x);             // a + i b
+    } else if (idx >= N - kxm) {
+      const float2 a = U0[N - idx], b = U1[N - idx];
+      return mk(a.x + b.y, b.x - a.y);             // conj(a) + i conj(b)
+    }
+    return mk(0.f, 0.f);
+  });
+  float *__restrict__ r0 = p.img + ((size_t)s * N + y0) * N;
+  float *__restrict__ r1 = p.img + ((size_t)s * N + y1) * N;
+  fft_tail<N>(v, t, line, p.tw, [&](int x, cf32 z) { r0[x] = z.x; r1[x] = z.y; });
+}
+
+template <int N> static int run_image_n(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st) {
+  using C = ImgCfg<N>;
+  const size_t smem_a = sizeof(cf32) * C::CT * C::LS, smem_b = sizeof(cf32) * C::RP * C::LS;
+  static thread_local bool attr_done = false;
+  if (!attr_done) {
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_image_cols<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a),
+                   "k_image_cols smem attribute");
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_image_rows<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b),
+                   "k_image_rows smem attribute");
+    attr_done = true;
+  }
+  const int chunk = std::max(1, p->chunk_snapshots);
+  for (int base = 0; base < n_snap; base += chunk) {
+    const int cs = std::min(chunk, n_snap - base);
+    ip.snap_base = base;
+    k_image_cols<N><<<dim3(p->wu / C::CT, cs), C::THREADS_A, smem_a, st>>>(ip);
+    k_image_rows<N><<<dim3(N / 2 / C::RP, cs), C::THREADS_B, smem_b, st>>>(ip);
+  }
+  BLINK_CUDA_TRY(cudaGetLastError(), "k_image launch");
+  return BLINK_OK;
+}
+
+static int cols_per_cta(int N) { return N <= 1024 ? 16 : (N == 2048 ? 8 : 4); }
+
+int image_setup(blink_plan *p) {
+  const int ct = cols_per_cta(p->n_pix);
+  p->wu = ((p->kx_max_all + 1 + ct - 1) / ct) * ct;
+  p->image_path = 1;
+  // chunk of snapshots whose U scratch stays L2-resident between the two passes
+  size_t budget = 48u << 20;
+  if (const char *e = getenv("BLINK_IMAGE_CHUNK_MB")) {
+    long mb = atol(e);
+    if (mb > 0) budget = (size_t)mb << 20;
+  }
+  const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
+  p->chunk_snapshots = (int)std::max<size_t>(1, budget / per_snap);
+  return BLINK_OK;
+}
+
+int image_reserve(blink_plan *p, int n_t) {
+  const long long n_snap = (long long)n_t * p->n_ch;
+  const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
+  const size_t need = per_snap * (size_t)std::min<long long>(std::max<long long>(n_snap, 1), p->chunk_snapshots);
+  if (need <= p->scratch_bytes) return BLINK_OK;
+  if (p->d_scratch) {
+    BLINK_CUDA_TRY(cudaDeviceSynchronize(), "scratch regrow sync");
+    cudaFree(p->d_scratch);
+    p->d_scratch = nullptr;
+    p->scratch_bytes = 0;
+  }
+  cudaError_t e = cudaMalloc((void **)&p->d_scratch, need);
+  if (e != cudaSuccess) {
+    set_cuda_error(e, "scratch cudaMalloc");
+    return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
+  }
+  p->scratch_bytes = need;
+  return BLINK_OK;
+}
+
+int launch_image(const blink_plan *p, const float2 *uv, int n_t, float *img, cudaStream_t st) {
+  ImgParams ip;
+  ip.uv = uv; ip.img = img; ip.U = p->d_scratch; ip.chinfo = p->d_chinfo; ip.counts = p->d_counts;
+  ip.tw = p->d_tw; ip.n_ch = p->n_ch; ip.wu = p->wu; ip.uniform = p->weighting == BLINK_UNIFORM;
+  ip.snap_base = 0;
+  const int n_snap = n_t * p->n_ch;
+  switch (p->n_pix) {
+    case 32: return run_image_n<32>(p, ip, n_snap, st);
+    case 64: return run_image_n<64>(p, ip, n_snap, st);
+    case 128: return run_image_n<128>(p, ip, n_snap, st);
+    case 256: return run_image_n<256>(p, ip, n_snap, st);
+    case 512: return run_image_n<512>(p, ip, n_snap, st);
+    case 1024: return run_image_n<1024>(p, ip, n_snap, st);
+    case 2048: return run_image_n<2048>(p, ip, n_snap, st);
+    case 4096: return run_image_n<4096>(p, ip, n_snap, st);
+    default: return BLINK_EUNSUPPORTED;
+  }
+}
+
+}  // namespace blink
+
+extern "C" int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *images, void *stream) {
+  if (!plan || n_t < 0) return BLINK_EINVAL;
+  if (n_t == 0) return BLINK_OK;
+  if (!uv_grid || !images) return BLINK_EINVAL;
+  if (((uintptr_t)uv_grid & 7) || ((uintptr_t)images & 3)) return BLINK_EINVAL;
+  int rc = blink::image_reserve(const_cast<blink_plan *>(plan), n_t);
+  if (rc != BLINK_OK) return rc;
+  return blink::launch_image(plan, (const float2 *)uv_grid, n_t, (float *)images, (cudaStream_t)stream);
+}

@@ -1,0 +1,95 @@
+// blink_internal.h -- plan object shared by the libblink translation units (not part of the ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/blink.h"
+
+namespace blink {
+
+// flags in the high bits of a placement code; low bits = index j of the canonical-cell sum S[j]
+constexpr int kPlaceShift = 28;
+constexpr int32_t kPlaceMask = (1 << kPlaceShift) - 1;
+constexpr int32_t kPlaceDirect = 0;  // grid[cell] = S[j]
+constexpr int32_t kPlaceConj = 1;    // grid[cell] = conj(S[j])
+constexpr int32_t kPlaceBoth = 2;    // grid[cell] = S[j] + conj(S[j])   (self-conjugate cell: DC)
+
+constexpr int kBandCells = 4096;     // cells (complex64) per output band of the gridder = 32 KB
+
+struct ChannelInfo {   // mirrored on the device, one per channel
+  int32_t n_kept;      // baselines inside the grid
+  int32_t n_can;       // distinct canonical (half-plane) cells
+  int32_t n_place;     // occupied cells in the full plane
+  int32_t kx_max, ky_max;
+  float inv_norm;      // 1 / image normalisation
+};
+
+struct HostGather {    // cell-sorted tables of one channel (see blink_host_build_gather)
+  int32_t n_kept = 0, n_can = 0;
+  std::vector<int32_t> can_cell, seg_start, src;
+};
+
+}  // namespace blink
+
+struct blink_plan {
+  int n_ant = 0, n_bl = 0, n_ch = 0, n_pix = 0, weighting = 0;
+  double pixscale = 0.0;
+  int device = 0;
+  int sm_count = 148;
+  int max_smem_optin = 0;
+
+  // per-channel facts (host)
+  std::vector<int64_t> n_dropped, wsum, n_occ;
+  std::vector<double> norm;
+  std::vector<blink::ChannelInfo> chinfo;
+
+  // device tables
+  int32_t *d_cell = nullptr;        // [n_ch][n_bl]
+  uint32_t *d_counts = nullptr;     // [n_ch][N][N]
+  blink::ChannelInfo *d_chinfo = nullptr;  // [n_ch]
+  int32_t *d_src = nullptr;         // [n_ch][n_bl]      (bl << 1) | conj, sorted by (can cell, bl)
+  int32_t *d_seg = nullptr;         // [n_ch][n_bl + 1]  CSR offsets of canonical cells into d_src
+  int32_t *d_pcell = nullptr;       // [n_ch][2 n_bl]    occupied full-plane cells, ascending
+  int32_t *d_pcode = nullptr;       // [n_ch][2 n_bl]    j | flag << kPlaceShift
+  int32_t *d_pband = nullptr;       // [n_ch][n_bands+1] CSR of d_pcell by output band
+  float2 *d_tw = nullptr;           // [N] exp(+2 pi i k / N)
+  int n_bands = 0;                  // bands per snapshot = N*N / band_cells
+  int band_cells = 0;
+  int n_can_max = 0;
+  int kx_max_all = 0, ky_max_all = 0;
+
+  // blink_image scratch (two-pass path): U[chunk][N][wu] complex64
+  int wu = 0;                       // padded half-plane width
+  float2 *d_scratch = nullptr;
+  size_t scratch_bytes = 0;
+  int image_path = 1;
+  int chunk_snapshots = 0;
+};
+
+namespace blink {
+
+void set_cuda_error(cudaError_t e, const char *where);
+int build_gather_host(const int32_t *cell, int n_bl, int n_pix, HostGather &out);
+
+// kernels' host launchers (each returns a blink_status)
+int launch_index_kernel(blink_plan *p, const double *d_ant, const double *d_freq,
+                        const int32_t *d_pi, const int32_t *d_pj, cudaStream_t st);
+int launch_grid(const blink_plan *p, const float2 *vis, int n_t, float2 *uv, cudaStream_t st);
+int launch_image(const blink_plan *p, const float2 *uv, int n_t, float *img, cudaStream_t st);
+int image_setup(blink_plan *p);
+int image_reserve(blink_plan *p, int n_t);
+
+}  // namespace blink
+
+#define BLINK_CUDA_TRY(expr, where)                 \
+  do {                                              \
+    cudaError_t e__ = (expr);                       \
+    if (e__ != cudaSuccess) {                       \
+      blink::set_cuda_error(e__, where);            \
+      return BLINK_ECUDA;                           \
+    }                                               \
+  } while (0)

@@ -1,0 +1,389 @@
+// blink_plan.cu -- plan creation: step a0, the uv-index precompute that exploits the fixed array
+// geometry (the paper recomputes frequency, wavelength and the cell per thread
+// per launch).  The fp64 index kernel and the integer count kernel run on the
+// device; the cell-sorted gather / placement tables that make blink_grid atomic-free and
+// deterministic (the paper's planned "parallel reduction") are sorted on the
+// host once per plan.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "blink_internal.h"
+
+namespace blink {
+
+static thread_local std::string g_cuda_err;
+void set_cuda_error(cudaError_t e, const char *where) {
+  g_cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
+  cudaGetLastError();  // clear sticky-free errors
+}
+
+// ------------------------------------------------------------------------------------------
+// K0: one thread per (channel, baseline).  Operation order is part of the contract (blink.h
+// "Cell rule"): fp64, round-to-nearest intrinsics so that no FMA contraction can occur.
+__global__ void k_uv_index(const double *__restrict__ ant, const int32_t *__restrict__ pi,
+                           const int32_t *__restrict__ pj, const double *__restrict__ freq,
+                           int n_bl, int n_ch, int N, double G, int32_t *__restrict__ cell,
+                           uint32_t *__restrict__ counts) {
+  const int bl = blockIdx.x * blockDim.x + threadIdx.x;
+  const int ch = blockIdx.y;
+  if (bl >= n_bl || ch >= n_ch) return;
+  const double sc = __ddiv_rn(freq[ch], 299792458.0);
+  const int i = pi[bl], j = pj[bl];
+  const double de = __dsub_rn(ant[3 * j + 0], ant[3 * i + 0]);
+  const double dn = __dsub_rn(ant[3 * j + 1], ant[3 * i + 1]);
+  const double u = __dmul_rn(de, sc);
+  const double v = __dmul_rn(dn, sc);
+  const long long kx = llround(__dmul_rn(u, G));
+  const long long ky = llround(__dmul_rn(v, G));
+  const long long kmax = N / 2 - 1;
+  int32_t c = -1;
+  if (kx >= -kmax && kx <= kmax && ky >= -kmax && ky <= kmax) {
+    const int ix = (int)((kx + N) % N), iy = (int)((ky + N) % N);
+    const int cx = (N - ix) % N, cy = (N - iy) % N;
+    c = iy * N + ix;
+    uint32_t *cnt = counts + (size_t)ch * N * N;
+    atomicAdd(cnt + c, 1u);                 // integer atomics: exact, order-independent
+    atomicAdd(cnt + cy * N + cx, 1u);       // ("counter of the number of visibilities")
+  }
+  cell[(size_t)ch * n_bl + bl] = c;
+}
+
+int launch_index_kernel(blink_plan *p, const double *d_ant, const double *d_freq,
+                        const int32_t *d_pi, const int32_t *d_pj, cudaStream_t st) {
+  const int N = p->n_pix;
+  const double G = (double)N * p->pixscale;
+  BLINK_CUDA_TRY(cudaMemsetAsync(p->d_counts, 0, sizeof(uint32_t) * (size_t)p->n_ch * N * N, st),
+                 "memset counts");
+  dim3 grid((p->n_bl + 255) / 256, p->n_ch);
+  k_uv_index<<<grid, 256, 0, st>>>(d_ant, d_pi, d_pj, d_freq, p->n_bl, p->n_ch, N, G, p->d_cell,
+                                   p->d_counts);
+  BLINK_CUDA_TRY(cudaGetLastError(), "k_uv_index launch");
+  return BLINK_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// Host: canonical-cell gather table of one channel.  A kept baseline with cell c (centred
+// coordinates kx, ky) contributes V to c and conj(V) to c*.  Exactly one of {c, c*} lies in the
+// canonical half-plane (ky > 0, or ky == 0 and kx >= 0); the baseline is filed under that cell, as
+// V (flag 0) or conj(V) (flag 1).  Sorting by (canonical cell, baseline) makes every cell's sum
+// a contiguous segment in ascending-baseline order -- the oracle's summation order.
+int build_gather_host(const int32_t *cell, int n_bl, int n_pix, HostGather &out) {
+  const int N = n_pix;
+  struct Ent { int32_t can; int32_t code; };
+  std::vector<Ent> ents;
+  ents.reserve(n_bl);
+  for (int bl = 0; bl < n_bl; ++bl) {
+    const int32_t c = cell[bl];
+    if (c < 0) continue;
+    if (c >= N * N) return BLINK_EINVAL;
+    const int ix = c % N, iy = c / N;
+    const int kx = ix < N / 2 ? ix : ix - N, ky = iy < N / 2 ? iy : iy - N;
+    const bool canonical = (ky > 0) || (ky == 0 && kx >= 0);
+    Ent e;
+    if (canonical) {
+      e.can = c;
+      e.code = (bl << 1);
+    } else {
+      e.can = ((N - iy) % N) * N + ((N - ix) % N);
+      e.code = (bl << 1) | 1;
+    }
+    ents.push_back(e);
+  }
+  std::stable_sort(ents.begin(), ents.end(), [](const Ent &a, const Ent &b) { return a.can < b.can; });
+  out.n_kept = (int32_t)ents.size();
+  out.src.resize(ents.size());
+  out.can_cell.clear();
+  out.seg_start.clear();
+  for (size_t e = 0; e < ents.size(); ++e) {
+    if (e == 0 || ents[e].can != ents[e - 1].can) {
+      out.can_cell.push_back(ents[e].can);
+      out.seg_start.push_back((int32_t)e);
+    }
+    out.src[e] = ents[e].code;
+  }
+  out.seg_start.push_back((int32_t)ents.size());
+  out.n_can = (int32_t)out.can_cell.size();
+  return BLINK_OK;
+}
+
+template <class T> static int dev_alloc(T **p, size_t n) {
+  if (n == 0) n = 1;
+  cudaError_t e = cudaMalloc((void **)p, n * sizeof(T));
+  if (e != cudaSuccess) {
+    set_cuda_error(e, "cudaMalloc");
+    *p = nullptr;
+    return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
+  }
+  return BLINK_OK;
+}
+
+static void plan_free(blink_plan *p) {
+  if (!p) return;
+  cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
+  cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband);
+  cudaFree(p->d_tw); cudaFree(p->d_scratch);
+  delete p;
+}
+
+static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+}  // namespace blink
+
+using namespace blink;
+
+extern "C" int blink_version(void) { return BLINK_VERSION; }
+
+extern "C" const char *blink_strerror(int status) {
+  switch (status) {
+    case BLINK_OK: return "ok";
+    case BLINK_EINVAL: return "invalid argument";
+    case BLINK_ENOMEM: return "out of memory";
+    case BLINK_ECUDA: return "CUDA error or no CUDA device";
+    case BLINK_EUNSUPPORTED: return "not supported by this build";
+    default: return "unknown status";
+  }
+}
+
+extern "C" const char *blink_last_cuda_error(void) { return g_cuda_err.c_str(); }
+
+extern "C" int blink_host_build_gather(const int32_t *cell, int n_bl, int n_pix, int32_t *n_can_out,
+                                       int32_t *can_cell, int32_t *seg_start, int32_t *src) {
+  if (!cell || n_bl < 0 || n_pix < 2 || (n_pix & 1) || !n_can_out || !can_cell || !seg_start || !src)
+    return BLINK_EINVAL;
+  HostGather g;
+  int rc = build_gather_host(cell, n_bl, n_pix, g);
+  if (rc != BLINK_OK) return rc;
+  *n_can_out = g.n_can;
+  std::copy(g.can_cell.begin(), g.can_cell.end(), can_cell);
+  std::copy(g.seg_start.begin(), g.seg_start.end(), seg_start);
+  std::copy(g.src.begin(), g.src.end(), src);
+  return g.n_kept;
+}
+
+extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int n_ant,
+                                 const double *freq_hz, int n_ch, int n_pix, double pixscale,
+                                 int weighting, void *stream) {
+  if (!out || !ant_enu_m || !freq_hz || n_ant < 2 || n_ant > 4096 || n_ch < 1 || n_ch > 65535 ||
+      !(pixscale > 0.0) || (weighting != BLINK_NATURAL && weighting != BLINK_UNIFORM))
+    return BLINK_EINVAL;
+  if (n_pix < 2 || (n_pix & 1)) return BLINK_EINVAL;
+  if (!is_pow2(n_pix) || n_pix < 32 || n_pix > 4096) return BLINK_EUNSUPPORTED;
+  for (int c = 0; c < n_ch; ++c)
+    if (!(freq_hz[c] > 0.0)) return BLINK_EINVAL;
+
+  int dev = 0;
+  BLINK_CUDA_TRY(cudaGetDevice(&dev), "cudaGetDevice");
+  cudaStream_t st = (cudaStream_t)stream;
+  blink_plan *p = new (std::nothrow) blink_plan();
+  if (!p) return BLINK_ENOMEM;
+  p->device = dev;
+  p->n_ant = n_ant;
+  p->n_bl = n_ant * (n_ant - 1) / 2;
+  p->n_ch = n_ch;
+  p->n_pix = n_pix;
+  p->pixscale = pixscale;
+  p->weighting = weighting;
+  cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  const int N = n_pix, n_bl = p->n_bl;
+  const size_t NN = (size_t)N * N;
+
+#define PLAN_TRY(expr)        \
+  do {                        \
+    int rc__ = (expr);        \
+    if (rc__ != BLINK_OK) {   \
+      plan_free(p);           \
+      return rc__;            \
+    }                         \
+  } while (0)
+#define PLAN_CUDA(expr, where)              \
+  do {                                      \
+    cudaError_t e__ = (expr);               \
+    if (e__ != cudaSuccess) {               \
+      set_cuda_error(e__, where);           \
+      plan_free(p);                         \
+      return BLINK_ECUDA;                   \
+    }                                       \
+  } while (0)
+
+  // ---- inputs to the device, K0 --------------------------------------------------------
+  std::vector<int32_t> pi(n_bl), pj(n_bl);
+  {
+    int bl = 0;
+    for (int i = 0; i < n_ant; ++i)
+      for (int j = i + 1; j < n_ant; ++j, ++bl) { pi[bl] = i; pj[bl] = j; }
+  }
+  double *d_ant = nullptr, *d_freq = nullptr;
+  int32_t *d_pi = nullptr, *d_pj = nullptr;
+  PLAN_TRY(dev_alloc(&p->d_cell, (size_t)n_ch * n_bl));
+  PLAN_TRY(dev_alloc(&p->d_counts, (size_t)n_ch * NN));
+  int rc = BLINK_OK;
+  if ((rc = dev_alloc(&d_ant, (size_t)3 * n_ant)) || (rc = dev_alloc(&d_freq, (size_t)n_ch)) ||
+      (rc = dev_alloc(&d_pi, (size_t)n_bl)) || (rc = dev_alloc(&d_pj, (size_t)n_bl))) {
+    cudaFree(d_ant); cudaFree(d_freq); cudaFree(d_pi); cudaFree(d_pj);
+    plan_free(p);
+    return rc;
+  }
+  std::vector<int32_t> h_cell((size_t)n_ch * n_bl);
+  cudaError_t ce = cudaSuccess;
+  auto step = [&](cudaError_t e) { if (ce == cudaSuccess) ce = e; };
+  step(cudaMemcpyAsync(d_ant, ant_enu_m, sizeof(double) * 3 * n_ant, cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(d_freq, freq_hz, sizeof(double) * n_ch, cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(d_pi, pi.data(), sizeof(int32_t) * n_bl, cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(d_pj, pj.data(), sizeof(int32_t) * n_bl, cudaMemcpyHostToDevice, st));
+  if (ce == cudaSuccess) rc = launch_index_kernel(p, d_ant, d_freq, d_pi, d_pj, st);
+  step(cudaMemcpyAsync(h_cell.data(), p->d_cell, sizeof(int32_t) * h_cell.size(),
+                       cudaMemcpyDeviceToHost, st));
+  step(cudaStreamSynchronize(st));
+  cudaFree(d_ant); cudaFree(d_freq); cudaFree(d_pi); cudaFree(d_pj);
+  if (rc != BLINK_OK) { plan_free(p); return rc; }
+  PLAN_CUDA(ce, "plan upload / index kernel");
+
+  // ---- host: per-channel facts, gather and placement tables -------------------------------
+  p->band_cells = (int)std::min<size_t>(NN, (size_t)kBandCells);
+  p->n_bands = (int)(NN / p->band_cells);
+  p->n_dropped.assign(n_ch, 0); p->wsum.assign(n_ch, 0); p->n_occ.assign(n_ch, 0);
+  p->norm.assign(n_ch, 0.0); p->chinfo.assign(n_ch, ChannelInfo());
+  std::vector<int32_t> h_src((size_t)n_ch * n_bl, 0), h_seg((size_t)n_ch * (n_bl + 1), 0);
+  std::vector<int32_t> h_pcell((size_t)n_ch * 2 * n_bl, 0), h_pcode((size_t)n_ch * 2 * n_bl, 0);
+  std::vector<int32_t> h_pband((size_t)n_ch * (p->n_bands + 1), 0);
+  for (int ch = 0; ch < n_ch; ++ch) {
+    HostGather g;
+    PLAN_TRY(build_gather_host(h_cell.data() + (size_t)ch * n_bl, n_bl, N, g));
+    ChannelInfo &ci = p->chinfo[ch];
+    ci.n_kept = g.n_kept;
+    ci.n_can = g.n_can;
+    p->n_dropped[ch] = n_bl - g.n_kept;
+    p->wsum[ch] = 2 * (int64_t)g.n_kept;
+    std::copy(g.src.begin(), g.src.end(), h_src.begin() + (size_t)ch * n_bl);
+    std::copy(g.seg_start.begin(), g.seg_start.end(), h_seg.begin() + (size_t)ch * (n_bl + 1));
+    // placement: every canonical cell and its mirror, sorted by full-plane cell index
+    std::vector<std::pair<int32_t, int32_t>> pl;
+    pl.reserve(2 * (size_t)g.n_can);
+    int kxm = 0, kym = 0;
+    for (int j = 0; j < g.n_can; ++j) {
+      const int c = g.can_cell[j], ix = c % N, iy = c / N;
+      const int kx = ix < N / 2 ? ix : ix - N, ky = iy;  // canonical: ky >= 0
+      kxm = std::max(kxm, std::abs(kx));
+      kym = std::max(kym, ky);
+      const int cc = ((N - iy) % N) * N + ((N - ix) % N);
+      if (cc == c) {
+        pl.push_back({c, j | (kPlaceBoth << kPlaceShift)});
+      } else {
+        pl.push_back({c, j | (kPlaceDirect << kPlaceShift)});
+        pl.push_back({cc, j | (kPlaceConj << kPlaceShift)});
+      }
+    }
+    std::sort(pl.begin(), pl.end());
+    ci.n_place = (int32_t)pl.size();
+    ci.kx_max = kxm;
+    ci.ky_max = kym;
+    p->n_occ[ch] = ci.n_place;
+    p->norm[ch] = weighting == BLINK_NATURAL ? (double)p->wsum[ch] : (double)p->n_occ[ch];
+    ci.inv_norm = p->norm[ch] > 0.0 ? (float)(1.0 / p->norm[ch]) : 0.0f;
+    int32_t *pb = h_pband.data() + (size_t)ch * (p->n_bands + 1);
+    size_t e = 0;
+    for (int b = 0; b < p->n_bands; ++b) {
+      pb[b] = (int32_t)e;
+      const int64_t hi = (int64_t)(b + 1) * p->band_cells;
+      while (e < pl.size() && pl[e].first < hi) ++e;
+    }
+    pb[p->n_bands] = (int32_t)pl.size();
+    for (size_t k = 0; k < pl.size(); ++k) {
+      h_pcell[(size_t)ch * 2 * n_bl + k] = pl[k].first;
+      h_pcode[(size_t)ch * 2 * n_bl + k] = pl[k].second;
+    }
+    p->n_can_max = std::max(p->n_can_max, (int)g.n_can);
+    p->kx_max_all = std::max(p->kx_max_all, kxm);
+    p->ky_max_all = std::max(p->ky_max_all, kym);
+  }
+  if (p->n_can_max > kPlaceMask) { plan_free(p); return BLINK_EUNSUPPORTED; }
+
+  // twiddles exp(+2 pi i k / N), fp64 -> fp32
+  std::vector<float2> h_tw(N);
+  for (int k = 0; k < N; ++k) {
+    const double a = 2.0 * 3.14159265358979323846264338327950288 * (double)k / (double)N;
+    h_tw[k] = make_float2((float)cos(a), (float)sin(a));
+  }
+
+  PLAN_TRY(dev_alloc(&p->d_chinfo, (size_t)n_ch));
+  PLAN_TRY(dev_alloc(&p->d_src, h_src.size()));
+  PLAN_TRY(dev_alloc(&p->d_seg, h_seg.size()));
+  PLAN_TRY(dev_alloc(&p->d_pcell, h_pcell.size()));
+  PLAN_TRY(dev_alloc(&p->d_pcode, h_pcode.size()));
+  PLAN_TRY(dev_alloc(&p->d_pband, h_pband.size()));
+  PLAN_TRY(dev_alloc(&p->d_tw, (size_t)N));
+  step(cudaMemcpyAsync(p->d_chinfo, p->chinfo.data(), sizeof(ChannelInfo) * n_ch, cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_src, h_src.data(), sizeof(int32_t) * h_src.size(), cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_seg, h_seg.data(), sizeof(int32_t) * h_seg.size(), cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_pcell, h_pcell.data(), sizeof(int32_t) * h_pcell.size(), cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_pcode, h_pcode.data(), sizeof(int32_t) * h_pcode.size(), cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_pband, h_pband.data(), sizeof(int32_t) * h_pband.size(), cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_tw, h_tw.data(), sizeof(float2) * N, cudaMemcpyHostToDevice, st));
+  step(cudaStreamSynchronize(st));
+  PLAN_CUDA(ce, "plan table upload");
+  PLAN_TRY(image_setup(p));
+#undef PLAN_TRY
+#undef PLAN_CUDA
+  *out = p;
+  return BLINK_OK;
+}
+
+extern "C" int blink_plan_destroy(blink_plan *plan) {
+  plan_free(plan);
+  return BLINK_OK;
+}
+
+extern "C" int blink_plan_reserve(blink_plan *plan, int n_t) {
+  if (!plan || n_t < 0) return BLINK_EINVAL;
+  return image_reserve(plan, n_t);
+}
+
+extern "C" int blink_plan_read(const blink_plan *p, int what, int ch, void *dst, size_t bytes) {
+  if (!p || !dst || ch < 0 || ch >= p->n_ch) return BLINK_EINVAL;
+  const void *src = nullptr;
+  size_t need = 0;
+  if (what == BLINK_Q_CELL_IDX) {
+    need = sizeof(int32_t) * (size_t)p->n_bl;
+    src = p->d_cell + (size_t)ch * p->n_bl;
+  } else if (what == BLINK_Q_COUNTS) {
+    need = sizeof(uint32_t) * (size_t)p->n_pix * p->n_pix;
+    src = p->d_counts + (size_t)ch * p->n_pix * p->n_pix;
+  } else {
+    return BLINK_EINVAL;
+  }
+  if (bytes != need) return BLINK_EINVAL;
+  BLINK_CUDA_TRY(cudaMemcpy(dst, src, need, cudaMemcpyDeviceToHost), "blink_plan_read");
+  return BLINK_OK;
+}
+
+extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *out) {
+  if (!p || !out) return BLINK_EINVAL;
+  const int ch = index & 0xffff;
+  const bool per_ch = what == BLINK_Q_N_DROPPED || what == BLINK_Q_WSUM || what == BLINK_Q_N_OCC ||
+                      what == BLINK_Q_BBOX || what == BLINK_Q_NORM;
+  if (per_ch && ch >= p->n_ch) return BLINK_EINVAL;
+  switch (what) {
+    case BLINK_Q_N_ANT: *(int32_t *)out = p->n_ant; break;
+    case BLINK_Q_N_BL: *(int32_t *)out = p->n_bl; break;
+    case BLINK_Q_N_CH: *(int32_t *)out = p->n_ch; break;
+    case BLINK_Q_N_PIX: *(int32_t *)out = p->n_pix; break;
+    case BLINK_Q_N_DROPPED: *(int64_t *)out = p->n_dropped[ch]; break;
+    case BLINK_Q_WSUM: *(int64_t *)out = p->wsum[ch]; break;
+    case BLINK_Q_N_OCC: *(int64_t *)out = p->n_occ[ch]; break;
+    case BLINK_Q_BBOX:
+      ((int32_t *)out)[0] = p->chinfo[ch].kx_max;
+      ((int32_t *)out)[1] = p->chinfo[ch].ky_max;
+      break;
+    case BLINK_Q_NORM: *(double *)out = p->norm[ch]; break;
+    case BLINK_Q_CELL_IDX: *(const int32_t **)out = p->d_cell; break;
+    case BLINK_Q_COUNTS: *(const uint32_t **)out = p->d_counts; break;
+    case BLINK_Q_IMAGE_PATH: *(int32_t *)out = p->image_path; break;
+    case BLINK_Q_SCRATCH_BYTES: *(int64_t *)out = (int64_t)p->scratch_bytes; break;
+    default: return BLINK_EINVAL;
+  }
+  return BLINK_OK;
+}

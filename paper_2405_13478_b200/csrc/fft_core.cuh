@@ -1,0 +1,173 @@
+// fft_core.cuh -- register/shared-memory Stockham building blocks for the batched inverse FFT
+// (step a4; the paper calls cuFFT/hipFFT PlanMany + ExecC2C, this is the
+// hand-written replacement).  Inverse direction only: X[n] = sum_k x[k] exp(+2 pi i k n / N)
+// (sign from Eq. 4-5), unnormalised.
+//
+// Every thread owns E = 16 complex points of one length-N transform (T = N/16 threads per
+// transform).  A transform is 2 or 3 radix-{2,4,8,16} Stockham autosort stages; between stages the
+// points are exchanged through a padded shared-memory line.  The per-thread phases (load / twiddle
+// + butterfly / store) are plain inline functions usable from host code too, so the index algebra
+// is unit-tested on the CPU (tests/host_fft_check.cpp) before it ever runs on a GPU.
+#pragma once
+
+#if defined(__CUDACC__)
+#define BLINK_HD __host__ __device__ __forceinline__
+#include <cuda_runtime.h>
+typedef float2 cf32;
+#else
+#define BLINK_HD inline
+struct cf32 { float x, y; };
+#endif
+
+namespace blinkfft {
+
+BLINK_HD cf32 mk(float x, float y) { cf32 r; r.x = x; r.y = y; return r; }
+BLINK_HD cf32 cadd(cf32 a, cf32 b) { return mk(a.x + b.x, a.y + b.y); }
+BLINK_HD cf32 csub(cf32 a, cf32 b) { return mk(a.x - b.x, a.y - b.y); }
+BLINK_HD cf32 cmul(cf32 a, cf32 b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+BLINK_HD cf32 cconj(cf32 a) { return mk(a.x, -a.y); }
+BLINK_HD cf32 mul_i(cf32 a) { return mk(-a.y, a.x); }   // a * (+i)
+
+#define BLINK_SQRT1_2 0.70710678118654752440f
+#define BLINK_COS_PI_8 0.92387953251128675613f
+#define BLINK_SIN_PI_8 0.38268343236508977173f
+
+// ---- inverse DFT butterflies, natural-order in, natural-order out --------------------------
+BLINK_HD void dft2(cf32 &a, cf32 &b) {
+  cf32 t = a;
+  a = cadd(t, b);
+  b = csub(t, b);
+}
+
+BLINK_HD void dft4(cf32 &a, cf32 &b, cf32 &c, cf32 &d) {
+  cf32 t0 = cadd(a, c), t1 = csub(a, c), t2 = cadd(b, d), t3 = mul_i(csub(b, d));
+  a = cadd(t0, t2);
+  c = csub(t0, t2);
+  b = cadd(t1, t3);
+  d = csub(t1, t3);
+}
+
+BLINK_HD void dft8(cf32 *v) {  // v[0..7]
+  cf32 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6];
+  cf32 o0 = v[1], o1 = v[3], o2 = v[5], o3 = v[7];
+  dft4(e0, e1, e2, e3);
+  dft4(o0, o1, o2, o3);
+  // o[k] *= w8^k, w8 = exp(+i pi/4)
+  o1 = mk(BLINK_SQRT1_2 * (o1.x - o1.y), BLINK_SQRT1_2 * (o1.x + o1.y));
+  o2 = mul_i(o2);
+  o3 = mk(-BLINK_SQRT1_2 * (o3.x + o3.y), BLINK_SQRT1_2 * (o3.x - o3.y));
+  v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+  v[1] = cadd(e1, o1); v[5] = csub(e1, o1);
+  v[2] = cadd(e2, o2); v[6] = csub(e2, o2);
+  v[3] = cadd(e3, o3); v[7] = csub(e3, o3);
+}
+
+BLINK_HD void dft16(cf32 *v) {  // v[0..15]
+  cf32 e[8], o[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { e[k] = v[2 * k]; o[k] = v[2 * k + 1]; }
+  dft8(e);
+  dft8(o);
+  // o[k] *= w16^k, w16 = exp(+i pi/8) = (C, S)
+  const float C = BLINK_COS_PI_8, S = BLINK_SIN_PI_8, Q = BLINK_SQRT1_2;
+  o[1] = cmul(o[1], mk(C, S));
+  o[2] = mk(Q * (o[2].x - o[2].y), Q * (o[2].x + o[2].y));
+  o[3] = cmul(o[3], mk(S, C));
+  o[4] = mul_i(o[4]);
+  o[5] = cmul(o[5], mk(-S, C));
+  o[6] = mk(-Q * (o[6].x + o[6].y), Q * (o[6].x - o[6].y));
+  o[7] = cmul(o[7], mk(-C, S));
+#pragma unroll
+  for (int k = 0; k < 8; ++k) { v[k] = cadd(e[k], o[k]); v[k + 8] = csub(e[k], o[k]); }
+}
+
+template <int R> BLINK_HD void dft(cf32 *v);
+template <> BLINK_HD void dft<2>(cf32 *v) { dft2(v[0], v[1]); }
+template <> BLINK_HD void dft<4>(cf32 *v) { dft4(v[0], v[1], v[2], v[3]); }
+template <> BLINK_HD void dft<8>(cf32 *v) { dft8(v); }
+template <> BLINK_HD void dft<16>(cf32 *v) { dft16(v); }
+
+// ---- per-N stage plan ------------------------------------------------------------------------
+template <int N> struct Radices;
+template <> struct Radices<32>   { static constexpr int n = 2, r0 = 16, r1 = 2,  r2 = 1; };
+template <> struct Radices<64>   { static constexpr int n = 2, r0 = 16, r1 = 4,  r2 = 1; };
+template <> struct Radices<128>  { static constexpr int n = 2, r0 = 16, r1 = 8,  r2 = 1; };
+template <> struct Radices<256>  { static constexpr int n = 2, r0 = 16, r1 = 16, r2 = 1; };
+template <> struct Radices<512>  { static constexpr int n = 3, r0 = 16, r1 = 8,  r2 = 4; };
+template <> struct Radices<1024> { static constexpr int n = 3, r0 = 16, r1 = 8,  r2 = 8; };
+template <> struct Radices<2048> { static constexpr int n = 3, r0 = 16, r1 = 16, r2 = 8; };
+template <> struct Radices<4096> { static constexpr int n = 3, r0 = 16, r1 = 16, r2 = 16; };
+
+// shared-memory line padding: one extra complex slot per 16 keeps the stride-16 scatter of the
+// first stage and the unit-stride gathers of later stages both conflict-free for 8-byte accesses
+BLINK_HD int pad16(int i) { return i + (i >> 4); }
+template <int N> struct LineSize { static constexpr int value = N + N / 16; };
+
+template <int N> struct Fft {
+  static constexpr int E = 16;
+  static constexpr int T = N / E;  // threads per transform
+  using RD = Radices<N>;
+  static constexpr int NSTAGE = RD::n;
+
+  template <int S> static constexpr int radix() { return S == 0 ? RD::r0 : (S == 1 ? RD::r1 : RD::r2); }
+  template <int S> static constexpr int ns() { return S == 0 ? 1 : (S == 1 ? RD::r0 : RD::r0 * RD::r1); }
+
+  // Phase 1 of stage S: v[b*R + r] = in[j + r * N/R], j = t + b*T.  `ld(idx)` returns the point
+  // at natural index idx of this stage's input.
+  template <int S, class Load> BLINK_HD static void load(cf32 *v, int t, Load ld) {
+    constexpr int R = radix<S>();
+#pragma unroll
+    for (int b = 0; b < E / R; ++b) {
+      const int j = t + b * T;
+#pragma unroll
+      for (int r = 0; r < R; ++r) v[b * R + r] = ld(j + r * (N / R));
+    }
+  }
+
+  // Phase 2 of stage S: twiddle by w_{Ns R}^{r k}, k = j mod Ns, then the radix-R butterfly.
+  // tw[m] = exp(+2 pi i m / N), m = 0..N-1.  Powers of the base twiddle are formed by a
+  // depth <= 4 product tree from one table lookup.
+  template <int S> BLINK_HD static void compute(cf32 *v, int t, const cf32 *tw) {
+    constexpr int R = radix<S>();
+    constexpr int Ns = ns<S>();
+#pragma unroll
+    for (int b = 0; b < E / R; ++b) {
+      cf32 *x = v + b * R;
+      if (Ns > 1) {
+        const int j = t + b * T;
+        const int k = j & (Ns - 1);
+        cf32 w[R > 1 ? R : 2];
+        w[1] = tw[k * (N / (Ns * R))];
+        if (R > 2) { w[2] = cmul(w[1], w[1]); w[3] = cmul(w[2], w[1]); }
+        if (R > 4) {
+          w[4] = cmul(w[2], w[2]);
+          w[5] = cmul(w[4], w[1]); w[6] = cmul(w[4], w[2]); w[7] = cmul(w[4], w[3]);
+        }
+        if (R > 8) {
+          w[8] = cmul(w[4], w[4]);
+#pragma unroll
+          for (int r = 9; r < 16; ++r) w[r] = cmul(w[8], w[r - 8]);
+        }
+#pragma unroll
+        for (int r = 1; r < R; ++r) x[r] = cmul(x[r], w[r]);
+      }
+      dft<R>(x);
+    }
+  }
+
+  // Phase 3 of stage S: out[(j/Ns) Ns R + k + r Ns] = v[b*R + r].  `st(idx, val)`.
+  template <int S, class Store> BLINK_HD static void store(const cf32 *v, int t, Store st) {
+    constexpr int R = radix<S>();
+    constexpr int Ns = ns<S>();
+#pragma unroll
+    for (int b = 0; b < E / R; ++b) {
+      const int j = t + b * T;
+      const int k = j & (Ns - 1);
+      const int j0 = (j - k) * R + k;
+#pragma unroll
+      for (int r = 0; r < R; ++r) st(j0 + r * Ns, v[b * R + r]);
+    }
+  }
+};
+
+}  // namespace blinkfft

@@ -1,0 +1,87 @@
+// Host-side check of the Stockham stage algebra in paper_2405_13478_b200/csrc/fft_core.cuh:
+// emulates the T threads of one transform phase by phase (load all / compute / store all, with a
+// padded line standing in for shared memory) and compares with a naive fp64 inverse DFT.
+// Built and run by tests/test_host_logic.py (CPU only).  Prints "OK" or "FAIL ...".
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <vector>
+
+#include "../paper_2405_13478_b200/csrc/fft_core.cuh"
+
+using namespace blinkfft;
+
+template <int N, int S> struct RunStages {
+  static void run(std::vector<cf32> &line, const std::vector<cf32> &tw) {
+    using F = Fft<N>;
+    std::vector<cf32> regs(F::T * 16);
+    for (int t = 0; t < F::T; ++t)
+      F::template load<S>(&regs[t * 16], t, [&](int idx) { return line[pad16(idx)]; });
+    for (int t = 0; t < F::T; ++t) F::template compute<S>(&regs[t * 16], t, tw.data());
+    for (int t = 0; t < F::T; ++t)
+      F::template store<S>(&regs[t * 16], t, [&](int idx, cf32 v) { line[pad16(idx)] = v; });
+    if (S + 1 < F::NSTAGE) RunStages<N, (S + 1 < F::NSTAGE ? S + 1 : S)>::run_next(line, tw);
+  }
+  static void run_next(std::vector<cf32> &line, const std::vector<cf32> &tw) { run(line, tw); }
+};
+
+template <int N> int check() {
+  std::vector<cf32> tw(N), line(LineSize<N>::value);
+  for (int k = 0; k < N; ++k) {
+    double a = 2.0 * M_PI * k / N;
+    tw[k] = mk((float)cos(a), (float)sin(a));
+  }
+  std::vector<double> xr(N), xi(N);
+  srand(1234 + N);
+  for (int k = 0; k < N; ++k) {
+    xr[k] = rand() / (double)RAND_MAX - 0.5;
+    xi[k] = rand() / (double)RAND_MAX - 0.5;
+    line[pad16(k)] = mk((float)xr[k], (float)xi[k]);
+  }
+  RunStages<N, 0>::run(line, tw);
+  double maxerr = 0, maxref = 0;
+  for (int n = 0; n < N; ++n) {
+    double sr = 0, si = 0;
+    for (int k = 0; k < N; ++k) {
+      double a = 2.0 * M_PI * ((long long)k * n % N) / N;
+      sr += (double)(float)xr[k] * cos(a) - (double)(float)xi[k] * sin(a);
+      si += (double)(float)xr[k] * sin(a) + (double)(float)xi[k] * cos(a);
+    }
+    cf32 g = line[pad16(n)];
+    maxerr = fmax(maxerr, fmax(fabs(g.x - sr), fabs(g.y - si)));
+    maxref = fmax(maxref, fmax(fabs(sr), fabs(si)));
+  }
+  double rel = maxerr / maxref;
+  printf("N=%d rel_err=%.3e\n", N, rel);
+  return rel < 2e-6 ? 0 : 1;
+}
+
+int main() {
+  int bad = 0;
+  bad += check<32>();
+  bad += check<64>();
+  bad += check<128>();
+  bad += check<256>();
+  bad += check<512>();
+  bad += check<1024>();
+  bad += check<2048>();
+  bad += check<4096>();
+  // small butterflies against the definition
+  for (int R : {2, 4, 8, 16}) {
+    cf32 v[16];
+    double xr[16], xi[16];
+    for (int k = 0; k < R; ++k) { xr[k] = k * 0.37 - 1.0; xi[k] = 0.5 - k * k * 0.011; v[k] = mk((float)xr[k], (float)xi[k]); }
+    if (R == 2) dft<2>(v); else if (R == 4) dft<4>(v); else if (R == 8) dft<8>(v); else dft<16>(v);
+    for (int n = 0; n < R; ++n) {
+      double sr = 0, si = 0;
+      for (int k = 0; k < R; ++k) {
+        double a = 2.0 * M_PI * k * n / R;
+        sr += (float)xr[k] * cos(a) - (float)xi[k] * sin(a);
+        si += (float)xr[k] * sin(a) + (float)xi[k] * cos(a);
+      }
+      if (fabs(v[n].x - sr) > 2e-5 || fabs(v[n].y - si) > 2e-5) { printf("FAIL dft%d n=%d\n", R, n); ++bad; }
+    }
+  }
+  puts(bad ? "FAIL" : "OK");
+  return bad;
+}

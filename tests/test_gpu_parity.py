@@ -1,0 +1,240 @@
+"""GPU parity: the CUDA path (through the C ABI, via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Bars (BASELINE.json north_star):
+  - uv cell indices and weight counts: BIT-EXACT;
+  - grids: max|d| <= 1e-5 * max|grid| (fp32 sums of <= ~100 terms vs fp64), zeros exactly zero;
+  - images: max|d| <= 1e-4 * image peak.
+"""
+import numpy as np
+import pytest
+
+from paper_2405_13478_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+GRID_TOL = 1e-5
+IMG_TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test run without a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def blink():
+    from paper_2405_13478_b200 import blink as b
+    b.load()  # raises if libblink.so is missing: there is no fallback
+    return b
+
+
+def _workload(name):
+    if name == "tiny":
+        return synth.config_tiny()
+    if name == "station":
+        return synth.config_station(n_t=3, n_ch=32)
+    if name == "station128":
+        return synth.config_station(n_t=2, n_ch=3, n_pix=128)
+    if name == "station512":
+        return synth.config_station(n_t=2, n_ch=2, n_pix=512)
+    if name == "mwa1":
+        return synth.config_mwa1(n_t=2, n_ch=3)
+    if name == "mwa2":
+        return synth.config_mwa2(n_t=1, n_ch=2)
+    if name == "mwa1_natural_64":   # small-field geometry on a small grid: most baselines dropped
+        w = synth.config_mwa1(n_t=2, n_ch=2)
+        w.n_pix, w.weighting = 64, synth.NATURAL
+        return w
+    if name == "station_uniform_32":
+        w = synth.config_station(n_t=2, n_ch=2, n_pix=32)
+        w.weighting = synth.UNIFORM
+        return w
+    raise KeyError(name)
+
+
+ALL = ["tiny", "station", "station128", "station512", "mwa1", "mwa2", "mwa1_natural_64",
+       "station_uniform_32"]
+
+
+def _plan(blink, w):
+    return blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+
+
+@pytest.mark.parametrize("name", ALL)
+def test_indices_and_counts_bit_exact(torch_cuda, blink, oracle, name):
+    w = _workload(name)
+    plan = _plan(blink, w)
+    for ch in range(w.n_ch):
+        r = oracle.uv_cells(w.ant_enu_m, w.freq_hz[ch], w.n_pix, w.pixscale)
+        assert np.array_equal(plan.cell_idx(ch), r["cell"]), f"cell indices differ, ch {ch}"
+        cnt = oracle.counts(r["cell"], r["cell_conj"], w.n_pix)
+        assert np.array_equal(plan.counts(ch), cnt), f"weight counts differ, ch {ch}"
+        assert plan.n_dropped(ch) == r["n_dropped"]
+        assert plan.wsum(ch) == int(cnt.sum())
+        assert plan.n_occ(ch) == int(np.count_nonzero(cnt))
+        exp_norm = cnt.sum() if w.weighting == synth.NATURAL else np.count_nonzero(cnt)
+        assert plan.norm(ch) == float(exp_norm)
+    if name == "mwa1":
+        assert plan.n_dropped(0) > 0          # the literal config drops outlier-outlier baselines
+    plan.close()
+
+
+def _run_gpu(torch, plan, vis):
+    v = torch.from_numpy(vis).cuda()
+    uv = torch.full((vis.shape[0], plan.n_ch, plan.n_pix, plan.n_pix), float("nan"),
+                    dtype=torch.complex64, device="cuda")        # must be fully overwritten
+    plan.grid(v, uv)
+    img = torch.full(uv.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.image(uv, img)
+    torch.cuda.synchronize()
+    return uv.cpu().numpy(), img.cpu().numpy()
+
+
+@pytest.mark.parametrize("name", ["tiny", "station", "station128", "station512", "mwa1",
+                                  "mwa1_natural_64", "station_uniform_32"])
+def test_grid_and_image_match_oracle(torch_cuda, blink, oracle, name):
+    w = _workload(name)
+    vis = w.vis()
+    plan = _plan(blink, w)
+    uv, img = _run_gpu(torch_cuda, plan, vis)
+    n_snap = w.n_t * w.n_ch
+    if w.n_pix >= 1024:
+        sel = np.array([0, n_snap - 1], np.int64)
+    elif name == "station":
+        sel = np.array([0, 1, 31, 32, 50, n_snap - 1], np.int64)   # spans t and ch
+    else:
+        sel = np.arange(n_snap, dtype=np.int64)
+    ref = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel,
+                             want_grids=True)
+    uvf = uv.reshape(n_snap, w.n_pix, w.n_pix)
+    imf = img.reshape(n_snap, w.n_pix, w.n_pix)
+    idx = (-np.arange(w.n_pix)) % w.n_pix
+    for q, s in enumerate(sel):
+        g_ref, i_ref = ref["grids"][q], ref["images"][q]
+        g = uvf[s]
+        assert np.all(np.isfinite(g.view(np.float32))), "grid not fully overwritten"
+        gmax = np.max(np.abs(g_ref))
+        assert np.max(np.abs(g - g_ref)) <= GRID_TOL * gmax, f"grid snapshot {s}"
+        assert np.all(g[g_ref == 0] == 0), "cells with no visibility must be exactly zero"
+        assert np.array_equal(g, np.conj(g[idx][:, idx])), "grid must be exactly Hermitian"
+        im = imf[s]
+        assert np.all(np.isfinite(im)), "image not fully overwritten"
+        peak = np.max(np.abs(i_ref))
+        err = np.max(np.abs(im - i_ref))
+        assert err <= IMG_TOL * peak, f"image snapshot {s}: err {err:.3e} peak {peak:.3e}"
+    plan.close()
+
+
+def test_mwa2_4096_sampled_pixels(torch_cuda, blink, oracle):
+    """4096^2: full grids are compared exactly as above; images on sampled pixels the oracle
+    computes one by one (literal sum over the occupied cells)."""
+    w = _workload("mwa2")
+    vis = w.vis()
+    plan = _plan(blink, w)
+    uv, img = _run_gpu(torch_cuda, plan, vis)
+    n = w.n_pix
+    rng = np.random.Generator(np.random.PCG64(99))
+    yx = np.concatenate([rng.integers(0, n, (200, 2)),
+                         [[0, 0], [n - 1, n - 1], [n // 2, n // 2], [n // 2 - 1, n // 2 + 1], [0, n - 1]]]).astype(np.int32)
+    for s in range(w.n_t * w.n_ch):
+        ch = s % w.n_ch
+        r = oracle.uv_cells(w.ant_enu_m, w.freq_hz[ch], n, w.pixscale)
+        g_ref, cnt = oracle.grid(r["cell"], r["cell_conj"], vis[s // w.n_ch, ch], n)
+        g = uv.reshape(-1, n, n)[s]
+        assert np.max(np.abs(g - g_ref)) <= GRID_TOL * np.max(np.abs(g_ref))
+        assert np.all(g[g_ref == 0] == 0)
+        gw, norm = oracle.weight(g_ref, cnt, w.weighting)
+        px = oracle.dft2_pixels(gw, norm, yx).real
+        # peak of the image: the centre of a natural-weighted dirty image is bounded by sum|V|/norm;
+        # use the max over the GPU image itself cross-checked on the sampled oracle pixels
+        im = img.reshape(-1, n, n)[s]
+        yp, xp = np.unravel_index(np.argmax(np.abs(im)), im.shape)
+        peak = abs(oracle.dft2_pixels(gw, norm, np.array([[yp, xp]], np.int32)).real[0])
+        assert abs(peak - abs(im[yp, xp])) <= IMG_TOL * peak
+        err = np.max(np.abs(im[yx[:, 0], yx[:, 1]] - px))
+        assert err <= IMG_TOL * peak, f"snapshot {s}: err {err:.3e} peak {peak:.3e}"
+    plan.close()
+
+
+def test_unit_source_gives_one_at_centre(torch_cuda, blink):
+    """Property that holds at any size: V = 1 -> centre pixel 1 (both weightings)."""
+    torch = torch_cuda
+    for wt in (synth.NATURAL, synth.UNIFORM):
+        w = synth.config_station(n_t=1, n_ch=2, n_pix=256)
+        plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, wt)
+        vis = torch.ones((1, w.n_ch, w.n_bl), dtype=torch.complex64, device="cuda")
+        img = plan.image(plan.grid(vis)).cpu().numpy()
+        for ch in range(w.n_ch):
+            assert abs(img[0, ch, 128, 128] - 1.0) < 2e-6
+            assert img[0, ch].max() <= 1.0 + 2e-6
+        plan.close()
+
+
+def test_deterministic_and_chunk_invariant(torch_cuda, blink):
+    """Bit-reproducible run to run (PAPER.md:386 reports the atomic version is not), and the result
+    of a snapshot does not depend on how the batch is split across calls."""
+    torch = torch_cuda
+    w = synth.config_station(n_t=5, n_ch=4, n_pix=256)
+    vis = torch.from_numpy(w.vis()).cuda()
+    plan = _plan(blink, w)
+    uv1 = plan.grid(vis).clone()
+    im1 = plan.image(uv1).clone()
+    uv2 = plan.grid(vis)
+    im2 = plan.image(uv2)
+    assert torch.equal(uv1.view(torch.float32), uv2.view(torch.float32)) and torch.equal(im1, im2)
+    uv3 = torch.cat([plan.grid(vis[:2].contiguous()), plan.grid(vis[2:].contiguous())])
+    im3 = torch.cat([plan.image(uv3[:3].contiguous()), plan.image(uv3[3:].contiguous())])
+    assert torch.equal(uv1.view(torch.float32), uv3.view(torch.float32)) and torch.equal(im1, im3)
+    plan.close()
+
+
+def test_edge_cases(torch_cuda, blink):
+    torch = torch_cuda
+    w = synth.config_tiny()
+    plan = _plan(blink, w)
+    # n_t = 0 is a no-op
+    e = torch.empty((0, 1, w.n_bl), dtype=torch.complex64, device="cuda")
+    assert plan.grid(e).shape[0] == 0
+    assert plan.image(torch.empty((0, 1, 128, 128), dtype=torch.complex64, device="cuda")).shape[0] == 0
+    plan.close()
+    # every baseline outside the grid: grid and image are exactly zero, norm 0
+    far = blink.Plan(w.ant_enu_m * 1e4, w.freq_hz, 32, 2.0 / 32, synth.NATURAL)
+    assert far.n_dropped(0) == w.n_bl and far.norm(0) == 0.0
+    vis = torch.from_numpy(w.vis()).cuda()
+    uv = far.grid(vis)
+    img = far.image(uv)
+    assert torch.count_nonzero(uv.view(torch.float32)) == 0 and torch.count_nonzero(img) == 0
+    far.close()
+    # bad arguments are refused, not crashed on
+    with pytest.raises(blink.BlinkError):
+        blink.Plan(w.ant_enu_m, w.freq_hz, 130, 2.0 / 130)        # not a power of two
+    with pytest.raises(blink.BlinkError):
+        blink.Plan(w.ant_enu_m, w.freq_hz, 127, 2.0 / 127)        # odd
+    with pytest.raises(blink.BlinkError):
+        blink.Plan(w.ant_enu_m[:1], w.freq_hz, 128, 2.0 / 128)    # one antenna
+
+
+def test_full_size_station_launch_configuration(torch_cuda, blink, oracle):
+    """BASELINE.json configs[1] at FULL size (100 t x 32 ch x 32640 bl, 256^2), in the launch
+    configuration bench.py times; parity on sampled snapshots."""
+    torch = torch_cuda
+    w = synth.config_station()
+    vis = w.vis()
+    plan = _plan(blink, w)
+    v = torch.from_numpy(vis).cuda()
+    uv = plan.grid(v)
+    img = plan.image(uv)
+    torch.cuda.synchronize()
+    n_snap = w.n_t * w.n_ch
+    sel = np.array([0, 777, 1600, n_snap - 1], np.int64)
+    ref = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel,
+                             want_grids=True)
+    uvh = uv.view(n_snap, 256, 256)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    imh = img.view(n_snap, 256, 256)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        assert np.max(np.abs(uvh[q] - ref["grids"][q])) <= GRID_TOL * np.max(np.abs(ref["grids"][q]))
+        peak = np.max(np.abs(ref["images"][q]))
+        assert np.max(np.abs(imh[q] - ref["images"][q])) <= IMG_TOL * peak
+    plan.close()
