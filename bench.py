@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the BLINK hot path (blink_grid + blink_image) on synthetic workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload station|mwa1|mwa2|sweep256|...]
+    python bench.py --impl reference ...        # times the CPU oracle instead (reference arm)
+
+A "step" is one pass of the whole hot path (grid every snapshot, image every snapshot) over one
+batch of synthetic visibilities already resident in HBM.  Prints ONE JSON line (rank 0).
+Default workload = BASELINE.json configs[1] (SKA-Low station, 100 t x 32 ch x 32640 bl, 256^2).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2405_13478_b200 import synth  # noqa: E402
+
+
+def make_workload(name: str):
+    if name == "station":
+        return synth.config_station()
+    if name == "tiny":
+        return synth.config_tiny()
+    if name == "mwa1":
+        return synth.config_mwa1()
+    if name == "mwa2":
+        return synth.config_mwa2()
+    if name.startswith("sweep"):
+        return synth.config_sweep(int(name[5:]))
+    raise SystemExit(f"unknown workload {name}")
+
+
+def algorithmic_bytes(w):
+    """per snapshot, blink_grid reads 8 n_bl and writes 8 N^2; blink_image
+    reads 8 N^2 and writes 4 N^2 (count/index tables are per-plan, excluded)."""
+    nn = w.n_pix * w.n_pix
+    return dict(grid=8 * w.n_bl + 8 * nn, image=12 * nn, step=8 * w.n_bl + 20 * nn)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu, self.proc = gpu_index, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smax.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(smax)) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def run_reference(args, w):
+    """Reference arm = the CPU oracle as it stands, on the host cores, on a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    orc.build()
+    n_t_s = max(1, min(w.n_t, args.ref_time_steps))
+    vis = w.vis(0, n_t_s)
+    sel = np.arange(n_t_s * w.n_ch, dtype=np.int64)
+    per = []
+    threads = 1
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        out = orc.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel,
+                              want_grids=False, want_images=True, n_threads=0)
+        dt = time.perf_counter() - t0
+        threads = out["threads"]
+        if it >= args.warmup:
+            per.append(dt)
+    ms = 1e3 * float(np.mean(per))
+    val = len(sel) / (ms / 1e3)
+    sample = f"{n_t_s} of {w.n_t} time steps x {w.n_ch} channels = {len(sel)} snapshots per step"
+    print(json.dumps({
+        "impl": "reference", "metric": "dirty_images_per_s", "value": val, "unit": "images/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "mvis_per_s": val * w.n_bl / 1e6,
+        "config": workload_config(w, args.workload),
+        "cpu_baseline": {"value": val, "unit": "images/s", "cores": threads, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": "images/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def workload_config(w, name):
+    return {"workload": f"{name}: {w.n_ant} antennas, {w.n_bl} baselines, {w.n_t} time steps x "
+                        f"{w.n_ch} channels = {w.n_snapshots} snapshots, {w.n_pix}x{w.n_pix} image, "
+                        f"{'natural' if w.weighting == 0 else 'uniform'} weighting",
+            "n_ant": w.n_ant, "n_bl": w.n_bl, "n_t": w.n_t, "n_ch": w.n_ch, "n_pix": w.n_pix,
+            "weighting": "natural" if w.weighting == 0 else "uniform",
+            "l2_policy": "inputs larger than L2: each step streams vis, uv grids and images "
+                         "(>= 0.8 GB each) through the 126 MB L2"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="station")
+    ap.add_argument("--impl", default="blink", choices=["blink", "reference"])
+    ap.add_argument("--n-t", type=int, default=0, help="override time steps per batch (0 = config)")
+    ap.add_argument("--ref-time-steps", type=int, default=4,
+                    help="time steps per step of the CPU reference / cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    w = make_workload(args.workload)
+    if args.n_t > 0:
+        w.n_t = args.n_t
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2405_13478_b200 import blink
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    blink.load()
+
+    # ---- inputs: every rank images its own full batch (independent snapshots, no collective)
+    w.seed = w.seed + 1000 * rank if rank else w.seed
+    vis_h = torch.from_numpy(w.vis()).pin_memory()
+    plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    plan.reserve(w.n_t)
+    vis = vis_h.cuda(non_blocking=True)
+    shape = (w.n_t, w.n_ch, w.n_pix, w.n_pix)
+    uv = torch.empty(shape, dtype=torch.complex64, device="cuda")
+    img = torch.empty(shape, dtype=torch.float32, device="cuda")
+    img_h = torch.empty(shape, dtype=torch.float32).pin_memory()
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        plan.grid(vis, uv)
+        plan.image(uv, img)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3 * args.steps + 1)]
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    barrier()
+    ev[0].record(stream)
+    for k in range(args.steps):
+        plan.grid(vis, uv)
+        ev[3 * k + 1].record(stream)
+        plan.image(uv, img)
+        ev[3 * k + 2].record(stream)
+        ev[3 * k + 3].record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = ev[0].elapsed_time(ev[3 * args.steps])
+    grid_ms = float(np.mean([ev[3 * k].elapsed_time(ev[3 * k + 1]) for k in range(args.steps)]))
+    image_ms = float(np.mean([ev[3 * k + 1].elapsed_time(ev[3 * k + 2]) for k in range(args.steps)]))
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    n_snap = w.n_snapshots
+    value = world * n_snap / (ms_per_step / 1e3)
+
+    # ---- end to end: pinned host visibilities in, images back to pinned host memory, per step
+    e2e = None
+    if not args.no_e2e:
+        def e2e_step():
+            vis.copy_(vis_h, non_blocking=True)
+            plan.grid(vis, uv)
+            plan.image(uv, img)
+            img_h.copy_(img, non_blocking=True)
+        e2e_step()
+        barrier()
+        n_e = max(1, min(args.steps, 3))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(n_e):
+            e2e_step()
+        e1.record(stream)
+        barrier()
+        te = torch.tensor([e0.elapsed_time(e1) / n_e], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * n_snap / (float(te.item()) / 1e3), "unit": "images/s",
+               "ms_per_step": float(te.item()),
+               "h2d_bytes_per_step": int(vis_h.numel() * vis_h.element_size()),
+               "d2h_bytes_per_step": int(img_h.numel() * img_h.element_size())}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline (HBM-bound scan/scatter work), dominant call
+    peak, peak_src = measured_peaks()
+    ab = algorithmic_bytes(w)
+    calls = {"blink_grid": (grid_ms, ab["grid"]), "blink_image": (image_ms, ab["image"])}
+    dom = max(calls, key=lambda k: calls[k][0])
+    achieved = calls[dom][1] * n_snap / (calls[dom][0] / 1e3) / 1e9
+    step_gbs = ab["step"] * n_snap / (ms_per_step / 1e3) / 1e9
+    chunks = -(-n_snap // max(1, plan.query_i32(blink.Q_IMAGE_CHUNK)))
+    launches_per_step = 1 + 2 * chunks
+    out = {
+        "metric": "dirty_images_per_s", "value": value, "unit": "images/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "mvis_per_s": value * w.n_bl / 1e6,
+        "config": workload_config(w, args.workload),
+        "per_call_ms": {"blink_grid": grid_ms, "blink_image": image_ms},
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_snapshot": calls[dom][1]},
+        "roofline_step": {"bound": "hbm", "achieved": step_gbs, "peak": peak, "unit": "GB/s",
+                          "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": ab["step"]},
+        "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
+    }
+    if not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(w, args)
+    print(json.dumps(out))
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(w, args):
+    """The oracle as it stands, timed on this box's host cores, on a bounded sample."""
+    from oracle import oracle as orc
+    orc.build()
+    n_t_s = max(1, min(w.n_t, args.ref_time_steps))
+    vis = w.vis(0, n_t_s)
+    sel = np.arange(n_t_s * w.n_ch, dtype=np.int64)
+    t0 = time.perf_counter()
+    out = orc.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel,
+                          want_grids=False, want_images=True, n_threads=0)
+    dt = time.perf_counter() - t0
+    return {"value": len(sel) / dt, "unit": "images/s", "cores": out["threads"], "kind": "oracle",
+            "seconds": dt,
+            "sample": f"first {n_t_s} of {w.n_t} time steps x {w.n_ch} channels = {len(sel)} snapshots, "
+                      "fp64 gridding + naive separable DFT (O(N^3)), OpenMP over snapshots"}
+
+
+if __name__ == "__main__":
+    main()

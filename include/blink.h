@@ -71,7 +71,8 @@ typedef enum blink_query {
   BLINK_Q_CELL_IDX = 9,   /* out: const int32* DEVICE [n_ch][n_bl], cell of V, -1 = dropped */
   BLINK_Q_COUNTS = 10,    /* out: const uint32* DEVICE [n_ch][N][N] weight counts  */
   BLINK_Q_IMAGE_PATH = 11,/* out: int32   0 = shared-memory single pass, 1 = two-pass */
-  BLINK_Q_SCRATCH_BYTES = 12 /* out: int64 device scratch currently held by the plan */
+  BLINK_Q_SCRATCH_BYTES = 12, /* out: int64 device scratch currently held by the plan */
+  BLINK_Q_IMAGE_CHUNK = 13 /* out: int32  snapshots per launch pair of the two-pass imaging path */
 } blink_query;
 
 typedef struct blink_plan blink_plan; /* opaque */

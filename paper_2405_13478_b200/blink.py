@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libblink.so")
 NATURAL, UNIFORM = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
 (Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
- Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES) = range(13)
+ Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK) = range(14)
 
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create",
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
