@@ -24,12 +24,9 @@ using namespace blinkfft;
 
 template <int N> struct ImgCfg {
   static constexpr int T = N / 16;                                   // threads per transform
-  static constexpr int CT = (N <= 1024) ? 16 : (N == 2048 ? 8 : 4);  // columns per CTA, pass A
-  static constexpr int RP0 = (N <= 256) ? (256 / T) : (512 / T);
-  static constexpr int RP = RP0 < N / 2 ? RP0 : N / 2;                // row pairs per CTA, pass B
   static constexpr int LS = ((LineSize<N>::value + 15) / 16) * 16 + 1;  // line stride, = 1 mod 16
-  static constexpr int THREADS_A = CT * T;
-  static constexpr int THREADS_B = RP * T;
+  static constexpr int CT_MAX = (1024 / T) < 16 ? (1024 / T) : 16;   // columns per CTA, pass A
+  static constexpr int RP_MAX = (N / 2) < (512 / T) ? (N / 2) : (512 / T > 0 ? 512 / T : 1);
 };
 
 struct ImgParams {
@@ -37,9 +34,10 @@ struct ImgParams {
   float *img;
   float2 *U;
   const ChannelInfo *chinfo;
-  const uint32_t *counts;
+  const int32_t *wkey, *wcol;
+  const float *wval;
   const float2 *tw;
-  int n_ch, wu, uniform, snap_base;
+  int n_ch, n_bl, wu, uniform, snap_base;
 };
 
 // run stages 1.. of the transform; stage 0's load is done by the caller
@@ -65,38 +63,47 @@ __device__ __forceinline__ void fft_tail(cf32 *v, int t, cf32 *line, const cf32 
   }
 }
 
-template <int N>
-__global__ void __launch_bounds__(ImgCfg<N>::THREADS_A) k_image_cols(const ImgParams p) {
+template <int N, int CT>
+__global__ void __launch_bounds__(CT * (N / 16)) k_image_cols(const ImgParams p) {
   using C = ImgCfg<N>;
+  constexpr int THREADS = CT * C::T;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cf32 *lines = reinterpret_cast<cf32 *>(smem_raw);
   const int tid = threadIdx.x;
   const int sl = blockIdx.y, s = p.snap_base + sl, ch = s % p.n_ch;
   const ChannelInfo ci = p.chinfo[ch];
-  const int kx0 = blockIdx.x * C::CT;
+  const int kx0 = blockIdx.x * CT;
   const float2 *__restrict__ G = p.uv + (size_t)s * N * N;
 
-  for (int i = tid; i < C::CT * C::LS; i += C::THREADS_A) lines[i] = mk(0.f, 0.f);
+  for (int i = tid; i < CT * C::LS; i += THREADS) lines[i] = mk(0.f, 0.f);
   __syncthreads();
   const int nrow = 2 * ci.ky_max + 1;
-  const uint32_t *__restrict__ cnt = p.counts + (size_t)ch * N * N;
-  for (int e = tid; e < nrow * C::CT; e += C::THREADS_A) {
-    const int c = e % C::CT, ky = e / C::CT - ci.ky_max, kx = kx0 + c;
+  const float w0 = 0.5f * ci.inv_norm;
+  for (int e = tid; e < nrow * CT; e += THREADS) {
+    const int c = e % CT, ky = e / CT - ci.ky_max, kx = kx0 + c;
     if (kx > ci.kx_max) continue;
     const int iy = (ky + N) & (N - 1);
-    const float2 a = __ldg(G + (size_t)iy * N + kx);
-    const float2 b = __ldg(G + (size_t)((N - iy) & (N - 1)) * N + ((N - kx) & (N - 1)));
-    float w = 0.5f * ci.inv_norm;
-    if (p.uniform) {
-      const uint32_t n = __ldg(cnt + (size_t)iy * N + kx);
-      w = n ? w / (float)n : 0.f;
-    }
-    if ((kx + ky) & 1) w = -w;
+    const float2 a = __ldcs(G + (size_t)iy * N + kx);
+    const float2 b = __ldcs(G + (size_t)((N - iy) & (N - 1)) * N + ((N - kx) & (N - 1)));
+    const float w = ((kx + ky) & 1) ? -w0 : w0;
     lines[c * C::LS + pad16(iy)] = mk((a.x + b.x) * w, (a.y - b.y) * w);
   }
   __syncthreads();
+  if (p.uniform) {   // sparse 1/count on the occupied cells of these columns
+    const int32_t *__restrict__ wcol = p.wcol + (size_t)ch * (p.wu + 1);
+    const int e0 = wcol[kx0], e1 = wcol[min(kx0 + CT, p.wu)];
+    const int32_t *__restrict__ wkey = p.wkey + (size_t)ch * 2 * p.n_bl;
+    const float *__restrict__ wval = p.wval + (size_t)ch * 2 * p.n_bl;
+    for (int e = e0 + tid; e < e1; e += THREADS) {
+      const int key = wkey[e];
+      const float w = wval[e];
+      cf32 *q = lines + ((key >> 16) - kx0) * C::LS + pad16(key & 0xffff);
+      *q = mk(q->x * w, q->y * w);
+    }
+    __syncthreads();
+  }
 
-  const int c = tid % C::CT, t = tid / C::CT;
+  const int c = tid % CT, t = tid / CT;
   cf32 *line = lines + c * C::LS;
   cf32 v[16];
   Fft<N>::template load<0>(v, t, [&](int idx) { return line[pad16(idx)]; });
@@ -105,8 +112,8 @@ __global__ void __launch_bounds__(ImgCfg<N>::THREADS_A) k_image_cols(const ImgPa
   fft_tail<N>(v, t, line, p.tw, [&](int y, cf32 x) { U[(size_t)y * p.wu] = x; });
 }
 
-template <int N>
-__global__ void __launch_bounds__(ImgCfg<N>::THREADS_B) k_image_rows(const ImgParams p) {
+template <int N, int RP>
+__global__ void __launch_bounds__(RP * (N / 16)) k_image_rows(const ImgParams p) {
   using C = ImgCfg<N>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cf32 *lines = reinterpret_cast<cf32 *>(smem_raw);
@@ -114,7 +121,7 @@ __global__ void __launch_bounds__(ImgCfg<N>::THREADS_B) k_image_rows(const ImgPa
   const int sl = blockIdx.y, s = p.snap_base + sl, ch = s % p.n_ch;
   const int kxm = p.chinfo[ch].kx_max;
   const int pr = tid / C::T, t = tid % C::T;
-  const int y0 = blockIdx.x * C::RP + pr, y1 = y0 + N / 2;
+  const int y0 = blockIdx.x * RP + pr, y1 = y0 + N / 2;
   const float2 *__restrict__ U0 = p.U + ((size_t)sl * N + y0) * p.wu;
   const float2 *__restrict__ U1 = p.U + ((size_t)sl * N + y1) * p.wu;
   cf32 *line = lines + pr * C::LS;
@@ -131,36 +138,64 @@ __global__ void __launch_bounds__(ImgCfg<N>::THREADS_B) k_image_rows(const ImgPa
   });
   float *__restrict__ r0 = p.img + ((size_t)s * N + y0) * N;
   float *__restrict__ r1 = p.img + ((size_t)s * N + y1) * N;
-  fft_tail<N>(v, t, line, p.tw, [&](int x, cf32 z) { r0[x] = z.x; r1[x] = z.y; });
+  fft_tail<N>(v, t, line, p.tw, [&](int x, cf32 z) { __stcs(r0 + x, z.x); __stcs(r1 + x, z.y); });
 }
 
-template <int N> static int run_image_n(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st) {
+template <class K> static int prep_kernel(K kern, size_t smem) {
+  BLINK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                 "image kernel smem attribute");
+  BLINK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100),
+                 "image kernel carveout");
+  return BLINK_OK;
+}
+
+template <int N, int CT, int RP>
+static int run_image_cfg(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st) {
   using C = ImgCfg<N>;
-  const size_t smem_a = sizeof(cf32) * C::CT * C::LS, smem_b = sizeof(cf32) * C::RP * C::LS;
+  const size_t smem_a = sizeof(cf32) * CT * C::LS, smem_b = sizeof(cf32) * RP * C::LS;
   static thread_local bool attr_done = false;
   if (!attr_done) {
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_image_cols<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a),
-                   "k_image_cols smem attribute");
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_image_rows<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b),
-                   "k_image_rows smem attribute");
+    int rc = prep_kernel(k_image_cols<N, CT>, smem_a);
+    if (rc == BLINK_OK) rc = prep_kernel(k_image_rows<N, RP>, smem_b);
+    if (rc != BLINK_OK) return rc;
     attr_done = true;
   }
   const int chunk = std::max(1, p->chunk_snapshots);
   for (int base = 0; base < n_snap; base += chunk) {
     const int cs = std::min(chunk, n_snap - base);
     ip.snap_base = base;
-    k_image_cols<N><<<dim3(p->wu / C::CT, cs), C::THREADS_A, smem_a, st>>>(ip);
-    k_image_rows<N><<<dim3(N / 2 / C::RP, cs), C::THREADS_B, smem_b, st>>>(ip);
+    k_image_cols<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
+    k_image_rows<N, RP><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
   }
   BLINK_CUDA_TRY(cudaGetLastError(), "k_image launch");
   return BLINK_OK;
 }
 
-static int cols_per_cta(int N) { return N <= 1024 ? 16 : (N == 2048 ? 8 : 4); }
+// default tile shapes per N; N = 512 / 1024 also carry alternatives selectable through the plan
+template <int N> static int run_image_n(const blink_plan *p, const ImgParams &ip, int n_snap, cudaStream_t st) {
+  using C = ImgCfg<N>;
+  if constexpr (N == 1024) {
+    if (p->img_ct == 16) return run_image_cfg<N, 16, 4>(p, ip, n_snap, st);
+    if (p->img_ct == 4) return run_image_cfg<N, 4, 4>(p, ip, n_snap, st);
+    if (p->img_rp == 8) return run_image_cfg<N, 8, 8>(p, ip, n_snap, st);
+    if (p->img_rp == 2) return run_image_cfg<N, 8, 2>(p, ip, n_snap, st);
+    return run_image_cfg<N, 8, 4>(p, ip, n_snap, st);
+  } else if constexpr (N == 512) {
+    if (p->img_ct == 16) return run_image_cfg<N, 16, 8>(p, ip, n_snap, st);
+    return run_image_cfg<N, 8, 8>(p, ip, n_snap, st);
+  } else if constexpr (N <= 256) {
+    constexpr int RP = (N / 2) < (256 / C::T) ? (N / 2) : (256 / C::T);
+    return run_image_cfg<N, 16, RP>(p, ip, n_snap, st);
+  } else {
+    return run_image_cfg<N, C::CT_MAX, (256 / C::T > 0 ? 256 / C::T : 1)>(p, ip, n_snap, st);
+  }
+}
+
 
 int image_setup(blink_plan *p) {
-  const int ct = cols_per_cta(p->n_pix);
-  p->wu = ((p->kx_max_all + 1 + ct - 1) / ct) * ct;
+  p->wu = ((p->kx_max_all + 1 + 15) / 16) * 16;   // multiple of every column-tile width
+  if (const char *e = getenv("BLINK_IMAGE_CT")) p->img_ct = atoi(e);
+  if (const char *e = getenv("BLINK_IMAGE_RP")) p->img_rp = atoi(e);
   p->image_path = 1;
   // chunk of snapshots whose U scratch stays L2-resident between the two passes
   size_t budget = 48u << 20;
@@ -195,7 +230,8 @@ int image_reserve(blink_plan *p, int n_t) {
 
 int launch_image(const blink_plan *p, const float2 *uv, int n_t, float *img, cudaStream_t st) {
   ImgParams ip;
-  ip.uv = uv; ip.img = img; ip.U = p->d_scratch; ip.chinfo = p->d_chinfo; ip.counts = p->d_counts;
+  ip.uv = uv; ip.img = img; ip.U = p->d_scratch; ip.chinfo = p->d_chinfo;
+  ip.wkey = p->d_wkey; ip.wval = p->d_wval; ip.wcol = p->d_wcol; ip.n_bl = p->n_bl;
   ip.tw = p->d_tw; ip.n_ch = p->n_ch; ip.wu = p->wu; ip.uniform = p->weighting == BLINK_UNIFORM;
   ip.snap_base = 0;
   const int n_snap = n_t * p->n_ch;

@@ -18,7 +18,9 @@ constexpr int32_t kPlaceDirect = 0;  // grid[cell] = S[j]
 constexpr int32_t kPlaceConj = 1;    // grid[cell] = conj(S[j])
 constexpr int32_t kPlaceBoth = 2;    // grid[cell] = S[j] + conj(S[j])   (self-conjugate cell: DC)
 
-constexpr int kBandCells = 4096;     // cells (complex64) per output band of the gridder = 32 KB
+constexpr int kBandCellsDefault = 2048;  // cells (complex64) per output band of the gridder = 16 KB
+constexpr uint16_t kScatDropped = 0xFFFFu;  // scatter code of a baseline outside the grid
+constexpr int kGridCellsPerThread = 8;      // register accumulators per thread in the per-cell sums
 
 struct ChannelInfo {   // mirrored on the device, one per channel
   int32_t n_kept;      // baselines inside the grid
@@ -56,7 +58,23 @@ struct blink_plan {
   int32_t *d_pcell = nullptr;       // [n_ch][2 n_bl]    occupied full-plane cells, ascending
   int32_t *d_pcode = nullptr;       // [n_ch][2 n_bl]    j | flag << kPlaceShift
   int32_t *d_pband = nullptr;       // [n_ch][n_bands+1] CSR of d_pcell by output band
+  uint16_t *d_scat = nullptr;       // [n_ch][n_bl]      slot in its pass's rank-major stage | conj << 15
+  uint32_t *d_cellrec = nullptr;    // [n_ch][n_pass][n_can_max] j | len << 16, by descending len
+  uint16_t *d_roff = nullptr;       // [n_ch][n_pass][roff_stride] stage offset of rank r
+  int32_t *d_nact = nullptr;        // [n_ch][n_pass]    cells with >= 1 baseline in the pass
+  int roff_stride = 0;
+  int stage_cap = 0;                // baselines staged in shared memory per pass
+  int n_pass = 0;                   // ceil(n_bl / stage_cap)
+  int grid_nbuf = 3;                // band buffers in flight per CTA
+  int grid_ctas_per_sm = 1;
+  int grid_threads = 512, grid_prefetch = 16;  // CTA shape: stage_cap = threads * prefetch
+  size_t grid_smem = 0;
   float2 *d_tw = nullptr;           // [N] exp(+2 pi i k / N)
+  // uniform weighting: sparse per-column list of the occupied half-plane cells and 1/count
+  int32_t *d_wkey = nullptr;        // [n_ch][2 n_bl] (kx << 16) | iy, sorted by kx then iy
+  float *d_wval = nullptr;          // [n_ch][2 n_bl] 1 / count
+  int32_t *d_wcol = nullptr;        // [n_ch][wu + 1] CSR by column kx
+  int img_ct = 0, img_rp = 0;       // tuning: columns per CTA (pass A), row pairs per CTA (pass B)
   int n_bands = 0;                  // bands per snapshot = N*N / band_cells
   int band_cells = 0;
   int n_can_max = 0;

@@ -5,6 +5,7 @@
 // deterministic (the paper's planned "parallel reduction") are sorted on the
 // host once per plan.
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -123,7 +124,7 @@ template <class T> static int dev_alloc(T **p, size_t n) {
 static void plan_free(blink_plan *p) {
   if (!p) return;
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
-  cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband);
+  cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
   cudaFree(p->d_tw); cudaFree(p->d_scratch);
   delete p;
 }
@@ -243,15 +244,21 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   PLAN_CUDA(ce, "plan upload / index kernel");
 
   // ---- host: per-channel facts, gather and placement tables -------------------------------
-  p->band_cells = (int)std::min<size_t>(NN, (size_t)kBandCells);
+  {
+    long bc = kBandCellsDefault;
+    if (const char *e = getenv("BLINK_GRID_BAND_CELLS")) bc = atol(e);
+    if (bc < 256 || (bc & (bc - 1))) bc = kBandCellsDefault;
+    p->band_cells = (int)std::min<size_t>(NN, (size_t)bc);
+  }
   p->n_bands = (int)(NN / p->band_cells);
   p->n_dropped.assign(n_ch, 0); p->wsum.assign(n_ch, 0); p->n_occ.assign(n_ch, 0);
   p->norm.assign(n_ch, 0.0); p->chinfo.assign(n_ch, ChannelInfo());
   std::vector<int32_t> h_src((size_t)n_ch * n_bl, 0), h_seg((size_t)n_ch * (n_bl + 1), 0);
   std::vector<int32_t> h_pcell((size_t)n_ch * 2 * n_bl, 0), h_pcode((size_t)n_ch * 2 * n_bl, 0);
   std::vector<int32_t> h_pband((size_t)n_ch * (p->n_bands + 1), 0);
+  std::vector<HostGather> gathers(n_ch);
   for (int ch = 0; ch < n_ch; ++ch) {
-    HostGather g;
+    HostGather &g = gathers[ch];
     PLAN_TRY(build_gather_host(h_cell.data() + (size_t)ch * n_bl, n_bl, N, g));
     ChannelInfo &ci = p->chinfo[ch];
     ci.n_kept = g.n_kept;
@@ -302,6 +309,86 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   }
   if (p->n_can_max > kPlaceMask) { plan_free(p); return BLINK_EUNSUPPORTED; }
 
+  // ---- gridder tables: rank-major stage slots, cells by descending per-pass length ------------
+  // Pass q stages baselines [q C, (q+1) C).  Within a pass the cells that receive something are
+  // ordered by descending number of baselines (position k); the r-th baseline (ascending index)
+  // of the cell at position k sits at stage[roff[r] + k].  Thread k then adds stage[roff[r] + k],
+  // r = 0..len-1: consecutive threads read consecutive slots (no bank conflicts), warps see
+  // near-uniform trip counts, and the summation order is the oracle's (ascending baseline).
+  {
+    int nbuf = 3;
+    if (const char *e = getenv("BLINK_GRID_NBUF")) nbuf = atoi(e);
+    if (nbuf < 2 || nbuf > 4) nbuf = 3;
+    p->grid_nbuf = nbuf;
+    // CTA shape (threads, prefetch, CTAs/SM): variant 0 = 512 x 16 x 1, 1 = 256 x 16 x 2,
+    // 2 = 512 x 8 x 2, 3 = 256 x 8 x 3
+    int variant = 1;
+    if (const char *e = getenv("BLINK_GRID_VARIANT")) variant = atoi(e);
+    static const int kVar[4][3] = {{512, 16, 1}, {256, 16, 2}, {512, 8, 2}, {256, 8, 3}};
+    if (variant < 0 || variant > 3) variant = 1;
+    p->grid_threads = kVar[variant][0];
+    p->grid_prefetch = kVar[variant][1];
+    p->grid_ctas_per_sm = kVar[variant][2];
+    const int kStageCap = p->grid_threads * p->grid_prefetch;
+    p->stage_cap = kStageCap;
+    p->n_pass = (n_bl + kStageCap - 1) / kStageCap;
+    if (p->n_pass < 1) p->n_pass = 1;
+    p->grid_smem = sizeof(float2) * ((size_t)p->band_cells + (size_t)p->n_can_max +
+                                     (size_t)p->stage_cap) + 64;
+    if (p->max_smem_optin > 0 && p->grid_smem > (size_t)p->max_smem_optin) { plan_free(p); return BLINK_EUNSUPPORTED; }
+  }
+  const int kStageCap = p->stage_cap;
+  const int n_pass = p->n_pass, ncm = std::max(p->n_can_max, 1);
+  std::vector<uint16_t> h_scat((size_t)n_ch * n_bl, kScatDropped);
+  std::vector<uint32_t> h_cellrec((size_t)n_ch * n_pass * ncm, 0);
+  std::vector<int32_t> h_nact((size_t)n_ch * n_pass, 0);
+  std::vector<std::vector<uint16_t>> roffs((size_t)n_ch * n_pass);
+  int maxlen = 0;
+  for (int ch = 0; ch < n_ch; ++ch) {
+    const HostGather &g = gathers[ch];
+    uint16_t *sc = h_scat.data() + (size_t)ch * n_bl;
+    for (int q = 0; q < n_pass; ++q) {
+      const int lo = q * kStageCap, hi = std::min(n_bl, lo + kStageCap);
+      // per cell: entries of this pass are a contiguous sub-range of its (baseline-sorted) segment
+      std::vector<std::array<int32_t, 3>> cells;   // {len, j, first entry}
+      for (int j = 0; j < g.n_can; ++j) {
+        int e0 = g.seg_start[j], e1 = g.seg_start[j + 1];
+        while (e0 < e1 && (g.src[e0] >> 1) < lo) ++e0;
+        int e2 = e0;
+        while (e2 < e1 && (g.src[e2] >> 1) < hi) ++e2;
+        if (e2 > e0) cells.push_back({e2 - e0, j, e0});
+      }
+      std::stable_sort(cells.begin(), cells.end(),
+                       [](const std::array<int32_t, 3> &a, const std::array<int32_t, 3> &b) { return a[0] > b[0]; });
+      const int n_act = (int)cells.size();
+      h_nact[(size_t)ch * n_pass + q] = n_act;
+      const int ml = n_act ? cells[0][0] : 0;
+      maxlen = std::max(maxlen, ml);
+      std::vector<uint16_t> &ro = roffs[(size_t)ch * n_pass + q];
+      ro.assign(ml + 1, 0);
+      int off = 0, nr = n_act;
+      for (int r = 0; r < ml; ++r) {
+        while (nr > 0 && cells[nr - 1][0] <= r) --nr;   // cells with len > r form a prefix
+        ro[r] = (uint16_t)off;
+        off += nr;
+      }
+      ro[ml] = (uint16_t)off;
+      uint32_t *cr = h_cellrec.data() + ((size_t)ch * n_pass + q) * ncm;
+      for (int k = 0; k < n_act; ++k) {
+        cr[k] = (uint32_t)cells[k][1] | ((uint32_t)cells[k][0] << 16);
+        for (int r = 0; r < cells[k][0]; ++r) {
+          const int code = g.src[cells[k][2] + r];
+          sc[code >> 1] = (uint16_t)((ro[r] + k) | ((code & 1) << 15));
+        }
+      }
+    }
+  }
+  if (p->n_can_max > 0xFFFF || kStageCap > 0x7FFF) { plan_free(p); return BLINK_EUNSUPPORTED; }
+  p->roff_stride = maxlen + 1;
+  std::vector<uint16_t> h_roff((size_t)n_ch * n_pass * p->roff_stride, 0);
+  for (size_t i = 0; i < roffs.size(); ++i)
+    std::copy(roffs[i].begin(), roffs[i].end(), h_roff.begin() + i * p->roff_stride);
+
   // twiddles exp(+2 pi i k / N), fp64 -> fp32
   std::vector<float2> h_tw(N);
   for (int k = 0; k < N; ++k) {
@@ -316,6 +403,14 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   PLAN_TRY(dev_alloc(&p->d_pcode, h_pcode.size()));
   PLAN_TRY(dev_alloc(&p->d_pband, h_pband.size()));
   PLAN_TRY(dev_alloc(&p->d_tw, (size_t)N));
+  PLAN_TRY(dev_alloc(&p->d_scat, h_scat.size()));
+  PLAN_TRY(dev_alloc(&p->d_cellrec, h_cellrec.size()));
+  PLAN_TRY(dev_alloc(&p->d_roff, h_roff.size()));
+  PLAN_TRY(dev_alloc(&p->d_nact, h_nact.size()));
+  step(cudaMemcpyAsync(p->d_scat, h_scat.data(), sizeof(uint16_t) * h_scat.size(), cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_cellrec, h_cellrec.data(), sizeof(uint32_t) * h_cellrec.size(), cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_roff, h_roff.data(), sizeof(uint16_t) * h_roff.size(), cudaMemcpyHostToDevice, st));
+  step(cudaMemcpyAsync(p->d_nact, h_nact.data(), sizeof(int32_t) * h_nact.size(), cudaMemcpyHostToDevice, st));
   step(cudaMemcpyAsync(p->d_chinfo, p->chinfo.data(), sizeof(ChannelInfo) * n_ch, cudaMemcpyHostToDevice, st));
   step(cudaMemcpyAsync(p->d_src, h_src.data(), sizeof(int32_t) * h_src.size(), cudaMemcpyHostToDevice, st));
   step(cudaMemcpyAsync(p->d_seg, h_seg.data(), sizeof(int32_t) * h_seg.size(), cudaMemcpyHostToDevice, st));
@@ -326,6 +421,47 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   step(cudaStreamSynchronize(st));
   PLAN_CUDA(ce, "plan table upload");
   PLAN_TRY(image_setup(p));
+  if (weighting == BLINK_UNIFORM) {
+    // canonical cells are exactly the occupied half-plane cells with ky > 0 or (ky == 0, kx >= 0);
+    // pass A of blink_image works on columns kx >= 0 and all ky, so list every occupied cell with
+    // kx >= 0 (canonical cells with kx >= 0, and mirrors of canonical cells with kx < 0 -- and of
+    // kx == 0, ky > 0).  count = segment length (+ mirror symmetry: count[c] == count[c*]).
+    std::vector<int32_t> h_wkey((size_t)n_ch * 2 * n_bl, 0), h_wcol((size_t)n_ch * (p->wu + 1), 0);
+    std::vector<float> h_wval((size_t)n_ch * 2 * n_bl, 0.f);
+    for (int ch = 0; ch < n_ch; ++ch) {
+      const HostGather &g = gathers[ch];
+      std::vector<std::pair<int32_t, float>> ent;
+      for (int j = 0; j < g.n_can; ++j) {
+        const int c = g.can_cell[j], ix = c % N, iy = c / N;
+        const int kx = ix < N / 2 ? ix : ix - N;
+        int cnt = g.seg_start[j + 1] - g.seg_start[j];
+        if (c == 0) cnt *= 2;                       // DC holds V and conj(V) of each baseline
+        const float w = 1.0f / (float)cnt;
+        if (kx >= 0) ent.push_back({(kx << 16) | iy, w});
+        if (kx <= 0 && c != 0) ent.push_back({((-kx) << 16) | ((N - iy) % N), w});
+      }
+      std::sort(ent.begin(), ent.end());
+      int32_t *wc = h_wcol.data() + (size_t)ch * (p->wu + 1);
+      size_t e = 0;
+      for (int kx = 0; kx < p->wu; ++kx) {
+        wc[kx] = (int32_t)e;
+        while (e < ent.size() && (ent[e].first >> 16) == kx) ++e;
+      }
+      wc[p->wu] = (int32_t)ent.size();
+      for (size_t k = 0; k < ent.size(); ++k) {
+        h_wkey[(size_t)ch * 2 * n_bl + k] = ent[k].first;
+        h_wval[(size_t)ch * 2 * n_bl + k] = ent[k].second;
+      }
+    }
+    PLAN_TRY(dev_alloc(&p->d_wkey, h_wkey.size()));
+    PLAN_TRY(dev_alloc(&p->d_wval, h_wval.size()));
+    PLAN_TRY(dev_alloc(&p->d_wcol, h_wcol.size()));
+    step(cudaMemcpyAsync(p->d_wkey, h_wkey.data(), sizeof(int32_t) * h_wkey.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_wval, h_wval.data(), sizeof(float) * h_wval.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_wcol, h_wcol.data(), sizeof(int32_t) * h_wcol.size(), cudaMemcpyHostToDevice, st));
+    step(cudaStreamSynchronize(st));
+    PLAN_CUDA(ce, "weight table upload");
+  }
 #undef PLAN_TRY
 #undef PLAN_CUDA
   *out = p;
