@@ -156,6 +156,8 @@ def main():
     ap.add_argument("--n-t", type=int, default=0, help="override time steps per batch (0 = config)")
     ap.add_argument("--ref-time-steps", type=int, default=4,
                     help="time steps per step of the CPU reference / cpu_baseline sample")
+    ap.add_argument("--path", default="separate", choices=["separate", "fused"],
+                    help="separate = blink_grid + blink_image; fused = blink_grid_image")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -189,7 +191,8 @@ def main():
     plan.reserve(w.n_t)
     vis = vis_h.cuda(non_blocking=True)
     shape = (w.n_t, w.n_ch, w.n_pix, w.n_pix)
-    uv = torch.empty(shape, dtype=torch.complex64, device="cuda")
+    fused = args.path == "fused"
+    uv = None if fused else torch.empty(shape, dtype=torch.complex64, device="cuda")
     img = torch.empty(shape, dtype=torch.float32, device="cuda")
     img_h = torch.empty(shape, dtype=torch.float32).pin_memory()
     stream = torch.cuda.current_stream()
@@ -200,8 +203,11 @@ def main():
         torch.cuda.synchronize()
 
     def step():
-        plan.grid(vis, uv)
-        plan.image(uv, img)
+        if fused:
+            plan.grid_image(vis, img)
+        else:
+            plan.grid(vis, uv)
+            plan.image(uv, img)
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -216,9 +222,13 @@ def main():
     barrier()
     ev[0].record(stream)
     for k in range(args.steps):
-        plan.grid(vis, uv)
-        ev[3 * k + 1].record(stream)
-        plan.image(uv, img)
+        if fused:
+            plan.grid_image(vis, img)
+            ev[3 * k + 1].record(stream)
+        else:
+            plan.grid(vis, uv)
+            ev[3 * k + 1].record(stream)
+            plan.image(uv, img)
         ev[3 * k + 2].record(stream)
         ev[3 * k + 3].record(stream)
     barrier()
@@ -239,8 +249,7 @@ def main():
     if not args.no_e2e:
         def e2e_step():
             vis.copy_(vis_h, non_blocking=True)
-            plan.grid(vis, uv)
-            plan.image(uv, img)
+            step()
             img_h.copy_(img, non_blocking=True)
         e2e_step()
         barrier()
@@ -267,19 +276,29 @@ def main():
     # ---- roofline (HBM-bound scan/scatter work), dominant call
     peak, peak_src = measured_peaks()
     ab = algorithmic_bytes(w)
-    calls = {"blink_grid": (grid_ms, ab["grid"]), "blink_image": (image_ms, ab["image"])}
+    if fused:
+        nn = w.n_pix * w.n_pix
+        ab["fused"] = 8 * w.n_bl + 4 * nn          # SURVEY.md 8(d) B_fused: no uv grid in HBM
+        calls = {"blink_grid_image": (grid_ms, ab["fused"])}
+        ab["step"] = ab["fused"]
+    else:
+        calls = {"blink_grid": (grid_ms, ab["grid"]), "blink_image": (image_ms, ab["image"])}
     dom = max(calls, key=lambda k: calls[k][0])
     achieved = calls[dom][1] * n_snap / (calls[dom][0] / 1e3) / 1e9
     step_gbs = ab["step"] * n_snap / (ms_per_step / 1e3) / 1e9
     chunks = -(-n_snap // max(1, plan.query_i32(blink.Q_IMAGE_CHUNK)))
-    launches_per_step = 1 + 2 * chunks
+    if fused:
+        launches_per_step = 3 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))
+    else:
+        launches_per_step = 1 + 2 * chunks
     out = {
         "metric": "dirty_images_per_s", "value": value, "unit": "images/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "mvis_per_s": value * w.n_bl / 1e6,
         "config": workload_config(w, args.workload),
-        "per_call_ms": {"blink_grid": grid_ms, "blink_image": image_ms},
+        "path": args.path, "per_call_ms": {k: v[0] for k, v in calls.items()},
+        "images_per_s_vs_sep_roofline": value / (peak * 1e9 / (8 * w.n_bl + 20 * w.n_pix * w.n_pix)),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                      "algorithmic_bytes_per_snapshot": calls[dom][1]},

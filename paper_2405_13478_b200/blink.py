@@ -17,11 +17,11 @@ LIB_PATH = os.path.join(_HERE, "libblink.so")
 NATURAL, UNIFORM = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
 (Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
- Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK) = range(14)
+ Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK) = range(16)
 
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create",
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
-           "blink_grid",
+           "blink_grid", "blink_grid_image",
            "blink_image", "blink_host_build_gather"]
 
 _lib = None
@@ -64,6 +64,8 @@ def load() -> ctypes.CDLL:
     lib.blink_grid.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_image.restype = ci
     lib.blink_image.argtypes = [vp, vp, ci, vp, vp]
+    lib.blink_grid_image.restype = ci
+    lib.blink_grid_image.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_host_build_gather.restype = ci
     lib.blink_host_build_gather.argtypes = [vp, ci, ci, vp, vp, vp, vp]
     _lib = lib
@@ -200,4 +202,19 @@ class Plan:
         assert images.is_cuda and images.dtype == torch.float32 and images.is_contiguous()
         _check(self._lib.blink_image(self._h, uv_grid.data_ptr(), n_t, images.data_ptr(),
                                      _stream_ptr(stream)), "blink_image")
+        return images
+
+    def grid_image(self, vis, images=None, stream=None):
+        """blink_grid_image: vis complex64 [n_t, n_ch, n_bl] -> images float32 [n_t, n_ch, N, N]."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        n_t = vis.shape[0]
+        assert tuple(vis.shape[1:]) == (self.n_ch, self.n_bl)
+        if images is None:
+            images = torch.empty((n_t, self.n_ch, self.n_pix, self.n_pix), dtype=torch.float32,
+                                 device=vis.device)
+        assert images.is_cuda and images.dtype == torch.float32 and images.is_contiguous()
+        assert tuple(images.shape) == (n_t, self.n_ch, self.n_pix, self.n_pix)
+        _check(self._lib.blink_grid_image(self._h, vis.data_ptr(), n_t, images.data_ptr(),
+                                          _stream_ptr(stream)), "blink_grid_image")
         return images

@@ -23,23 +23,9 @@
 #include <algorithm>
 
 #include "blink_internal.h"
+#include "sphase.cuh"
 
 namespace blink {
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) {
-  return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void bulk_store(void *gdst, const void *ssrc, uint32_t bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst),
-               "r"(smem_u32(ssrc)), "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void bulk_wait_read() {
-  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
-}
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 struct GridParams {
   const float2 *vis;
@@ -49,43 +35,13 @@ struct GridParams {
   const uint32_t *cellrec;
   const int32_t *nact;
   const int32_t *pcell, *pcode, *pband;
-  int n_bl, n_ch, n_snap, n_bands, band_cells, parts, n_can_max, n_pass, roff_stride, dbg;
+  int n_bl, n_ch, n_snap, n_bands, band_cells, parts, n_can_max, n_pass, roff_stride, dbg, ch0;
   long long grid_cells;  // N*N
 };
-
-// registers of one pass: PF visibilities per thread and their stage slots
-template <int PF> struct PassRegs {
-  float2 v[PF];
-  uint16_t sc[PF];
-};
-
-template <int THREADS, int PF>
-__device__ __forceinline__ void pass_load(PassRegs<PF> &r, const float2 *__restrict__ vis,
-                                          const uint16_t *__restrict__ scat, int b0, int cnt, int tid) {
-#pragma unroll
-  for (int q = 0; q < PF; ++q) {
-    const int i = q * THREADS + tid;
-    r.sc[q] = kScatDropped;
-    if (i < cnt) {
-      r.sc[q] = scat[b0 + i];
-      r.v[q] = __ldcs(vis + b0 + i);               // streamed once: evict-first
-    }
-  }
-}
-
-template <int PF> __device__ __forceinline__ void pass_scatter(const PassRegs<PF> &r, float2 *stage) {
-#pragma unroll
-  for (int q = 0; q < PF; ++q) {
-    const uint32_t sc = r.sc[q];
-    if (sc != kScatDropped)
-      stage[sc & 0x7FFFu] = make_float2(r.v[q].x, (sc & 0x8000u) ? -r.v[q].y : r.v[q].y);
-  }
-}
 
 template <int THREADS, int PF, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
   constexpr int CAP = THREADS * PF;
-  constexpr int CPT = kGridCellsPerThread;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float2 *zero = reinterpret_cast<float2 *>(smem_raw);           // [band_cells]
   float2 *S = zero + p.band_cells;                               // [n_can_max]
@@ -105,12 +61,12 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
   PassRegs<PF> regs;
   if (blockIdx.x < n_items) {   // prefetch pass 0 of the first item
     const int s = (int)(blockIdx.x / p.parts);
-    pass_load<THREADS, PF>(regs, p.vis + (size_t)s * p.n_bl, p.scat + (size_t)(s % p.n_ch) * p.n_bl, 0,
+    pass_load<THREADS, PF>(regs, p.vis + (size_t)s * p.n_bl, p.scat + (size_t)((s + p.ch0) % p.n_ch) * p.n_bl, 0,
                            min(CAP, p.n_bl), tid);
   }
   for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
     const int s = (int)(item / p.parts), part = (int)(item % p.parts);
-    const int ch = s % p.n_ch;
+    const int ch = (s + p.ch0) % p.n_ch;
     const ChannelInfo ci = p.chinfo[ch];
     const float2 *__restrict__ vis = p.vis + (size_t)s * p.n_bl;
     const uint16_t *__restrict__ scat = p.scat + (size_t)ch * p.n_bl;
@@ -135,49 +91,13 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
         pass_load<THREADS, PF>(regs, vis, scat, b0, min(CAP, p.n_bl - b0), tid);
       } else if (item + gridDim.x < n_items) {
         const int s2 = (int)((item + gridDim.x) / p.parts);
-        pass_load<THREADS, PF>(regs, p.vis + (size_t)s2 * p.n_bl, p.scat + (size_t)(s2 % p.n_ch) * p.n_bl,
+        pass_load<THREADS, PF>(regs, p.vis + (size_t)s2 * p.n_bl, p.scat + (size_t)((s2 + p.ch0) % p.n_ch) * p.n_bl,
                                0, min(CAP, p.n_bl), tid);
       }
       const size_t cp = (size_t)ch * p.n_pass + pass;
-      const uint32_t *__restrict__ cellrec = p.cellrec + cp * max(p.n_can_max, 1);
-      const uint16_t *__restrict__ roff = p.roff + cp * p.roff_stride;
-      const int n_act = p.nact[cp];
-      // cells are ordered by descending length: rank r is held by the first n_r cells, so every
-      // thread runs the same r loop and its CPT accumulators are independent (ILP, no divergence)
-      for (int k0 = 0; k0 < n_act && !(p.dbg & 2); k0 += CPT * THREADS) {
-        uint32_t rec[CPT];
-        float2 acc[CPT];
-#pragma unroll
-        for (int c = 0; c < CPT; ++c) {
-          const int k = k0 + c * THREADS + tid;
-          rec[c] = k < n_act ? cellrec[k] : 0u;
-          acc[c] = make_float2(0.f, 0.f);
-        }
-        const int maxlen = (int)(cellrec[k0] >> 16);
-        int off = roff[0];
-        for (int r = 0; r < maxlen; ++r) {
-          const int off1 = roff[r + 1];
-          const int n_r = off1 - off;            // cells (from position 0) that have a rank-r entry
-#pragma unroll
-          for (int c = 0; c < CPT; ++c) {
-            const int k = k0 + c * THREADS + tid;
-            if (k < n_r) {
-              const float2 v = stage[off + k];
-              acc[c].x += v.x;
-              acc[c].y += v.y;
-            }
-          }
-          off = off1;
-        }
-#pragma unroll
-        for (int c = 0; c < CPT; ++c) {
-          if (rec[c] >> 16) {
-            const int j = rec[c] & 0xFFFFu;
-            const float2 a = S[j];
-            S[j] = make_float2(a.x + acc[c].x, a.y + acc[c].y);
-          }
-        }
-      }
+      if (!(p.dbg & 2))
+        sphase_sums<THREADS>(p.cellrec + cp * max(p.n_can_max, 1), p.roff + cp * p.roff_stride, p.nact[cp],
+                             stage, S, tid);
       if (pass + 1 == p.n_pass && tid == 0) bulk_wait_all();   // the zero fill has landed
       __syncthreads();
     }
@@ -230,11 +150,11 @@ static int launch_grid_v(const blink_plan *p, const GridParams &g0, cudaStream_t
   return BLINK_OK;
 }
 
-int launch_grid(const blink_plan *p, const float2 *vis, int n_t, float2 *uv, cudaStream_t st) {
+int launch_grid(const blink_plan *p, const float2 *vis, int n_snap, int ch0, float2 *uv, cudaStream_t st) {
   GridParams g;
   g.vis = vis; g.uv = uv; g.chinfo = p->d_chinfo;
   g.scat = p->d_scat; g.roff = p->d_roff; g.cellrec = p->d_cellrec; g.nact = p->d_nact; g.pcell = p->d_pcell; g.pcode = p->d_pcode; g.pband = p->d_pband;
-  g.n_bl = p->n_bl; g.n_ch = p->n_ch; g.n_snap = n_t * p->n_ch;
+  g.n_bl = p->n_bl; g.n_ch = p->n_ch; g.n_snap = n_snap; g.ch0 = ch0;
   g.n_bands = p->n_bands; g.band_cells = p->band_cells; g.n_can_max = p->n_can_max;
   g.n_pass = p->n_pass; g.roff_stride = p->roff_stride; g.parts = 1;
   g.dbg = 0;
@@ -253,5 +173,5 @@ extern "C" int blink_grid(const blink_plan *plan, const void *vis, int n_t, void
   if (n_t == 0) return BLINK_OK;
   if (!vis || !uv_grid) return BLINK_EINVAL;
   if (((uintptr_t)vis & 7) || ((uintptr_t)uv_grid & 15)) return BLINK_EINVAL;
-  return blink::launch_grid(plan, (const float2 *)vis, n_t, (float2 *)uv_grid, (cudaStream_t)stream);
+  return blink::launch_grid(plan, (const float2 *)vis, n_t * plan->n_ch, 0, (float2 *)uv_grid, (cudaStream_t)stream);
 }

@@ -37,7 +37,7 @@ struct ImgParams {
   const int32_t *wkey, *wcol;
   const float *wval;
   const float2 *tw;
-  int n_ch, n_bl, wu, uniform, snap_base;
+  int n_ch, n_bl, wu, uniform, snap_base, ch0;
 };
 
 // run stages 1.. of the transform; stage 0's load is done by the caller
@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_image_cols(const ImgParams p)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cf32 *lines = reinterpret_cast<cf32 *>(smem_raw);
   const int tid = threadIdx.x;
-  const int sl = blockIdx.y, s = p.snap_base + sl, ch = s % p.n_ch;
+  const int sl = blockIdx.y, s = p.snap_base + sl, ch = (s + p.ch0) % p.n_ch;
   const ChannelInfo ci = p.chinfo[ch];
   const int kx0 = blockIdx.x * CT;
   const float2 *__restrict__ G = p.uv + (size_t)s * N * N;
@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(RP * (N / 16)) k_image_rows(const ImgParams p)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cf32 *lines = reinterpret_cast<cf32 *>(smem_raw);
   const int tid = threadIdx.x;
-  const int sl = blockIdx.y, s = p.snap_base + sl, ch = s % p.n_ch;
+  const int sl = blockIdx.y, s = p.snap_base + sl, ch = (s + p.ch0) % p.n_ch;
   const int kxm = p.chinfo[ch].kx_max;
   const int pr = tid / C::T, t = tid % C::T;
   const int y0 = blockIdx.x * RP + pr, y1 = y0 + N / 2;
@@ -160,7 +160,9 @@ static int run_image_cfg(const blink_plan *p, ImgParams ip, int n_snap, cudaStre
     if (rc != BLINK_OK) return rc;
     attr_done = true;
   }
-  const int chunk = std::max(1, p->chunk_snapshots);
+  const size_t per_snap = sizeof(float2) * (size_t)N * p->wu;
+  const int chunk = (int)std::min<size_t>((size_t)std::max(1, p->chunk_snapshots), p->scratch_bytes / per_snap);
+  if (chunk < 1) return BLINK_ENOMEM;
   for (int base = 0; base < n_snap; base += chunk) {
     const int cs = std::min(chunk, n_snap - base);
     ip.snap_base = base;
@@ -228,13 +230,13 @@ int image_reserve(blink_plan *p, int n_t) {
   return BLINK_OK;
 }
 
-int launch_image(const blink_plan *p, const float2 *uv, int n_t, float *img, cudaStream_t st) {
+int launch_image(const blink_plan *p, const float2 *uv, int n_snap, int ch0, float *img, cudaStream_t st) {
   ImgParams ip;
   ip.uv = uv; ip.img = img; ip.U = p->d_scratch; ip.chinfo = p->d_chinfo;
   ip.wkey = p->d_wkey; ip.wval = p->d_wval; ip.wcol = p->d_wcol; ip.n_bl = p->n_bl;
   ip.tw = p->d_tw; ip.n_ch = p->n_ch; ip.wu = p->wu; ip.uniform = p->weighting == BLINK_UNIFORM;
   ip.snap_base = 0;
-  const int n_snap = n_t * p->n_ch;
+  ip.ch0 = ch0;
   switch (p->n_pix) {
     case 32: return run_image_n<32>(p, ip, n_snap, st);
     case 64: return run_image_n<64>(p, ip, n_snap, st);
@@ -257,5 +259,5 @@ extern "C" int blink_image(const blink_plan *plan, const void *uv_grid, int n_t,
   if (((uintptr_t)uv_grid & 7) || ((uintptr_t)images & 3)) return BLINK_EINVAL;
   int rc = blink::image_reserve(const_cast<blink_plan *>(plan), n_t);
   if (rc != BLINK_OK) return rc;
-  return blink::launch_image(plan, (const float2 *)uv_grid, n_t, (float *)images, (cudaStream_t)stream);
+  return blink::launch_image(plan, (const float2 *)uv_grid, n_t * plan->n_ch, 0, (float *)images, (cudaStream_t)stream);
 }

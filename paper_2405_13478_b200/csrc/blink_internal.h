@@ -86,6 +86,19 @@ struct blink_plan {
   size_t scratch_bytes = 0;
   int image_path = 1;
   int chunk_snapshots = 0;
+
+  // blink_grid_image
+  int fused_path = 0;               // 1 = shared-memory single kernel, 0 = chunked grid + image
+  int fused_chunk = 0;              // snapshots per chunk of the chunked route
+  float2 *d_uv_scratch = nullptr;   // [fused_chunk][N][N]
+  // shared-memory route: occupied cells with kx >= 0 -> slot in the column lines, source, weight
+  int32_t *d_hpos = nullptr;        // [n_ch][2 n_bl] kx * LS + pad16(iy)
+  int32_t *d_hcode = nullptr;       // [n_ch][2 n_bl] j | flag << kPlaceShift
+  float *d_hw = nullptr;            // [n_ch][2 n_bl] sign * (1/norm) * (1/count if uniform)
+  int32_t *d_hcount = nullptr;      // [n_ch]
+  int fused_threads = 512, fused_prefetch = 16;
+  size_t fused_smem = 0;
+  size_t uv_scratch_bytes = 0;
 };
 
 namespace blink {
@@ -96,10 +109,16 @@ int build_gather_host(const int32_t *cell, int n_bl, int n_pix, HostGather &out)
 // kernels' host launchers (each returns a blink_status)
 int launch_index_kernel(blink_plan *p, const double *d_ant, const double *d_freq,
                         const int32_t *d_pi, const int32_t *d_pj, cudaStream_t st);
-int launch_grid(const blink_plan *p, const float2 *vis, int n_t, float2 *uv, cudaStream_t st);
-int launch_image(const blink_plan *p, const float2 *uv, int n_t, float *img, cudaStream_t st);
+// n_snap consecutive snapshots whose first one is channel ch0 (channel of snapshot s = (ch0 + s) % n_ch)
+int launch_grid(const blink_plan *p, const float2 *vis, int n_snap, int ch0, float2 *uv, cudaStream_t st);
+int launch_image(const blink_plan *p, const float2 *uv, int n_snap, int ch0, float *img, cudaStream_t st);
 int image_setup(blink_plan *p);
 int image_reserve(blink_plan *p, int n_t);
+int fused_setup(blink_plan *p);
+int fused_line_stride(int n_pix);
+size_t fused_smem_bytes(const blink_plan *p, int threads, int prefetch);
+int fused_reserve(blink_plan *p, int n_t);
+int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);
 
 }  // namespace blink
 

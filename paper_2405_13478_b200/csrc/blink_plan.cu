@@ -125,7 +125,7 @@ static void plan_free(blink_plan *p) {
   if (!p) return;
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
-  cudaFree(p->d_tw); cudaFree(p->d_scratch);
+  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_uv_scratch); cudaFree(p->d_hpos); cudaFree(p->d_hcode); cudaFree(p->d_hw); cudaFree(p->d_hcount);
   delete p;
 }
 
@@ -421,6 +421,50 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   step(cudaStreamSynchronize(st));
   PLAN_CUDA(ce, "plan table upload");
   PLAN_TRY(image_setup(p));
+  PLAN_TRY(fused_setup(p));
+  if (p->fused_path == 1) {
+    const int LS = fused_line_stride(N);
+    std::vector<int32_t> h_hpos((size_t)n_ch * 2 * n_bl, 0), h_hcode((size_t)n_ch * 2 * n_bl, 0), h_hcount(n_ch, 0);
+    std::vector<float> h_hw((size_t)n_ch * 2 * n_bl, 0.f);
+    for (int ch = 0; ch < n_ch; ++ch) {
+      const HostGather &g = gathers[ch];
+      const float inv_norm = p->chinfo[ch].inv_norm;
+      size_t n = 0;
+      const size_t base = (size_t)ch * 2 * n_bl;
+      for (int j = 0; j < g.n_can; ++j) {
+        const int c = g.can_cell[j], ix = c % N, iy = c / N;
+        const int kx = ix < N / 2 ? ix : ix - N, ky = iy;          // canonical: 0 <= ky < N/2
+        int cnt = g.seg_start[j + 1] - g.seg_start[j];
+        if (c == 0) cnt *= 2;
+        float w = ((kx + ky) & 1) ? -inv_norm : inv_norm;
+        if (weighting == BLINK_UNIFORM) w /= (float)cnt;
+        auto pad16 = [](int i) { return i + (i >> 4); };
+        if (kx >= 0) {
+          h_hpos[base + n] = kx * LS + pad16(iy);
+          h_hcode[base + n] = j | ((c == 0 ? kPlaceBoth : kPlaceDirect) << kPlaceShift);
+          h_hw[base + n] = w;
+          ++n;
+        }
+        if (kx <= 0 && c != 0) {
+          h_hpos[base + n] = (-kx) * LS + pad16((N - iy) % N);
+          h_hcode[base + n] = j | (kPlaceConj << kPlaceShift);
+          h_hw[base + n] = w;
+          ++n;
+        }
+      }
+      h_hcount[ch] = (int32_t)n;
+    }
+    PLAN_TRY(dev_alloc(&p->d_hpos, h_hpos.size()));
+    PLAN_TRY(dev_alloc(&p->d_hcode, h_hcode.size()));
+    PLAN_TRY(dev_alloc(&p->d_hw, h_hw.size()));
+    PLAN_TRY(dev_alloc(&p->d_hcount, h_hcount.size()));
+    step(cudaMemcpyAsync(p->d_hpos, h_hpos.data(), sizeof(int32_t) * h_hpos.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_hcode, h_hcode.data(), sizeof(int32_t) * h_hcode.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_hw, h_hw.data(), sizeof(float) * h_hw.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_hcount, h_hcount.data(), sizeof(int32_t) * n_ch, cudaMemcpyHostToDevice, st));
+    step(cudaStreamSynchronize(st));
+    PLAN_CUDA(ce, "fused table upload");
+  }
   if (weighting == BLINK_UNIFORM) {
     // canonical cells are exactly the occupied half-plane cells with ky > 0 or (ky == 0, kx >= 0);
     // pass A of blink_image works on columns kx >= 0 and all ky, so list every occupied cell with
@@ -475,7 +519,9 @@ extern "C" int blink_plan_destroy(blink_plan *plan) {
 
 extern "C" int blink_plan_reserve(blink_plan *plan, int n_t) {
   if (!plan || n_t < 0) return BLINK_EINVAL;
-  return image_reserve(plan, n_t);
+  int rc = image_reserve(plan, n_t);
+  if (rc != BLINK_OK) return rc;
+  return fused_reserve(plan, n_t);
 }
 
 extern "C" int blink_plan_read(const blink_plan *p, int what, int ch, void *dst, size_t bytes) {
@@ -520,6 +566,8 @@ extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *
     case BLINK_Q_IMAGE_PATH: *(int32_t *)out = p->image_path; break;
     case BLINK_Q_SCRATCH_BYTES: *(int64_t *)out = (int64_t)p->scratch_bytes; break;
     case BLINK_Q_IMAGE_CHUNK: *(int32_t *)out = p->chunk_snapshots; break;
+    case BLINK_Q_FUSED_PATH: *(int32_t *)out = p->fused_path; break;
+    case BLINK_Q_FUSED_CHUNK: *(int32_t *)out = p->fused_chunk; break;
     default: return BLINK_EINVAL;
   }
   return BLINK_OK;

@@ -238,3 +238,34 @@ def test_full_size_station_launch_configuration(torch_cuda, blink, oracle):
         peak = np.max(np.abs(ref["images"][q]))
         assert np.max(np.abs(imh[q] - ref["images"][q])) <= IMG_TOL * peak
     plan.close()
+
+
+@pytest.mark.parametrize("name", ["tiny", "station", "station128", "mwa1", "station_uniform_32",
+                                  "mwa1_natural_64"])
+def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name):
+    """blink_grid_image (one call, no uv grid in caller memory; shared-memory route where the plan
+    allows it, chunked route otherwise) against blink_grid + blink_image (fp32 rounding apart) and
+    against the oracle at the image bar."""
+    torch = torch_cuda
+    w = _workload(name)
+    vis_h = w.vis()
+    vis = torch.from_numpy(vis_h).cuda()
+    plan = _plan(blink, w)
+    ref = plan.image(plan.grid(vis))
+    img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(vis, img)
+    assert torch.isfinite(img).all()
+    peak = ref.abs().amax(dim=(-2, -1), keepdim=True)
+    assert ((img - ref).abs() <= 1e-5 * peak).all()
+    n_snap = w.n_t * w.n_ch
+    sel = np.array([0, n_snap - 1], np.int64) if w.n_pix >= 512 else np.arange(min(n_snap, 8), dtype=np.int64)
+    orc = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_h, sel)
+    got = img.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        pk = np.max(np.abs(orc["images"][q]))
+        assert np.max(np.abs(got[q] - orc["images"][q])) <= IMG_TOL * pk
+    if name in ("tiny", "station", "station128", "station_uniform_32"):
+        assert plan.query_i32(blink.Q_FUSED_PATH) == 1     # these fit the shared-memory route
+    if name == "mwa1":
+        assert plan.query_i32(blink.Q_FUSED_PATH) == 0
+    plan.close()
