@@ -156,8 +156,9 @@ def main():
     ap.add_argument("--n-t", type=int, default=0, help="override time steps per batch (0 = config)")
     ap.add_argument("--ref-time-steps", type=int, default=4,
                     help="time steps per step of the CPU reference / cpu_baseline sample")
-    ap.add_argument("--path", default="separate", choices=["separate", "fused"],
-                    help="separate = blink_grid + blink_image; fused = blink_grid_image")
+    ap.add_argument("--path", default="auto", choices=["auto", "separate", "fused"],
+                    help="separate = blink_grid + blink_image (uv grid in HBM); fused = blink_grid_image; "
+                         "auto = fused when the plan has the shared-memory route, else separate")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -191,7 +192,8 @@ def main():
     plan.reserve(w.n_t)
     vis = vis_h.cuda(non_blocking=True)
     shape = (w.n_t, w.n_ch, w.n_pix, w.n_pix)
-    fused = args.path == "fused"
+    fused = args.path == "fused" or (args.path == "auto" and plan.query_i32(blink.Q_FUSED_PATH) == 1)
+    args.path = "fused" if fused else "separate"
     uv = None if fused else torch.empty(shape, dtype=torch.complex64, device="cuda")
     img = torch.empty(shape, dtype=torch.float32, device="cuda")
     img_h = torch.empty(shape, dtype=torch.float32).pin_memory()
@@ -288,7 +290,10 @@ def main():
     step_gbs = ab["step"] * n_snap / (ms_per_step / 1e3) / 1e9
     chunks = -(-n_snap // max(1, plan.query_i32(blink.Q_IMAGE_CHUNK)))
     if fused:
-        launches_per_step = 3 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))
+        if plan.query_i32(blink.Q_FUSED_PATH) == 1:
+            launches_per_step = 1
+        else:
+            launches_per_step = 3 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))
     else:
         launches_per_step = 1 + 2 * chunks
     out = {

@@ -35,8 +35,10 @@ struct FusedParams {
   const int32_t *nact, *hpos, *hcode, *hcount;
   const float *hw;
   const float2 *tw;
-  int n_bl, n_ch, n_snap, n_can_max, n_pass, roff_stride, n_col, ky_max_all;
+  int n_bl, n_ch, n_snap, n_can_max, n_pass, roff_stride, n_col, ky_max_all, h_max;
 };
+
+constexpr int kHPer = 5;   // phase-H table entries fetched per thread at a time
 
 int fused_line_stride(int n_pix) { return ((n_pix + n_pix / 16 + 15) / 16) * 16 + 1; }
 
@@ -67,8 +69,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
     const uint16_t *__restrict__ scat = p.scat + (size_t)ch * p.n_bl;
 
     // ---- phase S ----------------------------------------------------------------------------
-    for (int j = tid; j < ci.n_can; j += THREADS) S[j] = make_float2(0.f, 0.f);
+    for (int j = tid; j < p.n_can_max; j += THREADS) S[j] = make_float2(0.f, 0.f);
     for (int pass = 0; pass < p.n_pass; ++pass) {
+      const size_t cp = (size_t)ch * p.n_pass + pass;
+      const uint32_t *__restrict__ cellrec = p.cellrec + cp * max(p.n_can_max, 1);
+      SumsRegs<THREADS> sr;
+      sums_prefetch<THREADS>(sr, cellrec, p.n_can_max, tid);
       pass_scatter<PF>(regs, X);
       __syncthreads();
       if (pass + 1 < p.n_pass) {
@@ -79,9 +85,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
         pass_load<THREADS, PF>(regs, p.vis + (size_t)s2 * p.n_bl, p.scat + (size_t)(s2 % p.n_ch) * p.n_bl,
                                0, min(CAP, p.n_bl), tid);
       }
-      const size_t cp = (size_t)ch * p.n_pass + pass;
-      sphase_sums<THREADS>(p.cellrec + cp * max(p.n_can_max, 1), p.roff + cp * p.roff_stride, p.nact[cp],
-                           X, S, tid);
+      sums_run<THREADS>(sr, cellrec, p.roff + cp * p.roff_stride, p.n_can_max, X, S, tid);
       __syncthreads();
     }
 
@@ -91,21 +95,32 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
       const int c = e / nrow, iy = (e % nrow - kym + N) & (N - 1);
       lines[c * LS + pad16(iy)] = make_float2(0.f, 0.f);
     }
-    __syncthreads();
     {
       const size_t hb = (size_t)ch * 2 * p.n_bl;
-      const int nh = p.hcount[ch];
-      for (int e = tid; e < nh; e += THREADS) {
-        const int code = p.hcode[hb + e];
-        const float w = p.hw[hb + e];
-        const float2 v = S[code & kPlaceMask];
-        const int flag = code >> kPlaceShift;
-        float2 o;
-        if (flag == kPlaceDirect) o = make_float2(v.x * w, v.y * w);
-        else if (flag == kPlaceConj) o = make_float2(v.x * w, -v.y * w);
-        else o = make_float2((v.x + v.x) * w, 0.f);
-        lines[p.hpos[hb + e]] = o;
+      for (int e0 = 0; e0 < p.h_max; e0 += kHPer * THREADS) {
+        int code[kHPer], pos[kHPer];
+        float w[kHPer];
+#pragma unroll
+        for (int c = 0; c < kHPer; ++c) {          // independent table loads, issued together
+          const int e = e0 + c * THREADS + tid;
+          pos[c] = e < p.h_max ? __ldg(p.hpos + hb + e) : -1;
+          code[c] = e < p.h_max ? __ldg(p.hcode + hb + e) : 0;
+          w[c] = e < p.h_max ? __ldg(p.hw + hb + e) : 0.f;
+        }
+        if (e0 == 0) __syncthreads();               // the zero fill above is complete
+#pragma unroll
+        for (int c = 0; c < kHPer; ++c) {
+          if (pos[c] < 0) continue;                  // tables are padded with pos = -1
+          const float2 v = S[code[c] & kPlaceMask];
+          const int flag = code[c] >> kPlaceShift;
+          float2 o;
+          if (flag == kPlaceDirect) o = make_float2(v.x * w[c], v.y * w[c]);
+          else if (flag == kPlaceConj) o = make_float2(v.x * w[c], -v.y * w[c]);
+          else o = make_float2((v.x + v.x) * w[c], 0.f);
+          lines[pos[c]] = o;
+        }
       }
+      if (p.h_max == 0) __syncthreads();
     }
     __syncthreads();
 
@@ -229,7 +244,7 @@ static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *
   fp.hcount = p->d_hcount; fp.hw = p->d_hw; fp.tw = p->d_tw;
   fp.n_bl = p->n_bl; fp.n_ch = p->n_ch; fp.n_snap = n_t * p->n_ch; fp.n_can_max = p->n_can_max;
   fp.n_pass = p->n_pass; fp.roff_stride = p->roff_stride; fp.n_col = p->kx_max_all + 1;
-  fp.ky_max_all = p->ky_max_all;
+  fp.ky_max_all = p->ky_max_all; fp.h_max = p->h_max;
   const bool pf16 = p->fused_prefetch == 16;
   switch (p->n_pix) {
     case 32: return pf16 ? launch_fused_n<32, 16>(p, fp, st) : launch_fused_n<32, 8>(p, fp, st);

@@ -81,8 +81,12 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
     }
 
     // ---- phase S: table-driven sort into the rank-major stage, then per-cell sums -----------
-    for (int j = tid; j < ci.n_can; j += THREADS) S[j] = make_float2(0.f, 0.f);
+    for (int j = tid; j < p.n_can_max; j += THREADS) S[j] = make_float2(0.f, 0.f);
     for (int pass = 0; pass < p.n_pass; ++pass) {
+      const size_t cp = (size_t)ch * p.n_pass + pass;
+      const uint32_t *__restrict__ cellrec = p.cellrec + cp * max(p.n_can_max, 1);
+      SumsRegs<THREADS> sr;
+      sums_prefetch<THREADS>(sr, cellrec, p.n_can_max, tid);
       if (!(p.dbg & 4)) pass_scatter<PF>(regs, stage);
       __syncthreads();
       // loads of the next pass (or of the next item's first pass) fly during the sums and phase P
@@ -94,10 +98,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
         pass_load<THREADS, PF>(regs, p.vis + (size_t)s2 * p.n_bl, p.scat + (size_t)((s2 + p.ch0) % p.n_ch) * p.n_bl,
                                0, min(CAP, p.n_bl), tid);
       }
-      const size_t cp = (size_t)ch * p.n_pass + pass;
-      if (!(p.dbg & 2))
-        sphase_sums<THREADS>(p.cellrec + cp * max(p.n_can_max, 1), p.roff + cp * p.roff_stride, p.nact[cp],
-                             stage, S, tid);
+      if (!(p.dbg & 2)) sums_run<THREADS>(sr, cellrec, p.roff + cp * p.roff_stride, p.n_can_max, stage, S, tid);
       if (pass + 1 == p.n_pass && tid == 0) bulk_wait_all();   // the zero fill has landed
       __syncthreads();
     }

@@ -20,7 +20,7 @@ constexpr int32_t kPlaceBoth = 2;    // grid[cell] = S[j] + conj(S[j])   (self-c
 
 constexpr int kBandCellsDefault = 2048;  // cells (complex64) per output band of the gridder = 16 KB
 constexpr uint16_t kScatDropped = 0xFFFFu;  // scatter code of a baseline outside the grid
-constexpr int kGridCellsPerThread = 8;      // register accumulators per thread in the per-cell sums
+constexpr int kGridCellsPerThread = 5;      // register accumulators per thread in the per-cell sums
 
 struct ChannelInfo {   // mirrored on the device, one per channel
   int32_t n_kept;      // baselines inside the grid
@@ -96,6 +96,7 @@ struct blink_plan {
   int32_t *d_hcode = nullptr;       // [n_ch][2 n_bl] j | flag << kPlaceShift
   float *d_hw = nullptr;            // [n_ch][2 n_bl] sign * (1/norm) * (1/count if uniform)
   int32_t *d_hcount = nullptr;      // [n_ch]
+  int h_max = 0;                    // max over channels of the entry count; tables padded with pos = -1
   int fused_threads = 512, fused_prefetch = 16;
   size_t fused_smem = 0;
   size_t uv_scratch_bytes = 0;

@@ -322,10 +322,10 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     p->grid_nbuf = nbuf;
     // CTA shape (threads, prefetch, CTAs/SM): variant 0 = 512 x 16 x 1, 1 = 256 x 16 x 2,
     // 2 = 512 x 8 x 2, 3 = 256 x 8 x 3
-    int variant = 1;
+    int variant = 0;
     if (const char *e = getenv("BLINK_GRID_VARIANT")) variant = atoi(e);
     static const int kVar[4][3] = {{512, 16, 1}, {256, 16, 2}, {512, 8, 2}, {256, 8, 3}};
-    if (variant < 0 || variant > 3) variant = 1;
+    if (variant < 0 || variant > 3) variant = 0;
     p->grid_threads = kVar[variant][0];
     p->grid_prefetch = kVar[variant][1];
     p->grid_ctas_per_sm = kVar[variant][2];
@@ -384,7 +384,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     }
   }
   if (p->n_can_max > 0xFFFF || kStageCap > 0x7FFF) { plan_free(p); return BLINK_EUNSUPPORTED; }
-  p->roff_stride = maxlen + 1;
+  p->roff_stride = ((maxlen + 1 + 3) / 4) * 4;   // rows stay 8-byte aligned for ushort4 reads
   std::vector<uint16_t> h_roff((size_t)n_ch * n_pass * p->roff_stride, 0);
   for (size_t i = 0; i < roffs.size(); ++i)
     std::copy(roffs[i].begin(), roffs[i].end(), h_roff.begin() + i * p->roff_stride);
@@ -424,7 +424,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   PLAN_TRY(fused_setup(p));
   if (p->fused_path == 1) {
     const int LS = fused_line_stride(N);
-    std::vector<int32_t> h_hpos((size_t)n_ch * 2 * n_bl, 0), h_hcode((size_t)n_ch * 2 * n_bl, 0), h_hcount(n_ch, 0);
+    std::vector<int32_t> h_hpos((size_t)n_ch * 2 * n_bl, -1), h_hcode((size_t)n_ch * 2 * n_bl, 0), h_hcount(n_ch, 0);
     std::vector<float> h_hw((size_t)n_ch * 2 * n_bl, 0.f);
     for (int ch = 0; ch < n_ch; ++ch) {
       const HostGather &g = gathers[ch];
@@ -453,6 +453,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
         }
       }
       h_hcount[ch] = (int32_t)n;
+      p->h_max = std::max(p->h_max, (int)n);
     }
     PLAN_TRY(dev_alloc(&p->d_hpos, h_hpos.size()));
     PLAN_TRY(dev_alloc(&p->d_hcode, h_hcode.size()));

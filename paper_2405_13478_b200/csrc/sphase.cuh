@@ -52,47 +52,57 @@ template <int PF> __device__ __forceinline__ void pass_scatter(const PassRegs<PF
   }
 }
 
-// Per-cell sums of one pass.  Cells are ordered by descending length: rank r is held by the first
-// n_r cells, so every thread runs the same r loop and its CPT accumulators are independent (ILP,
-// no divergence); consecutive threads read consecutive stage slots (no bank conflicts).
+// Per-cell sums of one pass.  Cells are ordered by descending length, so the lanes of a warp own
+// cells of (nearly) equal length: each thread walks its own cell, rank by rank, reading
+// stage[roff[r] + k] -- consecutive threads read consecutive slots (no bank conflicts, no atomics)
+// -- and adds in ascending baseline order.  roff is read four ranks at a time.  The cell records
+// of a pass are fetched into registers BEFORE the scatter and its barrier (sums_prefetch), so no
+// table latency is exposed between the barrier and the first shared-memory read; the tables are
+// zero-padded to n_can_max, so the prefetch needs no bound from memory.
+template <int THREADS> struct SumsRegs { uint32_t rec[kGridCellsPerThread]; };
+
 template <int THREADS>
-__device__ __forceinline__ void sphase_sums(const uint32_t *__restrict__ cellrec,
-                                            const uint16_t *__restrict__ roff, int n_act,
-                                            const float2 *stage, float2 *S, int tid) {
-  constexpr int CPT = kGridCellsPerThread;
-  for (int k0 = 0; k0 < n_act; k0 += CPT * THREADS) {
-    uint32_t rec[CPT];
-    float2 acc[CPT];
+__device__ __forceinline__ void sums_prefetch(SumsRegs<THREADS> &sr, const uint32_t *__restrict__ cellrec,
+                                              int n_can_max, int tid) {
 #pragma unroll
-    for (int c = 0; c < CPT; ++c) {
-      const int k = k0 + c * THREADS + tid;
-      rec[c] = k < n_act ? cellrec[k] : 0u;
-      acc[c] = make_float2(0.f, 0.f);
-    }
-    const int maxlen = (int)(cellrec[k0] >> 16);
-    int off = roff[0];
-    for (int r = 0; r < maxlen; ++r) {
-      const int off1 = roff[r + 1];
-      const int n_r = off1 - off;            // cells (from position 0) that have a rank-r entry
+  for (int c = 0; c < kGridCellsPerThread; ++c) {
+    const int k = tid + c * THREADS;
+    sr.rec[c] = k < n_can_max ? __ldg(cellrec + k) : 0u;
+  }
+}
+
+__device__ __forceinline__ void sum_cell(uint32_t rec, int k, const uint16_t *__restrict__ roff,
+                                         const float2 *stage, float2 *S) {
+  const int j = rec & 0xFFFFu, len = rec >> 16;
+  const float2 *__restrict__ col = stage + k;
+  float ax = 0.f, ay = 0.f;
+  int r = 0;
+  for (; r + 4 <= len; r += 4) {
+    const ushort4 o = *reinterpret_cast<const ushort4 *>(roff + r);     // roff stride is 4-aligned
+    const float2 v0 = col[o.x], v1 = col[o.y], v2 = col[o.z], v3 = col[o.w];
+    ax += v0.x; ay += v0.y;
+    ax += v1.x; ay += v1.y;
+    ax += v2.x; ay += v2.y;
+    ax += v3.x; ay += v3.y;
+  }
+  for (; r < len; ++r) {
+    const float2 v = col[roff[r]];
+    ax += v.x; ay += v.y;
+  }
+  const float2 a = S[j];
+  S[j] = make_float2(a.x + ax, a.y + ay);
+}
+
+template <int THREADS>
+__device__ __forceinline__ void sums_run(const SumsRegs<THREADS> &sr, const uint32_t *__restrict__ cellrec,
+                                         const uint16_t *__restrict__ roff, int n_can_max,
+                                         const float2 *stage, float2 *S, int tid) {
 #pragma unroll
-      for (int c = 0; c < CPT; ++c) {
-        const int k = k0 + c * THREADS + tid;
-        if (k < n_r) {
-          const float2 v = stage[off + k];
-          acc[c].x += v.x;
-          acc[c].y += v.y;
-        }
-      }
-      off = off1;
-    }
-#pragma unroll
-    for (int c = 0; c < CPT; ++c) {
-      if (rec[c] >> 16) {
-        const int j = rec[c] & 0xFFFFu;
-        const float2 a = S[j];
-        S[j] = make_float2(a.x + acc[c].x, a.y + acc[c].y);
-      }
-    }
+  for (int c = 0; c < kGridCellsPerThread; ++c)
+    if (sr.rec[c] >> 16) sum_cell(sr.rec[c], tid + c * THREADS, roff, stage, S);
+  for (int k = tid + kGridCellsPerThread * THREADS; k < n_can_max; k += THREADS) {
+    const uint32_t rec = cellrec[k];
+    if (rec >> 16) sum_cell(rec, k, roff, stage, S);
   }
 }
 
