@@ -100,6 +100,15 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def ref_time_steps(args, w):
+    """Bounded oracle sample: ~10-30 s of host work (naive separable DFT is O(N^3) per snapshot)."""
+    if args.ref_time_steps > 0:
+        return max(1, min(w.n_t, args.ref_time_steps))
+    target = {32: 1 << 20, 64: 1 << 18, 128: 1 << 15, 256: 4096, 512: 512, 1024: 96, 2048: 24, 4096: 24}
+    snaps = target.get(w.n_pix, 64)
+    return max(1, min(w.n_t, -(-snaps // w.n_ch)))
+
+
 def run_reference(args, w):
     """Reference arm = the CPU oracle as it stands, on the host cores, on a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
@@ -107,7 +116,7 @@ def run_reference(args, w):
         return
     from oracle import oracle as orc
     orc.build()
-    n_t_s = max(1, min(w.n_t, args.ref_time_steps))
+    n_t_s = ref_time_steps(args, w)
     vis = w.vis(0, n_t_s)
     sel = np.arange(n_t_s * w.n_ch, dtype=np.int64)
     per = []
@@ -154,8 +163,9 @@ def main():
     ap.add_argument("--workload", default="station")
     ap.add_argument("--impl", default="blink", choices=["blink", "reference"])
     ap.add_argument("--n-t", type=int, default=0, help="override time steps per batch (0 = config)")
-    ap.add_argument("--ref-time-steps", type=int, default=4,
-                    help="time steps per step of the CPU reference / cpu_baseline sample")
+    ap.add_argument("--ref-time-steps", type=int, default=0,
+                    help="time steps per step of the CPU reference / cpu_baseline sample "
+                         "(0 = sized for roughly 10-30 s of CPU work)")
     ap.add_argument("--path", default="auto", choices=["auto", "separate", "fused"],
                     help="separate = blink_grid + blink_image (uv grid in HBM); fused = blink_grid_image; "
                          "auto = fused when the plan has the shared-memory route, else separate")
@@ -323,7 +333,7 @@ def cpu_baseline(w, args):
     """The oracle as it stands, timed on this box's host cores, on a bounded sample."""
     from oracle import oracle as orc
     orc.build()
-    n_t_s = max(1, min(w.n_t, args.ref_time_steps))
+    n_t_s = ref_time_steps(args, w)
     vis = w.vis(0, n_t_s)
     sel = np.arange(n_t_s * w.n_ch, dtype=np.int64)
     t0 = time.perf_counter()
