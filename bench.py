@@ -100,12 +100,12 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def ref_time_steps(args, w):
+def ref_time_steps(args, w, scale=1.0):
     """Bounded oracle sample: ~10-30 s of host work (naive separable DFT is O(N^3) per snapshot)."""
     if args.ref_time_steps > 0:
         return max(1, min(w.n_t, args.ref_time_steps))
     target = {32: 1 << 20, 64: 1 << 18, 128: 1 << 15, 256: 4096, 512: 512, 1024: 96, 2048: 24, 4096: 24}
-    snaps = target.get(w.n_pix, 64)
+    snaps = max(1, int(target.get(w.n_pix, 64) * scale))
     return max(1, min(w.n_t, -(-snaps // w.n_ch)))
 
 
@@ -116,7 +116,7 @@ def run_reference(args, w):
         return
     from oracle import oracle as orc
     orc.build()
-    n_t_s = ref_time_steps(args, w)
+    n_t_s = ref_time_steps(args, w, 0.25)   # per step; K + W steps must end within minutes
     vis = w.vis(0, n_t_s)
     sel = np.arange(n_t_s * w.n_ch, dtype=np.int64)
     per = []
@@ -168,7 +168,7 @@ def main():
                          "(0 = sized for roughly 10-30 s of CPU work)")
     ap.add_argument("--path", default="auto", choices=["auto", "separate", "fused"],
                     help="separate = blink_grid + blink_image (uv grid in HBM); fused = blink_grid_image; "
-                         "auto = fused when the plan has the shared-memory route, else separate")
+                         "auto = fused")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -202,7 +202,7 @@ def main():
     plan.reserve(w.n_t)
     vis = vis_h.cuda(non_blocking=True)
     shape = (w.n_t, w.n_ch, w.n_pix, w.n_pix)
-    fused = args.path == "fused" or (args.path == "auto" and plan.query_i32(blink.Q_FUSED_PATH) == 1)
+    fused = args.path in ("fused", "auto")       # blink_grid_image is the fast public call
     args.path = "fused" if fused else "separate"
     uv = None if fused else torch.empty(shape, dtype=torch.complex64, device="cuda")
     img = torch.empty(shape, dtype=torch.float32, device="cuda")
@@ -303,7 +303,7 @@ def main():
         if plan.query_i32(blink.Q_FUSED_PATH) == 1:
             launches_per_step = 1
         else:
-            launches_per_step = 3 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))
+            launches_per_step = 2 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))
     else:
         launches_per_step = 1 + 2 * chunks
     out = {

@@ -73,8 +73,8 @@ typedef enum blink_query {
   BLINK_Q_IMAGE_PATH = 11,/* out: int32   0 = shared-memory single pass, 1 = two-pass */
   BLINK_Q_SCRATCH_BYTES = 12, /* out: int64 device scratch currently held by the plan */
   BLINK_Q_IMAGE_CHUNK = 13, /* out: int32  snapshots per launch pair of the two-pass imaging path */
-  BLINK_Q_FUSED_PATH = 14,  /* out: int32  route of blink_grid_image: 1 = shared memory, 0 = chunked */
-  BLINK_Q_FUSED_CHUNK = 15  /* out: int32  snapshots per chunk of the chunked route */
+  BLINK_Q_FUSED_PATH = 14,  /* out: int32  route of blink_grid_image: 1 = shared memory, 0 = two kernels */
+  BLINK_Q_FUSED_CHUNK = 15  /* out: int32  snapshots per chunk of the two-kernel route */
 } blink_query;
 
 typedef struct blink_plan blink_plan; /* opaque */
@@ -143,13 +143,15 @@ int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *imag
 
 /*
  * blink_grid_image -- steps a1-a5 in one call: images straight from visibilities, with no uv grid
- * in caller memory (the paper's aim of processing "fully inside GPU
- * memory" with minimal I/O).  Result is identical, bit for bit, to
- * blink_grid followed by blink_image.  Two internal routes, chosen by the plan:
+ * in HBM at all (the paper's aim of processing "fully inside GPU
+ * memory" with minimal I/O).  Same result as blink_grid followed by blink_image
+ * up to fp32 rounding order (both meet the oracle bars).  Two internal routes, chosen by the plan:
  *   - shared-memory route (BLINK_Q_FUSED_PATH == 1; small bounding box, N <= 256): one kernel;
  *     the gridded half-plane never leaves the SM;
- *   - chunked route: blink_grid + blink_image over chunks of snapshots small enough that the uv
- *     grids of a chunk stay resident in the 126 MB L2 between the kernels, using plan-owned scratch.
+ *   - two-kernel route: the column transforms are fed straight from the visibilities through the
+ *     plan's cell-sorted tables (each occupied cell sums its own baselines in ascending order), the
+ *     row transforms follow; only the half-plane intermediate U passes through plan-owned scratch,
+ *     in chunks of BLINK_Q_FUSED_CHUNK snapshots sized to stay L2-resident.
  *   vis     DEVICE complex64 [n_t][n_ch][n_bl]
  *   images  DEVICE float32   [n_t][n_ch][N][N]
  * Asynchronous on `stream`; may grow plan-owned scratch on first use (see blink_plan_reserve).

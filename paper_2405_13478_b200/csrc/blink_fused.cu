@@ -193,13 +193,7 @@ size_t fused_smem_bytes(const blink_plan *p, int threads, int prefetch) {
 
 int fused_setup(blink_plan *p) {
   p->fused_path = 0;
-  size_t budget = 1024u << 20;   // uv scratch of a chunk of the chunked route
-  if (const char *e = getenv("BLINK_FUSED_CHUNK_MB")) {
-    long mb = atol(e);
-    if (mb > 0) budget = (size_t)mb << 20;
-  }
-  const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->n_pix;
-  p->fused_chunk = (int)std::max<size_t>(1, budget / per_snap);
+  p->fused_chunk = p->chunk_snapshots;   // the two-kernel route chunks like blink_image
   // shared-memory route: two-stage transforms (N <= 256) and everything resident in one SM.
   // Its stage capacity must equal the gridder's (the scatter tables are built for one capacity).
   int want = 1;
@@ -255,43 +249,11 @@ static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *
   }
 }
 
-int fused_reserve(blink_plan *p, int n_t) {
-  if (p->fused_path == 1) return BLINK_OK;
-  const long long n_snap = (long long)n_t * p->n_ch;
-  const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->n_pix;
-  const size_t need = per_snap * (size_t)std::min<long long>(std::max<long long>(n_snap, 1), p->fused_chunk);
-  if (need <= p->uv_scratch_bytes) return BLINK_OK;
-  if (p->d_uv_scratch) {
-    BLINK_CUDA_TRY(cudaDeviceSynchronize(), "uv scratch regrow sync");
-    cudaFree(p->d_uv_scratch);
-    p->d_uv_scratch = nullptr;
-    p->uv_scratch_bytes = 0;
-  }
-  cudaError_t e = cudaMalloc((void **)&p->d_uv_scratch, need);
-  if (e != cudaSuccess) {
-    set_cuda_error(e, "uv scratch cudaMalloc");
-    return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
-  }
-  p->uv_scratch_bytes = need;
-  return BLINK_OK;
-}
+int fused_reserve(blink_plan *p, int n_t) { return image_reserve(p, n_t); }
 
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st) {
   if (p->fused_path == 1) return launch_fused(p, vis, n_t, img, st);
-  const long long n_snap = (long long)n_t * p->n_ch;
-  const size_t grid_cells = (size_t)p->n_pix * p->n_pix;
-  const long long cap = (long long)(p->uv_scratch_bytes / (sizeof(float2) * grid_cells));
-  const long long chunk = std::min<long long>(p->fused_chunk, cap);
-  if (chunk < 1) return BLINK_ENOMEM;
-  for (long long s0 = 0; s0 < n_snap; s0 += chunk) {
-    const int ns = (int)std::min<long long>(chunk, n_snap - s0);
-    const int ch0 = (int)(s0 % p->n_ch);
-    int rc = launch_grid(p, vis + (size_t)s0 * p->n_bl, ns, ch0, p->d_uv_scratch, st);
-    if (rc != BLINK_OK) return rc;
-    rc = launch_image(p, p->d_uv_scratch, ns, ch0, img + (size_t)s0 * grid_cells, st);
-    if (rc != BLINK_OK) return rc;
-  }
-  return BLINK_OK;
+  return launch_image_from_vis(p, vis, n_t * p->n_ch, img, st);
 }
 
 }  // namespace blink
@@ -302,8 +264,7 @@ extern "C" int blink_grid_image(const blink_plan *plan, const void *vis, int n_t
   if (!vis || !images) return BLINK_EINVAL;
   if (((uintptr_t)vis & 7) || ((uintptr_t)images & 3)) return BLINK_EINVAL;
   blink_plan *mp = const_cast<blink_plan *>(plan);
-  int rc = blink::fused_reserve(mp, n_t);
-  if (rc == BLINK_OK) rc = blink::image_reserve(mp, n_t);
+  int rc = blink::image_reserve(mp, n_t);
   if (rc != BLINK_OK) return rc;
   return blink::launch_grid_image(plan, (const float2 *)vis, n_t, (float *)images, (cudaStream_t)stream);
 }

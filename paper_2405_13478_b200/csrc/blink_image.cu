@@ -36,6 +36,10 @@ struct ImgParams {
   const ChannelInfo *chinfo;
   const int32_t *wkey, *wcol;
   const float *wval;
+  // pass A straight from visibilities (blink_grid_image, two-kernel route)
+  const float2 *vis;
+  const int32_t *src, *vkey, *vseg, *vlen, *vcol;
+  const float *vw;
   const float2 *tw;
   int n_ch, n_bl, wu, uniform, snap_base, ch0;
 };
@@ -75,18 +79,39 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_image_cols(const ImgParams p)
   const int kx0 = blockIdx.x * CT;
   const float2 *__restrict__ G = p.uv + (size_t)s * N * N;
 
-  for (int i = tid; i < CT * C::LS; i += THREADS) lines[i] = mk(0.f, 0.f);
-  __syncthreads();
-  const int nrow = 2 * ci.ky_max + 1;
-  const float w0 = 0.5f * ci.inv_norm;
-  for (int e = tid; e < nrow * CT; e += THREADS) {
-    const int c = e % CT, ky = e / CT - ci.ky_max, kx = kx0 + c;
-    if (kx > ci.kx_max) continue;
-    const int iy = (ky + N) & (N - 1);
-    const float2 a = __ldcs(G + (size_t)iy * N + kx);
-    const float2 b = __ldcs(G + (size_t)((N - iy) & (N - 1)) * N + ((N - kx) & (N - 1)));
-    const float w = ((kx + ky) & 1) ? -w0 : w0;
-    lines[c * C::LS + pad16(iy)] = mk((a.x + b.x) * w, (a.y - b.y) * w);
+  // thread -> fixed column c, rows ky = -ky_max + r0 + i*RS: no div/mod or 64-bit index math in the
+  // loop, 4 rows (8 independent 8-byte loads) in flight per thread.  Rows of the bounding box are
+  // always written (zeros included), so only the rows outside it need an explicit zero fill.
+  constexpr int RS = THREADS / CT;
+  const int c = tid % CT, r0 = tid / CT, kx = kx0 + c, kym = ci.ky_max;
+  cf32 *myline = lines + c * C::LS;
+  if (kx > ci.kx_max) {
+    for (int i = r0; i < N; i += RS) myline[pad16(i)] = mk(0.f, 0.f);
+  } else {
+    for (int i = kym + 1 + r0; i < N - kym; i += RS) myline[pad16(i)] = mk(0.f, 0.f);
+    const float2 *__restrict__ Ga = G + kx;
+    const float2 *__restrict__ Gb = G + ((N - kx) & (N - 1));
+    const float w0 = 0.5f * ci.inv_norm;
+    for (int ky = -kym + r0; ky <= kym; ky += 4 * RS) {
+      float2 a[4], b[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int kyu = ky + u * RS;
+        if (kyu <= kym) {
+          const int iy = kyu & (N - 1);
+          a[u] = __ldcs(Ga + iy * N);
+          b[u] = __ldcs(Gb + ((N - iy) & (N - 1)) * N);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int kyu = ky + u * RS;
+        if (kyu <= kym) {
+          const float w = ((kx + kyu) & 1) ? -w0 : w0;
+          myline[pad16(kyu & (N - 1))] = mk((a[u].x + b[u].x) * w, (a[u].y - b[u].y) * w);
+        }
+      }
+    }
   }
   __syncthreads();
   if (p.uniform) {   // sparse 1/count on the occupied cells of these columns
@@ -103,6 +128,55 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_image_cols(const ImgParams p)
     __syncthreads();
   }
 
+  const int t = tid / CT;
+  cf32 *line = myline;
+  cf32 v[16];
+  Fft<N>::template load<0>(v, t, [&](int idx) { return line[pad16(idx)]; });
+  __syncthreads();
+  float2 *__restrict__ U = p.U + (size_t)sl * N * p.wu + kx0 + c;
+  fft_tail<N>(v, t, line, p.tw, [&](int y, cf32 x) { U[(size_t)y * p.wu] = x; });
+}
+
+// Pass A of blink_grid_image (two-kernel route): the column lines are filled straight from the
+// visibilities -- every occupied cell of these columns sums its own (short) segment of the
+// cell-sorted baseline list, in ascending baseline order, and is stored weighted, normalised and
+// sign-flipped -- so the dense uv grid is never written or read.
+template <int N, int CT>
+__global__ void __launch_bounds__(CT * (N / 16)) k_cols_from_vis(const ImgParams p) {
+  using C = ImgCfg<N>;
+  constexpr int THREADS = CT * C::T;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cf32 *lines = reinterpret_cast<cf32 *>(smem_raw);
+  const int tid = threadIdx.x;
+  const int sl = blockIdx.y, s = p.snap_base + sl, ch = (s + p.ch0) % p.n_ch;
+  const int kx0 = blockIdx.x * CT;
+  const int32_t *__restrict__ vcol = p.vcol + (size_t)ch * (p.wu + 1);
+  const int e0 = vcol[kx0], e1 = vcol[min(kx0 + CT, p.wu)];
+  for (int i = tid; i < CT * C::LS; i += THREADS) lines[i] = mk(0.f, 0.f);
+  __syncthreads();
+  {
+    const size_t tb = (size_t)ch * 2 * p.n_bl;
+    const float2 *__restrict__ vis = p.vis + (size_t)s * p.n_bl;
+    const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
+    for (int e = e0 + tid; e < e1; e += THREADS) {
+      const int key = __ldg(p.vkey + tb + e), st = __ldg(p.vseg + tb + e), lf = __ldg(p.vlen + tb + e);
+      const float w = __ldg(p.vw + tb + e);
+      const int len = lf & 0xFFFFFF, flag = lf >> 24;
+      float ar = 0.f, ai = 0.f;
+      for (int q = st; q < st + len; ++q) {
+        const int code = __ldg(src + q);
+        const float2 v = __ldg(vis + (code >> 1));
+        ar += v.x;
+        ai += (code & 1) ? -v.y : v.y;
+      }
+      cf32 o;
+      if (flag == kPlaceDirect) o = mk(ar * w, ai * w);
+      else if (flag == kPlaceConj) o = mk(ar * w, -ai * w);
+      else o = mk((ar + ar) * w, 0.f);
+      lines[((key >> 16) - kx0) * C::LS + pad16(key & 0xffff)] = o;
+    }
+  }
+  __syncthreads();
   const int c = tid % CT, t = tid / CT;
   cf32 *line = lines + c * C::LS;
   cf32 v[16];
@@ -126,16 +200,23 @@ __global__ void __launch_bounds__(RP * (N / 16)) k_image_rows(const ImgParams p)
   const float2 *__restrict__ U1 = p.U + ((size_t)sl * N + y1) * p.wu;
   cf32 *line = lines + pr * C::LS;
   cf32 v[16];
-  Fft<N>::template load<0>(v, t, [&](int idx) {
-    if (idx <= kxm) {
-      const float2 a = U0[idx], b = U1[idx];
-      return mk(a.x - b.y, a.y + b.x);             // a + i b
-    } else if (idx >= N - kxm) {
-      const float2 a = U0[N - idx], b = U1[N - idx];
-      return mk(a.x + b.y, b.x - a.y);             // conj(a) + i conj(b)
+  // stage-0 inputs Z[idx], idx = t + r*T: r < 8 is the direct half (Z = a + i b), r >= 8 the mirrored
+  // half (Z = conj a + i conj b at k = N - idx) -- static per r, so the 32 loads are branch-free and
+  // all in flight together
+  {
+    float2 a[16], b[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+      const int idx = t + r * C::T;
+      const int k = r < 8 ? idx : N - idx;
+      const bool ok = k <= kxm;
+      a[r] = ok ? __ldg(U0 + k) : make_float2(0.f, 0.f);
+      b[r] = ok ? __ldg(U1 + k) : make_float2(0.f, 0.f);
     }
-    return mk(0.f, 0.f);
-  });
+#pragma unroll
+    for (int r = 0; r < 16; ++r)
+      v[r] = r < 8 ? mk(a[r].x - b[r].y, a[r].y + b[r].x) : mk(a[r].x + b[r].y, b[r].x - a[r].y);
+  }
   float *__restrict__ r0 = p.img + ((size_t)s * N + y0) * N;
   float *__restrict__ r1 = p.img + ((size_t)s * N + y1) * N;
   fft_tail<N>(v, t, line, p.tw, [&](int x, cf32 z) { __stcs(r0 + x, z.x); __stcs(r1 + x, z.y); });
@@ -152,10 +233,12 @@ template <class K> static int prep_kernel(K kern, size_t smem) {
 template <int N, int CT, int RP>
 static int run_image_cfg(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st) {
   using C = ImgCfg<N>;
+  const bool from_vis = ip.vis != nullptr;
   const size_t smem_a = sizeof(cf32) * CT * C::LS, smem_b = sizeof(cf32) * RP * C::LS;
   static thread_local bool attr_done = false;
   if (!attr_done) {
     int rc = prep_kernel(k_image_cols<N, CT>, smem_a);
+    if (rc == BLINK_OK) rc = prep_kernel(k_cols_from_vis<N, CT>, smem_a);
     if (rc == BLINK_OK) rc = prep_kernel(k_image_rows<N, RP>, smem_b);
     if (rc != BLINK_OK) return rc;
     attr_done = true;
@@ -166,7 +249,8 @@ static int run_image_cfg(const blink_plan *p, ImgParams ip, int n_snap, cudaStre
   for (int base = 0; base < n_snap; base += chunk) {
     const int cs = std::min(chunk, n_snap - base);
     ip.snap_base = base;
-    k_image_cols<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
+    if (from_vis) k_cols_from_vis<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
+    else k_image_cols<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
     k_image_rows<N, RP><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
   }
   BLINK_CUDA_TRY(cudaGetLastError(), "k_image launch");
@@ -230,8 +314,10 @@ int image_reserve(blink_plan *p, int n_t) {
   return BLINK_OK;
 }
 
-int launch_image(const blink_plan *p, const float2 *uv, int n_snap, int ch0, float *img, cudaStream_t st) {
+static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2 *vis, int n_snap, int ch0, float *img, cudaStream_t st) {
   ImgParams ip;
+  ip.vis = vis; ip.src = p->d_src; ip.vkey = p->d_vkey; ip.vseg = p->d_vseg; ip.vlen = p->d_vlen;
+  ip.vcol = p->d_vcol; ip.vw = p->d_vw;
   ip.uv = uv; ip.img = img; ip.U = p->d_scratch; ip.chinfo = p->d_chinfo;
   ip.wkey = p->d_wkey; ip.wval = p->d_wval; ip.wcol = p->d_wcol; ip.n_bl = p->n_bl;
   ip.tw = p->d_tw; ip.n_ch = p->n_ch; ip.wu = p->wu; ip.uniform = p->weighting == BLINK_UNIFORM;
@@ -248,6 +334,14 @@ int launch_image(const blink_plan *p, const float2 *uv, int n_snap, int ch0, flo
     case 4096: return run_image_n<4096>(p, ip, n_snap, st);
     default: return BLINK_EUNSUPPORTED;
   }
+}
+
+int launch_image(const blink_plan *p, const float2 *uv, int n_snap, int ch0, float *img, cudaStream_t st) {
+  return launch_image_impl(p, uv, nullptr, n_snap, ch0, img, st);
+}
+
+int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, float *img, cudaStream_t st) {
+  return launch_image_impl(p, nullptr, vis, n_snap, 0, img, st);
 }
 
 }  // namespace blink

@@ -90,7 +90,13 @@ struct blink_plan {
   // blink_grid_image
   int fused_path = 0;               // 1 = shared-memory single kernel, 0 = chunked grid + image
   int fused_chunk = 0;              // snapshots per chunk of the chunked route
-  float2 *d_uv_scratch = nullptr;   // [fused_chunk][N][N]
+  // two-kernel route of blink_grid_image: pass A straight from the visibilities.  Occupied cells
+  // with kx >= 0, sorted by column: where they go, which segment of d_src feeds them, weight
+  int32_t *d_vkey = nullptr;        // [n_ch][2 n_bl] (kx << 16) | iy
+  int32_t *d_vseg = nullptr;        // [n_ch][2 n_bl] first entry in d_src (channel-relative)
+  int32_t *d_vlen = nullptr;        // [n_ch][2 n_bl] entries | flag << 24
+  float *d_vw = nullptr;            // [n_ch][2 n_bl] sign * (1/norm) * (1/count if uniform)
+  int32_t *d_vcol = nullptr;        // [n_ch][wu + 1] CSR by column
   // shared-memory route: occupied cells with kx >= 0 -> slot in the column lines, source, weight
   int32_t *d_hpos = nullptr;        // [n_ch][2 n_bl] kx * LS + pad16(iy)
   int32_t *d_hcode = nullptr;       // [n_ch][2 n_bl] j | flag << kPlaceShift
@@ -99,7 +105,7 @@ struct blink_plan {
   int h_max = 0;                    // max over channels of the entry count; tables padded with pos = -1
   int fused_threads = 512, fused_prefetch = 16;
   size_t fused_smem = 0;
-  size_t uv_scratch_bytes = 0;
+
 };
 
 namespace blink {
@@ -120,6 +126,7 @@ int fused_line_stride(int n_pix);
 size_t fused_smem_bytes(const blink_plan *p, int threads, int prefetch);
 int fused_reserve(blink_plan *p, int n_t);
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);
+int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, float *img, cudaStream_t st);
 
 }  // namespace blink
 

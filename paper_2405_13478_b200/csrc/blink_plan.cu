@@ -125,7 +125,7 @@ static void plan_free(blink_plan *p) {
   if (!p) return;
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
-  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_uv_scratch); cudaFree(p->d_hpos); cudaFree(p->d_hcode); cudaFree(p->d_hw); cudaFree(p->d_hcount);
+  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_hpos); cudaFree(p->d_hcode); cudaFree(p->d_hw); cudaFree(p->d_hcount); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol);
   delete p;
 }
 
@@ -422,6 +422,55 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   PLAN_CUDA(ce, "plan table upload");
   PLAN_TRY(image_setup(p));
   PLAN_TRY(fused_setup(p));
+  {
+    // pass-A-from-visibilities tables (any N): every occupied cell with kx >= 0, by column
+    std::vector<int32_t> h_vkey((size_t)n_ch * 2 * n_bl, 0), h_vseg((size_t)n_ch * 2 * n_bl, 0),
+        h_vlen((size_t)n_ch * 2 * n_bl, 0), h_vcol((size_t)n_ch * (p->wu + 1), 0);
+    std::vector<float> h_vw((size_t)n_ch * 2 * n_bl, 0.f);
+    struct VEnt { int32_t key, seg, len; float w; };
+    for (int ch = 0; ch < n_ch; ++ch) {
+      const HostGather &g = gathers[ch];
+      const float inv_norm = p->chinfo[ch].inv_norm;
+      std::vector<VEnt> ent;
+      for (int j = 0; j < g.n_can; ++j) {
+        const int c = g.can_cell[j], ix = c % N, iy = c / N;
+        const int kx = ix < N / 2 ? ix : ix - N, ky = iy;
+        const int len = g.seg_start[j + 1] - g.seg_start[j];
+        const int cnt = c == 0 ? 2 * len : len;
+        float w = ((kx + ky) & 1) ? -inv_norm : inv_norm;
+        if (weighting == BLINK_UNIFORM) w /= (float)cnt;
+        if (kx >= 0)
+          ent.push_back({(kx << 16) | iy, g.seg_start[j], len | ((c == 0 ? kPlaceBoth : kPlaceDirect) << 24), w});
+        if (kx <= 0 && c != 0)
+          ent.push_back({((-kx) << 16) | ((N - iy) % N), g.seg_start[j], len | (kPlaceConj << 24), w});
+      }
+      std::sort(ent.begin(), ent.end(), [](const VEnt &a, const VEnt &b) { return a.key < b.key; });
+      int32_t *vc = h_vcol.data() + (size_t)ch * (p->wu + 1);
+      size_t e = 0;
+      for (int kx = 0; kx < p->wu; ++kx) {
+        vc[kx] = (int32_t)e;
+        while (e < ent.size() && (ent[e].key >> 16) == kx) ++e;
+      }
+      vc[p->wu] = (int32_t)ent.size();
+      const size_t base = (size_t)ch * 2 * n_bl;
+      for (size_t k = 0; k < ent.size(); ++k) {
+        h_vkey[base + k] = ent[k].key; h_vseg[base + k] = ent[k].seg;
+        h_vlen[base + k] = ent[k].len; h_vw[base + k] = ent[k].w;
+      }
+    }
+    PLAN_TRY(dev_alloc(&p->d_vkey, h_vkey.size()));
+    PLAN_TRY(dev_alloc(&p->d_vseg, h_vseg.size()));
+    PLAN_TRY(dev_alloc(&p->d_vlen, h_vlen.size()));
+    PLAN_TRY(dev_alloc(&p->d_vw, h_vw.size()));
+    PLAN_TRY(dev_alloc(&p->d_vcol, h_vcol.size()));
+    step(cudaMemcpyAsync(p->d_vkey, h_vkey.data(), sizeof(int32_t) * h_vkey.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_vseg, h_vseg.data(), sizeof(int32_t) * h_vseg.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_vlen, h_vlen.data(), sizeof(int32_t) * h_vlen.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_vw, h_vw.data(), sizeof(float) * h_vw.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_vcol, h_vcol.data(), sizeof(int32_t) * h_vcol.size(), cudaMemcpyHostToDevice, st));
+    step(cudaStreamSynchronize(st));
+    PLAN_CUDA(ce, "vis-route table upload");
+  }
   if (p->fused_path == 1) {
     const int LS = fused_line_stride(N);
     std::vector<int32_t> h_hpos((size_t)n_ch * 2 * n_bl, -1), h_hcode((size_t)n_ch * 2 * n_bl, 0), h_hcount(n_ch, 0);
