@@ -159,16 +159,23 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
       const int o0 = pad16(y0), o1 = pad16(y1);
       cf32 v[16];
       if (act) {
-        F::template load<0>(v, t, [&](int idx) {
-          if (idx <= kxm) {
-            const float2 a = lines[idx * LS + o0], b = lines[idx * LS + o1];
-            return mk(a.x - b.y, a.y + b.x);             // a + i b
-          } else if (idx >= N - kxm) {
-            const float2 a = lines[(N - idx) * LS + o0], b = lines[(N - idx) * LS + o1];
-            return mk(a.x + b.y, b.x - a.y);             // conj(a) + i conj(b)
+        // stage-0 inputs Z[idx], idx = t + r*T: r < 8 direct half (a + i b), r >= 8 mirrored half
+        // (conj a + i conj b at k = N - idx) -- static per r, branch-free, all loads in flight
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          float2 a[8], b[8];
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const int idx = t + (8 * h + q) * T;
+            const int k = h == 0 ? idx : N - idx;
+            const bool ok = k <= kxm;
+            a[q] = ok ? lines[k * LS + o0] : make_float2(0.f, 0.f);
+            b[q] = ok ? lines[k * LS + o1] : make_float2(0.f, 0.f);
           }
-          return mk(0.f, 0.f);
-        });
+#pragma unroll
+          for (int q = 0; q < 8; ++q)
+            v[8 * h + q] = h == 0 ? mk(a[q].x - b[q].y, a[q].y + b[q].x) : mk(a[q].x + b[q].y, b[q].x - a[q].y);
+        }
         F::template compute<0>(v, t, p.tw);
       }
       __syncwarp();                                   // previous round's reads of xl are done
