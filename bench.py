@@ -259,10 +259,16 @@ def main():
     # ---- end to end: pinned host visibilities in, images back to pinned host memory, per step
     e2e = None
     if not args.no_e2e:
+        from paper_2405_13478_b200.pipeline import HostPipeline
+        pipe = HostPipeline(plan, w.n_t) if fused else None
+
         def e2e_step():
-            vis.copy_(vis_h, non_blocking=True)
-            step()
-            img_h.copy_(img, non_blocking=True)
+            if pipe is not None:                      # chunked, transfers overlapped with imaging
+                pipe.run(vis_h, img_h)
+            else:
+                vis.copy_(vis_h, non_blocking=True)
+                step()
+                img_h.copy_(img, non_blocking=True)
         e2e_step()
         barrier()
         n_e = max(1, min(args.steps, 3))

@@ -269,3 +269,19 @@ def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name
     if name == "mwa1":
         assert plan.query_i32(blink.Q_FUSED_PATH) == 0
     plan.close()
+
+
+def test_host_pipeline_matches_device_path(torch_cuda, blink):
+    """The host-to-host streaming wrapper (chunked, overlapped transfers) returns exactly what
+    blink_grid_image returns on resident data, including a ragged last chunk."""
+    torch = torch_cuda
+    from paper_2405_13478_b200.pipeline import HostPipeline
+    w = synth.config_station(n_t=7, n_ch=4, n_pix=128)
+    vis_h = torch.from_numpy(w.vis()).pin_memory()
+    plan = _plan(blink, w)
+    ref = plan.grid_image(vis_h.cuda())
+    img_h = torch.full(tuple(ref.shape), float("nan"), dtype=torch.float32).pin_memory()
+    HostPipeline(plan, w.n_t, chunk_t=3, depth=2).run(vis_h, img_h)
+    torch.cuda.synchronize()
+    assert torch.equal(img_h, ref.cpu())
+    plan.close()
