@@ -103,8 +103,15 @@ struct blink_plan {
   float *d_hw = nullptr;            // [n_ch][2 n_bl] sign * (1/norm) * (1/count if uniform)
   int32_t *d_hcount = nullptr;      // [n_ch]
   int h_max = 0;                    // max over channels of the entry count; tables padded with pos = -1
-  int fused_threads = 512, fused_prefetch = 16;
+  int fused_threads = 512;
   size_t fused_smem = 0;
+  // shared-memory route, phase S: bulk-copied chunks of `fused_chunk_vis` baselines and the
+  // rank-major gather tables built for that chunk size (see RankTables in blink_plan.cu)
+  int fused_chunk_vis = 0, fused_n_chunk = 0, fused_nbuf = 0, frow_stride = 0;
+  uint32_t fused_off_dedicated = 0, fused_off_S = 0, fused_off_bar = 0;
+  uint2 *d_frec = nullptr;          // [n_ch][n_chunk][n_can_max] {j | len << 16, ranks 0,1}
+  uint32_t *d_fpair = nullptr;      // [n_ch][n_chunk][chunk_vis] rows q >= 1: ranks 2q, 2q+1
+  int2 *d_frow = nullptr;           // [n_ch][n_chunk][frow_stride] {offset into fpair, cells in row}
 
 };
 
@@ -123,7 +130,6 @@ int image_setup(blink_plan *p);
 int image_reserve(blink_plan *p, int n_t);
 int fused_setup(blink_plan *p);
 int fused_line_stride(int n_pix);
-size_t fused_smem_bytes(const blink_plan *p, int threads, int prefetch);
 int fused_reserve(blink_plan *p, int n_t);
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);
 int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, float *img, cudaStream_t st);

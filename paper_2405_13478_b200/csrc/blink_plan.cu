@@ -110,6 +110,80 @@ int build_gather_host(const int32_t *cell, int n_bl, int n_pix, HostGather &out)
   return BLINK_OK;
 }
 
+// Rank-major tables of the per-cell sums (blink_grid, blink_grid_image).  Pass q takes baselines
+// [q cap, (q+1) cap).  Within a pass the cells that receive something are ordered by descending
+// number of baselines (position k); the r-th baseline (ascending index) of the cell at position k
+// has rank-major slot roff[r] + k.  Thread k then walks slots roff[r] + k, r = 0..len-1:
+// consecutive threads touch consecutive slots, the lanes of a warp see near-equal trip counts,
+// and the summation order is the oracle's (ascending baseline).
+//   scat[bl]        slot | conj << 15 (0xFFFF = dropped)              -- scatter form (k_grid)
+//   list[slot]      (bl - q cap) | conj << 15                          -- gather form (k_fused)
+//   cellrec[k]      j | len << 16 (j = index of the canonical cell sum)
+struct RankTables {
+  int cap = 0, n_pass = 0, roff_stride = 0;
+  std::vector<uint16_t> scat, list, roff;
+  std::vector<uint32_t> cellrec;
+  std::vector<int32_t> nact;
+};
+
+static void build_rank_tables(const std::vector<HostGather> &gathers, int n_ch, int n_bl, int ncm,
+                              int cap, RankTables &t) {
+  t.cap = cap;
+  t.n_pass = std::max(1, (n_bl + cap - 1) / cap);
+  const int n_pass = t.n_pass;
+  t.scat.assign((size_t)n_ch * n_bl, kScatDropped);
+  t.list.assign((size_t)n_ch * n_pass * cap, 0);
+  t.cellrec.assign((size_t)n_ch * n_pass * ncm, 0);
+  t.nact.assign((size_t)n_ch * n_pass, 0);
+  std::vector<std::vector<uint16_t>> roffs((size_t)n_ch * n_pass);
+  int maxlen = 0;
+  for (int ch = 0; ch < n_ch; ++ch) {
+    const HostGather &g = gathers[ch];
+    uint16_t *sc = t.scat.data() + (size_t)ch * n_bl;
+    for (int q = 0; q < n_pass; ++q) {
+      const int lo = q * cap, hi = std::min(n_bl, lo + cap);
+      // per cell: entries of this pass are a contiguous sub-range of its (baseline-sorted) segment
+      std::vector<std::array<int32_t, 3>> cells;   // {len, j, first entry}
+      for (int j = 0; j < g.n_can; ++j) {
+        int e0 = g.seg_start[j], e1 = g.seg_start[j + 1];
+        while (e0 < e1 && (g.src[e0] >> 1) < lo) ++e0;
+        int e2 = e0;
+        while (e2 < e1 && (g.src[e2] >> 1) < hi) ++e2;
+        if (e2 > e0) cells.push_back({e2 - e0, j, e0});
+      }
+      std::stable_sort(cells.begin(), cells.end(),
+                       [](const std::array<int32_t, 3> &a, const std::array<int32_t, 3> &b) { return a[0] > b[0]; });
+      const int n_act = (int)cells.size();
+      t.nact[(size_t)ch * n_pass + q] = n_act;
+      const int ml = n_act ? cells[0][0] : 0;
+      maxlen = std::max(maxlen, ml);
+      std::vector<uint16_t> &ro = roffs[(size_t)ch * n_pass + q];
+      ro.assign(ml + 1, 0);
+      int off = 0, nr = n_act;
+      for (int r = 0; r < ml; ++r) {
+        while (nr > 0 && cells[nr - 1][0] <= r) --nr;   // cells with len > r form a prefix
+        ro[r] = (uint16_t)off;
+        off += nr;
+      }
+      ro[ml] = (uint16_t)off;
+      uint32_t *cr = t.cellrec.data() + ((size_t)ch * n_pass + q) * ncm;
+      uint16_t *ls = t.list.data() + ((size_t)ch * n_pass + q) * cap;
+      for (int k = 0; k < n_act; ++k) {
+        cr[k] = (uint32_t)cells[k][1] | ((uint32_t)cells[k][0] << 16);
+        for (int r = 0; r < cells[k][0]; ++r) {
+          const int code = g.src[cells[k][2] + r];
+          sc[code >> 1] = (uint16_t)((ro[r] + k) | ((code & 1) << 15));
+          ls[ro[r] + k] = (uint16_t)(((code >> 1) - lo) | ((code & 1) << 15));
+        }
+      }
+    }
+  }
+  t.roff_stride = ((maxlen + 1 + 3) / 4) * 4;   // rows stay 8-byte aligned for ushort4 reads
+  t.roff.assign((size_t)n_ch * n_pass * t.roff_stride, 0);
+  for (size_t i = 0; i < roffs.size(); ++i)
+    std::copy(roffs[i].begin(), roffs[i].end(), t.roff.begin() + i * t.roff_stride);
+}
+
 template <class T> static int dev_alloc(T **p, size_t n) {
   if (n == 0) n = 1;
   cudaError_t e = cudaMalloc((void **)p, n * sizeof(T));
@@ -126,6 +200,7 @@ static void plan_free(blink_plan *p) {
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
   cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_hpos); cudaFree(p->d_hcode); cudaFree(p->d_hw); cudaFree(p->d_hcount); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol);
+  cudaFree(p->d_frec); cudaFree(p->d_fpair); cudaFree(p->d_frow);
   delete p;
 }
 
@@ -310,11 +385,6 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   if (p->n_can_max > kPlaceMask) { plan_free(p); return BLINK_EUNSUPPORTED; }
 
   // ---- gridder tables: rank-major stage slots, cells by descending per-pass length ------------
-  // Pass q stages baselines [q C, (q+1) C).  Within a pass the cells that receive something are
-  // ordered by descending number of baselines (position k); the r-th baseline (ascending index)
-  // of the cell at position k sits at stage[roff[r] + k].  Thread k then adds stage[roff[r] + k],
-  // r = 0..len-1: consecutive threads read consecutive slots (no bank conflicts), warps see
-  // near-uniform trip counts, and the summation order is the oracle's (ascending baseline).
   {
     int nbuf = 3;
     if (const char *e = getenv("BLINK_GRID_NBUF")) nbuf = atoi(e);
@@ -337,57 +407,15 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
                                      (size_t)p->stage_cap) + 64;
     if (p->max_smem_optin > 0 && p->grid_smem > (size_t)p->max_smem_optin) { plan_free(p); return BLINK_EUNSUPPORTED; }
   }
-  const int kStageCap = p->stage_cap;
+  if (p->n_can_max > 0xFFFF || p->stage_cap > 0x7FFF) { plan_free(p); return BLINK_EUNSUPPORTED; }
   const int n_pass = p->n_pass, ncm = std::max(p->n_can_max, 1);
-  std::vector<uint16_t> h_scat((size_t)n_ch * n_bl, kScatDropped);
-  std::vector<uint32_t> h_cellrec((size_t)n_ch * n_pass * ncm, 0);
-  std::vector<int32_t> h_nact((size_t)n_ch * n_pass, 0);
-  std::vector<std::vector<uint16_t>> roffs((size_t)n_ch * n_pass);
-  int maxlen = 0;
-  for (int ch = 0; ch < n_ch; ++ch) {
-    const HostGather &g = gathers[ch];
-    uint16_t *sc = h_scat.data() + (size_t)ch * n_bl;
-    for (int q = 0; q < n_pass; ++q) {
-      const int lo = q * kStageCap, hi = std::min(n_bl, lo + kStageCap);
-      // per cell: entries of this pass are a contiguous sub-range of its (baseline-sorted) segment
-      std::vector<std::array<int32_t, 3>> cells;   // {len, j, first entry}
-      for (int j = 0; j < g.n_can; ++j) {
-        int e0 = g.seg_start[j], e1 = g.seg_start[j + 1];
-        while (e0 < e1 && (g.src[e0] >> 1) < lo) ++e0;
-        int e2 = e0;
-        while (e2 < e1 && (g.src[e2] >> 1) < hi) ++e2;
-        if (e2 > e0) cells.push_back({e2 - e0, j, e0});
-      }
-      std::stable_sort(cells.begin(), cells.end(),
-                       [](const std::array<int32_t, 3> &a, const std::array<int32_t, 3> &b) { return a[0] > b[0]; });
-      const int n_act = (int)cells.size();
-      h_nact[(size_t)ch * n_pass + q] = n_act;
-      const int ml = n_act ? cells[0][0] : 0;
-      maxlen = std::max(maxlen, ml);
-      std::vector<uint16_t> &ro = roffs[(size_t)ch * n_pass + q];
-      ro.assign(ml + 1, 0);
-      int off = 0, nr = n_act;
-      for (int r = 0; r < ml; ++r) {
-        while (nr > 0 && cells[nr - 1][0] <= r) --nr;   // cells with len > r form a prefix
-        ro[r] = (uint16_t)off;
-        off += nr;
-      }
-      ro[ml] = (uint16_t)off;
-      uint32_t *cr = h_cellrec.data() + ((size_t)ch * n_pass + q) * ncm;
-      for (int k = 0; k < n_act; ++k) {
-        cr[k] = (uint32_t)cells[k][1] | ((uint32_t)cells[k][0] << 16);
-        for (int r = 0; r < cells[k][0]; ++r) {
-          const int code = g.src[cells[k][2] + r];
-          sc[code >> 1] = (uint16_t)((ro[r] + k) | ((code & 1) << 15));
-        }
-      }
-    }
-  }
-  if (p->n_can_max > 0xFFFF || kStageCap > 0x7FFF) { plan_free(p); return BLINK_EUNSUPPORTED; }
-  p->roff_stride = ((maxlen + 1 + 3) / 4) * 4;   // rows stay 8-byte aligned for ushort4 reads
-  std::vector<uint16_t> h_roff((size_t)n_ch * n_pass * p->roff_stride, 0);
-  for (size_t i = 0; i < roffs.size(); ++i)
-    std::copy(roffs[i].begin(), roffs[i].end(), h_roff.begin() + i * p->roff_stride);
+  RankTables rt;
+  build_rank_tables(gathers, n_ch, n_bl, ncm, p->stage_cap, rt);
+  p->roff_stride = rt.roff_stride;
+  std::vector<uint16_t> &h_scat = rt.scat, &h_roff = rt.roff;
+  std::vector<uint32_t> &h_cellrec = rt.cellrec;
+  std::vector<int32_t> &h_nact = rt.nact;
+  (void)n_pass;
 
   // twiddles exp(+2 pi i k / N), fp64 -> fp32
   std::vector<float2> h_tw(N);
@@ -472,6 +500,45 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     PLAN_CUDA(ce, "vis-route table upload");
   }
   if (p->fused_path == 1) {
+    // phase-S gather tables for chunks of fused_chunk_vis baselines: per (channel, chunk) the cells
+    // by descending length with ranks 0,1 packed beside the record, and rows q >= 1 holding ranks
+    // 2q, 2q+1 of the cells with more than 2q entries (0xFFFF = no second entry)
+    RankTables ft;
+    build_rank_tables(gathers, n_ch, n_bl, ncm, p->fused_chunk_vis, ft);
+    const int C = p->fused_chunk_vis, n_chunk = ft.n_pass;
+    if (n_chunk != p->fused_n_chunk) { plan_free(p); return BLINK_EUNSUPPORTED; }
+    int maxlen = 0;
+    for (size_t i = 0; i < ft.cellrec.size(); ++i) maxlen = std::max(maxlen, (int)(ft.cellrec[i] >> 16));
+    p->frow_stride = std::max(2, (maxlen + 1) / 2 + 1);
+    std::vector<uint2> h_frec((size_t)n_ch * n_chunk * ncm, make_uint2(0u, 0u));
+    std::vector<uint32_t> h_fpair((size_t)n_ch * n_chunk * C, 0u);
+    std::vector<int2> h_frow((size_t)n_ch * n_chunk * p->frow_stride, make_int2(0, 0));
+    for (size_t cp = 0; cp < (size_t)n_ch * n_chunk; ++cp) {
+      const uint32_t *cr = ft.cellrec.data() + cp * ncm;
+      const uint16_t *ls = ft.list.data() + cp * C;
+      const uint16_t *ro = ft.roff.data() + cp * ft.roff_stride;
+      const int n_act = ft.nact[cp];
+      auto entry = [&](int k, int r) -> uint32_t {
+        return r < (int)(cr[k] >> 16) ? (uint32_t)ls[ro[r] + k] : 0xFFFFu;
+      };
+      for (int k = 0; k < n_act; ++k) h_frec[cp * ncm + k] = make_uint2(cr[k], entry(k, 0) | (entry(k, 1) << 16));
+      int off = 0;
+      for (int q = 1; q < p->frow_stride; ++q) {
+        int cnt = 0;
+        while (cnt < n_act && (int)(cr[cnt] >> 16) > 2 * q) ++cnt;     // lengths descend
+        h_frow[cp * p->frow_stride + q] = make_int2(off, cnt);
+        for (int k = 0; k < cnt; ++k) h_fpair[cp * C + off + k] = entry(k, 2 * q) | (entry(k, 2 * q + 1) << 16);
+        off += cnt;
+      }
+    }
+    PLAN_TRY(dev_alloc(&p->d_frec, h_frec.size()));
+    PLAN_TRY(dev_alloc(&p->d_fpair, h_fpair.size()));
+    PLAN_TRY(dev_alloc(&p->d_frow, h_frow.size()));
+    step(cudaMemcpyAsync(p->d_frec, h_frec.data(), sizeof(uint2) * h_frec.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_fpair, h_fpair.data(), sizeof(uint32_t) * h_fpair.size(), cudaMemcpyHostToDevice, st));
+    step(cudaMemcpyAsync(p->d_frow, h_frow.data(), sizeof(int2) * h_frow.size(), cudaMemcpyHostToDevice, st));
+    step(cudaStreamSynchronize(st));
+    PLAN_CUDA(ce, "fused gather table upload");
     const int LS = fused_line_stride(N);
     std::vector<int32_t> h_hpos((size_t)n_ch * 2 * n_bl, -1), h_hcode((size_t)n_ch * 2 * n_bl, 0), h_hcount(n_ch, 0);
     std::vector<float> h_hw((size_t)n_ch * 2 * n_bl, 0.f);

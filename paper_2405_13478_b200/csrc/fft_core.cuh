@@ -155,6 +155,29 @@ template <int N> struct Fft {
     }
   }
 
+  // The twiddles of butterfly j of stage S, w[r] = w_{Ns R}^{r k}, k = j mod Ns, each read straight
+  // from the table (no product tree): for callers that keep them in registers across transforms.
+  template <int S> BLINK_HD static void twiddles(cf32 *w, int j, const cf32 *tw) {
+    constexpr int R = radix<S>();
+    constexpr int Ns = ns<S>();
+    const int k = j & (Ns - 1);
+    w[0] = mk(1.f, 0.f);
+#pragma unroll
+    for (int r = 1; r < R; ++r) w[r] = tw[(r * k * (N / (Ns * R))) & (N - 1)];
+  }
+
+  // Phase 2 with caller-held twiddles: w[b][r] from twiddles<S>(w[b], t + b*T, tw).
+  template <int S, int WR> BLINK_HD static void compute_tw(cf32 *v, const cf32 (*w)[WR]) {
+    constexpr int R = radix<S>();
+#pragma unroll
+    for (int b = 0; b < E / R; ++b) {
+      cf32 *x = v + b * R;
+#pragma unroll
+      for (int r = 1; r < R; ++r) x[r] = cmul(x[r], w[b][r]);
+      dft<R>(x);
+    }
+  }
+
   // Phase 3 of stage S: out[(j/Ns) Ns R + k + r Ns] = v[b*R + r].  `st(idx, val)`.
   template <int S, class Store> BLINK_HD static void store(const cf32 *v, int t, Store st) {
     constexpr int R = radix<S>();
