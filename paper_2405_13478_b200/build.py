@@ -17,7 +17,8 @@ LIB = os.path.join(HERE, "libblink.so")
 SOURCES = ["blink_plan.cu", "blink_grid.cu", "blink_image.cu", "blink_fused.cu"]
 HEADERS = ["blink_internal.h", "fft_core.cuh", "sphase.cuh", os.path.join("..", "..", "include", "blink.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "--expt-extended-lambda", "--expt-relaxed-constexpr"]
+              "-Xcompiler", "-fPIC", "--expt-extended-lambda", "--expt-relaxed-constexpr"]
+OBJ_DIR = os.path.join(HERE, "build")
 
 
 def _stale() -> bool:
@@ -32,13 +33,27 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not (force or _stale()):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-          [os.path.join(CSRC, f) for f in SOURCES] + ["-o", LIB]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    extra = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(src):          # one translation unit -> object file (the units compile in parallel)
+        obj = os.path.join(OBJ_DIR, src.replace(".cu", ".o"))
+        cmd = [nvcc] + NVCC_FLAGS + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
+        return obj, subprocess.run(cmd, capture_output=True, text=True)
+
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+        results = list(ex.map(compile_one, SOURCES))
+    for _, res in results:
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+    if any(res.returncode != 0 for _, res in results):
         raise RuntimeError("nvcc failed building libblink.so")
+    link = subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] +
+                          [obj for obj, _ in results] + ["-o", LIB], capture_output=True, text=True)
+    if link.returncode != 0:
+        sys.stderr.write(link.stdout + link.stderr)
+        raise RuntimeError("nvcc failed linking libblink.so")
     return LIB
 
 

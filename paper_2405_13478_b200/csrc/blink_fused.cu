@@ -5,6 +5,9 @@
 // read back while still resident in the 126 MB L2 and (ideally) never reach HBM: the DRAM traffic
 // of a snapshot falls from 8 n_bl + 20 N^2 towards 8 n_bl + 4 N^2 bytes.
 #include <algorithm>
+#include <array>
+#include <cstdio>
+#include <cstring>
 
 #include "blink_internal.h"
 #include "fft_core.cuh"
@@ -18,38 +21,43 @@ using namespace blinkfft;
 // grid ever leaving the SM:
 //   phase S   the snapshot's visibilities arrive in shared memory in INPUT order, in chunks of
 //             `chunk_vis` baselines, by bulk asynchronous copies (cp.async.bulk global -> shared,
-//             completion on an mbarrier; no thread instructions, no registers).  For every chunk
-//             one thread per canonical (half-plane) cell walks the plan's rank-major gather list
-//             -- (local baseline | conj << 15), two ranks per 32-bit word -- and adds its
-//             visibilities in ascending baseline order into S[j].  No atomics, no scatter.
-//             Chunk buffers: one dedicated (so the first chunk of the NEXT snapshot streams in
-//             during passes A and B) plus as many as fit in the space of the column lines and the
-//             pass-B exchange lines, which are idle during phase S.
-//   phase H   the occupied cells with kx >= 0 are written, already weighted, normalised and
-//             sign-flipped for the fftshift, into per-column lines in shared memory (the grid is
-//             exactly Hermitian by construction, so the half-plane is all that is needed);
+//             completion on an mbarrier; no thread instructions, no registers), each chunk together
+//             with the plan's gather table for that (channel, chunk), so every table access in the
+//             inner loop is a shared-memory read.  Every canonical (half-plane) cell is OWNED by one
+//             warp for the whole kernel, so the sums need no atomics and no barriers between warps:
+//             per chunk a warp walks its cells in groups of 32 (one cell per lane, grouped by
+//             descending number of baselines in the chunk, rows padded with a pointer to a zero slot)
+//             and adds each group's sums into S[j].  Chunk buffers form a ring with full/empty
+//             mbarriers: buffer 0 is dedicated (so the first chunk of the NEXT snapshot streams in
+//             during phase H and passes A and B), the others alias the column lines and the pass-B
+//             exchange lines, which are idle during phase S.  Thread 0 is the producer.
+//   phase H   every cell of the bounding box with kx >= 0 is written -- weighted, normalised and
+//             sign-flipped for the fftshift, zero where no baseline lands -- into per-column lines in
+//             shared memory (the grid is exactly Hermitian by construction, so the half-plane is all
+//             that is needed);
 //   pass A    column transforms along ky, in place in the lines, loads pruned to the bounding box;
 //   pass B    row transforms, two real image rows per complex transform, read from the lines across
 //             columns and stored to global memory straight from the last butterfly stage.
 // A transform is owned by T = N/16 <= 16 lanes of one warp, so the exchanges inside it need only
 // __syncwarp.  The last-stage twiddles depend only on the lane, so they live in registers for the
 // whole kernel.
+constexpr int kFusedThreads = 512;
+constexpr int kFusedWarps = kFusedThreads / 32;
+constexpr int kFusedMaxGroups = 255;  // groups of one length per (warp, chunk)
+constexpr int kFusedLcap = 4;         // rows per group: longer per-chunk cell lists are split into pieces
+constexpr int kHPer = 7;              // phase-H records fetched per thread ahead of the barrier
+
 struct FusedParams {
   const float2 *vis;
   float *img;
   const ChannelInfo *chinfo;
-  const uint2 *frec;        // [n_ch][n_chunk][n_can_max]  {j | len << 16, ranks 0,1 of the gather list}
-  const uint32_t *fpair;    // [n_ch][n_chunk][chunk_vis]  rows q >= 1: ranks 2q, 2q+1
-  const int2 *frow;         // [n_ch][n_chunk][frow_stride] row q: {offset into fpair, cells with len > 2q}
-  const int32_t *hpos, *hcode;
-  const float *hw;
+  const unsigned char *gtab;  // [n_ch][n_chunk][tab_stride] phase-S gather tables (see fused_build)
+  const uint32_t *gsize;      // [n_ch][n_chunk] bytes of each table (multiple of 16)
+  const uint2 *hrec;          // [n_ch][h_max] {pos | j << 16 | flag << 30, weight}; pos 0xFFFF = padding
   const float2 *tw;
-  int n_bl, n_ch, n_snap, n_can_max, n_chunk, chunk_vis, nbuf, frow_stride, n_col, h_max;
-  uint32_t off_dedicated, off_S, off_bar;   // byte offsets into dynamic shared memory
+  int n_bl, n_ch, n_snap, n_can_max, n_chunk, chunk_vis, nbuf, tab_stride, n_col, h_max;
+  uint32_t buf_bytes, off_dedicated, off_S, off_bar;   // byte offsets into dynamic shared memory
 };
-
-constexpr int kHPer = 5;       // phase-H table entries fetched per thread at a time
-constexpr int kCellsPf = 5;    // cells per thread whose records are prefetched ahead of the data
 
 int fused_line_stride(int n_pix) { return ((n_pix + n_pix / 16 + 15) / 16) * 16 + 1; }
 
@@ -58,6 +66,9 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   uint32_t done;
@@ -77,11 +88,39 @@ __device__ __forceinline__ void bulk_load(void *sdst, const void *gsrc, uint32_t
                ::"r"(smem_u32(sdst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-// one gather-list entry: add (conj-flagged) visibility e of the chunk to the accumulator
-__device__ __forceinline__ void add_entry(const float2 *__restrict__ buf, uint32_t e, float &ax, float &ay) {
-  const float2 v = buf[e & 0x7FFFu];
-  ax += v.x;
-  ay += __uint_as_float(__float_as_uint(v.y) ^ ((e & 0x8000u) << 16));
+__device__ __forceinline__ uint2 lds_u2(uint32_t addr) {
+  uint2 r;
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(addr));
+  return r;
+}
+
+// One group of phase S: lane l adds its (at most L) visibilities and folds the sum into its cell.
+// blk = shared address of the lane's column of the group block: row 0 the slot of the cell sum,
+// rows 1..L the entries, read sign-extended so that conj (bit 15) lands in the sign bit.
+template <int L> __device__ __forceinline__ void gather_group(uint32_t blk, uint32_t sm_base, uint32_t S_base) {
+  uint32_t j;
+  int e[L];
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(j) : "r"(blk));
+#pragma unroll
+  for (int r = 0; r < L; ++r) asm volatile("ld.shared.s16 %0, [%1];" : "=r"(e[r]) : "r"(blk + 64u * (r + 1)));
+  float2 v[L];
+#pragma unroll
+  for (int r = 0; r < L; ++r) {
+    const uint32_t addr = sm_base + ((uint32_t)(e[r] & 0x7FFF) << 3);
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v[r].x), "=f"(v[r].y) : "r"(addr));
+  }
+  float ax = v[0].x, ay = __uint_as_float(__float_as_uint(v[0].y) ^ ((uint32_t)e[0] & 0x80000000u));
+#pragma unroll
+  for (int r = 1; r < L; ++r) {
+    ax += v[r].x;
+    ay += __uint_as_float(__float_as_uint(v[r].y) ^ ((uint32_t)e[r] & 0x80000000u));
+  }
+  const uint32_t sa = S_base + (j << 3);
+  float2 a;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(a.x), "=f"(a.y) : "r"(sa));
+  a.x += ax;
+  a.y += ay;
+  asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(sa), "f"(a.x), "f"(a.y) : "memory");
 }
 
 template <int N, int THREADS>
@@ -92,31 +131,50 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   constexpr int LSB = LineSize<N>::value;
   using F = Fft<N>;
   static_assert(F::NSTAGE == 2 && T <= 32, "shared-memory route needs a two-stage warp-local transform");
+  static_assert(THREADS == kFusedThreads, "the gather tables are built for kFusedWarps warps");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float2 *lines = reinterpret_cast<float2 *>(smem_raw);                       // [n_col][LS]
   float2 *X = lines + (size_t)p.n_col * LS;                                   // exchange lines [G][LSB]
-  float2 *S = reinterpret_cast<float2 *>(smem_raw + p.off_S);                 // [n_can_max]
-  uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + p.off_bar);         // [nbuf]
+  float2 *S = reinterpret_cast<float2 *>(smem_raw + p.off_S);                 // [n_can_max up to 16 | 16 sinks]
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + p.off_bar);        // [nbuf]
+  uint64_t *empty = full + p.nbuf;                                            // [nbuf]
+  const uint32_t sm_base = smem_u32(smem_raw), S_base = sm_base + p.off_S;
   const int tid = threadIdx.x;
+  const int warp = tid >> 5, lane = tid & 31;
   const int grp = tid / T, t = tid % T;
-  const uint32_t chunk_bytes = (uint32_t)p.chunk_vis * sizeof(float2);
+  const uint32_t vis_bytes = (uint32_t)p.chunk_vis * sizeof(float2);
   // chunk c of every snapshot lives in buffer c % nbuf; buffer 0 is the dedicated one, the others
   // alias the lines / exchange area
-  auto buf_of = [&](int b) -> float2 * {
-    return reinterpret_cast<float2 *>(b == 0 ? smem_raw + p.off_dedicated : smem_raw + (size_t)(b - 1) * chunk_bytes);
+  auto buf_of = [&](int b) -> unsigned char * {
+    return b == 0 ? smem_raw + p.off_dedicated : smem_raw + (size_t)(b - 1) * p.buf_bytes;
   };
-  auto issue = [&](int s, int c) {      // one thread
+  uint32_t fphase = 0;                  // bit b: parity of the next wait on full[b]
+  uint32_t ephase = 0;                  // producer only: bit b: parity of the last completed empty[b] phase
+  auto produce = [&](int s, int c) {    // thread 0 only
     const int b = c % p.nbuf;
+    mbar_wait(empty + b, ((ephase >> b) & 1u) ^ 1u);   // every warp has let go of the buffer
+    ephase ^= 1u << b;
     const int cnt = min(p.chunk_vis, p.n_bl - c * p.chunk_vis);
-    const uint32_t bytes = (uint32_t)cnt * sizeof(float2);
-    mbar_expect_tx(bar + b, bytes);
-    bulk_load(buf_of(b), p.vis + (size_t)s * p.n_bl + (size_t)c * p.chunk_vis, bytes, bar + b);
+    const uint32_t vb = (uint32_t)cnt * sizeof(float2);
+    const size_t cp = (size_t)(s % p.n_ch) * p.n_chunk + c;
+    const uint32_t tb = __ldg(p.gsize + cp);
+    unsigned char *dst = buf_of(b);
+    mbar_expect_tx(full + b, vb + tb);
+    bulk_load(dst, p.vis + (size_t)s * p.n_bl + (size_t)c * p.chunk_vis, vb, full + b);
+    bulk_load(dst + vis_bytes, p.gtab + cp * p.tab_stride, tb, full + b);
   };
 
   if (tid == 0) {
-    for (int b = 0; b < p.nbuf; ++b) mbar_init(bar + b, 1);
+    for (int b = 0; b < p.nbuf; ++b) {
+      mbar_init(full + b, 1);
+      mbar_init(empty + b, kFusedWarps);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // S[0..n_can_max-1] cell sums; S[sink0 + b], b = 0..15: one always-zero slot per bank (sinks of
+  // padded lanes and the "zero visibility" padded entries point at)
+  const int n_S = ((p.n_can_max + 15) & ~15) + 16;
+  for (int j = tid; j < n_S; j += THREADS) S[j] = make_float2(0.f, 0.f);
   // last-stage twiddles w^(r k), k fixed per lane: registers for the whole kernel
   constexpr int R1 = F::template radix<1>();
   constexpr int NB1 = 16 / R1;
@@ -124,101 +182,67 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
 #pragma unroll
   for (int b = 0; b < NB1; ++b) F::template twiddles<1>(tw1[b], t + b * T, p.tw);
   __syncthreads();
-  if (tid == 0 && blockIdx.x < p.n_snap) issue(blockIdx.x, 0);
+  if (tid == 0 && blockIdx.x < p.n_snap) produce(blockIdx.x, 0);
   const int c_last0 = ((p.n_chunk - 1) / p.nbuf) * p.nbuf;   // last chunk of a snapshot in buffer 0
-  uint32_t phase = 0;                                        // bit b: parity of the next wait on buffer b
 
   for (int s = blockIdx.x; s < p.n_snap; s += gridDim.x) {
     const int ch = s % p.n_ch;
     const ChannelInfo ci = p.chinfo[ch];
     // the lines / exchange area is idle until phase H: fill it with this snapshot's next chunks
     if (tid == 0)
-      for (int c = 1; c < min(p.n_chunk, p.nbuf); ++c) issue(s, c);
+      for (int c = 1; c < min(p.n_chunk, p.nbuf); ++c) produce(s, c);
 
     // ---- phase S ----------------------------------------------------------------------------
-    for (int j = tid; j < p.n_can_max; j += THREADS) S[j] = make_float2(0.f, 0.f);
-    __syncthreads();
     for (int c = 0; c < p.n_chunk; ++c) {
       const int b = c % p.nbuf;
-      const size_t cp = (size_t)ch * p.n_chunk + c;
-      const uint2 *__restrict__ frec = p.frec + cp * max(p.n_can_max, 1);
-      const uint32_t *__restrict__ fpair = p.fpair + cp * p.chunk_vis;
-      const int2 *__restrict__ frow = p.frow + cp * p.frow_stride;
-      // table records first: they do not depend on the data, so their latency hides behind the wait
-      uint2 rec[kCellsPf];
-      uint32_t pr1[kCellsPf];
-      const int2 row1 = __ldg(frow + 1);
-#pragma unroll
-      for (int q = 0; q < kCellsPf; ++q) {
-        const int k = tid + q * THREADS;
-        rec[q] = k < p.n_can_max ? __ldg(frec + k) : make_uint2(0u, 0u);
-        pr1[q] = k < row1.y ? __ldg(fpair + row1.x + k) : 0u;
-      }
-      mbar_wait(bar + b, (phase >> b) & 1u);
-      phase ^= 1u << b;
-      const float2 *__restrict__ buf = buf_of(b);
-      auto sum_cell = [&](uint2 rc, uint32_t p1, int k) {
-        const int len = rc.x >> 16;
-        if (len == 0) return;
-        float ax = 0.f, ay = 0.f;
-        add_entry(buf, rc.y & 0xFFFFu, ax, ay);
-        if (len > 1) add_entry(buf, rc.y >> 16, ax, ay);
-        if (len > 2) add_entry(buf, p1 & 0xFFFFu, ax, ay);
-        if (len > 3) add_entry(buf, p1 >> 16, ax, ay);
-        for (int q = 2; 2 * q < len; ++q) {
-          const uint32_t pq = __ldg(fpair + __ldg(frow + q).x + k);
-          add_entry(buf, pq & 0xFFFFu, ax, ay);
-          if (2 * q + 1 < len) add_entry(buf, pq >> 16, ax, ay);
-        }
-        const int j = rc.x & 0xFFFFu;
-        const float2 a = S[j];
-        S[j] = make_float2(a.x + ax, a.y + ay);
-      };
-#pragma unroll
-      for (int q = 0; q < kCellsPf; ++q) sum_cell(rec[q], pr1[q], tid + q * THREADS);
-      for (int k = tid + kCellsPf * THREADS; k < p.n_can_max; k += THREADS)
-        sum_cell(__ldg(frec + k), k < row1.y ? __ldg(fpair + row1.x + k) : 0u, k);
-      __syncthreads();                  // buffer b is free, S is consistent
+      mbar_wait(full + b, (fphase >> b) & 1u);
+      fphase ^= 1u << b;
+      // this warp's stream: groups of 32 lanes ordered by descending rows L; counts of each L in wd.y
+      const uint32_t tab = smem_u32(buf_of(b)) + vis_bytes;
+      const uint2 wd = lds_u2(tab + 8u * warp);
+      uint32_t blk = tab + wd.x + 2u * lane;
+      for (int n = wd.y & 0xFF; n > 0; --n, blk += 5 * 64) gather_group<4>(blk, sm_base, S_base);
+      for (int n = (wd.y >> 8) & 0xFF; n > 0; --n, blk += 4 * 64) gather_group<3>(blk, sm_base, S_base);
+      for (int n = (wd.y >> 16) & 0xFF; n > 0; --n, blk += 3 * 64) gather_group<2>(blk, sm_base, S_base);
+      for (int n = wd.y >> 24; n > 0; --n, blk += 2 * 64) gather_group<1>(blk, sm_base, S_base);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + b);    // this warp is done with the buffer
       if (tid == 0) {
-        if (c + p.nbuf < p.n_chunk) issue(s, c + p.nbuf);
-        else if (c == c_last0 && s + (int)gridDim.x < p.n_snap) issue(s + gridDim.x, 0);
+        if (c + p.nbuf < p.n_chunk) produce(s, c + p.nbuf);
+        else if (c == c_last0 && s + (int)gridDim.x < p.n_snap) produce(s + gridDim.x, 0);
       }
     }
 
-    // ---- phase H: zero the bounding-box rows of the lines, then drop in the occupied cells ------
-    const int kym = ci.ky_max, nrow = 2 * kym + 1;
-    for (int e = tid; e < nrow * p.n_col; e += THREADS) {
-      const int c = e / nrow, iy = (e % nrow - kym + N) & (N - 1);
-      lines[c * LS + pad16(iy)] = make_float2(0.f, 0.f);
-    }
+    // ---- phase H: every bounding-box cell with kx >= 0, weighted, into the column lines --------
+    const int kym = ci.ky_max;
     {
-      const size_t hb = (size_t)ch * 2 * p.n_bl;
-      for (int e0 = 0; e0 < p.h_max; e0 += kHPer * THREADS) {
-        int code[kHPer], pos[kHPer];
-        float w[kHPer];
+      const uint2 *__restrict__ hrec = p.hrec + (size_t)ch * p.h_max;
+      uint2 hr[kHPer];
 #pragma unroll
-        for (int c = 0; c < kHPer; ++c) {          // independent table loads, issued together
-          const int e = e0 + c * THREADS + tid;
-          pos[c] = e < p.h_max ? __ldg(p.hpos + hb + e) : -1;
-          code[c] = e < p.h_max ? __ldg(p.hcode + hb + e) : 0;
-          w[c] = e < p.h_max ? __ldg(p.hw + hb + e) : 0.f;
-        }
-        if (e0 == 0) __syncthreads();               // the zero fill above is complete
-#pragma unroll
-        for (int c = 0; c < kHPer; ++c) {
-          if (pos[c] < 0) continue;                  // tables are padded with pos = -1
-          const float2 v = S[code[c] & kPlaceMask];
-          const int flag = code[c] >> kPlaceShift;
-          float2 o;
-          if (flag == kPlaceDirect) o = make_float2(v.x * w[c], v.y * w[c]);
-          else if (flag == kPlaceConj) o = make_float2(v.x * w[c], -v.y * w[c]);
-          else o = make_float2((v.x + v.x) * w[c], 0.f);
-          lines[pos[c]] = o;
-        }
+      for (int q = 0; q < kHPer; ++q) {            // records do not depend on the sums: fetch first
+        const int e = tid + q * THREADS;
+        hr[q] = e < p.h_max ? __ldg(hrec + e) : make_uint2(0xFFFFu, 0u);
       }
-      if (p.h_max == 0) __syncthreads();
+      __syncthreads();                              // all sums done, all chunk buffers released
+      auto place = [&](uint2 r) {
+        const uint32_t pos = r.x & 0xFFFFu;
+        if (pos == 0xFFFFu) return;
+        const float2 v = S[(r.x >> 16) & 0x3FFFu];
+        const uint32_t flag = r.x >> 30;
+        const float w = __uint_as_float(r.y);
+        float2 o;
+        if (flag == kPlaceDirect) o = make_float2(v.x * w, v.y * w);
+        else if (flag == kPlaceConj) o = make_float2(v.x * w, -v.y * w);
+        else o = make_float2((v.x + v.x) * w, 0.f);
+        lines[pos] = o;
+      };
+#pragma unroll
+      for (int q = 0; q < kHPer; ++q) place(hr[q]);
+      for (int e = tid + kHPer * THREADS; e < p.h_max; e += THREADS) place(__ldg(hrec + e));
     }
     __syncthreads();
+    // the sums are consumed: clear them for the next snapshot (sink and zero slot stay zero)
+    for (int j = tid; j < p.n_can_max; j += THREADS) S[j] = make_float2(0.f, 0.f);
 
     // ---- pass A: columns kx = 0..kx_max, in place ----------------------------------------------
     for (int c0 = 0; c0 <= ci.kx_max; c0 += G) {
@@ -291,55 +315,374 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   }
 }
 
-// shared-memory plan of the route; returns false if it does not fit.  Layout (bytes):
-//   [0, region)            column lines + pass-B exchange lines; doubles as chunk buffers 1..nbuf-1
-//   [off_dedicated, +C*8)  chunk buffer 0
-//   [off_S, +n_can_max*8)  canonical cell sums
-//   [off_bar, +nbuf*8)     mbarriers
-static bool fused_layout(blink_plan *p, int threads) {
-  const int N = p->n_pix, T = N / 16, G = threads / std::max(T, 1);
-  const size_t region = sizeof(float2) * ((size_t)(p->kx_max_all + 1) * fused_line_stride(N) + (size_t)G * (N + N / 16));
-  const size_t region_al = (region + 127) / 128 * 128;
-  const size_t s_bytes = (sizeof(float2) * (size_t)std::max(p->n_can_max, 1) + 15) / 16 * 16;
-  const size_t limit = (size_t)p->max_smem_optin;
-  for (int n_chunk = 1; n_chunk <= 64; ++n_chunk) {
-    int C = (p->n_bl + n_chunk - 1) / n_chunk;
-    C = (C + 1) & ~1;                              // 16-byte multiples
-    if (C > 0x8000) continue;                      // 15-bit local baseline index
-    const size_t cb = sizeof(float2) * (size_t)C;
-    const int nbuf = 1 + (int)std::min<size_t>(7, region / cb);
-    if (nbuf < 2 && n_chunk > 1) continue;         // the ring needs a second buffer
-    const size_t total = region_al + cb + s_bytes + 8 * (size_t)nbuf + 64;
-    if (total > limit) continue;
-    p->fused_chunk_vis = C;
-    p->fused_n_chunk = (p->n_bl + C - 1) / C;
-    p->fused_nbuf = std::min(nbuf, std::max(p->fused_n_chunk, 1));
-    p->fused_off_dedicated = (uint32_t)region_al;
-    p->fused_off_S = (uint32_t)(region_al + cb);
-    p->fused_off_bar = (uint32_t)(region_al + cb + s_bytes);
-    p->fused_smem = region_al + cb + s_bytes + 8 * (size_t)p->fused_nbuf + 16;
-    return true;
+// ---------------------------------------------------------------------------------------------
+// Host: phase-S gather tables and the shared-memory plan of the route.
+//
+// Cells are dealt to the kFusedWarps warps once per channel (longest first, to the least loaded
+// warp) and numbered so that the cells of a warp cycle through the 16 shared-memory banks (an
+// 8-byte slot's bank is slot mod 16).  For a chunk [lo, hi) of baselines and a warp, each of the
+// warp's cells with baselines in the chunk gives one piece (its baselines in the chunk), or several
+// pieces of at most kFusedLcap baselines.  The pieces are packed, longest first, into groups of 32
+// lanes (two half-warps of 16) of L <= kFusedLcap rows: a piece goes to the lane and rows where it
+// collides least with what is already there -- in a half-warp the 16 cell sums should sit in 16
+// different banks, and so should the 16 visibilities of every row -- so the shared-memory reads of
+// the inner loop are (nearly) conflict-free.  Pieces of one cell never share a group.  Table of one
+// (channel, chunk), all offsets in bytes from its start:
+//   [0, 128)                per warp: uint32 offset of its stream, uint32 number of groups with
+//                           L = 4, 3, 2, 1 (one byte each, from the low byte)
+//   stream of a warp:       groups in descending L; per group: uint16 j[32]  slot of the cell sum in S
+//                             (empty lanes: the zero slot of a bank the half-warp does not use)
+//                           L rows of uint16 e[32]: slot | conj << 15, where slot is the visibility's
+//                             position in shared memory in 8-byte units (padding: a zero slot in a
+//                             bank the half-row does not use)
+struct AbstractTable {           // entries still relative to the chunk: (bl - lo) | conj << 15, 0x7FFF = padding
+  std::vector<unsigned char> bytes;
+  long rows = 0, halfrow_wavefronts = 0, groups = 0, rmw_wavefronts = 0;   // statistics
+};
+
+struct FusedPiece { int32_t len, slot, first; };   // first: index into HostGather::src
+
+struct PackGroup {
+  int L = 0;
+  int n[2] = {0, 0};                       // lanes used per half
+  uint32_t sbank[2] = {0, 0};              // banks of the cell sums per half (bit mask)
+  int scount[2][16] = {};                  // cell sums per bank per half
+  int bcount[2][kFusedLcap][16] = {};      // visibilities per bank per half-row
+  std::vector<int32_t> cells;              // slots of the cells in the group
+  int32_t lane_slot[32];
+  int32_t lane_entry[32][kFusedLcap];      // index into HostGather::src or -1
+};
+
+static void build_chunk_table(const HostGather &g, const std::vector<int> &owner, const std::vector<int> &slot,
+                              int lo, int hi, int sink0, AbstractTable &out, bool &ok) {
+  std::vector<std::vector<FusedPiece>> pieces(kFusedWarps);
+  for (int j = 0; j < g.n_can; ++j) {
+    int e0 = g.seg_start[j], e1 = g.seg_start[j + 1];
+    while (e0 < e1 && (g.src[e0] >> 1) < lo) ++e0;
+    int e2 = e0;
+    while (e2 < e1 && (g.src[e2] >> 1) < hi) ++e2;
+    const int n = e2 - e0;
+    if (n == 0) continue;
+    const int n_pieces = (n + kFusedLcap - 1) / kFusedLcap;
+    int first = e0;
+    for (int q = 0; q < n_pieces; ++q) {
+      const int len = n / n_pieces + (q < n % n_pieces ? 1 : 0);
+      pieces[owner[j]].push_back({len, slot[j], first});
+      first += len;
+    }
   }
-  return false;
+  std::vector<unsigned char> &o = out.bytes;
+  o.assign(128, 0);
+  static const int perms[24][4] = {{0,1,2,3},{0,1,3,2},{0,2,1,3},{0,2,3,1},{0,3,1,2},{0,3,2,1},{1,0,2,3},{1,0,3,2},
+                                   {1,2,0,3},{1,2,3,0},{1,3,0,2},{1,3,2,0},{2,0,1,3},{2,0,3,1},{2,1,0,3},{2,1,3,0},
+                                   {2,3,0,1},{2,3,1,0},{3,0,1,2},{3,0,2,1},{3,1,0,2},{3,1,2,0},{3,2,0,1},{3,2,1,0}};
+  for (int w = 0; w < kFusedWarps; ++w) {
+    auto &pw = pieces[w];
+    std::stable_sort(pw.begin(), pw.end(), [](const FusedPiece &a, const FusedPiece &b) { return a.len > b.len; });
+    std::vector<PackGroup> groups;
+    for (const FusedPiece &pc : pw) {
+      int bank[kFusedLcap];
+      for (int k = 0; k < pc.len; ++k) bank[k] = ((g.src[pc.first + k] >> 1) - lo) & 15;   // buffers are 128-byte aligned
+      int best_cost = 1 << 30, best_g = -1, best_h = 0, best_perm = 0;
+      for (int gi = 0; gi < (int)groups.size() && best_cost > 0; ++gi) {
+        PackGroup &G = groups[gi];
+        if (std::find(G.cells.begin(), G.cells.end(), pc.slot) != G.cells.end()) continue;
+        for (int h = 0; h < 2 && best_cost > 0; ++h) {
+          if (G.n[h] >= 16) continue;
+          const int sc = 2 * G.scount[h][pc.slot & 15];
+          for (int pi = 0; pi < 24; ++pi) {
+            // the piece's k-th visibility goes to row perms[pi][k]; rows must be < L and distinct
+            bool valid = true;
+            int cost = sc;
+            for (int k = 0; k < pc.len; ++k) {
+              const int r = perms[pi][k];
+              if (r >= G.L) { valid = false; break; }
+              cost += G.bcount[h][r][bank[k]];
+            }
+            if (valid && cost < best_cost) { best_cost = cost; best_g = gi; best_h = h; best_perm = pi; }
+            if (best_cost == 0) break;
+          }
+        }
+      }
+      if (best_g < 0) {                      // no free lane anywhere: a new group, as long as this piece
+        PackGroup G;
+        G.L = pc.len;
+        std::fill(&G.lane_slot[0], &G.lane_slot[32], -1);
+        for (auto &le : G.lane_entry) std::fill(&le[0], &le[kFusedLcap], -1);
+        groups.push_back(G);
+        best_g = (int)groups.size() - 1; best_h = 0; best_perm = 0;
+      }
+      PackGroup &G = groups[best_g];
+      const int lane = best_h * 16 + G.n[best_h]++;
+      G.cells.push_back(pc.slot);
+      G.lane_slot[lane] = pc.slot;
+      G.scount[best_h][pc.slot & 15]++;
+      G.sbank[best_h] |= 1u << (pc.slot & 15);
+      for (int k = 0; k < pc.len; ++k) {
+        const int r = perms[best_perm][k];
+        G.lane_entry[lane][r] = pc.first + k;
+        G.bcount[best_h][r][bank[k]]++;
+      }
+    }
+    std::stable_sort(groups.begin(), groups.end(), [](const PackGroup &a, const PackGroup &b) { return a.L > b.L; });
+    uint32_t counts = 0;
+    int per_L[kFusedLcap + 1] = {};
+    for (const PackGroup &G : groups) per_L[G.L]++;
+    for (int L = 1; L <= kFusedLcap; ++L) {
+      if (per_L[L] > kFusedMaxGroups) { ok = false; return; }
+      counts |= (uint32_t)per_L[L] << (8 * (kFusedLcap - L));
+    }
+    const uint32_t off = (uint32_t)o.size();
+    std::memcpy(o.data() + 8 * w, &off, 4);
+    std::memcpy(o.data() + 8 * w + 4, &counts, 4);
+    for (const PackGroup &G : groups) {
+      const size_t base = o.size();
+      o.resize(base + (size_t)(G.L + 1) * 64, 0);
+      uint16_t *rows = reinterpret_cast<uint16_t *>(o.data() + base);
+      out.groups++;
+      out.rows += G.L;
+      for (int h = 0; h < 2; ++h) {
+        int mx = 1;
+        for (int bk = 0; bk < 16; ++bk) mx = std::max(mx, G.scount[h][bk]);
+        out.rmw_wavefronts += mx;
+        for (int r = 0; r < G.L; ++r) {
+          int m = 1;
+          for (int bk = 0; bk < 16; ++bk) m = std::max(m, G.bcount[h][r][bk]);
+          out.halfrow_wavefronts += m;
+        }
+        // empty lanes fold zero into the zero slot of a bank the half does not use
+        int fb = 0;
+        for (int l = h * 16; l < h * 16 + 16; ++l) {
+          if (G.lane_slot[l] >= 0) { rows[l] = (uint16_t)G.lane_slot[l]; continue; }
+          while (fb < 15 && (G.sbank[h] >> fb & 1u)) ++fb;
+          rows[l] = (uint16_t)(sink0 + fb);
+          if (fb < 15) ++fb;
+        }
+      }
+      for (int l = 0; l < 32; ++l)
+        for (int r = 0; r < G.L; ++r) {
+          uint16_t e = 0x7FFFu;
+          if (G.lane_entry[l][r] >= 0) {
+            const int code = g.src[G.lane_entry[l][r]];
+            e = (uint16_t)(((code >> 1) - lo) | ((code & 1) << 15));
+          }
+          rows[(size_t)(r + 1) * 32 + l] = e;
+        }
+    }
+  }
+  o.resize((o.size() + 15) / 16 * 16, 0);
 }
 
 int fused_setup(blink_plan *p) {
   p->fused_path = 0;
   p->fused_chunk = p->chunk_snapshots;   // the two-kernel route chunks like blink_image
-  // shared-memory route: two-stage transforms (N <= 256), everything resident in one SM, and
-  // 16-byte aligned snapshots (even n_bl) for the bulk copies
+  return BLINK_OK;
+}
+
+// Decide whether the shared-memory route applies (two-stage transforms, N <= 256; everything
+// resident in one SM; 16-byte aligned snapshots, i.e. even n_bl, for the bulk copies), lay out
+// shared memory, build and upload the tables.  Layout (bytes):
+//   [0, region)             column lines + pass-B exchange lines; doubles as chunk buffers 1..nbuf-1
+//   [off_dedicated, +B)     chunk buffer 0            (B = chunk_vis * 8 + tab_stride, 128-aligned)
+//   [off_S, ...)            canonical cell sums, sink, zero slot
+//   [off_bar, ...)          full[nbuf], empty[nbuf] mbarriers
+int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st) {
   int want = 1;
   if (const char *e = getenv("BLINK_FUSED_SMEM")) want = atoi(e);
-  if (want && p->n_pix <= 256 && p->n_pix >= 32 && (p->n_bl & 1) == 0 && p->max_smem_optin > 0) {
-    p->fused_threads = 512;
-    if (fused_layout(p, p->fused_threads)) p->fused_path = 1;
+  const int N = p->n_pix, n_bl = p->n_bl, n_ch = p->n_ch;
+  if (!want || N > 256 || N < 32 || (n_bl & 1) || p->max_smem_optin <= 0) return BLINK_OK;
+  const int sink0 = (p->n_can_max + 15) & ~15;                    // S[sink0 + b]: the always-zero slot of bank b
+  const int n_S = sink0 + 16;
+  if (n_S > 0x3FFF) return BLINK_OK;                              // 14-bit slot index in the phase-H records
+  const int LS = fused_line_stride(N);
+  const int n_col = p->kx_max_all + 1;
+  if ((size_t)n_col * LS >= 0xFFFFu) return BLINK_OK;             // 16-bit line position
+  const int T = N / 16, G = kFusedThreads / T;
+  const size_t region = sizeof(float2) * ((size_t)n_col * LS + (size_t)G * (N + N / 16));
+  const size_t region_al = (region + 127) / 128 * 128;
+  const size_t s_bytes = sizeof(float2) * (size_t)n_S;
+  const size_t limit = (size_t)p->max_smem_optin;
+
+  // cell -> warp, per channel: longest first to the least loaded warp; the cells of a warp get
+  // consecutive slots of S in that order, so their banks cycle
+  std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
+  for (int ch = 0; ch < n_ch; ++ch) {
+    const HostGather &g = gathers[ch];
+    std::vector<int> order(g.n_can);
+    for (int j = 0; j < g.n_can; ++j) order[j] = j;
+    auto len = [&](int j) { return g.seg_start[j + 1] - g.seg_start[j]; };
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len(a) > len(b); });
+    std::vector<long> load(kFusedWarps, 0);
+    owner[ch].assign(g.n_can, 0);
+    for (int j : order) {
+      const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+      owner[ch][j] = w;
+      load[w] += len(j) + 2;            // + the cost of folding the group sum into S[j]
+    }
+    slot[ch].assign(g.n_can, 0);
+    int next = 0;
+    for (int w = 0; w < kFusedWarps; ++w)
+      for (int j : order)
+        if (owner[ch][j] == w) slot[ch][j] = next++;
   }
+
+  int force_chunks = 0;
+  if (const char *e = getenv("BLINK_FUSED_CHUNKS")) force_chunks = atoi(e);
+  std::vector<AbstractTable> tabs;
+  int n_chunk = 0, C = 0, nbuf = 0;
+  size_t tab_stride = 0, buf_bytes = 0;
+  bool found = false;
+  for (n_chunk = std::max(1, force_chunks); n_chunk <= 64 && !found; ++n_chunk) {
+    C = (n_bl + n_chunk - 1) / n_chunk;
+    C = (C + 1) & ~1;                                  // 16-byte multiples
+    if (C > 0x7FFE) continue;                          // 15-bit slot index relative to the chunk
+    if ((n_bl + C - 1) / C != n_chunk) continue;
+    if (sizeof(float2) * (size_t)C + region_al + s_bytes > limit) continue;   // cannot fit whatever the tables
+    tabs.assign((size_t)n_ch * n_chunk, AbstractTable());
+    bool ok = true;
+    tab_stride = 0;
+    for (int ch = 0; ch < n_ch && ok; ++ch)
+      for (int c = 0; c < n_chunk && ok; ++c) {
+        AbstractTable &t = tabs[(size_t)ch * n_chunk + c];
+        build_chunk_table(gathers[ch], owner[ch], slot[ch], c * C, std::min(n_bl, (c + 1) * C), sink0, t, ok);
+        tab_stride = std::max(tab_stride, t.bytes.size());
+      }
+    if (!ok) continue;
+    buf_bytes = (sizeof(float2) * (size_t)C + tab_stride + 127) / 128 * 128;
+    nbuf = 1 + (int)std::min<size_t>(7, region / buf_bytes);
+    nbuf = std::min(nbuf, n_chunk);
+    if (nbuf < 2 && n_chunk > 1) continue;             // the ring needs a second buffer
+    const size_t total = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 64;
+    if (total > limit || total > 0x7FFFu * 8u) continue;
+    found = true;
+    break;
+  }
+  if (!found) return BLINK_OK;
+
+  p->fused_chunk_vis = C;
+  p->fused_n_chunk = n_chunk;
+  p->fused_nbuf = nbuf;
+  p->fused_tab_stride = (int)tab_stride;
+  p->fused_buf_bytes = (uint32_t)buf_bytes;
+  p->fused_off_dedicated = (uint32_t)region_al;
+  p->fused_off_S = (uint32_t)(region_al + buf_bytes);      // multiple of 128: slot s of S sits in bank s mod 16
+  p->fused_off_bar = (uint32_t)(region_al + buf_bytes + s_bytes);
+  p->fused_smem = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 16;
+  p->fused_threads = kFusedThreads;
+  if (getenv("BLINK_DEBUG")) {
+    long rows = 0, hw = 0, groups = 0, rmw = 0;
+    for (const AbstractTable &t : tabs) { rows += t.rows; hw += t.halfrow_wavefronts; groups += t.groups; rmw += t.rmw_wavefronts; }
+    fprintf(stderr, "blink fused route: %d chunks of %d baselines, table stride %zu B, buffer %zu B x %d, smem %zu B\n"
+            "  per snapshot: %.0f groups, %.0f rows (ideal %.0f), %.2f wavefronts per half-row, %.2f per half cell-sum access\n",
+            n_chunk, C, tab_stride, buf_bytes, nbuf, p->fused_smem, (double)groups / n_ch, (double)rows / n_ch,
+            (double)n_bl / 32, (double)hw / (2.0 * std::max(rows, 1L)), (double)rmw / (2.0 * std::max(groups, 1L)));
+  }
+
+  // relative entries -> shared-memory slots of the buffer the chunk will land in; a padded entry
+  // reads the zero slot of a bank that the real entries of its half-row leave free
+  const uint32_t s_slot0 = p->fused_off_S / 8;
+  std::vector<unsigned char> h_tab((size_t)n_ch * n_chunk * tab_stride, 0);
+  std::vector<uint32_t> h_size((size_t)n_ch * n_chunk, 0);
+  for (int ch = 0; ch < n_ch; ++ch)
+    for (int c = 0; c < n_chunk; ++c) {
+      const size_t cp = (size_t)ch * n_chunk + c;
+      std::vector<unsigned char> &b = tabs[cp].bytes;
+      const int bi = c % nbuf;
+      const uint32_t base_slot = (uint32_t)((bi == 0 ? p->fused_off_dedicated : (uint32_t)(bi - 1) * p->fused_buf_bytes) / 8);
+      for (int w = 0; w < kFusedWarps; ++w) {
+        uint32_t off, counts;
+        std::memcpy(&off, b.data() + 8 * w, 4);
+        std::memcpy(&counts, b.data() + 8 * w + 4, 4);
+        size_t blk = off;
+        for (int L = kFusedLcap; L >= 1; --L)
+          for (int gi = (counts >> (8 * (kFusedLcap - L))) & 0xFF; gi > 0; --gi) {
+            uint16_t *rows = reinterpret_cast<uint16_t *>(b.data() + blk);
+            for (int r = 1; r <= L; ++r)
+              for (int half = 0; half < 2; ++half) {
+                uint16_t *e = rows + (size_t)r * 32 + half * 16;
+                uint32_t used = 0;
+                for (int l = 0; l < 16; ++l)
+                  if ((e[l] & 0x7FFFu) != 0x7FFFu) {
+                    const uint32_t sl = base_slot + (e[l] & 0x7FFFu);
+                    e[l] = (uint16_t)(sl | (e[l] & 0x8000u));
+                    used |= 1u << (sl & 15);
+                  } else {
+                    e[l] = 0xFFFFu;                                             // marks padding until the bank is chosen
+                  }
+                int free_bank = 0;
+                while (free_bank < 15 && (used >> free_bank & 1u)) ++free_bank;
+                for (int l = 0; l < 16; ++l)
+                  if (e[l] == 0xFFFFu) e[l] = (uint16_t)(s_slot0 + sink0 + ((free_bank - (int)s_slot0) & 15));
+              }
+            blk += (size_t)(L + 1) * 64;
+          }
+      }
+      std::memcpy(h_tab.data() + cp * tab_stride, b.data(), b.size());
+      h_size[cp] = (uint32_t)b.size();
+    }
+
+  // phase-H records: every bounding-box cell with kx >= 0, column by column
+  std::vector<std::vector<uint2>> hrecs(n_ch);
+  p->h_max = 0;
+  for (int ch = 0; ch < n_ch; ++ch) {
+    const HostGather &g = gathers[ch];
+    const ChannelInfo &ci = p->chinfo[ch];
+    auto find_j = [&](int cell) -> int {
+      auto it = std::lower_bound(g.can_cell.begin(), g.can_cell.end(), cell);
+      return (it != g.can_cell.end() && *it == cell) ? (int)(it - g.can_cell.begin()) : -1;
+    };
+    auto pad16h = [](int i) { return i + (i >> 4); };
+    if (g.n_can == 0) continue;
+    for (int kx = 0; kx <= ci.kx_max; ++kx)
+      for (int ky = -ci.ky_max; ky <= ci.ky_max; ++ky) {
+        const int ix = kx, iy = (ky + N) % N;
+        const bool canonical = (ky > 0) || (ky == 0 && kx >= 0);
+        const int c = canonical ? iy * N + ix : ((N - iy) % N) * N + ((N - ix) % N);
+        const int j = find_j(c);
+        const uint32_t pos = (uint32_t)(kx * LS + pad16h(iy));
+        uint2 r;
+        if (j < 0) {
+          r = make_uint2(pos | ((uint32_t)sink0 << 16), 0u);                    // a zero slot x 0
+        } else {
+          int cnt = g.seg_start[j + 1] - g.seg_start[j];
+          if (c == 0) cnt *= 2;
+          float w = ((kx + ky) & 1) ? -ci.inv_norm : ci.inv_norm;
+          if (p->weighting == BLINK_UNIFORM) w /= (float)cnt;
+          const uint32_t flag = c == 0 ? kPlaceBoth : (canonical ? kPlaceDirect : kPlaceConj);
+          uint32_t wb;
+          std::memcpy(&wb, &w, 4);
+          r = make_uint2(pos | ((uint32_t)slot[ch][j] << 16) | (flag << 30), wb);
+        }
+        hrecs[ch].push_back(r);
+      }
+    p->h_max = std::max(p->h_max, (int)hrecs[ch].size());
+  }
+  std::vector<uint2> h_hrec((size_t)n_ch * std::max(p->h_max, 1), make_uint2(0xFFFFu, 0u));
+  for (int ch = 0; ch < n_ch; ++ch)
+    std::copy(hrecs[ch].begin(), hrecs[ch].end(), h_hrec.begin() + (size_t)ch * p->h_max);
+
+  auto upload = [&](void **dst, const void *src, size_t bytes) -> int {
+    cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
+    if (e != cudaSuccess) {
+      set_cuda_error(e, "fused table cudaMalloc");
+      *dst = nullptr;
+      return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
+    }
+    BLINK_CUDA_TRY(cudaMemcpyAsync(*dst, src, bytes, cudaMemcpyHostToDevice, st), "fused table upload");
+    return BLINK_OK;
+  };
+  int rc;
+  if ((rc = upload((void **)&p->d_gtab, h_tab.data(), h_tab.size())) != BLINK_OK) return rc;
+  if ((rc = upload((void **)&p->d_gsize, h_size.data(), sizeof(uint32_t) * h_size.size())) != BLINK_OK) return rc;
+  if ((rc = upload((void **)&p->d_hrec, h_hrec.data(), sizeof(uint2) * h_hrec.size())) != BLINK_OK) return rc;
+  BLINK_CUDA_TRY(cudaStreamSynchronize(st), "fused table upload sync");
+  p->fused_path = 1;
   return BLINK_OK;
 }
 
 template <int N>
 static int launch_fused_n(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
-  constexpr int THREADS = 512;
+  constexpr int THREADS = kFusedThreads;
   static thread_local size_t smem_set = 0;
   if (p->fused_smem > smem_set) {
     BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -358,11 +701,11 @@ static int launch_fused_n(const blink_plan *p, const FusedParams &fp, cudaStream
 static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st) {
   FusedParams fp;
   fp.vis = vis; fp.img = img; fp.chinfo = p->d_chinfo;
-  fp.frec = p->d_frec; fp.fpair = p->d_fpair; fp.frow = p->d_frow;
-  fp.hpos = p->d_hpos; fp.hcode = p->d_hcode; fp.hw = p->d_hw; fp.tw = p->d_tw;
+  fp.gtab = p->d_gtab; fp.gsize = p->d_gsize; fp.hrec = p->d_hrec; fp.tw = p->d_tw;
   fp.n_bl = p->n_bl; fp.n_ch = p->n_ch; fp.n_snap = n_t * p->n_ch; fp.n_can_max = p->n_can_max;
   fp.n_chunk = p->fused_n_chunk; fp.chunk_vis = p->fused_chunk_vis; fp.nbuf = p->fused_nbuf;
-  fp.frow_stride = p->frow_stride; fp.n_col = p->kx_max_all + 1; fp.h_max = p->h_max;
+  fp.tab_stride = p->fused_tab_stride; fp.n_col = p->kx_max_all + 1; fp.h_max = p->h_max;
+  fp.buf_bytes = p->fused_buf_bytes;
   fp.off_dedicated = p->fused_off_dedicated; fp.off_S = p->fused_off_S; fp.off_bar = p->fused_off_bar;
   switch (p->n_pix) {
     case 32: return launch_fused_n<32>(p, fp, st);

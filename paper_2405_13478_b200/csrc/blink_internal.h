@@ -97,21 +97,15 @@ struct blink_plan {
   int32_t *d_vlen = nullptr;        // [n_ch][2 n_bl] entries | flag << 24
   float *d_vw = nullptr;            // [n_ch][2 n_bl] sign * (1/norm) * (1/count if uniform)
   int32_t *d_vcol = nullptr;        // [n_ch][wu + 1] CSR by column
-  // shared-memory route: occupied cells with kx >= 0 -> slot in the column lines, source, weight
-  int32_t *d_hpos = nullptr;        // [n_ch][2 n_bl] kx * LS + pad16(iy)
-  int32_t *d_hcode = nullptr;       // [n_ch][2 n_bl] j | flag << kPlaceShift
-  float *d_hw = nullptr;            // [n_ch][2 n_bl] sign * (1/norm) * (1/count if uniform)
-  int32_t *d_hcount = nullptr;      // [n_ch]
-  int h_max = 0;                    // max over channels of the entry count; tables padded with pos = -1
+  // shared-memory route (see fused_build in blink_fused.cu)
+  int h_max = 0;                    // phase-H records per channel (padded with pos = 0xFFFF)
   int fused_threads = 512;
   size_t fused_smem = 0;
-  // shared-memory route, phase S: bulk-copied chunks of `fused_chunk_vis` baselines and the
-  // rank-major gather tables built for that chunk size (see RankTables in blink_plan.cu)
-  int fused_chunk_vis = 0, fused_n_chunk = 0, fused_nbuf = 0, frow_stride = 0;
-  uint32_t fused_off_dedicated = 0, fused_off_S = 0, fused_off_bar = 0;
-  uint2 *d_frec = nullptr;          // [n_ch][n_chunk][n_can_max] {j | len << 16, ranks 0,1}
-  uint32_t *d_fpair = nullptr;      // [n_ch][n_chunk][chunk_vis] rows q >= 1: ranks 2q, 2q+1
-  int2 *d_frow = nullptr;           // [n_ch][n_chunk][frow_stride] {offset into fpair, cells in row}
+  int fused_chunk_vis = 0, fused_n_chunk = 0, fused_nbuf = 0, fused_tab_stride = 0;
+  uint32_t fused_buf_bytes = 0, fused_off_dedicated = 0, fused_off_S = 0, fused_off_bar = 0;
+  unsigned char *d_gtab = nullptr;  // [n_ch][n_chunk][tab_stride] phase-S gather tables
+  uint32_t *d_gsize = nullptr;      // [n_ch][n_chunk] bytes of each table
+  uint2 *d_hrec = nullptr;          // [n_ch][h_max] {line position | j << 16 | flag << 30, weight}
 
 };
 
@@ -129,6 +123,7 @@ int launch_image(const blink_plan *p, const float2 *uv, int n_snap, int ch0, flo
 int image_setup(blink_plan *p);
 int image_reserve(blink_plan *p, int n_t);
 int fused_setup(blink_plan *p);
+int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st);
 int fused_line_stride(int n_pix);
 int fused_reserve(blink_plan *p, int n_t);
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);

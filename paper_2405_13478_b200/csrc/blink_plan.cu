@@ -199,8 +199,8 @@ static void plan_free(blink_plan *p) {
   if (!p) return;
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
-  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_hpos); cudaFree(p->d_hcode); cudaFree(p->d_hw); cudaFree(p->d_hcount); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol);
-  cudaFree(p->d_frec); cudaFree(p->d_fpair); cudaFree(p->d_frow);
+  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol);
+  cudaFree(p->d_gtab); cudaFree(p->d_gsize); cudaFree(p->d_hrec);
   delete p;
 }
 
@@ -499,89 +499,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     step(cudaStreamSynchronize(st));
     PLAN_CUDA(ce, "vis-route table upload");
   }
-  if (p->fused_path == 1) {
-    // phase-S gather tables for chunks of fused_chunk_vis baselines: per (channel, chunk) the cells
-    // by descending length with ranks 0,1 packed beside the record, and rows q >= 1 holding ranks
-    // 2q, 2q+1 of the cells with more than 2q entries (0xFFFF = no second entry)
-    RankTables ft;
-    build_rank_tables(gathers, n_ch, n_bl, ncm, p->fused_chunk_vis, ft);
-    const int C = p->fused_chunk_vis, n_chunk = ft.n_pass;
-    if (n_chunk != p->fused_n_chunk) { plan_free(p); return BLINK_EUNSUPPORTED; }
-    int maxlen = 0;
-    for (size_t i = 0; i < ft.cellrec.size(); ++i) maxlen = std::max(maxlen, (int)(ft.cellrec[i] >> 16));
-    p->frow_stride = std::max(2, (maxlen + 1) / 2 + 1);
-    std::vector<uint2> h_frec((size_t)n_ch * n_chunk * ncm, make_uint2(0u, 0u));
-    std::vector<uint32_t> h_fpair((size_t)n_ch * n_chunk * C, 0u);
-    std::vector<int2> h_frow((size_t)n_ch * n_chunk * p->frow_stride, make_int2(0, 0));
-    for (size_t cp = 0; cp < (size_t)n_ch * n_chunk; ++cp) {
-      const uint32_t *cr = ft.cellrec.data() + cp * ncm;
-      const uint16_t *ls = ft.list.data() + cp * C;
-      const uint16_t *ro = ft.roff.data() + cp * ft.roff_stride;
-      const int n_act = ft.nact[cp];
-      auto entry = [&](int k, int r) -> uint32_t {
-        return r < (int)(cr[k] >> 16) ? (uint32_t)ls[ro[r] + k] : 0xFFFFu;
-      };
-      for (int k = 0; k < n_act; ++k) h_frec[cp * ncm + k] = make_uint2(cr[k], entry(k, 0) | (entry(k, 1) << 16));
-      int off = 0;
-      for (int q = 1; q < p->frow_stride; ++q) {
-        int cnt = 0;
-        while (cnt < n_act && (int)(cr[cnt] >> 16) > 2 * q) ++cnt;     // lengths descend
-        h_frow[cp * p->frow_stride + q] = make_int2(off, cnt);
-        for (int k = 0; k < cnt; ++k) h_fpair[cp * C + off + k] = entry(k, 2 * q) | (entry(k, 2 * q + 1) << 16);
-        off += cnt;
-      }
-    }
-    PLAN_TRY(dev_alloc(&p->d_frec, h_frec.size()));
-    PLAN_TRY(dev_alloc(&p->d_fpair, h_fpair.size()));
-    PLAN_TRY(dev_alloc(&p->d_frow, h_frow.size()));
-    step(cudaMemcpyAsync(p->d_frec, h_frec.data(), sizeof(uint2) * h_frec.size(), cudaMemcpyHostToDevice, st));
-    step(cudaMemcpyAsync(p->d_fpair, h_fpair.data(), sizeof(uint32_t) * h_fpair.size(), cudaMemcpyHostToDevice, st));
-    step(cudaMemcpyAsync(p->d_frow, h_frow.data(), sizeof(int2) * h_frow.size(), cudaMemcpyHostToDevice, st));
-    step(cudaStreamSynchronize(st));
-    PLAN_CUDA(ce, "fused gather table upload");
-    const int LS = fused_line_stride(N);
-    std::vector<int32_t> h_hpos((size_t)n_ch * 2 * n_bl, -1), h_hcode((size_t)n_ch * 2 * n_bl, 0), h_hcount(n_ch, 0);
-    std::vector<float> h_hw((size_t)n_ch * 2 * n_bl, 0.f);
-    for (int ch = 0; ch < n_ch; ++ch) {
-      const HostGather &g = gathers[ch];
-      const float inv_norm = p->chinfo[ch].inv_norm;
-      size_t n = 0;
-      const size_t base = (size_t)ch * 2 * n_bl;
-      for (int j = 0; j < g.n_can; ++j) {
-        const int c = g.can_cell[j], ix = c % N, iy = c / N;
-        const int kx = ix < N / 2 ? ix : ix - N, ky = iy;          // canonical: 0 <= ky < N/2
-        int cnt = g.seg_start[j + 1] - g.seg_start[j];
-        if (c == 0) cnt *= 2;
-        float w = ((kx + ky) & 1) ? -inv_norm : inv_norm;
-        if (weighting == BLINK_UNIFORM) w /= (float)cnt;
-        auto pad16 = [](int i) { return i + (i >> 4); };
-        if (kx >= 0) {
-          h_hpos[base + n] = kx * LS + pad16(iy);
-          h_hcode[base + n] = j | ((c == 0 ? kPlaceBoth : kPlaceDirect) << kPlaceShift);
-          h_hw[base + n] = w;
-          ++n;
-        }
-        if (kx <= 0 && c != 0) {
-          h_hpos[base + n] = (-kx) * LS + pad16((N - iy) % N);
-          h_hcode[base + n] = j | (kPlaceConj << kPlaceShift);
-          h_hw[base + n] = w;
-          ++n;
-        }
-      }
-      h_hcount[ch] = (int32_t)n;
-      p->h_max = std::max(p->h_max, (int)n);
-    }
-    PLAN_TRY(dev_alloc(&p->d_hpos, h_hpos.size()));
-    PLAN_TRY(dev_alloc(&p->d_hcode, h_hcode.size()));
-    PLAN_TRY(dev_alloc(&p->d_hw, h_hw.size()));
-    PLAN_TRY(dev_alloc(&p->d_hcount, h_hcount.size()));
-    step(cudaMemcpyAsync(p->d_hpos, h_hpos.data(), sizeof(int32_t) * h_hpos.size(), cudaMemcpyHostToDevice, st));
-    step(cudaMemcpyAsync(p->d_hcode, h_hcode.data(), sizeof(int32_t) * h_hcode.size(), cudaMemcpyHostToDevice, st));
-    step(cudaMemcpyAsync(p->d_hw, h_hw.data(), sizeof(float) * h_hw.size(), cudaMemcpyHostToDevice, st));
-    step(cudaMemcpyAsync(p->d_hcount, h_hcount.data(), sizeof(int32_t) * n_ch, cudaMemcpyHostToDevice, st));
-    step(cudaStreamSynchronize(st));
-    PLAN_CUDA(ce, "fused table upload");
-  }
+  PLAN_TRY(fused_build(p, gathers, st));
   if (weighting == BLINK_UNIFORM) {
     // canonical cells are exactly the occupied half-plane cells with ky > 0 or (ky == 0, kx >= 0);
     // pass A of blink_image works on columns kx >= 0 and all ky, so list every occupied cell with
