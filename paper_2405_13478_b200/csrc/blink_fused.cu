@@ -43,7 +43,7 @@ using namespace blinkfft;
 // whole kernel.
 constexpr int kFusedThreads = 512;
 constexpr int kFusedWarps = kFusedThreads / 32;
-constexpr int kFusedMaxGroups = 255;  // groups of one length per (warp, chunk)
+constexpr int kFusedMaxGroups = 16;   // groups per (warp, chunk): their lengths fit one 32-bit word
 constexpr int kFusedLcap = 4;         // rows per group: longer per-chunk cell lists are split into pieces
 constexpr int kHPer = 7;              // phase-H records fetched per thread ahead of the barrier
 
@@ -94,30 +94,37 @@ __device__ __forceinline__ uint2 lds_u2(uint32_t addr) {
   return r;
 }
 
-// One group of phase S: lane l adds its (at most L) visibilities and folds the sum into its cell.
-// blk = shared address of the lane's column of the group block: row 0 the slot of the cell sum,
-// rows 1..L the entries, read sign-extended so that conj (bit 15) lands in the sign bit.
-template <int L> __device__ __forceinline__ void gather_group(uint32_t blk, uint32_t sm_base, uint32_t S_base) {
+// Phase S works through a warp's groups with a one-group software pipeline: the index column of
+// the next group (slot of the cell sum, kFusedLcap entries -- rows beyond the group's L are read
+// too and ignored) is requested before the visibilities of the current group are gathered, so a
+// group costs about one shared-memory latency instead of three.
+struct GroupIdx {
   uint32_t j;
-  int e[L];
-  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(j) : "r"(blk));
+  int e[kFusedLcap];     // sign-extended: conj (bit 15) lands in the sign bit
+};
+
+__device__ __forceinline__ void load_idx(GroupIdx &gi, uint32_t blk) {
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(gi.j) : "r"(blk));
 #pragma unroll
-  for (int r = 0; r < L; ++r) asm volatile("ld.shared.s16 %0, [%1];" : "=r"(e[r]) : "r"(blk + 64u * (r + 1)));
-  float2 v[L];
+  for (int r = 0; r < kFusedLcap; ++r) asm volatile("ld.shared.s16 %0, [%1];" : "=r"(gi.e[r]) : "r"(blk + 64u * (r + 1)));
+}
+
+// lane l adds its L visibilities and folds the sum into its cell
+template <int L> __device__ __forceinline__ void fold_group(const GroupIdx &gi, uint32_t sm_base, uint32_t S_base) {
+  float2 v[L], a;
 #pragma unroll
   for (int r = 0; r < L; ++r) {
-    const uint32_t addr = sm_base + ((uint32_t)(e[r] & 0x7FFF) << 3);
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v[r].x), "=f"(v[r].y) : "r"(addr));
+    asm volatile("{\n.reg .b32 t;\nand.b32 t, %2, 0x7FFF;\nmad.lo.u32 t, t, 8, %3;\nld.shared.v2.f32 {%0, %1}, [t];\n}"
+                 : "=f"(v[r].x), "=f"(v[r].y) : "r"(gi.e[r]), "r"(sm_base));
   }
-  float ax = v[0].x, ay = __uint_as_float(__float_as_uint(v[0].y) ^ ((uint32_t)e[0] & 0x80000000u));
+  uint32_t sa;
+  asm volatile("mad.lo.u32 %2, %3, 8, %4;\nld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(a.x), "=f"(a.y), "=r"(sa) : "r"(gi.j), "r"(S_base));
+  float ax = v[0].x, ay = __uint_as_float(__float_as_uint(v[0].y) ^ ((uint32_t)gi.e[0] & 0x80000000u));
 #pragma unroll
   for (int r = 1; r < L; ++r) {
     ax += v[r].x;
-    ay += __uint_as_float(__float_as_uint(v[r].y) ^ ((uint32_t)e[r] & 0x80000000u));
+    ay += __uint_as_float(__float_as_uint(v[r].y) ^ ((uint32_t)gi.e[r] & 0x80000000u));
   }
-  const uint32_t sa = S_base + (j << 3);
-  float2 a;
-  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(a.x), "=f"(a.y) : "r"(sa));
   a.x += ax;
   a.y += ay;
   asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(sa), "f"(a.x), "f"(a.y) : "memory");
@@ -150,8 +157,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   };
   uint32_t fphase = 0;                  // bit b: parity of the next wait on full[b]
   uint32_t ephase = 0;                  // producer only: bit b: parity of the last completed empty[b] phase
-  auto produce = [&](int s, int c) {    // thread 0 only
-    const int b = c % p.nbuf;
+  auto produce = [&](int s, int c, int b) {    // thread 0 only; b = c % nbuf
     mbar_wait(empty + b, ((ephase >> b) & 1u) ^ 1u);   // every warp has let go of the buffer
     ephase ^= 1u << b;
     const int cnt = min(p.chunk_vis, p.n_bl - c * p.chunk_vis);
@@ -182,7 +188,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
 #pragma unroll
   for (int b = 0; b < NB1; ++b) F::template twiddles<1>(tw1[b], t + b * T, p.tw);
   __syncthreads();
-  if (tid == 0 && blockIdx.x < p.n_snap) produce(blockIdx.x, 0);
+  if (tid == 0 && blockIdx.x < p.n_snap) produce(blockIdx.x, 0, 0);
   const int c_last0 = ((p.n_chunk - 1) / p.nbuf) * p.nbuf;   // last chunk of a snapshot in buffer 0
 
   for (int s = blockIdx.x; s < p.n_snap; s += gridDim.x) {
@@ -190,39 +196,58 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
     const ChannelInfo ci = p.chinfo[ch];
     // the lines / exchange area is idle until phase H: fill it with this snapshot's next chunks
     if (tid == 0)
-      for (int c = 1; c < min(p.n_chunk, p.nbuf); ++c) produce(s, c);
+      for (int c = 1; c < min(p.n_chunk, p.nbuf); ++c) produce(s, c, c);
+
+    // phase-H records do not depend on the sums: request them now, they arrive during phase S
+    uint2 hr[kHPer];
+    const uint2 *__restrict__ hrec = p.hrec + (size_t)ch * p.h_max;
+#pragma unroll
+    for (int q = 0; q < kHPer; ++q) {
+      const int e = tid + q * THREADS;
+      hr[q] = e < p.h_max ? __ldg(hrec + e) : make_uint2(0xFFFFu, 0u);
+    }
 
     // ---- phase S ----------------------------------------------------------------------------
-    for (int c = 0; c < p.n_chunk; ++c) {
-      const int b = c % p.nbuf;
+    for (int c = 0, b = 0; c < p.n_chunk; ++c) {
       mbar_wait(full + b, (fphase >> b) & 1u);
       fphase ^= 1u << b;
-      // this warp's stream: groups of 32 lanes ordered by descending rows L; counts of each L in wd.y
+      // this warp's stream of groups: wd.x = offset | number of groups << 24, wd.y = L - 1 of each
+      // group, two bits apiece
       const uint32_t tab = smem_u32(buf_of(b)) + vis_bytes;
       const uint2 wd = lds_u2(tab + 8u * warp);
-      uint32_t blk = tab + wd.x + 2u * lane;
-      for (int n = wd.y & 0xFF; n > 0; --n, blk += 5 * 64) gather_group<4>(blk, sm_base, S_base);
-      for (int n = (wd.y >> 8) & 0xFF; n > 0; --n, blk += 4 * 64) gather_group<3>(blk, sm_base, S_base);
-      for (int n = (wd.y >> 16) & 0xFF; n > 0; --n, blk += 3 * 64) gather_group<2>(blk, sm_base, S_base);
-      for (int n = wd.y >> 24; n > 0; --n, blk += 2 * 64) gather_group<1>(blk, sm_base, S_base);
+      uint32_t blk = tab + (wd.x & 0xFFFFFFu) + 2u * lane;
+      uint32_t lseq = wd.y;
+      int n = wd.x >> 24;
+      GroupIdx ga, gb;                         // two index sets, used alternately
+      load_idx(ga, blk);
+      auto step = [&](const GroupIdx &cur, GroupIdx &nxt) {
+        const int L = (lseq & 3u) + 1;
+        lseq >>= 2;
+        blk += (L + 1) * 64;
+        load_idx(nxt, blk);                    // past the last group: reads the bytes that follow, unused
+        if (L == 4) fold_group<4>(cur, sm_base, S_base);
+        else if (L == 3) fold_group<3>(cur, sm_base, S_base);
+        else if (L == 2) fold_group<2>(cur, sm_base, S_base);
+        else fold_group<1>(cur, sm_base, S_base);
+      };
+      while (n > 0) {
+        step(ga, gb);
+        if (--n == 0) break;
+        step(gb, ga);
+        --n;
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(empty + b);    // this warp is done with the buffer
       if (tid == 0) {
-        if (c + p.nbuf < p.n_chunk) produce(s, c + p.nbuf);
-        else if (c == c_last0 && s + (int)gridDim.x < p.n_snap) produce(s + gridDim.x, 0);
+        if (c + p.nbuf < p.n_chunk) produce(s, c + p.nbuf, b);
+        else if (c == c_last0 && s + (int)gridDim.x < p.n_snap) produce(s + gridDim.x, 0, 0);
       }
+      if (++b == p.nbuf) b = 0;
     }
 
     // ---- phase H: every bounding-box cell with kx >= 0, weighted, into the column lines --------
     const int kym = ci.ky_max;
     {
-      const uint2 *__restrict__ hrec = p.hrec + (size_t)ch * p.h_max;
-      uint2 hr[kHPer];
-#pragma unroll
-      for (int q = 0; q < kHPer; ++q) {            // records do not depend on the sums: fetch first
-        const int e = tid + q * THREADS;
-        hr[q] = e < p.h_max ? __ldg(hrec + e) : make_uint2(0xFFFFu, 0u);
-      }
       __syncthreads();                              // all sums done, all chunk buffers released
       auto place = [&](uint2 r) {
         const uint32_t pos = r.x & 0xFFFFu;
@@ -328,8 +353,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
 // different banks, and so should the 16 visibilities of every row -- so the shared-memory reads of
 // the inner loop are (nearly) conflict-free.  Pieces of one cell never share a group.  Table of one
 // (channel, chunk), all offsets in bytes from its start:
-//   [0, 128)                per warp: uint32 offset of its stream, uint32 number of groups with
-//                           L = 4, 3, 2, 1 (one byte each, from the low byte)
+//   [0, 128)                per warp: uint32 offset of its stream | number of groups << 24, uint32 with
+//                           L - 1 of each group (two bits apiece, first group in the low bits)
 //   stream of a warp:       groups in descending L; per group: uint16 j[32]  slot of the cell sum in S
 //                             (empty lanes: the zero slot of a bank the half-warp does not use)
 //                           L rows of uint16 e[32]: slot | conj << 15, where slot is the visibility's
@@ -380,6 +405,9 @@ static void build_chunk_table(const HostGather &g, const std::vector<int> &owner
     auto &pw = pieces[w];
     std::stable_sort(pw.begin(), pw.end(), [](const FusedPiece &a, const FusedPiece &b) { return a.len > b.len; });
     std::vector<PackGroup> groups;
+    static const int spare = getenv("BLINK_FUSED_SPARE") ? atoi(getenv("BLINK_FUSED_SPARE")) : 0;
+    static const int thresh = getenv("BLINK_FUSED_THRESH") ? atoi(getenv("BLINK_FUSED_THRESH")) : 99;
+    const int max_groups = ((int)pw.size() + 31) / 32 + spare;
     for (const FusedPiece &pc : pw) {
       int bank[kFusedLcap];
       for (int k = 0; k < pc.len; ++k) bank[k] = ((g.src[pc.first + k] >> 1) - lo) & 15;   // buffers are 128-byte aligned
@@ -404,7 +432,9 @@ static void build_chunk_table(const HostGather &g, const std::vector<int> &owner
           }
         }
       }
-      if (best_g < 0) {                      // no free lane anywhere: a new group, as long as this piece
+      // no free lane anywhere, or only badly colliding ones while a spare group is allowed: a new
+      // group, as long as this piece
+      if (best_g < 0 || (best_cost >= thresh && (int)groups.size() < max_groups)) {
         PackGroup G;
         G.L = pc.len;
         std::fill(&G.lane_slot[0], &G.lane_slot[32], -1);
@@ -425,16 +455,12 @@ static void build_chunk_table(const HostGather &g, const std::vector<int> &owner
       }
     }
     std::stable_sort(groups.begin(), groups.end(), [](const PackGroup &a, const PackGroup &b) { return a.L > b.L; });
-    uint32_t counts = 0;
-    int per_L[kFusedLcap + 1] = {};
-    for (const PackGroup &G : groups) per_L[G.L]++;
-    for (int L = 1; L <= kFusedLcap; ++L) {
-      if (per_L[L] > kFusedMaxGroups) { ok = false; return; }
-      counts |= (uint32_t)per_L[L] << (8 * (kFusedLcap - L));
-    }
-    const uint32_t off = (uint32_t)o.size();
+    if ((int)groups.size() > kFusedMaxGroups) { ok = false; return; }
+    uint32_t lseq = 0;
+    for (size_t gi = 0; gi < groups.size(); ++gi) lseq |= (uint32_t)(groups[gi].L - 1) << (2 * gi);
+    const uint32_t off = (uint32_t)o.size() | ((uint32_t)groups.size() << 24);
     std::memcpy(o.data() + 8 * w, &off, 4);
-    std::memcpy(o.data() + 8 * w + 4, &counts, 4);
+    std::memcpy(o.data() + 8 * w + 4, &lseq, 4);
     for (const PackGroup &G : groups) {
       const size_t base = o.size();
       o.resize(base + (size_t)(G.L + 1) * 64, 0);
@@ -513,6 +539,8 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
     auto len = [&](int j) { return g.seg_start[j + 1] - g.seg_start[j]; };
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len(a) > len(b); });
     std::vector<long> load(kFusedWarps, 0);
+    static const int w0bias = getenv("BLINK_FUSED_W0BIAS") ? atoi(getenv("BLINK_FUSED_W0BIAS")) : 4;
+    load[0] = (long)g.n_kept * w0bias / (100 * kFusedWarps);     // warp 0 also runs the chunk ring (thread 0)
     owner[ch].assign(g.n_can, 0);
     for (int j : order) {
       const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
@@ -590,12 +618,12 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
       const int bi = c % nbuf;
       const uint32_t base_slot = (uint32_t)((bi == 0 ? p->fused_off_dedicated : (uint32_t)(bi - 1) * p->fused_buf_bytes) / 8);
       for (int w = 0; w < kFusedWarps; ++w) {
-        uint32_t off, counts;
+        uint32_t off, lseq;
         std::memcpy(&off, b.data() + 8 * w, 4);
-        std::memcpy(&counts, b.data() + 8 * w + 4, 4);
-        size_t blk = off;
-        for (int L = kFusedLcap; L >= 1; --L)
-          for (int gi = (counts >> (8 * (kFusedLcap - L))) & 0xFF; gi > 0; --gi) {
+        std::memcpy(&lseq, b.data() + 8 * w + 4, 4);
+        size_t blk = off & 0xFFFFFFu;
+        for (int gi = (int)(off >> 24); gi > 0; --gi, lseq >>= 2) {
+            const int L = (int)(lseq & 3u) + 1;
             uint16_t *rows = reinterpret_cast<uint16_t *>(b.data() + blk);
             for (int r = 1; r <= L; ++r)
               for (int half = 0; half < 2; ++half) {
