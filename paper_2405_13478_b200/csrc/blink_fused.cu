@@ -130,7 +130,9 @@ template <int L> __device__ __forceinline__ void fold_group(const GroupIdx &gi, 
   asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(sa), "f"(a.x), "f"(a.y) : "memory");
 }
 
-template <int N, int THREADS>
+// NZ: the first radix-16 stage of both passes reads inputs r = 0..NZ-1 and 16-NZ..15 only (the
+// bounding box reaches at most NZ * N/16 - 1 cells from the origin); NZ = 8 reads everything.
+template <int N, int THREADS, int NZ>
 __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   constexpr int T = N / 16;             // lanes per transform
   constexpr int G = THREADS / T;        // transforms in flight per CTA
@@ -139,6 +141,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   using F = Fft<N>;
   static_assert(F::NSTAGE == 2 && T <= 32, "shared-memory route needs a two-stage warp-local transform");
   static_assert(THREADS == kFusedThreads, "the gather tables are built for kFusedWarps warps");
+  constexpr unsigned BM = BandMask<NZ>::value;
+  constexpr int NZL = NZ >= 8 ? 8 : NZ;         // inputs read from each end of a first-stage butterfly
   extern __shared__ __align__(128) unsigned char smem_raw[];
   float2 *lines = reinterpret_cast<float2 *>(smem_raw);                       // [n_col][LS]
   float2 *X = lines + (size_t)p.n_col * LS;                                   // exchange lines [G][LSB]
@@ -275,13 +279,18 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
       const bool act = c <= ci.kx_max;            // uniform per transform group (T lanes)
       float2 *line = lines + (size_t)(act ? c : 0) * LS;
       cf32 v[16];
-      if (act)
-        F::template load<0>(v, t, [&](int idx) {
-          return (idx <= kym || idx >= N - kym) ? line[pad16(idx)] : mk(0.f, 0.f);
-        });
+      if (act) {
+        // stage-0 inputs idx = t + r*T: only r < NZL and r >= 16 - NZL can lie inside the bounding box
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+          if (r >= NZL && r < 16 - NZL) continue;
+          const int idx = t + r * T;
+          v[r] = (idx <= kym || idx >= N - kym) ? line[pad16(idx)] : mk(0.f, 0.f);
+        }
+      }
       __syncwarp();
       if (act) {
-        F::template compute<0>(v, t, p.tw);
+        F::template compute0_pruned<BM>(v);
         F::template store<0>(v, t, [&](int idx, cf32 x) { line[pad16(idx)] = x; });
       }
       __syncwarp();
@@ -308,20 +317,23 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
         // (conj a + i conj b at k = N - idx) -- static per r, branch-free, all loads in flight
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-          float2 a[8], b[8];
+          float2 a[NZL], b[NZL];
 #pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            const int idx = t + (8 * h + q) * T;
+          for (int q = 0; q < NZL; ++q) {
+            const int r = h == 0 ? q : 16 - NZL + q;
+            const int idx = t + r * T;
             const int k = h == 0 ? idx : N - idx;
             const bool ok = k <= kxm;
             a[q] = ok ? lines[k * LS + o0] : make_float2(0.f, 0.f);
             b[q] = ok ? lines[k * LS + o1] : make_float2(0.f, 0.f);
           }
 #pragma unroll
-          for (int q = 0; q < 8; ++q)
-            v[8 * h + q] = h == 0 ? mk(a[q].x - b[q].y, a[q].y + b[q].x) : mk(a[q].x + b[q].y, b[q].x - a[q].y);
+          for (int q = 0; q < NZL; ++q) {
+            const int r = h == 0 ? q : 16 - NZL + q;
+            v[r] = h == 0 ? mk(a[q].x - b[q].y, a[q].y + b[q].x) : mk(a[q].x + b[q].y, b[q].x - a[q].y);
+          }
         }
-        F::template compute<0>(v, t, p.tw);
+        F::template compute0_pruned<BM>(v);
       }
       __syncwarp();                                   // previous round's reads of xl are done
       if (act) F::template store<0>(v, t, [&](int idx, cf32 x) { xl[pad16(idx)] = x; });
@@ -708,20 +720,20 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   return BLINK_OK;
 }
 
-template <int N>
+template <int N, int NZ>
 static int launch_fused_n(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
   constexpr int THREADS = kFusedThreads;
   static thread_local size_t smem_set = 0;
   if (p->fused_smem > smem_set) {
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)p->fused_smem), "k_fused smem attribute");
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS>, cudaFuncAttributePreferredSharedMemoryCarveout, 100),
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS, NZ>, cudaFuncAttributePreferredSharedMemoryCarveout, 100),
                    "k_fused carveout");
     smem_set = p->fused_smem;
   }
   const int blocks = std::min(fp.n_snap, p->sm_count);
   if (blocks <= 0) return BLINK_OK;
-  k_fused<N, THREADS><<<blocks, THREADS, p->fused_smem, st>>>(fp);
+  k_fused<N, THREADS, NZ><<<blocks, THREADS, p->fused_smem, st>>>(fp);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_fused launch");
   return BLINK_OK;
 }
@@ -735,11 +747,18 @@ static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *
   fp.tab_stride = p->fused_tab_stride; fp.n_col = p->kx_max_all + 1; fp.h_max = p->h_max;
   fp.buf_bytes = p->fused_buf_bytes;
   fp.off_dedicated = p->fused_off_dedicated; fp.off_S = p->fused_off_S; fp.off_bar = p->fused_off_bar;
+  // band limit of the first transform stage, in units of N/16 cells
+  const int reach = std::max(p->kx_max_all, p->ky_max_all) + 1, T = p->n_pix / 16;
+  const int nz = (reach + T - 1) / T;
   switch (p->n_pix) {
-    case 32: return launch_fused_n<32>(p, fp, st);
-    case 64: return launch_fused_n<64>(p, fp, st);
-    case 128: return launch_fused_n<128>(p, fp, st);
-    case 256: return launch_fused_n<256>(p, fp, st);
+    case 32: return launch_fused_n<32, 8>(p, fp, st);
+    case 64: return launch_fused_n<64, 8>(p, fp, st);
+    case 128: return launch_fused_n<128, 8>(p, fp, st);
+    case 256:
+      if (nz <= 2) return launch_fused_n<256, 2>(p, fp, st);
+      if (nz <= 3) return launch_fused_n<256, 3>(p, fp, st);
+      if (nz <= 4) return launch_fused_n<256, 4>(p, fp, st);
+      return launch_fused_n<256, 8>(p, fp, st);
     default: return BLINK_EUNSUPPORTED;
   }
 }

@@ -87,6 +87,78 @@ template <> BLINK_HD void dft<4>(cf32 *v) { dft4(v[0], v[1], v[2], v[3]); }
 template <> BLINK_HD void dft<8>(cf32 *v) { dft8(v); }
 template <> BLINK_HD void dft<16>(cf32 *v) { dft16(v); }
 
+// ---- pruned butterflies: inputs known to be zero at compile time --------------------------------
+// dftp<R, M>(v) is dft<R>(v) for inputs whose bit in M is clear being zero (their v[] entries are
+// never read).  Decimation in time: the even- and odd-indexed inputs are transformed separately
+// with their own masks and combined; a half with no non-zero input costs nothing, and the other
+// half's outputs are then copied (or negated) instead of added.  Used for the first stage of the
+// image transforms, whose inputs vanish outside the plan's bounding box.
+template <int A> BLINK_HD cf32 mul_w16(cf32 x) {   // x * exp(+i pi A / 8), A = 0..7
+  if constexpr (A == 0) return x;
+  else if constexpr (A == 4) return mul_i(x);
+  else if constexpr (A == 2) return mk(BLINK_SQRT1_2 * (x.x - x.y), BLINK_SQRT1_2 * (x.x + x.y));
+  else if constexpr (A == 6) return mk(-BLINK_SQRT1_2 * (x.x + x.y), BLINK_SQRT1_2 * (x.x - x.y));
+  else if constexpr (A == 1) return cmul(x, mk(BLINK_COS_PI_8, BLINK_SIN_PI_8));
+  else if constexpr (A == 3) return cmul(x, mk(BLINK_SIN_PI_8, BLINK_COS_PI_8));
+  else if constexpr (A == 5) return cmul(x, mk(-BLINK_SIN_PI_8, BLINK_COS_PI_8));
+  else return cmul(x, mk(-BLINK_COS_PI_8, BLINK_SIN_PI_8));
+}
+
+constexpr unsigned prune_even(unsigned m, int r) {   // mask of the even-indexed inputs, compacted
+  unsigned o = 0;
+  for (int k = 0; k < r / 2; ++k) o |= ((m >> (2 * k)) & 1u) << k;
+  return o;
+}
+constexpr unsigned prune_odd(unsigned m, int r) { return prune_even(m >> 1, r); }
+
+template <int R, unsigned M> BLINK_HD void dftp(cf32 *v);
+
+template <int R, int K, bool HAS_E, bool HAS_O> struct PruneCombine {
+  BLINK_HD static void run(cf32 *v, const cf32 *e, const cf32 *o) {
+    if constexpr (K < R / 2) {
+      if constexpr (HAS_E && HAS_O) {
+        const cf32 t = mul_w16<K * (16 / R)>(o[K]);
+        v[K] = cadd(e[K], t);
+        v[K + R / 2] = csub(e[K], t);
+      } else if constexpr (HAS_E) {
+        v[K] = e[K];
+        v[K + R / 2] = e[K];
+      } else {
+        const cf32 t = mul_w16<K * (16 / R)>(o[K]);
+        v[K] = t;
+        v[K + R / 2] = mk(-t.x, -t.y);
+      }
+      PruneCombine<R, K + 1, HAS_E, HAS_O>::run(v, e, o);
+    }
+  }
+};
+
+template <int R, unsigned M> BLINK_HD void dftp(cf32 *v) {
+  static_assert(R == 1 || R == 2 || R == 4 || R == 8 || R == 16, "radix");
+  constexpr unsigned FULL = (1u << R) - 1u;
+  if constexpr (R == 1 || (M & FULL) == 0) {
+    return;
+  } else if constexpr ((M & FULL) == FULL) {
+    dft<R>(v);
+  } else {
+    constexpr unsigned EM = prune_even(M & FULL, R), OM = prune_odd(M & FULL, R);
+    cf32 e[R / 2], o[R / 2];
+#pragma unroll
+    for (int k = 0; k < R / 2; ++k) {
+      e[k] = ((EM >> k) & 1u) ? v[2 * k] : mk(0.f, 0.f);
+      o[k] = ((OM >> k) & 1u) ? v[2 * k + 1] : mk(0.f, 0.f);
+    }
+    dftp<R / 2, EM>(e);
+    dftp<R / 2, OM>(o);
+    PruneCombine<R, 0, EM != 0, OM != 0>::run(v, e, o);
+  }
+}
+
+// mask of a first-stage butterfly whose inputs r = NZ .. 15 - NZ are zero (band-limited line)
+template <int NZ> struct BandMask {
+  static constexpr unsigned value = NZ >= 8 ? 0xFFFFu : (((1u << NZ) - 1u) | (((1u << NZ) - 1u) << (16 - NZ)));
+};
+
 // ---- per-N stage plan ------------------------------------------------------------------------
 template <int N> struct Radices;
 template <> struct Radices<32>   { static constexpr int n = 2, r0 = 16, r1 = 2,  r2 = 1; };
@@ -153,6 +225,12 @@ template <int N> struct Fft {
       }
       dft<R>(x);
     }
+  }
+
+  // Stage 0 (no twiddles) with inputs r outside the mask M known to be zero; radix 16 only.
+  template <unsigned M> BLINK_HD static void compute0_pruned(cf32 *v) {
+    static_assert(RD::r0 == 16, "first stage is radix 16");
+    dftp<16, M>(v);
   }
 
   // The twiddles of butterfly j of stage S, w[r] = w_{Ns R}^{r k}, k = j mod Ns, each read straight
