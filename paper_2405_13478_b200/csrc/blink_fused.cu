@@ -149,6 +149,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   float2 *S = reinterpret_cast<float2 *>(smem_raw + p.off_S);                 // [n_can_max up to 16 | 16 sinks]
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + p.off_bar);        // [nbuf]
   uint64_t *empty = full + p.nbuf;                                            // [nbuf]
+  uint64_t *region_free = empty + p.nbuf;   // every warp has finished pass B: lines / exchange area reusable
   const uint32_t sm_base = smem_u32(smem_raw), S_base = sm_base + p.off_S;
   const int tid = threadIdx.x;
   const int warp = tid >> 5, lane = tid & 31;
@@ -161,6 +162,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   };
   uint32_t fphase = 0;                  // bit b: parity of the next wait on full[b]
   uint32_t ephase = 0;                  // producer only: bit b: parity of the last completed empty[b] phase
+  uint32_t rphase = 0;                  // producer only: parity of the next wait on region_free
   auto produce = [&](int s, int c, int b) {    // thread 0 only; b = c % nbuf
     mbar_wait(empty + b, ((ephase >> b) & 1u) ^ 1u);   // every warp has let go of the buffer
     ephase ^= 1u << b;
@@ -179,6 +181,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
       mbar_init(full + b, 1);
       mbar_init(empty + b, kFusedWarps);
     }
+    mbar_init(region_free, kFusedWarps);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   // S[0..n_can_max-1] cell sums; S[sink0 + b], b = 0..15: one always-zero slot per bank (sinks of
@@ -198,9 +201,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   for (int s = blockIdx.x; s < p.n_snap; s += gridDim.x) {
     const int ch = s % p.n_ch;
     const ChannelInfo ci = p.chinfo[ch];
-    // the lines / exchange area is idle until phase H: fill it with this snapshot's next chunks
-    if (tid == 0)
+    // the lines / exchange area is idle until phase H: fill it with this snapshot's next chunks, once
+    // every warp has left pass B of the previous snapshot (the other warps start on chunk 0 meanwhile)
+    if (tid == 0) {
+      if (s != (int)blockIdx.x) {
+        mbar_wait(region_free, rphase);
+        rphase ^= 1u;
+      }
       for (int c = 1; c < min(p.n_chunk, p.nbuf); ++c) produce(s, c, c);
+    }
 
     // phase-H records do not depend on the sums: request them now, they arrive during phase S
     uint2 hr[kHPer];
@@ -346,9 +355,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
       }
     }
     // generic-proxy writes to the lines / exchange area are ordered before the next snapshot's
-    // bulk copies into the same bytes
+    // bulk copies into the same bytes; no CTA-wide barrier: a warp that is done moves on to phase S
+    // of the next snapshot (its own cell sums, the dedicated buffer) while others finish pass B
     fence_async_smem();
-    __syncthreads();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(region_free);
   }
 }
 
@@ -523,7 +534,7 @@ int fused_setup(blink_plan *p) {
 //   [0, region)             column lines + pass-B exchange lines; doubles as chunk buffers 1..nbuf-1
 //   [off_dedicated, +B)     chunk buffer 0            (B = chunk_vis * 8 + tab_stride, 128-aligned)
 //   [off_S, ...)            canonical cell sums, sink, zero slot
-//   [off_bar, ...)          full[nbuf], empty[nbuf] mbarriers
+//   [off_bar, ...)          full[nbuf], empty[nbuf], region_free mbarriers
 int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st) {
   int want = 1;
   if (const char *e = getenv("BLINK_FUSED_SMEM")) want = atoi(e);
@@ -592,7 +603,7 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
     nbuf = 1 + (int)std::min<size_t>(7, region / buf_bytes);
     nbuf = std::min(nbuf, n_chunk);
     if (nbuf < 2 && n_chunk > 1) continue;             // the ring needs a second buffer
-    const size_t total = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 64;
+    const size_t total = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 8 + 64;
     if (total > limit || total > 0x7FFFu * 8u) continue;
     found = true;
     break;
@@ -607,7 +618,7 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   p->fused_off_dedicated = (uint32_t)region_al;
   p->fused_off_S = (uint32_t)(region_al + buf_bytes);      // multiple of 128: slot s of S sits in bank s mod 16
   p->fused_off_bar = (uint32_t)(region_al + buf_bytes + s_bytes);
-  p->fused_smem = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 16;
+  p->fused_smem = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 8 + 16;
   p->fused_threads = kFusedThreads;
   if (getenv("BLINK_DEBUG")) {
     long rows = 0, hw = 0, groups = 0, rmw = 0;
