@@ -184,6 +184,22 @@ int blink_plan_reserve(blink_plan *plan, int n_t);
 int blink_host_build_gather(const int32_t *cell, int n_bl, int n_pix, int32_t *n_can_out,
                             int32_t *can_cell, int32_t *seg_start, int32_t *src);
 
+/*
+ * Host emulation of the gridding phase of blink_grid_image's shared-memory route (steps a1/a2,
+ * PAPER.md:348-370), exported so its plan tables are testable without a GPU.  For ONE channel it
+ * builds the gather tables the kernel streams through shared memory -- cells owned by warps,
+ * baselines taken in chunks of chunk_vis (even, <= 32766), groups of 32 lanes x at most 4 rows --
+ * and walks them over a host model of shared memory exactly as a warp does.
+ *   cell       HOST int32 [n_bl], -1 = dropped (BLINK_Q_CELL_IDX of the channel)
+ *   vis        HOST complex64 [n_bl] (interleaved floats)
+ *   sums       HOST complex64 [n_can] out: per canonical cell (blink_host_build_gather's order) the
+ *              sum of V (or conj V) over its baselines, fp32, in the kernel's summation order
+ *   stats      HOST int32 [3] out (may be NULL): n_can, groups, rows over all chunks
+ * Returns 0 or a negative blink_status.
+ */
+int blink_host_fused_emulate(const int32_t *cell, int n_bl, int n_pix, int chunk_vis, const float *vis,
+                             float *sums, int32_t *stats);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,7 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create",
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
            "blink_grid", "blink_grid_image",
-           "blink_image", "blink_host_build_gather"]
+           "blink_image", "blink_host_build_gather", "blink_host_fused_emulate"]
 
 _lib = None
 
@@ -68,6 +68,8 @@ def load() -> ctypes.CDLL:
     lib.blink_grid_image.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_host_build_gather.restype = ci
     lib.blink_host_build_gather.argtypes = [vp, ci, ci, vp, vp, vp, vp]
+    lib.blink_host_fused_emulate.restype = ci
+    lib.blink_host_fused_emulate.argtypes = [vp, ci, ci, ci, vp, vp, vp]
     _lib = lib
     return lib
 
@@ -98,6 +100,21 @@ def host_build_gather(cell: np.ndarray, n_pix: int):
         raise BlinkError(rc, "blink_host_build_gather")
     n = n_can.value
     return dict(n_kept=rc, n_can=n, can_cell=can_cell[:n], seg_start=seg[:n + 1], src=src[:rc])
+
+
+def host_fused_emulate(cell: np.ndarray, n_pix: int, chunk_vis: int, vis: np.ndarray):
+    """blink_host_fused_emulate: phase S of the shared-memory route walked on the host (no GPU)."""
+    lib = load()
+    cell = np.ascontiguousarray(cell, np.int32)
+    vis = np.ascontiguousarray(vis, np.complex64)
+    n_bl = cell.shape[0]
+    sums = np.zeros(max(n_bl, 1), np.complex64)
+    stats = np.zeros(3, np.int32)
+    rc = lib.blink_host_fused_emulate(cell.ctypes.data, n_bl, int(n_pix), int(chunk_vis), vis.ctypes.data,
+                                      sums.ctypes.data, stats.ctypes.data)
+    if rc < 0:
+        raise BlinkError(rc, "blink_host_fused_emulate")
+    return dict(sums=sums[:stats[0]], n_can=int(stats[0]), groups=int(stats[1]), rows=int(stats[2]))
 
 
 class Plan:

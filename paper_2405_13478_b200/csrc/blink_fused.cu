@@ -386,7 +386,10 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
 struct AbstractTable {           // entries still relative to the chunk: (bl - lo) | conj << 15, 0x7FFF = padding
   std::vector<unsigned char> bytes;
   long rows = 0, halfrow_wavefronts = 0, groups = 0, rmw_wavefronts = 0;   // statistics
+  long warp_cost[16] = {};       // estimated issue slots per warp (see fused_build's rebalancing)
 };
+
+constexpr int kGroupCost = 22, kRowCost = 8;   // instructions per group / per row of phase S (from the SASS)
 
 struct FusedPiece { int32_t len, slot, first; };   // first: index into HostGather::src
 
@@ -490,6 +493,7 @@ static void build_chunk_table(const HostGather &g, const std::vector<int> &owner
       uint16_t *rows = reinterpret_cast<uint16_t *>(o.data() + base);
       out.groups++;
       out.rows += G.L;
+      out.warp_cost[w] += kGroupCost + kRowCost * G.L;
       for (int h = 0; h < 2; ++h) {
         int mx = 1;
         for (int bk = 0; bk < 16; ++bk) mx = std::max(mx, G.scount[h][bk]);
@@ -522,6 +526,63 @@ static void build_chunk_table(const HostGather &g, const std::vector<int> &owner
   o.resize((o.size() + 15) / 16 * 16, 0);
 }
 
+// cell -> warp: longest first to the least loaded warp; the cells of a warp get consecutive slots
+// of S in that order, so their banks cycle
+static void assign_cells(const HostGather &g, std::vector<int> &owner, std::vector<int> &slot) {
+  std::vector<int> order(g.n_can);
+  for (int j = 0; j < g.n_can; ++j) order[j] = j;
+  auto len = [&](int j) { return g.seg_start[j + 1] - g.seg_start[j]; };
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len(a) > len(b); });
+  std::vector<long> load(kFusedWarps, 0);
+  static const int w0bias = getenv("BLINK_FUSED_W0BIAS") ? atoi(getenv("BLINK_FUSED_W0BIAS")) : 4;
+  load[0] = (long)g.n_kept * w0bias / (100 * kFusedWarps);     // warp 0 also runs the chunk ring (thread 0)
+  owner.assign(g.n_can, 0);
+  for (int j : order) {
+    const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+    owner[j] = w;
+    load[w] += len(j) + 2;            // + the cost of folding the group sum into S[j]
+  }
+  slot.assign(g.n_can, 0);
+  int next = 0;
+  for (int w = 0; w < kFusedWarps; ++w)
+    for (int j : order)
+      if (owner[j] == w) slot[j] = next++;
+}
+
+// relative entries -> shared-memory slots of the buffer the chunk will land in (base_slot, in
+// 8-byte units); a padded entry reads the zero slot of a bank that the real entries of its
+// half-row leave free (zero slots: S[sink0 + b], S starting at slot s_slot0)
+static void finalize_chunk_table(std::vector<unsigned char> &b, uint32_t base_slot, uint32_t s_slot0, int sink0) {
+  for (int w = 0; w < kFusedWarps; ++w) {
+    uint32_t off, lseq;
+    std::memcpy(&off, b.data() + 8 * w, 4);
+    std::memcpy(&lseq, b.data() + 8 * w + 4, 4);
+    size_t blk = off & 0xFFFFFFu;
+    for (int gi = (int)(off >> 24); gi > 0; --gi, lseq >>= 2) {
+      const int L = (int)(lseq & 3u) + 1;
+      uint16_t *rows = reinterpret_cast<uint16_t *>(b.data() + blk);
+      for (int r = 1; r <= L; ++r)
+        for (int half = 0; half < 2; ++half) {
+          uint16_t *e = rows + (size_t)r * 32 + half * 16;
+          uint32_t used = 0;
+          for (int l = 0; l < 16; ++l)
+            if ((e[l] & 0x7FFFu) != 0x7FFFu) {
+              const uint32_t sl = base_slot + (e[l] & 0x7FFFu);
+              e[l] = (uint16_t)(sl | (e[l] & 0x8000u));
+              used |= 1u << (sl & 15);
+            } else {
+              e[l] = 0xFFFFu;                                             // marks padding until the bank is chosen
+            }
+          int free_bank = 0;
+          while (free_bank < 15 && (used >> free_bank & 1u)) ++free_bank;
+          for (int l = 0; l < 16; ++l)
+            if (e[l] == 0xFFFFu) e[l] = (uint16_t)(s_slot0 + sink0 + ((free_bank - (int)s_slot0) & 15));
+        }
+      blk += (size_t)(L + 1) * 64;
+    }
+  }
+}
+
 int fused_setup(blink_plan *p) {
   p->fused_path = 0;
   p->fused_chunk = p->chunk_snapshots;   // the two-kernel route chunks like blink_image
@@ -552,30 +613,8 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   const size_t s_bytes = sizeof(float2) * (size_t)n_S;
   const size_t limit = (size_t)p->max_smem_optin;
 
-  // cell -> warp, per channel: longest first to the least loaded warp; the cells of a warp get
-  // consecutive slots of S in that order, so their banks cycle
   std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
-  for (int ch = 0; ch < n_ch; ++ch) {
-    const HostGather &g = gathers[ch];
-    std::vector<int> order(g.n_can);
-    for (int j = 0; j < g.n_can; ++j) order[j] = j;
-    auto len = [&](int j) { return g.seg_start[j + 1] - g.seg_start[j]; };
-    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len(a) > len(b); });
-    std::vector<long> load(kFusedWarps, 0);
-    static const int w0bias = getenv("BLINK_FUSED_W0BIAS") ? atoi(getenv("BLINK_FUSED_W0BIAS")) : 4;
-    load[0] = (long)g.n_kept * w0bias / (100 * kFusedWarps);     // warp 0 also runs the chunk ring (thread 0)
-    owner[ch].assign(g.n_can, 0);
-    for (int j : order) {
-      const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
-      owner[ch][j] = w;
-      load[w] += len(j) + 2;            // + the cost of folding the group sum into S[j]
-    }
-    slot[ch].assign(g.n_can, 0);
-    int next = 0;
-    for (int w = 0; w < kFusedWarps; ++w)
-      for (int j : order)
-        if (owner[ch][j] == w) slot[ch][j] = next++;
-  }
+  for (int ch = 0; ch < n_ch; ++ch) assign_cells(gathers[ch], owner[ch], slot[ch]);
 
   int force_chunks = 0;
   if (const char *e = getenv("BLINK_FUSED_CHUNKS")) force_chunks = atoi(e);
@@ -623,14 +662,21 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   if (getenv("BLINK_DEBUG")) {
     long rows = 0, hw = 0, groups = 0, rmw = 0;
     for (const AbstractTable &t : tabs) { rows += t.rows; hw += t.halfrow_wavefronts; groups += t.groups; rmw += t.rmw_wavefronts; }
+    double worst = 0;
+    for (int ch = 0; ch < n_ch; ++ch) {
+      long wc[kFusedWarps] = {}, tot = 0, mx = 0;
+      for (int c = 0; c < n_chunk; ++c)
+        for (int w = 0; w < kFusedWarps; ++w) wc[w] += tabs[(size_t)ch * n_chunk + c].warp_cost[w];
+      for (int w = 0; w < kFusedWarps; ++w) { tot += wc[w]; mx = std::max(mx, wc[w]); }
+      worst = std::max(worst, (double)mx * kFusedWarps / std::max(tot, 1L));
+    }
+    fprintf(stderr, "  phase S warp imbalance (max / mean of the estimated cost), worst channel: %.3f\n", worst);
     fprintf(stderr, "blink fused route: %d chunks of %d baselines, table stride %zu B, buffer %zu B x %d, smem %zu B\n"
             "  per snapshot: %.0f groups, %.0f rows (ideal %.0f), %.2f wavefronts per half-row, %.2f per half cell-sum access\n",
             n_chunk, C, tab_stride, buf_bytes, nbuf, p->fused_smem, (double)groups / n_ch, (double)rows / n_ch,
             (double)n_bl / 32, (double)hw / (2.0 * std::max(rows, 1L)), (double)rmw / (2.0 * std::max(groups, 1L)));
   }
 
-  // relative entries -> shared-memory slots of the buffer the chunk will land in; a padded entry
-  // reads the zero slot of a bank that the real entries of its half-row leave free
   const uint32_t s_slot0 = p->fused_off_S / 8;
   std::vector<unsigned char> h_tab((size_t)n_ch * n_chunk * tab_stride, 0);
   std::vector<uint32_t> h_size((size_t)n_ch * n_chunk, 0);
@@ -640,34 +686,7 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
       std::vector<unsigned char> &b = tabs[cp].bytes;
       const int bi = c % nbuf;
       const uint32_t base_slot = (uint32_t)((bi == 0 ? p->fused_off_dedicated : (uint32_t)(bi - 1) * p->fused_buf_bytes) / 8);
-      for (int w = 0; w < kFusedWarps; ++w) {
-        uint32_t off, lseq;
-        std::memcpy(&off, b.data() + 8 * w, 4);
-        std::memcpy(&lseq, b.data() + 8 * w + 4, 4);
-        size_t blk = off & 0xFFFFFFu;
-        for (int gi = (int)(off >> 24); gi > 0; --gi, lseq >>= 2) {
-            const int L = (int)(lseq & 3u) + 1;
-            uint16_t *rows = reinterpret_cast<uint16_t *>(b.data() + blk);
-            for (int r = 1; r <= L; ++r)
-              for (int half = 0; half < 2; ++half) {
-                uint16_t *e = rows + (size_t)r * 32 + half * 16;
-                uint32_t used = 0;
-                for (int l = 0; l < 16; ++l)
-                  if ((e[l] & 0x7FFFu) != 0x7FFFu) {
-                    const uint32_t sl = base_slot + (e[l] & 0x7FFFu);
-                    e[l] = (uint16_t)(sl | (e[l] & 0x8000u));
-                    used |= 1u << (sl & 15);
-                  } else {
-                    e[l] = 0xFFFFu;                                             // marks padding until the bank is chosen
-                  }
-                int free_bank = 0;
-                while (free_bank < 15 && (used >> free_bank & 1u)) ++free_bank;
-                for (int l = 0; l < 16; ++l)
-                  if (e[l] == 0xFFFFu) e[l] = (uint16_t)(s_slot0 + sink0 + ((free_bank - (int)s_slot0) & 15));
-              }
-            blk += (size_t)(L + 1) * 64;
-          }
-      }
+      finalize_chunk_table(b, base_slot, s_slot0, sink0);
       std::memcpy(h_tab.data() + cp * tab_stride, b.data(), b.size());
       h_size[cp] = (uint32_t)b.size();
     }
@@ -792,4 +811,66 @@ extern "C" int blink_grid_image(const blink_plan *plan, const void *vis, int n_t
   int rc = blink::image_reserve(mp, n_t);
   if (rc != BLINK_OK) return rc;
   return blink::launch_grid_image(plan, (const float2 *)vis, n_t, (float *)images, (cudaStream_t)stream);
+}
+
+// Host emulation of phase S of k_fused for ONE channel (tests without a GPU): builds the gather
+// tables exactly as fused_build does for chunks of chunk_vis baselines, then walks them the way a
+// warp does over a byte-for-byte model of shared memory.
+extern "C" int blink_host_fused_emulate(const int32_t *cell, int n_bl, int n_pix, int chunk_vis,
+                                        const float *vis, float *sums, int32_t *stats) {
+  using namespace blink;
+  if (!cell || !vis || !sums || n_bl < 1 || chunk_vis < 2 || (chunk_vis & 1) || chunk_vis > 0x7FFE) return BLINK_EINVAL;
+  HostGather g;
+  int rc = build_gather_host(cell, n_bl, n_pix, g);
+  if (rc != BLINK_OK) return rc;
+  std::vector<int> owner, slot;
+  assign_cells(g, owner, slot);
+  const int sink0 = (g.n_can + 15) & ~15, n_S = sink0 + 16;
+  const uint32_t s_slot0 = (uint32_t)((chunk_vis + 15) & ~15);        // S right after the chunk buffer
+  if (s_slot0 + (uint32_t)n_S > 0x7FFFu) return BLINK_EUNSUPPORTED;
+  std::vector<float> sm(2 * (size_t)(s_slot0 + n_S), 0.f);           // shared memory as float2 slots
+  long groups = 0, rows = 0;
+  for (int lo = 0; lo < n_bl; lo += chunk_vis) {
+    const int hi = std::min(n_bl, lo + chunk_vis);
+    AbstractTable t;
+    bool ok = true;
+    build_chunk_table(g, owner, slot, lo, hi, sink0, t, ok);
+    if (!ok) return BLINK_EUNSUPPORTED;
+    finalize_chunk_table(t.bytes, 0u, s_slot0, sink0);
+    groups += t.groups;
+    rows += t.rows;
+    std::memcpy(sm.data(), vis + 2 * (size_t)lo, sizeof(float) * 2 * (size_t)(hi - lo));
+    const unsigned char *tab = t.bytes.data();
+    for (int w = 0; w < kFusedWarps; ++w) {
+      uint32_t wx, lseq;
+      std::memcpy(&wx, tab + 8 * w, 4);
+      std::memcpy(&lseq, tab + 8 * w + 4, 4);
+      size_t blk = wx & 0xFFFFFFu;
+      for (int n = (int)(wx >> 24); n > 0; --n, lseq >>= 2) {
+        const int L = (int)(lseq & 3u) + 1;
+        const uint16_t *row = reinterpret_cast<const uint16_t *>(tab + blk);
+        for (int lane = 0; lane < 32; ++lane) {
+          float ax = 0.f, ay = 0.f;
+          for (int r = 0; r < L; ++r) {
+            const uint16_t e = row[(size_t)(r + 1) * 32 + lane];
+            const float vx = sm[2 * (size_t)(e & 0x7FFF)], vy = sm[2 * (size_t)(e & 0x7FFF) + 1];
+            if (r == 0) { ax = vx; ay = (e & 0x8000) ? -vy : vy; }
+            else { ax += vx; ay += (e & 0x8000) ? -vy : vy; }
+          }
+          const size_t sj = 2 * ((size_t)s_slot0 + row[lane]);
+          sm[sj] += ax;
+          sm[sj + 1] += ay;
+        }
+        blk += (size_t)(L + 1) * 64;
+      }
+    }
+  }
+  for (int j = 0; j < g.n_can; ++j) {
+    sums[2 * j] = sm[2 * ((size_t)s_slot0 + slot[j])];
+    sums[2 * j + 1] = sm[2 * ((size_t)s_slot0 + slot[j]) + 1];
+  }
+  for (int b = 0; b < 16; ++b)                      // the zero slots must still be zero
+    if (sm[2 * ((size_t)s_slot0 + sink0 + b)] != 0.f || sm[2 * ((size_t)s_slot0 + sink0 + b) + 1] != 0.f) return BLINK_EINVAL;
+  if (stats) { stats[0] = g.n_can; stats[1] = (int32_t)groups; stats[2] = (int32_t)rows; }
+  return BLINK_OK;
 }

@@ -89,6 +89,27 @@ def test_host_gather_tables_reproduce_oracle_grid(blink, oracle, cfg):
     assert np.allclose(2 * sums[dc].real, ref[dc].real, rtol=1e-12, atol=1e-12)
 
 
+@pytest.mark.parametrize("cfg,chunk", [("tiny", 62), ("tiny", 496), ("station", 4664), ("station", 32640 // 4)])
+def test_fused_gather_tables_on_host(blink, oracle, cfg, chunk):
+    """The shared-memory route's phase-S tables (warp-owned cells, chunks, groups of 32 lanes x <= 4
+    rows, zero-slot padding), walked on the host the way a warp walks them, give every canonical
+    cell's sum -- against numpy's per-segment sums of the same visibilities."""
+    w = {"tiny": synth.config_tiny, "station": lambda: synth.config_station(n_t=1, n_ch=1)}[cfg]()
+    n = w.n_pix
+    r = oracle.uv_cells(w.ant_enu_m, w.freq_hz[0], n, w.pixscale)
+    g = blink.host_build_gather(r["cell"], n)
+    vis = w.vis()[0, 0]
+    out = blink.host_fused_emulate(r["cell"], n, chunk, vis)
+    assert out["n_can"] == g["n_can"]
+    bl = g["src"] >> 1
+    val = np.where(g["src"] & 1, np.conj(vis[bl]), vis[bl]).astype(np.complex128)
+    ref = np.add.reduceat(val, g["seg_start"][:-1])
+    scale = np.max(np.abs(ref))
+    assert np.max(np.abs(out["sums"] - ref)) <= 1e-5 * scale
+    # every baseline is read exactly once: rows x 32 lanes >= kept baselines, groups cover the cells
+    assert out["rows"] * 32 >= g["n_kept"] and out["groups"] * 32 >= g["n_can"]
+
+
 def test_fft_stage_algebra_on_host(tmp_path):
     exe = str(tmp_path / "host_fft_check")
     subprocess.run(["g++", "-O1", "-std=c++17", os.path.join(ROOT, "tests", "host_fft_check.cpp"),
