@@ -46,6 +46,11 @@ def algorithmic_bytes(w):
     return dict(grid=8 * w.n_bl + 8 * nn, image=12 * nn, step=8 * w.n_bl + 20 * nn)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch at the bench's own
+# size, from `ncu --set full` captures (profiles/r01_README.md); None where no capture exists
+NCU_TRAFFIC_BYTES = {("station", "fused", 100): 848_063_232 + 784_796_416}
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -321,7 +326,8 @@ def main():
         "path": args.path, "per_call_ms": {k: v[0] for k, v in calls.items()},
         "images_per_s_vs_sep_roofline": value / (peak * 1e9 / (8 * w.n_bl + 20 * w.n_pix * w.n_pix)),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "frac": achieved / peak,
+                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.path, w.n_t)), "peak_source": peak_src,
                      "algorithmic_bytes_per_snapshot": calls[dom][1]},
         "roofline_step": {"bound": "hbm", "achieved": step_gbs, "peak": peak, "unit": "GB/s",
                           "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": ab["step"]},
