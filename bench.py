@@ -317,6 +317,18 @@ def main():
             launches_per_step = 2 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))
     else:
         launches_per_step = 1 + 2 * chunks
+    # side bound: fp32 work of the Hermitian two-pass transform + the gridding adds,
+    # against the rate the unit counts give (148 SMs x 128 lanes x SM clock, no FMA); DESIGN.md 7
+    import math
+    kxm = max(plan.bbox(c)[0] for c in range(w.n_ch))
+    flops = 5.0 * w.n_pix * math.log2(w.n_pix) * ((kxm + 1) + w.n_pix / 2) + 4.0 * w.n_bl
+    fp32_rate = 148 * 128 * 1.965e9
+    t_alu_us, t_hbm_us = flops / fp32_rate * 1e6, ab["step"] / (peak * 1e9) * 1e6
+    t_meas_us = ms_per_step * 1e3 / n_snap
+    side = {"hbm_us_per_snapshot": t_hbm_us, "alu_us_per_snapshot": t_alu_us,
+            "measured_us_per_snapshot": t_meas_us, "binding": "alu" if t_alu_us > t_hbm_us else "hbm",
+            "frac_of_binding": max(t_alu_us, t_hbm_us) / t_meas_us,
+            "flops_per_snapshot": flops, "fp32_rate_no_fma": fp32_rate}
     out = {
         "metric": "dirty_images_per_s", "value": value, "unit": "images/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
@@ -331,7 +343,7 @@ def main():
                      "algorithmic_bytes_per_snapshot": calls[dom][1]},
         "roofline_step": {"bound": "hbm", "achieved": step_gbs, "peak": peak, "unit": "GB/s",
                           "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": ab["step"]},
-        "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
+        "side_bounds": side, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
     }
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, args)

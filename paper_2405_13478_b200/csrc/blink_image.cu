@@ -41,7 +41,7 @@ struct ImgParams {
   const int32_t *src, *vkey, *vseg, *vlen, *vcol;
   const float *vw;
   const float2 *tw;
-  int n_ch, n_bl, wu, uniform, snap_base, ch0;
+  int n_ch, n_bl, wu, uniform, snap_base, ch0, direct_max;
 };
 
 // run stages 1.. of the transform; stage 0's load is done by the caller
@@ -152,6 +152,66 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_cols_from_vis(const ImgParams
   const int kx0 = blockIdx.x * CT;
   const int32_t *__restrict__ vcol = p.vcol + (size_t)ch * (p.wu + 1);
   const int e0 = vcol[kx0], e1 = vcol[min(kx0 + CT, p.wu)];
+  // Sparse tiles: when none of the CT columns holds more than direct_max occupied cells, the
+  // column transforms are cheaper as direct sums U[y] = sum_cells H exp(+2 pi i ky y / N).  One
+  // column per W warps; a lane owns 16 outputs y = y0 + 32 i and steps its twiddle by w^(32 ky).
+  constexpr int W = THREADS / 32 / CT;            // warps per column (N / 512)
+  if constexpr (W >= 1) {
+    int nmax = 0;
+#pragma unroll
+    for (int c = 0; c < CT; ++c) nmax = max(nmax, __ldg(vcol + kx0 + c + 1) - __ldg(vcol + kx0 + c));
+    if (nmax <= p.direct_max) {
+      const int wv = tid >> 5, lane = tid & 31, c = wv % CT, part = wv / CT;
+      const int c0 = __ldg(vcol + kx0 + c), n_c = __ldg(vcol + kx0 + c + 1) - c0;
+      const size_t tb = (size_t)ch * 2 * p.n_bl;
+      cf32 val = mk(0.f, 0.f);
+      int iy = 0;
+      if (lane < n_c) {                            // lane l forms the l-th cell of the column
+        const int e = c0 + lane;
+        const float2 *__restrict__ vis = p.vis + (size_t)s * p.n_bl;
+        const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
+        const int st = __ldg(p.vseg + tb + e), lf = __ldg(p.vlen + tb + e);
+        const float w = __ldg(p.vw + tb + e);
+        iy = __ldg(p.vkey + tb + e) & 0xffff;
+        const int len = lf & 0xFFFFFF, flag = lf >> 24;
+        float ar = 0.f, ai = 0.f;
+        for (int q = st; q < st + len; ++q) {
+          const int code = __ldg(src + q);
+          const float2 v = __ldg(vis + (code >> 1));
+          ar += v.x;
+          ai += (code & 1) ? -v.y : v.y;
+        }
+        if (flag == kPlaceDirect) val = mk(ar * w, ai * w);
+        else if (flag == kPlaceConj) val = mk(ar * w, -ai * w);
+        else val = mk((ar + ar) * w, 0.f);
+      }
+      const int y0 = part * (N / W) + lane;
+      cf32 acc[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) acc[i] = mk(0.f, 0.f);
+      for (int k = 0; k < n_c; ++k) {
+        const cf32 vk = mk(__shfl_sync(0xffffffffu, val.x, k), __shfl_sync(0xffffffffu, val.y, k));
+        const int ik = __shfl_sync(0xffffffffu, iy, k);
+        const cf32 step = __ldg(p.tw + ((ik * 32) & (N - 1)));
+        cf32 t = cmul(vk, __ldg(p.tw + ((ik * y0) & (N - 1))));
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          acc[i] = cadd(acc[i], t);
+          t = cmul(t, step);
+        }
+      }
+      cf32 *line = lines + c * C::LS;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) line[pad16(y0 + 32 * i)] = acc[i];
+      __syncthreads();
+      float2 *__restrict__ U = p.U + (size_t)sl * N * p.wu + kx0;
+      for (int idx = tid; idx < CT * N; idx += THREADS) {
+        const int cc = idx % CT, y = idx / CT;
+        U[(size_t)y * p.wu + cc] = lines[cc * C::LS + pad16(y)];
+      }
+      return;
+    }
+  }
   for (int i = tid; i < CT * C::LS; i += THREADS) lines[i] = mk(0.f, 0.f);
   __syncthreads();
   {
@@ -328,6 +388,8 @@ static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2
   ip.tw = p->d_tw; ip.n_ch = p->n_ch; ip.wu = p->wu; ip.uniform = p->weighting == BLINK_UNIFORM;
   ip.snap_base = 0;
   ip.ch0 = ch0;
+  ip.direct_max = 12;
+  if (const char *e = getenv("BLINK_IMAGE_DIRECT")) ip.direct_max = std::min(32, std::max(0, atoi(e)));
   switch (p->n_pix) {
     case 32: return run_image_n<32>(p, ip, n_snap, st);
     case 64: return run_image_n<64>(p, ip, n_snap, st);
