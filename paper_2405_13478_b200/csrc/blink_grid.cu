@@ -21,8 +21,10 @@
 // One CTA works on one (snapshot, part) item at a time and strides over items (persistent grid),
 // "part" splitting a snapshot's bands when there are few snapshots.
 #include <algorithm>
+#include <cstdio>
 
 #include "blink_internal.h"
+#include "sgather.cuh"
 #include "sphase.cuh"
 
 namespace blink {
@@ -122,6 +124,267 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Ring route (small grids, many snapshots): phase S as in k_fused (blink_fused.cu, sgather.cuh) --
+// the snapshot's visibilities stream through a ring of shared-memory buffers by bulk copies, each
+// chunk with its gather table; cells are owned by warps, sums need no atomics and no barrier between
+// chunks -- and because nothing else needs the shared memory here, the ring runs ahead across
+// snapshots without ever draining.  Phase P as above: bulk zero fill, then the occupied cells.
+struct GridRingParams {
+  const float2 *vis;
+  float2 *uv;
+  const ChannelInfo *chinfo;
+  const unsigned char *rtab;   // [n_ch][n_chunk][tab_stride]
+  const uint32_t *rsize;       // [n_ch][n_chunk]
+  const int2 *rplace;          // [n_ch][2 n_bl] {cell, slot | flag << 30}
+  int n_bl, n_ch, n_snap, n_can_max, n_chunk, chunk_vis, nbuf, tab_stride, n_bands, band_cells, ch0;
+  uint32_t buf_bytes, off_buf, off_S, off_bar;
+  long long grid_cells;
+};
+
+constexpr int kRingPlacePf = 10;   // placement records fetched per thread ahead of the barrier
+
+__global__ void __launch_bounds__(kFusedThreads, 1) k_grid_ring(const GridRingParams p) {
+  constexpr int THREADS = kFusedThreads;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  float2 *zero = reinterpret_cast<float2 *>(smem_raw);                        // [band_cells]
+  float2 *S = reinterpret_cast<float2 *>(smem_raw + p.off_S);
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + p.off_bar);
+  uint64_t *empty = full + p.nbuf;
+  const uint32_t sm_base = smem_u32(smem_raw), S_base = sm_base + p.off_S;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t vis_bytes = (uint32_t)p.chunk_vis * sizeof(float2);
+  const uint32_t band_bytes = (uint32_t)p.band_cells * sizeof(float2);
+  const int n_S = ((p.n_can_max + 15) & ~15) + 16;
+
+  if (tid == 0) {
+    for (int b = 0; b < p.nbuf; ++b) {
+      mbar_init(full + b, 1);
+      mbar_init(empty + b, kFusedWarps);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  {
+    float4 *z4 = reinterpret_cast<float4 *>(smem_raw);
+    for (int i = tid; i < p.band_cells / 2; i += THREADS) z4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  for (int j = tid; j < n_S; j += THREADS) S[j] = make_float2(0.f, 0.f);
+  fence_async_smem();
+  __syncthreads();
+
+  // this CTA's snapshots: s = blockIdx.x + k gridDim.x, k < K; their chunks form one sequence q
+  const int K = (p.n_snap - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int Q = K * p.n_chunk;
+  uint32_t fphase = 0, ephase = 0;
+  int pq = 0, pk = 0, pc = 0, pb = 0;        // producer (thread 0): next chunk to request
+  auto produce = [&]() {
+    mbar_wait(empty + pb, ((ephase >> pb) & 1u) ^ 1u);
+    ephase ^= 1u << pb;
+    const int s = (int)blockIdx.x + pk * (int)gridDim.x;
+    const int cnt = min(p.chunk_vis, p.n_bl - pc * p.chunk_vis);
+    const uint32_t vb = (uint32_t)cnt * sizeof(float2);
+    const size_t cp = (size_t)((s + p.ch0) % p.n_ch) * p.n_chunk + pc;
+    const uint32_t tb = __ldg(p.rsize + cp);
+    unsigned char *dst = smem_raw + p.off_buf + (size_t)pb * p.buf_bytes;
+    mbar_expect_tx(full + pb, vb + tb);
+    bulk_load(dst, p.vis + (size_t)s * p.n_bl + (size_t)pc * p.chunk_vis, vb, full + pb);
+    bulk_load(dst + vis_bytes, p.rtab + cp * p.tab_stride, tb, full + pb);
+    ++pq;
+    if (++pc == p.n_chunk) { pc = 0; ++pk; }
+    if (++pb == p.nbuf) pb = 0;
+  };
+  if (tid == 0)
+    while (pq < min(p.nbuf, Q)) produce();
+
+  int b = 0, q = 0;
+  for (int k = 0; k < K; ++k) {
+    const int s = (int)blockIdx.x + k * (int)gridDim.x;
+    const int ch = (s + p.ch0) % p.n_ch;
+    float2 *__restrict__ grid = p.uv + (size_t)s * p.grid_cells;
+    // ---- phase P, first half: zero-fill the snapshot; drains while phase S runs ----------------
+    if (tid == 0) {
+      for (int bd = 0; bd < p.n_bands; ++bd) bulk_store(grid + (size_t)bd * p.band_cells, zero, band_bytes);
+      bulk_commit();
+    }
+    const int n_place = p.chinfo[ch].n_place;
+    const int2 *__restrict__ place = p.rplace + (size_t)ch * 2 * p.n_bl;
+    int2 pr[kRingPlacePf];
+#pragma unroll
+    for (int i = 0; i < kRingPlacePf; ++i) {
+      const int e = tid + i * THREADS;
+      pr[i] = e < n_place ? __ldg(place + e) : make_int2(-1, 0);
+    }
+    // ---- phase S ----------------------------------------------------------------------------
+    for (int c = 0; c < p.n_chunk; ++c, ++q) {
+      mbar_wait(full + b, (fphase >> b) & 1u);
+      fphase ^= 1u << b;
+      consume_chunk(sm_base + p.off_buf + (uint32_t)b * p.buf_bytes + vis_bytes, warp, lane, sm_base, S_base);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + b);
+      if (tid == 0 && pq < Q) produce();     // chunk q + nbuf into the buffer just released
+      if (++b == p.nbuf) b = 0;
+    }
+    if (tid == 0) bulk_wait_all();            // the zero fill has landed
+    __syncthreads();
+    // ---- phase P, second half: occupied cells on top of the zeros -----------------------------
+    auto put = [&](int2 r) {
+      if (r.x < 0) return;
+      const float2 v = S[r.y & 0x3FFFFFFF];
+      const uint32_t flag = (uint32_t)r.y >> 30;
+      float2 o;
+      if (flag == kPlaceDirect) o = v;
+      else if (flag == kPlaceConj) o = make_float2(v.x, -v.y);
+      else o = make_float2(v.x + v.x, 0.f);
+      grid[r.x] = o;
+    };
+#pragma unroll
+    for (int i = 0; i < kRingPlacePf; ++i) put(pr[i]);
+    for (int e = tid + kRingPlacePf * THREADS; e < n_place; e += THREADS) put(__ldg(place + e));
+    __syncthreads();
+    for (int j = tid; j < p.n_can_max; j += THREADS) S[j] = make_float2(0.f, 0.f);
+    __syncthreads();
+  }
+}
+
+
+// Shared-memory plan and tables of the ring route.  Layout (bytes):
+//   [0, band)               zero band (source of the bulk zero fill)
+//   [off_buf, +nbuf * B)    chunk buffers (B = chunk_vis * 8 + tab_stride, 128-aligned)
+//   [off_S, ...)            canonical cell sums + 16 zero slots
+//   [off_bar, ...)          full[nbuf], empty[nbuf] mbarriers
+// n_chunk is a multiple of nbuf, so chunk c of every snapshot lands in buffer c % nbuf and the ring
+// never has to drain between snapshots.
+int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st) {
+  p->ring_path = 0;
+  int want = 1;
+  if (const char *e = getenv("BLINK_GRID_RING")) want = atoi(e);
+  const int N = p->n_pix, n_bl = p->n_bl, n_ch = p->n_ch;
+  if (!want || N > 512 || (n_bl & 1) || p->max_smem_optin <= 0 || p->n_can_max < 1) return BLINK_OK;
+  const int sink0 = (p->n_can_max + 15) & ~15, n_S = sink0 + 16;
+  if (n_S > 0x7FFF) return BLINK_OK;
+  const size_t band = (sizeof(float2) * (size_t)p->band_cells + 127) / 128 * 128;
+  const size_t s_bytes = (sizeof(float2) * (size_t)n_S + 127) / 128 * 128;
+  const size_t limit = (size_t)p->max_smem_optin;
+  if (band + s_bytes + 1024 > limit) return BLINK_OK;
+  std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
+  for (int ch = 0; ch < n_ch; ++ch) assign_cells(gathers[ch], owner[ch], slot[ch]);
+
+  std::vector<AbstractTable> tabs;
+  int n_chunk = 0, C = 0, nbuf = 0;
+  size_t tab_stride = 0, buf_bytes = 0;
+  bool found = false;
+  static const int kNbufOrder[3] = {3, 2, 4};
+  for (int oi = 0; oi < 3 && !found; ++oi) {
+    nbuf = kNbufOrder[oi];
+    const size_t room = (limit - band - s_bytes - 16 * (size_t)nbuf - 64) / nbuf / 128 * 128;   // bytes per buffer
+    for (n_chunk = nbuf; n_chunk <= 16 * nbuf && !found; n_chunk += nbuf) {
+      C = (n_bl + n_chunk - 1) / n_chunk;
+      C = (C + 1) & ~1;
+      if (C > 0x7FFE || (n_bl + C - 1) / C != n_chunk) continue;
+      if (sizeof(float2) * (size_t)C > room) continue;
+      tabs.assign((size_t)n_ch * n_chunk, AbstractTable());
+      bool ok = true;
+      tab_stride = 0;
+      for (int ch = 0; ch < n_ch && ok; ++ch)
+        for (int c = 0; c < n_chunk && ok; ++c) {
+          AbstractTable &t = tabs[(size_t)ch * n_chunk + c];
+          build_chunk_table(gathers[ch], owner[ch], slot[ch], c * C, std::min(n_bl, (c + 1) * C), sink0, t, ok);
+          tab_stride = std::max(tab_stride, t.bytes.size());
+        }
+      if (!ok) continue;
+      buf_bytes = (sizeof(float2) * (size_t)C + tab_stride + 127) / 128 * 128;
+      if (buf_bytes > room) continue;
+      found = true;
+      break;
+    }
+  }
+  if (!found) return BLINK_OK;
+  p->ring_chunk_vis = C;
+  p->ring_n_chunk = n_chunk;
+  p->ring_nbuf = nbuf;
+  p->ring_tab_stride = (int)tab_stride;
+  p->ring_buf_bytes = (uint32_t)buf_bytes;
+  p->ring_off_buf = (uint32_t)band;
+  p->ring_off_S = (uint32_t)(band + (size_t)nbuf * buf_bytes);
+  p->ring_off_bar = (uint32_t)(p->ring_off_S + s_bytes);
+  p->ring_smem = p->ring_off_bar + 16 * (size_t)nbuf + 16;
+  if (p->ring_smem > limit || p->ring_smem > 0x7FFFu * 8u) return BLINK_OK;
+  if (getenv("BLINK_DEBUG"))
+    fprintf(stderr, "blink grid ring route: %d chunks of %d baselines, %d buffers of %zu B, smem %zu B\n", n_chunk, C,
+            nbuf, buf_bytes, p->ring_smem);
+
+  const uint32_t s_slot0 = p->ring_off_S / 8;
+  std::vector<unsigned char> h_tab((size_t)n_ch * n_chunk * tab_stride, 0);
+  std::vector<uint32_t> h_size((size_t)n_ch * n_chunk, 0);
+  for (int ch = 0; ch < n_ch; ++ch)
+    for (int c = 0; c < n_chunk; ++c) {
+      const size_t cp = (size_t)ch * n_chunk + c;
+      std::vector<unsigned char> &b = tabs[cp].bytes;
+      finalize_chunk_table(b, (uint32_t)((p->ring_off_buf + (size_t)(c % nbuf) * buf_bytes) / 8), s_slot0, sink0);
+      std::memcpy(h_tab.data() + cp * tab_stride, b.data(), b.size());
+      h_size[cp] = (uint32_t)b.size();
+    }
+  // placement records: every canonical cell and its mirror, ascending cell index (coalesced-ish stores)
+  std::vector<int2> h_place((size_t)n_ch * 2 * n_bl, make_int2(-1, 0));
+  for (int ch = 0; ch < n_ch; ++ch) {
+    const HostGather &g = gathers[ch];
+    std::vector<std::pair<int32_t, int32_t>> pl;
+    pl.reserve(2 * (size_t)g.n_can);
+    for (int j = 0; j < g.n_can; ++j) {
+      const int c = g.can_cell[j], ix = c % N, iy = c / N;
+      const int cc = ((N - iy) % N) * N + ((N - ix) % N);
+      if (cc == c) {
+        pl.push_back({c, slot[ch][j] | (int32_t)((uint32_t)kPlaceBoth << 30)});
+      } else {
+        pl.push_back({c, slot[ch][j] | (int32_t)((uint32_t)kPlaceDirect << 30)});
+        pl.push_back({cc, slot[ch][j] | (int32_t)((uint32_t)kPlaceConj << 30)});
+      }
+    }
+    std::sort(pl.begin(), pl.end());
+    for (size_t k = 0; k < pl.size(); ++k) h_place[(size_t)ch * 2 * n_bl + k] = make_int2(pl[k].first, pl[k].second);
+  }
+  auto upload = [&](void **dst, const void *src, size_t bytes) -> int {
+    cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
+    if (e != cudaSuccess) {
+      set_cuda_error(e, "ring table cudaMalloc");
+      *dst = nullptr;
+      return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
+    }
+    BLINK_CUDA_TRY(cudaMemcpyAsync(*dst, src, bytes, cudaMemcpyHostToDevice, st), "ring table upload");
+    return BLINK_OK;
+  };
+  int rc;
+  if ((rc = upload((void **)&p->d_rtab, h_tab.data(), h_tab.size())) != BLINK_OK) return rc;
+  if ((rc = upload((void **)&p->d_rsize, h_size.data(), sizeof(uint32_t) * h_size.size())) != BLINK_OK) return rc;
+  if ((rc = upload((void **)&p->d_rplace, h_place.data(), sizeof(int2) * h_place.size())) != BLINK_OK) return rc;
+  BLINK_CUDA_TRY(cudaStreamSynchronize(st), "ring table upload sync");
+  p->ring_min_snap = p->sm_count;
+  if (const char *e = getenv("BLINK_GRID_RING_MIN")) p->ring_min_snap = atoi(e);
+  p->ring_path = 1;
+  return BLINK_OK;
+}
+
+static int launch_grid_ring(const blink_plan *p, const float2 *vis, int n_snap, int ch0, float2 *uv, cudaStream_t st) {
+  GridRingParams g;
+  g.vis = vis; g.uv = uv; g.chinfo = p->d_chinfo; g.rtab = p->d_rtab; g.rsize = p->d_rsize; g.rplace = p->d_rplace;
+  g.n_bl = p->n_bl; g.n_ch = p->n_ch; g.n_snap = n_snap; g.n_can_max = p->n_can_max; g.n_chunk = p->ring_n_chunk;
+  g.chunk_vis = p->ring_chunk_vis; g.nbuf = p->ring_nbuf; g.tab_stride = p->ring_tab_stride; g.n_bands = p->n_bands;
+  g.band_cells = p->band_cells; g.ch0 = ch0; g.buf_bytes = p->ring_buf_bytes; g.off_buf = p->ring_off_buf;
+  g.off_S = p->ring_off_S; g.off_bar = p->ring_off_bar; g.grid_cells = (long long)p->n_pix * p->n_pix;
+  static thread_local size_t smem_set = 0;
+  if (p->ring_smem > smem_set) {
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_grid_ring, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ring_smem),
+                   "k_grid_ring smem attribute");
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_grid_ring, cudaFuncAttributePreferredSharedMemoryCarveout, 100), "k_grid_ring carveout");
+    smem_set = p->ring_smem;
+  }
+  const int blocks = std::min(n_snap, p->sm_count);
+  k_grid_ring<<<blocks, kFusedThreads, p->ring_smem, st>>>(g);
+  BLINK_CUDA_TRY(cudaGetLastError(), "k_grid_ring launch");
+  return BLINK_OK;
+}
+
 template <int THREADS, int PF, int MINB>
 static int launch_grid_v(const blink_plan *p, const GridParams &g0, cudaStream_t st) {
   GridParams g = g0;
@@ -152,6 +415,9 @@ static int launch_grid_v(const blink_plan *p, const GridParams &g0, cudaStream_t
 }
 
 int launch_grid(const blink_plan *p, const float2 *vis, int n_snap, int ch0, float2 *uv, cudaStream_t st) {
+  // many snapshots of a small grid: the ring route; few snapshots (or large grids): the band route,
+  // which can split one snapshot over several CTAs
+  if (p->ring_path == 1 && n_snap >= p->ring_min_snap) return launch_grid_ring(p, vis, n_snap, ch0, uv, st);
   GridParams g;
   g.vis = vis; g.uv = uv; g.chinfo = p->d_chinfo;
   g.scat = p->d_scat; g.roff = p->d_roff; g.cellrec = p->d_cellrec; g.nact = p->d_nact; g.pcell = p->d_pcell; g.pcode = p->d_pcode; g.pband = p->d_pband;

@@ -97,6 +97,16 @@ struct blink_plan {
   int32_t *d_vlen = nullptr;        // [n_ch][2 n_bl] entries | flag << 24
   float *d_vw = nullptr;            // [n_ch][2 n_bl] sign * (1/norm) * (1/count if uniform)
   int32_t *d_vcol = nullptr;        // [n_ch][wu + 1] CSR by column
+  // blink_grid, ring route (see grid_ring_build in blink_grid.cu): phase S as in k_fused
+  int ring_path = 0;                // 1 = k_grid_ring available
+  int ring_min_snap = 0;            // fewer snapshots per call take the band route
+  int ring_chunk_vis = 0, ring_n_chunk = 0, ring_nbuf = 0, ring_tab_stride = 0;
+  uint32_t ring_buf_bytes = 0, ring_off_buf = 0, ring_off_S = 0, ring_off_bar = 0;
+  size_t ring_smem = 0;
+  unsigned char *d_rtab = nullptr;  // [n_ch][n_chunk][tab_stride]
+  uint32_t *d_rsize = nullptr;      // [n_ch][n_chunk]
+  int2 *d_rplace = nullptr;         // [n_ch][2 n_bl] {cell, slot of S | flag << 30}, ascending cell
+
   // shared-memory route (see fused_build in blink_fused.cu)
   int h_max = 0;                    // phase-H records per channel (padded with pos = 0xFFFF)
   int fused_threads = 512;
@@ -122,6 +132,7 @@ int launch_grid(const blink_plan *p, const float2 *vis, int n_snap, int ch0, flo
 int launch_image(const blink_plan *p, const float2 *uv, int n_snap, int ch0, float *img, cudaStream_t st);
 int image_setup(blink_plan *p);
 int image_reserve(blink_plan *p, int n_t);
+int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st);
 int fused_setup(blink_plan *p);
 int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st);
 int fused_line_stride(int n_pix);

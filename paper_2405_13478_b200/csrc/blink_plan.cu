@@ -201,6 +201,7 @@ static void plan_free(blink_plan *p) {
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
   cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol);
   cudaFree(p->d_gtab); cudaFree(p->d_gsize); cudaFree(p->d_hrec);
+  cudaFree(p->d_rtab); cudaFree(p->d_rsize); cudaFree(p->d_rplace);
   delete p;
 }
 
@@ -500,6 +501,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     PLAN_CUDA(ce, "vis-route table upload");
   }
   PLAN_TRY(fused_build(p, gathers, st));
+  PLAN_TRY(grid_ring_build(p, gathers, st));
   if (weighting == BLINK_UNIFORM) {
     // canonical cells are exactly the occupied half-plane cells with ky > 0 or (ky == 0, kx >= 0);
     // pass A of blink_image works on columns kx >= 0 and all ky, so list every occupied cell with

@@ -127,6 +127,32 @@ def test_grid_and_image_match_oracle(torch_cuda, blink, oracle, name):
     plan.close()
 
 
+@pytest.mark.parametrize("name", ["tiny", "station", "station128", "station512", "station_uniform_32"])
+def test_grid_ring_route_matches_oracle(torch_cuda, blink, oracle, name, monkeypatch):
+    """blink_grid's ring route (k_grid_ring: gather tables streamed through shared memory with the
+    visibilities) forced on small batches; bench-size batches take it by themselves."""
+    monkeypatch.setenv("BLINK_GRID_RING_MIN", "1")
+    w = _workload(name)
+    vis = w.vis()
+    plan = _plan(blink, w)
+    uv, _ = _run_gpu(torch_cuda, plan, vis)
+    uv2, _ = _run_gpu(torch_cuda, plan, vis)
+    assert np.array_equal(uv.view(np.float32), uv2.view(np.float32)), "ring route must be bit-reproducible"
+    n_snap = w.n_t * w.n_ch
+    sel = np.arange(n_snap, dtype=np.int64) if n_snap <= 12 else np.array([0, 1, 31, 32, 50, n_snap - 1], np.int64)
+    ref = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel,
+                             want_grids=True, want_images=False)
+    uvf = uv.reshape(n_snap, w.n_pix, w.n_pix)
+    idx = (-np.arange(w.n_pix)) % w.n_pix
+    for q, s in enumerate(sel):
+        g_ref, g = ref["grids"][q], uvf[s]
+        assert np.all(np.isfinite(g.view(np.float32))), "grid not fully overwritten"
+        assert np.max(np.abs(g - g_ref)) <= GRID_TOL * np.max(np.abs(g_ref)), f"grid snapshot {s}"
+        assert np.all(g[g_ref == 0] == 0), "cells with no visibility must be exactly zero"
+        assert np.array_equal(g, np.conj(g[idx][:, idx])), "grid must be exactly Hermitian"
+    plan.close()
+
+
 def test_mwa2_4096_sampled_pixels(torch_cuda, blink, oracle):
     """4096^2: full grids are compared exactly as above; images on sampled pixels the oracle
     computes one by one (literal sum over the occupied cells)."""
