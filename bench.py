@@ -311,7 +311,7 @@ def main():
     step_gbs = ab["step"] * n_snap / (ms_per_step / 1e3) / 1e9
     chunks = -(-n_snap // max(1, plan.query_i32(blink.Q_IMAGE_CHUNK)))
     if fused:
-        if plan.query_i32(blink.Q_FUSED_PATH) == 1:
+        if plan.query_i32(blink.Q_FUSED_PATH) in (1, 2):
             launches_per_step = 1
         else:
             launches_per_step = 2 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))

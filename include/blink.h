@@ -73,7 +73,7 @@ typedef enum blink_query {
   BLINK_Q_IMAGE_PATH = 11,/* out: int32   0 = shared-memory single pass, 1 = two-pass */
   BLINK_Q_SCRATCH_BYTES = 12, /* out: int64 device scratch currently held by the plan */
   BLINK_Q_IMAGE_CHUNK = 13, /* out: int32  snapshots per launch pair of the two-pass imaging path */
-  BLINK_Q_FUSED_PATH = 14,  /* out: int32  route of blink_grid_image: 1 = shared memory, 0 = two kernels */
+  BLINK_Q_FUSED_PATH = 14,  /* out: int32  route of blink_grid_image: 1 = shared memory, 2 = warp-per-transform, 0 = two kernels */
   BLINK_Q_FUSED_CHUNK = 15  /* out: int32  snapshots per chunk of the two-kernel route */
 } blink_query;
 
@@ -145,10 +145,15 @@ int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *imag
  * blink_grid_image -- steps a1-a5 in one call: images straight from visibilities, with no uv grid
  * in HBM at all (the paper's aim of processing "fully inside GPU
  * memory" with minimal I/O).  Same result as blink_grid followed by blink_image
- * up to fp32 rounding order (both meet the oracle bars).  Two internal routes, chosen by the plan:
+ * up to fp32 rounding order (both meet the oracle bars).  Three internal routes, chosen by the plan:
  *   - shared-memory route (BLINK_Q_FUSED_PATH == 1; small bounding box, N <= 256): one kernel;
  *     the gridded half-plane never leaves the SM;
- *   - two-kernel route: the column transforms are fed straight from the visibilities through the
+ *   - warp-per-transform route (BLINK_Q_FUSED_PATH == 2; N = 1024 with a wide, sparsely filled
+ *     half-plane, e.g. MWA): one cooperative launch in which one group of CTAs forms the column
+ *     transforms as sparse sums straight from the visibilities and a second group runs the row
+ *     transforms behind it; the intermediate U lives in a 32 MB ring of plan-owned scratch that
+ *     stays in L2;
+ *   - two-kernel route (BLINK_Q_FUSED_PATH == 0): the column transforms are fed straight from the visibilities through the
  *     plan's cell-sorted tables (each occupied cell sums its own baselines in ascending order), the
  *     row transforms follow; only the half-plane intermediate U passes through plan-owned scratch,
  *     in chunks of BLINK_Q_FUSED_CHUNK snapshots sized to stay L2-resident.

@@ -29,21 +29,6 @@ template <int N> struct ImgCfg {
   static constexpr int RP_MAX = (N / 2) < (512 / T) ? (N / 2) : (512 / T > 0 ? 512 / T : 1);
 };
 
-struct ImgParams {
-  const float2 *uv;
-  float *img;
-  float2 *U;
-  const ChannelInfo *chinfo;
-  const int32_t *wkey, *wcol;
-  const float *wval;
-  // pass A straight from visibilities (blink_grid_image, two-kernel route)
-  const float2 *vis;
-  const int32_t *src, *vkey, *vseg, *vlen, *vcol;
-  const float *vw;
-  const float2 *tw;
-  int n_ch, n_bl, wu, uniform, snap_base, ch0, direct_max;
-};
-
 // run stages 1.. of the transform; stage 0's load is done by the caller
 template <int N, class Store>
 __device__ __forceinline__ void fft_tail(cf32 *v, int t, cf32 *line, const cf32 *__restrict__ tw, Store st) {
@@ -362,7 +347,8 @@ int image_setup(blink_plan *p) {
 int image_reserve(blink_plan *p, int n_t) {
   const long long n_snap = (long long)n_t * p->n_ch;
   const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
-  const size_t need = per_snap * (size_t)std::min<long long>(std::max<long long>(n_snap, 1), p->chunk_snapshots);
+  size_t need = per_snap * (size_t)std::min<long long>(std::max<long long>(n_snap, 1), p->chunk_snapshots);
+  if (p->warp_route) need = std::max(need, warp_route_scratch_bytes(p, std::max<long long>(n_snap, 1)));
   if (need <= p->scratch_bytes) return BLINK_OK;
   if (p->d_scratch) {
     BLINK_CUDA_TRY(cudaDeviceSynchronize(), "scratch regrow sync");
@@ -382,7 +368,8 @@ int image_reserve(blink_plan *p, int n_t) {
 static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2 *vis, int n_snap, int ch0, float *img, cudaStream_t st) {
   ImgParams ip;
   ip.vis = vis; ip.src = p->d_src; ip.vkey = p->d_vkey; ip.vseg = p->d_vseg; ip.vlen = p->d_vlen;
-  ip.vcol = p->d_vcol; ip.vw = p->d_vw;
+  ip.vcol = p->d_vcol; ip.vw = p->d_vw; ip.tw32 = p->d_tw32;
+  ip.cell_cap = (std::max(p->vtile8_max, 1) + 3) / 4 * 4;
   ip.uv = uv; ip.img = img; ip.U = p->d_scratch; ip.chinfo = p->d_chinfo;
   ip.wkey = p->d_wkey; ip.wval = p->d_wval; ip.wcol = p->d_wcol; ip.n_bl = p->n_bl;
   ip.tw = p->d_tw; ip.n_ch = p->n_ch; ip.wu = p->wu; ip.uniform = p->weighting == BLINK_UNIFORM;
@@ -390,6 +377,8 @@ static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2
   ip.ch0 = ch0;
   ip.direct_max = 12;
   if (const char *e = getenv("BLINK_IMAGE_DIRECT")) ip.direct_max = std::min(32, std::max(0, atoi(e)));
+  if (p->warp_route && vis != nullptr)      // persistent warp-per-transform kernel (blink_image_w.cu)
+    return launch_img1024(p, ip, n_snap, st);
   switch (p->n_pix) {
     case 32: return run_image_n<32>(p, ip, n_snap, st);
     case 64: return run_image_n<64>(p, ip, n_snap, st);

@@ -97,6 +97,10 @@ struct blink_plan {
   int32_t *d_vlen = nullptr;        // [n_ch][2 n_bl] entries | flag << 24
   float *d_vw = nullptr;            // [n_ch][2 n_bl] sign * (1/norm) * (1/count if uniform)
   int32_t *d_vcol = nullptr;        // [n_ch][wu + 1] CSR by column
+  uint4 *d_vrec = nullptr;          // [n_ch][2 n_bl] packed cell records: iy | flag << 16 | len << 18, weight, source 0, source 1 / segment
+  int vtile8_max = 0;               // most cells in any 8-column tile of any channel
+  float2 *d_tw32 = nullptr;         // [32][32] exp(+2 pi i b n1 / 1024) (wfft.cuh), N = 1024 only
+  int warp_route = 0;               // 1 = blink_grid_image takes the warp-per-transform kernel (blink_image_w.cu)
   // blink_grid, ring route (see grid_ring_build in blink_grid.cu): phase S as in k_fused
   int ring_path = 0;                // 1 = k_grid_ring available
   int ring_min_snap = 0;            // fewer snapshots per call take the band route
@@ -118,6 +122,31 @@ struct blink_plan {
   uint2 *d_hrec = nullptr;          // [n_ch][h_max] {line position | j << 16 | flag << 30, weight}
 
 };
+
+namespace blink {
+
+// arguments of the imaging kernels (blink_image.cu, blink_image_w.cu)
+struct ImgParams {
+  const float2 *uv;
+  float *img;
+  float2 *U;
+  const ChannelInfo *chinfo;
+  const int32_t *wkey, *wcol;
+  const float *wval;
+  // pass A straight from visibilities (blink_grid_image, two-kernel route)
+  const float2 *vis;
+  const int32_t *src, *vkey, *vseg, *vlen, *vcol;
+  const float *vw;
+  const float2 *tw, *tw32;
+  int n_ch, n_bl, wu, uniform, snap_base, ch0, direct_max, cell_cap;
+};
+
+// warp-per-transform persistent kernel at N = 1024 (blink_image_w.cu)
+int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st);
+bool warp_route_applies(const blink_plan *p);
+size_t warp_route_scratch_bytes(const blink_plan *p, long long n_snap);
+
+}  // namespace blink
 
 namespace blink {
 

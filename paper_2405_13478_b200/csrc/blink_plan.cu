@@ -199,7 +199,7 @@ static void plan_free(blink_plan *p) {
   if (!p) return;
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
-  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol);
+  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol); cudaFree(p->d_vrec); cudaFree(p->d_tw32);
   cudaFree(p->d_gtab); cudaFree(p->d_gsize); cudaFree(p->d_hrec);
   cudaFree(p->d_rtab); cudaFree(p->d_rsize); cudaFree(p->d_rplace);
   delete p;
@@ -447,6 +447,16 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   step(cudaMemcpyAsync(p->d_pcode, h_pcode.data(), sizeof(int32_t) * h_pcode.size(), cudaMemcpyHostToDevice, st));
   step(cudaMemcpyAsync(p->d_pband, h_pband.data(), sizeof(int32_t) * h_pband.size(), cudaMemcpyHostToDevice, st));
   step(cudaMemcpyAsync(p->d_tw, h_tw.data(), sizeof(float2) * N, cudaMemcpyHostToDevice, st));
+  std::vector<float2> h_tw32(32 * 32);
+  if (N == 1024) {   // inner-step twiddles of the warp-per-transform kernels, [n1][b]
+    for (int n1 = 0; n1 < 32; ++n1)
+      for (int b = 0; b < 32; ++b) {
+        const double a = 2.0 * 3.14159265358979323846264338327950288 * (double)(b * n1) / 1024.0;
+        h_tw32[n1 * 32 + b] = make_float2((float)cos(a), (float)sin(a));
+      }
+    PLAN_TRY(dev_alloc(&p->d_tw32, h_tw32.size()));
+    step(cudaMemcpyAsync(p->d_tw32, h_tw32.data(), sizeof(float2) * h_tw32.size(), cudaMemcpyHostToDevice, st));
+  }
   step(cudaStreamSynchronize(st));
   PLAN_CUDA(ce, "plan table upload");
   PLAN_TRY(image_setup(p));
@@ -456,6 +466,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     std::vector<int32_t> h_vkey((size_t)n_ch * 2 * n_bl, 0), h_vseg((size_t)n_ch * 2 * n_bl, 0),
         h_vlen((size_t)n_ch * 2 * n_bl, 0), h_vcol((size_t)n_ch * (p->wu + 1), 0);
     std::vector<float> h_vw((size_t)n_ch * 2 * n_bl, 0.f);
+    std::vector<uint4> h_vrec((size_t)n_ch * 2 * n_bl, make_uint4(0, 0, 0, 0));
     struct VEnt { int32_t key, seg, len; float w; };
     for (int ch = 0; ch < n_ch; ++ch) {
       const HostGather &g = gathers[ch];
@@ -473,7 +484,10 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
         if (kx <= 0 && c != 0)
           ent.push_back({((-kx) << 16) | ((N - iy) % N), g.seg_start[j], len | (kPlaceConj << 24), w});
       }
-      std::sort(ent.begin(), ent.end(), [](const VEnt &a, const VEnt &b) { return a.key < b.key; });
+      // within a column: by iy mod 32, then iy / 32 -- the order the warp-per-column pass A
+      // (blink_image_w.cu) consumes; the line-scatter kernels do not care
+      auto vorder = [](int32_t key) { return ((key >> 16) << 16) | ((key & 31) << 11) | ((key & 0xffff) >> 5); };
+      std::sort(ent.begin(), ent.end(), [&](const VEnt &a, const VEnt &b) { return vorder(a.key) < vorder(b.key); });
       int32_t *vc = h_vcol.data() + (size_t)ch * (p->wu + 1);
       size_t e = 0;
       for (int kx = 0; kx < p->wu; ++kx) {
@@ -485,13 +499,24 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
       for (size_t k = 0; k < ent.size(); ++k) {
         h_vkey[base + k] = ent[k].key; h_vseg[base + k] = ent[k].seg;
         h_vlen[base + k] = ent[k].len; h_vw[base + k] = ent[k].w;
+        {   // one 16-byte record per cell for the warp-per-column pass A (blink_image_w.cu)
+          const int len = ent[k].len & 0xFFFFFF, flag = ent[k].len >> 24;
+          uint32_t wbits;
+          memcpy(&wbits, &ent[k].w, 4);
+          h_vrec[base + k] = make_uint4((uint32_t)(ent[k].key & 0xffff) | ((uint32_t)flag << 16) | ((uint32_t)len << 18), wbits,
+                                        (uint32_t)g.src[ent[k].seg],
+                                        len == 2 ? (uint32_t)g.src[ent[k].seg + 1] : (uint32_t)ent[k].seg);
+        }
       }
+      for (int kx = 0; kx < p->wu; kx += 8) p->vtile8_max = std::max(p->vtile8_max, vc[std::min(kx + 8, p->wu)] - vc[kx]);
     }
     PLAN_TRY(dev_alloc(&p->d_vkey, h_vkey.size()));
     PLAN_TRY(dev_alloc(&p->d_vseg, h_vseg.size()));
     PLAN_TRY(dev_alloc(&p->d_vlen, h_vlen.size()));
     PLAN_TRY(dev_alloc(&p->d_vw, h_vw.size()));
     PLAN_TRY(dev_alloc(&p->d_vcol, h_vcol.size()));
+    PLAN_TRY(dev_alloc(&p->d_vrec, h_vrec.size()));
+    step(cudaMemcpyAsync(p->d_vrec, h_vrec.data(), sizeof(uint4) * h_vrec.size(), cudaMemcpyHostToDevice, st));
     step(cudaMemcpyAsync(p->d_vkey, h_vkey.data(), sizeof(int32_t) * h_vkey.size(), cudaMemcpyHostToDevice, st));
     step(cudaMemcpyAsync(p->d_vseg, h_vseg.data(), sizeof(int32_t) * h_vseg.size(), cudaMemcpyHostToDevice, st));
     step(cudaMemcpyAsync(p->d_vlen, h_vlen.data(), sizeof(int32_t) * h_vlen.size(), cudaMemcpyHostToDevice, st));
@@ -499,6 +524,8 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     step(cudaMemcpyAsync(p->d_vcol, h_vcol.data(), sizeof(int32_t) * h_vcol.size(), cudaMemcpyHostToDevice, st));
     step(cudaStreamSynchronize(st));
     PLAN_CUDA(ce, "vis-route table upload");
+    p->warp_route = warp_route_applies(p) ? 1 : 0;
+    if (const char *e = getenv("BLINK_IMAGE_WARP")) p->warp_route = (atoi(e) != 0 && warp_route_applies(p)) ? 1 : 0;
   }
   PLAN_TRY(fused_build(p, gathers, st));
   PLAN_TRY(grid_ring_build(p, gathers, st));
@@ -603,7 +630,7 @@ extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *
     case BLINK_Q_IMAGE_PATH: *(int32_t *)out = p->image_path; break;
     case BLINK_Q_SCRATCH_BYTES: *(int64_t *)out = (int64_t)p->scratch_bytes; break;
     case BLINK_Q_IMAGE_CHUNK: *(int32_t *)out = p->chunk_snapshots; break;
-    case BLINK_Q_FUSED_PATH: *(int32_t *)out = p->fused_path; break;
+    case BLINK_Q_FUSED_PATH: *(int32_t *)out = p->fused_path == 1 ? 1 : (p->warp_route ? 2 : 0); break;
     case BLINK_Q_FUSED_CHUNK: *(int32_t *)out = p->fused_chunk; break;
     default: return BLINK_EINVAL;
   }

@@ -86,6 +86,8 @@ template <> BLINK_HD void dft<2>(cf32 *v) { dft2(v[0], v[1]); }
 template <> BLINK_HD void dft<4>(cf32 *v) { dft4(v[0], v[1], v[2], v[3]); }
 template <> BLINK_HD void dft<8>(cf32 *v) { dft8(v); }
 template <> BLINK_HD void dft<16>(cf32 *v) { dft16(v); }
+BLINK_HD void dft32(cf32 *v);
+template <> BLINK_HD void dft<32>(cf32 *v) { dft32(v); }
 
 // ---- pruned butterflies: inputs known to be zero at compile time --------------------------------
 // dftp<R, M>(v) is dft<R>(v) for inputs whose bit in M is clear being zero (their v[] entries are
@@ -102,6 +104,45 @@ template <int A> BLINK_HD cf32 mul_w16(cf32 x) {   // x * exp(+i pi A / 8), A = 
   else if constexpr (A == 3) return cmul(x, mk(BLINK_SIN_PI_8, BLINK_COS_PI_8));
   else if constexpr (A == 5) return cmul(x, mk(-BLINK_SIN_PI_8, BLINK_COS_PI_8));
   else return cmul(x, mk(-BLINK_COS_PI_8, BLINK_SIN_PI_8));
+}
+
+// 32-point butterfly: radix-2 decimation in time over two 16-point butterflies (used by the
+// warp-per-transform kernels, wfft.cuh, where a lane owns 32 points of a 1024-point transform)
+#define BLINK_COS_PI_16 0.98078528040323044913f
+#define BLINK_SIN_PI_16 0.19509032201612826785f
+#define BLINK_COS_3PI_16 0.83146961230254523708f
+#define BLINK_SIN_3PI_16 0.55557023301960222474f
+
+template <int A> BLINK_HD cf32 mul_w32(cf32 x) {   // x * exp(+i pi A / 16), A = 0..15
+  if constexpr ((A & 1) == 0) return mul_w16<A / 2>(x);
+  else if constexpr (A == 1) return cmul(x, mk(BLINK_COS_PI_16, BLINK_SIN_PI_16));
+  else if constexpr (A == 3) return cmul(x, mk(BLINK_COS_3PI_16, BLINK_SIN_3PI_16));
+  else if constexpr (A == 5) return cmul(x, mk(BLINK_SIN_3PI_16, BLINK_COS_3PI_16));
+  else if constexpr (A == 7) return cmul(x, mk(BLINK_SIN_PI_16, BLINK_COS_PI_16));
+  else if constexpr (A == 9) return cmul(x, mk(-BLINK_SIN_PI_16, BLINK_COS_PI_16));
+  else if constexpr (A == 11) return cmul(x, mk(-BLINK_SIN_3PI_16, BLINK_COS_3PI_16));
+  else if constexpr (A == 13) return cmul(x, mk(-BLINK_COS_3PI_16, BLINK_SIN_3PI_16));
+  else return cmul(x, mk(-BLINK_COS_PI_16, BLINK_SIN_PI_16));
+}
+
+template <int K> struct Combine32 {
+  BLINK_HD static void run(cf32 *v, const cf32 *e, const cf32 *o) {
+    if constexpr (K < 16) {
+      const cf32 t = mul_w32<K>(o[K]);
+      v[K] = cadd(e[K], t);
+      v[K + 16] = csub(e[K], t);
+      Combine32<K + 1>::run(v, e, o);
+    }
+  }
+};
+
+BLINK_HD void dft32(cf32 *v) {  // v[0..31]
+  cf32 e[16], o[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) { e[k] = v[2 * k]; o[k] = v[2 * k + 1]; }
+  dft16(e);
+  dft16(o);
+  Combine32<0>::run(v, e, o);
 }
 
 constexpr unsigned prune_even(unsigned m, int r) {   // mask of the even-indexed inputs, compacted

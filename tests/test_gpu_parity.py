@@ -41,6 +41,8 @@ def _workload(name):
         return synth.config_station(n_t=2, n_ch=2, n_pix=512)
     if name == "mwa1":
         return synth.config_mwa1(n_t=2, n_ch=3)
+    if name == "station1024":
+        return synth.config_station(n_t=1, n_ch=2, n_pix=1024)
     if name == "mwa2":
         return synth.config_mwa2(n_t=1, n_ch=2)
     if name == "mwa1_natural_64":   # small-field geometry on a small grid: most baselines dropped
@@ -267,7 +269,7 @@ def test_full_size_station_launch_configuration(torch_cuda, blink, oracle):
 
 
 @pytest.mark.parametrize("name", ["tiny", "station", "station128", "mwa1", "station_uniform_32",
-                                  "mwa1_natural_64"])
+                                  "mwa1_natural_64", "station1024"])
 def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name):
     """blink_grid_image (one call, no uv grid in caller memory; shared-memory route where the plan
     allows it, chunked route otherwise) against blink_grid + blink_image (fp32 rounding apart) and
@@ -293,7 +295,45 @@ def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name
     if name in ("tiny", "station", "station128", "station_uniform_32"):
         assert plan.query_i32(blink.Q_FUSED_PATH) == 1     # these fit the shared-memory route
     if name == "mwa1":
-        assert plan.query_i32(blink.Q_FUSED_PATH) == 0
+        assert plan.query_i32(blink.Q_FUSED_PATH) == 2     # wide sparse half-plane at N = 1024: warp route
+    if name == "station1024":
+        assert plan.query_i32(blink.Q_FUSED_PATH) == 0     # compact array at N = 1024: two-kernel route
+    plan.close()
+
+
+def test_warp_route_ring_reuse(torch_cuda, blink, oracle, monkeypatch):
+    """blink_grid_image, warp-per-transform route (k_img1024), on more snapshots than its ring of U
+    slots holds (here a ring of 3), so that pass A has to wait for pass B to release a slot: every
+    snapshot against the two-kernel route (same tables, fp32 rounding apart), sampled ones against
+    the oracle at the image bar."""
+    torch = torch_cuda
+    w = synth.config_mwa1(n_t=7, n_ch=3)
+    vis_h = w.vis()
+    vis = torch.from_numpy(vis_h).cuda()
+    monkeypatch.setenv("BLINK_IMAGE_WARP", "0")
+    plan0 = _plan(blink, w)
+    assert plan0.query_i32(blink.Q_FUSED_PATH) == 0
+    ref = torch.empty((w.n_t, w.n_ch, w.n_pix, w.n_pix), dtype=torch.float32, device="cuda")
+    plan0.grid_image(vis, ref)
+    plan0.close()
+    monkeypatch.delenv("BLINK_IMAGE_WARP")
+    monkeypatch.setenv("BLINK_W_RING", "3")
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 2
+    img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    for _ in range(2):                      # twice: the counters are reset per call
+        plan.grid_image(vis, img)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img).all()
+    peak = ref.abs().amax(dim=(-2, -1), keepdim=True)
+    assert ((img - ref).abs() <= 1e-5 * peak).all()
+    n_snap = w.n_t * w.n_ch
+    sel = np.array([0, 10, n_snap - 1], np.int64)
+    orc = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_h, sel)
+    got = img.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        pk = np.max(np.abs(orc["images"][q]))
+        assert np.max(np.abs(got[q] - orc["images"][q])) <= IMG_TOL * pk
     plan.close()
 
 
