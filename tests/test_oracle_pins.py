@@ -294,3 +294,89 @@ def test_image_batch_matches_stepwise(oracle):
         _, g, _, img, _ = _chain(oracle, w, vis[t, ch], ch)
         assert np.array_equal(out["grids"][q], g)
         assert np.array_equal(out["images"][q], img)
+
+
+# ------------------------------------------------------------------ pre-gridding corrections (f2)
+def _voltage_visibilities(ant, freq, src_lmS, gains, cables):
+    """Visibilities from per-antenna VOLTAGES (first principles, independent of oracle/corrections):
+    a source of flux S at (l, m, n) gives antenna i the phasor sqrt(S) exp(+2 pi i (x l + y m + z (n-1)) nu/c);
+    the receiver chain multiplies it by g_i and delays it by L_i / c (a factor exp(-2 pi i nu L_i/c));
+    the correlator forms V_ij = E_i conj(E_j) per source (sources are incoherent)."""
+    n_ant = ant.shape[0]
+    out = np.zeros((len(freq), n_ant * (n_ant - 1) // 2), np.complex128)
+    for ch, nu in enumerate(freq):
+        for (l, m, S) in src_lmS:
+            n = math.sqrt(1 - l * l - m * m)
+            E = np.array([math.sqrt(S) * np.exp(2j * math.pi * (ant[i, 0] * l + ant[i, 1] * m + ant[i, 2] * (n - 1)) * nu / C)
+                          for i in range(n_ant)])
+            E = E * gains[ch] * np.exp(-2j * math.pi * nu * cables / C)
+            bl = 0
+            for i in range(n_ant):
+                for j in range(i + 1, n_ant):
+                    out[ch, bl] += E[i] * np.conj(E[j])
+                    bl += 1
+    return out
+
+
+def test_corrections_identity_is_exactly_one():
+    from oracle import corrections as oc
+    w = synth.config_tiny()
+    F = oc.correction_factors(w.ant_enu_m, w.freq_hz)
+    assert np.all(F == 1.0 + 0.0j)          # a stray phase or a wrong default fails this
+
+
+def test_corrections_restore_ideal_visibilities_from_corrupted_voltages():
+    """Catches a wrong sign of the cable phase, g_i conj(g_j) transposed, gains multiplied instead
+    of divided, a dropped w term."""
+    from oracle import corrections as oc
+    rng = np.random.default_rng(5)
+    ant = rng.uniform(-20, 20, (9, 3))
+    ant[:, 2] = rng.uniform(-0.5, 0.5, 9)              # non-coplanar: exercises w
+    freq = np.array([150e6, 170e6])
+    gains = (rng.uniform(0.5, 1.5, (2, 9)) * np.exp(2j * np.pi * rng.uniform(0, 1, (2, 9))))
+    cables = rng.uniform(0, 120.0, 9)
+    src = [(0.3, -0.2, 2.0), (-0.5, 0.4, 1.0)]
+    ideal = _voltage_visibilities(ant, freq, src, np.ones((2, 9)), np.zeros(9))
+    meas = _voltage_visibilities(ant, freq, src, gains, cables)
+    assert np.max(np.abs(meas - ideal)) > 0.5           # the corruption is not a no-op
+    F = oc.correction_factors(ant, freq, gains, cables)
+    got = oc.apply_corrections(meas[None], F)[0]
+    assert np.max(np.abs(got - ideal)) <= 1e-9 * np.max(np.abs(ideal))
+    # and the ideal ones agree with Eq. 5's sign convention used by the imaging oracle (c10)
+    l, m, S = src[0]
+    n = math.sqrt(1 - l * l - m * m)
+    one = _voltage_visibilities(ant, freq[:1], [src[0]], np.ones((1, 9)), np.zeros(9))[0]
+    u = (ant[1, 0] - ant[0, 0]) * freq[0] / C
+    v = (ant[1, 1] - ant[0, 1]) * freq[0] / C
+    ww = (ant[1, 2] - ant[0, 2]) * freq[0] / C
+    assert abs(one[0] - S * np.exp(-2j * math.pi * (u * l + v * m + ww * (n - 1)))) < 1e-9
+
+
+def test_geometric_rotation_moves_source_to_phase_centre(oracle):
+    """A unit source at (l0, m0): after the rotation every visibility is 1, so the image of the
+    corrected visibilities is the dirty beam with exactly 1.0 at the centre pixel (north_star's
+    phase-centre check, through the correction).  Catches the wrong sign of (iii)."""
+    from oracle import corrections as oc
+    w = synth.config_tiny()
+    l0, m0 = 0.25, -0.4
+    vis = _voltage_visibilities(w.ant_enu_m, w.freq_hz, [(l0, m0, 1.0)], np.ones((1, w.n_ant)), np.zeros(w.n_ant))
+    F = oc.correction_factors(w.ant_enu_m, w.freq_hz, l0=l0, m0=m0)
+    cor = oc.apply_corrections(vis[None], F)
+    assert np.max(np.abs(cor - 1.0)) < 1e-9
+    out = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting,
+                             cor.astype(np.complex64), np.array([0], np.int64))
+    img = out["images"][0]
+    c = w.n_pix // 2
+    assert abs(img[c, c] - 1.0) < 1e-6 and np.argmax(img) == c * w.n_pix + c
+
+
+def test_corrections_antenna_swap_conjugates_factor():
+    from oracle import corrections as oc
+    rng = np.random.default_rng(6)
+    ant = rng.uniform(-20, 20, (2, 3))
+    freq = np.array([160e6])
+    gains = rng.uniform(0.5, 1.5, (1, 2)) * np.exp(2j * np.pi * rng.uniform(0, 1, (1, 2)))
+    cables = np.array([10.0, 55.0])
+    F = oc.correction_factors(ant, freq, gains, cables, 0.1, 0.2)[0, 0]
+    Fs = oc.correction_factors(ant[::-1], freq, gains[:, ::-1], cables[::-1], 0.1, 0.2)[0, 0]
+    assert abs(Fs - np.conj(F)) < 1e-12 * abs(F)
