@@ -176,6 +176,8 @@ def main():
                          "auto = fused")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-corrections", action="store_true",
+                    help="skip the side measurement of blink_correct (SURVEY.md 8(f) item f2)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -261,6 +263,30 @@ def main():
     n_snap = w.n_snapshots
     value = world * n_snap / (ms_per_step / 1e3)
 
+    # ---- side measurement, outside the step: blink_correct (f2), a streaming complex multiply of the
+    # whole batch by the plan's factor table; algorithmic bytes 16 per visibility (read 8, write 8)
+    corr = None
+    if not args.no_corrections:
+        rng = np.random.default_rng(w.seed + 7)
+        n_ant = w.ant_enu_m.shape[0]
+        gains = rng.uniform(0.5, 2.0, (w.n_ch, n_ant)) * np.exp(1j * rng.uniform(-np.pi, np.pi, (w.n_ch, n_ant)))
+        plan.set_corrections(gains, rng.uniform(0.0, 300.0, n_ant), 0.1, -0.2)
+        vis_c = torch.empty_like(vis)
+        for _ in range(3):
+            plan.correct(vis, vis_c)
+        barrier()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record(stream)
+        for _ in range(args.steps):
+            plan.correct(vis, vis_c)
+        c1.record(stream)
+        barrier()
+        c_ms = c0.elapsed_time(c1) / args.steps
+        c_bytes = 16 * vis.numel()
+        corr = {"call": "blink_correct", "ms": c_ms, "algorithmic_bytes": c_bytes,
+                "achieved_gbs": c_bytes / (c_ms / 1e3) / 1e9, "gvis_per_s": vis.numel() / (c_ms / 1e3) / 1e9}
+        del vis_c
+
     # ---- end to end: pinned host visibilities in, images back to pinned host memory, per step
     e2e = None
     if not args.no_e2e:
@@ -343,7 +369,9 @@ def main():
                      "algorithmic_bytes_per_snapshot": calls[dom][1]},
         "roofline_step": {"bound": "hbm", "achieved": step_gbs, "peak": peak, "unit": "GB/s",
                           "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": ab["step"]},
-        "side_bounds": side, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
+        "side_bounds": side,
+        "f2_corrections": dict(corr, frac_of_hbm_peak=corr["achieved_gbs"] / peak) if corr else None,
+        "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
     }
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, args)

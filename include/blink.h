@@ -74,7 +74,8 @@ typedef enum blink_query {
   BLINK_Q_SCRATCH_BYTES = 12, /* out: int64 device scratch currently held by the plan */
   BLINK_Q_IMAGE_CHUNK = 13, /* out: int32  snapshots per launch pair of the two-pass imaging path */
   BLINK_Q_FUSED_PATH = 14,  /* out: int32  route of blink_grid_image: 1 = shared memory, 2 = warp-per-transform, 0 = two kernels */
-  BLINK_Q_FUSED_CHUNK = 15  /* out: int32  snapshots per chunk of the two-kernel route */
+  BLINK_Q_FUSED_CHUNK = 15, /* out: int32  snapshots per chunk of the two-kernel route */
+  BLINK_Q_CORR = 16         /* out: const float2* DEVICE [n_ch][n_bl] correction factors (NULL until set) */
 } blink_query;
 
 typedef struct blink_plan blink_plan; /* opaque */
@@ -142,6 +143,34 @@ int blink_grid(const blink_plan *plan, const void *vis, int n_t, void *uv_grid, 
 int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *images, void *stream);
 
 /*
+ * blink_plan_set_corrections -- the pre-gridding corrections of PAPER.md section 4.2 (:142-156):
+ * (i) cable-length phase, (ii) calibration in phase and amplitude, (iii) geometric phase rotation of
+ * the phase centre.  "In the presented software, most of these corrections are already implemented
+ * as GPU kernels and are executed post-correlation"; the paper gives no formulas, the
+ * readings are DESIGN.md c18-c20:
+ *   antenna model   measured V_ij = a_i conj(a_j) V_ij(true),  a_i(nu) = g_i(nu) exp(-2 pi i nu L_i / c)
+ *   correction      F[ch][bl(i,j)] = exp(+2 pi i (u l0 + v m0 + w (n0 - 1))) / (a_i conj(a_j)),
+ *                   (u, v, w) = (r_j - r_i) nu / c un-snapped, n0 = sqrt(1 - l0^2 - m0^2)
+ * A device kernel builds F once (fp64, stored complex64); geometry, gains, cables and pointing are
+ * fixed across the snapshots of a plan, like the uv indices.
+ *   gains        HOST double [n_ch][n_ant][2] (re, im) calibration solutions g_i, or NULL (all 1);
+ *                every |g_i| must be > 0 and finite
+ *   cable_len_m  HOST double [n_ant] electrical lengths L_i in metres, or NULL (all 0)
+ *   l0, m0       direction cosines of the new phase centre, l0^2 + m0^2 < 1; (0, 0) = none
+ * Copies its inputs; synchronises `stream`; replaces any earlier table.  BLINK_EINVAL on bad values.
+ */
+int blink_plan_set_corrections(blink_plan *plan, const double *gains, const double *cable_len_m,
+                               double l0, double m0, void *stream);
+
+/*
+ * blink_correct -- vis_out[t][ch][bl] = vis_in[t][ch][bl] * F[ch][bl] (complex64 product), the
+ * table set by blink_plan_set_corrections (BLINK_EINVAL if none is set).
+ *   vis_in, vis_out  DEVICE complex64 [n_t][n_ch][n_bl]; may be the same buffer (in place)
+ * Asynchronous on `stream`; no allocation.  Algorithmic bytes: 16 per visibility.
+ */
+int blink_correct(const blink_plan *plan, const void *vis_in, int n_t, void *vis_out, void *stream);
+
+/*
  * blink_grid_image -- steps a1-a5 in one call: images straight from visibilities, with no uv grid
  * in HBM at all (the paper's aim of processing "fully inside GPU
  * memory" with minimal I/O).  Same result as blink_grid followed by blink_image
@@ -165,7 +194,8 @@ int blink_grid_image(const blink_plan *plan, const void *vis, int n_t, void *ima
 
 /*
  * blink_plan_read -- copies one channel's slice of a plan table to HOST memory (synchronous):
- *   what = BLINK_Q_CELL_IDX -> int32 [n_bl];  what = BLINK_Q_COUNTS -> uint32 [N*N].
+ *   what = BLINK_Q_CELL_IDX -> int32 [n_bl];  what = BLINK_Q_COUNTS -> uint32 [N*N];
+ *   what = BLINK_Q_CORR -> complex64 [n_bl] (BLINK_EINVAL until blink_plan_set_corrections).
  * `bytes` must equal the slice size.  This is how a harness checks indices and counts bit-exactly.
  */
 int blink_plan_read(const blink_plan *plan, int what, int ch, void *dst_host, size_t bytes);

@@ -17,11 +17,11 @@ LIB_PATH = os.path.join(_HERE, "libblink.so")
 NATURAL, UNIFORM = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
 (Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
- Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK) = range(16)
+ Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK, Q_CORR) = range(17)
 
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create",
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
-           "blink_grid", "blink_grid_image",
+           "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct",
            "blink_image", "blink_host_build_gather", "blink_host_fused_emulate"]
 
 _lib = None
@@ -66,6 +66,10 @@ def load() -> ctypes.CDLL:
     lib.blink_image.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_grid_image.restype = ci
     lib.blink_grid_image.argtypes = [vp, vp, ci, vp, vp]
+    lib.blink_plan_set_corrections.restype = ci
+    lib.blink_plan_set_corrections.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp]
+    lib.blink_correct.restype = ci
+    lib.blink_correct.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_host_build_gather.restype = ci
     lib.blink_host_build_gather.argtypes = [vp, ci, ci, vp, vp, vp, vp]
     lib.blink_host_fused_emulate.restype = ci
@@ -187,6 +191,40 @@ class Plan:
     def counts(self, ch):
         """uint32 [N, N] weight counts of channel ch, host copy."""
         return self._read(Q_COUNTS, ch, self.n_pix * self.n_pix, np.uint32).reshape(self.n_pix, self.n_pix)
+
+    # ---- pre-gridding corrections (PAPER.md section 4.2)
+    def set_corrections(self, gains=None, cable_len_m=None, l0: float = 0.0, m0: float = 0.0, stream=None):
+        """blink_plan_set_corrections: gains complex [n_ch, n_ant] or None, cable lengths [n_ant] or None,
+        new phase centre (l0, m0)."""
+        g = c = None
+        if gains is not None:
+            g = np.ascontiguousarray(gains, np.complex128)
+            if g.shape != (self.n_ch, self.n_ant):
+                raise ValueError("gains must be [n_ch, n_ant]")
+        if cable_len_m is not None:
+            c = np.ascontiguousarray(cable_len_m, np.float64)
+            if c.shape != (self.n_ant,):
+                raise ValueError("cable_len_m must be [n_ant]")
+        _check(self._lib.blink_plan_set_corrections(self._h, g.ctypes.data if g is not None else None,
+                                                    c.ctypes.data if c is not None else None,
+                                                    float(l0), float(m0), _stream_ptr(stream)),
+               "blink_plan_set_corrections")
+
+    def corr_table(self, ch):
+        """complex64 [n_bl] correction factors of channel ch, host copy."""
+        return self._read(Q_CORR, ch, self.n_bl, np.complex64)
+
+    def correct(self, vis, out=None, stream=None):
+        """blink_correct: out = vis * F (out may be vis itself)."""
+        import torch
+        assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
+        assert tuple(vis.shape[1:]) == (self.n_ch, self.n_bl)
+        if out is None:
+            out = torch.empty_like(vis)
+        assert out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous() and out.shape == vis.shape
+        _check(self._lib.blink_correct(self._h, vis.data_ptr(), vis.shape[0], out.data_ptr(),
+                                       _stream_ptr(stream)), "blink_correct")
+        return out
 
     # ---- hot path
     def reserve(self, n_t: int):

@@ -44,6 +44,10 @@ struct blink_plan {
   int sm_count = 148;
   int max_smem_optin = 0;
 
+  // inputs kept for blink_plan_set_corrections
+  std::vector<double> h_ant, h_freq;
+  float2 *d_corr = nullptr;         // [n_ch][n_bl] correction factors F (blink_correct.cu), NULL until set
+
   // per-channel facts (host)
   std::vector<int64_t> n_dropped, wsum, n_occ;
   std::vector<double> norm;

@@ -199,7 +199,7 @@ static void plan_free(blink_plan *p) {
   if (!p) return;
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
-  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol); cudaFree(p->d_vrec); cudaFree(p->d_tw32);
+  cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol); cudaFree(p->d_vrec); cudaFree(p->d_corr); cudaFree(p->d_tw32);
   cudaFree(p->d_gtab); cudaFree(p->d_gsize); cudaFree(p->d_hrec);
   cudaFree(p->d_rtab); cudaFree(p->d_rsize); cudaFree(p->d_rplace);
   delete p;
@@ -286,6 +286,8 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     }                                       \
   } while (0)
 
+  p->h_ant.assign(ant_enu_m, ant_enu_m + (size_t)3 * n_ant);
+  p->h_freq.assign(freq_hz, freq_hz + n_ch);
   // ---- inputs to the device, K0 --------------------------------------------------------
   std::vector<int32_t> pi(n_bl), pj(n_bl);
   {
@@ -598,6 +600,9 @@ extern "C" int blink_plan_read(const blink_plan *p, int what, int ch, void *dst,
   } else if (what == BLINK_Q_COUNTS) {
     need = sizeof(uint32_t) * (size_t)p->n_pix * p->n_pix;
     src = p->d_counts + (size_t)ch * p->n_pix * p->n_pix;
+  } else if (what == BLINK_Q_CORR && p->d_corr) {
+    need = sizeof(float2) * (size_t)p->n_bl;
+    src = p->d_corr + (size_t)ch * p->n_bl;
   } else {
     return BLINK_EINVAL;
   }
@@ -632,6 +637,7 @@ extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *
     case BLINK_Q_IMAGE_CHUNK: *(int32_t *)out = p->chunk_snapshots; break;
     case BLINK_Q_FUSED_PATH: *(int32_t *)out = p->fused_path == 1 ? 1 : (p->warp_route ? 2 : 0); break;
     case BLINK_Q_FUSED_CHUNK: *(int32_t *)out = p->fused_chunk; break;
+    case BLINK_Q_CORR: *(const void **)out = p->d_corr; break;
     default: return BLINK_EINVAL;
   }
   return BLINK_OK;

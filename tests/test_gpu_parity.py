@@ -351,3 +351,106 @@ def test_host_pipeline_matches_device_path(torch_cuda, blink):
     torch.cuda.synchronize()
     assert torch.equal(img_h, ref.cpu())
     plan.close()
+
+
+# ------------------------------------------------------------------ pre-gridding corrections (f2)
+CORR_TOL = 2e-6   # relative: fp64 factor rounded once to complex64 (6e-8) + one fp32 complex product (<= 3 ulp)
+
+
+def _corr_inputs(w, seed):
+    rng = np.random.default_rng(seed)
+    n_ant = w.ant_enu_m.shape[0]
+    amp = rng.uniform(0.5, 2.0, (w.n_ch, n_ant))
+    ph = rng.uniform(-np.pi, np.pi, (w.n_ch, n_ant))
+    gains = amp * np.exp(1j * ph)
+    cables = rng.uniform(0.0, 300.0, n_ant)          # metres: hundreds of turns of phase at 160 MHz
+    ant = np.array(w.ant_enu_m, np.float64)
+    ant[:, 2] = rng.uniform(-0.5, 0.5, n_ant)        # non-coplanar so the w term is exercised
+    return ant, gains, cables
+
+
+@pytest.mark.parametrize("name,n_t", [("tiny", 1), ("station128", 5), ("mwa1", 7)])
+def test_corrections_match_oracle(torch_cuda, blink, name, n_t):
+    """blink_plan_set_corrections + blink_correct against oracle/corrections.py: the factor table
+    element by element, then the corrected visibilities (out of place and in place)."""
+    torch = torch_cuda
+    from oracle import corrections as oc
+    w = _workload(name)
+    ant, gains, cables = _corr_inputs(w, 11)
+    l0, m0 = 0.31, -0.42
+    plan = blink.Plan(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    with pytest.raises(blink.BlinkError):            # no table yet
+        plan.correct(torch.zeros((1, w.n_ch, w.n_bl), dtype=torch.complex64, device="cuda"))
+    plan.set_corrections(gains, cables, l0, m0)
+    F_ref = oc.correction_factors(ant, w.freq_hz, gains, cables, l0, m0)
+    for ch in range(w.n_ch):
+        F = plan.corr_table(ch)
+        assert np.max(np.abs(F - F_ref[ch]) / np.abs(F_ref[ch])) <= 2e-7, f"factor table channel {ch}"
+    rng = np.random.default_rng(5)
+    vis = (rng.standard_normal((n_t, w.n_ch, w.n_bl)) + 1j * rng.standard_normal((n_t, w.n_ch, w.n_bl))).astype(np.complex64)
+    ref = oc.apply_corrections(vis, F_ref)
+    d = torch.from_numpy(vis).cuda()
+    out = plan.correct(d)
+    assert torch.equal(d.cpu(), torch.from_numpy(vis)), "out-of-place call must not touch its input"
+    got = out.cpu().numpy()
+    assert np.max(np.abs(got - ref) / np.abs(ref)) <= CORR_TOL
+    plan.correct(d, out=d)                           # in place
+    assert torch.equal(d, out)
+    # identity inputs: factors exactly 1, visibilities returned bit for bit
+    plan.set_corrections()
+    assert np.all(plan.corr_table(0) == np.complex64(1.0))
+    d2 = torch.from_numpy(vis).cuda()
+    assert torch.equal(plan.correct(d2), d2)
+    # bad inputs refused
+    with pytest.raises(blink.BlinkError):
+        plan.set_corrections(l0=0.8, m0=0.8)         # outside the unit circle
+    g0 = gains.copy(); g0[0, 0] = 0.0
+    with pytest.raises(blink.BlinkError):
+        plan.set_corrections(g0)
+    plan.close()
+
+
+def test_corrections_odd_table_and_unaligned_views(torch_cuda, blink):
+    """Odd n_ch * n_bl and an 8-byte-aligned (not 16) buffer take the one-visibility kernel."""
+    torch = torch_cuda
+    from oracle import corrections as oc
+    rng = np.random.default_rng(3)
+    ant = rng.uniform(-20, 20, (7, 3))               # 21 baselines, 1 channel: odd table
+    freq = np.array([150e6])
+    plan = blink.Plan(ant, freq, 64, 2.0 / 64, synth.NATURAL)
+    cables = rng.uniform(0, 50, 7)
+    plan.set_corrections(None, cables, 0.1, 0.05)
+    F_ref = oc.correction_factors(ant, freq, None, cables, 0.1, 0.05)
+    vis = (rng.standard_normal((3, 1, 21)) + 1j * rng.standard_normal((3, 1, 21))).astype(np.complex64)
+    ref = oc.apply_corrections(vis, F_ref)
+    buf = torch.zeros(3 * 21 + 1, dtype=torch.complex64, device="cuda")
+    d = buf[1:].view(3, 1, 21)                       # 8-byte aligned only
+    d.copy_(torch.from_numpy(vis))
+    got = plan.correct(d).cpu().numpy()
+    assert np.max(np.abs(got - ref) / np.abs(ref)) <= CORR_TOL
+    plan.close()
+
+
+def test_corrected_source_images_to_one_at_centre(torch_cuda, blink):
+    """Whole chain on the GPU: a unit source at (l0, m0), rotated to the phase centre by
+    blink_correct, images to 1.0 at the centre pixel (north_star's phase-centre check through f2)."""
+    torch = torch_cuda
+    w = synth.config_tiny()
+    l0, m0 = 0.25, -0.125
+    C = 299792458.0
+    ant = np.asarray(w.ant_enu_m, np.float64)
+    vis = np.empty((1, 1, w.n_bl), np.complex64)
+    bl = 0
+    for i in range(ant.shape[0]):
+        for j in range(i + 1, ant.shape[0]):
+            u = (ant[j, 0] - ant[i, 0]) * w.freq_hz[0] / C
+            v = (ant[j, 1] - ant[i, 1]) * w.freq_hz[0] / C
+            vis[0, 0, bl] = np.exp(-2j * np.pi * (u * l0 + v * m0))
+            bl += 1
+    plan = _plan(blink, w)
+    plan.set_corrections(l0=l0, m0=m0)
+    img = plan.grid_image(plan.correct(torch.from_numpy(vis).cuda())).cpu().numpy()[0, 0]
+    c = w.n_pix // 2
+    assert abs(img[c, c] - 1.0) <= 1e-5
+    assert np.unravel_index(np.argmax(img), img.shape) == (c, c)
+    plan.close()
