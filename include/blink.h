@@ -130,11 +130,13 @@ int blink_grid(const blink_plan *plan, const void *vis, int n_t, void *uv_grid, 
  *   img[s][y][x] = Re sum_{ky,kx} G'[ky][kx] exp(+2 pi i (kx (x-N/2) + ky (y-N/2)) / N) / norm[ch]
  * i.e. unnormalised inverse DFT, fftshift so pixel (N/2, N/2) is the phase centre
  * (l = (x-N/2) dx East, m = (y-N/2) dx North), 1/norm, real part.
- *   uv_grid  DEVICE complex64 [n_t][n_ch][N][N], const (never used as scratch).  CONTRACT: cells
- *            outside the plan's bounding box (|kx| > kx_max or |ky| > ky_max, BLINK_Q_BBOX) must be
- *            zero -- true of every blink_grid output -- and are not read.  Inside the box any
- *            values are accepted; the real part of the transform is formed exactly, i.e. a
- *            non-Hermitian grid is symmetrised, (G[k] + conj(G[-k])) / 2.
+ *   uv_grid  DEVICE complex64 [n_t][n_ch][N][N], const (never used as scratch).  CONTRACT: it is a
+ *            grid OF THIS PLAN -- zero in every cell whose weight count (BLINK_Q_COUNTS) is zero and
+ *            Hermitian, G[-k] = conj(G[k]); true of every blink_grid output.  A route may rely on
+ *            either fact: the line kernels read the whole bounding box (BLINK_Q_BBOX) and form the
+ *            real part exactly, i.e. symmetrise a non-Hermitian grid, (G[k] + conj(G[-k])) / 2; the
+ *            warp-per-transform route (N = 1024, wide sparse half-planes: BLINK_Q_FUSED_PATH == 2)
+ *            reads only the occupied cells with kx >= 0.  Cells outside the box are never read.
  *   images   DEVICE float32 [n_t][n_ch][N][N] row-major [y][x]; completely overwritten
  * Asynchronous on `stream`.  May grow the plan's internal device scratch on first use with a
  * larger n_t (the only allocation; query BLINK_Q_SCRATCH_BYTES) -- call blink_plan_reserve first

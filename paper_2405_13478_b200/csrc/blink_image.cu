@@ -377,7 +377,7 @@ static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2
   ip.ch0 = ch0;
   ip.direct_max = 12;
   if (const char *e = getenv("BLINK_IMAGE_DIRECT")) ip.direct_max = std::min(32, std::max(0, atoi(e)));
-  if (p->warp_route && vis != nullptr)      // persistent warp-per-transform kernel (blink_image_w.cu)
+  if (p->warp_route)                        // persistent warp-per-transform kernel (blink_image_w.cu)
     return launch_img1024(p, ip, n_snap, st);
   switch (p->n_pix) {
     case 32: return run_image_n<32>(p, ip, n_snap, st);

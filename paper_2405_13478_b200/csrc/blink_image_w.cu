@@ -21,8 +21,9 @@
 //     issued for the NEXT item as soon as the tile is free, so the loads overlap the outer butterfly
 //     and the stores; a warp-wide store of one register is 128 contiguous bytes of an image row.
 //
-// Used by blink_grid_image when warp_route_applies(); blink_image (dense uv grids) and compact arrays
-// keep the line kernels of blink_image.cu.
+// Used by blink_grid_image and blink_image when warp_route_applies() (blink_image: the same kernel with
+// the cell values read from the uv grid at the plan's occupied cells instead of summed from the
+// visibilities); compact arrays keep the line kernels of blink_image.cu.
 #include <algorithm>
 
 #include "blink_internal.h"
@@ -47,7 +48,8 @@ struct WParams {
   ImgParams ip;
   int n_snap, items_a, g_a, ring;   // items_a = wu / 8; CTAs 0 .. g_a - 1 run pass A; ring slots of U
   int *done_a, *done_b;             // per snapshot, zeroed before the launch
-  const uint4 *vrec;                // pass-A cell records (blink_grid_image)
+  const uint4 *vrec;                // pass-A cell records
+  const float2 *uvsrc;              // blink_image: cell values come from this uv grid; NULL = from visibilities
 };
 
 __device__ __forceinline__ int ld_acquire(const int *p) {
@@ -149,12 +151,27 @@ __global__ void __launch_bounds__(kWThreads, 2) k_img1024(const WParams q) {
             // One 16-byte record per cell: iy | flag << 16 | len << 18, weight, first source code,
             // second source code (len = 2) or the cell's segment in src (len > 2)
           const float2 *__restrict__ vis = p.vis + (size_t)(p.snap_base + s) * p.n_bl;
-          if (cur.idx == 0 && tid == 0 && s + 2 < q.n_snap && (p.n_bl & 1) == 0) {
+          if (q.uvsrc == nullptr && cur.idx == 0 && tid == 0 && s + 2 < q.n_snap && (p.n_bl & 1) == 0) {
             // the visibilities of a snapshot two rounds ahead: into L2 before their pass A needs them
             const float2 *nv = vis + (size_t)2 * p.n_bl;
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nv), "r"((uint32_t)(p.n_bl * sizeof(float2))) : "memory");
           }
           const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
+          if (q.uvsrc != nullptr) {
+            // blink_image: the occupied cells of the item's 8 columns straight from the uv grid (the
+            // half-plane kx >= 0 only; empty cells are zero by contract and never read)
+            const float2 *__restrict__ g = q.uvsrc + (size_t)(p.snap_base + s) * N * N + kx0;
+            for (int e = e0 + tid; e < e1; e += kWThreads) {
+              const uint4 r = recs[e - e0];
+              const int iy = (int)(r.x & 0xffff), flag = (r.x >> 16) & 3;
+              int c = 0;
+              while (e >= off[c + 1]) ++c;
+              const float w = __uint_as_float(r.y);
+              const float2 v = __ldg(g + (size_t)iy * N + c);
+              cv[e - e0] = mk(v.x * w, (flag == kPlaceDirect || flag == kPlaceConj) ? v.y * w : 0.f);
+              ck[e - e0] = iy;
+            }
+          } else
           for (int e = e0 + tid; e < e1; e += kWThreads) {
             const uint4 r = recs[e - e0];
             const int flag = (r.x >> 16) & 3, len = (int)(r.x >> 18);
@@ -346,6 +363,7 @@ int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t s
   q.done_a = cnt;
   q.done_b = cnt + n_snap;
   q.vrec = p->d_vrec;
+  q.uvsrc = ip.vis == nullptr ? ip.uv : nullptr;
   ip.snap_base = 0;
   ip.U = p->d_scratch;
   q.ip = ip;

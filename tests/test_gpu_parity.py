@@ -315,6 +315,8 @@ def test_warp_route_ring_reuse(torch_cuda, blink, oracle, monkeypatch):
     assert plan0.query_i32(blink.Q_FUSED_PATH) == 0
     ref = torch.empty((w.n_t, w.n_ch, w.n_pix, w.n_pix), dtype=torch.float32, device="cuda")
     plan0.grid_image(vis, ref)
+    uv = plan0.grid(vis)
+    img_lines = plan0.image(uv)             # blink_image on the line kernels (dense bounding-box read)
     plan0.close()
     monkeypatch.delenv("BLINK_IMAGE_WARP")
     monkeypatch.setenv("BLINK_W_RING", "3")
@@ -327,6 +329,13 @@ def test_warp_route_ring_reuse(torch_cuda, blink, oracle, monkeypatch):
     assert torch.isfinite(img).all()
     peak = ref.abs().amax(dim=(-2, -1), keepdim=True)
     assert ((img - ref).abs() <= 1e-5 * peak).all()
+    assert ((img_lines - ref).abs() <= 1e-5 * peak).all()
+    # blink_image on the same kernel: cell values read from the uv grid at the plan's occupied cells
+    img_uv = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.image(uv, img_uv)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img_uv).all()
+    assert ((img_uv - ref).abs() <= 1e-5 * peak).all()
     n_snap = w.n_t * w.n_ch
     sel = np.array([0, 10, n_snap - 1], np.int64)
     orc = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_h, sel)
