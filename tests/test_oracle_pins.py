@@ -380,3 +380,95 @@ def test_corrections_antenna_swap_conjugates_factor():
     F = oc.correction_factors(ant, freq, gains, cables, 0.1, 0.2)[0, 0]
     Fs = oc.correction_factors(ant[::-1], freq, gains[:, ::-1], cables[::-1], 0.1, 0.2)[0, 0]
     assert abs(Fs - np.conj(F)) < 1e-12 * abs(F)
+
+
+# ------------------------------------------------------------------ dynamic spectra front end (f4)
+def _cube(seed, n_t=9, n_ch=3, n=4):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((n_t, n_ch, n, n)), rng.standard_normal((n_ch, n, n))
+
+
+def test_dynspec_alpha_one_is_difference_with_preceding_image():
+    """alpha = 1: the reference is 'the preceding dirty image' -> numpy.diff along t.
+    Catches a reference that includes the current image or lags by two."""
+    from oracle import dynspec as od
+    img, r0 = _cube(1)
+    dyn, r_out = od.dynamic_spectra(img, 1.0, r0)
+    want = np.diff(np.concatenate([r0[None], img], axis=0), axis=0)        # [t][ch][y][x]
+    for t in range(img.shape[0]):
+        for ch in range(img.shape[1]):
+            assert np.allclose(dyn[:, :, ch, t], want[t, ch], rtol=0, atol=1e-15)
+    assert np.array_equal(r_out, img[-1])
+
+
+def test_dynspec_alpha_zero_is_fixed_model_image():
+    """alpha = 0: a fixed model / prepared reference is subtracted from every image and
+    returned unchanged."""
+    from oracle import dynspec as od
+    img, r0 = _cube(2)
+    dyn, r_out = od.dynamic_spectra(img, 0.0, r0)
+    assert np.array_equal(np.moveaxis(dyn, (2, 3), (1, 0)), img - r0[None])   # -> [t][ch][y][x]
+    assert np.array_equal(r_out, r0)
+    dyn0, _ = od.dynamic_spectra(img, 0.0)                                  # no reference: the cube itself
+    assert np.array_equal(np.moveaxis(dyn0, (2, 3), (1, 0)), img)
+
+
+def test_dynspec_running_average_closed_form():
+    """0 < alpha < 1: R_t = (1-a)^t R_0 + a sum_{k<t} (1-a)^(t-1-k) I_k, written out with explicit
+    weights (no recurrence).  Catches swapped alpha / (1 - alpha) and an off-by-one in the window."""
+    from oracle import dynspec as od
+    img, r0 = _cube(3, n_t=12)
+    a = 0.3
+    dyn, r_out = od.dynamic_spectra(img, a, r0)
+    n_t = img.shape[0]
+    for t in range(n_t + 1):
+        R = (1 - a) ** t * r0
+        for k in range(t):
+            R = R + a * (1 - a) ** (t - 1 - k) * img[k]
+        if t < n_t:
+            got = np.moveaxis(dyn[:, :, :, t], 2, 0)
+            assert np.max(np.abs(got - (img[t] - R))) < 1e-13
+        else:
+            assert np.max(np.abs(r_out - R)) < 1e-13
+
+
+def test_dynspec_static_sky_vanishes_and_pulse_survives():
+    """The purpose of the step: a static dirty image (side-lobes included) subtracts
+    to zero once the reference has converged, a one-step transient stands out at full amplitude and
+    leaves an echo of -alpha (1-alpha)^(k-1) in the following steps."""
+    from oracle import dynspec as od
+    rng = np.random.default_rng(4)
+    sky = rng.standard_normal((2, 4, 4))
+    img = np.repeat(sky[None], 10, axis=0)
+    img[6, 1, 2, 3] += 5.0
+    a = 0.25
+    dyn, _ = od.dynamic_spectra(img, a, sky)          # reference already equal to the static sky
+    want = np.zeros(10)
+    want[6] = 5.0
+    for k in range(1, 4):
+        want[6 + k] = -a * (1 - a) ** (k - 1) * 5.0
+    assert np.max(np.abs(dyn[2, 3, 1, :] - want)) < 1e-14
+    dyn[2, 3, 1, :] = 0
+    assert np.max(np.abs(dyn)) < 1e-14
+
+
+def test_dynspec_layout_and_batch_chaining():
+    """dyn[y][x][ch][t] is the (channel, time) plane of pixel (y, x), checked with
+    hand-written indices on a cube whose value encodes its own coordinates; two consecutive batches
+    with the state carried over equal one long batch (reading c23)."""
+    from oracle import dynspec as od
+    n_t, n_ch, n = 5, 2, 3
+    img = np.zeros((n_t, n_ch, n, n))
+    for t in range(n_t):
+        for ch in range(n_ch):
+            for y in range(n):
+                for x in range(n):
+                    img[t, ch, y, x] = 1000 * t + 100 * ch + 10 * y + x
+    dyn, _ = od.dynamic_spectra(img, 0.0)
+    assert dyn.shape == (n, n, n_ch, n_t)
+    assert dyn[2, 1, 1, 4] == 4121 and dyn[0, 2, 0, 3] == 3002
+    img, r0 = _cube(5, n_t=11)
+    one, r_one = od.dynamic_spectra(img, 0.4, r0)
+    a, r_a = od.dynamic_spectra(img[:4], 0.4, r0)
+    b, r_b = od.dynamic_spectra(img[4:], 0.4, r_a)
+    assert np.array_equal(np.concatenate([a, b], axis=3), one) and np.array_equal(r_b, r_one)
