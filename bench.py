@@ -178,6 +178,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-corrections", action="store_true",
                     help="skip the side measurement of blink_correct (SURVEY.md 8(f) item f2)")
+    ap.add_argument("--no-dynspec", action="store_true",
+                    help="skip the side measurement of blink_dynspec (SURVEY.md 8(f) item f4)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -287,6 +289,27 @@ def main():
                 "achieved_gbs": c_bytes / (c_ms / 1e3) / 1e9, "gvis_per_s": vis.numel() / (c_ms / 1e3) / 1e9}
         del vis_c
 
+    # ---- side measurement, outside the step: blink_dynspec (f4) on the step's own image cube:
+    # reference subtraction + transpose to [y][x][ch][t]; algorithmic bytes 8 per voxel
+    dyn = None
+    if not args.no_dynspec:
+        state = torch.zeros((w.n_ch, w.n_pix, w.n_pix), dtype=torch.float32, device="cuda")
+        dyn_out = torch.empty((w.n_pix, w.n_pix, w.n_ch, w.n_t), dtype=torch.float32, device="cuda")
+        for _ in range(3):
+            plan.dynspec(img, 0.1, state, dyn_out)
+        barrier()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(stream)
+        for _ in range(args.steps):
+            plan.dynspec(img, 0.1, state, dyn_out)
+        d1.record(stream)
+        barrier()
+        d_ms = d0.elapsed_time(d1) / args.steps
+        d_bytes = 8 * img.numel() + 8 * state.numel()
+        dyn = {"call": "blink_dynspec", "alpha": 0.1, "ms": d_ms, "algorithmic_bytes": d_bytes,
+               "achieved_gbs": d_bytes / (d_ms / 1e3) / 1e9, "images_per_s": n_snap / (d_ms / 1e3)}
+        del dyn_out, state
+
     # ---- end to end: pinned host visibilities in, images back to pinned host memory, per step
     e2e = None
     if not args.no_e2e:
@@ -371,6 +394,7 @@ def main():
                           "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": ab["step"]},
         "side_bounds": side,
         "f2_corrections": dict(corr, frac_of_hbm_peak=corr["achieved_gbs"] / peak) if corr else None,
+        "f4_dynspec": dict(dyn, frac_of_hbm_peak=dyn["achieved_gbs"] / peak) if dyn else None,
         "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
     }
     if not args.no_cpu_baseline:

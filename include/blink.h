@@ -173,6 +173,25 @@ int blink_plan_set_corrections(blink_plan *plan, const double *gains, const doub
 int blink_correct(const blink_plan *plan, const void *vis_in, int n_t, void *vis_out, void *stream);
 
 /*
+ * blink_dynspec -- the stage right after imaging: subtraction of a running reference image and
+ * transposition of the image cube into per-pixel dynamic spectra (the paper
+ * prints no formula, readings DESIGN.md c21-c23).  Per channel and pixel, for t = 0 .. n_t-1:
+ *     D_t = I_t - R_t;   R_{t+1} = (1 - alpha) R_t + alpha I_t;   dynspec[y][x][ch][t] = D_t
+ * alpha = 1: R_t is the preceding dirty image; alpha = 0: a fixed model / prepared image;
+ * 0 < alpha < 1: an exponentially weighted average of the previous images.
+ *   images     DEVICE float32 [n_t][n_ch][N][N] (a blink_image / blink_grid_image output), const
+ *   alpha      in [0, 1] (BLINK_EINVAL otherwise)
+ *   ref_state  DEVICE float32 [n_ch][N][N], in/out: R_0 on entry, R_{n_t} on return, so consecutive
+ *              batches chain like one long batch; NULL = R_0 is zero and no state is kept
+ *   dynspec    DEVICE float32 [N][N][n_ch][n_t], time fastest; completely overwritten; must not
+ *              overlap `images`
+ * Asynchronous on `stream`; no allocation.  Algorithmic bytes: 8 per voxel (+ 8 per (ch, pixel) of
+ * state).  n_t == 0 is a no-op.
+ */
+int blink_dynspec(const blink_plan *plan, const void *images, int n_t, double alpha, void *ref_state,
+                  void *dynspec, void *stream);
+
+/*
  * blink_grid_image -- steps a1-a5 in one call: images straight from visibilities, with no uv grid
  * in HBM at all (the paper's aim of processing "fully inside GPU
  * memory" with minimal I/O).  Same result as blink_grid followed by blink_image

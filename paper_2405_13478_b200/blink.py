@@ -21,7 +21,7 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
 
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create",
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
-           "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct",
+           "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct", "blink_dynspec",
            "blink_image", "blink_host_build_gather", "blink_host_fused_emulate"]
 
 _lib = None
@@ -70,6 +70,8 @@ def load() -> ctypes.CDLL:
     lib.blink_plan_set_corrections.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp]
     lib.blink_correct.restype = ci
     lib.blink_correct.argtypes = [vp, vp, ci, vp, vp]
+    lib.blink_dynspec.restype = ci
+    lib.blink_dynspec.argtypes = [vp, vp, ci, ctypes.c_double, vp, vp, vp]
     lib.blink_host_build_gather.restype = ci
     lib.blink_host_build_gather.argtypes = [vp, ci, ci, vp, vp, vp, vp]
     lib.blink_host_fused_emulate.restype = ci
@@ -224,6 +226,27 @@ class Plan:
         assert out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous() and out.shape == vis.shape
         _check(self._lib.blink_correct(self._h, vis.data_ptr(), vis.shape[0], out.data_ptr(),
                                        _stream_ptr(stream)), "blink_correct")
+        return out
+
+    # ---- dynamic spectra (the stage after imaging)
+    def dynspec(self, images, alpha: float, ref_state=None, out=None, stream=None):
+        """blink_dynspec: images [n_t, n_ch, N, N] -> dynamic spectra [N, N, n_ch, n_t]; ref_state
+        [n_ch, N, N] is updated in place (None: zero reference, no state kept)."""
+        import torch
+        n = self.n_pix
+        assert images.is_cuda and images.dtype == torch.float32 and images.is_contiguous()
+        assert tuple(images.shape[1:]) == (self.n_ch, n, n)
+        n_t = images.shape[0]
+        if ref_state is not None:
+            assert ref_state.is_cuda and ref_state.dtype == torch.float32 and ref_state.is_contiguous()
+            assert tuple(ref_state.shape) == (self.n_ch, n, n)
+        if out is None:
+            out = torch.empty((n, n, self.n_ch, n_t), dtype=torch.float32, device=images.device)
+        assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+        assert tuple(out.shape) == (n, n, self.n_ch, n_t)
+        _check(self._lib.blink_dynspec(self._h, images.data_ptr(), n_t, float(alpha),
+                                       ref_state.data_ptr() if ref_state is not None else None,
+                                       out.data_ptr(), _stream_ptr(stream)), "blink_dynspec")
         return out
 
     # ---- hot path

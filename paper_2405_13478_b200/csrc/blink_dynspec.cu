@@ -1,0 +1,194 @@
+// blink_dynspec.cu -- the stage right after imaging: subtraction of a
+// running reference image and transposition of the image cube into per-pixel dynamic spectra.
+//
+//   "imaging artefacts like side-lobes can be removed by subtracting a reference image of the same
+//    field (formed as a combination of previous images or prepared prior to the processing)"
+//    (PAPER.md:76); the reference "can be the preceding dirty image, some form of an average of the
+//    sequence of previous images ... or a model image"; "once the data cube of images
+//    ... are created, dynamic spectra from all pixels (i.e time series in different directions in
+//    the sky) will be formed".
+//
+// The paper prints no formula; readings DESIGN.md c21-c23.  Per channel and pixel, R_0 handed in:
+//     D_t = I_t - R_t,   R_{t+1} = (1 - alpha) R_t + alpha I_t,   dyn[y][x][ch][t] = D_t
+// alpha = 1: preceding image; alpha = 0: fixed model image; in between: exponential running average.
+//
+// Pure streaming work, 8 bytes per voxel (read the image once, write the spectrum once).  A thread
+// owns one pixel of a 256-pixel tile: it loads 32 time steps of its pixel (each load instruction of a
+// warp is 128 contiguous bytes of an image row, 32 loads in flight per thread, issued one tile ahead
+// so that they overlap the previous tile's barrier and stores), runs the recurrence
+// in registers and drops the differences into a [32 t][256 pixel] shared tile (row stride 257, so both
+// the pixel-major writes and the time-major reads are bank-conflict free); then each warp writes, for
+// 32 pixels in turn, the 32 time steps of one pixel: 128 contiguous bytes of that pixel's spectrum.
+// A CTA walks all channels of its group, so the (channel, time) plane of a pixel is written by one
+// CTA in address order and partially covered 32-byte sectors at channel boundaries merge in L2.
+#include <cmath>
+#include <cstdlib>
+
+#include "blink_internal.h"
+#include "sgather.cuh"
+
+namespace blink {
+
+constexpr int kDsPix = 256;          // pixels per CTA = threads per CTA
+constexpr int kDsT = 32;             // time steps per tile
+constexpr int kDsStride = kDsPix + 1;
+
+template <int MINB>
+__global__ void __launch_bounds__(kDsPix, MINB) k_dynspec(const float *__restrict__ img, float *__restrict__ ref,
+                                                    float *__restrict__ dyn, int n_t, int n_ch, long long nn,
+                                                    int ch_per, float alpha) {
+  __shared__ float tile[kDsT * kDsStride];
+  const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
+  const long long pix0 = (long long)blockIdx.x * kDsPix, pix = pix0 + tid;
+  const int ch_begin = blockIdx.y * ch_per, ch_end = min(n_ch, ch_begin + ch_per);
+  const float beta = 1.0f - alpha;
+  const long long t_stride = (long long)n_ch * nn;
+  const int total = (ch_end - ch_begin) * ((n_t + kDsT - 1) / kDsT);
+  // tiles q = 0 .. total-1 run channel-major; the loads of tile q + 1 (and the reference of a channel
+  // about to start) are issued as soon as tile q's differences sit in shared memory -- v is dead by
+  // then -- so they are in flight during the barrier and the store phase of tile q
+  float v[kDsT];
+  float r_next = 0.0f;
+  auto issue = [&](int ch, int t0) {
+    const float *__restrict__ src = img + (long long)ch * nn + pix + (long long)t0 * t_stride;
+#pragma unroll
+    for (int k = 0; k < kDsT; ++k) v[k] = (t0 + k < n_t) ? __ldcs(src + (long long)k * t_stride) : 0.0f;
+    if (t0 == 0 && ref) r_next = ref[(long long)ch * nn + pix];
+  };
+  if (total > 0) issue(ch_begin, 0);
+  float R = 0.0f;
+  int ch = ch_begin, t0 = 0;
+  for (int q = 0; q < total; ++q) {
+    if (t0 == 0) R = r_next;
+#pragma unroll
+    for (int k = 0; k < kDsT; ++k) {
+      tile[k * kDsStride + tid] = v[k] - R;
+      if (t0 + k < n_t) R = fmaf(alpha, v[k], beta * R);
+    }
+    if (t0 + kDsT >= n_t && ref) ref[(long long)ch * nn + pix] = R;
+    const bool last_tile = t0 + kDsT >= n_t;
+    const int ch_n = last_tile ? ch + 1 : ch, t0_n = last_tile ? 0 : t0 + kDsT;
+    if (q + 1 < total) issue(ch_n, t0_n);
+    __syncthreads();
+    if (t0 + lane < n_t) {
+      float *__restrict__ dst = dyn + ((pix0 + wv * 32) * n_ch + ch) * (long long)n_t + t0 + lane;
+      const long long p_stride = (long long)n_ch * n_t;
+#pragma unroll 8
+      for (int pp = 0; pp < 32; ++pp) __stcs(dst + pp * p_stride, tile[lane * kDsStride + wv * 32 + pp]);
+    }
+    __syncthreads();
+    ch = ch_n;
+    t0 = t0_n;
+  }
+}
+
+// Same work with the loads done by the copy engine: warp 0 posts, per tile, one 1 KB bulk copy
+// (cp.async.bulk, SASS UBLKCP) per time step into a two-stage ring of [32 t][256 pixel] input tiles,
+// completion counted by an mbarrier per stage.  No load instruction, address arithmetic or register
+// staging is left in the threads; a stage is refilled (tile q + 2) as soon as the recurrence of tile q
+// has read it, i.e. before tile q's stores, so one or two tiles per CTA (32-64 KB, two CTAs per SM)
+// are always in flight.  Needs 16-byte aligned image rows (any torch allocation).
+constexpr int kDsStages = 2;
+constexpr size_t kDsTmaSmem = sizeof(float) * (kDsStages * kDsT * kDsPix + kDsT * kDsStride) + 8 * kDsStages;
+
+__global__ void __launch_bounds__(kDsPix, 2) k_dynspec_tma(const float *__restrict__ img, float *__restrict__ ref,
+                                                           float *__restrict__ dyn, int n_t, int n_ch, long long nn,
+                                                           int ch_per, float alpha) {
+  extern __shared__ __align__(128) unsigned char ds_smem[];
+  float *in = reinterpret_cast<float *>(ds_smem);                    // [stage][32 t][256 pixels]
+  float *tile = in + kDsStages * kDsT * kDsPix;                      // [32 t][257]
+  uint64_t *full = reinterpret_cast<uint64_t *>(tile + kDsT * kDsStride);
+  const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
+  const long long pix0 = (long long)blockIdx.x * kDsPix, pix = pix0 + tid;
+  const int ch_begin = blockIdx.y * ch_per, ch_end = min(n_ch, ch_begin + ch_per);
+  const float beta = 1.0f - alpha;
+  const int n_tt = (n_t + kDsT - 1) / kDsT, total = (ch_end - ch_begin) * n_tt;
+  if (tid < kDsStages) mbar_init(full + tid, 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  __syncthreads();
+  // warp 0: post the copies of tile q into stage q % kDsStages (lane k = time step t0 + k)
+  auto issue = [&](int q) {
+    const int ch = ch_begin + q / n_tt, t0 = (q % n_tt) * kDsT, st = q % kDsStages;
+    const int rows = min(kDsT, n_t - t0);
+    if (lane == 0) mbar_expect_tx(full + st, (uint32_t)rows * kDsPix * sizeof(float));
+    __syncwarp();
+    if (lane < rows)
+      bulk_load(in + (st * kDsT + lane) * kDsPix, img + ((long long)(t0 + lane) * n_ch + ch) * nn + pix0,
+                kDsPix * sizeof(float), full + st);
+  };
+  if (wv == 0) {
+    if (total > 0) issue(0);
+    if (total > 1) issue(1);
+  }
+  float R = 0.0f, r_next = (ref && total > 0) ? ref[(long long)ch_begin * nn + pix] : 0.0f;
+  int ch = ch_begin, t0 = 0;
+  for (int q = 0; q < total; ++q) {
+    const int st = q % kDsStages;
+    mbar_wait(full + st, (uint32_t)(q / kDsStages) & 1u);
+    if (t0 == 0) R = r_next;
+    const float *__restrict__ x = in + st * kDsT * kDsPix + tid;
+#pragma unroll
+    for (int k = 0; k < kDsT; ++k) {
+      const float v = x[k * kDsPix];
+      tile[k * kDsStride + tid] = v - R;
+      if (t0 + k < n_t) R = fmaf(alpha, v, beta * R);
+    }
+    const bool last_tile = t0 + kDsT >= n_t;
+    if (last_tile && ref) {
+      ref[(long long)ch * nn + pix] = R;
+      if (ch + 1 < ch_end) r_next = ref[(long long)(ch + 1) * nn + pix];
+    }
+    __syncthreads();                       // stage st has been read by everyone; the difference tile is complete
+    if (wv == 0 && q + kDsStages < total) {
+      fence_async_smem();                  // generic reads of the stage before the copy engine overwrites it
+      issue(q + kDsStages);
+    }
+    if (t0 + lane < n_t) {
+      float *__restrict__ dst = dyn + ((pix0 + wv * 32) * n_ch + ch) * (long long)n_t + t0 + lane;
+      const long long p_stride = (long long)n_ch * n_t;
+#pragma unroll 8
+      for (int pp = 0; pp < 32; ++pp) __stcs(dst + pp * p_stride, tile[lane * kDsStride + wv * 32 + pp]);
+    }
+    __syncthreads();
+    if (last_tile) { ++ch; t0 = 0; } else { t0 += kDsT; }
+  }
+}
+
+}  // namespace blink
+
+extern "C" int blink_dynspec(const blink_plan *p, const void *images, int n_t, double alpha, void *ref_state,
+                             void *dynspec, void *stream) {
+  using namespace blink;
+  if (!p || n_t < 0 || !(alpha >= 0.0 && alpha <= 1.0)) return BLINK_EINVAL;
+  if (n_t == 0) return BLINK_OK;
+  if (!images || !dynspec || images == dynspec) return BLINK_EINVAL;
+  if (((uintptr_t)images & 3) || ((uintptr_t)dynspec & 3) || ((uintptr_t)ref_state & 3)) return BLINK_EINVAL;
+  const long long nn = (long long)p->n_pix * p->n_pix;     // a multiple of 256 for every supported N (>= 32)
+  if (nn % kDsPix) return BLINK_EUNSUPPORTED;
+  const int tiles = (int)(nn / kDsPix);
+  // enough CTAs for three rounds of four per SM; a CTA keeps whole channels.  When a pixel's time row is
+  // not a whole number of 32-byte sectors, an even channel count per CTA keeps the group boundaries
+  // on sector boundaries for even n_t.
+  const int target = p->sm_count * 12;
+  int groups = std::min(p->n_ch, (target + tiles - 1) / tiles);
+  int ch_per = (p->n_ch + groups - 1) / groups;
+  if ((n_t & 7) && (ch_per & 1) && ch_per < p->n_ch) ++ch_per;
+  groups = (p->n_ch + ch_per - 1) / ch_per;
+  static const int route = [] { const char *e = getenv("BLINK_DS_ROUTE"); return e ? atoi(e) : 0; }();   // 1 = register loads
+  const dim3 grid(tiles, groups);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (route != 1 && ((uintptr_t)images & 15) == 0) {
+    static thread_local bool attr_set = false;
+    if (!attr_set) {
+      BLINK_CUDA_TRY(cudaFuncSetAttribute(k_dynspec_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDsTmaSmem), "k_dynspec_tma smem attribute");
+      attr_set = true;
+    }
+    k_dynspec_tma<<<grid, kDsPix, kDsTmaSmem, st>>>((const float *)images, (float *)ref_state, (float *)dynspec, n_t, p->n_ch, nn,
+                                                    ch_per, (float)alpha);
+  } else {
+    k_dynspec<3><<<grid, kDsPix, 0, st>>>((const float *)images, (float *)ref_state, (float *)dynspec, n_t, p->n_ch, nn, ch_per,
+                                          (float)alpha);
+  }
+  BLINK_CUDA_TRY(cudaGetLastError(), "k_dynspec launch");
+  return BLINK_OK;
+}

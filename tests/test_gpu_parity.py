@@ -268,6 +268,29 @@ def test_full_size_station_launch_configuration(torch_cuda, blink, oracle):
     plan.close()
 
 
+def test_full_size_mwa1_launch_configuration(torch_cuda, blink, oracle):
+    """BASELINE.json configs[2] at FULL size (100 t x 24 ch x 8128 bl, 1024^2, uniform weighting) in
+    the launch configuration bench.py times (one blink_grid_image call, 2400 snapshots through the
+    ring of k_img1024); parity on sampled snapshots, every image checked to be fully written."""
+    torch = torch_cuda
+    w = synth.config_mwa1()
+    vis = w.vis()
+    plan = _plan(blink, w)
+    plan.reserve(w.n_t)
+    n_snap = w.n_t * w.n_ch
+    img = torch.full((w.n_t, w.n_ch, w.n_pix, w.n_pix), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(torch.from_numpy(vis).cuda(), img)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(img.view(n_snap, -1).sum(dim=1)).all()), "some image not fully written"
+    sel = np.array([0, 1203, n_snap - 1], np.int64)
+    ref = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel)
+    imh = img.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        peak = np.max(np.abs(ref["images"][q]))
+        assert np.max(np.abs(imh[q] - ref["images"][q])) <= IMG_TOL * peak, f"snapshot {sel[q]}"
+    plan.close()
+
+
 @pytest.mark.parametrize("name", ["tiny", "station", "station128", "mwa1", "station_uniform_32",
                                   "mwa1_natural_64", "station1024"])
 def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name):
@@ -462,4 +485,86 @@ def test_corrected_source_images_to_one_at_centre(torch_cuda, blink):
     c = w.n_pix // 2
     assert abs(img[c, c] - 1.0) <= 1e-5
     assert np.unravel_index(np.argmax(img), img.shape) == (c, c)
+    plan.close()
+
+
+# ------------------------------------------------------------------ dynamic spectra front end (f4)
+DYN_TOL = 1e-5   # of max|I|: the reference is an fp32 recurrence of n_t steps, each (1-a) R + a I with
+                 # |R| <= max|I| (<= 2 ulp per step, damped by (1 - a)); D = I - R adds one rounding
+
+
+@pytest.mark.parametrize("n_pix,n_ch,n_t,alpha", [(32, 3, 1, 1.0), (64, 5, 37, 0.25), (128, 4, 100, 0.1),
+                                                  (256, 2, 33, 1.0), (64, 7, 64, 0.0)])
+def test_dynspec_matches_oracle(torch_cuda, blink, n_pix, n_ch, n_t, alpha):
+    """blink_dynspec against oracle/dynspec.py element by element: ragged time tiles (n_t not a
+    multiple of 32), odd channel counts (channel groups with a short tail), the three kinds of
+    reference (alpha = 1, 0, in between), state in and out, and batch chaining."""
+    torch = torch_cuda
+    from oracle import dynspec as od
+    rng = np.random.default_rng(100 + n_pix + n_t)
+    ant = rng.uniform(-15, 15, (4, 3))
+    freq = 150e6 + 1e5 * np.arange(n_ch)
+    plan = blink.Plan(ant, freq, n_pix, 2.0 / n_pix, synth.NATURAL)
+    img = rng.standard_normal((n_t, n_ch, n_pix, n_pix)).astype(np.float32)
+    r0 = rng.standard_normal((n_ch, n_pix, n_pix)).astype(np.float32)
+    want, r_want = od.dynamic_spectra(img, alpha, r0)
+    scale = float(np.max(np.abs(img)))
+    d_img = torch.from_numpy(img).cuda()
+    state = torch.from_numpy(r0).cuda()
+    out = torch.full((n_pix, n_pix, n_ch, n_t), float("nan"), dtype=torch.float32, device="cuda")
+    plan.dynspec(d_img, alpha, state, out)
+    got = out.cpu().numpy()
+    assert np.all(np.isfinite(got)), "dynamic spectra not fully overwritten"
+    assert np.max(np.abs(got - want)) <= DYN_TOL * scale
+    assert np.max(np.abs(state.cpu().numpy() - r_want)) <= DYN_TOL * scale
+    assert torch.equal(d_img.cpu(), torch.from_numpy(img)), "input cube must not be touched"
+    if alpha in (0.0, 1.0):      # no rounding in the reference at the two ends: only the subtraction rounds
+        assert np.max(np.abs(got - want)) <= 2.0 ** -23 * 2 * scale
+        assert np.array_equal(state.cpu().numpy(), r_want.astype(np.float32))
+    if n_t >= 2:                 # two batches with the state carried over == one batch, bit for bit
+        cut = n_t // 3 + 1
+        st2 = torch.from_numpy(r0).cuda()
+        a = plan.dynspec(d_img[:cut].contiguous(), alpha, st2)
+        b = plan.dynspec(d_img[cut:].contiguous(), alpha, st2)
+        assert torch.equal(torch.cat([a, b], dim=3), out) and torch.equal(st2, state)
+    # no state: zero reference
+    want0, _ = od.dynamic_spectra(img, alpha)
+    got0 = plan.dynspec(d_img, alpha).cpu().numpy()
+    assert np.max(np.abs(got0 - want0)) <= DYN_TOL * scale
+    plan.close()
+
+
+def test_dynspec_edge_cases_and_pipeline(torch_cuda, blink):
+    """Bad arguments refused; n_t = 0 is a no-op; and the whole chain on the GPU: a static sky plus
+    a one-step transient source, imaged by blink_grid_image, leaves only the transient in the
+    dynamic spectra once the reference is the static image."""
+    torch = torch_cuda
+    w = synth.config_tiny()
+    w.n_t = 6
+    plan = _plan(blink, w)
+    with pytest.raises(blink.BlinkError):
+        plan.dynspec(torch.zeros((1, 1, 128, 128), device="cuda"), 1.5)
+    with pytest.raises(blink.BlinkError):
+        plan.dynspec(torch.zeros((1, 1, 128, 128), device="cuda"), float("nan"))
+    assert plan.dynspec(torch.zeros((0, 1, 128, 128), device="cuda"), 0.5).shape == (128, 128, 1, 0)
+    # static sky: V = 2 at the phase centre; transient of flux 3 at pixel (y0, x0), time step 4 only
+    C = 299792458.0
+    ant = np.asarray(w.ant_enu_m, np.float64)
+    y0, x0 = 80, 40
+    l0, m0 = (x0 - 64) * w.pixscale, (y0 - 64) * w.pixscale
+    vis = np.full((w.n_t, 1, w.n_bl), 2.0 + 0j, np.complex64)
+    bl = 0
+    for i in range(ant.shape[0]):
+        for j in range(i + 1, ant.shape[0]):
+            u = (ant[j, 0] - ant[i, 0]) * w.freq_hz[0] / C
+            v = (ant[j, 1] - ant[i, 1]) * w.freq_hz[0] / C
+            vis[4, 0, bl] += 3.0 * np.exp(-2j * np.pi * (u * l0 + v * m0))
+            bl += 1
+    img = plan.grid_image(torch.from_numpy(vis).cuda())
+    state = img[0].clone()                                   # reference = the static dirty image
+    dyn = plan.dynspec(img, 0.0, state).cpu().numpy()
+    series = dyn[y0, x0, 0]
+    assert abs(series[4] - 3.0) < 0.2 * 3.0                  # cell snapping smears an off-lattice source a little
+    assert np.max(np.abs(np.delete(dyn, 4, axis=3))) < 1e-5  # every other time step subtracts to zero
+    assert np.unravel_index(np.argmax(dyn[:, :, 0, 4]), (128, 128)) == (y0, x0)
     plan.close()
