@@ -178,6 +178,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-corrections", action="store_true",
                     help="skip the side measurement of blink_correct (SURVEY.md 8(f) item f2)")
+    ap.add_argument("--no-cufft-ref", action="store_true",
+                    help="skip the library reference (blink_grid + torch.fft.ifft2 = cuFFT C2C + shift/real/scale)")
     ap.add_argument("--no-dynspec", action="store_true",
                     help="skip the side measurement of blink_dynspec (SURVEY.md 8(f) item f4)")
     args = ap.parse_args()
@@ -289,6 +291,53 @@ def main():
                 "achieved_gbs": c_bytes / (c_ms / 1e3) / 1e9, "gvis_per_s": vis.numel() / (c_ms / 1e3) / 1e9}
         del vis_c
 
+    # ---- library reference timed beside the hand-written transform (north_star item 3):
+    # the paper's own design -- a dense batched C2C inverse FFT (cuFFT through torch.fft.ifft2) on the
+    # uv grids of blink_grid, then weighting, fftshift, real part and 1/norm as torch elementwise ops --
+    # on a chunk of the batch that keeps the extra buffers under ~2 GB each.  Context, not the product.
+    cufft = None
+    if not args.no_cufft_ref:
+        per_t = w.n_ch * w.n_pix * w.n_pix * 8
+        n_tc = int(max(1, min(w.n_t, (2 << 30) // per_t)))
+        uv_c = plan.grid(vis[:n_tc].contiguous())
+        scale = torch.tensor([1.0 / plan.norm(c) if plan.norm(c) > 0 else 0.0 for c in range(w.n_ch)],
+                             dtype=torch.float32, device="cuda").view(1, w.n_ch, 1, 1)
+        wgt = None
+        if w.weighting == synth.UNIFORM:
+            cnt = torch.from_numpy(np.stack([plan.counts(c) for c in range(w.n_ch)]).astype(np.float32)).cuda()
+            wgt = torch.where(cnt > 0, 1.0 / cnt.clamp(min=1.0), torch.zeros_like(cnt)).unsqueeze(0)
+
+        def cufft_step():
+            g = uv_c if wgt is None else uv_c * wgt
+            f = torch.fft.ifft2(g, norm="forward")            # unnormalised inverse, e^{+i...}
+            return torch.fft.fftshift(f.real, dim=(-2, -1)) * scale
+        for _ in range(3):
+            ref_img = cufft_step()
+        barrier()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_f = max(1, min(args.steps, 5))
+        f0.record(stream)
+        for _ in range(n_f):
+            ref_img = cufft_step()
+        f1.record(stream)
+        barrier()
+        f_ms = f0.elapsed_time(f1) / n_f
+        ours = plan.image(uv_c)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(stream)
+        for _ in range(n_f):
+            plan.image(uv_c, ours)
+        g1.record(stream)
+        barrier()
+        o_ms = g0.elapsed_time(g1) / n_f
+        peak_img = float(ref_img.abs().max())
+        cufft = {"what": "torch.fft.ifft2 (cuFFT C2C inverse, batched) + weighting/fftshift/real/scale as torch ops, "
+                         "on blink_grid's uv grids", "snapshots": n_tc * w.n_ch, "ms": f_ms,
+                 "images_per_s": n_tc * w.n_ch / (f_ms / 1e3),
+                 "blink_image_ms_same_chunk": o_ms, "blink_image_images_per_s": n_tc * w.n_ch / (o_ms / 1e3),
+                 "max_abs_diff_vs_blink_image_over_peak": float((ours - ref_img).abs().max()) / peak_img}
+        del uv_c, ref_img, ours
+
     # ---- side measurement, outside the step: blink_dynspec (f4) on the step's own image cube:
     # reference subtraction + transpose to [y][x][ch][t]; algorithmic bytes 8 per voxel
     dyn = None
@@ -394,6 +443,7 @@ def main():
                           "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": ab["step"]},
         "side_bounds": side,
         "f2_corrections": dict(corr, frac_of_hbm_peak=corr["achieved_gbs"] / peak) if corr else None,
+        "cufft_reference": cufft,
         "f4_dynspec": dict(dyn, frac_of_hbm_peak=dyn["achieved_gbs"] / peak) if dyn else None,
         "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
     }

@@ -82,74 +82,100 @@ __global__ void __launch_bounds__(kDsPix, MINB) k_dynspec(const float *__restric
   }
 }
 
-// Same work with the loads done by the copy engine: warp 0 posts, per tile, one 1 KB bulk copy
-// (cp.async.bulk, SASS UBLKCP) per time step into a two-stage ring of [32 t][256 pixel] input tiles,
-// completion counted by an mbarrier per stage.  No load instruction, address arithmetic or register
-// staging is left in the threads; a stage is refilled (tile q + 2) as soon as the recurrence of tile q
-// has read it, i.e. before tile q's stores, so one or two tiles per CTA (32-64 KB, two CTAs per SM)
-// are always in flight.  Needs 16-byte aligned image rows (any torch allocation).
-constexpr int kDsStages = 2;
-constexpr size_t kDsTmaSmem = sizeof(float) * (kDsStages * kDsT * kDsPix + kDsT * kDsStride) + 8 * kDsStages;
+// Same work with the loads done by the copy engine and no CTA-wide barrier.  A ninth warp is the
+// producer: per tile it posts one 1 KB bulk copy (cp.async.bulk, SASS UBLKCP) per time step into a ring
+// of three [32 t][256 pixel] stages, completion counted by a `full` mbarrier per stage; it re-arms a
+// stage once the eight consumer warps have arrived on its `empty` mbarrier.  A consumer warp owns 32
+// pixels for the whole kernel and works IN PLACE on its 32 x 32 corner of the stage: recurrence with
+// lane = pixel, the difference of (time k, pixel p) written back to column p ^ k of row k (a
+// permutation of the 32 banks, and the row's inputs have all been read by then), __syncwarp, then
+// stores with lane = time step reading column pp ^ lane of row lane (again a permutation): 128
+// contiguous bytes of one pixel's spectrum per instruction, no bank conflict in either direction and
+// no second buffer.  Two of the three stages (64 KB per CTA, two CTAs per SM) are in flight while a
+// warp works on the third; warps drift apart, so loads, arithmetic and stores of different warps
+// overlap.  Needs 16-byte aligned image rows (any torch allocation).
+constexpr int kDsStages = 3;
+constexpr int kDsWarps = kDsPix / 32;                 // consumer warps
+constexpr size_t kDsTmaSmem = sizeof(float) * kDsStages * kDsT * kDsPix + 16 * kDsStages;
 
-__global__ void __launch_bounds__(kDsPix, 2) k_dynspec_tma(const float *__restrict__ img, float *__restrict__ ref,
-                                                           float *__restrict__ dyn, int n_t, int n_ch, long long nn,
-                                                           int ch_per, float alpha) {
+__global__ void __launch_bounds__(kDsPix + 32, 2) k_dynspec_tma(const float *__restrict__ img, float *__restrict__ ref,
+                                                                float *__restrict__ dyn, int n_t, int n_ch, long long nn,
+                                                                int ch_per, float alpha) {
   extern __shared__ __align__(128) unsigned char ds_smem[];
   float *in = reinterpret_cast<float *>(ds_smem);                    // [stage][32 t][256 pixels]
-  float *tile = in + kDsStages * kDsT * kDsPix;                      // [32 t][257]
-  uint64_t *full = reinterpret_cast<uint64_t *>(tile + kDsT * kDsStride);
+  uint64_t *full = reinterpret_cast<uint64_t *>(in + kDsStages * kDsT * kDsPix);
+  uint64_t *empty = full + kDsStages;
   const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
-  const long long pix0 = (long long)blockIdx.x * kDsPix, pix = pix0 + tid;
+  const long long pix0 = (long long)blockIdx.x * kDsPix;
   const int ch_begin = blockIdx.y * ch_per, ch_end = min(n_ch, ch_begin + ch_per);
-  const float beta = 1.0f - alpha;
   const int n_tt = (n_t + kDsT - 1) / kDsT, total = (ch_end - ch_begin) * n_tt;
-  if (tid < kDsStages) mbar_init(full + tid, 1);
+  if (tid < kDsStages) {
+    mbar_init(full + tid, 1);
+    mbar_init(empty + tid, kDsWarps);
+  }
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();
-  // warp 0: post the copies of tile q into stage q % kDsStages (lane k = time step t0 + k)
-  auto issue = [&](int q) {
-    const int ch = ch_begin + q / n_tt, t0 = (q % n_tt) * kDsT, st = q % kDsStages;
-    const int rows = min(kDsT, n_t - t0);
-    if (lane == 0) mbar_expect_tx(full + st, (uint32_t)rows * kDsPix * sizeof(float));
-    __syncwarp();
-    if (lane < rows)
-      bulk_load(in + (st * kDsT + lane) * kDsPix, img + ((long long)(t0 + lane) * n_ch + ch) * nn + pix0,
-                kDsPix * sizeof(float), full + st);
-  };
-  if (wv == 0) {
-    if (total > 0) issue(0);
-    if (total > 1) issue(1);
+  if (wv == kDsWarps) {
+    // ---------------------------------------------------------------- producer warp (lane k = time step t0 + k)
+    int ch = ch_begin, t0 = 0;
+    for (int q = 0; q < total; ++q) {
+      const int st = q % kDsStages;
+      if (q >= kDsStages) {
+        mbar_wait(empty + st, (uint32_t)(q / kDsStages - 1) & 1u);
+        fence_async_smem();                // the consumers' generic reads before the copy engine overwrites the stage
+      }
+      const int rows = min(kDsT, n_t - t0);
+      if (lane == 0) mbar_expect_tx(full + st, (uint32_t)rows * kDsPix * sizeof(float));
+      __syncwarp();
+      if (lane < rows)
+        bulk_load(in + (st * kDsT + lane) * kDsPix, img + ((long long)(t0 + lane) * n_ch + ch) * nn + pix0,
+                  kDsPix * sizeof(float), full + st);
+      if (t0 + kDsT >= n_t) { ++ch; t0 = 0; } else { t0 += kDsT; }
+    }
+    return;
   }
+  // ------------------------------------------------------------------ consumer warps
+  const float beta = 1.0f - alpha;
+  const long long pix = pix0 + tid;
+  const long long p_stride = (long long)n_ch * n_t;
   float R = 0.0f, r_next = (ref && total > 0) ? ref[(long long)ch_begin * nn + pix] : 0.0f;
   int ch = ch_begin, t0 = 0;
   for (int q = 0; q < total; ++q) {
     const int st = q % kDsStages;
     mbar_wait(full + st, (uint32_t)(q / kDsStages) & 1u);
     if (t0 == 0) R = r_next;
-    const float *__restrict__ x = in + st * kDsT * kDsPix + tid;
+    float *__restrict__ x = in + st * kDsT * kDsPix + wv * 32;   // this warp's corner: x[k * 256 + column]
+    if (t0 + kDsT <= n_t) {
 #pragma unroll
-    for (int k = 0; k < kDsT; ++k) {
-      const float v = x[k * kDsPix];
-      tile[k * kDsStride + tid] = v - R;
-      if (t0 + k < n_t) R = fmaf(alpha, v, beta * R);
+      for (int k = 0; k < kDsT; ++k) {
+        const float v = x[k * kDsPix + lane];
+        x[k * kDsPix + (lane ^ k)] = v - R;
+        R = fmaf(alpha, v, beta * R);
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < kDsT; ++k) {
+        if (t0 + k < n_t) {
+          const float v = x[k * kDsPix + lane];
+          x[k * kDsPix + (lane ^ k)] = v - R;
+          R = fmaf(alpha, v, beta * R);
+        }
+      }
     }
+    __syncwarp();
     const bool last_tile = t0 + kDsT >= n_t;
     if (last_tile && ref) {
       ref[(long long)ch * nn + pix] = R;
       if (ch + 1 < ch_end) r_next = ref[(long long)(ch + 1) * nn + pix];
     }
-    __syncthreads();                       // stage st has been read by everyone; the difference tile is complete
-    if (wv == 0 && q + kDsStages < total) {
-      fence_async_smem();                  // generic reads of the stage before the copy engine overwrites it
-      issue(q + kDsStages);
-    }
     if (t0 + lane < n_t) {
       float *__restrict__ dst = dyn + ((pix0 + wv * 32) * n_ch + ch) * (long long)n_t + t0 + lane;
-      const long long p_stride = (long long)n_ch * n_t;
+      const float *__restrict__ row = x + lane * kDsPix;
 #pragma unroll 8
-      for (int pp = 0; pp < 32; ++pp) __stcs(dst + pp * p_stride, tile[lane * kDsStride + wv * 32 + pp]);
+      for (int pp = 0; pp < 32; ++pp, dst += p_stride) __stcs(dst, row[pp ^ lane]);
     }
-    __syncthreads();
+    __syncwarp();                          // the warp is done with its corner of the stage
+    if (lane == 0) mbar_arrive(empty + st);
     if (last_tile) { ++ch; t0 = 0; } else { t0 += kDsT; }
   }
 }
@@ -183,8 +209,8 @@ extern "C" int blink_dynspec(const blink_plan *p, const void *images, int n_t, d
       BLINK_CUDA_TRY(cudaFuncSetAttribute(k_dynspec_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDsTmaSmem), "k_dynspec_tma smem attribute");
       attr_set = true;
     }
-    k_dynspec_tma<<<grid, kDsPix, kDsTmaSmem, st>>>((const float *)images, (float *)ref_state, (float *)dynspec, n_t, p->n_ch, nn,
-                                                    ch_per, (float)alpha);
+    k_dynspec_tma<<<grid, kDsPix + 32, kDsTmaSmem, st>>>((const float *)images, (float *)ref_state, (float *)dynspec, n_t, p->n_ch, nn,
+                                                         ch_per, (float)alpha);
   } else {
     k_dynspec<3><<<grid, kDsPix, 0, st>>>((const float *)images, (float *)ref_state, (float *)dynspec, n_t, p->n_ch, nn, ch_per,
                                           (float)alpha);

@@ -6,6 +6,7 @@
 // of a snapshot falls from 8 n_bl + 20 N^2 towards 8 n_bl + 4 N^2 bytes.
 #include <algorithm>
 #include <array>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 
@@ -51,6 +52,8 @@ struct FusedParams {
   const unsigned char *gtab;  // [n_ch][n_chunk][tab_stride] phase-S gather tables (see fused_build)
   const uint32_t *gsize;      // [n_ch][n_chunk] bytes of each table (multiple of 16)
   const uint2 *hrec;          // [n_ch][h_max] {pos | j << 16 | flag << 30, weight}; pos 0xFFFF = padding
+  const float2 *hw;           // D > 1: [n_ch][D][h_max] complex phase-H weights of the sub-image rows b (see k_fused)
+  const float2 *pha;          // D > 1: [D][N/2] column phases e^{2 pi i kx a / (D N)} of the sub-image columns a
   const float2 *tw;
   int n_bl, n_ch, n_snap, n_can_max, n_chunk, chunk_vis, nbuf, tab_stride, n_col, h_max;
   uint32_t buf_bytes, off_dedicated, off_S, off_bar;   // byte offsets into dynamic shared memory
@@ -61,7 +64,18 @@ int fused_line_stride(int n_pix) { return ((n_pix + n_pix / 16 + 15) / 16) * 16 
 
 // NZ: the first radix-16 stage of both passes reads inputs r = 0..NZ-1 and 16-NZ..15 only (the
 // bounding box reaches at most NZ * N/16 - 1 cells from the origin); NZ = 8 reads everything.
-template <int N, int THREADS, int NZ>
+//
+// D > 1 (polyphase route for compact arrays on large images): the image has D N x D N pixels but the
+// bounding box still fits an N x N transform (|k| < N/2).  Writing X = D x' + a, Y = D y' + b,
+//   I[Y][X] = sum_k (G[k] e^{2 pi i (kx a + ky b) / (D N)}) e^{2 pi i (kx (x' - N/2) + ky (y' - N/2)) / N},
+// i.e. the image is D*D interleaved N x N images of the SAME cell sums, each with its own unit-modulus
+// factor per cell (odd in k, so the modulated grid stays Hermitian and the two-rows-per-transform
+// trick still holds).  The ky part of the factor is folded into the phase-H weight, the kx part is
+// constant along a column, so it commutes with pass A and is applied when pass B loads the column
+// values.  Phase S runs once per snapshot, phases H and A once per b, pass B once per (b, a) with the
+// a loop innermost; no transform longer than N is ever taken and no zero outside the bounding box is
+// ever touched.
+template <int N, int THREADS, int NZ, int D>
 __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   constexpr int T = N / 16;             // lanes per transform
   constexpr int G = THREADS / T;        // transforms in flight per CTA
@@ -165,27 +179,41 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
 
     // ---- phase H: every bounding-box cell with kx >= 0, weighted, into the column lines --------
     const int kym = ci.ky_max;
+    const int kxm = ci.kx_max;
+    float2 *xl = X + (size_t)grp * LSB;
+#pragma unroll 1
+    for (int sub_b = 0; sub_b < D; ++sub_b) {
     {
-      __syncthreads();                              // all sums done, all chunk buffers released
-      auto place = [&](uint2 r) {
+      __syncthreads();                              // all sums done, all chunk buffers released (sub > 0: pass B done with the lines)
+      auto place = [&](uint2 r, int e) {
         const uint32_t pos = r.x & 0xFFFFu;
         if (pos == 0xFFFFu) return;
         const float2 v = S[(r.x >> 16) & 0x3FFFu];
         const uint32_t flag = r.x >> 30;
-        const float w = __uint_as_float(r.y);
         float2 o;
-        if (flag == kPlaceDirect) o = make_float2(v.x * w, v.y * w);
-        else if (flag == kPlaceConj) o = make_float2(v.x * w, -v.y * w);
-        else o = make_float2((v.x + v.x) * w, 0.f);
+        if constexpr (D == 1) {
+          const float w = __uint_as_float(r.y);
+          if (flag == kPlaceDirect) o = make_float2(v.x * w, v.y * w);
+          else if (flag == kPlaceConj) o = make_float2(v.x * w, -v.y * w);
+          else o = make_float2((v.x + v.x) * w, 0.f);
+        } else {
+          const float2 w = __ldg(p.hw + ((size_t)ch * D + sub_b) * p.h_max + e);
+          float2 z;
+          if (flag == kPlaceDirect) z = v;
+          else if (flag == kPlaceConj) z = make_float2(v.x, -v.y);
+          else z = make_float2(v.x + v.x, 0.f);
+          o = make_float2(z.x * w.x - z.y * w.y, z.x * w.y + z.y * w.x);
+        }
         lines[pos] = o;
       };
 #pragma unroll
-      for (int q = 0; q < kHPer; ++q) place(hr[q]);
-      for (int e = tid + kHPer * THREADS; e < p.h_max; e += THREADS) place(__ldg(hrec + e));
+      for (int q = 0; q < kHPer; ++q) place(hr[q], tid + q * THREADS);
+      for (int e = tid + kHPer * THREADS; e < p.h_max; e += THREADS) place(__ldg(hrec + e), e);
     }
     __syncthreads();
     // the sums are consumed: clear them for the next snapshot (sink and zero slot stay zero)
-    for (int j = tid; j < p.n_can_max; j += THREADS) S[j] = make_float2(0.f, 0.f);
+    if (sub_b == D - 1)
+      for (int j = tid; j < p.n_can_max; j += THREADS) S[j] = make_float2(0.f, 0.f);
 
     // ---- pass A: columns kx = 0..kx_max, in place ----------------------------------------------
     for (int c0 = 0; c0 <= ci.kx_max; c0 += G) {
@@ -218,13 +246,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
     __syncthreads();
 
     // ---- pass B: row pairs (y, y + N/2) --------------------------------------------------------
-    const int kxm = ci.kx_max;
-    float2 *xl = X + (size_t)grp * LSB;
-    float *__restrict__ img = p.img + (size_t)s * N * N;
+    float *__restrict__ img = p.img + (size_t)s * (D * N) * (D * N) + (size_t)sub_b * (D * N);
     for (int q0 = 0; q0 < N / 2; q0 += G) {
       const bool act = q0 + grp < N / 2;
       const int y0 = act ? q0 + grp : 0, y1 = y0 + N / 2;
       const int o0 = pad16(y0), o1 = pad16(y1);
+      // D > 1: the D sub-images of this row pair one after the other, so that the D interleaved
+      // partial writes of every 32-byte sector reach L2 within a microsecond of each other
+#pragma unroll 1
+      for (int sub_a = 0; sub_a < D; ++sub_a) {
       cf32 v[16];
       if (act) {
         // stage-0 inputs Z[idx], idx = t + r*T: r < 8 direct half (a + i b), r >= 8 mirrored half
@@ -245,6 +275,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
           for (int q = 0; q < NZL; ++q) {
             const int r = h == 0 ? q : 16 - NZL + q;
             v[r] = h == 0 ? mk(a[q].x - b[q].y, a[q].y + b[q].x) : mk(a[q].x + b[q].y, b[q].x - a[q].y);
+            if constexpr (D > 1) {
+              // column phase e^{2 pi i kx a / (D N)} of sub-image a: kx = +k for the direct half, -k mirrored
+              const int idx = t + r * T;
+              const int k = h == 0 ? idx : N - idx;
+              if (k <= kxm) {
+                const float2 ph = __ldg(p.pha + sub_a * (N / 2) + k);
+                v[r] = h == 0 ? cmul(v[r], mk(ph.x, ph.y)) : cmul(v[r], mk(ph.x, -ph.y));
+              }
+            }
           }
         }
         F::template compute0_pruned<BM>(v);
@@ -255,10 +294,16 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
       if (act) {
         F::template load<1>(v, t, [&](int idx) { return xl[pad16(idx)]; });
         F::template compute_tw<1>(v, tw1);
-        float *__restrict__ r0 = img + (size_t)y0 * N, *__restrict__ r1 = img + (size_t)y1 * N;
-        F::template store<1>(v, t, [&](int x, cf32 z) { __stcs(r0 + x, z.x); __stcs(r1 + x, z.y); });
+        float *__restrict__ r0 = img + (size_t)y0 * (D * D * N) + sub_a, *__restrict__ r1 = img + (size_t)y1 * (D * D * N) + sub_a;
+        if constexpr (D == 1) {
+          F::template store<1>(v, t, [&](int x, cf32 z) { __stcs(r0 + x, z.x); __stcs(r1 + x, z.y); });
+        } else {
+          F::template store<1>(v, t, [&](int x, cf32 z) { r0[D * x] = z.x; r1[D * x] = z.y; });
+        }
       }
+      }   // sub_a
     }
+    }   // sub_b
     // generic-proxy writes to the lines / exchange area are ordered before the next snapshot's
     // bulk copies into the same bytes; no CTA-wide barrier: a warp that is done moves on to phase S
     // of the next snapshot (its own cell sums, the dedicated buffer) while others finish pass B
@@ -285,15 +330,26 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   int want = 1;
   if (const char *e = getenv("BLINK_FUSED_SMEM")) want = atoi(e);
   const int N = p->n_pix, n_bl = p->n_bl, n_ch = p->n_ch;
-  if (!want || N > 256 || N < 32 || (n_bl & 1) || p->max_smem_optin <= 0) return BLINK_OK;
+  if (!want || N < 32 || (n_bl & 1) || p->max_smem_optin <= 0) return BLINK_OK;
+  // polyphase route (see k_fused): a compact array on a large image is imaged as D x D interleaved
+  // Ns x Ns sub-images, Ns = 256, when the bounding box fits the Ns transform
+  int Ns = N, D = 1;
+  if (N > 256) {
+    int poly = 1;
+    if (const char *e = getenv("BLINK_FUSED_POLY")) poly = atoi(e);
+    Ns = 256;
+    D = N / Ns;
+    if (!poly || D > 4 || std::max(p->kx_max_all, p->ky_max_all) >= Ns / 2) return BLINK_OK;
+  }
+  p->fused_D = D;
   const int sink0 = (p->n_can_max + 15) & ~15;                    // S[sink0 + b]: the always-zero slot of bank b
   const int n_S = sink0 + 16;
   if (n_S > 0x3FFF) return BLINK_OK;                              // 14-bit slot index in the phase-H records
-  const int LS = fused_line_stride(N);
+  const int LS = fused_line_stride(Ns);
   const int n_col = p->kx_max_all + 1;
   if ((size_t)n_col * LS >= 0xFFFFu) return BLINK_OK;             // 16-bit line position
-  const int T = N / 16, G = kFusedThreads / T;
-  const size_t region = sizeof(float2) * ((size_t)n_col * LS + (size_t)G * (N + N / 16));
+  const int T = Ns / 16, G = kFusedThreads / T;
+  const size_t region = sizeof(float2) * ((size_t)n_col * LS + (size_t)G * (Ns + Ns / 16));
   const size_t region_al = (region + 127) / 128 * 128;
   const size_t s_bytes = sizeof(float2) * (size_t)n_S;
   const size_t limit = (size_t)p->max_smem_optin;
@@ -376,8 +432,12 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
       h_size[cp] = (uint32_t)b.size();
     }
 
-  // phase-H records: every bounding-box cell with kx >= 0, column by column
+  // phase-H records: every bounding-box cell with kx >= 0, column by column; for D > 1 also the
+  // complex weight of every record in every sub-image (a, b): w e^{2 pi i (kx a + ky b) / N}
   std::vector<std::vector<uint2>> hrecs(n_ch);
+  std::vector<std::vector<float2>> hws(n_ch);       // [sub][record], records in hrecs order
+  struct HCell { int kx, ky; double w; };
+  std::vector<std::vector<HCell>> hcells(n_ch);
   p->h_max = 0;
   for (int ch = 0; ch < n_ch; ++ch) {
     const HostGather &g = gathers[ch];
@@ -394,8 +454,9 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
         const bool canonical = (ky > 0) || (ky == 0 && kx >= 0);
         const int c = canonical ? iy * N + ix : ((N - iy) % N) * N + ((N - ix) % N);
         const int j = find_j(c);
-        const uint32_t pos = (uint32_t)(kx * LS + pad16h(iy));
+        const uint32_t pos = (uint32_t)(kx * LS + pad16h((ky + Ns) % Ns));
         uint2 r;
+        double wd = 0.0;
         if (j < 0) {
           r = make_uint2(pos | ((uint32_t)sink0 << 16), 0u);                    // a zero slot x 0
         } else {
@@ -403,18 +464,41 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
           if (c == 0) cnt *= 2;
           float w = ((kx + ky) & 1) ? -ci.inv_norm : ci.inv_norm;
           if (p->weighting == BLINK_UNIFORM) w /= (float)cnt;
+          wd = (double)w;
           const uint32_t flag = c == 0 ? kPlaceBoth : (canonical ? kPlaceDirect : kPlaceConj);
           uint32_t wb;
           std::memcpy(&wb, &w, 4);
           r = make_uint2(pos | ((uint32_t)slot[ch][j] << 16) | (flag << 30), wb);
         }
         hrecs[ch].push_back(r);
+        hcells[ch].push_back(HCell{kx, ky, wd});
       }
     p->h_max = std::max(p->h_max, (int)hrecs[ch].size());
   }
   std::vector<uint2> h_hrec((size_t)n_ch * std::max(p->h_max, 1), make_uint2(0xFFFFu, 0u));
   for (int ch = 0; ch < n_ch; ++ch)
     std::copy(hrecs[ch].begin(), hrecs[ch].end(), h_hrec.begin() + (size_t)ch * p->h_max);
+  std::vector<float2> h_hw, h_pha;
+  if (D > 1) {
+    h_hw.assign((size_t)n_ch * D * std::max(p->h_max, 1), make_float2(0.f, 0.f));
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int ch = 0; ch < n_ch; ++ch)
+      for (int b = 0; b < D; ++b) {
+        float2 *dst = h_hw.data() + ((size_t)ch * D + b) * p->h_max;
+        for (size_t e = 0; e < hcells[ch].size(); ++e) {
+          const HCell &hc = hcells[ch][e];
+          const int m = ((hc.ky * b) % N + N) % N;               // phase index, exact in integers
+          const double ang = two_pi * (double)m / (double)N;
+          dst[e] = make_float2((float)(hc.w * std::cos(ang)), (float)(hc.w * std::sin(ang)));
+        }
+      }
+    h_pha.resize((size_t)D * (Ns / 2));
+    for (int a = 0; a < D; ++a)
+      for (int k = 0; k < Ns / 2; ++k) {
+        const double ang = two_pi * (double)((k * a) % N) / (double)N;
+        h_pha[(size_t)a * (Ns / 2) + k] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+      }
+  }
 
   auto upload = [&](void **dst, const void *src, size_t bytes) -> int {
     cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
@@ -430,25 +514,35 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   if ((rc = upload((void **)&p->d_gtab, h_tab.data(), h_tab.size())) != BLINK_OK) return rc;
   if ((rc = upload((void **)&p->d_gsize, h_size.data(), sizeof(uint32_t) * h_size.size())) != BLINK_OK) return rc;
   if ((rc = upload((void **)&p->d_hrec, h_hrec.data(), sizeof(uint2) * h_hrec.size())) != BLINK_OK) return rc;
+  if (D > 1) {
+    if ((rc = upload((void **)&p->d_hw, h_hw.data(), sizeof(float2) * h_hw.size())) != BLINK_OK) return rc;
+    if ((rc = upload((void **)&p->d_pha, h_pha.data(), sizeof(float2) * h_pha.size())) != BLINK_OK) return rc;
+    std::vector<float2> h_tws(Ns);                  // exp(+2 pi i m / Ns), the sub-transforms' twiddles
+    for (int m = 0; m < Ns; ++m) {
+      const double ang = 6.283185307179586476925286766559 * (double)m / (double)Ns;
+      h_tws[m] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+    }
+    if ((rc = upload((void **)&p->d_tw_sub, h_tws.data(), sizeof(float2) * h_tws.size())) != BLINK_OK) return rc;
+  }
   BLINK_CUDA_TRY(cudaStreamSynchronize(st), "fused table upload sync");
   p->fused_path = 1;
   return BLINK_OK;
 }
 
-template <int N, int NZ>
+template <int N, int NZ, int D = 1>
 static int launch_fused_n(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
   constexpr int THREADS = kFusedThreads;
   static thread_local size_t smem_set = 0;
   if (p->fused_smem > smem_set) {
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS, NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS, NZ, D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)p->fused_smem), "k_fused smem attribute");
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS, NZ>, cudaFuncAttributePreferredSharedMemoryCarveout, 100),
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS, NZ, D>, cudaFuncAttributePreferredSharedMemoryCarveout, 100),
                    "k_fused carveout");
     smem_set = p->fused_smem;
   }
   const int blocks = std::min(fp.n_snap, p->sm_count);
   if (blocks <= 0) return BLINK_OK;
-  k_fused<N, THREADS, NZ><<<blocks, THREADS, p->fused_smem, st>>>(fp);
+  k_fused<N, THREADS, NZ, D><<<blocks, THREADS, p->fused_smem, st>>>(fp);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_fused launch");
   return BLINK_OK;
 }
@@ -456,15 +550,19 @@ static int launch_fused_n(const blink_plan *p, const FusedParams &fp, cudaStream
 static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st) {
   FusedParams fp;
   fp.vis = vis; fp.img = img; fp.chinfo = p->d_chinfo;
-  fp.gtab = p->d_gtab; fp.gsize = p->d_gsize; fp.hrec = p->d_hrec; fp.tw = p->d_tw;
+  fp.gtab = p->d_gtab; fp.gsize = p->d_gsize; fp.hrec = p->d_hrec; fp.hw = p->d_hw; fp.pha = p->d_pha;
+  fp.tw = p->fused_D > 1 ? p->d_tw_sub : p->d_tw;
   fp.n_bl = p->n_bl; fp.n_ch = p->n_ch; fp.n_snap = n_t * p->n_ch; fp.n_can_max = p->n_can_max;
   fp.n_chunk = p->fused_n_chunk; fp.chunk_vis = p->fused_chunk_vis; fp.nbuf = p->fused_nbuf;
   fp.tab_stride = p->fused_tab_stride; fp.n_col = p->kx_max_all + 1; fp.h_max = p->h_max;
   fp.buf_bytes = p->fused_buf_bytes;
   fp.off_dedicated = p->fused_off_dedicated; fp.off_S = p->fused_off_S; fp.off_bar = p->fused_off_bar;
   // band limit of the first transform stage, in units of N/16 cells
-  const int reach = std::max(p->kx_max_all, p->ky_max_all) + 1, T = p->n_pix / 16;
+  const int n_sub = p->n_pix / p->fused_D;
+  const int reach = std::max(p->kx_max_all, p->ky_max_all) + 1, T = n_sub / 16;
   const int nz = (reach + T - 1) / T;
+  if (p->fused_D == 2) return nz <= 3 ? launch_fused_n<256, 3, 2>(p, fp, st) : launch_fused_n<256, 8, 2>(p, fp, st);
+  if (p->fused_D == 4) return nz <= 3 ? launch_fused_n<256, 3, 4>(p, fp, st) : launch_fused_n<256, 8, 4>(p, fp, st);
   switch (p->n_pix) {
     case 32: return launch_fused_n<32, 8>(p, fp, st);
     case 64: return launch_fused_n<64, 8>(p, fp, st);

@@ -124,6 +124,10 @@ struct blink_plan {
   unsigned char *d_gtab = nullptr;  // [n_ch][n_chunk][tab_stride] phase-S gather tables
   uint32_t *d_gsize = nullptr;      // [n_ch][n_chunk] bytes of each table
   uint2 *d_hrec = nullptr;          // [n_ch][h_max] {line position | j << 16 | flag << 30, weight}
+  int fused_D = 1;                  // polyphase route: the image is fused_D x fused_D interleaved sub-images of n_pix / fused_D
+  float2 *d_hw = nullptr;           // [n_ch][fused_D][h_max] complex phase-H weights of the sub-image rows
+  float2 *d_pha = nullptr;          // [fused_D][n_pix / fused_D / 2] column phases of the sub-image columns
+  float2 *d_tw_sub = nullptr;       // [n_pix / fused_D] twiddles of the sub-transforms
 
 };
 

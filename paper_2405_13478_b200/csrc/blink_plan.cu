@@ -200,7 +200,7 @@ static void plan_free(blink_plan *p) {
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
   cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol); cudaFree(p->d_vrec); cudaFree(p->d_corr); cudaFree(p->d_tw32);
-  cudaFree(p->d_gtab); cudaFree(p->d_gsize); cudaFree(p->d_hrec);
+  cudaFree(p->d_gtab); cudaFree(p->d_gsize); cudaFree(p->d_hrec); cudaFree(p->d_hw); cudaFree(p->d_pha); cudaFree(p->d_tw_sub);
   cudaFree(p->d_rtab); cudaFree(p->d_rsize); cudaFree(p->d_rplace);
   delete p;
 }

@@ -292,7 +292,7 @@ def test_full_size_mwa1_launch_configuration(torch_cuda, blink, oracle):
 
 
 @pytest.mark.parametrize("name", ["tiny", "station", "station128", "mwa1", "station_uniform_32",
-                                  "mwa1_natural_64", "station1024"])
+                                  "mwa1_natural_64", "station512", "station1024"])
 def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name):
     """blink_grid_image (one call, no uv grid in caller memory; shared-memory route where the plan
     allows it, chunked route otherwise) against blink_grid + blink_image (fp32 rounding apart) and
@@ -319,8 +319,43 @@ def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name
         assert plan.query_i32(blink.Q_FUSED_PATH) == 1     # these fit the shared-memory route
     if name == "mwa1":
         assert plan.query_i32(blink.Q_FUSED_PATH) == 2     # wide sparse half-plane at N = 1024: warp route
-    if name == "station1024":
-        assert plan.query_i32(blink.Q_FUSED_PATH) == 0     # compact array at N = 1024: two-kernel route
+    if name in ("station512", "station1024"):
+        assert plan.query_i32(blink.Q_FUSED_PATH) == 1     # compact array on a large image: polyphase shared-memory route
+    plan.close()
+
+
+@pytest.mark.parametrize("n_pix", [512, 1024])
+def test_polyphase_route_matches_two_kernel_route(torch_cuda, blink, oracle, n_pix, monkeypatch):
+    """blink_grid_image on a compact array imaged at 512^2 / 1024^2 with uniform weighting: the
+    polyphase shared-memory route (D x D interleaved 256^2 sub-images of one set of cell sums)
+    against the two-kernel route (BLINK_FUSED_POLY=0) on every snapshot, and against the oracle."""
+    torch = torch_cuda
+    w = synth.config_station(n_t=3, n_ch=3, n_pix=n_pix)
+    w.weighting = synth.UNIFORM
+    vis_h = w.vis()
+    vis = torch.from_numpy(vis_h).cuda()
+    monkeypatch.setenv("BLINK_FUSED_POLY", "0")
+    plan0 = _plan(blink, w)
+    assert plan0.query_i32(blink.Q_FUSED_PATH) == 0
+    ref = plan0.grid_image(vis)
+    plan0.close()
+    monkeypatch.delenv("BLINK_FUSED_POLY")
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 1
+    img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    for _ in range(2):
+        plan.grid_image(vis, img)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img).all(), "image not fully overwritten"
+    peak = ref.abs().amax(dim=(-2, -1), keepdim=True)
+    assert ((img - ref).abs() <= 1e-5 * peak).all()
+    n_snap = w.n_t * w.n_ch
+    sel = np.array([0, 4, n_snap - 1], np.int64)
+    orc = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_h, sel)
+    got = img.view(n_snap, n_pix, n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        pk = np.max(np.abs(orc["images"][q]))
+        assert np.max(np.abs(got[q] - orc["images"][q])) <= IMG_TOL * pk
     plan.close()
 
 
