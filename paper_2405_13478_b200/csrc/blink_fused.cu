@@ -73,7 +73,7 @@ int fused_line_stride(int n_pix) { return ((n_pix + n_pix / 16 + 15) / 16) * 16 
 // trick still holds).  The ky part of the factor is folded into the phase-H weight, the kx part is
 // constant along a column, so it commutes with pass A and is applied when pass B loads the column
 // values.  Phase S runs once per snapshot, phases H and A once per b, pass B once per (b, a) with the
-// a loop innermost; no transform longer than N is ever taken and no zero outside the bounding box is
+// D transform groups of a row pair side by side in a warp; no transform longer than N is ever taken and no zero outside the bounding box is
 // ever touched.
 template <int N, int THREADS, int NZ, int D>
 __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
@@ -131,6 +131,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   // padded lanes and the "zero visibility" padded entries point at)
   const int n_S = ((p.n_can_max + 15) & ~15) + 16;
   for (int j = tid; j < n_S; j += THREADS) S[j] = make_float2(0.f, 0.f);
+  const float2 *pha_s = S + n_S;        // D > 1: [D][N/2] column phases of the sub-images, right after the sums
+  if constexpr (D > 1)
+    for (int j = tid; j < D * (N / 2); j += THREADS) S[n_S + j] = __ldg(p.pha + j);
   // last-stage twiddles w^(r k), k fixed per lane: registers for the whole kernel
   constexpr int R1 = F::template radix<1>();
   constexpr int NB1 = 16 / R1;
@@ -247,14 +250,14 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
 
     // ---- pass B: row pairs (y, y + N/2) --------------------------------------------------------
     float *__restrict__ img = p.img + (size_t)s * (D * N) * (D * N) + (size_t)sub_b * (D * N);
-    for (int q0 = 0; q0 < N / 2; q0 += G) {
-      const bool act = q0 + grp < N / 2;
-      const int y0 = act ? q0 + grp : 0, y1 = y0 + N / 2;
+    // items = (row pair, sub-image column a), a fastest: the D transform groups of one row pair are
+    // neighbours in a warp (D = 2: its two half-warps), so a warp-wide store of one register covers
+    // interleaved pixels D x' + a -- 128 contiguous bytes at D = 2.  a = grp % D is fixed per thread.
+    const int my_a = D > 1 ? grp % D : 0;
+    for (int q0 = 0; q0 < (N / 2) * D; q0 += G) {
+      const bool act = q0 + grp < (N / 2) * D;
+      const int y0 = act ? (q0 + grp) / D : 0, y1 = y0 + N / 2;
       const int o0 = pad16(y0), o1 = pad16(y1);
-      // D > 1: the D sub-images of this row pair one after the other, so that the D interleaved
-      // partial writes of every 32-byte sector reach L2 within a microsecond of each other
-#pragma unroll 1
-      for (int sub_a = 0; sub_a < D; ++sub_a) {
       cf32 v[16];
       if (act) {
         // stage-0 inputs Z[idx], idx = t + r*T: r < 8 direct half (a + i b), r >= 8 mirrored half
@@ -279,10 +282,8 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
               // column phase e^{2 pi i kx a / (D N)} of sub-image a: kx = +k for the direct half, -k mirrored
               const int idx = t + r * T;
               const int k = h == 0 ? idx : N - idx;
-              if (k <= kxm) {
-                const float2 ph = __ldg(p.pha + sub_a * (N / 2) + k);
-                v[r] = h == 0 ? cmul(v[r], mk(ph.x, ph.y)) : cmul(v[r], mk(ph.x, -ph.y));
-              }
+              const float2 ph = pha_s[my_a * (N / 2) + (k & (N / 2 - 1))];
+              v[r] = h == 0 ? cmul(v[r], mk(ph.x, ph.y)) : cmul(v[r], mk(ph.x, -ph.y));
             }
           }
         }
@@ -294,14 +295,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
       if (act) {
         F::template load<1>(v, t, [&](int idx) { return xl[pad16(idx)]; });
         F::template compute_tw<1>(v, tw1);
-        float *__restrict__ r0 = img + (size_t)y0 * (D * D * N) + sub_a, *__restrict__ r1 = img + (size_t)y1 * (D * D * N) + sub_a;
-        if constexpr (D == 1) {
-          F::template store<1>(v, t, [&](int x, cf32 z) { __stcs(r0 + x, z.x); __stcs(r1 + x, z.y); });
-        } else {
-          F::template store<1>(v, t, [&](int x, cf32 z) { r0[D * x] = z.x; r1[D * x] = z.y; });
-        }
+        float *__restrict__ r0 = img + (size_t)y0 * (D * D * N) + my_a, *__restrict__ r1 = img + (size_t)y1 * (D * D * N) + my_a;
+        F::template store<1>(v, t, [&](int x, cf32 z) { __stcs(r0 + D * x, z.x); __stcs(r1 + D * x, z.y); });
       }
-      }   // sub_a
     }
     }   // sub_b
     // generic-proxy writes to the lines / exchange area are ordered before the next snapshot's
@@ -351,7 +347,7 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   const int T = Ns / 16, G = kFusedThreads / T;
   const size_t region = sizeof(float2) * ((size_t)n_col * LS + (size_t)G * (Ns + Ns / 16));
   const size_t region_al = (region + 127) / 128 * 128;
-  const size_t s_bytes = sizeof(float2) * (size_t)n_S;
+  const size_t s_bytes = sizeof(float2) * ((size_t)n_S + (D > 1 ? (size_t)D * (Ns / 2) : 0));   // sums (+ column phases)
   const size_t limit = (size_t)p->max_smem_optin;
 
   std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
