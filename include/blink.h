@@ -196,8 +196,11 @@ int blink_dynspec(const blink_plan *plan, const void *images, int n_t, double al
  * in HBM at all (the paper's aim of processing "fully inside GPU
  * memory" with minimal I/O).  Same result as blink_grid followed by blink_image
  * up to fp32 rounding order (both meet the oracle bars).  Three internal routes, chosen by the plan:
- *   - shared-memory route (BLINK_Q_FUSED_PATH == 1; small bounding box, N <= 256): one kernel;
- *     the gridded half-plane never leaves the SM;
+ *   - shared-memory route (BLINK_Q_FUSED_PATH == 1; small bounding box): one kernel; the gridded
+ *     half-plane never leaves the SM.  N <= 256 directly; N = 512 / 1024 with a bounding box inside
+ *     |k| < 128 (a compact array on a large image) as 2 x 2 / 4 x 4 interleaved 256^2 sub-images of
+ *     the same cell sums (polyphase split of the inverse DFT: each sub-image is the 256^2 transform
+ *     of the grid times a unit-modulus factor per cell);
  *   - warp-per-transform route (BLINK_Q_FUSED_PATH == 2; N = 1024 with a wide, sparsely filled
  *     half-plane, e.g. MWA): one cooperative launch in which one group of CTAs forms the column
  *     transforms as sparse sums straight from the visibilities and a second group runs the row

@@ -331,6 +331,8 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   // Ns x Ns sub-images, Ns = 256, when the bounding box fits the Ns transform
   int Ns = N, D = 1;
   if (N > 256) {
+    // (128-point sub-transforms were measured too: station 256^2 as 2 x 2 of 128^2 0.65 ms against
+    // 0.42 ms direct, sweep512 as 4 x 4 1.92 ms against 1.36 ms as 2 x 2 of 256^2)
     int poly = 1;
     if (const char *e = getenv("BLINK_FUSED_POLY")) poly = atoi(e);
     Ns = 256;
