@@ -94,43 +94,52 @@ __global__ void __launch_bounds__(kDsPix, MINB) k_dynspec(const float *__restric
 // no second buffer.  Two of the three stages (64 KB per CTA, two CTAs per SM) are in flight while a
 // warp works on the third; warps drift apart, so loads, arithmetic and stores of different warps
 // overlap.  Needs 16-byte aligned image rows (any torch allocation).
-constexpr int kDsStages = 3;
-constexpr int kDsWarps = kDsPix / 32;                 // consumer warps
-constexpr size_t kDsTmaSmem = sizeof(float) * kDsStages * kDsT * kDsPix + 16 * kDsStages;
+// Template parameters: P pixels per CTA (P / 32 consumer warps), T time steps per tile (a multiple of
+// 32; a pixel's run of T * 4 bytes is written by T / 32 back-to-back store instructions), STAGES.
+template <int P, int T, int STAGES>
+struct DsCfg {
+  static constexpr int kWarps = P / 32;
+  static constexpr size_t kSmem = sizeof(float) * STAGES * T * P + 16 * STAGES;
+};
 
-__global__ void __launch_bounds__(kDsPix + 32, 2) k_dynspec_tma(const float *__restrict__ img, float *__restrict__ ref,
-                                                                float *__restrict__ dyn, int n_t, int n_ch, long long nn,
-                                                                int ch_per, float alpha) {
+template <int P, int T, int STAGES, int MINB>
+__global__ void __launch_bounds__(P + 32, MINB) k_dynspec_tma(const float *__restrict__ img, float *__restrict__ ref,
+                                                              float *__restrict__ dyn, int n_t, int n_ch, long long nn,
+                                                              int ch_per, float alpha) {
+  constexpr int CW = P / 32;
   extern __shared__ __align__(128) unsigned char ds_smem[];
-  float *in = reinterpret_cast<float *>(ds_smem);                    // [stage][32 t][256 pixels]
-  uint64_t *full = reinterpret_cast<uint64_t *>(in + kDsStages * kDsT * kDsPix);
-  uint64_t *empty = full + kDsStages;
+  float *in = reinterpret_cast<float *>(ds_smem);                    // [stage][T t][P pixels]
+  uint64_t *full = reinterpret_cast<uint64_t *>(in + STAGES * T * P);
+  uint64_t *empty = full + STAGES;
   const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
-  const long long pix0 = (long long)blockIdx.x * kDsPix;
+  const long long pix0 = (long long)blockIdx.x * P;
   const int ch_begin = blockIdx.y * ch_per, ch_end = min(n_ch, ch_begin + ch_per);
-  const int n_tt = (n_t + kDsT - 1) / kDsT, total = (ch_end - ch_begin) * n_tt;
-  if (tid < kDsStages) {
+  const int n_tt = (n_t + T - 1) / T, total = (ch_end - ch_begin) * n_tt;
+  if (tid < STAGES) {
     mbar_init(full + tid, 1);
-    mbar_init(empty + tid, kDsWarps);
+    mbar_init(empty + tid, CW);
   }
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();
-  if (wv == kDsWarps) {
-    // ---------------------------------------------------------------- producer warp (lane k = time step t0 + k)
+  if (wv == CW) {
+    // ---------------------------------------------------------------- producer warp (lane k = time steps t0 + k + 32 m)
     int ch = ch_begin, t0 = 0;
     for (int q = 0; q < total; ++q) {
-      const int st = q % kDsStages;
-      if (q >= kDsStages) {
-        mbar_wait(empty + st, (uint32_t)(q / kDsStages - 1) & 1u);
+      const int st = q % STAGES;
+      if (q >= STAGES) {
+        mbar_wait(empty + st, (uint32_t)(q / STAGES - 1) & 1u);
         fence_async_smem();                // the consumers' generic reads before the copy engine overwrites the stage
       }
-      const int rows = min(kDsT, n_t - t0);
-      if (lane == 0) mbar_expect_tx(full + st, (uint32_t)rows * kDsPix * sizeof(float));
+      const int rows = min(T, n_t - t0);
+      if (lane == 0) mbar_expect_tx(full + st, (uint32_t)rows * P * sizeof(float));
       __syncwarp();
-      if (lane < rows)
-        bulk_load(in + (st * kDsT + lane) * kDsPix, img + ((long long)(t0 + lane) * n_ch + ch) * nn + pix0,
-                  kDsPix * sizeof(float), full + st);
-      if (t0 + kDsT >= n_t) { ++ch; t0 = 0; } else { t0 += kDsT; }
+#pragma unroll
+      for (int m = 0; m < T / 32; ++m) {
+        const int k = lane + 32 * m;
+        if (k < rows)
+          bulk_load(in + (st * T + k) * P, img + ((long long)(t0 + k) * n_ch + ch) * nn + pix0, P * sizeof(float), full + st);
+      }
+      if (t0 + T >= n_t) { ++ch; t0 = 0; } else { t0 += T; }
     }
     return;
   }
@@ -141,43 +150,73 @@ __global__ void __launch_bounds__(kDsPix + 32, 2) k_dynspec_tma(const float *__r
   float R = 0.0f, r_next = (ref && total > 0) ? ref[(long long)ch_begin * nn + pix] : 0.0f;
   int ch = ch_begin, t0 = 0;
   for (int q = 0; q < total; ++q) {
-    const int st = q % kDsStages;
-    mbar_wait(full + st, (uint32_t)(q / kDsStages) & 1u);
+    const int st = q % STAGES;
+    mbar_wait(full + st, (uint32_t)(q / STAGES) & 1u);
     if (t0 == 0) R = r_next;
-    float *__restrict__ x = in + st * kDsT * kDsPix + wv * 32;   // this warp's corner: x[k * 256 + column]
-    if (t0 + kDsT <= n_t) {
+    float *__restrict__ x = in + st * T * P + wv * 32;   // this warp's corner: x[k * P + column]
+    if (t0 + T <= n_t) {
 #pragma unroll
-      for (int k = 0; k < kDsT; ++k) {
-        const float v = x[k * kDsPix + lane];
-        x[k * kDsPix + (lane ^ k)] = v - R;
+      for (int k = 0; k < T; ++k) {
+        const float v = x[k * P + lane];
+        x[k * P + (lane ^ (k & 31))] = v - R;
         R = fmaf(alpha, v, beta * R);
       }
     } else {
 #pragma unroll
-      for (int k = 0; k < kDsT; ++k) {
+      for (int k = 0; k < T; ++k) {
         if (t0 + k < n_t) {
-          const float v = x[k * kDsPix + lane];
-          x[k * kDsPix + (lane ^ k)] = v - R;
+          const float v = x[k * P + lane];
+          x[k * P + (lane ^ (k & 31))] = v - R;
           R = fmaf(alpha, v, beta * R);
         }
       }
     }
     __syncwarp();
-    const bool last_tile = t0 + kDsT >= n_t;
+    const bool last_tile = t0 + T >= n_t;
     if (last_tile && ref) {
       ref[(long long)ch * nn + pix] = R;
       if (ch + 1 < ch_end) r_next = ref[(long long)(ch + 1) * nn + pix];
     }
-    if (t0 + lane < n_t) {
+    {
       float *__restrict__ dst = dyn + ((pix0 + wv * 32) * n_ch + ch) * (long long)n_t + t0 + lane;
-      const float *__restrict__ row = x + lane * kDsPix;
-#pragma unroll 8
-      for (int pp = 0; pp < 32; ++pp, dst += p_stride) __stcs(dst, row[pp ^ lane]);
+      const float *__restrict__ row = x + lane * P;
+#pragma unroll 4
+      for (int pp = 0; pp < 32; ++pp, dst += p_stride) {
+#pragma unroll
+        for (int m = 0; m < T / 32; ++m)
+          if (t0 + lane + 32 * m < n_t) __stcs(dst + 32 * m, row[32 * m * P + (pp ^ lane)]);
+      }
     }
     __syncwarp();                          // the warp is done with its corner of the stage
     if (lane == 0) mbar_arrive(empty + st);
-    if (last_tile) { ++ch; t0 = 0; } else { t0 += kDsT; }
+    if (last_tile) { ++ch; t0 = 0; } else { t0 += T; }
   }
+}
+
+template <int P, int T, int STAGES, int MINB>
+static int launch_dynspec_tma(const blink_plan *p, const float *images, float *ref_state, float *dynspec, int n_t, double alpha,
+                              cudaStream_t st) {
+  const long long nn = (long long)p->n_pix * p->n_pix;
+  const int tiles = (int)(nn / P);
+  // enough CTAs for a few rounds per SM; a CTA keeps whole channels.  When a pixel's time row is not a
+  // whole number of 32-byte sectors, an even channel count per CTA keeps the group boundaries on
+  // sector boundaries for even n_t.
+  const int target = p->sm_count * 12;
+  int groups = std::min(p->n_ch, (target + tiles - 1) / tiles);
+  int ch_per = (p->n_ch + groups - 1) / groups;
+  if ((n_t & 7) && (ch_per & 1) && ch_per < p->n_ch) ++ch_per;
+  groups = (p->n_ch + ch_per - 1) / ch_per;
+  constexpr size_t smem = DsCfg<P, T, STAGES>::kSmem;
+  static thread_local bool attr_set = false;
+  if (!attr_set) {
+    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_dynspec_tma<P, T, STAGES, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
+                   "k_dynspec_tma smem attribute");
+    attr_set = true;
+  }
+  k_dynspec_tma<P, T, STAGES, MINB><<<dim3(tiles, groups), P + 32, smem, st>>>(images, ref_state, dynspec, n_t, p->n_ch, nn, ch_per,
+                                                                               (float)alpha);
+  BLINK_CUDA_TRY(cudaGetLastError(), "k_dynspec_tma launch");
+  return BLINK_OK;
 }
 
 }  // namespace blink
@@ -191,30 +230,28 @@ extern "C" int blink_dynspec(const blink_plan *p, const void *images, int n_t, d
   if (((uintptr_t)images & 3) || ((uintptr_t)dynspec & 3) || ((uintptr_t)ref_state & 3)) return BLINK_EINVAL;
   const long long nn = (long long)p->n_pix * p->n_pix;     // a multiple of 256 for every supported N (>= 32)
   if (nn % kDsPix) return BLINK_EUNSUPPORTED;
+  static const int route = [] { const char *e = getenv("BLINK_DS_ROUTE"); return e ? atoi(e) : 0; }();   // 1 = register loads
+  cudaStream_t st = (cudaStream_t)stream;
+  if (route != 1 && ((uintptr_t)images & 15) == 0) {
+    const float *im = (const float *)images;
+    float *rs = (float *)ref_state, *ds = (float *)dynspec;
+    switch (route) {   // tile shapes kept for comparison (K5); 0 = default
+      case 2: return launch_dynspec_tma<128, 64, 3, 2>(p, im, rs, ds, n_t, alpha, st);
+      case 3: return launch_dynspec_tma<128, 64, 2, 3>(p, im, rs, ds, n_t, alpha, st);
+      case 4: return launch_dynspec_tma<64, 128, 3, 2>(p, im, rs, ds, n_t, alpha, st);
+      case 5: return launch_dynspec_tma<64, 128, 2, 3>(p, im, rs, ds, n_t, alpha, st);
+      case 6: return launch_dynspec_tma<128, 128, 3, 1>(p, im, rs, ds, n_t, alpha, st);
+      default: return launch_dynspec_tma<256, 32, 3, 2>(p, im, rs, ds, n_t, alpha, st);
+    }
+  }
   const int tiles = (int)(nn / kDsPix);
-  // enough CTAs for three rounds of four per SM; a CTA keeps whole channels.  When a pixel's time row is
-  // not a whole number of 32-byte sectors, an even channel count per CTA keeps the group boundaries
-  // on sector boundaries for even n_t.
   const int target = p->sm_count * 12;
   int groups = std::min(p->n_ch, (target + tiles - 1) / tiles);
   int ch_per = (p->n_ch + groups - 1) / groups;
   if ((n_t & 7) && (ch_per & 1) && ch_per < p->n_ch) ++ch_per;
   groups = (p->n_ch + ch_per - 1) / ch_per;
-  static const int route = [] { const char *e = getenv("BLINK_DS_ROUTE"); return e ? atoi(e) : 0; }();   // 1 = register loads
-  const dim3 grid(tiles, groups);
-  cudaStream_t st = (cudaStream_t)stream;
-  if (route != 1 && ((uintptr_t)images & 15) == 0) {
-    static thread_local bool attr_set = false;
-    if (!attr_set) {
-      BLINK_CUDA_TRY(cudaFuncSetAttribute(k_dynspec_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kDsTmaSmem), "k_dynspec_tma smem attribute");
-      attr_set = true;
-    }
-    k_dynspec_tma<<<grid, kDsPix + 32, kDsTmaSmem, st>>>((const float *)images, (float *)ref_state, (float *)dynspec, n_t, p->n_ch, nn,
-                                                         ch_per, (float)alpha);
-  } else {
-    k_dynspec<3><<<grid, kDsPix, 0, st>>>((const float *)images, (float *)ref_state, (float *)dynspec, n_t, p->n_ch, nn, ch_per,
-                                          (float)alpha);
-  }
+  k_dynspec<3><<<dim3(tiles, groups), kDsPix, 0, st>>>((const float *)images, (float *)ref_state, (float *)dynspec, n_t, p->n_ch, nn,
+                                                       ch_per, (float)alpha);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_dynspec launch");
   return BLINK_OK;
 }
