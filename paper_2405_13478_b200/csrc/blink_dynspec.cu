@@ -83,16 +83,16 @@ __global__ void __launch_bounds__(kDsPix, MINB) k_dynspec(const float *__restric
 }
 
 // Same work with the loads done by the copy engine and no CTA-wide barrier.  A ninth warp is the
-// producer: per tile it posts one 1 KB bulk copy (cp.async.bulk, SASS UBLKCP) per time step into a ring
-// of three [32 t][256 pixel] stages, completion counted by a `full` mbarrier per stage; it re-arms a
-// stage once the eight consumer warps have arrived on its `empty` mbarrier.  A consumer warp owns 32
-// pixels for the whole kernel and works IN PLACE on its 32 x 32 corner of the stage: recurrence with
-// lane = pixel, the difference of (time k, pixel p) written back to column p ^ k of row k (a
+// producer: per tile it posts one bulk copy (cp.async.bulk, SASS UBLKCP) of P pixels per time step into
+// a ring of [T t][P pixel] stages, completion counted by a `full` mbarrier per stage; it re-arms a
+// stage once the consumer warps have arrived on its `empty` mbarrier.  A consumer warp owns 32
+// pixels for the whole kernel and works IN PLACE on its T x 32 corner of the stage: recurrence with
+// lane = pixel, the difference of (time k, pixel p) written back to column p ^ (k mod 32) of row k (a
 // permutation of the 32 banks, and the row's inputs have all been read by then), __syncwarp, then
-// stores with lane = time step reading column pp ^ lane of row lane (again a permutation): 128
-// contiguous bytes of one pixel's spectrum per instruction, no bank conflict in either direction and
-// no second buffer.  Two of the three stages (64 KB per CTA, two CTAs per SM) are in flight while a
-// warp works on the third; warps drift apart, so loads, arithmetic and stores of different warps
+// stores with lane = time step reading column pp ^ lane of rows lane + 32 m (again a permutation):
+// 128 contiguous bytes of one pixel's spectrum per instruction, T / 32 instructions back to back per
+// pixel, no bank conflict in either direction and no second buffer.  The other stage(s) are in flight
+// while a warp works on one; warps drift apart, so loads, arithmetic and stores of different warps
 // overlap.  Needs 16-byte aligned image rows (any torch allocation).
 // Template parameters: P pixels per CTA (P / 32 consumer warps), T time steps per tile (a multiple of
 // 32; a pixel's run of T * 4 bytes is written by T / 32 back-to-back store instructions), STAGES.
@@ -235,14 +235,12 @@ extern "C" int blink_dynspec(const blink_plan *p, const void *images, int n_t, d
   if (route != 1 && ((uintptr_t)images & 15) == 0) {
     const float *im = (const float *)images;
     float *rs = (float *)ref_state, *ds = (float *)dynspec;
-    switch (route) {   // tile shapes kept for comparison (K5); 0 = default
-      case 2: return launch_dynspec_tma<128, 64, 3, 2>(p, im, rs, ds, n_t, alpha, st);
-      case 3: return launch_dynspec_tma<128, 64, 2, 3>(p, im, rs, ds, n_t, alpha, st);
-      case 4: return launch_dynspec_tma<64, 128, 3, 2>(p, im, rs, ds, n_t, alpha, st);
-      case 5: return launch_dynspec_tma<64, 128, 2, 3>(p, im, rs, ds, n_t, alpha, st);
-      case 6: return launch_dynspec_tma<128, 128, 3, 1>(p, im, rs, ds, n_t, alpha, st);
-      default: return launch_dynspec_tma<256, 32, 3, 2>(p, im, rs, ds, n_t, alpha, st);
-    }
+    // tile shape: 128 pixels x 64 time steps, two stages, three CTAs per SM.  Measured on the station
+    // cube (n_t = 100), ms per call: <256,32,3> 0.368, <128,32,3> 0.378, <128,64,3> 0.335, <128,64,2> 0.331,
+    // <64,64,3> 0.338, <256,64,2> 0.376, <64,128,2> 0.393, <128,128,3> 0.492, <64,128,3> 0.505: longer runs
+    // per pixel on the write side pay until too few consumer warps are left per SM.
+    if (route == 10) return launch_dynspec_tma<256, 32, 3, 2>(p, im, rs, ds, n_t, alpha, st);
+    return launch_dynspec_tma<128, 64, 2, 3>(p, im, rs, ds, n_t, alpha, st);
   }
   const int tiles = (int)(nn / kDsPix);
   const int target = p->sm_count * 12;
