@@ -57,6 +57,12 @@ __device__ __forceinline__ int ld_acquire(const int *p) {
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
+__device__ __forceinline__ int ld_relaxed(const int *p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 struct WItem { int kind, snap, idx; };   // kind 0 = pass A, 1 = pass B, -1 = none
@@ -296,6 +302,10 @@ __global__ void __launch_bounds__(kWThreads, 2) k_img1024(const WParams q) {
       // this warp's share of the snapshot's U has been consumed: the bulk copies have completed (the
       // mbarrier said so) and the values are in registers, so a relaxed add is enough to let the slot go
       if (lane == 0) atomicAdd(q.done_b + s, 1);
+      // the next item's pass-A counter: a relaxed load issued now, its round trip to L2 hidden behind the
+      // inner butterflies; the acquire fence follows only if the count says the rows are there
+      int cnt_next = 0;
+      if (nxt.kind == 1 && lane == 0) cnt_next = ld_relaxed(q.done_a + nxt.snap);
       wf_inner(t, lane, [&](int i) { return tws[i]; });
       wf_put(tile, lane, t);
       __syncwarp();
@@ -305,8 +315,11 @@ __global__ void __launch_bounds__(kWThreads, 2) k_img1024(const WParams q) {
       if (nxt.kind == 1) {               // rows of the next item, if its pass A is already complete
         int ready = 0;
         if (lane == 0) {
-          ready = ld_acquire(q.done_a + nxt.snap) >= q.items_a;
-          if (ready) issue_rows(q, nxt, wv, tile, bar);
+          ready = cnt_next >= q.items_a;
+          if (ready) {
+            fence_acq_rel_gpu();
+            issue_rows(q, nxt, wv, tile, bar);
+          }
         }
         pending = __shfl_sync(0xffffffffu, ready, 0) != 0;
       }
