@@ -116,3 +116,32 @@ def test_fft_stage_algebra_on_host(tmp_path):
                     "-o", exe], check=True)
     out = subprocess.run([exe], capture_output=True, text=True)
     assert out.returncode == 0 and out.stdout.strip().endswith("OK"), out.stdout
+
+
+def test_polyphase_identity_behind_the_large_image_route():
+    """The identity k_fused<256, ..., D> rests on (blink_fused.cu): for a grid confined to |k| < N'/2,
+    the D N' x D N' image is D x D interleaved N' x N' images of the same cells, each the N' transform
+    of the grid times exp(2 pi i (kx a + ky b) / (D N')).  Checked with numpy's FFT on a random
+    Hermitian band-limited grid, fftshift and centred pixel coordinates included."""
+    rng = np.random.default_rng(12)
+    ns, d, reach = 32, 4, 11
+    n = ns * d
+    g = np.zeros((n, n), np.complex128)           # FFT-native order, DC at [0][0]
+    ks = np.arange(-reach, reach + 1)
+    for ky in ks:
+        for kx in ks:
+            g[ky % n, kx % n] = rng.standard_normal() + 1j * rng.standard_normal()
+    idx = (-np.arange(n)) % n
+    g = g + np.conj(g[idx][:, idx])               # Hermitian
+    full = np.fft.fftshift(np.fft.ifft2(g) * n * n).real        # I[Y][X], pixel (n/2, n/2) = phase centre
+    got = np.empty_like(full)
+    for b in range(d):
+        for a in range(d):
+            gs = np.zeros((ns, ns), np.complex128)
+            for ky in ks:
+                for kx in ks:
+                    gs[ky % ns, kx % ns] = g[ky % n, kx % n] * np.exp(2j * np.pi * (kx * a + ky * b) / n)
+            sub = np.fft.fftshift(np.fft.ifft2(gs) * ns * ns)
+            assert np.max(np.abs(sub.imag)) < 1e-9 * np.max(np.abs(sub.real))   # the modulated grid stays Hermitian
+            got[b::d, a::d] = sub.real
+    assert np.max(np.abs(got - full)) < 1e-10 * np.max(np.abs(full))
