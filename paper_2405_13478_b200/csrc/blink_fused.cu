@@ -10,6 +10,9 @@
 #include <cstdio>
 #include <cstring>
 
+// complex adds as scalar FADDs here: the packed FADD2 form (fft_core.cuh) measured 2 % slower on
+// k_fused<256> (station 0.419 -> 0.427 ms; 6 % faster on k_img1024, which keeps it)
+#define BLINK_SCALAR_COMPLEX
 #include "blink_internal.h"
 #include "fft_core.cuh"
 #include "sgather.cuh"

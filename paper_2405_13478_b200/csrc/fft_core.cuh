@@ -22,8 +22,22 @@ struct cf32 { float x, y; };
 namespace blinkfft {
 
 BLINK_HD cf32 mk(float x, float y) { cf32 r; r.x = x; r.y = y; return r; }
+#if defined(__CUDA_ARCH__) && !defined(BLINK_SCALAR_COMPLEX)
+// sm_100a packed fp32 pairs (SASS FADD2): one issue slot per complex add; same rounding as two FADDs
+__device__ __forceinline__ cf32 cadd(cf32 a, cf32 b) {
+  unsigned long long r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(reinterpret_cast<const unsigned long long &>(a)), "l"(reinterpret_cast<const unsigned long long &>(b)));
+  return reinterpret_cast<const cf32 &>(r);
+}
+__device__ __forceinline__ cf32 csub(cf32 a, cf32 b) {
+  unsigned long long r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(reinterpret_cast<const unsigned long long &>(a)), "l"(reinterpret_cast<const unsigned long long &>(b)));
+  return reinterpret_cast<const cf32 &>(r);
+}
+#else
 BLINK_HD cf32 cadd(cf32 a, cf32 b) { return mk(a.x + b.x, a.y + b.y); }
 BLINK_HD cf32 csub(cf32 a, cf32 b) { return mk(a.x - b.x, a.y - b.y); }
+#endif
 BLINK_HD cf32 cmul(cf32 a, cf32 b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 BLINK_HD cf32 cconj(cf32 a) { return mk(a.x, -a.y); }
 BLINK_HD cf32 mul_i(cf32 a) { return mk(-a.y, a.x); }   // a * (+i)
