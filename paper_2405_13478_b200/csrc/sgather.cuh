@@ -77,6 +77,20 @@ template <int L> __device__ __forceinline__ void fold_group(const GroupIdx &gi, 
   }
   uint32_t sa;
   asm volatile("mad.lo.u32 %2, %3, 8, %4;\nld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(a.x), "=f"(a.y), "=r"(sa) : "r"(gi.j), "r"(S_base));
+#if defined(BLINK_PHASE_S_PACKED)
+  // packed fp32 pairs (SASS FADD2): one issue slot per visibility added; same sums in the same order
+#pragma unroll
+  for (int r = 0; r < L; ++r) v[r].y = __uint_as_float(__float_as_uint(v[r].y) ^ ((uint32_t)gi.e[r] & 0x80000000u));
+  unsigned long long acc = reinterpret_cast<const unsigned long long &>(v[0]);
+#pragma unroll
+  for (int r = 1; r < L; ++r)
+    asm("add.rn.f32x2 %0, %0, %1;" : "+l"(acc) : "l"(reinterpret_cast<const unsigned long long &>(v[r])));
+  {
+    unsigned long long aa = reinterpret_cast<const unsigned long long &>(a);
+    asm("add.rn.f32x2 %0, %0, %1;" : "+l"(aa) : "l"(acc));
+    a = reinterpret_cast<const float2 &>(aa);
+  }
+#else
   float ax = v[0].x, ay = __uint_as_float(__float_as_uint(v[0].y) ^ ((uint32_t)gi.e[0] & 0x80000000u));
 #pragma unroll
   for (int r = 1; r < L; ++r) {
@@ -85,6 +99,7 @@ template <int L> __device__ __forceinline__ void fold_group(const GroupIdx &gi, 
   }
   a.x += ax;
   a.y += ay;
+#endif
   asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(sa), "f"(a.x), "f"(a.y) : "memory");
 }
 
