@@ -48,7 +48,8 @@ def algorithmic_bytes(w):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch at the bench's own
 # size, from `ncu --set full` captures (profiles/r01_README.md); None where no capture exists
-NCU_TRAFFIC_BYTES = {("station", "fused", 100): 848_063_232 + 784_796_416}
+NCU_TRAFFIC_BYTES = {("station", "fused", 100): 848_063_232 + 784_796_416,      # k_fused<256,512,3,1>
+                     ("mwa1", "fused", 100): 175_624_704 + 10_052_818_000}      # k_img1024 (profiles/r01aa_k_img1024_summary.txt)
 
 
 def measured_peaks():
