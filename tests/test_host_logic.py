@@ -145,3 +145,24 @@ def test_polyphase_identity_behind_the_large_image_route():
             assert np.max(np.abs(sub.imag)) < 1e-9 * np.max(np.abs(sub.real))   # the modulated grid stays Hermitian
             got[b::d, a::d] = sub.real
     assert np.max(np.abs(got - full)) < 1e-10 * np.max(np.abs(full))
+
+
+def test_bench_reference_arm_runs_on_cpu_and_prints_the_contract_line():
+    """`bench.py --impl reference` times the oracle on the host cores and prints ONE JSON line with the
+    contract's keys (no GPU involved; rank 0 only under torchrun)."""
+    import json
+    import sys
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "tiny",
+                          "--steps", "1", "--warmup", "1"], capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-500:]
+    lines = [l for l in out.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == "dirty_images_per_s" and d["unit"] == "images/s"
+    assert d["value"] > 0 and d["higher_is_better"] is True and d["gpu_launches"] == 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    other = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "tiny",
+                            "--steps", "1", "--warmup", "1"], capture_output=True, text=True, timeout=300, env=env)
+    assert other.returncode == 0 and other.stdout.strip() == ""      # the other ranks exit 0 without work
