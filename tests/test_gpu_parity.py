@@ -291,6 +291,30 @@ def test_full_size_mwa1_launch_configuration(torch_cuda, blink, oracle):
     plan.close()
 
 
+def test_full_size_sweep512_launch_configuration(torch_cuda, blink, oracle):
+    """BASELINE.json configs[4] at 512^2, FULL size (1000 t x 4 ch x 32640 bl: the dispersed-pulse
+    sweep) in the launch configuration bench.py times: one blink_grid_image call on the polyphase
+    shared-memory route, 4000 snapshots over 148 persistent CTAs; parity on sampled snapshots, every
+    image checked to be fully written."""
+    torch = torch_cuda
+    w = synth.config_sweep(512)
+    vis = w.vis()
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 1
+    n_snap = w.n_t * w.n_ch
+    img = torch.full((w.n_t, w.n_ch, w.n_pix, w.n_pix), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(torch.from_numpy(vis).cuda(), img)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(img.view(n_snap, -1).sum(dim=1)).all()), "some image not fully written"
+    sel = np.array([0, 1777, n_snap - 1], np.int64)
+    ref = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel)
+    imh = img.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        peak = np.max(np.abs(ref["images"][q]))
+        assert np.max(np.abs(imh[q] - ref["images"][q])) <= IMG_TOL * peak, f"snapshot {sel[q]}"
+    plan.close()
+
+
 @pytest.mark.parametrize("name", ["tiny", "station", "station128", "mwa1", "station_uniform_32",
                                   "mwa1_natural_64", "station512", "station1024"])
 def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name):
