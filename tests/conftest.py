@@ -17,3 +17,18 @@ def oracle():
     from oracle import oracle as orc
     orc.build()
     return orc
+
+
+@pytest.fixture(scope="session")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test run without a CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="session")
+def blink():
+    from paper_2405_13478_b200 import blink as b
+    b.load()  # raises if libblink.so is missing: there is no fallback
+    return b

@@ -1,0 +1,139 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configurations bench.py times: one
+blink_grid_image call over the whole batch (persistent CTAs that image many snapshots each), NaN-
+prefilled outputs, every image checked to be written, sampled snapshots against the CPU oracle at
+the north_star bar (max|d| <= 1e-4 * image peak).  Plus the sizes the library accepts but the
+small-case tests never reach (4096^2 through blink_grid_image, N = 2048)."""
+import numpy as np
+import pytest
+
+from paper_2405_13478_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+GRID_TOL = 1e-5
+IMG_TOL = 1e-4
+
+
+def _plan(blink, w, **kw):
+    return blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, **kw)
+
+
+def _fullsize_grid_image(torch, blink, oracle, w, sel, expect_path):
+    vis = w.vis()
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == expect_path
+    n_snap = w.n_t * w.n_ch
+    img = torch.full((w.n_t, w.n_ch, w.n_pix, w.n_pix), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(torch.from_numpy(vis).cuda(), img)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(img.view(n_snap, -1).sum(dim=1)).all()), "some image not fully written"
+    sel = np.asarray(sel, np.int64)
+    ref = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel)
+    imh = img.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        peak = np.max(np.abs(ref["images"][q]))
+        err = np.max(np.abs(imh[q] - ref["images"][q]))
+        assert err <= IMG_TOL * peak, f"snapshot {sel[q]}: err {err:.3e} peak {peak:.3e}"
+    plan.close()
+
+
+def test_full_size_station_grid_image(torch_cuda, blink, oracle):
+    """BASELINE.json configs[1] at FULL size through blink_grid_image -- the kernel instance bench.py's
+    headline times (k_fused<256,512,3,1>: 3200 snapshots over 148 persistent CTAs, > 21 snapshots per
+    CTA, so the hand-off between snapshots -- region_free, the next snapshot's chunk 0 in the dedicated
+    buffer, the clearing of the cell sums -- is what is being tested).  Sampled snapshots include the
+    first one of a CTA's second round (148), mid-batch ones and the last."""
+    w = synth.config_station()
+    n_snap = w.n_t * w.n_ch
+    _fullsize_grid_image(torch_cuda, blink, oracle, w, [0, 147, 148, 149, 777, 1600, 3051, n_snap - 1], 1)
+
+
+@pytest.mark.parametrize("n_pix,sel", [(128, [0, 148, 2222, 3999]), (256, [0, 148, 2222, 3999]),
+                                       (1024, [0, 149, 3999])])
+def test_full_size_sweep_grid_image(torch_cuda, blink, oracle, n_pix, sel):
+    """BASELINE.json configs[4] (1000 t x 4 coarse channels x 32640 bl, dispersed pulse) at 128^2,
+    256^2 and 1024^2 (512^2 is in test_gpu_parity.py), full size, one blink_grid_image call: direct
+    shared-memory route at 128 / 256, polyphase D = 4 at 1024."""
+    w = synth.config_sweep(n_pix)
+    _fullsize_grid_image(torch_cuda, blink, oracle, w, sel, 1)
+
+
+def _sampled_pixel_check(oracle, w, vis, s, im, yx, uv=None):
+    """One snapshot of a large image against the oracle on sampled pixels (literal sums over the
+    occupied cells), the peak taken at the GPU image's arg-max and cross-checked there."""
+    n = w.n_pix
+    ch = s % w.n_ch
+    r = oracle.uv_cells(w.ant_enu_m, w.freq_hz[ch], n, w.pixscale)
+    g_ref, cnt = oracle.grid(r["cell"], r["cell_conj"], vis[s // w.n_ch, ch], n)
+    if uv is not None:
+        assert np.max(np.abs(uv - g_ref)) <= GRID_TOL * np.max(np.abs(g_ref))
+        assert np.all(uv[g_ref == 0] == 0)
+    gw, norm = oracle.weight(g_ref, cnt, w.weighting)
+    yp, xp = np.unravel_index(np.argmax(np.abs(im)), im.shape)
+    peak = abs(oracle.dft2_pixels(gw, norm, np.array([[yp, xp]], np.int32)).real[0])
+    assert abs(peak - abs(im[yp, xp])) <= IMG_TOL * peak
+    px = oracle.dft2_pixels(gw, norm, yx).real
+    err = np.max(np.abs(im[yx[:, 0], yx[:, 1]] - px))
+    assert err <= IMG_TOL * peak, f"snapshot {s}: err {err:.3e} peak {peak:.3e}"
+
+
+def _pixels(n, seed):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    return np.concatenate([rng.integers(0, n, (200, 2)),
+                           [[0, 0], [n - 1, n - 1], [n // 2, n // 2], [n // 2 - 1, n // 2 + 1], [0, n - 1],
+                            [n // 2, 0], [n - 1, n // 2]]]).astype(np.int32)
+
+
+def test_mwa2_4096_grid_image_sampled_pixels(torch_cuda, blink, oracle):
+    """BASELINE.json configs[3] (4096^2) through blink_grid_image (two-kernel route: column transforms
+    straight from the visibilities, k_cols_from_vis<4096> + k_image_rows<4096>), more snapshots than
+    one time step so the channel index wraps; every image fully written, every snapshot checked on
+    sampled pixels."""
+    torch = torch_cuda
+    w = synth.config_mwa2(n_t=2, n_ch=3)
+    vis = w.vis()
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 0
+    n = w.n_pix
+    img = torch.full((w.n_t, w.n_ch, n, n), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(torch.from_numpy(vis).cuda(), img)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img).all(), "image not fully written"
+    imh = img.cpu().numpy().reshape(-1, n, n)
+    yx = _pixels(n, 41)
+    for s in range(w.n_t * w.n_ch):
+        _sampled_pixel_check(oracle, w, vis, s, imh[s], yx)
+    plan.close()
+
+
+@pytest.mark.parametrize("weighting", [synth.NATURAL, synth.UNIFORM])
+def test_n2048_all_calls(torch_cuda, blink, oracle, weighting):
+    """N = 2048 (accepted by blink_plan_create, instantiated as k_image_rows<2048> etc.): the MWA
+    Phase II layout imaged at 30 arcsec per pixel.  Indices and counts bit-exact, blink_grid at the
+    grid bar, blink_image and blink_grid_image on sampled pixels, both weightings."""
+    torch = torch_cuda
+    w = synth.config_mwa2(n_t=2, n_ch=2)
+    w.n_pix, w.pixscale, w.weighting = 2048, 30.0 * synth.ARCSEC, weighting
+    vis = w.vis()
+    plan = _plan(blink, w)
+    n = w.n_pix
+    for ch in range(w.n_ch):
+        r = oracle.uv_cells(w.ant_enu_m, w.freq_hz[ch], n, w.pixscale)
+        assert np.array_equal(plan.cell_idx(ch), r["cell"])
+        assert np.array_equal(plan.counts(ch), oracle.counts(r["cell"], r["cell_conj"], n))
+    v = torch.from_numpy(vis).cuda()
+    uv = torch.full((w.n_t, w.n_ch, n, n), float("nan"), dtype=torch.complex64, device="cuda")
+    plan.grid(v, uv)
+    img = torch.full((w.n_t, w.n_ch, n, n), float("nan"), dtype=torch.float32, device="cuda")
+    plan.image(uv, img)
+    img2 = torch.full((w.n_t, w.n_ch, n, n), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(v, img2)
+    torch.cuda.synchronize()
+    assert torch.isfinite(uv.view(torch.float32)).all() and torch.isfinite(img).all() and torch.isfinite(img2).all()
+    uvh = uv.cpu().numpy().reshape(-1, n, n)
+    imh, imh2 = img.cpu().numpy().reshape(-1, n, n), img2.cpu().numpy().reshape(-1, n, n)
+    yx = _pixels(n, 43)
+    for s in range(w.n_t * w.n_ch):
+        _sampled_pixel_check(oracle, w, vis, s, imh[s], yx, uv=uvh[s])
+        _sampled_pixel_check(oracle, w, vis, s, imh2[s], yx)
+    plan.close()

@@ -15,21 +15,6 @@ GRID_TOL = 1e-5
 IMG_TOL = 1e-4
 
 
-@pytest.fixture(scope="module")
-def torch_cuda():
-    import torch
-    if not torch.cuda.is_available():
-        pytest.fail("gpu-marked test run without a CUDA device")
-    return torch
-
-
-@pytest.fixture(scope="module")
-def blink():
-    from paper_2405_13478_b200 import blink as b
-    b.load()  # raises if libblink.so is missing: there is no fallback
-    return b
-
-
 def _workload(name):
     if name == "tiny":
         return synth.config_tiny()
@@ -244,9 +229,11 @@ def test_edge_cases(torch_cuda, blink):
         blink.Plan(w.ant_enu_m[:1], w.freq_hz, 128, 2.0 / 128)    # one antenna
 
 
-def test_full_size_station_launch_configuration(torch_cuda, blink, oracle):
-    """BASELINE.json configs[1] at FULL size (100 t x 32 ch x 32640 bl, 256^2), in the launch
-    configuration bench.py times; parity on sampled snapshots."""
+def test_full_size_station_two_call_route(torch_cuda, blink, oracle):
+    """BASELINE.json configs[1] at FULL size (100 t x 32 ch x 32640 bl, 256^2) through the TWO-CALL
+    route, blink_grid (ring route, 3200 snapshots) + blink_image, as `bench.py --path separate` times
+    it; parity of grids and images on sampled snapshots.  (The one-call route bench.py's headline
+    times is tests/test_gpu_fullsize.py::test_full_size_station_grid_image.)"""
     torch = torch_cuda
     w = synth.config_station()
     vis = w.vis()
