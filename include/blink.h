@@ -18,7 +18,7 @@
  *   - complex64 = interleaved float (re, im) pairs, i.e. float2 / cufftComplex layout
  *     ("gpufftComplex");
  *   - there is NO CPU fallback: without a CUDA device every call except blink_version,
- *     blink_strerror and the blink_host_* table helpers returns BLINK_ECUDA.
+ *     blink_strerror returns BLINK_ECUDA.
  *
  * Baseline order (cross-correlations only):
  *   bl(i,j) = i (2 n_ant - i - 1) / 2 + (j - i - 1)  for 0 <= i < j < n_ant,  b_ij = r_j - r_i.
@@ -41,14 +41,16 @@
 extern "C" {
 #endif
 
-#define BLINK_VERSION 100 /* 0.1.0 */
+#define BLINK_VERSION 200 /* 0.2.0 */
 
 typedef enum blink_status {
   BLINK_OK = 0,
   BLINK_EINVAL = -1, /* bad argument (NULL, odd / unsupported n_pix, n_ant < 2, ...) */
   BLINK_ENOMEM = -2, /* host or device allocation failed */
   BLINK_ECUDA = -3,  /* CUDA runtime error or no device (see blink_last_cuda_error) */
-  BLINK_EUNSUPPORTED = -4 /* valid request outside what this build implements */
+  BLINK_EUNSUPPORTED = -4, /* valid request outside what this build implements */
+  BLINK_ERESERVE = -5 /* the plan's device scratch is too small for this n_t: call blink_plan_reserve(plan, n_t)
+                         first (hot calls never allocate) */
 } blink_status;
 
 typedef enum blink_weighting {
@@ -80,6 +82,24 @@ typedef enum blink_query {
 
 typedef struct blink_plan blink_plan; /* opaque */
 
+/*
+ * Optional arguments of blink_plan_create_opts.  Zero-initialise, set struct_size = sizeof(blink_options)
+ * and change what is needed; every field's 0 means "let the plan decide".  The route fields exist so
+ * that a harness can compare the library's alternative routes against each other and the oracle; the
+ * library reads no environment variable.
+ */
+typedef struct blink_options {
+  int32_t struct_size;        /* sizeof(blink_options) of the caller's header */
+  int32_t fused_route;        /* blink_grid_image shared-memory route (BLINK_Q_FUSED_PATH 1): 0 auto, -1 never */
+  int32_t polyphase;          /* its polyphase form for N = 512 / 1024: 0 auto, -1 never */
+  int32_t warp_route;         /* warp-per-transform route at N = 1024 (BLINK_Q_FUSED_PATH 2): 0 auto, -1 never */
+  int32_t warp_ring;          /* snapshots of intermediate U kept in flight by that route: 0 auto (32 MB), else >= 2 */
+  int32_t grid_ring;          /* blink_grid ring route: 0 auto, -1 never */
+  int32_t grid_ring_min_snap; /* fewest snapshots per call that take it: 0 auto (one per SM), else >= 1 */
+  int32_t image_chunk_mb;     /* scratch budget (MiB) of the two-kernel imaging routes: 0 auto (512) */
+  int32_t tune[8];            /* implementation tuning knobs, meaning private to this version (csrc/blink_internal.h) */
+} blink_options;
+
 int blink_version(void);
 const char *blink_strerror(int status);
 /* text of the last CUDA error seen by this thread's last failing call ("" if none) */
@@ -104,6 +124,22 @@ const char *blink_last_cuda_error(void);
 int blink_plan_create(blink_plan **out, const double *ant_enu_m, int n_ant, const double *freq_hz,
                       int n_ch, int n_pix, double pixscale, int weighting, void *stream);
 
+/* same, with options (NULL = defaults = blink_plan_create); BLINK_EINVAL on an unknown struct_size or value */
+int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m, int n_ant, const double *freq_hz,
+                           int n_ch, int n_pix, double pixscale, int weighting, void *stream,
+                           const blink_options *opts);
+
+/*
+ * Threads, streams, devices.  A plan belongs to the device that was current at blink_plan_create; every
+ * call that takes it returns BLINK_EINVAL when another device is current.  Calls that use plan-owned
+ * scratch (blink_image always; blink_grid_image when BLINK_Q_FUSED_PATH != 1) must not overlap in time
+ * with each other on the same plan: issue them on one stream, or order the streams.  blink_grid,
+ * blink_correct, blink_dynspec and blink_grid_image on the shared-memory route (BLINK_Q_FUSED_PATH == 1)
+ * use no plan scratch and may run concurrently.  Plan-mutating calls (blink_plan_reserve,
+ * blink_plan_set_corrections, blink_plan_refresh, blink_plan_destroy) must not run concurrently with
+ * anything else on the same plan.
+ */
+
 /* frees the plan and its device memory; NULL is a no-op */
 int blink_plan_destroy(blink_plan *plan);
 
@@ -114,9 +150,12 @@ int blink_plan_query(const blink_plan *plan, int what, int index, void *out);
  * blink_grid -- steps a1/a2: gridding.  For each snapshot s = t*n_ch + ch:
  *   uv_grid[s][cell(bl)] += vis[s][bl];  uv_grid[s][cell*(bl)] += conj(vis[s][bl])
  * over all kept baselines, every other cell = 0.  Unweighted sums regardless of the plan's
- * weighting.  The per-cell summation order is fixed (ascending baseline index), so the result is
- * bit-reproducible run to run -- the deterministic reduction the paper plans.
- *   vis      DEVICE complex64 [n_t][n_ch][n_bl], baseline fastest; 16-byte aligned base
+ * weighting.  The per-cell summation order is fixed by the plan (ascending baseline index; the
+ * bulk-copy route adds them in pieces of up to four), so the result is bit-reproducible run to run for
+ * the same plan, batch size and alignment -- the deterministic reduction the paper plans
+ * (PAPER.md:370, :396).
+ *   vis      DEVICE complex64 [n_t][n_ch][n_bl], baseline fastest; 8-byte aligned (a 16-byte aligned
+ *            base lets the call take its bulk-copy route)
  *   uv_grid  DEVICE complex64 [n_t][n_ch][N][N] row-major [ky][kx], FFT-native order (DC at
  *            [0][0]); COMPLETELY overwritten, zeros included (no memset needed); 16-byte aligned
  *   n_t      number of time steps in this call (any >= 0; 0 is a no-op)
@@ -138,9 +177,9 @@ int blink_grid(const blink_plan *plan, const void *vis, int n_t, void *uv_grid, 
  *            warp-per-transform route (N = 1024, wide sparse half-planes: BLINK_Q_FUSED_PATH == 2)
  *            reads only the occupied cells with kx >= 0.  Cells outside the box are never read.
  *   images   DEVICE float32 [n_t][n_ch][N][N] row-major [y][x]; completely overwritten
- * Asynchronous on `stream`.  May grow the plan's internal device scratch on first use with a
- * larger n_t (the only allocation; query BLINK_Q_SCRATCH_BYTES) -- call blink_plan_reserve first
- * to keep the hot call allocation-free.
+ * Asynchronous on `stream`; no allocation, no host synchronisation: the intermediate of the two passes
+ * lives in plan-owned scratch that blink_plan_reserve(plan, n_t) must have sized for this n_t (or a
+ * larger one) beforehand, else BLINK_ERESERVE.
  */
 int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *images, void *stream);
 
@@ -210,9 +249,11 @@ int blink_dynspec(const blink_plan *plan, const void *images, int n_t, double al
  *     plan's cell-sorted tables (each occupied cell sums its own baselines in ascending order), the
  *     row transforms follow; only the half-plane intermediate U passes through plan-owned scratch,
  *     in chunks of BLINK_Q_FUSED_CHUNK snapshots sized to stay L2-resident.
- *   vis     DEVICE complex64 [n_t][n_ch][n_bl]
+ *   vis     DEVICE complex64 [n_t][n_ch][n_bl]; 16-byte aligned base (BLINK_EINVAL otherwise: the routes
+ *           read it with bulk asynchronous copies)
  *   images  DEVICE float32   [n_t][n_ch][N][N]
- * Asynchronous on `stream`; may grow plan-owned scratch on first use (see blink_plan_reserve).
+ * Asynchronous on `stream`; no allocation, no host synchronisation.  The shared-memory route needs no
+ * scratch; the other two need blink_plan_reserve(plan, n_t) beforehand (BLINK_ERESERVE otherwise).
  */
 int blink_grid_image(const blink_plan *plan, const void *vis, int n_t, void *images, void *stream);
 
@@ -224,40 +265,25 @@ int blink_grid_image(const blink_plan *plan, const void *vis, int n_t, void *ima
  */
 int blink_plan_read(const blink_plan *plan, int what, int ch, void *dst_host, size_t bytes);
 
-/* pre-allocates whatever scratch blink_image needs for up to n_t time steps per call */
+/*
+ * blink_plan_reserve -- sizes the plan's device scratch for blink_image / blink_grid_image calls of up
+ * to n_t time steps (BLINK_Q_SCRATCH_BYTES reports it).  The only place scratch is allocated: may
+ * synchronise the device and free / allocate memory; never shrinks.  BLINK_ENOMEM if it does not fit.
+ */
 int blink_plan_reserve(blink_plan *plan, int n_t);
 
 /*
- * Host-side table helper, exported so the host logic is testable without a GPU.
- * Builds the cell-sorted gather tables blink_grid uses from per-baseline cell indices of ONE
- * channel (as returned by BLINK_Q_CELL_IDX): every kept baseline contributes once to its
- * canonical cell (the member of {cell, cell*} in the half-plane ky > 0 or ky == 0, kx >= 0), as V
- * or as conj(V).  Entries are sorted by (canonical cell, baseline).
- *   cell        HOST int32 [n_bl], -1 = dropped
- *   n_can_out   HOST number of distinct canonical cells
- *   can_cell    HOST int32 [n_bl]   out: canonical cell index per segment (first n_can valid)
- *   seg_start   HOST int32 [n_bl+1] out: CSR offsets into src (first n_can+1 valid)
- *   src         HOST int32 [n_bl]   out: (baseline << 1) | conj_flag, n_kept entries
- * Returns the number of kept baselines or a negative blink_status.
+ * blink_grid_validate -- checks blink_image's input contract on a uv grid: counts the cells that are
+ * non-zero although the plan's weight count there is zero, plus the cells G[k] != conj(G[-k]) (bitwise).
+ * 0 for every blink_grid output.  blink_image's result is defined by the transform of PAPER.md:372-376
+ * only for grids that pass (a route may read just the plan's occupied cells); a harness that feeds it
+ * grids from elsewhere calls this first.
+ *   uv_grid       DEVICE complex64 [n_t][n_ch][N][N]
+ *   n_violations  HOST   int64, out
+ * Synchronous (waits for `stream`).
  */
-int blink_host_build_gather(const int32_t *cell, int n_bl, int n_pix, int32_t *n_can_out,
-                            int32_t *can_cell, int32_t *seg_start, int32_t *src);
-
-/*
- * Host emulation of the gridding phase of blink_grid_image's shared-memory route (steps a1/a2,
- * PAPER.md:348-370), exported so its plan tables are testable without a GPU.  For ONE channel it
- * builds the gather tables the kernel streams through shared memory -- cells owned by warps,
- * baselines taken in chunks of chunk_vis (even, <= 32766), groups of 32 lanes x at most 4 rows --
- * and walks them over a host model of shared memory exactly as a warp does.
- *   cell       HOST int32 [n_bl], -1 = dropped (BLINK_Q_CELL_IDX of the channel)
- *   vis        HOST complex64 [n_bl] (interleaved floats)
- *   sums       HOST complex64 [n_can] out: per canonical cell (blink_host_build_gather's order) the
- *              sum of V (or conj V) over its baselines, fp32, in the kernel's summation order
- *   stats      HOST int32 [3] out (may be NULL): n_can, groups, rows over all chunks
- * Returns 0 or a negative blink_status.
- */
-int blink_host_fused_emulate(const int32_t *cell, int n_bl, int n_pix, int chunk_vis, const float *vis,
-                             float *sums, int32_t *stats);
+int blink_grid_validate(const blink_plan *plan, const void *uv_grid, int n_t, int64_t *n_violations,
+                        void *stream);
 
 #ifdef __cplusplus
 }

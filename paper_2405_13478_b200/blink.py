@@ -15,14 +15,36 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libblink.so")
 
 NATURAL, UNIFORM = 0, 1
-OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED = 0, -1, -2, -3, -4
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ERESERVE = 0, -1, -2, -3, -4, -5
 (Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
  Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK, Q_CORR) = range(17)
 
-EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create",
+# include/blink.h (the product ABI) and include/blink_testing.h (host-only test hooks)
+EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create", "blink_plan_create_opts",
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
            "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct", "blink_dynspec",
-           "blink_image", "blink_host_build_gather", "blink_host_fused_emulate"]
+           "blink_image", "blink_grid_validate"]
+TESTING_EXPORTS = ["blink_host_build_gather", "blink_host_fused_emulate"]
+
+
+class Options(ctypes.Structure):
+    """blink_options (include/blink.h): zero = let the plan decide."""
+    _fields_ = [("struct_size", ctypes.c_int32), ("fused_route", ctypes.c_int32), ("polyphase", ctypes.c_int32),
+                ("warp_route", ctypes.c_int32), ("warp_ring", ctypes.c_int32), ("grid_ring", ctypes.c_int32),
+                ("grid_ring_min_snap", ctypes.c_int32), ("image_chunk_mb", ctypes.c_int32),
+                ("tune", ctypes.c_int32 * 8)]
+
+    def __init__(self, **kw):
+        super().__init__()
+        self.struct_size = ctypes.sizeof(Options)
+        for k, v in kw.items():
+            if k == "tune":
+                for i, t in dict(v).items():
+                    self.tune[int(i)] = int(t)
+            else:
+                if not hasattr(self, k):
+                    raise TypeError(f"unknown blink option {k}")
+                setattr(self, k, int(v))
 
 _lib = None
 
@@ -52,6 +74,10 @@ def load() -> ctypes.CDLL:
     lib.blink_last_cuda_error.restype = ctypes.c_char_p
     lib.blink_plan_create.restype = ci
     lib.blink_plan_create.argtypes = [ctypes.POINTER(vp), vp, ci, vp, ci, ci, cd, ci, vp]
+    lib.blink_plan_create_opts.restype = ci
+    lib.blink_plan_create_opts.argtypes = [ctypes.POINTER(vp), vp, ci, vp, ci, ci, cd, ci, vp, ctypes.POINTER(Options)]
+    lib.blink_grid_validate.restype = ci
+    lib.blink_grid_validate.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_int64), vp]
     lib.blink_plan_destroy.restype = ci
     lib.blink_plan_destroy.argtypes = [vp]
     lib.blink_plan_query.restype = ci
@@ -127,7 +153,7 @@ class Plan:
     """blink_plan_create / blink_plan_destroy and the calls that take a plan."""
 
     def __init__(self, ant_enu_m, freq_hz, n_pix: int, pixscale: float, weighting: int = NATURAL,
-                 stream=None):
+                 stream=None, options: "Options | dict | None" = None):
         lib = load()
         ant = np.ascontiguousarray(ant_enu_m, np.float64)
         fr = np.ascontiguousarray(freq_hz, np.float64).reshape(-1)
@@ -135,9 +161,18 @@ class Plan:
             raise ValueError("ant_enu_m must be [n_ant, 3]")
         self._h = ctypes.c_void_p(None)
         self._lib = lib
-        _check(lib.blink_plan_create(ctypes.byref(self._h), ant.ctypes.data, ant.shape[0],
-                                     fr.ctypes.data, fr.shape[0], int(n_pix), float(pixscale),
-                                     int(weighting), _stream_ptr(stream)), "blink_plan_create")
+        if isinstance(options, dict):
+            options = Options(**options)
+        if options is None:
+            _check(lib.blink_plan_create(ctypes.byref(self._h), ant.ctypes.data, ant.shape[0],
+                                         fr.ctypes.data, fr.shape[0], int(n_pix), float(pixscale),
+                                         int(weighting), _stream_ptr(stream)), "blink_plan_create")
+        else:
+            _check(lib.blink_plan_create_opts(ctypes.byref(self._h), ant.ctypes.data, ant.shape[0],
+                                              fr.ctypes.data, fr.shape[0], int(n_pix), float(pixscale),
+                                              int(weighting), _stream_ptr(stream), ctypes.byref(options)),
+                   "blink_plan_create_opts")
+        self._reserved_n_t = 0
         self.n_ant, self.n_ch, self.n_pix = ant.shape[0], fr.shape[0], int(n_pix)
         self.n_bl = self.query_i32(Q_N_BL)
         self.weighting = int(weighting)
@@ -251,7 +286,24 @@ class Plan:
 
     # ---- hot path
     def reserve(self, n_t: int):
+        """blink_plan_reserve: the one place plan scratch is allocated (the hot calls never allocate and
+        return BLINK_ERESERVE when it is too small)."""
         _check(self._lib.blink_plan_reserve(self._h, int(n_t)), "blink_plan_reserve")
+        self._reserved_n_t = max(self._reserved_n_t, int(n_t))
+
+    def _ensure_reserved(self, n_t: int, auto_reserve: bool):
+        if auto_reserve and n_t > self._reserved_n_t:
+            self.reserve(n_t)
+
+    def validate(self, uv_grid, stream=None) -> int:
+        """blink_grid_validate: number of cells of uv_grid that break blink_image's input contract."""
+        import torch
+        assert uv_grid.is_cuda and uv_grid.dtype == torch.complex64 and uv_grid.is_contiguous()
+        assert tuple(uv_grid.shape[1:]) == (self.n_ch, self.n_pix, self.n_pix)
+        n = ctypes.c_int64(0)
+        _check(self._lib.blink_grid_validate(self._h, uv_grid.data_ptr(), uv_grid.shape[0], ctypes.byref(n),
+                                             _stream_ptr(stream)), "blink_grid_validate")
+        return int(n.value)
 
     def grid(self, vis, uv_grid=None, stream=None):
         """blink_grid: vis complex64 cuda [n_t, n_ch, n_bl] -> uv_grid complex64 [n_t, n_ch, N, N]."""
@@ -268,8 +320,10 @@ class Plan:
                                     _stream_ptr(stream)), "blink_grid")
         return uv_grid
 
-    def image(self, uv_grid, images=None, stream=None):
-        """blink_image: uv_grid complex64 [n_t, n_ch, N, N] -> images float32 [n_t, n_ch, N, N]."""
+    def image(self, uv_grid, images=None, stream=None, auto_reserve=True):
+        """blink_image: uv_grid complex64 [n_t, n_ch, N, N] -> images float32 [n_t, n_ch, N, N].
+        auto_reserve: call blink_plan_reserve first when this n_t is larger than any reserved so far
+        (a convenience of the binding; pass False to see the C call's own BLINK_ERESERVE)."""
         import torch
         assert uv_grid.is_cuda and uv_grid.dtype == torch.complex64 and uv_grid.is_contiguous()
         n_t = uv_grid.shape[0]
@@ -278,11 +332,12 @@ class Plan:
             images = torch.empty((n_t, self.n_ch, self.n_pix, self.n_pix), dtype=torch.float32,
                                  device=uv_grid.device)
         assert images.is_cuda and images.dtype == torch.float32 and images.is_contiguous()
+        self._ensure_reserved(n_t, auto_reserve)
         _check(self._lib.blink_image(self._h, uv_grid.data_ptr(), n_t, images.data_ptr(),
                                      _stream_ptr(stream)), "blink_image")
         return images
 
-    def grid_image(self, vis, images=None, stream=None):
+    def grid_image(self, vis, images=None, stream=None, auto_reserve=True):
         """blink_grid_image: vis complex64 [n_t, n_ch, n_bl] -> images float32 [n_t, n_ch, N, N]."""
         import torch
         assert vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous()
@@ -293,6 +348,7 @@ class Plan:
                                  device=vis.device)
         assert images.is_cuda and images.dtype == torch.float32 and images.is_contiguous()
         assert tuple(images.shape) == (n_t, self.n_ch, self.n_pix, self.n_pix)
+        self._ensure_reserved(n_t, auto_reserve)
         _check(self._lib.blink_grid_image(self._h, vis.data_ptr(), n_t, images.data_ptr(),
                                           _stream_ptr(stream)), "blink_grid_image")
         return images

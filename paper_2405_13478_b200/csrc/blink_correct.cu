@@ -171,6 +171,7 @@ extern "C" int blink_correct(const blink_plan *p, const void *vis_in, int n_t, v
   if (n_t == 0) return BLINK_OK;
   if (!vis_in || !vis_out || !p->d_corr) return BLINK_EINVAL;
   if (((uintptr_t)vis_in & 7) || ((uintptr_t)vis_out & 7)) return BLINK_EINVAL;
+  { const int rc = check_device(p); if (rc != BLINK_OK) return rc; }
   cudaStream_t st = (cudaStream_t)stream;
   const long long tab = (long long)p->n_ch * p->n_bl;
   const int blocks = p->sm_count * 8;

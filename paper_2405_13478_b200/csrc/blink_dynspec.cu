@@ -207,12 +207,9 @@ static int launch_dynspec_tma(const blink_plan *p, const float *images, float *r
   if ((n_t & 7) && (ch_per & 1) && ch_per < p->n_ch) ++ch_per;
   groups = (p->n_ch + ch_per - 1) / ch_per;
   constexpr size_t smem = DsCfg<P, T, STAGES>::kSmem;
-  static thread_local bool attr_set = false;
-  if (!attr_set) {
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_dynspec_tma<P, T, STAGES, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
-                   "k_dynspec_tma smem attribute");
-    attr_set = true;
-  }
+  static std::atomic<uint64_t> attr{0};
+  const int rc = ensure_max_smem(k_dynspec_tma<P, T, STAGES, MINB>, p, attr, "k_dynspec_tma smem attribute", false);
+  if (rc != BLINK_OK) return rc;
   k_dynspec_tma<P, T, STAGES, MINB><<<dim3(tiles, groups), P + 32, smem, st>>>(images, ref_state, dynspec, n_t, p->n_ch, nn, ch_per,
                                                                                (float)alpha);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_dynspec_tma launch");
@@ -230,7 +227,8 @@ extern "C" int blink_dynspec(const blink_plan *p, const void *images, int n_t, d
   if (((uintptr_t)images & 3) || ((uintptr_t)dynspec & 3) || ((uintptr_t)ref_state & 3)) return BLINK_EINVAL;
   const long long nn = (long long)p->n_pix * p->n_pix;     // a multiple of 256 for every supported N (>= 32)
   if (nn % kDsPix) return BLINK_EUNSUPPORTED;
-  static const int route = [] { const char *e = getenv("BLINK_DS_ROUTE"); return e ? atoi(e) : 0; }();   // 1 = register loads
+  const int route = p->opt.tune[kTuneDynspecRoute];   // 1 = register loads even for aligned cubes
+  { const int rc = check_device(p); if (rc != BLINK_OK) return rc; }
   cudaStream_t st = (cudaStream_t)stream;
   if (route != 1 && ((uintptr_t)images & 15) == 0) {
     const float *im = (const float *)images;
@@ -239,7 +237,6 @@ extern "C" int blink_dynspec(const blink_plan *p, const void *images, int n_t, d
     // cube (n_t = 100), ms per call: <256,32,3> 0.368, <128,32,3> 0.378, <128,64,3> 0.335, <128,64,2> 0.331,
     // <64,64,3> 0.338, <256,64,2> 0.376, <64,128,2> 0.393, <128,128,3> 0.492, <64,128,3> 0.505: longer runs
     // per pixel on the write side pay until too few consumer warps are left per SM.
-    if (route == 10) return launch_dynspec_tma<256, 32, 3, 2>(p, im, rs, ds, n_t, alpha, st);
     return launch_dynspec_tma<128, 64, 2, 3>(p, im, rs, ds, n_t, alpha, st);
   }
   const int tiles = (int)(nn / kDsPix);

@@ -42,8 +42,7 @@ int fused_setup(blink_plan *p) {
 //   [off_S, ...)            canonical cell sums, sink, zero slot
 //   [off_bar, ...)          full[nbuf], empty[nbuf], region_free mbarriers
 int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st) {
-  int want = 1;
-  if (const char *e = getenv("BLINK_FUSED_SMEM")) want = atoi(e);
+  const int want = p->opt.fused_route != -1;
   const int N = p->n_pix, n_bl = p->n_bl, n_ch = p->n_ch;
   if (!want || N < 32 || (n_bl & 1) || p->max_smem_optin <= 0) return BLINK_OK;
   // polyphase route (see k_fused): a compact array on a large image is imaged as D x D interleaved
@@ -52,8 +51,7 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   if (N > 256) {
     // (128-point sub-transforms were measured too: station 256^2 as 2 x 2 of 128^2 0.65 ms against
     // 0.42 ms direct, sweep512 as 4 x 4 1.92 ms against 1.36 ms as 2 x 2 of 256^2)
-    int poly = 1;
-    if (const char *e = getenv("BLINK_FUSED_POLY")) poly = atoi(e);
+    const int poly = p->opt.polyphase != -1;
     Ns = 256;
     D = N / Ns;
     if (!poly || D > 4 || std::max(p->kx_max_all, p->ky_max_all) >= Ns / 2) return BLINK_OK;
@@ -74,8 +72,7 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
   for (int ch = 0; ch < n_ch; ++ch) assign_cells(gathers[ch], owner[ch], slot[ch]);
 
-  int force_chunks = 0;
-  if (const char *e = getenv("BLINK_FUSED_CHUNKS")) force_chunks = atoi(e);
+  const int force_chunks = p->opt.tune[kTuneFusedChunks];
   std::vector<AbstractTable> tabs;
   int n_chunk = 0, C = 0, nbuf = 0;
   size_t tab_stride = 0, buf_bytes = 0;
@@ -117,24 +114,6 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
   p->fused_off_bar = (uint32_t)(region_al + buf_bytes + s_bytes);
   p->fused_smem = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 8 + 16;
   p->fused_threads = kFusedThreads;
-  if (getenv("BLINK_DEBUG")) {
-    long rows = 0, hw = 0, groups = 0, rmw = 0;
-    for (const AbstractTable &t : tabs) { rows += t.rows; hw += t.halfrow_wavefronts; groups += t.groups; rmw += t.rmw_wavefronts; }
-    double worst = 0;
-    for (int ch = 0; ch < n_ch; ++ch) {
-      long wc[kFusedWarps] = {}, tot = 0, mx = 0;
-      for (int c = 0; c < n_chunk; ++c)
-        for (int w = 0; w < kFusedWarps; ++w) wc[w] += tabs[(size_t)ch * n_chunk + c].warp_cost[w];
-      for (int w = 0; w < kFusedWarps; ++w) { tot += wc[w]; mx = std::max(mx, wc[w]); }
-      worst = std::max(worst, (double)mx * kFusedWarps / std::max(tot, 1L));
-    }
-    fprintf(stderr, "  phase S warp imbalance (max / mean of the estimated cost), worst channel: %.3f\n", worst);
-    fprintf(stderr, "blink fused route: %d chunks of %d baselines, table stride %zu B, buffer %zu B x %d, smem %zu B\n"
-            "  per snapshot: %.0f groups, %.0f rows (ideal %.0f), %.2f wavefronts per half-row, %.2f per half cell-sum access\n",
-            n_chunk, C, tab_stride, buf_bytes, nbuf, p->fused_smem, (double)groups / n_ch, (double)rows / n_ch,
-            (double)n_bl / 32, (double)hw / (2.0 * std::max(rows, 1L)), (double)rmw / (2.0 * std::max(groups, 1L)));
-  }
-
   const uint32_t s_slot0 = p->fused_off_S / 8;
   std::vector<unsigned char> h_tab((size_t)n_ch * n_chunk * tab_stride, 0);
   std::vector<uint32_t> h_size((size_t)n_ch * n_chunk, 0);
@@ -275,8 +254,6 @@ static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *
   }
 }
 
-int fused_reserve(blink_plan *p, int n_t) { return image_reserve(p, n_t); }
-
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st) {
   if (p->fused_path == 1) return launch_fused(p, vis, n_t, img, st);
   return launch_image_from_vis(p, vis, n_t * p->n_ch, img, st);
@@ -288,10 +265,10 @@ extern "C" int blink_grid_image(const blink_plan *plan, const void *vis, int n_t
   if (!plan || n_t < 0) return BLINK_EINVAL;
   if (n_t == 0) return BLINK_OK;
   if (!vis || !images) return BLINK_EINVAL;
-  if (((uintptr_t)vis & 7) || ((uintptr_t)images & 3)) return BLINK_EINVAL;
-  blink_plan *mp = const_cast<blink_plan *>(plan);
-  int rc = blink::image_reserve(mp, n_t);
+  if (((uintptr_t)vis & 15) || ((uintptr_t)images & 3)) return BLINK_EINVAL;
+  int rc = check_device(plan);
   if (rc != BLINK_OK) return rc;
+  if (blink::scratch_need(plan, n_t, true) > plan->scratch_bytes) return BLINK_ERESERVE;
   return blink::launch_grid_image(plan, (const float2 *)vis, n_t, (float *)images, (cudaStream_t)stream);
 }
 

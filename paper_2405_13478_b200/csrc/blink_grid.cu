@@ -37,7 +37,7 @@ struct GridParams {
   const uint32_t *cellrec;
   const int32_t *nact;
   const int32_t *pcell, *pcode, *pband;
-  int n_bl, n_ch, n_snap, n_bands, band_cells, parts, n_can_max, n_pass, roff_stride, dbg, ch0;
+  int n_bl, n_ch, n_snap, n_bands, band_cells, parts, n_can_max, n_pass, roff_stride, ch0;
   long long grid_cells;  // N*N
 };
 
@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
     float2 *__restrict__ grid = p.uv + (size_t)s * p.grid_cells;
 
     // ---- phase P, first half: zero-fill this part; drains while phase S runs -----------------
-    if (tid == 0 && !(p.dbg & 1)) {
+    if (tid == 0) {
       for (int b = b_lo; b < b_hi; ++b) bulk_store(grid + (size_t)b * p.band_cells, zero, band_bytes);
       bulk_commit();
     }
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
       const uint32_t *__restrict__ cellrec = p.cellrec + cp * max(p.n_can_max, 1);
       SumsRegs<THREADS> sr;
       sums_prefetch<THREADS>(sr, cellrec, p.n_can_max, tid);
-      if (!(p.dbg & 4)) pass_scatter<PF>(regs, stage);
+      pass_scatter<PF>(regs, stage);
       __syncthreads();
       // loads of the next pass (or of the next item's first pass) fly during the sums and phase P
       if (pass + 1 < p.n_pass) {
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
         pass_load<THREADS, PF>(regs, p.vis + (size_t)s2 * p.n_bl, p.scat + (size_t)((s2 + p.ch0) % p.n_ch) * p.n_bl,
                                0, min(CAP, p.n_bl), tid);
       }
-      if (!(p.dbg & 2)) sums_run<THREADS>(sr, cellrec, p.roff + cp * p.roff_stride, p.n_can_max, stage, S, tid);
+      sums_run<THREADS>(sr, cellrec, p.roff + cp * p.roff_stride, p.n_can_max, stage, S, tid);
       if (pass + 1 == p.n_pass && tid == 0) bulk_wait_all();   // the zero fill has landed
       __syncthreads();
     }
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
     const int32_t *__restrict__ pcell = p.pcell + (size_t)ch * 2 * p.n_bl;
     const int32_t *__restrict__ pcode = p.pcode + (size_t)ch * 2 * p.n_bl;
     const int e0 = pband[b_lo], e1 = pband[b_hi];
-    for (int e = e0 + tid; e < e1 && !(p.dbg & 8); e += THREADS) {
+    for (int e = e0 + tid; e < e1; e += THREADS) {
       const int code = pcode[e];
       const float2 v = S[code & kPlaceMask];
       const int flag = code >> kPlaceShift;
@@ -257,8 +257,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_grid_ring(const GridRingPa
 // never has to drain between snapshots.
 int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st) {
   p->ring_path = 0;
-  int want = 1;
-  if (const char *e = getenv("BLINK_GRID_RING")) want = atoi(e);
+  const int want = p->opt.grid_ring != -1;
   const int N = p->n_pix, n_bl = p->n_bl, n_ch = p->n_ch;
   if (!want || N > 512 || (n_bl & 1) || p->max_smem_optin <= 0 || p->n_can_max < 1) return BLINK_OK;
   const int sink0 = (p->n_can_max + 15) & ~15, n_S = sink0 + 16;
@@ -310,9 +309,6 @@ int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaS
   p->ring_off_bar = (uint32_t)(p->ring_off_S + s_bytes);
   p->ring_smem = p->ring_off_bar + 16 * (size_t)nbuf + 16;
   if (p->ring_smem > limit || p->ring_smem > 0x7FFFu * 8u) return BLINK_OK;
-  if (getenv("BLINK_DEBUG"))
-    fprintf(stderr, "blink grid ring route: %d chunks of %d baselines, %d buffers of %zu B, smem %zu B\n", n_chunk, C,
-            nbuf, buf_bytes, p->ring_smem);
 
   const uint32_t s_slot0 = p->ring_off_S / 8;
   std::vector<unsigned char> h_tab((size_t)n_ch * n_chunk * tab_stride, 0);
@@ -359,8 +355,7 @@ int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaS
   if ((rc = upload((void **)&p->d_rsize, h_size.data(), sizeof(uint32_t) * h_size.size())) != BLINK_OK) return rc;
   if ((rc = upload((void **)&p->d_rplace, h_place.data(), sizeof(int2) * h_place.size())) != BLINK_OK) return rc;
   BLINK_CUDA_TRY(cudaStreamSynchronize(st), "ring table upload sync");
-  p->ring_min_snap = p->sm_count;
-  if (const char *e = getenv("BLINK_GRID_RING_MIN")) p->ring_min_snap = atoi(e);
+  p->ring_min_snap = p->opt.grid_ring_min_snap > 0 ? p->opt.grid_ring_min_snap : p->sm_count;
   p->ring_path = 1;
   return BLINK_OK;
 }
@@ -372,13 +367,9 @@ static int launch_grid_ring(const blink_plan *p, const float2 *vis, int n_snap, 
   g.chunk_vis = p->ring_chunk_vis; g.nbuf = p->ring_nbuf; g.tab_stride = p->ring_tab_stride; g.n_bands = p->n_bands;
   g.band_cells = p->band_cells; g.ch0 = ch0; g.buf_bytes = p->ring_buf_bytes; g.off_buf = p->ring_off_buf;
   g.off_S = p->ring_off_S; g.off_bar = p->ring_off_bar; g.grid_cells = (long long)p->n_pix * p->n_pix;
-  static thread_local size_t smem_set = 0;
-  if (p->ring_smem > smem_set) {
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_grid_ring, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->ring_smem),
-                   "k_grid_ring smem attribute");
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_grid_ring, cudaFuncAttributePreferredSharedMemoryCarveout, 100), "k_grid_ring carveout");
-    smem_set = p->ring_smem;
-  }
+  static std::atomic<uint64_t> attr{0};
+  const int rc = ensure_max_smem(k_grid_ring, p, attr, "k_grid_ring smem attribute");
+  if (rc != BLINK_OK) return rc;
   const int blocks = std::min(n_snap, p->sm_count);
   k_grid_ring<<<blocks, kFusedThreads, p->ring_smem, st>>>(g);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_grid_ring launch");
@@ -390,14 +381,9 @@ static int launch_grid_v(const blink_plan *p, const GridParams &g0, cudaStream_t
   GridParams g = g0;
   const size_t smem = p->grid_smem;
   if (smem > (size_t)p->max_smem_optin) return BLINK_EUNSUPPORTED;
-  static thread_local size_t smem_set = 0;
-  if (smem > smem_set) {
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_grid<THREADS, PF, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
-                   "k_grid smem attribute");
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_grid<THREADS, PF, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout, 100),
-                   "k_grid carveout");
-    smem_set = smem;
-  }
+  static std::atomic<uint64_t> attr{0};
+  const int rc = ensure_max_smem(k_grid<THREADS, PF, MINB>, p, attr, "k_grid smem attribute");
+  if (rc != BLINK_OK) return rc;
   int occ = 1;
   BLINK_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_grid<THREADS, PF, MINB>, THREADS, smem),
                  "k_grid occupancy");
@@ -417,20 +403,17 @@ static int launch_grid_v(const blink_plan *p, const GridParams &g0, cudaStream_t
 int launch_grid(const blink_plan *p, const float2 *vis, int n_snap, int ch0, float2 *uv, cudaStream_t st) {
   // many snapshots of a small grid: the ring route; few snapshots (or large grids): the band route,
   // which can split one snapshot over several CTAs
-  if (p->ring_path == 1 && n_snap >= p->ring_min_snap) return launch_grid_ring(p, vis, n_snap, ch0, uv, st);
+  // (the ring route reads the visibilities with bulk copies: 16-byte aligned base)
+  if (p->ring_path == 1 && n_snap >= p->ring_min_snap && ((uintptr_t)vis & 15) == 0)
+    return launch_grid_ring(p, vis, n_snap, ch0, uv, st);
   GridParams g;
   g.vis = vis; g.uv = uv; g.chinfo = p->d_chinfo;
   g.scat = p->d_scat; g.roff = p->d_roff; g.cellrec = p->d_cellrec; g.nact = p->d_nact; g.pcell = p->d_pcell; g.pcode = p->d_pcode; g.pband = p->d_pband;
   g.n_bl = p->n_bl; g.n_ch = p->n_ch; g.n_snap = n_snap; g.ch0 = ch0;
   g.n_bands = p->n_bands; g.band_cells = p->band_cells; g.n_can_max = p->n_can_max;
   g.n_pass = p->n_pass; g.roff_stride = p->roff_stride; g.parts = 1;
-  g.dbg = 0;
-  if (const char *e = getenv("BLINK_GRID_DEBUG")) g.dbg = atoi(e);   // timing experiments only
   g.grid_cells = (long long)p->n_pix * p->n_pix;
-  if (p->grid_threads == 512 && p->grid_prefetch == 16) return launch_grid_v<512, 16, 1>(p, g, st);
-  if (p->grid_threads == 512 && p->grid_prefetch == 8) return launch_grid_v<512, 8, 2>(p, g, st);
-  if (p->grid_threads == 256 && p->grid_prefetch == 8) return launch_grid_v<256, 8, 3>(p, g, st);
-  return launch_grid_v<256, 16, 2>(p, g, st);
+  return launch_grid_v<512, 16, 1>(p, g, st);
 }
 
 }  // namespace blink
@@ -440,5 +423,60 @@ extern "C" int blink_grid(const blink_plan *plan, const void *vis, int n_t, void
   if (n_t == 0) return BLINK_OK;
   if (!vis || !uv_grid) return BLINK_EINVAL;
   if (((uintptr_t)vis & 7) || ((uintptr_t)uv_grid & 15)) return BLINK_EINVAL;
+  const int rc = check_device(plan);
+  if (rc != BLINK_OK) return rc;
   return blink::launch_grid(plan, (const float2 *)vis, n_t * plan->n_ch, 0, (float2 *)uv_grid, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// blink_grid_validate: the input contract of blink_image checked cell by cell (see blink.h).
+namespace blink {
+__global__ void __launch_bounds__(256) k_grid_validate(const float2 *__restrict__ uv, const uint32_t *__restrict__ counts,
+                                                       int N, int n_ch, long long n_cells_total,
+                                                       unsigned long long *__restrict__ n_bad) {
+  const long long NN = (long long)N * N;
+  unsigned long long bad = 0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_cells_total;
+       i += (long long)gridDim.x * blockDim.x) {
+    const long long s = i / NN;
+    const int c = (int)(i - s * NN), iy = c / N, ix = c - iy * N;
+    const int cm = ((N - iy) & (N - 1)) * N + ((N - ix) & (N - 1));
+    const float2 g = uv[i], m = uv[s * NN + cm];
+    const uint32_t cnt = counts[(size_t)(s % n_ch) * NN + c];
+    const bool nonplan = cnt == 0 && !(g.x == 0.f && g.y == 0.f);
+    const bool nonherm = !(g.x == m.x && g.y == -m.y);
+    bad += (nonplan || nonherm) ? 1u : 0u;
+  }
+  for (int o = 16; o > 0; o >>= 1) bad += __shfl_down_sync(0xffffffffu, bad, o);
+  if ((threadIdx.x & 31) == 0 && bad) atomicAdd(n_bad, bad);
+}
+}  // namespace blink
+
+extern "C" int blink_grid_validate(const blink_plan *plan, const void *uv_grid, int n_t, int64_t *n_violations,
+                                   void *stream) {
+  if (!plan || n_t < 0 || !n_violations) return BLINK_EINVAL;
+  *n_violations = 0;
+  if (n_t == 0) return BLINK_OK;
+  if (!uv_grid || ((uintptr_t)uv_grid & 7)) return BLINK_EINVAL;
+  const int rc = check_device(plan);
+  if (rc != BLINK_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  unsigned long long *d_bad = nullptr, h_bad = 0;
+  BLINK_CUDA_TRY(cudaMalloc((void **)&d_bad, sizeof(*d_bad)), "blink_grid_validate cudaMalloc");
+  const long long total = (long long)n_t * plan->n_ch * plan->n_pix * plan->n_pix;
+  cudaError_t e = cudaMemsetAsync(d_bad, 0, sizeof(*d_bad), st);
+  if (e == cudaSuccess) {
+    blink::k_grid_validate<<<plan->sm_count * 8, 256, 0, st>>>((const float2 *)uv_grid, plan->d_counts, plan->n_pix, plan->n_ch,
+                                                                total, d_bad);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&h_bad, d_bad, sizeof(h_bad), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(d_bad);
+  if (e != cudaSuccess) {
+    blink::set_cuda_error(e, "blink_grid_validate");
+    return BLINK_ECUDA;
+  }
+  *n_violations = (int64_t)h_bad;
+  return BLINK_OK;
 }

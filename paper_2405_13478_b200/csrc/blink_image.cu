@@ -267,27 +267,17 @@ __global__ void __launch_bounds__(RP * (N / 16)) k_image_rows(const ImgParams p)
   fft_tail<N>(v, t, line, p.tw, [&](int x, cf32 z) { __stcs(r0 + x, z.x); __stcs(r1 + x, z.y); });
 }
 
-template <class K> static int prep_kernel(K kern, size_t smem) {
-  BLINK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem),
-                 "image kernel smem attribute");
-  BLINK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100),
-                 "image kernel carveout");
-  return BLINK_OK;
-}
-
 template <int N, int CT, int RP>
 static int run_image_cfg(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st) {
   using C = ImgCfg<N>;
   const bool from_vis = ip.vis != nullptr;
   const size_t smem_a = sizeof(cf32) * CT * C::LS, smem_b = sizeof(cf32) * RP * C::LS;
-  static thread_local bool attr_done = false;
-  if (!attr_done) {
-    int rc = prep_kernel(k_image_cols<N, CT>, smem_a);
-    if (rc == BLINK_OK) rc = prep_kernel(k_cols_from_vis<N, CT>, smem_a);
-    if (rc == BLINK_OK) rc = prep_kernel(k_image_rows<N, RP>, smem_b);
-    if (rc != BLINK_OK) return rc;
-    attr_done = true;
-  }
+  if (std::max(smem_a, smem_b) > (size_t)p->max_smem_optin) return BLINK_EUNSUPPORTED;
+  static std::atomic<uint64_t> attr_a{0}, attr_v{0}, attr_b{0};
+  int rc = ensure_max_smem(k_image_cols<N, CT>, p, attr_a, "k_image_cols smem attribute");
+  if (rc == BLINK_OK) rc = ensure_max_smem(k_cols_from_vis<N, CT>, p, attr_v, "k_cols_from_vis smem attribute");
+  if (rc == BLINK_OK) rc = ensure_max_smem(k_image_rows<N, RP>, p, attr_b, "k_image_rows smem attribute");
+  if (rc != BLINK_OK) return rc;
   const size_t per_snap = sizeof(float2) * (size_t)N * p->wu;
   const int chunk = (int)std::min<size_t>((size_t)std::max(1, p->chunk_snapshots), p->scratch_bytes / per_snap);
   if (chunk < 1) return BLINK_ENOMEM;
@@ -328,28 +318,35 @@ template <int N> static int run_image_n(const blink_plan *p, const ImgParams &ip
 
 int image_setup(blink_plan *p) {
   p->wu = ((p->kx_max_all + 1 + 15) / 16) * 16;   // multiple of every column-tile width
-  if (const char *e = getenv("BLINK_IMAGE_CT")) p->img_ct = atoi(e);
-  if (const char *e = getenv("BLINK_IMAGE_RP")) p->img_rp = atoi(e);
+  p->img_ct = p->opt.tune[kTuneImageCt];
+  p->img_rp = p->opt.tune[kTuneImageRp];
   p->image_path = 1;
   // snapshots per launch pair.  The transforms are instruction-bound, not HBM-bound, so fewer and
   // larger launches win over keeping U L2-resident (measured: 48 MB -> 11.1 ms, 400 MB -> 10.0 ms
   // per 2400 MWA-I snapshots)
   size_t budget = 512u << 20;
-  if (const char *e = getenv("BLINK_IMAGE_CHUNK_MB")) {
-    long mb = atol(e);
-    if (mb > 0) budget = (size_t)mb << 20;
-  }
+  if (p->opt.image_chunk_mb > 0) budget = (size_t)p->opt.image_chunk_mb << 20;
   const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
-  p->chunk_snapshots = (int)std::max<size_t>(1, budget / per_snap);
+  // a chunk's snapshots are the launch's gridDim.y: at most 65535
+  p->chunk_snapshots = (int)std::min<size_t>(65535, std::max<size_t>(1, budget / per_snap));
   return BLINK_OK;
 }
 
-int image_reserve(blink_plan *p, int n_t) {
-  const long long n_snap = (long long)n_t * p->n_ch;
+// Device scratch of a call of n_t time steps.  The shared-memory route of blink_grid_image needs none;
+// the two-kernel routes hold U of one chunk of snapshots; the warp route a ring of U slots plus two
+// completion counters per snapshot.
+size_t scratch_need(const blink_plan *p, long long n_t, bool fused) {
+  if (fused && p->fused_path == 1) return 0;
+  const long long n_snap = std::max<long long>(n_t * p->n_ch, 1);
+  if (p->warp_route) return warp_route_scratch_bytes(p, n_snap);
   const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
-  size_t need = per_snap * (size_t)std::min<long long>(std::max<long long>(n_snap, 1), p->chunk_snapshots);
-  if (p->warp_route) need = std::max(need, warp_route_scratch_bytes(p, std::max<long long>(n_snap, 1)));
-  if (need <= p->scratch_bytes) return BLINK_OK;
+  return per_snap * (size_t)std::min<long long>(n_snap, p->chunk_snapshots);
+}
+
+int image_reserve(blink_plan *p, int n_t) {
+  const long long n_snap = std::max<long long>((long long)n_t * p->n_ch, 1);
+  const size_t need = std::max(scratch_need(p, n_t, false), scratch_need(p, n_t, true));
+  if (need <= p->scratch_bytes && (!p->warp_route || n_snap <= p->warp_snap_cap)) return BLINK_OK;
   if (p->d_scratch) {
     BLINK_CUDA_TRY(cudaDeviceSynchronize(), "scratch regrow sync");
     cudaFree(p->d_scratch);
@@ -362,6 +359,12 @@ int image_reserve(blink_plan *p, int n_t) {
     return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
   }
   p->scratch_bytes = need;
+  if (p->warp_route) {
+    // the route's completion counters follow the ring; the kernel leaves them zero behind itself
+    const size_t ring = warp_route_ring_bytes(p);
+    BLINK_CUDA_TRY(cudaMemset(reinterpret_cast<unsigned char *>(p->d_scratch) + ring, 0, need - ring), "scratch counters");
+    p->warp_snap_cap = n_snap;
+  }
   return BLINK_OK;
 }
 
@@ -375,8 +378,7 @@ static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2
   ip.tw = p->d_tw; ip.n_ch = p->n_ch; ip.wu = p->wu; ip.uniform = p->weighting == BLINK_UNIFORM;
   ip.snap_base = 0;
   ip.ch0 = ch0;
-  ip.direct_max = 12;
-  if (const char *e = getenv("BLINK_IMAGE_DIRECT")) ip.direct_max = std::min(32, std::max(0, atoi(e)));
+  ip.direct_max = p->opt.tune[kTuneDirectMax] > 0 ? std::min(32, p->opt.tune[kTuneDirectMax] - 1) : 12;
   if (p->warp_route)                        // persistent warp-per-transform kernel (blink_image_w.cu)
     return launch_img1024(p, ip, n_snap, st);
   switch (p->n_pix) {
@@ -407,7 +409,8 @@ extern "C" int blink_image(const blink_plan *plan, const void *uv_grid, int n_t,
   if (n_t == 0) return BLINK_OK;
   if (!uv_grid || !images) return BLINK_EINVAL;
   if (((uintptr_t)uv_grid & 7) || ((uintptr_t)images & 3)) return BLINK_EINVAL;
-  int rc = blink::image_reserve(const_cast<blink_plan *>(plan), n_t);
+  int rc = check_device(plan);
   if (rc != BLINK_OK) return rc;
+  if (blink::scratch_need(plan, n_t, false) > plan->scratch_bytes) return BLINK_ERESERVE;
   return blink::launch_image(plan, (const float2 *)uv_grid, n_t * plan->n_ch, 0, (float *)images, (cudaStream_t)stream);
 }

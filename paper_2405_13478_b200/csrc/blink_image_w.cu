@@ -47,7 +47,8 @@ constexpr size_t kWFixedBytes = kWRegionBytes + sizeof(cf32) * (1024 + 32) + 8 *
 struct WParams {
   ImgParams ip;
   int n_snap, items_a, g_a, ring;   // items_a = wu / 8; CTAs 0 .. g_a - 1 run pass A; ring slots of U
-  int *done_a, *done_b;             // per snapshot, zeroed before the launch
+  int *done_a, *done_b;             // per snapshot; zero at launch, zeroed again by the last CTA to finish
+  int *finished;                    // CTAs that have finished (same protocol)
   const uint4 *vrec;                // pass-A cell records
   const float2 *uvsrc;              // blink_image: cell values come from this uv grid; NULL = from visibilities
 };
@@ -333,11 +334,28 @@ __global__ void __launch_bounds__(kWThreads, 2) k_img1024(const WParams q) {
       }
     }
   }
+  // The last CTA to get here clears the counters, so the next launch finds them zero without a memset:
+  // a CTA takes its ticket after its last counter access, so once all tickets are out nobody reads or
+  // bumps a counter any more.
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    s_off[47] = atomicAdd(q.finished, 1) == (int)gridDim.x - 1;     // s_off[36..47] are spare
+  }
+  __syncthreads();
+  if (s_off[47]) {
+    __threadfence();
+    for (int i = tid; i < q.n_snap; i += kWThreads) {
+      q.done_a[i] = 0;
+      q.done_b[i] = 0;
+    }
+    if (tid == 0) *q.finished = 0;
+  }
 }
 
 static int w_grid(const blink_plan *p) {
   int per_sm = 2;
-  if (const char *e = getenv("BLINK_W_CTAS")) per_sm = std::max(1, std::min(2, atoi(e)));
+  if (p->opt.tune[kTuneWarpCtasPerSm] > 0) per_sm = std::max(1, std::min(2, (int)p->opt.tune[kTuneWarpCtasPerSm]));
   return std::max(2, per_sm * p->sm_count);
 }
 static int w_ring(const blink_plan *p) {
@@ -345,15 +363,16 @@ static int w_ring(const blink_plan *p) {
   // stay in L2 (default 32 MB at wu = 512)
   const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
   int ring = (int)std::max<size_t>(4, std::min<size_t>(64, ((size_t)32 << 20) / per_snap));
-  if (const char *e = getenv("BLINK_W_RING")) ring = std::max(2, atoi(e));
+  if (p->opt.warp_ring >= 2) ring = p->opt.warp_ring;
   return ring;
 }
 
-// scratch: ring of U slots, then the counters (done_a[n_snap], done_b[n_snap])
+// scratch: ring of U slots, then the counters (finished + padding [64], done_a[n_snap], done_b[n_snap])
+size_t warp_route_ring_bytes(const blink_plan *p) {
+  return sizeof(float2) * (size_t)p->n_pix * p->wu * (size_t)w_ring(p);
+}
 size_t warp_route_scratch_bytes(const blink_plan *p, long long n_snap) {
-  const int ring = w_ring(p);
-  const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
-  return per_snap * (size_t)ring + sizeof(int) * (size_t)(2 * n_snap + 64);
+  return warp_route_ring_bytes(p) + sizeof(int) * (size_t)(2 * n_snap + 64);
 }
 
 int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st) {
@@ -365,16 +384,15 @@ int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t s
   q.ring = w_ring(p);
   {   // split of the grid between the passes (measured on MWA Phase I: pass A needs the larger share)
     double fa = 0.6;
-    if (const char *e = getenv("BLINK_W_FRAC_A")) fa = std::min(0.9, std::max(0.1, atof(e)));
+    if (p->opt.tune[kTuneWarpFracA] > 0) fa = std::min(0.9, std::max(0.1, 0.01 * p->opt.tune[kTuneWarpFracA]));
     q.g_a = std::min(grid - 1, std::max(1, (int)(fa * grid + 0.5)));
   }
-  const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
-  const size_t ring_bytes = per_snap * (size_t)q.ring;
-  const size_t cnt_bytes = sizeof(int) * (2 * (size_t)n_snap + 64);
-  if (ring_bytes + cnt_bytes > p->scratch_bytes) return BLINK_ENOMEM;
+  const size_t ring_bytes = warp_route_ring_bytes(p);
+  if (warp_route_scratch_bytes(p, n_snap) > p->scratch_bytes || n_snap > p->warp_snap_cap) return BLINK_ERESERVE;
   int *cnt = reinterpret_cast<int *>(reinterpret_cast<unsigned char *>(p->d_scratch) + ring_bytes);
-  q.done_a = cnt;
-  q.done_b = cnt + n_snap;
+  q.finished = cnt;
+  q.done_a = cnt + 64;
+  q.done_b = cnt + 64 + n_snap;
   q.vrec = p->d_vrec;
   q.uvsrc = ip.vis == nullptr ? ip.uv : nullptr;
   ip.snap_base = 0;
@@ -383,13 +401,9 @@ int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t s
   // on top of the fixed part: cell values + their iy, the record buffer, the offsets ring
   const size_t smem = kWFixedBytes + (size_t)ip.cell_cap * (sizeof(cf32) + sizeof(int32_t) + sizeof(uint4)) + 48 * sizeof(int32_t);
   if (p->max_smem_optin > 0 && smem > (size_t)p->max_smem_optin) return BLINK_EUNSUPPORTED;
-  static thread_local size_t smem_set = 0;
-  if (smem_set < smem) {
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_img1024, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "k_img1024 smem attribute");
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_img1024, cudaFuncAttributePreferredSharedMemoryCarveout, 100), "k_img1024 carveout");
-    smem_set = smem;
-  }
-  BLINK_CUDA_TRY(cudaMemsetAsync(cnt, 0, cnt_bytes, st), "k_img1024 counters");
+  static std::atomic<uint64_t> attr{0};
+  const int rc = ensure_max_smem(k_img1024, p, attr, "k_img1024 smem attribute");
+  if (rc != BLINK_OK) return rc;
   void *args[] = {(void *)&q};
   // cooperative: the item sequences are dealt statically, so every CTA of the grid must be resident
   BLINK_CUDA_TRY(cudaLaunchCooperativeKernel((const void *)k_img1024, dim3(grid), dim3(kWThreads), args, smem, st), "k_img1024 launch");
@@ -400,6 +414,7 @@ int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t s
 // (a station imaged at 1024^2: 48 columns holding 100 cells each) stay on the line kernels
 bool warp_route_applies(const blink_plan *p) {
   if (p->n_pix != kWN || p->wu < 256 || p->wu % kWWarps) return false;
+  if (p->seg_len_max > 0x3FFF) return false;          // the cell records carry the segment length in 14 bits
   const size_t smem = kWFixedBytes + (size_t)((p->vtile8_max + 3) / 4 * 4) * (sizeof(cf32) + sizeof(int32_t) + sizeof(uint4)) + 48 * sizeof(int32_t);
   return 2 * (smem + 1024) <= (size_t)228 * 1024 && (p->max_smem_optin <= 0 || smem <= (size_t)p->max_smem_optin);
 }

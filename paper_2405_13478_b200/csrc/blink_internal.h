@@ -4,10 +4,12 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <string>
 #include <vector>
 
 #include "../../include/blink.h"
+#include "../../include/blink_testing.h"
 
 namespace blink {
 
@@ -30,6 +32,18 @@ struct ChannelInfo {   // mirrored on the device, one per channel
   float inv_norm;      // 1 / image normalisation
 };
 
+// blink_options::tune[] slots (0 = default), private to this version
+enum TuneSlot {
+  kTuneWarpFracA = 0,     // warp route: percent of the grid's CTAs that run pass A (default 60)
+  kTuneWarpCtasPerSm = 1, // warp route: resident CTAs per SM
+  kTuneFusedChunks = 2,   // shared-memory route: smallest number of chunks per snapshot tried
+  kTuneImageCt = 3,       // two-pass imaging: columns per CTA (pass A)
+  kTuneImageRp = 4,       // two-pass imaging: row pairs per CTA (pass B)
+  kTuneDirectMax = 5,     // two-kernel route: most cells per column for the direct-sum column transform, +1 (default 13)
+  kTuneDynspecRoute = 6,  // blink_dynspec: 1 = register-load kernel even for aligned cubes
+  kTuneSpare = 7
+};
+
 struct HostGather {    // cell-sorted tables of one channel (see blink_host_build_gather)
   int32_t n_kept = 0, n_can = 0;
   std::vector<int32_t> can_cell, seg_start, src;
@@ -43,6 +57,7 @@ struct blink_plan {
   int device = 0;
   int sm_count = 148;
   int max_smem_optin = 0;
+  blink_options opt = {};           // as given to blink_plan_create_opts (zeros = defaults)
 
   // inputs kept for blink_plan_set_corrections
   std::vector<double> h_ant, h_freq;
@@ -105,6 +120,9 @@ struct blink_plan {
   int vtile8_max = 0;               // most cells in any 8-column tile of any channel
   float2 *d_tw32 = nullptr;         // [32][32] exp(+2 pi i b n1 / 1024) (wfft.cuh), N = 1024 only
   int warp_route = 0;               // 1 = blink_grid_image takes the warp-per-transform kernel (blink_image_w.cu)
+  int seg_len_max = 0;              // most baselines in any canonical cell of any channel
+  int warp_ring = 0;                // slots of U in the warp route's ring
+  long long warp_snap_cap = 0;      // snapshots per call the warp route's counters in scratch are sized for
   // blink_grid, ring route (see grid_ring_build in blink_grid.cu): phase S as in k_fused
   int ring_path = 0;                // 1 = k_grid_ring available
   int ring_min_snap = 0;            // fewer snapshots per call take the band route
@@ -153,6 +171,7 @@ struct ImgParams {
 int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st);
 bool warp_route_applies(const blink_plan *p);
 size_t warp_route_scratch_bytes(const blink_plan *p, long long n_snap);
+size_t warp_route_ring_bytes(const blink_plan *p);
 
 }  // namespace blink
 
@@ -169,15 +188,23 @@ int launch_grid(const blink_plan *p, const float2 *vis, int n_snap, int ch0, flo
 int launch_image(const blink_plan *p, const float2 *uv, int n_snap, int ch0, float *img, cudaStream_t st);
 int image_setup(blink_plan *p);
 int image_reserve(blink_plan *p, int n_t);
+// device scratch a call of n_t time steps needs: blink_image (fused = false) or blink_grid_image
+size_t scratch_need(const blink_plan *p, long long n_t, bool fused);
 int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st);
 int fused_setup(blink_plan *p);
 int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st);
 int fused_line_stride(int n_pix);
-int fused_reserve(blink_plan *p, int n_t);
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);
 int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, float *img, cudaStream_t st);
 
 }  // namespace blink
+
+// hot calls: the plan's device must be current
+inline int check_device(const blink_plan *p) {
+  int d = -1;
+  if (cudaGetDevice(&d) != cudaSuccess) return BLINK_ECUDA;
+  return d == p->device ? BLINK_OK : BLINK_EINVAL;
+}
 
 #define BLINK_CUDA_TRY(expr, where)                 \
   do {                                              \
@@ -187,3 +214,17 @@ int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, fl
       return BLINK_ECUDA;                           \
     }                                               \
   } while (0)
+
+namespace blink {
+// cudaFuncSetAttribute is per device: `done` holds one bit per device ordinal that has it.  The
+// attribute is set to the device's opt-in maximum once, so no launch ever needs to raise it again.
+template <class K> inline int ensure_max_smem(K kern, const blink_plan *p, std::atomic<uint64_t> &done, const char *what,
+                                              bool carveout = true) {
+  const uint64_t bit = 1ull << (p->device & 63);
+  if (done.load(std::memory_order_acquire) & bit) return BLINK_OK;
+  BLINK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, p->max_smem_optin), what);
+  if (carveout) BLINK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100), what);
+  done.fetch_or(bit, std::memory_order_release);
+  return BLINK_OK;
+}
+}  // namespace blink

@@ -220,6 +220,7 @@ extern "C" const char *blink_strerror(int status) {
     case BLINK_ENOMEM: return "out of memory";
     case BLINK_ECUDA: return "CUDA error or no CUDA device";
     case BLINK_EUNSUPPORTED: return "not supported by this build";
+    case BLINK_ERESERVE: return "plan scratch too small for this n_t: call blink_plan_reserve first";
     default: return "unknown status";
   }
 }
@@ -243,6 +244,21 @@ extern "C" int blink_host_build_gather(const int32_t *cell, int n_bl, int n_pix,
 extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int n_ant,
                                  const double *freq_hz, int n_ch, int n_pix, double pixscale,
                                  int weighting, void *stream) {
+  return blink_plan_create_opts(out, ant_enu_m, n_ant, freq_hz, n_ch, n_pix, pixscale, weighting, stream, nullptr);
+}
+
+extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m, int n_ant,
+                                      const double *freq_hz, int n_ch, int n_pix, double pixscale,
+                                      int weighting, void *stream, const blink_options *opts) {
+  blink_options opt = {};
+  if (opts) {
+    if (opts->struct_size != (int32_t)sizeof(blink_options)) return BLINK_EINVAL;
+    opt = *opts;
+    auto route_ok = [](int32_t v) { return v == 0 || v == -1; };
+    if (!route_ok(opt.fused_route) || !route_ok(opt.polyphase) || !route_ok(opt.warp_route) || !route_ok(opt.grid_ring) ||
+        opt.warp_ring < 0 || opt.warp_ring == 1 || opt.grid_ring_min_snap < 0 || opt.image_chunk_mb < 0)
+      return BLINK_EINVAL;
+  }
   if (!out || !ant_enu_m || !freq_hz || n_ant < 2 || n_ant > 4096 || n_ch < 1 || n_ch > 65535 ||
       !(pixscale > 0.0) || (weighting != BLINK_NATURAL && weighting != BLINK_UNIFORM))
     return BLINK_EINVAL;
@@ -257,6 +273,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   blink_plan *p = new (std::nothrow) blink_plan();
   if (!p) return BLINK_ENOMEM;
   p->device = dev;
+  p->opt = opt;
   p->n_ant = n_ant;
   p->n_bl = n_ant * (n_ant - 1) / 2;
   p->n_ch = n_ch;
@@ -322,12 +339,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
   PLAN_CUDA(ce, "plan upload / index kernel");
 
   // ---- host: per-channel facts, gather and placement tables -------------------------------
-  {
-    long bc = kBandCellsDefault;
-    if (const char *e = getenv("BLINK_GRID_BAND_CELLS")) bc = atol(e);
-    if (bc < 256 || (bc & (bc - 1))) bc = kBandCellsDefault;
-    p->band_cells = (int)std::min<size_t>(NN, (size_t)bc);
-  }
+  p->band_cells = (int)std::min<size_t>(NN, (size_t)kBandCellsDefault);
   p->n_bands = (int)(NN / p->band_cells);
   p->n_dropped.assign(n_ch, 0); p->wsum.assign(n_ch, 0); p->n_occ.assign(n_ch, 0);
   p->norm.assign(n_ch, 0.0); p->chinfo.assign(n_ch, ChannelInfo());
@@ -382,6 +394,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
       h_pcode[(size_t)ch * 2 * n_bl + k] = pl[k].second;
     }
     p->n_can_max = std::max(p->n_can_max, (int)g.n_can);
+    for (int j = 0; j < g.n_can; ++j) p->seg_len_max = std::max(p->seg_len_max, g.seg_start[j + 1] - g.seg_start[j]);
     p->kx_max_all = std::max(p->kx_max_all, kxm);
     p->ky_max_all = std::max(p->ky_max_all, kym);
   }
@@ -389,19 +402,12 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
 
   // ---- gridder tables: rank-major stage slots, cells by descending per-pass length ------------
   {
-    int nbuf = 3;
-    if (const char *e = getenv("BLINK_GRID_NBUF")) nbuf = atoi(e);
-    if (nbuf < 2 || nbuf > 4) nbuf = 3;
-    p->grid_nbuf = nbuf;
-    // CTA shape (threads, prefetch, CTAs/SM): variant 0 = 512 x 16 x 1, 1 = 256 x 16 x 2,
-    // 2 = 512 x 8 x 2, 3 = 256 x 8 x 3
-    int variant = 0;
-    if (const char *e = getenv("BLINK_GRID_VARIANT")) variant = atoi(e);
-    static const int kVar[4][3] = {{512, 16, 1}, {256, 16, 2}, {512, 8, 2}, {256, 8, 3}};
-    if (variant < 0 || variant > 3) variant = 0;
-    p->grid_threads = kVar[variant][0];
-    p->grid_prefetch = kVar[variant][1];
-    p->grid_ctas_per_sm = kVar[variant][2];
+    // CTA shape: 512 threads x 16 visibilities in registers, one CTA per SM (256 x 16 x 2, 512 x 8 x 2 and
+    // 256 x 8 x 3 measured slower in round 1)
+    p->grid_nbuf = 3;
+    p->grid_threads = 512;
+    p->grid_prefetch = 16;
+    p->grid_ctas_per_sm = 1;
     const int kStageCap = p->grid_threads * p->grid_prefetch;
     p->stage_cap = kStageCap;
     p->n_pass = (n_bl + kStageCap - 1) / kStageCap;
@@ -526,8 +532,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
     step(cudaMemcpyAsync(p->d_vcol, h_vcol.data(), sizeof(int32_t) * h_vcol.size(), cudaMemcpyHostToDevice, st));
     step(cudaStreamSynchronize(st));
     PLAN_CUDA(ce, "vis-route table upload");
-    p->warp_route = warp_route_applies(p) ? 1 : 0;
-    if (const char *e = getenv("BLINK_IMAGE_WARP")) p->warp_route = (atoi(e) != 0 && warp_route_applies(p)) ? 1 : 0;
+    p->warp_route = (p->opt.warp_route != -1 && warp_route_applies(p)) ? 1 : 0;
   }
   PLAN_TRY(fused_build(p, gathers, st));
   PLAN_TRY(grid_ring_build(p, gathers, st));
@@ -585,9 +590,9 @@ extern "C" int blink_plan_destroy(blink_plan *plan) {
 
 extern "C" int blink_plan_reserve(blink_plan *plan, int n_t) {
   if (!plan || n_t < 0) return BLINK_EINVAL;
-  int rc = image_reserve(plan, n_t);
+  int rc = check_device(plan);
   if (rc != BLINK_OK) return rc;
-  return fused_reserve(plan, n_t);
+  return image_reserve(plan, n_t);
 }
 
 extern "C" int blink_plan_read(const blink_plan *p, int what, int ch, void *dst, size_t bytes) {

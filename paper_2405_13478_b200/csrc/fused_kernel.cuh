@@ -302,14 +302,9 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
 template <int N, int NZ, int D = 1>
 static int launch_fused_n(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
   constexpr int THREADS = kFusedThreads;
-  static thread_local size_t smem_set = 0;
-  if (p->fused_smem > smem_set) {
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS, NZ, D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        (int)p->fused_smem), "k_fused smem attribute");
-    BLINK_CUDA_TRY(cudaFuncSetAttribute(k_fused<N, THREADS, NZ, D>, cudaFuncAttributePreferredSharedMemoryCarveout, 100),
-                   "k_fused carveout");
-    smem_set = p->fused_smem;
-  }
+  static std::atomic<uint64_t> attr{0};
+  const int rc = ensure_max_smem(k_fused<N, THREADS, NZ, D>, p, attr, "k_fused smem attribute");
+  if (rc != BLINK_OK) return rc;
   const int blocks = std::min(fp.n_snap, p->sm_count);
   if (blocks <= 0) return BLINK_OK;
   k_fused<N, THREADS, NZ, D><<<blocks, THREADS, p->fused_smem, st>>>(fp);

@@ -199,9 +199,8 @@ static void build_chunk_table(const HostGather &g, const std::vector<int> &owner
     auto &pw = pieces[w];
     std::stable_sort(pw.begin(), pw.end(), [](const FusedPiece &a, const FusedPiece &b) { return a.len > b.len; });
     std::vector<PackGroup> groups;
-    static const int spare = getenv("BLINK_FUSED_SPARE") ? atoi(getenv("BLINK_FUSED_SPARE")) : 0;
-    static const int thresh = getenv("BLINK_FUSED_THRESH") ? atoi(getenv("BLINK_FUSED_THRESH")) : 99;
-    const int max_groups = ((int)pw.size() + 31) / 32 + spare;
+    constexpr int thresh = 99;               // a spare group is never opened for a colliding piece (measured: no gain)
+    const int max_groups = ((int)pw.size() + 31) / 32;
     for (const FusedPiece &pc : pw) {
       int bank[kFusedLcap];
       for (int k = 0; k < pc.len; ++k) bank[k] = ((g.src[pc.first + k] >> 1) - lo) & 15;   // buffers are 128-byte aligned
@@ -302,7 +301,7 @@ static void assign_cells(const HostGather &g, std::vector<int> &owner, std::vect
   auto len = [&](int j) { return g.seg_start[j + 1] - g.seg_start[j]; };
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return len(a) > len(b); });
   std::vector<long> load(kFusedWarps, 0);
-  static const int w0bias = getenv("BLINK_FUSED_W0BIAS") ? atoi(getenv("BLINK_FUSED_W0BIAS")) : 4;
+  constexpr int w0bias = 4;                  // percent of a warp's share
   load[0] = (long)g.n_kept * w0bias / (100 * kFusedWarps);     // warp 0 also runs the chunk ring (thread 0)
   owner.assign(g.n_can, 0);
   for (int j : order) {

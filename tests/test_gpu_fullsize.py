@@ -14,8 +14,8 @@ GRID_TOL = 1e-5
 IMG_TOL = 1e-4
 
 
-def _plan(blink, w, **kw):
-    return blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, **kw)
+def _plan(blink, w, **options):
+    return blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=options or None)
 
 
 def _fullsize_grid_image(torch, blink, oracle, w, sel, expect_path):

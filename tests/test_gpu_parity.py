@@ -45,8 +45,8 @@ ALL = ["tiny", "station", "station128", "station512", "mwa1", "mwa2", "mwa1_natu
        "station_uniform_32"]
 
 
-def _plan(blink, w):
-    return blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+def _plan(blink, w, **options):
+    return blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=options or None)
 
 
 @pytest.mark.parametrize("name", ALL)
@@ -115,13 +115,12 @@ def test_grid_and_image_match_oracle(torch_cuda, blink, oracle, name):
 
 
 @pytest.mark.parametrize("name", ["tiny", "station", "station128", "station512", "station_uniform_32"])
-def test_grid_ring_route_matches_oracle(torch_cuda, blink, oracle, name, monkeypatch):
+def test_grid_ring_route_matches_oracle(torch_cuda, blink, oracle, name):
     """blink_grid's ring route (k_grid_ring: gather tables streamed through shared memory with the
     visibilities) forced on small batches; bench-size batches take it by themselves."""
-    monkeypatch.setenv("BLINK_GRID_RING_MIN", "1")
     w = _workload(name)
     vis = w.vis()
-    plan = _plan(blink, w)
+    plan = _plan(blink, w, grid_ring_min_snap=1)
     uv, _ = _run_gpu(torch_cuda, plan, vis)
     uv2, _ = _run_gpu(torch_cuda, plan, vis)
     assert np.array_equal(uv.view(np.float32), uv2.view(np.float32)), "ring route must be bit-reproducible"
@@ -336,21 +335,19 @@ def test_grid_image_matches_two_calls_and_oracle(torch_cuda, blink, oracle, name
 
 
 @pytest.mark.parametrize("n_pix", [512, 1024])
-def test_polyphase_route_matches_two_kernel_route(torch_cuda, blink, oracle, n_pix, monkeypatch):
+def test_polyphase_route_matches_two_kernel_route(torch_cuda, blink, oracle, n_pix):
     """blink_grid_image on a compact array imaged at 512^2 / 1024^2 with uniform weighting: the
     polyphase shared-memory route (D x D interleaved 256^2 sub-images of one set of cell sums)
-    against the two-kernel route (BLINK_FUSED_POLY=0) on every snapshot, and against the oracle."""
+    against the two-kernel route (option polyphase = -1) on every snapshot, and against the oracle."""
     torch = torch_cuda
     w = synth.config_station(n_t=3, n_ch=3, n_pix=n_pix)
     w.weighting = synth.UNIFORM
     vis_h = w.vis()
     vis = torch.from_numpy(vis_h).cuda()
-    monkeypatch.setenv("BLINK_FUSED_POLY", "0")
-    plan0 = _plan(blink, w)
+    plan0 = _plan(blink, w, polyphase=-1)
     assert plan0.query_i32(blink.Q_FUSED_PATH) == 0
     ref = plan0.grid_image(vis)
     plan0.close()
-    monkeypatch.delenv("BLINK_FUSED_POLY")
     plan = _plan(blink, w)
     assert plan.query_i32(blink.Q_FUSED_PATH) == 1
     img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
@@ -370,7 +367,7 @@ def test_polyphase_route_matches_two_kernel_route(torch_cuda, blink, oracle, n_p
     plan.close()
 
 
-def test_warp_route_ring_reuse(torch_cuda, blink, oracle, monkeypatch):
+def test_warp_route_ring_reuse(torch_cuda, blink, oracle):
     """blink_grid_image, warp-per-transform route (k_img1024), on more snapshots than its ring of U
     slots holds (here a ring of 3), so that pass A has to wait for pass B to release a slot: every
     snapshot against the two-kernel route (same tables, fp32 rounding apart), sampled ones against
@@ -379,20 +376,17 @@ def test_warp_route_ring_reuse(torch_cuda, blink, oracle, monkeypatch):
     w = synth.config_mwa1(n_t=7, n_ch=3)
     vis_h = w.vis()
     vis = torch.from_numpy(vis_h).cuda()
-    monkeypatch.setenv("BLINK_IMAGE_WARP", "0")
-    plan0 = _plan(blink, w)
+    plan0 = _plan(blink, w, warp_route=-1)
     assert plan0.query_i32(blink.Q_FUSED_PATH) == 0
     ref = torch.empty((w.n_t, w.n_ch, w.n_pix, w.n_pix), dtype=torch.float32, device="cuda")
     plan0.grid_image(vis, ref)
     uv = plan0.grid(vis)
     img_lines = plan0.image(uv)             # blink_image on the line kernels (dense bounding-box read)
     plan0.close()
-    monkeypatch.delenv("BLINK_IMAGE_WARP")
-    monkeypatch.setenv("BLINK_W_RING", "3")
-    plan = _plan(blink, w)
+    plan = _plan(blink, w, warp_ring=3)
     assert plan.query_i32(blink.Q_FUSED_PATH) == 2
     img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
-    for _ in range(2):                      # twice: the counters are reset per call
+    for _ in range(3):                      # repeatedly: the kernel leaves its counters zero behind itself
         plan.grid_image(vis, img)
     torch.cuda.synchronize()
     assert torch.isfinite(img).all()
@@ -428,6 +422,119 @@ def test_host_pipeline_matches_device_path(torch_cuda, blink):
     HostPipeline(plan, w.n_t, chunk_t=3, depth=2).run(vis_h, img_h)
     torch.cuda.synchronize()
     assert torch.equal(img_h, ref.cpu())
+    plan.close()
+
+
+def test_boundary_contracts(torch_cuda, blink, oracle):
+    """What include/blink.h promises about the hot calls' arguments: (i) no allocation -- scratch comes
+    from blink_plan_reserve, else BLINK_ERESERVE; (ii) blink_grid accepts an 8-byte aligned vis (and
+    then avoids its bulk-copy route), blink_grid_image refuses one; (iii) options are validated."""
+    torch = torch_cuda
+    w = synth.config_station(n_t=2, n_ch=3, n_pix=128)
+    vis_h = w.vis()
+    plan = _plan(blink, w, grid_ring_min_snap=1)                      # would take the ring route if it could
+    uv = plan.grid(torch.from_numpy(vis_h).cuda())
+    with pytest.raises(blink.BlinkError) as ei:                       # blink_image needs scratch for U
+        plan.image(uv, auto_reserve=False)
+    assert ei.value.status == blink.ERESERVE
+    plan.reserve(1)
+    with pytest.raises(blink.BlinkError) as ei:                       # reserved for fewer time steps
+        plan.image(uv, auto_reserve=False)
+    assert ei.value.status == blink.ERESERVE
+    plan.reserve(w.n_t)
+    img = plan.image(uv, auto_reserve=False)
+    img2 = plan.grid_image(torch.from_numpy(vis_h).cuda(), auto_reserve=False)   # shared-memory route: no scratch
+    assert ((img - img2).abs() <= 1e-5 * img.abs().amax()).all()
+    # vis on an odd complex64 element: 8-byte aligned only
+    buf = torch.zeros(vis_h.size + 1, dtype=torch.complex64, device="cuda")
+    view = buf[1:].view(vis_h.shape)
+    view.copy_(torch.from_numpy(vis_h))
+    assert view.data_ptr() % 16 == 8
+    uv2 = plan.grid(view)
+    # the band route adds a cell's visibilities one by one, the ring route in pieces of up to four: equal up to fp32 rounding
+    assert (uv - uv2).abs().max() <= GRID_TOL * uv.abs().max()
+    assert torch.equal(plan.grid(view).view(torch.float32), uv2.view(torch.float32))
+    with pytest.raises(blink.BlinkError) as ei:
+        plan.grid_image(view)
+    assert ei.value.status == blink.EINVAL
+    plan.close()
+    for bad in (dict(fused_route=2), dict(warp_ring=1), dict(grid_ring_min_snap=-3)):
+        with pytest.raises(blink.BlinkError):
+            _plan(blink, w, **bad)
+    o = blink.Options()
+    o.struct_size = 12                                                 # not this header's struct
+    with pytest.raises(blink.BlinkError):
+        blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=o)
+
+
+def test_image_input_contract(torch_cuda, blink, oracle):
+    """blink_image is defined on "a grid of the plan" (zero where the weight count is zero, Hermitian):
+    blink_grid_validate says whether a grid is one.  blink_grid's outputs pass; a grid with one
+    non-plan cell set, or one cell made non-Hermitian, does not -- on the warp-per-transform route
+    (which reads only the plan's occupied cells) and on the line kernels alike.  Inside the bounding
+    box the line kernels do more than the contract asks: they symmetrise, i.e. return the real part of
+    the transform of the grid as given, which is checked against the oracle."""
+    torch = torch_cuda
+    # (a) warp route, N = 1024
+    w = synth.config_mwa1(n_t=1, n_ch=2)
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 2
+    uv = plan.grid(torch.from_numpy(w.vis()).cuda())
+    assert plan.validate(uv) == 0
+    cnt = plan.counts(1)
+    iy, ix = [int(v[0]) for v in np.nonzero(cnt == 0)]
+    bad = uv.clone()
+    bad[0, 1, iy, ix] = 1.0 + 2.0j                                      # a cell no baseline of the plan lands in
+    assert plan.validate(bad) >= 1
+    oy, ox = [int(v[5]) for v in np.nonzero(cnt > 0)]
+    bad = uv.clone()
+    bad[0, 0, oy, ox] += 1.0j                                          # occupied, but no longer conj of its mirror
+    assert plan.validate(bad) == 2
+    plan.close()
+    # (b) line kernels, N = 128: a non-Hermitian grid inside the bounding box -> Re of its transform
+    w = synth.config_tiny()
+    plan = _plan(blink, w)
+    uv = plan.grid(torch.from_numpy(w.vis()).cuda())
+    assert plan.validate(uv) == 0
+    kxm, kym = plan.bbox(0)
+    rng = np.random.default_rng(8)
+    g = uv.cpu().numpy()[0, 0].astype(np.complex128)
+    for _ in range(20):                                                # perturb cells inside the box, one side only
+        ky, kx = int(rng.integers(-kym, kym + 1)), int(rng.integers(-kxm, kxm + 1))
+        g[ky % w.n_pix, kx % w.n_pix] += complex(rng.standard_normal(), rng.standard_normal()) * 10.0
+    gd = torch.from_numpy(g.astype(np.complex64)).cuda().view(1, 1, w.n_pix, w.n_pix).contiguous()
+    assert plan.validate(gd) > 0
+    img = plan.image(gd).cpu().numpy()[0, 0]
+    ref, _ = oracle.dft2_separable(g.astype(np.complex64).astype(np.complex128), plan.norm(0))
+    assert np.max(np.abs(img - ref)) <= IMG_TOL * np.max(np.abs(ref))
+    plan.close()
+
+
+def test_many_small_snapshots(torch_cuda, blink, oracle):
+    """More snapshots in one call than a launch's gridDim.y allows (65535): the two-kernel imaging
+    route must cut the batch into chunks itself.  8 antennas, 32^2 grids, 70 000 snapshots."""
+    torch = torch_cuda
+    rng = np.random.default_rng(21)
+    ant = np.zeros((8, 3))
+    ant[:, :2] = rng.uniform(-6.0, 6.0, (8, 2))
+    freq = np.array([160e6, 161e6])
+    n_t, n = 35000, 32
+    plan = blink.Plan(ant, freq, n, 2.0 / n, synth.NATURAL, options=dict(fused_route=-1))
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 0
+    vis_h = (rng.standard_normal((n_t, 2, 28)) + 1j * rng.standard_normal((n_t, 2, 28))).astype(np.complex64)
+    vis = torch.from_numpy(vis_h).cuda()
+    img = torch.full((n_t, 2, n, n), float("nan"), dtype=torch.float32, device="cuda")
+    plan.image(plan.grid(vis), img)
+    img2 = torch.full((n_t, 2, n, n), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(vis, img2)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img).all() and torch.isfinite(img2).all()
+    sel = np.array([0, 65534, 65535, 65536, 2 * n_t - 1], np.int64)
+    ref = oracle.image_batch(ant, freq, n, 2.0 / n, synth.NATURAL, vis_h, sel)
+    for got in (img, img2):
+        gh = got.view(-1, n, n)[torch.from_numpy(sel).cuda()].cpu().numpy()
+        for q in range(len(sel)):
+            assert np.max(np.abs(gh[q] - ref["images"][q])) <= IMG_TOL * np.max(np.abs(ref["images"][q]))
     plan.close()
 
 

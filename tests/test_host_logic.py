@@ -25,15 +25,17 @@ def blink():
 
 
 def test_library_exports_every_declared_symbol(blink):
-    hdr = open(os.path.join(ROOT, "include", "blink.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(blink_[a-z_]+)\s*\(", hdr))
-    assert declared, "no declarations parsed"
     lib = blink.load()
-    for name in declared:
-        assert hasattr(lib, name), f"{name} declared in blink.h but not exported"
-    assert declared == set(blink.EXPORTS)
-    assert lib.blink_version() == 100
+    for header, names in (("blink.h", blink.EXPORTS), ("blink_testing.h", blink.TESTING_EXPORTS)):
+        hdr = open(os.path.join(ROOT, "include", header)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        declared = set(re.findall(r"\b(blink_[a-z_]+)\s*\(", hdr))
+        assert declared, "no declarations parsed"
+        for name in declared:
+            assert hasattr(lib, name), f"{name} declared in {header} but not exported"
+        assert declared == set(names)
+    assert lib.blink_version() == 200
+    assert ctypes.sizeof(blink.Options) == 64          # blink_options: 8 + 8 int32
     assert lib.blink_strerror(-3).decode().startswith("CUDA")
 
 
