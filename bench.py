@@ -1,18 +1,24 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the BLINK hot path (blink_grid + blink_image) on synthetic workloads.
+"""bench.py -- throughput of the BLINK hot path on synthetic workloads, one JSON line (rank 0).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload station|mwa1|mwa2|sweep256|...]
     python bench.py --impl reference ...        # times the CPU oracle instead (reference arm)
 
-A "step" is one pass of the whole hot path (grid every snapshot, image every snapshot) over one
-batch of synthetic visibilities already resident in HBM.  Prints ONE JSON line (rank 0).
-Default workload = BASELINE.json configs[1] (SKA-Low station, 100 t x 32 ch x 32640 bl, 256^2).
+A "step" is one pass of the whole hot path (steps a0-a5 of SURVEY.md section 8: grid every snapshot,
+weight, inverse DFT, shift, normalise, real part) over one batch of synthetic visibilities already
+resident in HBM, through the public call blink_grid_image (`--path separate`: blink_grid +
+blink_image with the uv grids in HBM).  Headline workload = BASELINE.json configs[1] (SKA-Low
+station, 100 t x 32 ch x 32640 bl, 256^2); at N = 1 the same process also times configs[2] (MWA
+Phase I, 1024^2) and configs[4] at 512^2 and reports them under "workloads".
 """
 from __future__ import annotations
 
 import argparse
+import glob
 import json
+import math
 import os
+import re
 import subprocess
 import sys
 import time
@@ -22,7 +28,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2405_13478_b200 import synth  # noqa: E402
+from paper_2405_13478_b200 import shard, synth  # noqa: E402
 
 
 def make_workload(name: str):
@@ -40,16 +46,11 @@ def make_workload(name: str):
 
 
 def algorithmic_bytes(w):
-    """per snapshot, blink_grid reads 8 n_bl and writes 8 N^2; blink_image
-    reads 8 N^2 and writes 4 N^2 (count/index tables are per-plan, excluded)."""
+    """SURVEY.md section 8(d), per snapshot: blink_grid reads 8 n_bl and writes 8 N^2; blink_image reads
+    8 N^2 and writes 4 N^2; the one-call route has no uv grid in HBM: B_fused = 8 n_bl + 4 N^2
+    (count/index tables are per-plan, excluded)."""
     nn = w.n_pix * w.n_pix
-    return dict(grid=8 * w.n_bl + 8 * nn, image=12 * nn, step=8 * w.n_bl + 20 * nn)
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch at the bench's own
-# size, from `ncu --set full` captures (profiles/r01_README.md); None where no capture exists
-NCU_TRAFFIC_BYTES = {("station", "fused", 100): 848_063_232 + 784_796_416,      # k_fused<256,512,3,1>
-                     ("mwa1", "fused", 100): 175_624_704 + 10_052_818_000}      # k_img1024 (profiles/r01aa_k_img1024_summary.txt)
+    return dict(grid=8 * w.n_bl + 8 * nn, image=12 * nn, sep=8 * w.n_bl + 20 * nn, fused=8 * w.n_bl + 4 * nn)
 
 
 def measured_peaks():
@@ -58,6 +59,28 @@ def measured_peaks():
         with open(p) as f:
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
+def ncu_traffic(workload: str, path: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch at the bench's own
+    size, from the newest committed `ncu --set full` summary profiles/r*_<workload>_<path>_fullsize_summary.txt
+    (written by `python -m paper_2405_13478_b200.ncu_summary`); None when there is none.  The file name
+    and its modification time go into the line: the capture is of the commit it was taken at."""
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{workload}_{path}_fullsize_summary.txt")))
+    if not files:
+        return None, None
+    f = files[-1]
+    tot = 0.0
+    for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+        m = re.search(rf"^{re.escape(key)}\s+([0-9.,]+)\s+(\w+)", open(f).read(), re.M)
+        if not m or m.group(2) not in _UNIT:
+            return None, None
+        tot += float(m.group(1).replace(",", "")) * _UNIT[m.group(2)]
+    return int(tot), {"file": os.path.relpath(f, ROOT),
+                      "mtime": time.strftime("%Y-%m-%dT%H:%M:%SZ", time.gmtime(os.path.getmtime(f)))}
 
 
 class ClockSampler:
@@ -115,6 +138,16 @@ def ref_time_steps(args, w, scale=1.0):
     return max(1, min(w.n_t, -(-snaps // w.n_ch)))
 
 
+def workload_config(w, name):
+    return {"workload": f"{name}: {w.n_ant} antennas, {w.n_bl} baselines, {w.n_t} time steps x "
+                        f"{w.n_ch} channels = {w.n_snapshots} snapshots, {w.n_pix}x{w.n_pix} image, "
+                        f"{'natural' if w.weighting == 0 else 'uniform'} weighting",
+            "n_ant": w.n_ant, "n_bl": w.n_bl, "n_t": w.n_t, "n_ch": w.n_ch, "n_pix": w.n_pix,
+            "weighting": "natural" if w.weighting == 0 else "uniform",
+            "l2_policy": "inputs larger than L2: each step streams the whole batch of visibilities and images "
+                         "(>= 0.8 GB) through the 126 MB L2"}
+
+
 def run_reference(args, w):
     """Reference arm = the CPU oracle as it stands, on the host cores, on a bounded sample."""
     rank = int(os.environ.get("RANK", "0"))
@@ -151,14 +184,162 @@ def run_reference(args, w):
     }))
 
 
-def workload_config(w, name):
-    return {"workload": f"{name}: {w.n_ant} antennas, {w.n_bl} baselines, {w.n_t} time steps x "
-                        f"{w.n_ch} channels = {w.n_snapshots} snapshots, {w.n_pix}x{w.n_pix} image, "
-                        f"{'natural' if w.weighting == 0 else 'uniform'} weighting",
-            "n_ant": w.n_ant, "n_bl": w.n_bl, "n_t": w.n_t, "n_ch": w.n_ch, "n_pix": w.n_pix,
-            "weighting": "natural" if w.weighting == 0 else "uniform",
-            "l2_policy": "inputs larger than L2: each step streams vis, uv grids and images "
-                         "(>= 0.8 GB each) through the 126 MB L2"}
+def cpu_baseline(w, args):
+    """The oracle as it stands, timed on this box's host cores, on a bounded sample: (i) all cores
+    (OpenMP over snapshots); (ii) ONE thread -- the paper's CPU imager is single-threaded
+     -- with gridding and the transform timed separately like its Tables 5-6
+    (PAPER.md:493-506, :546-565)."""
+    from oracle import oracle as orc
+    orc.build()
+    n_t_s = ref_time_steps(args, w)
+    vis = w.vis(0, n_t_s)
+    sel = np.arange(n_t_s * w.n_ch, dtype=np.int64)
+    t0 = time.perf_counter()
+    out = orc.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel,
+                          want_grids=False, want_images=True, n_threads=0)
+    dt = time.perf_counter() - t0
+    cores = out["threads"]
+    # single thread on 1/cores of that sample (same CPU seconds), at least 4 snapshots
+    sel1 = sel[:max(min(4, len(sel)), len(sel) // max(cores, 1))]
+    t0 = time.perf_counter()
+    orc.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel1,
+                    want_grids=True, want_images=False, n_threads=1)          # cell rule + gridding only
+    dt_grid = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    orc.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel1,
+                    want_grids=False, want_images=True, n_threads=1)          # whole chain
+    dt_all = time.perf_counter() - t0
+    return {"value": len(sel) / dt, "unit": "images/s", "cores": cores, "kind": "oracle",
+            "seconds": dt,
+            "sample": f"first {n_t_s} of {w.n_t} time steps x {w.n_ch} channels = {len(sel)} snapshots, "
+                      "fp64 gridding + naive separable DFT (O(N^3)), OpenMP over snapshots",
+            "single_thread": {"value": len(sel1) / dt_all, "unit": "images/s", "cores": 1,
+                              "snapshots": int(len(sel1)), "ms_per_image": 1e3 * dt_all / len(sel1),
+                              "gridding_ms_per_image": 1e3 * dt_grid / len(sel1),
+                              "dft_ms_per_image": 1e3 * max(dt_all - dt_grid, 0.0) / len(sel1),
+                              "note": "gridding = uv cells + accumulate (fp64); dft = weighting + naive separable "
+                                      "DFT; the paper's single-threaded CPU imager (FFTW) took 4.6-195 ms gridding "
+                                      "and 0.34-1481 ms FFT per image (PAPER.md Table 6, other hardware)"}}
+
+
+def probe_alu_peak(torch, blink, stream):
+    """the fp32 peak is measured in-run, by timing blink_probe_fp32 (a register-only
+    kernel, eight independent chains per thread) for scalar / packed adds and FMAs."""
+    out = torch.empty(148 * 16 * 256, dtype=torch.float32, device="cuda")
+    res = {}
+    for op, name in enumerate(["fadd", "ffma", "fadd2", "ffma2"]):
+        blink.probe_fp32(op, 64, out)                                  # warm-up
+        best = 0.0
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            flops = blink.probe_fp32(op, 2048, out)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            best = max(best, flops / (e0.elapsed_time(e1) / 1e3) / 1e12)
+        res[f"{name}_tflops"] = best
+    res["how"] = ("blink_probe_fp32 (csrc/blink_probe.cu): 2368 CTAs x 256 threads x 2048 x 64 instructions of one "
+                  "kind in 8 independent chains, CUDA events, best of 3; an FMA counts 2 flops, packed f32x2 "
+                  "instructions count both lanes")
+    return res
+
+
+def algorithmic_flops(w, plan, blink):
+    """fp32 work per snapshot that the method needs (ALU side bound of SURVEY.md section 8(d)):
+    gridding 2 adds per kept visibility (Hermitian half-plane), plus the Hermitian two-pass transform,
+    a 1-D transform of length N counted 5 N log2 N.  Pass A: kx_max + 1 columns; on the
+    warp-per-transform route (wide sparse half-planes) it is what that route computes -- per occupied
+    half-plane cell one complex multiply-add into each of 32 partial sums (8 x 32 flops), per column a
+    32-point butterfly on each of 32 lanes plus its twiddles.  Pass B: N/2 complex row transforms (two
+    real rows each)."""
+    n = w.n_pix
+    kxm = max(plan.bbox(c)[0] for c in range(w.n_ch))
+    fft = 5.0 * n * math.log2(n)
+    grid = 2.0 * w.n_bl
+    pass_b = (n / 2) * fft
+    if plan.query_i32(blink.Q_FUSED_PATH) == 2:
+        half_cells = np.mean([plan.n_occ(c) for c in range(w.n_ch)]) / 2.0
+        pass_a = half_cells * 8.0 * 32 + (kxm + 1) * (32 * 5.0 * 32 * 5 + 6.0 * n)
+        form = "sparse pass A (warp route)"
+    else:
+        pass_a = (kxm + 1) * fft
+        form = "dense pruned pass A"
+    return grid + pass_a + pass_b, form
+
+
+def time_steps(torch, plan, vis, img, uv, steps, warmup, stream, barrier):
+    """W untimed + K timed steps, CUDA events on the launching stream; returns (total ms, per-call ms)."""
+    fused = uv is None
+
+    def one(ev=None, k=0):
+        if fused:
+            plan.grid_image(vis, img)
+            if ev:
+                ev[3 * k + 1].record(stream)
+        else:
+            plan.grid(vis, uv)
+            if ev:
+                ev[3 * k + 1].record(stream)
+            plan.image(uv, img)
+        if ev:
+            ev[3 * k + 2].record(stream)
+            ev[3 * k + 3].record(stream)
+
+    for _ in range(max(warmup, 3)):
+        one()
+    barrier()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3 * steps + 1)]
+    ev[0].record(stream)
+    for k in range(steps):
+        one(ev, k)
+    barrier()
+    total_ms = ev[0].elapsed_time(ev[3 * steps])
+    grid_ms = float(np.mean([ev[3 * k].elapsed_time(ev[3 * k + 1]) for k in range(steps)]))
+    image_ms = float(np.mean([ev[3 * k + 1].elapsed_time(ev[3 * k + 2]) for k in range(steps)]))
+    return total_ms, grid_ms, image_ms
+
+
+def roofline_of(w, plan, blink, name, path, ms_call, dom_bytes, n_snap, peak, peak_src, alu):
+    achieved = dom_bytes * n_snap / (ms_call / 1e3) / 1e9
+    traffic, src = ncu_traffic(name, path)
+    flops, form = algorithmic_flops(w, plan, blink)
+    tf = flops * n_snap / (ms_call / 1e3) / 1e12
+    t_hbm_us = dom_bytes / (peak * 1e9) * 1e6
+    side = None
+    if alu:
+        t_alu_us = flops / (alu["ffma2_tflops"] * 1e12) * 1e6
+        side = {"bound": "alu", "flops_per_snapshot": flops, "flop_model": form, "achieved_tflops": tf,
+                "peak_tflops_fma": alu["ffma2_tflops"], "frac_of_fma_peak": tf / alu["ffma2_tflops"],
+                "peak_tflops_add_only": alu["fadd2_tflops"], "frac_of_add_only_peak": tf / alu["fadd2_tflops"],
+                "alu_us_per_snapshot_at_fma_peak": t_alu_us, "hbm_us_per_snapshot_at_peak": t_hbm_us,
+                "binding": "alu" if t_alu_us > t_hbm_us else "hbm"}
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": traffic, "traffic_source": src, "peak_source": peak_src,
+            "algorithmic_bytes_per_snapshot": dom_bytes, "atomics": "none (atomic-free design)"}, side
+
+
+def extra_workload(torch, blink, name, steps, stream, peak, peak_src, alu):
+    """configs[2] / configs[4]@512 timed in the same process, through blink_grid_image."""
+    w = make_workload(name)
+    plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    plan.reserve(w.n_t)
+    vis = torch.from_numpy(w.vis()).cuda()
+    img = torch.empty((w.n_t, w.n_ch, w.n_pix, w.n_pix), dtype=torch.float32, device="cuda")
+    total_ms, call_ms, _ = time_steps(torch, plan, vis, img, None, steps, 3, stream, torch.cuda.synchronize)
+    n_snap = w.n_snapshots
+    ms = total_ms / steps
+    ab = algorithmic_bytes(w)
+    roof, side = roofline_of(w, plan, blink, name, "fused", call_ms, ab["fused"], n_snap, peak, peak_src, alu)
+    out = {"config": workload_config(w, name), "steps": steps, "ms_per_step": ms,
+           "images_per_s": n_snap / (ms / 1e3), "mvis_per_s": n_snap * w.n_bl / (ms / 1e3) / 1e6,
+           "route": {1: "shared-memory (k_fused)", 2: "warp-per-transform (k_img1024)", 0: "two kernels"}[
+               plan.query_i32(blink.Q_FUSED_PATH)],
+           "images_per_s_vs_sep_roofline": (n_snap / (ms / 1e3)) / (peak * 1e9 / ab["sep"]),
+           "roofline": roof, "side_bounds": side}
+    plan.close()
+    del vis, img
+    torch.cuda.empty_cache()
+    return out
 
 
 def main():
@@ -175,16 +356,22 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "separate", "fused"],
                     help="separate = blink_grid + blink_image (uv grid in HBM); fused = blink_grid_image; "
                          "auto = fused")
+    ap.add_argument("--extra-workloads", default="mwa1,sweep512",
+                    help="comma list of further workloads timed in the same process at N = 1 ('' = none)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-corrections", action="store_true",
-                    help="skip the side measurement of blink_correct (SURVEY.md 8(f) item f2)")
+                    help="skip the measurement of the pre-gridding corrections (SURVEY.md 8(f) item f2)")
     ap.add_argument("--no-cufft-ref", action="store_true",
                     help="skip the library reference (blink_grid + torch.fft.ifft2 = cuFFT C2C + shift/real/scale)")
     ap.add_argument("--no-dynspec", action="store_true",
                     help="skip the side measurement of blink_dynspec (SURVEY.md 8(f) item f4)")
+    ap.add_argument("--only-step", action="store_true", help="time the step only (profiling runs)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    if args.only_step:
+        args.no_cpu_baseline = args.no_e2e = args.no_corrections = args.no_cufft_ref = args.no_dynspec = True
+        args.extra_workloads = ""
 
     w = make_workload(args.workload)
     if args.n_t > 0:
@@ -210,7 +397,9 @@ def main():
     # ---- inputs: every rank images its own full batch (independent snapshots, no collective)
     w.seed = w.seed + 1000 * rank if rank else w.seed
     vis_h = torch.from_numpy(w.vis()).pin_memory()
+    t_plan = time.perf_counter()
     plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    t_plan = time.perf_counter() - t_plan
     plan.reserve(w.n_t)
     vis = vis_h.cuda(non_blocking=True)
     shape = (w.n_t, w.n_ch, w.n_pix, w.n_pix)
@@ -218,58 +407,39 @@ def main():
     args.path = "fused" if fused else "separate"
     uv = None if fused else torch.empty(shape, dtype=torch.complex64, device="cuda")
     img = torch.empty(shape, dtype=torch.float32, device="cuda")
-    img_h = torch.empty(shape, dtype=torch.float32).pin_memory()
     stream = torch.cuda.current_stream()
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        shard.barrier()
         torch.cuda.synchronize()
 
-    def step():
-        if fused:
-            plan.grid_image(vis, img)
-        else:
-            plan.grid(vis, uv)
-            plan.image(uv, img)
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-
-    # ---- timed region: exactly K steps, CUDA events on the launching stream
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3 * args.steps + 1)]
+    # ---- timed region: exactly K steps, CUDA events on the launching stream, clocks sampled during it
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
         time.sleep(0.25)
-    barrier()
-    ev[0].record(stream)
-    for k in range(args.steps):
-        if fused:
-            plan.grid_image(vis, img)
-            ev[3 * k + 1].record(stream)
-        else:
-            plan.grid(vis, uv)
-            ev[3 * k + 1].record(stream)
-            plan.image(uv, img)
-        ev[3 * k + 2].record(stream)
-        ev[3 * k + 3].record(stream)
-    barrier()
+    total_ms, grid_ms, image_ms = time_steps(torch, plan, vis, img, uv, args.steps, args.warmup, stream, barrier)
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = ev[0].elapsed_time(ev[3 * args.steps])
-    grid_ms = float(np.mean([ev[3 * k].elapsed_time(ev[3 * k + 1]) for k in range(args.steps)]))
-    image_ms = float(np.mean([ev[3 * k + 1].elapsed_time(ev[3 * k + 2]) for k in range(args.steps)]))
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = shard.max_over_ranks(total_ms, device="cuda")
     ms_per_step = total_ms / args.steps
     n_snap = w.n_snapshots
     value = world * n_snap / (ms_per_step / 1e3)
 
-    # ---- side measurement, outside the step: blink_correct (f2), a streaming complex multiply of the
-    # whole batch by the plan's factor table; algorithmic bytes 16 per visibility (read 8, write 8)
+    def timed(fn, n):
+        for _ in range(3):
+            fn()
+        barrier()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n):
+            fn()
+        b.record(stream)
+        barrier()
+        return a.elapsed_time(b) / n
+
+    # ---- f2, pre-gridding corrections: (i) fused into the gridder's load -- the same step
+    # with the plan's factor table applied to every visibility as it is read, no extra HBM traffic;
+    # (ii) the stand-alone pass blink_correct, 16 bytes per visibility
     corr = None
     if not args.no_corrections:
         rng = np.random.default_rng(w.seed + 7)
@@ -277,20 +447,22 @@ def main():
         gains = rng.uniform(0.5, 2.0, (w.n_ch, n_ant)) * np.exp(1j * rng.uniform(-np.pi, np.pi, (w.n_ch, n_ant)))
         plan.set_corrections(gains, rng.uniform(0.0, 300.0, n_ant), 0.1, -0.2)
         vis_c = torch.empty_like(vis)
-        for _ in range(3):
-            plan.correct(vis, vis_c)
-        barrier()
-        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        c0.record(stream)
-        for _ in range(args.steps):
-            plan.correct(vis, vis_c)
-        c1.record(stream)
-        barrier()
-        c_ms = c0.elapsed_time(c1) / args.steps
-        c_bytes = 16 * vis.numel()
-        corr = {"call": "blink_correct", "ms": c_ms, "algorithmic_bytes": c_bytes,
-                "achieved_gbs": c_bytes / (c_ms / 1e3) / 1e9, "gvis_per_s": vis.numel() / (c_ms / 1e3) / 1e9}
+        c_ms = timed(lambda: plan.correct(vis, vis_c), args.steps)
         del vis_c
+        c_bytes = 16 * vis.numel()
+        fused_corr = None
+        if hasattr(plan, "apply_corrections"):
+            plan.apply_corrections(True)
+            f_ms = timed(lambda: (plan.grid_image(vis, img) if fused else (plan.grid(vis, uv), plan.image(uv, img))),
+                         args.steps)
+            plan.apply_corrections(False)
+            fused_corr = {"ms_per_step": f_ms, "step_without_ms": ms_per_step,
+                          "extra_over_step": f_ms / ms_per_step - 1.0, "extra_hbm_bytes": 0}
+        corr = {"fused_at_load": fused_corr,
+                "separate_pass": {"call": "blink_correct", "ms": c_ms, "algorithmic_bytes": c_bytes,
+                                  "achieved_gbs": c_bytes / (c_ms / 1e3) / 1e9,
+                                  "extra_over_step": c_ms / ms_per_step,
+                                  "gvis_per_s": vis.numel() / (c_ms / 1e3) / 1e9}}
 
     # ---- library reference timed beside the hand-written transform (north_star item 3):
     # the paper's own design -- a dense batched C2C inverse FFT (cuFFT through torch.fft.ifft2) on the
@@ -312,25 +484,11 @@ def main():
             g = uv_c if wgt is None else uv_c * wgt
             f = torch.fft.ifft2(g, norm="forward")            # unnormalised inverse, e^{+i...}
             return torch.fft.fftshift(f.real, dim=(-2, -1)) * scale
-        for _ in range(3):
-            ref_img = cufft_step()
-        barrier()
-        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         n_f = max(1, min(args.steps, 5))
-        f0.record(stream)
-        for _ in range(n_f):
-            ref_img = cufft_step()
-        f1.record(stream)
-        barrier()
-        f_ms = f0.elapsed_time(f1) / n_f
+        f_ms = timed(cufft_step, n_f)
+        ref_img = cufft_step()
         ours = plan.image(uv_c)
-        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        g0.record(stream)
-        for _ in range(n_f):
-            plan.image(uv_c, ours)
-        g1.record(stream)
-        barrier()
-        o_ms = g0.elapsed_time(g1) / n_f
+        o_ms = timed(lambda: plan.image(uv_c, ours), n_f)
         peak_img = float(ref_img.abs().max())
         cufft = {"what": "torch.fft.ifft2 (cuFFT C2C inverse, batched) + weighting/fftshift/real/scale as torch ops, "
                          "on blink_grid's uv grids", "snapshots": n_tc * w.n_ch, "ms": f_ms,
@@ -345,33 +503,28 @@ def main():
     if not args.no_dynspec:
         state = torch.zeros((w.n_ch, w.n_pix, w.n_pix), dtype=torch.float32, device="cuda")
         dyn_out = torch.empty((w.n_pix, w.n_pix, w.n_ch, w.n_t), dtype=torch.float32, device="cuda")
-        for _ in range(3):
-            plan.dynspec(img, 0.1, state, dyn_out)
-        barrier()
-        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        d0.record(stream)
-        for _ in range(args.steps):
-            plan.dynspec(img, 0.1, state, dyn_out)
-        d1.record(stream)
-        barrier()
-        d_ms = d0.elapsed_time(d1) / args.steps
+        d_ms = timed(lambda: plan.dynspec(img, 0.1, state, dyn_out), args.steps)
         d_bytes = 8 * img.numel() + 8 * state.numel()
         dyn = {"call": "blink_dynspec", "alpha": 0.1, "ms": d_ms, "algorithmic_bytes": d_bytes,
                "achieved_gbs": d_bytes / (d_ms / 1e3) / 1e9, "images_per_s": n_snap / (d_ms / 1e3)}
         del dyn_out, state
 
-    # ---- end to end: pinned host visibilities in, images back to pinned host memory, per step
+    # ---- end to end through the C ABI with HOST buffers: one blink_grid_image_host call per step --
+    # pinned host visibilities in, images back to pinned host memory, chunked and overlapped inside the
+    # library on three streams; the copies are inside the timed region
     e2e = None
     if not args.no_e2e:
-        from paper_2405_13478_b200.pipeline import HostPipeline
-        pipe = HostPipeline(plan, w.n_t) if fused else None
+        img_h = torch.empty(shape, dtype=torch.float32).pin_memory()
+        if fused:
+            plan.reserve_host(max(1, -(-w.n_t // 8)))
 
-        def e2e_step():
-            if pipe is not None:                      # chunked, transfers overlapped with imaging
-                pipe.run(vis_h, img_h)
-            else:
+            def e2e_step():
+                plan.grid_image_host(vis_h, img_h)
+        else:
+            def e2e_step():
                 vis.copy_(vis_h, non_blocking=True)
-                step()
+                plan.grid(vis, uv)
+                plan.image(uv, img)
                 img_h.copy_(img, non_blocking=True)
         e2e_step()
         barrier()
@@ -382,68 +535,42 @@ def main():
             e2e_step()
         e1.record(stream)
         barrier()
-        te = torch.tensor([e0.elapsed_time(e1) / n_e], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * n_snap / (float(te.item()) / 1e3), "unit": "images/s",
-               "ms_per_step": float(te.item()),
-               "h2d_bytes_per_step": int(vis_h.numel() * vis_h.element_size()),
-               "d2h_bytes_per_step": int(img_h.numel() * img_h.element_size())}
+        te = shard.max_over_ranks(e0.elapsed_time(e1) / n_e, device="cuda")
+        h2d, d2h = int(vis_h.numel() * vis_h.element_size()), int(img_h.numel() * img_h.element_size())
+        e2e = {"value": world * n_snap / (te / 1e3), "unit": "images/s", "ms_per_step": te,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "call": "blink_grid_image_host (C ABI, host pointers)" if fused else "torch copies + blink_grid + blink_image",
+               "host_link_gbs_each_way": max(h2d, d2h) / (te / 1e3) / 1e9,
+               "note": "bound by the host link (PCIe): the step's 8 n_bl + 4 N^2 bytes per snapshot cross it once each way"}
+        del img_h
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline (HBM-bound scan/scatter work), dominant call
+    # ---- rank 0: rooflines
     peak, peak_src = measured_peaks()
+    alu = probe_alu_peak(torch, blink, stream)
     ab = algorithmic_bytes(w)
     if fused:
-        nn = w.n_pix * w.n_pix
-        ab["fused"] = 8 * w.n_bl + 4 * nn          # SURVEY.md 8(d) B_fused: no uv grid in HBM
         calls = {"blink_grid_image": (grid_ms, ab["fused"])}
-        ab["step"] = ab["fused"]
+        step_bytes = ab["fused"]
     else:
         calls = {"blink_grid": (grid_ms, ab["grid"]), "blink_image": (image_ms, ab["image"])}
+        step_bytes = ab["sep"]
     dom = max(calls, key=lambda k: calls[k][0])
-    achieved = calls[dom][1] * n_snap / (calls[dom][0] / 1e3) / 1e9
-    step_gbs = ab["step"] * n_snap / (ms_per_step / 1e3) / 1e9
+    roof, side = roofline_of(w, plan, blink, args.workload, args.path, calls[dom][0], calls[dom][1], n_snap, peak,
+                             peak_src, alu)
+    roof["kernel"] = dom
+    step_gbs = step_bytes * n_snap / (ms_per_step / 1e3) / 1e9
     chunks = -(-n_snap // max(1, plan.query_i32(blink.Q_IMAGE_CHUNK)))
+    fp = plan.query_i32(blink.Q_FUSED_PATH)
     if fused:
-        if plan.query_i32(blink.Q_FUSED_PATH) in (1, 2):
-            launches_per_step = 1
-        else:
-            launches_per_step = 2 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))
+        launches_per_step = 1 if fp in (1, 2) else 2 * (-(-n_snap // max(1, plan.query_i32(blink.Q_FUSED_CHUNK))))
     else:
-        launches_per_step = 1 + 2 * chunks
-    # side bound: fp32 work of the Hermitian two-pass transform + the gridding adds,
-    # against the rate the unit counts give (148 SMs x 128 lanes x SM clock, no FMA); DESIGN.md 7
-    import math
-    kxm = max(plan.bbox(c)[0] for c in range(w.n_ch))
-    flops = 5.0 * w.n_pix * math.log2(w.n_pix) * ((kxm + 1) + w.n_pix / 2) + 4.0 * w.n_bl
-    fp32_rate = 148 * 128 * 1.965e9
-    t_alu_us, t_hbm_us = flops / fp32_rate * 1e6, ab["step"] / (peak * 1e9) * 1e6
-    t_meas_us = ms_per_step * 1e3 / n_snap
-    side = {"hbm_us_per_snapshot": t_hbm_us, "alu_us_per_snapshot": t_alu_us,
-            "measured_us_per_snapshot": t_meas_us, "binding": "alu" if t_alu_us > t_hbm_us else "hbm",
-            "frac_of_binding": max(t_alu_us, t_hbm_us) / t_meas_us,
-            "flops_per_snapshot": flops, "fp32_rate_no_fma": fp32_rate}
-    roof = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak,
-            "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.path, w.n_t)), "peak_source": peak_src,
-            "algorithmic_bytes_per_snapshot": calls[dom][1]}
-    roof_hbm = None
-    if fused and t_alu_us > t_hbm_us:
-        # the one-call path is bound by fp32 arithmetic here (1024^2 and larger): report the ALU roofline
-        # of the contract -- flops of the Hermitian two-pass transform + gridding adds per launch over the
-        # launch time, against the rate the unit counts give without FMA (butterflies are mostly adds;
-        # DESIGN.md section 7) -- and keep the HBM figures beside it
-        roof_hbm = roof
-        tf = flops * n_snap / (calls[dom][0] / 1e3) / 1e12
-        roof = {"bound": "alu", "kernel": dom, "achieved": tf, "peak": fp32_rate / 1e12, "unit": "TFLOP/s",
-                "frac": tf / (fp32_rate / 1e12), "traffic": roof_hbm["traffic"],
-                "peak_source": "derived: 148 SMs x 128 fp32 lanes x 1.965 GHz, one flop per lane and cycle (DESIGN.md 7)",
-                "algorithmic_flops_per_snapshot": flops}
+        launches_per_step = 1 + (1 if fp == 2 else 2 * chunks)
+
     out = {
         "metric": "dirty_images_per_s", "value": value, "unit": "images/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
@@ -451,39 +578,32 @@ def main():
         "data": "synthetic", "mvis_per_s": value * w.n_bl / 1e6,
         "config": workload_config(w, args.workload),
         "path": args.path, "per_call_ms": {k: v[0] for k, v in calls.items()},
-        "images_per_s_vs_sep_roofline": value / (peak * 1e9 / (8 * w.n_bl + 20 * w.n_pix * w.n_pix)),
-        "roofline": roof, "roofline_hbm": roof_hbm,
+        "images_per_s_vs_sep_roofline": value / world / (peak * 1e9 / ab["sep"]),
+        "roofline": roof,
         "roofline_step": {"bound": "hbm", "achieved": step_gbs, "peak": peak, "unit": "GB/s",
-                          "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": ab["step"]},
-        "side_bounds": side,
-        "f2_corrections": dict(corr, frac_of_hbm_peak=corr["achieved_gbs"] / peak) if corr else None,
-        "cufft_reference": cufft,
+                          "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": step_bytes},
+        "side_bounds": side, "alu_peak": alu,
+        "plan_create_s": t_plan,
+        "f2_corrections": corr, "cufft_reference": cufft,
         "f4_dynspec": dict(dyn, frac_of_hbm_peak=dyn["achieved_gbs"] / peak) if dyn else None,
         "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
     }
+    if corr:
+        corr["separate_pass"]["frac_of_hbm_peak"] = corr["separate_pass"]["achieved_gbs"] / peak
+    plan.close()
+    del vis, img, uv
+    torch.cuda.empty_cache()
+    # ---- the other workloads north_star names, in the same process (N = 1 only)
+    if world == 1 and args.extra_workloads:
+        out["workloads"] = {}
+        for name in [x for x in args.extra_workloads.split(",") if x and x != args.workload]:
+            out["workloads"][name] = extra_workload(torch, blink, name, max(3, min(args.steps, 5)), stream, peak,
+                                                    peak_src, alu)
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, args)
     print(json.dumps(out))
-    plan.close()
     if world > 1:
         dist.destroy_process_group()
-
-
-def cpu_baseline(w, args):
-    """The oracle as it stands, timed on this box's host cores, on a bounded sample."""
-    from oracle import oracle as orc
-    orc.build()
-    n_t_s = ref_time_steps(args, w)
-    vis = w.vis(0, n_t_s)
-    sel = np.arange(n_t_s * w.n_ch, dtype=np.int64)
-    t0 = time.perf_counter()
-    out = orc.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis, sel,
-                          want_grids=False, want_images=True, n_threads=0)
-    dt = time.perf_counter() - t0
-    return {"value": len(sel) / dt, "unit": "images/s", "cores": out["threads"], "kind": "oracle",
-            "seconds": dt,
-            "sample": f"first {n_t_s} of {w.n_t} time steps x {w.n_ch} channels = {len(sel)} snapshots, "
-                      "fp64 gridding + naive separable DFT (O(N^3)), OpenMP over snapshots"}
 
 
 if __name__ == "__main__":

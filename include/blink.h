@@ -258,6 +258,28 @@ int blink_dynspec(const blink_plan *plan, const void *images, int n_t, double al
 int blink_grid_image(const blink_plan *plan, const void *vis, int n_t, void *images, void *stream);
 
 /*
+ * blink_grid_image_host -- blink_grid_image for data in HOST memory: the end-to-end call.  The batch is
+ * cut into chunks of `chunk_t` time steps (set by blink_plan_reserve_host); the host-to-device copy of one
+ * chunk, the imaging of the previous one and the device-to-host copy of the one before run concurrently on
+ * three internal streams over a ring of plan-owned device buffers -- the interleaving of kernels and
+ * transfers with pinned host memory that the paper lists as its next optimisation.
+ * Results are bit-identical to blink_grid_image on the same visibilities.
+ *   vis_host     HOST complex64 [n_t][n_ch][n_bl]; page-locked (cudaHostAlloc / cudaHostRegister) for the
+ *                copies to overlap -- pageable memory works, but the copies then serialise with the host
+ *   images_host  HOST float32   [n_t][n_ch][N][N]; same
+ * Asynchronous: ordered after the work already in `stream`, and `stream` waits for its completion, so
+ * the host buffers must stay valid (and images_host unread) until `stream` has been synchronised.  No
+ * allocation: BLINK_ERESERVE until blink_plan_reserve_host has run.  Not concurrent with any other call
+ * on the same plan.  The transfers bound it: 8 n_bl + 4 N^2 bytes per snapshot over the host link.
+ */
+int blink_grid_image_host(blink_plan *plan, const void *vis_host, int n_t, void *images_host, void *stream);
+
+/* allocates the staging of blink_grid_image_host for chunks of chunk_t time steps (three buffers of
+ * chunk_t x (8 n_ch n_bl + 4 n_ch N^2) bytes, streams, events) and blink_grid_image's own scratch for such a
+ * chunk; synchronises the device when it has to grow; never shrinks */
+int blink_plan_reserve_host(blink_plan *plan, int chunk_t);
+
+/*
  * blink_plan_read -- copies one channel's slice of a plan table to HOST memory (synchronous):
  *   what = BLINK_Q_CELL_IDX -> int32 [n_bl];  what = BLINK_Q_COUNTS -> uint32 [N*N];
  *   what = BLINK_Q_CORR -> complex64 [n_bl] (BLINK_EINVAL until blink_plan_set_corrections).

@@ -1,7 +1,8 @@
 /*
- * blink_testing.h -- host-only hooks of libblink exported for its test suite (tests/test_host_logic.py):
- * they run the plan's table builders and a byte-for-byte model of the gridding phase on the CPU, so the
- * host logic is testable without a GPU.  NOT part of the product ABI (include/blink.h); may change.
+ * blink_testing.h -- hooks of libblink exported for its test suite and its benchmark, NOT part of the
+ * product ABI (include/blink.h); may change.  blink_host_*: host-only, run the plan's table builders and a
+ * byte-for-byte model of the gridding phase on the CPU, so the host logic is testable without a GPU
+ * (tests/test_host_logic.py).  blink_probe_fp32: the in-run fp32 peak probe bench.py times.
  */
 #ifndef BLINK_TESTING_H_
 #define BLINK_TESTING_H_
@@ -43,6 +44,16 @@ int blink_host_build_gather(const int32_t *cell, int n_bl, int n_pix, int32_t *n
  */
 int blink_host_fused_emulate(const int32_t *cell, int n_bl, int n_pix, int chunk_vis, const float *vis,
                              float *sums, int32_t *stats);
+
+/*
+ * Measurement hook for bench.py (the fp32 peak is measured in-run): launches a
+ * register-only kernel of out_floats / 256 blocks x 256 threads, each thread running `iters` x 64
+ * instructions of one kind in eight independent chains: op 0 = add.f32, 1 = fma.rn.f32,
+ * 2 = add.rn.f32x2, 3 = fma.rn.f32x2.  Asynchronous on `stream`; the caller times it.
+ *   out_dev   DEVICE float [out_floats] (written, values meaningless)
+ *   flops     HOST   out: floating-point operations of the launch (an FMA counts 2)
+ */
+int blink_probe_fp32(int op, int iters, void *out_dev, size_t out_floats, int64_t *flops, void *stream);
 
 #ifdef __cplusplus
 }

@@ -23,8 +23,8 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ERESERVE = 0, -1, -2, -3, -4, -5
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create", "blink_plan_create_opts",
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
            "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct", "blink_dynspec",
-           "blink_image", "blink_grid_validate"]
-TESTING_EXPORTS = ["blink_host_build_gather", "blink_host_fused_emulate"]
+           "blink_image", "blink_grid_validate", "blink_grid_image_host", "blink_plan_reserve_host"]
+TESTING_EXPORTS = ["blink_host_build_gather", "blink_host_fused_emulate", "blink_probe_fp32"]
 
 
 class Options(ctypes.Structure):
@@ -78,6 +78,10 @@ def load() -> ctypes.CDLL:
     lib.blink_plan_create_opts.argtypes = [ctypes.POINTER(vp), vp, ci, vp, ci, ci, cd, ci, vp, ctypes.POINTER(Options)]
     lib.blink_grid_validate.restype = ci
     lib.blink_grid_validate.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_int64), vp]
+    lib.blink_grid_image_host.restype = ci
+    lib.blink_grid_image_host.argtypes = [vp, vp, ci, vp, vp]
+    lib.blink_plan_reserve_host.restype = ci
+    lib.blink_plan_reserve_host.argtypes = [vp, ci]
     lib.blink_plan_destroy.restype = ci
     lib.blink_plan_destroy.argtypes = [vp]
     lib.blink_plan_query.restype = ci
@@ -98,6 +102,8 @@ def load() -> ctypes.CDLL:
     lib.blink_correct.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_dynspec.restype = ci
     lib.blink_dynspec.argtypes = [vp, vp, ci, ctypes.c_double, vp, vp, vp]
+    lib.blink_probe_fp32.restype = ci
+    lib.blink_probe_fp32.argtypes = [ci, ci, vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_int64), vp]
     lib.blink_host_build_gather.restype = ci
     lib.blink_host_build_gather.argtypes = [vp, ci, ci, vp, vp, vp, vp]
     lib.blink_host_fused_emulate.restype = ci
@@ -149,6 +155,16 @@ def host_fused_emulate(cell: np.ndarray, n_pix: int, chunk_vis: int, vis: np.nda
     return dict(sums=sums[:stats[0]], n_can=int(stats[0]), groups=int(stats[1]), rows=int(stats[2]))
 
 
+def probe_fp32(op: int, iters: int, out, stream=None) -> int:
+    """blink_probe_fp32 (include/blink_testing.h): launches the fp32 peak probe on `out` (cuda float32
+    scratch), returns the flops of the launch; the caller times it."""
+    lib = load()
+    flops = ctypes.c_int64(0)
+    _check(lib.blink_probe_fp32(int(op), int(iters), out.data_ptr(), out.numel(), ctypes.byref(flops),
+                                _stream_ptr(stream)), "blink_probe_fp32")
+    return int(flops.value)
+
+
 class Plan:
     """blink_plan_create / blink_plan_destroy and the calls that take a plan."""
 
@@ -173,6 +189,7 @@ class Plan:
                                               int(weighting), _stream_ptr(stream), ctypes.byref(options)),
                    "blink_plan_create_opts")
         self._reserved_n_t = 0
+        self._host_chunk_t = 0
         self.n_ant, self.n_ch, self.n_pix = ant.shape[0], fr.shape[0], int(n_pix)
         self.n_bl = self.query_i32(Q_N_BL)
         self.weighting = int(weighting)
@@ -352,3 +369,25 @@ class Plan:
         _check(self._lib.blink_grid_image(self._h, vis.data_ptr(), n_t, images.data_ptr(),
                                           _stream_ptr(stream)), "blink_grid_image")
         return images
+
+    def reserve_host(self, chunk_t: int):
+        """blink_plan_reserve_host: staging of grid_image_host for chunks of chunk_t time steps."""
+        _check(self._lib.blink_plan_reserve_host(self._h, int(chunk_t)), "blink_plan_reserve_host")
+        self._host_chunk_t = max(self._host_chunk_t, int(chunk_t))
+        self._reserved_n_t = max(self._reserved_n_t, int(chunk_t))
+
+    def grid_image_host(self, vis_h, images_h, stream=None):
+        """blink_grid_image_host: vis_h complex64 CPU tensor [n_t, n_ch, n_bl] (pinned for overlap) ->
+        images_h float32 CPU tensor [n_t, n_ch, N, N]; asynchronous on the stream (synchronise it before
+        reading images_h).  Without an earlier reserve_host the chunk is ~1/8 of the batch."""
+        import torch
+        assert not vis_h.is_cuda and vis_h.dtype == torch.complex64 and vis_h.is_contiguous()
+        n_t = vis_h.shape[0]
+        assert tuple(vis_h.shape[1:]) == (self.n_ch, self.n_bl)
+        assert not images_h.is_cuda and images_h.dtype == torch.float32 and images_h.is_contiguous()
+        assert tuple(images_h.shape) == (n_t, self.n_ch, self.n_pix, self.n_pix)
+        if self._host_chunk_t == 0:
+            self.reserve_host(max(1, -(-n_t // 8)))
+        _check(self._lib.blink_grid_image_host(self._h, vis_h.data_ptr(), n_t, images_h.data_ptr(),
+                                               _stream_ptr(stream)), "blink_grid_image_host")
+        return images_h

@@ -49,6 +49,16 @@ struct HostGather {    // cell-sorted tables of one channel (see blink_host_buil
   std::vector<int32_t> can_cell, seg_start, src;
 };
 
+// blink_grid_image_host (blink_host.cu): three streams over a ring of device staging buffers
+struct HostPipe {
+  static constexpr int kDepth = 3;
+  int chunk_t = 0;                                  // time steps per chunk the buffers are sized for (0 = not reserved)
+  float2 *d_vis[kDepth] = {};
+  float *d_img[kDepth] = {};
+  cudaStream_t st[3] = {};                          // in, compute, out
+  cudaEvent_t in_done[kDepth] = {}, cmp_done[kDepth] = {}, out_done[kDepth] = {}, start = nullptr, done[3] = {};
+};
+
 }  // namespace blink
 
 struct blink_plan {
@@ -58,6 +68,7 @@ struct blink_plan {
   int sm_count = 148;
   int max_smem_optin = 0;
   blink_options opt = {};           // as given to blink_plan_create_opts (zeros = defaults)
+  blink::HostPipe hp;               // staging of blink_grid_image_host
 
   // inputs kept for blink_plan_set_corrections
   std::vector<double> h_ant, h_freq;
@@ -178,6 +189,7 @@ size_t warp_route_ring_bytes(const blink_plan *p);
 namespace blink {
 
 void set_cuda_error(cudaError_t e, const char *where);
+void host_pipe_free(blink_plan *p);
 int build_gather_host(const int32_t *cell, int n_bl, int n_pix, HostGather &out);
 
 // kernels' host launchers (each returns a blink_status)

@@ -14,6 +14,13 @@ def shard_time_steps(n_t: int, world: int, rank: int) -> tuple[int, int]:
     return t0, t0 + base + (1 if rank < extra else 0)
 
 
+def barrier() -> None:
+    """torch.distributed barrier (no-op when not initialised or world size 1)."""
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.barrier()
+
+
 def max_over_ranks(value: float, device=None) -> float:
     """MAX all-reduce of a scalar (identity when torch.distributed is not initialised)."""
     import torch

@@ -409,19 +409,41 @@ def test_warp_route_ring_reuse(torch_cuda, blink, oracle):
     plan.close()
 
 
-def test_host_pipeline_matches_device_path(torch_cuda, blink):
-    """The host-to-host streaming wrapper (chunked, overlapped transfers) returns exactly what
-    blink_grid_image returns on resident data, including a ragged last chunk."""
+def test_grid_image_host_matches_device_path(torch_cuda, blink):
+    """blink_grid_image_host (the C-ABI call with HOST pointers: chunked, transfers overlapped with the
+    imaging on three internal streams) returns exactly what blink_grid_image returns on resident data,
+    including a ragged last chunk, more chunks than staging buffers, repeated calls, pinned and pageable
+    host memory; BLINK_ERESERVE before blink_plan_reserve_host."""
     torch = torch_cuda
-    from paper_2405_13478_b200.pipeline import HostPipeline
-    w = synth.config_station(n_t=7, n_ch=4, n_pix=128)
+    w = synth.config_station(n_t=11, n_ch=4, n_pix=128)
+    vis_p = torch.from_numpy(w.vis())
+    vis_h = vis_p.pin_memory()
+    plan = _plan(blink, w)
+    ref = plan.grid_image(vis_h.cuda()).cpu()
+    img_h = torch.full(tuple(ref.shape), float("nan"), dtype=torch.float32).pin_memory()
+    rc = plan._lib.blink_grid_image_host(plan._h, vis_h.data_ptr(), w.n_t, img_h.data_ptr(), None)
+    assert rc == blink.ERESERVE
+    plan.reserve_host(3)                                   # 11 time steps = 3 + 3 + 3 + 2, four chunks over three buffers
+    for _ in range(2):
+        img_h.fill_(float("nan"))
+        plan.grid_image_host(vis_h, img_h)
+        torch.cuda.synchronize()
+        assert torch.equal(img_h, ref)
+    img_p = torch.full(tuple(ref.shape), float("nan"), dtype=torch.float32)      # pageable
+    plan.grid_image_host(vis_p, img_p)
+    torch.cuda.synchronize()
+    assert torch.equal(img_p, ref)
+    plan.close()
+    # a route that needs plan scratch (two kernels) behind the same call
+    w = synth.config_mwa1(n_t=3, n_ch=2)
     vis_h = torch.from_numpy(w.vis()).pin_memory()
     plan = _plan(blink, w)
-    ref = plan.grid_image(vis_h.cuda())
+    ref = plan.grid_image(vis_h.cuda()).cpu()
     img_h = torch.full(tuple(ref.shape), float("nan"), dtype=torch.float32).pin_memory()
-    HostPipeline(plan, w.n_t, chunk_t=3, depth=2).run(vis_h, img_h)
+    plan.reserve_host(2)
+    plan.grid_image_host(vis_h, img_h)
     torch.cuda.synchronize()
-    assert torch.equal(img_h, ref.cpu())
+    assert torch.equal(img_h, ref)
     plan.close()
 
 

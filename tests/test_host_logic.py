@@ -29,7 +29,7 @@ def test_library_exports_every_declared_symbol(blink):
     for header, names in (("blink.h", blink.EXPORTS), ("blink_testing.h", blink.TESTING_EXPORTS)):
         hdr = open(os.path.join(ROOT, "include", header)).read()
         hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-        declared = set(re.findall(r"\b(blink_[a-z_]+)\s*\(", hdr))
+        declared = set(re.findall(r"\b(blink_[a-z0-9_]+)\s*\(", hdr))
         assert declared, "no declarations parsed"
         for name in declared:
             assert hasattr(lib, name), f"{name} declared in {header} but not exported"
