@@ -77,7 +77,8 @@ typedef enum blink_query {
   BLINK_Q_IMAGE_CHUNK = 13, /* out: int32  snapshots per launch pair of the two-pass imaging path */
   BLINK_Q_FUSED_PATH = 14,  /* out: int32  route of blink_grid_image: 1 = shared memory, 2 = warp-per-transform, 0 = two kernels */
   BLINK_Q_FUSED_CHUNK = 15, /* out: int32  snapshots per chunk of the two-kernel route */
-  BLINK_Q_CORR = 16         /* out: const float2* DEVICE [n_ch][n_bl] correction factors (NULL until set) */
+  BLINK_Q_CORR = 16,        /* out: const float2* DEVICE [n_ch][n_bl] correction factors (NULL until set) */
+  BLINK_Q_CORR_FUSED = 17   /* out: int32  1 = blink_grid / blink_grid_image apply the factors at load */
 } blink_query;
 
 typedef struct blink_plan blink_plan; /* opaque */
@@ -202,6 +203,20 @@ int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *imag
  */
 int blink_plan_set_corrections(blink_plan *plan, const double *gains, const double *cable_len_m,
                                double l0, double m0, void *stream);
+
+/*
+ * blink_plan_apply_corrections -- the corrections fused into the gridder's load (SURVEY.md section 8(f)
+ * item f2).  on = 1: from now on blink_grid and blink_grid_image (and blink_grid_image_host) multiply
+ * every visibility by the plan's factor F[ch][bl] as they read it, i.e. they grid blink_correct's output
+ * without that pass existing: no extra kernel, and no extra HBM traffic beyond the 8-byte factors per
+ * (channel, baseline), which are shared by all time steps and stay in L2.  on = 0 (the default): the
+ * visibilities are gridded as given.  Needs a table (BLINK_EINVAL before blink_plan_set_corrections); a
+ * later blink_plan_set_corrections replaces the factors and leaves the switch as it is.  The first call
+ * with on = 1 builds the shared-memory table layouts that carry the factors (host work, synchronises
+ * `stream`); BLINK_Q_FUSED_PATH may change with the switch (a plan whose snapshots fit the SM without
+ * the factors but not with them falls back to the next route, which needs blink_plan_reserve).
+ */
+int blink_plan_apply_corrections(blink_plan *plan, int on, void *stream);
 
 /*
  * blink_correct -- vis_out[t][ch][bl] = vis_in[t][ch][bl] * F[ch][bl] (complex64 product), the

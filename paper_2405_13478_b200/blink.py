@@ -17,13 +17,14 @@ LIB_PATH = os.path.join(_HERE, "libblink.so")
 NATURAL, UNIFORM = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ERESERVE = 0, -1, -2, -3, -4, -5
 (Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
- Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK, Q_CORR) = range(17)
+ Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK, Q_CORR, Q_CORR_FUSED) = range(18)
 
 # include/blink.h (the product ABI) and include/blink_testing.h (host-only test hooks)
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create", "blink_plan_create_opts",
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
            "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct", "blink_dynspec",
-           "blink_image", "blink_grid_validate", "blink_grid_image_host", "blink_plan_reserve_host"]
+           "blink_image", "blink_grid_validate", "blink_grid_image_host", "blink_plan_reserve_host",
+           "blink_plan_apply_corrections"]
 TESTING_EXPORTS = ["blink_host_build_gather", "blink_host_fused_emulate", "blink_probe_fp32"]
 
 
@@ -98,6 +99,8 @@ def load() -> ctypes.CDLL:
     lib.blink_grid_image.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_plan_set_corrections.restype = ci
     lib.blink_plan_set_corrections.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp]
+    lib.blink_plan_apply_corrections.restype = ci
+    lib.blink_plan_apply_corrections.argtypes = [vp, ci, vp]
     lib.blink_correct.restype = ci
     lib.blink_correct.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_dynspec.restype = ci
@@ -263,6 +266,12 @@ class Plan:
                                                     c.ctypes.data if c is not None else None,
                                                     float(l0), float(m0), _stream_ptr(stream)),
                "blink_plan_set_corrections")
+
+    def apply_corrections(self, on: bool, stream=None):
+        """blink_plan_apply_corrections: on -> blink_grid / blink_grid_image multiply by the factors at load."""
+        _check(self._lib.blink_plan_apply_corrections(self._h, 1 if on else 0, _stream_ptr(stream)),
+               "blink_plan_apply_corrections")
+        self._reserved_n_t = 0 if on else self._reserved_n_t     # the route, hence the scratch needed, may change
 
     def corr_table(self, ch):
         """complex64 [n_bl] correction factors of channel ch, host copy."""

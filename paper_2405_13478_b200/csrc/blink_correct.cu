@@ -182,3 +182,23 @@ extern "C" int blink_correct(const blink_plan *p, const void *vis_in, int n_t, v
   BLINK_CUDA_TRY(cudaGetLastError(), "k_correct launch");
   return BLINK_OK;
 }
+
+// f2 as SURVEY.md section 8(f) words it: the corrections FUSED AT LOAD.  on = 1: blink_grid and
+// blink_grid_image multiply every visibility by its factor as they read it -- in shared memory on the
+// bulk-copy routes (the factors of a chunk ride in the same buffer as its visibilities and gather
+// table; their table layouts are built here, on first use), in registers on the others -- so no
+// separate 16-byte-per-visibility pass exists and the visibilities cross HBM once.
+extern "C" int blink_plan_apply_corrections(blink_plan *p, int on, void *stream) {
+  using namespace blink;
+  if (!p || (on != 0 && on != 1)) return BLINK_EINVAL;
+  int rc = check_device(p);
+  if (rc != BLINK_OK) return rc;
+  if (on && !p->d_corr) return BLINK_EINVAL;
+  if (on) {
+    cudaStream_t st = (cudaStream_t)stream;
+    if (p->fused_path == 1 && (rc = fused_layout(p, 1, st)) != BLINK_OK) return rc;
+    if (p->ring_path == 1 && (rc = grid_ring_layout(p, 1, st)) != BLINK_OK) return rc;
+  }
+  p->corr_on = on;
+  return BLINK_OK;
+}

@@ -34,43 +34,74 @@ int fused_setup(blink_plan *p) {
   return BLINK_OK;
 }
 
-// Decide whether the shared-memory route applies (two-stage transforms, N <= 256; everything
-// resident in one SM; 16-byte aligned snapshots, i.e. even n_bl, for the bulk copies), lay out
-// shared memory, build and upload the tables.  Layout (bytes):
-//   [0, region)             column lines + pass-B exchange lines; doubles as chunk buffers 1..nbuf-1
-//   [off_dedicated, +B)     chunk buffer 0            (B = chunk_vis * 8 + tab_stride, 128-aligned)
-//   [off_S, ...)            canonical cell sums, sink, zero slot
-//   [off_bar, ...)          full[nbuf], empty[nbuf], region_free mbarriers
-int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st) {
-  const int want = p->opt.fused_route != -1;
-  const int N = p->n_pix, n_bl = p->n_bl, n_ch = p->n_ch;
-  if (!want || N < 32 || (n_bl & 1) || p->max_smem_optin <= 0) return BLINK_OK;
+static int upload_table(void **dst, const void *src, size_t bytes, cudaStream_t st, const char *what) {
+  cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
+  if (e != cudaSuccess) {
+    set_cuda_error(e, what);
+    *dst = nullptr;
+    return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
+  }
+  BLINK_CUDA_TRY(cudaMemcpyAsync(*dst, src, bytes, cudaMemcpyHostToDevice, st), what);
+  return BLINK_OK;
+}
+
+// Geometry of the shared-memory route, common to its table layouts.  The route applies to two-stage
+// transforms (N <= 256 directly, 512 / 1024 as D x D sub-images of 256) whose bounding box fits, with
+// 16-byte aligned snapshots (even n_bl) for the bulk copies.
+struct FusedGeom {
+  int Ns, D, sink0, n_S, LS, n_col;
+  size_t region, region_al, s_bytes;
+};
+
+static bool fused_geom(const blink_plan *p, FusedGeom &g) {
+  const int N = p->n_pix;
+  if (p->opt.fused_route == -1 || N < 32 || (p->n_bl & 1) || p->max_smem_optin <= 0) return false;
   // polyphase route (see k_fused): a compact array on a large image is imaged as D x D interleaved
   // Ns x Ns sub-images, Ns = 256, when the bounding box fits the Ns transform
-  int Ns = N, D = 1;
+  g.Ns = N;
+  g.D = 1;
   if (N > 256) {
     // (128-point sub-transforms were measured too: station 256^2 as 2 x 2 of 128^2 0.65 ms against
     // 0.42 ms direct, sweep512 as 4 x 4 1.92 ms against 1.36 ms as 2 x 2 of 256^2)
-    const int poly = p->opt.polyphase != -1;
-    Ns = 256;
-    D = N / Ns;
-    if (!poly || D > 4 || std::max(p->kx_max_all, p->ky_max_all) >= Ns / 2) return BLINK_OK;
+    g.Ns = 256;
+    g.D = N / g.Ns;
+    if (p->opt.polyphase == -1 || g.D > 4 || std::max(p->kx_max_all, p->ky_max_all) >= g.Ns / 2) return false;
   }
-  p->fused_D = D;
-  const int sink0 = (p->n_can_max + 15) & ~15;                    // S[sink0 + b]: the always-zero slot of bank b
-  const int n_S = sink0 + 16;
-  if (n_S > 0x3FFF) return BLINK_OK;                              // 14-bit slot index in the phase-H records
-  const int LS = fused_line_stride(Ns);
-  const int n_col = p->kx_max_all + 1;
-  if ((size_t)n_col * LS >= 0xFFFFu) return BLINK_OK;             // 16-bit line position
-  const int T = Ns / 16, G = kFusedThreads / T;
-  const size_t region = sizeof(float2) * ((size_t)n_col * LS + (size_t)G * (Ns + Ns / 16));
-  const size_t region_al = (region + 127) / 128 * 128;
-  const size_t s_bytes = sizeof(float2) * ((size_t)n_S + (D > 1 ? (size_t)D * (Ns / 2) : 0));   // sums (+ column phases)
+  g.sink0 = (p->n_can_max + 15) & ~15;                            // S[sink0 + b]: the always-zero slot of bank b
+  g.n_S = g.sink0 + 16;
+  if (g.n_S > 0x3FFF) return false;                               // 14-bit slot index in the phase-H records
+  g.LS = fused_line_stride(g.Ns);
+  g.n_col = p->kx_max_all + 1;
+  if ((size_t)g.n_col * g.LS >= 0xFFFFu) return false;            // 16-bit line position
+  const int T = g.Ns / 16, G = kFusedThreads / T;
+  g.region = sizeof(float2) * ((size_t)g.n_col * g.LS + (size_t)G * (g.Ns + g.Ns / 16));
+  g.region_al = (g.region + 127) / 128 * 128;
+  g.s_bytes = sizeof(float2) * ((size_t)g.n_S + (g.D > 1 ? (size_t)g.D * (g.Ns / 2) : 0));   // sums (+ column phases)
+  return true;
+}
+
+// One table layout of the route: corr = 0 plain, 1 = every chunk carries its correction factors too.
+// Shared memory (bytes):
+//   [0, region)             column lines + pass-B exchange lines; doubles as chunk buffers 1..nbuf-1
+//   [off_first, +B)         chunk buffer 0 (dedicated)
+//   [off_S, ...)            canonical cell sums, 16 zero slots (sinks), column phases
+//   [off_bar, ...)          full[nbuf], empty[nbuf], region_free mbarriers
+// A buffer holds V visibility slots, the chunk's gather table (tab_off = 8 V bytes in) and, with
+// corr, V factor slots (f_off = 8 V + tab_stride bytes behind the visibilities); V = chunk_vis, or
+// chunk_vis + 16 with corr: the 16 extra slots of buffer 0 and their factor partners are zeroed once
+// by the kernel and never written again -- the "zero visibility" a padded table entry points at must
+// have a finite factor behind it.
+int fused_layout(blink_plan *p, int corr, cudaStream_t st) {
+  GatherLayout &L = p->fl[corr];
+  if (L.ok) return BLINK_OK;
+  FusedGeom g;
+  if (!fused_geom(p, g) || (int)p->gathers.size() != p->n_ch) return BLINK_OK;
+  const int n_bl = p->n_bl, n_ch = p->n_ch;
   const size_t limit = (size_t)p->max_smem_optin;
+  const int zpad = corr ? 16 : 0;
 
   std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
-  for (int ch = 0; ch < n_ch; ++ch) assign_cells(gathers[ch], owner[ch], slot[ch]);
+  for (int ch = 0; ch < n_ch; ++ch) assign_cells(p->gathers[ch], owner[ch], slot[ch]);
 
   const int force_chunks = p->opt.tune[kTuneFusedChunks];
   std::vector<AbstractTable> tabs;
@@ -82,39 +113,43 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
     C = (C + 1) & ~1;                                  // 16-byte multiples
     if (C > 0x7FFE) continue;                          // 15-bit slot index relative to the chunk
     if ((n_bl + C - 1) / C != n_chunk) continue;
-    if (sizeof(float2) * (size_t)C + region_al + s_bytes > limit) continue;   // cannot fit whatever the tables
+    const size_t data_bytes = sizeof(float2) * (size_t)(C + zpad) * (corr ? 2 : 1);
+    if (data_bytes + g.region_al + g.s_bytes > limit) continue;   // cannot fit whatever the tables
     tabs.assign((size_t)n_ch * n_chunk, AbstractTable());
     bool ok = true;
     tab_stride = 0;
     for (int ch = 0; ch < n_ch && ok; ++ch)
       for (int c = 0; c < n_chunk && ok; ++c) {
         AbstractTable &t = tabs[(size_t)ch * n_chunk + c];
-        build_chunk_table(gathers[ch], owner[ch], slot[ch], c * C, std::min(n_bl, (c + 1) * C), sink0, t, ok);
+        build_chunk_table(p->gathers[ch], owner[ch], slot[ch], c * C, std::min(n_bl, (c + 1) * C), g.sink0, t, ok);
         tab_stride = std::max(tab_stride, t.bytes.size());
       }
     if (!ok) continue;
-    buf_bytes = (sizeof(float2) * (size_t)C + tab_stride + 127) / 128 * 128;
-    nbuf = 1 + (int)std::min<size_t>(7, region / buf_bytes);
+    buf_bytes = (data_bytes + tab_stride + 127) / 128 * 128;
+    nbuf = 1 + (int)std::min<size_t>(7, g.region / buf_bytes);
     nbuf = std::min(nbuf, n_chunk);
     if (nbuf < 2 && n_chunk > 1) continue;             // the ring needs a second buffer
-    const size_t total = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 8 + 64;
+    const size_t total = g.region_al + buf_bytes + g.s_bytes + 16 * (size_t)nbuf + 8 + 64;
     if (total > limit || total > 0x7FFFu * 8u) continue;
     found = true;
     break;
   }
   if (!found) return BLINK_OK;
 
-  p->fused_chunk_vis = C;
-  p->fused_n_chunk = n_chunk;
-  p->fused_nbuf = nbuf;
-  p->fused_tab_stride = (int)tab_stride;
-  p->fused_buf_bytes = (uint32_t)buf_bytes;
-  p->fused_off_dedicated = (uint32_t)region_al;
-  p->fused_off_S = (uint32_t)(region_al + buf_bytes);      // multiple of 128: slot s of S sits in bank s mod 16
-  p->fused_off_bar = (uint32_t)(region_al + buf_bytes + s_bytes);
-  p->fused_smem = region_al + buf_bytes + s_bytes + 16 * (size_t)nbuf + 8 + 16;
-  p->fused_threads = kFusedThreads;
-  const uint32_t s_slot0 = p->fused_off_S / 8;
+  L.chunk_vis = C;
+  L.n_chunk = n_chunk;
+  L.nbuf = nbuf;
+  L.tab_stride = (int)tab_stride;
+  L.buf_bytes = (uint32_t)buf_bytes;
+  L.off_first = (uint32_t)g.region_al;
+  L.off_S = (uint32_t)(g.region_al + buf_bytes);      // multiple of 128: slot s of S sits in bank s mod 16
+  L.off_bar = (uint32_t)(g.region_al + buf_bytes + g.s_bytes);
+  L.smem = g.region_al + buf_bytes + g.s_bytes + 16 * (size_t)nbuf + 8 + 16;
+  L.tab_off = (uint32_t)(sizeof(float2) * (size_t)(C + zpad));
+  L.f_off = corr ? (uint32_t)(L.tab_off + tab_stride) : 0u;
+
+  const uint32_t s_slot0 = L.off_S / 8;
+  const uint32_t zslot0 = corr ? L.off_first / 8 + (uint32_t)C : s_slot0 + (uint32_t)g.sink0;
   std::vector<unsigned char> h_tab((size_t)n_ch * n_chunk * tab_stride, 0);
   std::vector<uint32_t> h_size((size_t)n_ch * n_chunk, 0);
   for (int ch = 0; ch < n_ch; ++ch)
@@ -122,11 +157,33 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
       const size_t cp = (size_t)ch * n_chunk + c;
       std::vector<unsigned char> &b = tabs[cp].bytes;
       const int bi = c % nbuf;
-      const uint32_t base_slot = (uint32_t)((bi == 0 ? p->fused_off_dedicated : (uint32_t)(bi - 1) * p->fused_buf_bytes) / 8);
-      finalize_chunk_table(b, base_slot, s_slot0, sink0);
+      const uint32_t base_slot = (uint32_t)((bi == 0 ? L.off_first : (uint32_t)(bi - 1) * L.buf_bytes) / 8);
+      finalize_chunk_table(b, base_slot, zslot0);
       std::memcpy(h_tab.data() + cp * tab_stride, b.data(), b.size());
       h_size[cp] = (uint32_t)b.size();
     }
+  int rc;
+  if ((rc = upload_table((void **)&L.d_tab, h_tab.data(), h_tab.size(), st, "fused table")) != BLINK_OK) return rc;
+  if ((rc = upload_table((void **)&L.d_size, h_size.data(), sizeof(uint32_t) * h_size.size(), st, "fused table")) != BLINK_OK) return rc;
+  BLINK_CUDA_TRY(cudaStreamSynchronize(st), "fused table upload sync");
+  L.ok = true;
+  return BLINK_OK;
+}
+
+// Lay out shared memory, build and upload the tables of the route (plain layout; the layout with
+// correction factors is built when blink_plan_apply_corrections first asks for it).
+int fused_build(blink_plan *p, cudaStream_t st) {
+  FusedGeom g;
+  if (!fused_geom(p, g)) return BLINK_OK;
+  const int N = p->n_pix, n_ch = p->n_ch, Ns = g.Ns, D = g.D, LS = g.LS, sink0 = g.sink0;
+  int rc = fused_layout(p, 0, st);
+  if (rc != BLINK_OK) return rc;
+  if (!p->fl[0].ok) return BLINK_OK;
+  p->fused_D = D;
+  p->fused_threads = kFusedThreads;
+  const std::vector<HostGather> &gathers = p->gathers;
+  std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
+  for (int ch = 0; ch < n_ch; ++ch) assign_cells(gathers[ch], owner[ch], slot[ch]);
 
   // phase-H records: every bounding-box cell with kx >= 0, column by column; for D > 1 also the
   // complex weight of every record in every sub-image (a, b): w e^{2 pi i (kx a + ky b) / N}
@@ -196,66 +253,62 @@ int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStrea
       }
   }
 
-  auto upload = [&](void **dst, const void *src, size_t bytes) -> int {
-    cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
-    if (e != cudaSuccess) {
-      set_cuda_error(e, "fused table cudaMalloc");
-      *dst = nullptr;
-      return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
-    }
-    BLINK_CUDA_TRY(cudaMemcpyAsync(*dst, src, bytes, cudaMemcpyHostToDevice, st), "fused table upload");
-    return BLINK_OK;
-  };
-  int rc;
-  if ((rc = upload((void **)&p->d_gtab, h_tab.data(), h_tab.size())) != BLINK_OK) return rc;
-  if ((rc = upload((void **)&p->d_gsize, h_size.data(), sizeof(uint32_t) * h_size.size())) != BLINK_OK) return rc;
-  if ((rc = upload((void **)&p->d_hrec, h_hrec.data(), sizeof(uint2) * h_hrec.size())) != BLINK_OK) return rc;
+  if ((rc = upload_table((void **)&p->d_hrec, h_hrec.data(), sizeof(uint2) * h_hrec.size(), st, "fused table")) != BLINK_OK) return rc;
   if (D > 1) {
-    if ((rc = upload((void **)&p->d_hw, h_hw.data(), sizeof(float2) * h_hw.size())) != BLINK_OK) return rc;
-    if ((rc = upload((void **)&p->d_pha, h_pha.data(), sizeof(float2) * h_pha.size())) != BLINK_OK) return rc;
+    if ((rc = upload_table((void **)&p->d_hw, h_hw.data(), sizeof(float2) * h_hw.size(), st, "fused table")) != BLINK_OK) return rc;
+    if ((rc = upload_table((void **)&p->d_pha, h_pha.data(), sizeof(float2) * h_pha.size(), st, "fused table")) != BLINK_OK) return rc;
     std::vector<float2> h_tws(Ns);                  // exp(+2 pi i m / Ns), the sub-transforms' twiddles
     for (int m = 0; m < Ns; ++m) {
       const double ang = 6.283185307179586476925286766559 * (double)m / (double)Ns;
       h_tws[m] = make_float2((float)std::cos(ang), (float)std::sin(ang));
     }
-    if ((rc = upload((void **)&p->d_tw_sub, h_tws.data(), sizeof(float2) * h_tws.size())) != BLINK_OK) return rc;
+    if ((rc = upload_table((void **)&p->d_tw_sub, h_tws.data(), sizeof(float2) * h_tws.size(), st, "fused table")) != BLINK_OK) return rc;
   }
   BLINK_CUDA_TRY(cudaStreamSynchronize(st), "fused table upload sync");
   p->fused_path = 1;
   return BLINK_OK;
 }
 
-static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st) {
-  FusedParams fp;
-  fp.vis = vis; fp.img = img; fp.chinfo = p->d_chinfo;
-  fp.gtab = p->d_gtab; fp.gsize = p->d_gsize; fp.hrec = p->d_hrec; fp.hw = p->d_hw; fp.pha = p->d_pha;
-  fp.tw = p->fused_D > 1 ? p->d_tw_sub : p->d_tw;
-  fp.n_bl = p->n_bl; fp.n_ch = p->n_ch; fp.n_snap = n_t * p->n_ch; fp.n_can_max = p->n_can_max;
-  fp.n_chunk = p->fused_n_chunk; fp.chunk_vis = p->fused_chunk_vis; fp.nbuf = p->fused_nbuf;
-  fp.tab_stride = p->fused_tab_stride; fp.n_col = p->kx_max_all + 1; fp.h_max = p->h_max;
-  fp.buf_bytes = p->fused_buf_bytes;
-  fp.off_dedicated = p->fused_off_dedicated; fp.off_S = p->fused_off_S; fp.off_bar = p->fused_off_bar;
+template <bool CORR>
+static int launch_fused_c(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
   // band limit of the first transform stage, in units of N/16 cells
   const int n_sub = p->n_pix / p->fused_D;
   const int reach = std::max(p->kx_max_all, p->ky_max_all) + 1, T = n_sub / 16;
   const int nz = (reach + T - 1) / T;
-  if (p->fused_D == 2) return nz <= 3 ? launch_fused_n<256, 3, 2>(p, fp, st) : launch_fused_n<256, 8, 2>(p, fp, st);
-  if (p->fused_D == 4) return nz <= 3 ? launch_fused_n<256, 3, 4>(p, fp, st) : launch_fused_n<256, 8, 4>(p, fp, st);
+  if (p->fused_D == 2) return nz <= 3 ? launch_fused_n<256, 3, 2, CORR>(p, fp, st) : launch_fused_n<256, 8, 2, CORR>(p, fp, st);
+  if (p->fused_D == 4) return nz <= 3 ? launch_fused_n<256, 3, 4, CORR>(p, fp, st) : launch_fused_n<256, 8, 4, CORR>(p, fp, st);
   switch (p->n_pix) {
     case 32:
     case 64:
     case 128: return launch_fused_small(p, fp, st);
     case 256:
-      if (nz <= 2) return launch_fused_n<256, 2>(p, fp, st);
-      if (nz <= 3) return launch_fused_n<256, 3>(p, fp, st);
-      if (nz <= 4) return launch_fused_n<256, 4>(p, fp, st);
-      return launch_fused_n<256, 8>(p, fp, st);
+      if constexpr (!CORR) {       // (with corrections: the two instances that cover every band limit)
+        if (nz <= 2) return launch_fused_n<256, 2, 1, CORR>(p, fp, st);
+        if (nz > 3 && nz <= 4) return launch_fused_n<256, 4, 1, CORR>(p, fp, st);
+      }
+      if (nz <= 3) return launch_fused_n<256, 3, 1, CORR>(p, fp, st);
+      return launch_fused_n<256, 8, 1, CORR>(p, fp, st);
     default: return BLINK_EUNSUPPORTED;
   }
 }
 
+static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st) {
+  const GatherLayout &L = p->fl[p->corr_on ? 1 : 0];
+  FusedParams fp;
+  fp.vis = vis; fp.img = img; fp.chinfo = p->d_chinfo;
+  fp.corr = p->corr_on ? p->d_corr : nullptr;
+  fp.gtab = L.d_tab; fp.gsize = L.d_size; fp.hrec = p->d_hrec; fp.hw = p->d_hw; fp.pha = p->d_pha;
+  fp.tw = p->fused_D > 1 ? p->d_tw_sub : p->d_tw;
+  fp.n_bl = p->n_bl; fp.n_ch = p->n_ch; fp.n_snap = n_t * p->n_ch; fp.n_can_max = p->n_can_max;
+  fp.n_chunk = L.n_chunk; fp.chunk_vis = L.chunk_vis; fp.nbuf = L.nbuf;
+  fp.tab_stride = L.tab_stride; fp.n_col = p->kx_max_all + 1; fp.h_max = p->h_max;
+  fp.buf_bytes = L.buf_bytes; fp.tab_off = L.tab_off; fp.f_off = L.f_off;
+  fp.off_dedicated = L.off_first; fp.off_S = L.off_S; fp.off_bar = L.off_bar; fp.smem = (uint32_t)L.smem;
+  return p->corr_on ? launch_fused_c<true>(p, fp, st) : launch_fused_c<false>(p, fp, st);
+}
+
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st) {
-  if (p->fused_path == 1) return launch_fused(p, vis, n_t, img, st);
+  if (fused_smem_route(p)) return launch_fused(p, vis, n_t, img, st);
   return launch_image_from_vis(p, vis, n_t * p->n_ch, img, st);
 }
 
@@ -295,7 +348,7 @@ extern "C" int blink_host_fused_emulate(const int32_t *cell, int n_bl, int n_pix
     bool ok = true;
     build_chunk_table(g, owner, slot, lo, hi, sink0, t, ok);
     if (!ok) return BLINK_EUNSUPPORTED;
-    finalize_chunk_table(t.bytes, 0u, s_slot0, sink0);
+    finalize_chunk_table(t.bytes, 0u, s_slot0 + (uint32_t)sink0);
     groups += t.groups;
     rows += t.rows;
     std::memcpy(sm.data(), vis + 2 * (size_t)lo, sizeof(float) * 2 * (size_t)(hi - lo));

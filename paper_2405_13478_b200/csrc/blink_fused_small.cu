@@ -13,6 +13,14 @@
 namespace blink {
 
 int launch_fused_small(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
+  if (fp.corr) {
+    switch (p->n_pix) {
+      case 32: return launch_fused_n<32, 8, 1, true>(p, fp, st);
+      case 64: return launch_fused_n<64, 8, 1, true>(p, fp, st);
+      case 128: return launch_fused_n<128, 8, 1, true>(p, fp, st);
+      default: return BLINK_EUNSUPPORTED;
+    }
+  }
   switch (p->n_pix) {
     case 32: return launch_fused_n<32, 8>(p, fp, st);
     case 64: return launch_fused_n<64, 8>(p, fp, st);

@@ -31,6 +31,7 @@ namespace blink {
 
 struct GridParams {
   const float2 *vis;
+  const float2 *corr;          // [n_ch][n_bl] correction factors applied as the visibilities are loaded, or NULL
   float2 *uv;
   const ChannelInfo *chinfo;
   const uint16_t *scat, *roff;
@@ -63,8 +64,9 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
   PassRegs<PF> regs;
   if (blockIdx.x < n_items) {   // prefetch pass 0 of the first item
     const int s = (int)(blockIdx.x / p.parts);
-    pass_load<THREADS, PF>(regs, p.vis + (size_t)s * p.n_bl, p.scat + (size_t)((s + p.ch0) % p.n_ch) * p.n_bl, 0,
-                           min(CAP, p.n_bl), tid);
+    const int ch = (s + p.ch0) % p.n_ch;
+    pass_load<THREADS, PF>(regs, p.vis + (size_t)s * p.n_bl, p.scat + (size_t)ch * p.n_bl, 0, min(CAP, p.n_bl), tid,
+                           p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr);
   }
   for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
     const int s = (int)(item / p.parts), part = (int)(item % p.parts);
@@ -94,11 +96,12 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
       // loads of the next pass (or of the next item's first pass) fly during the sums and phase P
       if (pass + 1 < p.n_pass) {
         const int b0 = (pass + 1) * CAP;
-        pass_load<THREADS, PF>(regs, vis, scat, b0, min(CAP, p.n_bl - b0), tid);
+        pass_load<THREADS, PF>(regs, vis, scat, b0, min(CAP, p.n_bl - b0), tid, p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr);
       } else if (item + gridDim.x < n_items) {
         const int s2 = (int)((item + gridDim.x) / p.parts);
-        pass_load<THREADS, PF>(regs, p.vis + (size_t)s2 * p.n_bl, p.scat + (size_t)((s2 + p.ch0) % p.n_ch) * p.n_bl,
-                               0, min(CAP, p.n_bl), tid);
+        const int ch2 = (s2 + p.ch0) % p.n_ch;
+        pass_load<THREADS, PF>(regs, p.vis + (size_t)s2 * p.n_bl, p.scat + (size_t)ch2 * p.n_bl, 0, min(CAP, p.n_bl), tid,
+                               p.corr ? p.corr + (size_t)ch2 * p.n_bl : nullptr);
       }
       sums_run<THREADS>(sr, cellrec, p.roff + cp * p.roff_stride, p.n_can_max, stage, S, tid);
       if (pass + 1 == p.n_pass && tid == 0) bulk_wait_all();   // the zero fill has landed
@@ -131,20 +134,33 @@ __global__ void __launch_bounds__(THREADS, MINB) k_grid(const GridParams p) {
 // chunk with its gather table; cells are owned by warps, sums need no atomics and no barrier between
 // chunks -- and because nothing else needs the shared memory here, the ring runs ahead across
 // snapshots without ever draining.  Phase P as above: bulk zero fill, then the occupied cells.
+static int ring_upload(void **dst, const void *src, size_t bytes, cudaStream_t st) {
+  cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
+  if (e != cudaSuccess) {
+    set_cuda_error(e, "ring table cudaMalloc");
+    *dst = nullptr;
+    return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
+  }
+  BLINK_CUDA_TRY(cudaMemcpyAsync(*dst, src, bytes, cudaMemcpyHostToDevice, st), "ring table upload");
+  return BLINK_OK;
+}
+
 struct GridRingParams {
   const float2 *vis;
+  const float2 *corr;          // CORR: [n_ch][n_bl] correction factors
   float2 *uv;
   const ChannelInfo *chinfo;
   const unsigned char *rtab;   // [n_ch][n_chunk][tab_stride]
   const uint32_t *rsize;       // [n_ch][n_chunk]
   const int2 *rplace;          // [n_ch][2 n_bl] {cell, slot | flag << 30}
   int n_bl, n_ch, n_snap, n_can_max, n_chunk, chunk_vis, nbuf, tab_stride, n_bands, band_cells, ch0;
-  uint32_t buf_bytes, off_buf, off_S, off_bar;
+  uint32_t buf_bytes, off_buf, off_S, off_bar, tab_off, f_off;
   long long grid_cells;
 };
 
 constexpr int kRingPlacePf = 10;   // placement records fetched per thread ahead of the barrier
 
+template <bool CORR>
 __global__ void __launch_bounds__(kFusedThreads, 1) k_grid_ring(const GridRingParams p) {
   constexpr int THREADS = kFusedThreads;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -154,10 +170,16 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_grid_ring(const GridRingPa
   uint64_t *empty = full + p.nbuf;
   const uint32_t sm_base = smem_u32(smem_raw), S_base = sm_base + p.off_S;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const uint32_t vis_bytes = (uint32_t)p.chunk_vis * sizeof(float2);
+  const uint32_t vis_bytes = p.tab_off;
   const uint32_t band_bytes = (uint32_t)p.band_cells * sizeof(float2);
   const int n_S = ((p.n_can_max + 15) & ~15) + 16;
 
+  if constexpr (CORR) {
+    // the 16 "zero visibility" slots behind chunk buffer 0's visibilities, and their factor partners
+    float2 *z = reinterpret_cast<float2 *>(smem_raw + p.off_buf) + p.chunk_vis;
+    if (tid < 16) z[tid] = make_float2(0.f, 0.f);
+    else if (tid < 32) reinterpret_cast<float2 *>(reinterpret_cast<unsigned char *>(z) + p.f_off)[tid - 16] = make_float2(0.f, 0.f);
+  }
   if (tid == 0) {
     for (int b = 0; b < p.nbuf; ++b) {
       mbar_init(full + b, 1);
@@ -187,9 +209,11 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_grid_ring(const GridRingPa
     const size_t cp = (size_t)((s + p.ch0) % p.n_ch) * p.n_chunk + pc;
     const uint32_t tb = __ldg(p.rsize + cp);
     unsigned char *dst = smem_raw + p.off_buf + (size_t)pb * p.buf_bytes;
-    mbar_expect_tx(full + pb, vb + tb);
+    mbar_expect_tx(full + pb, (CORR ? 2 * vb : vb) + tb);
     bulk_load(dst, p.vis + (size_t)s * p.n_bl + (size_t)pc * p.chunk_vis, vb, full + pb);
     bulk_load(dst + vis_bytes, p.rtab + cp * p.tab_stride, tb, full + pb);
+    if constexpr (CORR)
+      bulk_load(dst + p.f_off, p.corr + (size_t)((s + p.ch0) % p.n_ch) * p.n_bl + (size_t)pc * p.chunk_vis, vb, full + pb);
     ++pq;
     if (++pc == p.n_chunk) { pc = 0; ++pk; }
     if (++pb == p.nbuf) pb = 0;
@@ -219,7 +243,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_grid_ring(const GridRingPa
     for (int c = 0; c < p.n_chunk; ++c, ++q) {
       mbar_wait(full + b, (fphase >> b) & 1u);
       fphase ^= 1u << b;
-      consume_chunk(sm_base + p.off_buf + (uint32_t)b * p.buf_bytes + vis_bytes, warp, lane, sm_base, S_base);
+      consume_chunk<CORR>(sm_base + p.off_buf + (uint32_t)b * p.buf_bytes + vis_bytes, warp, lane, sm_base, S_base, p.f_off);
       __syncwarp();
       if (lane == 0) mbar_arrive(empty + b);
       if (tid == 0 && pq < Q) produce();     // chunk q + nbuf into the buffer just released
@@ -248,26 +272,30 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_grid_ring(const GridRingPa
 }
 
 
-// Shared-memory plan and tables of the ring route.  Layout (bytes):
+// Shared-memory plan and tables of the ring route; corr = 1: every chunk carries its correction factors
+// too (see fused_layout in blink_fused.cu for the buffer format).  Layout (bytes):
 //   [0, band)               zero band (source of the bulk zero fill)
-//   [off_buf, +nbuf * B)    chunk buffers (B = chunk_vis * 8 + tab_stride, 128-aligned)
+//   [off_first, +nbuf * B)  chunk buffers
 //   [off_S, ...)            canonical cell sums + 16 zero slots
 //   [off_bar, ...)          full[nbuf], empty[nbuf] mbarriers
 // n_chunk is a multiple of nbuf, so chunk c of every snapshot lands in buffer c % nbuf and the ring
 // never has to drain between snapshots.
-int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st) {
-  p->ring_path = 0;
-  const int want = p->opt.grid_ring != -1;
+int grid_ring_layout(blink_plan *p, int corr, cudaStream_t st) {
+  GatherLayout &L = p->rl[corr];
+  if (L.ok) return BLINK_OK;
   const int N = p->n_pix, n_bl = p->n_bl, n_ch = p->n_ch;
-  if (!want || N > 512 || (n_bl & 1) || p->max_smem_optin <= 0 || p->n_can_max < 1) return BLINK_OK;
+  if (p->opt.grid_ring == -1 || N > 512 || (n_bl & 1) || p->max_smem_optin <= 0 || p->n_can_max < 1 ||
+      (int)p->gathers.size() != n_ch)
+    return BLINK_OK;
   const int sink0 = (p->n_can_max + 15) & ~15, n_S = sink0 + 16;
   if (n_S > 0x7FFF) return BLINK_OK;
   const size_t band = (sizeof(float2) * (size_t)p->band_cells + 127) / 128 * 128;
   const size_t s_bytes = (sizeof(float2) * (size_t)n_S + 127) / 128 * 128;
   const size_t limit = (size_t)p->max_smem_optin;
   if (band + s_bytes + 1024 > limit) return BLINK_OK;
+  const int zpad = corr ? 16 : 0;
   std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
-  for (int ch = 0; ch < n_ch; ++ch) assign_cells(gathers[ch], owner[ch], slot[ch]);
+  for (int ch = 0; ch < n_ch; ++ch) assign_cells(p->gathers[ch], owner[ch], slot[ch]);
 
   std::vector<AbstractTable> tabs;
   int n_chunk = 0, C = 0, nbuf = 0;
@@ -281,50 +309,70 @@ int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaS
       C = (n_bl + n_chunk - 1) / n_chunk;
       C = (C + 1) & ~1;
       if (C > 0x7FFE || (n_bl + C - 1) / C != n_chunk) continue;
-      if (sizeof(float2) * (size_t)C > room) continue;
+      const size_t data_bytes = sizeof(float2) * (size_t)(C + zpad) * (corr ? 2 : 1);
+      if (data_bytes > room) continue;
       tabs.assign((size_t)n_ch * n_chunk, AbstractTable());
       bool ok = true;
       tab_stride = 0;
       for (int ch = 0; ch < n_ch && ok; ++ch)
         for (int c = 0; c < n_chunk && ok; ++c) {
           AbstractTable &t = tabs[(size_t)ch * n_chunk + c];
-          build_chunk_table(gathers[ch], owner[ch], slot[ch], c * C, std::min(n_bl, (c + 1) * C), sink0, t, ok);
+          build_chunk_table(p->gathers[ch], owner[ch], slot[ch], c * C, std::min(n_bl, (c + 1) * C), sink0, t, ok);
           tab_stride = std::max(tab_stride, t.bytes.size());
         }
       if (!ok) continue;
-      buf_bytes = (sizeof(float2) * (size_t)C + tab_stride + 127) / 128 * 128;
+      buf_bytes = (data_bytes + tab_stride + 127) / 128 * 128;
       if (buf_bytes > room) continue;
       found = true;
       break;
     }
   }
   if (!found) return BLINK_OK;
-  p->ring_chunk_vis = C;
-  p->ring_n_chunk = n_chunk;
-  p->ring_nbuf = nbuf;
-  p->ring_tab_stride = (int)tab_stride;
-  p->ring_buf_bytes = (uint32_t)buf_bytes;
-  p->ring_off_buf = (uint32_t)band;
-  p->ring_off_S = (uint32_t)(band + (size_t)nbuf * buf_bytes);
-  p->ring_off_bar = (uint32_t)(p->ring_off_S + s_bytes);
-  p->ring_smem = p->ring_off_bar + 16 * (size_t)nbuf + 16;
-  if (p->ring_smem > limit || p->ring_smem > 0x7FFFu * 8u) return BLINK_OK;
+  L.chunk_vis = C;
+  L.n_chunk = n_chunk;
+  L.nbuf = nbuf;
+  L.tab_stride = (int)tab_stride;
+  L.buf_bytes = (uint32_t)buf_bytes;
+  L.off_first = (uint32_t)band;
+  L.off_S = (uint32_t)(band + (size_t)nbuf * buf_bytes);
+  L.off_bar = (uint32_t)(L.off_S + s_bytes);
+  L.smem = L.off_bar + 16 * (size_t)nbuf + 16;
+  L.tab_off = (uint32_t)(sizeof(float2) * (size_t)(C + zpad));
+  L.f_off = corr ? (uint32_t)(L.tab_off + tab_stride) : 0u;
+  if (L.smem > limit || L.smem > 0x7FFFu * 8u) return BLINK_OK;
 
-  const uint32_t s_slot0 = p->ring_off_S / 8;
+  const uint32_t s_slot0 = L.off_S / 8;
+  const uint32_t zslot0 = corr ? L.off_first / 8 + (uint32_t)C : s_slot0 + (uint32_t)sink0;
   std::vector<unsigned char> h_tab((size_t)n_ch * n_chunk * tab_stride, 0);
   std::vector<uint32_t> h_size((size_t)n_ch * n_chunk, 0);
   for (int ch = 0; ch < n_ch; ++ch)
     for (int c = 0; c < n_chunk; ++c) {
       const size_t cp = (size_t)ch * n_chunk + c;
       std::vector<unsigned char> &b = tabs[cp].bytes;
-      finalize_chunk_table(b, (uint32_t)((p->ring_off_buf + (size_t)(c % nbuf) * buf_bytes) / 8), s_slot0, sink0);
+      finalize_chunk_table(b, (uint32_t)((L.off_first + (size_t)(c % nbuf) * buf_bytes) / 8), zslot0);
       std::memcpy(h_tab.data() + cp * tab_stride, b.data(), b.size());
       h_size[cp] = (uint32_t)b.size();
     }
+  int rc;
+  if ((rc = ring_upload((void **)&L.d_tab, h_tab.data(), h_tab.size(), st)) != BLINK_OK) return rc;
+  if ((rc = ring_upload((void **)&L.d_size, h_size.data(), sizeof(uint32_t) * h_size.size(), st)) != BLINK_OK) return rc;
+  BLINK_CUDA_TRY(cudaStreamSynchronize(st), "ring table upload sync");
+  L.ok = true;
+  return BLINK_OK;
+}
+
+int grid_ring_build(blink_plan *p, cudaStream_t st) {
+  p->ring_path = 0;
+  int rc = grid_ring_layout(p, 0, st);
+  if (rc != BLINK_OK) return rc;
+  if (!p->rl[0].ok) return BLINK_OK;
+  const int N = p->n_pix, n_bl = p->n_bl, n_ch = p->n_ch;
+  std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
+  for (int ch = 0; ch < n_ch; ++ch) assign_cells(p->gathers[ch], owner[ch], slot[ch]);
   // placement records: every canonical cell and its mirror, ascending cell index (coalesced-ish stores)
   std::vector<int2> h_place((size_t)n_ch * 2 * n_bl, make_int2(-1, 0));
   for (int ch = 0; ch < n_ch; ++ch) {
-    const HostGather &g = gathers[ch];
+    const HostGather &g = p->gathers[ch];
     std::vector<std::pair<int32_t, int32_t>> pl;
     pl.reserve(2 * (size_t)g.n_can);
     for (int j = 0; j < g.n_can; ++j) {
@@ -340,38 +388,29 @@ int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaS
     std::sort(pl.begin(), pl.end());
     for (size_t k = 0; k < pl.size(); ++k) h_place[(size_t)ch * 2 * n_bl + k] = make_int2(pl[k].first, pl[k].second);
   }
-  auto upload = [&](void **dst, const void *src, size_t bytes) -> int {
-    cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
-    if (e != cudaSuccess) {
-      set_cuda_error(e, "ring table cudaMalloc");
-      *dst = nullptr;
-      return e == cudaErrorMemoryAllocation ? BLINK_ENOMEM : BLINK_ECUDA;
-    }
-    BLINK_CUDA_TRY(cudaMemcpyAsync(*dst, src, bytes, cudaMemcpyHostToDevice, st), "ring table upload");
-    return BLINK_OK;
-  };
-  int rc;
-  if ((rc = upload((void **)&p->d_rtab, h_tab.data(), h_tab.size())) != BLINK_OK) return rc;
-  if ((rc = upload((void **)&p->d_rsize, h_size.data(), sizeof(uint32_t) * h_size.size())) != BLINK_OK) return rc;
-  if ((rc = upload((void **)&p->d_rplace, h_place.data(), sizeof(int2) * h_place.size())) != BLINK_OK) return rc;
+  if ((rc = ring_upload((void **)&p->d_rplace, h_place.data(), sizeof(int2) * h_place.size(), st)) != BLINK_OK) return rc;
   BLINK_CUDA_TRY(cudaStreamSynchronize(st), "ring table upload sync");
   p->ring_min_snap = p->opt.grid_ring_min_snap > 0 ? p->opt.grid_ring_min_snap : p->sm_count;
   p->ring_path = 1;
   return BLINK_OK;
 }
 
+template <bool CORR>
 static int launch_grid_ring(const blink_plan *p, const float2 *vis, int n_snap, int ch0, float2 *uv, cudaStream_t st) {
+  const GatherLayout &L = p->rl[CORR ? 1 : 0];
   GridRingParams g;
-  g.vis = vis; g.uv = uv; g.chinfo = p->d_chinfo; g.rtab = p->d_rtab; g.rsize = p->d_rsize; g.rplace = p->d_rplace;
-  g.n_bl = p->n_bl; g.n_ch = p->n_ch; g.n_snap = n_snap; g.n_can_max = p->n_can_max; g.n_chunk = p->ring_n_chunk;
-  g.chunk_vis = p->ring_chunk_vis; g.nbuf = p->ring_nbuf; g.tab_stride = p->ring_tab_stride; g.n_bands = p->n_bands;
-  g.band_cells = p->band_cells; g.ch0 = ch0; g.buf_bytes = p->ring_buf_bytes; g.off_buf = p->ring_off_buf;
-  g.off_S = p->ring_off_S; g.off_bar = p->ring_off_bar; g.grid_cells = (long long)p->n_pix * p->n_pix;
+  g.vis = vis; g.corr = CORR ? p->d_corr : nullptr; g.uv = uv; g.chinfo = p->d_chinfo;
+  g.rtab = L.d_tab; g.rsize = L.d_size; g.rplace = p->d_rplace;
+  g.n_bl = p->n_bl; g.n_ch = p->n_ch; g.n_snap = n_snap; g.n_can_max = p->n_can_max; g.n_chunk = L.n_chunk;
+  g.chunk_vis = L.chunk_vis; g.nbuf = L.nbuf; g.tab_stride = L.tab_stride; g.n_bands = p->n_bands;
+  g.band_cells = p->band_cells; g.ch0 = ch0; g.buf_bytes = L.buf_bytes; g.off_buf = L.off_first;
+  g.off_S = L.off_S; g.off_bar = L.off_bar; g.tab_off = L.tab_off; g.f_off = L.f_off;
+  g.grid_cells = (long long)p->n_pix * p->n_pix;
   static std::atomic<uint64_t> attr{0};
-  const int rc = ensure_max_smem(k_grid_ring, p, attr, "k_grid_ring smem attribute");
+  const int rc = ensure_max_smem(k_grid_ring<CORR>, p, attr, "k_grid_ring smem attribute");
   if (rc != BLINK_OK) return rc;
   const int blocks = std::min(n_snap, p->sm_count);
-  k_grid_ring<<<blocks, kFusedThreads, p->ring_smem, st>>>(g);
+  k_grid_ring<CORR><<<blocks, kFusedThreads, L.smem, st>>>(g);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_grid_ring launch");
   return BLINK_OK;
 }
@@ -404,10 +443,10 @@ int launch_grid(const blink_plan *p, const float2 *vis, int n_snap, int ch0, flo
   // many snapshots of a small grid: the ring route; few snapshots (or large grids): the band route,
   // which can split one snapshot over several CTAs
   // (the ring route reads the visibilities with bulk copies: 16-byte aligned base)
-  if (p->ring_path == 1 && n_snap >= p->ring_min_snap && ((uintptr_t)vis & 15) == 0)
-    return launch_grid_ring(p, vis, n_snap, ch0, uv, st);
+  if (p->ring_path == 1 && n_snap >= p->ring_min_snap && ((uintptr_t)vis & 15) == 0 && p->rl[p->corr_on ? 1 : 0].ok)
+    return p->corr_on ? launch_grid_ring<true>(p, vis, n_snap, ch0, uv, st) : launch_grid_ring<false>(p, vis, n_snap, ch0, uv, st);
   GridParams g;
-  g.vis = vis; g.uv = uv; g.chinfo = p->d_chinfo;
+  g.vis = vis; g.corr = p->corr_on ? p->d_corr : nullptr; g.uv = uv; g.chinfo = p->d_chinfo;
   g.scat = p->d_scat; g.roff = p->d_roff; g.cellrec = p->d_cellrec; g.nact = p->d_nact; g.pcell = p->d_pcell; g.pcode = p->d_pcode; g.pband = p->d_pband;
   g.n_bl = p->n_bl; g.n_ch = p->n_ch; g.n_snap = n_snap; g.ch0 = ch0;
   g.n_bands = p->n_bands; g.band_cells = p->band_cells; g.n_can_max = p->n_can_max;

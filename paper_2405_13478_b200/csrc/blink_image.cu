@@ -154,6 +154,7 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_cols_from_vis(const ImgParams
       if (lane < n_c) {                            // lane l forms the l-th cell of the column
         const int e = c0 + lane;
         const float2 *__restrict__ vis = p.vis + (size_t)s * p.n_bl;
+        const float2 *__restrict__ cf = p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr;
         const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
         const int st = __ldg(p.vseg + tb + e), lf = __ldg(p.vlen + tb + e);
         const float w = __ldg(p.vw + tb + e);
@@ -162,7 +163,7 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_cols_from_vis(const ImgParams
         float ar = 0.f, ai = 0.f;
         for (int q = st; q < st + len; ++q) {
           const int code = __ldg(src + q);
-          const float2 v = __ldg(vis + (code >> 1));
+          const float2 v = ld_vis(vis, cf, code >> 1);
           ar += v.x;
           ai += (code & 1) ? -v.y : v.y;
         }
@@ -202,6 +203,7 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_cols_from_vis(const ImgParams
   {
     const size_t tb = (size_t)ch * 2 * p.n_bl;
     const float2 *__restrict__ vis = p.vis + (size_t)s * p.n_bl;
+    const float2 *__restrict__ cf = p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr;
     const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
     for (int e = e0 + tid; e < e1; e += THREADS) {
       const int key = __ldg(p.vkey + tb + e), st = __ldg(p.vseg + tb + e), lf = __ldg(p.vlen + tb + e);
@@ -210,7 +212,7 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_cols_from_vis(const ImgParams
       float ar = 0.f, ai = 0.f;
       for (int q = st; q < st + len; ++q) {
         const int code = __ldg(src + q);
-        const float2 v = __ldg(vis + (code >> 1));
+        const float2 v = ld_vis(vis, cf, code >> 1);
         ar += v.x;
         ai += (code & 1) ? -v.y : v.y;
       }
@@ -336,7 +338,7 @@ int image_setup(blink_plan *p) {
 // the two-kernel routes hold U of one chunk of snapshots; the warp route a ring of U slots plus two
 // completion counters per snapshot.
 size_t scratch_need(const blink_plan *p, long long n_t, bool fused) {
-  if (fused && p->fused_path == 1) return 0;
+  if (fused && fused_smem_route(p)) return 0;
   const long long n_snap = std::max<long long>(n_t * p->n_ch, 1);
   if (p->warp_route) return warp_route_scratch_bytes(p, n_snap);
   const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
@@ -370,7 +372,7 @@ int image_reserve(blink_plan *p, int n_t) {
 
 static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2 *vis, int n_snap, int ch0, float *img, cudaStream_t st) {
   ImgParams ip;
-  ip.vis = vis; ip.src = p->d_src; ip.vkey = p->d_vkey; ip.vseg = p->d_vseg; ip.vlen = p->d_vlen;
+  ip.vis = vis; ip.corr = (vis != nullptr && p->corr_on) ? p->d_corr : nullptr; ip.src = p->d_src; ip.vkey = p->d_vkey; ip.vseg = p->d_vseg; ip.vlen = p->d_vlen;
   ip.vcol = p->d_vcol; ip.vw = p->d_vw; ip.tw32 = p->d_tw32;
   ip.cell_cap = (std::max(p->vtile8_max, 1) + 3) / 4 * 4;
   ip.uv = uv; ip.img = img; ip.U = p->d_scratch; ip.chinfo = p->d_chinfo;

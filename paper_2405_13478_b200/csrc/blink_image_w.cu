@@ -164,6 +164,7 @@ __global__ void __launch_bounds__(kWThreads, 2) k_img1024(const WParams q) {
             asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nv), "r"((uint32_t)(p.n_bl * sizeof(float2))) : "memory");
           }
           const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
+          const float2 *__restrict__ cf = p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr;
           if (q.uvsrc != nullptr) {
             // blink_image: the occupied cells of the item's 8 columns straight from the uv grid (the
             // half-plane kx >= 0 only; empty cells are zero by contract and never read)
@@ -183,9 +184,9 @@ __global__ void __launch_bounds__(kWThreads, 2) k_img1024(const WParams q) {
             const uint4 r = recs[e - e0];
             const int flag = (r.x >> 16) & 3, len = (int)(r.x >> 18);
             const float w = __uint_as_float(r.y);
-            const float2 v0 = __ldg(vis + (r.z >> 1));
+            const float2 v0 = ld_vis(vis, cf, r.z >> 1);
             float2 v1 = make_float2(0.f, 0.f);
-            if (len == 2) v1 = __ldg(vis + (r.w >> 1));
+            if (len == 2) v1 = ld_vis(vis, cf, r.w >> 1);
             float ar = v0.x, ai = (r.z & 1) ? -v0.y : v0.y;
             if (len == 2) {
               ar += v1.x;
@@ -193,7 +194,7 @@ __global__ void __launch_bounds__(kWThreads, 2) k_img1024(const WParams q) {
             } else if (len > 2) {
               for (int qq = (int)r.w + 1; qq < (int)r.w + len; ++qq) {
                 const int code = __ldg(src + qq);
-                const float2 v = __ldg(vis + (code >> 1));
+                const float2 v = ld_vis(vis, cf, code >> 1);
                 ar += v.x;
                 ai += (code & 1) ? -v.y : v.y;
               }

@@ -49,6 +49,19 @@ struct HostGather {    // cell-sorted tables of one channel (see blink_host_buil
   std::vector<int32_t> can_cell, seg_start, src;
 };
 
+// Shared-memory plan and device tables of one set of phase-S gather tables (sgather.cuh): chunks of
+// chunk_vis baselines stream through a ring of nbuf buffers, each chunk with its gather table
+// (tab_off bytes behind the visibilities) and -- when the pre-gridding corrections are fused in --
+// its correction factors (f_off bytes behind the visibilities; 0 = none).
+struct GatherLayout {
+  int chunk_vis = 0, n_chunk = 0, nbuf = 0, tab_stride = 0;
+  uint32_t buf_bytes = 0, off_first = 0, off_S = 0, off_bar = 0, tab_off = 0, f_off = 0;
+  size_t smem = 0;
+  unsigned char *d_tab = nullptr;   // [n_ch][n_chunk][tab_stride]
+  uint32_t *d_size = nullptr;       // [n_ch][n_chunk] bytes of each table (multiple of 16)
+  bool ok = false;
+};
+
 // blink_grid_image_host (blink_host.cu): three streams over a ring of device staging buffers
 struct HostPipe {
   static constexpr int kDepth = 3;
@@ -73,6 +86,8 @@ struct blink_plan {
   // inputs kept for blink_plan_set_corrections
   std::vector<double> h_ant, h_freq;
   float2 *d_corr = nullptr;         // [n_ch][n_bl] correction factors F (blink_correct.cu), NULL until set
+  int corr_on = 0;                  // 1 = blink_grid / blink_grid_image multiply by F as they load (blink_plan_apply_corrections)
+  std::vector<blink::HostGather> gathers;   // per-channel cell-sorted tables, kept for lazily built layouts
 
   // per-channel facts (host)
   std::vector<int64_t> n_dropped, wsum, n_occ;
@@ -137,21 +152,13 @@ struct blink_plan {
   // blink_grid, ring route (see grid_ring_build in blink_grid.cu): phase S as in k_fused
   int ring_path = 0;                // 1 = k_grid_ring available
   int ring_min_snap = 0;            // fewer snapshots per call take the band route
-  int ring_chunk_vis = 0, ring_n_chunk = 0, ring_nbuf = 0, ring_tab_stride = 0;
-  uint32_t ring_buf_bytes = 0, ring_off_buf = 0, ring_off_S = 0, ring_off_bar = 0;
-  size_t ring_smem = 0;
-  unsigned char *d_rtab = nullptr;  // [n_ch][n_chunk][tab_stride]
-  uint32_t *d_rsize = nullptr;      // [n_ch][n_chunk]
+  blink::GatherLayout rl[2];        // [0] plain, [1] with correction factors (built by blink_plan_apply_corrections)
   int2 *d_rplace = nullptr;         // [n_ch][2 n_bl] {cell, slot of S | flag << 30}, ascending cell
 
   // shared-memory route (see fused_build in blink_fused.cu)
   int h_max = 0;                    // phase-H records per channel (padded with pos = 0xFFFF)
   int fused_threads = 512;
-  size_t fused_smem = 0;
-  int fused_chunk_vis = 0, fused_n_chunk = 0, fused_nbuf = 0, fused_tab_stride = 0;
-  uint32_t fused_buf_bytes = 0, fused_off_dedicated = 0, fused_off_S = 0, fused_off_bar = 0;
-  unsigned char *d_gtab = nullptr;  // [n_ch][n_chunk][tab_stride] phase-S gather tables
-  uint32_t *d_gsize = nullptr;      // [n_ch][n_chunk] bytes of each table
+  blink::GatherLayout fl[2];        // [0] plain, [1] with correction factors; off_first = the dedicated buffer 0
   uint2 *d_hrec = nullptr;          // [n_ch][h_max] {line position | j << 16 | flag << 30, weight}
   int fused_D = 1;                  // polyphase route: the image is fused_D x fused_D interleaved sub-images of n_pix / fused_D
   float2 *d_hw = nullptr;           // [n_ch][fused_D][h_max] complex phase-H weights of the sub-image rows
@@ -176,7 +183,20 @@ struct ImgParams {
   const float *vw;
   const float2 *tw, *tw32;
   int n_ch, n_bl, wu, uniform, snap_base, ch0, direct_max, cell_cap;
+  const float2 *corr;   // [n_ch][n_bl] correction factors applied to the visibilities as they are loaded, or NULL
 };
+
+#if defined(__CUDACC__)
+// one visibility, corrected at load when a factor table is given (f2 fused: V * F, blink_correct.cu)
+__device__ __forceinline__ float2 ld_vis(const float2 *__restrict__ vis, const float2 *__restrict__ cf, int i) {
+  float2 v = __ldg(vis + i);
+  if (cf != nullptr) {
+    const float2 f = __ldg(cf + i);
+    v = make_float2(v.x * f.x - v.y * f.y, v.x * f.y + v.y * f.x);
+  }
+  return v;
+}
+#endif
 
 // warp-per-transform persistent kernel at N = 1024 (blink_image_w.cu)
 int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st);
@@ -202,9 +222,13 @@ int image_setup(blink_plan *p);
 int image_reserve(blink_plan *p, int n_t);
 // device scratch a call of n_t time steps needs: blink_image (fused = false) or blink_grid_image
 size_t scratch_need(const blink_plan *p, long long n_t, bool fused);
-int grid_ring_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st);
+int grid_ring_build(blink_plan *p, cudaStream_t st);
+int grid_ring_layout(blink_plan *p, int corr, cudaStream_t st);
 int fused_setup(blink_plan *p);
-int fused_build(blink_plan *p, const std::vector<HostGather> &gathers, cudaStream_t st);
+int fused_build(blink_plan *p, cudaStream_t st);
+int fused_layout(blink_plan *p, int corr, cudaStream_t st);
+// true when blink_grid_image takes the shared-memory kernel in the plan's current state
+inline bool fused_smem_route(const blink_plan *p) { return p->fused_path == 1 && p->fl[p->corr_on ? 1 : 0].ok; }
 int fused_line_stride(int n_pix);
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);
 int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, float *img, cudaStream_t st);

@@ -201,8 +201,10 @@ static void plan_free(blink_plan *p) {
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
   cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol); cudaFree(p->d_vrec); cudaFree(p->d_corr); cudaFree(p->d_tw32);
-  cudaFree(p->d_gtab); cudaFree(p->d_gsize); cudaFree(p->d_hrec); cudaFree(p->d_hw); cudaFree(p->d_pha); cudaFree(p->d_tw_sub);
-  cudaFree(p->d_rtab); cudaFree(p->d_rsize); cudaFree(p->d_rplace);
+  cudaFree(p->d_hrec); cudaFree(p->d_hw); cudaFree(p->d_pha); cudaFree(p->d_tw_sub); cudaFree(p->d_rplace);
+  for (int c = 0; c < 2; ++c) {
+    cudaFree(p->fl[c].d_tab); cudaFree(p->fl[c].d_size); cudaFree(p->rl[c].d_tab); cudaFree(p->rl[c].d_size);
+  }
   delete p;
 }
 
@@ -347,7 +349,8 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
   std::vector<int32_t> h_src((size_t)n_ch * n_bl, 0), h_seg((size_t)n_ch * (n_bl + 1), 0);
   std::vector<int32_t> h_pcell((size_t)n_ch * 2 * n_bl, 0), h_pcode((size_t)n_ch * 2 * n_bl, 0);
   std::vector<int32_t> h_pband((size_t)n_ch * (p->n_bands + 1), 0);
-  std::vector<HostGather> gathers(n_ch);
+  std::vector<HostGather> &gathers = p->gathers;
+  gathers.assign(n_ch, HostGather());
   for (int ch = 0; ch < n_ch; ++ch) {
     HostGather &g = gathers[ch];
     PLAN_TRY(build_gather_host(h_cell.data() + (size_t)ch * n_bl, n_bl, N, g));
@@ -535,8 +538,8 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
     PLAN_CUDA(ce, "vis-route table upload");
     p->warp_route = (p->opt.warp_route != -1 && warp_route_applies(p)) ? 1 : 0;
   }
-  PLAN_TRY(fused_build(p, gathers, st));
-  PLAN_TRY(grid_ring_build(p, gathers, st));
+  PLAN_TRY(fused_build(p, st));
+  PLAN_TRY(grid_ring_build(p, st));
   if (weighting == BLINK_UNIFORM) {
     // canonical cells are exactly the occupied half-plane cells with ky > 0 or (ky == 0, kx >= 0);
     // pass A of blink_image works on columns kx >= 0 and all ky, so list every occupied cell with
@@ -641,9 +644,10 @@ extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *
     case BLINK_Q_IMAGE_PATH: *(int32_t *)out = p->image_path; break;
     case BLINK_Q_SCRATCH_BYTES: *(int64_t *)out = (int64_t)p->scratch_bytes; break;
     case BLINK_Q_IMAGE_CHUNK: *(int32_t *)out = p->chunk_snapshots; break;
-    case BLINK_Q_FUSED_PATH: *(int32_t *)out = p->fused_path == 1 ? 1 : (p->warp_route ? 2 : 0); break;
+    case BLINK_Q_FUSED_PATH: *(int32_t *)out = fused_smem_route(p) ? 1 : (p->warp_route ? 2 : 0); break;
     case BLINK_Q_FUSED_CHUNK: *(int32_t *)out = p->fused_chunk; break;
     case BLINK_Q_CORR: *(const void **)out = p->d_corr; break;
+    case BLINK_Q_CORR_FUSED: *(int32_t *)out = p->corr_on; break;
     default: return BLINK_EINVAL;
   }
   return BLINK_OK;

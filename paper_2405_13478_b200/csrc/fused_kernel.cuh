@@ -38,6 +38,7 @@ constexpr int kHPer = 7;              // phase-H records fetched per thread ahea
 
 struct FusedParams {
   const float2 *vis;
+  const float2 *corr;         // CORR: [n_ch][n_bl] correction factors, copied chunk by chunk beside the visibilities
   float *img;
   const ChannelInfo *chinfo;
   const unsigned char *gtab;  // [n_ch][n_chunk][tab_stride] phase-S gather tables (see fused_build)
@@ -48,6 +49,7 @@ struct FusedParams {
   const float2 *tw;
   int n_bl, n_ch, n_snap, n_can_max, n_chunk, chunk_vis, nbuf, tab_stride, n_col, h_max;
   uint32_t buf_bytes, off_dedicated, off_S, off_bar;   // byte offsets into dynamic shared memory
+  uint32_t tab_off, f_off, smem;                       // table / factors behind a buffer's visibilities; launch smem bytes
 };
 
 
@@ -65,7 +67,7 @@ struct FusedParams {
 // values.  Phase S runs once per snapshot, phases H and A once per b, pass B once per (b, a) with the
 // D transform groups of a row pair side by side in a warp; no transform longer than N is ever taken and no zero outside the bounding box is
 // ever touched.
-template <int N, int THREADS, int NZ, int D>
+template <int N, int THREADS, int NZ, int D, bool CORR>
 __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   constexpr int T = N / 16;             // lanes per transform
   constexpr int G = THREADS / T;        // transforms in flight per CTA
@@ -87,7 +89,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   const int tid = threadIdx.x;
   const int warp = tid >> 5, lane = tid & 31;
   const int grp = tid / T, t = tid % T;
-  const uint32_t vis_bytes = (uint32_t)p.chunk_vis * sizeof(float2);
+  const uint32_t vis_bytes = p.tab_off;
   // chunk c of every snapshot lives in buffer c % nbuf; buffer 0 is the dedicated one, the others
   // alias the lines / exchange area
   auto buf_of = [&](int b) -> unsigned char * {
@@ -104,9 +106,11 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
     const size_t cp = (size_t)(s % p.n_ch) * p.n_chunk + c;
     const uint32_t tb = __ldg(p.gsize + cp);
     unsigned char *dst = buf_of(b);
-    mbar_expect_tx(full + b, vb + tb);
+    mbar_expect_tx(full + b, (CORR ? 2 * vb : vb) + tb);
     bulk_load(dst, p.vis + (size_t)s * p.n_bl + (size_t)c * p.chunk_vis, vb, full + b);
     bulk_load(dst + vis_bytes, p.gtab + cp * p.tab_stride, tb, full + b);
+    if constexpr (CORR)
+      bulk_load(dst + p.f_off, p.corr + (size_t)(s % p.n_ch) * p.n_bl + (size_t)c * p.chunk_vis, vb, full + b);
   };
 
   if (tid == 0) {
@@ -121,6 +125,12 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   // padded lanes and the "zero visibility" padded entries point at)
   const int n_S = ((p.n_can_max + 15) & ~15) + 16;
   for (int j = tid; j < n_S; j += THREADS) S[j] = make_float2(0.f, 0.f);
+  if constexpr (CORR) {
+    // the 16 "zero visibility" slots behind chunk buffer 0's visibilities, and their factor partners
+    float2 *z = reinterpret_cast<float2 *>(smem_raw + p.off_dedicated) + p.chunk_vis;
+    if (tid < 16) z[tid] = make_float2(0.f, 0.f);
+    else if (tid < 32) reinterpret_cast<float2 *>(reinterpret_cast<unsigned char *>(z) + p.f_off)[tid - 16] = make_float2(0.f, 0.f);
+  }
   const float2 *pha_s = S + n_S;        // D > 1: [D][N/2] column phases of the sub-images, right after the sums
   if constexpr (D > 1)
     for (int j = tid; j < D * (N / 2); j += THREADS) S[n_S + j] = __ldg(p.pha + j);
@@ -160,7 +170,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
     for (int c = 0, b = 0; c < p.n_chunk; ++c) {
       mbar_wait(full + b, (fphase >> b) & 1u);
       fphase ^= 1u << b;
-      consume_chunk(smem_u32(buf_of(b)) + vis_bytes, warp, lane, sm_base, S_base);
+      consume_chunk<CORR>(smem_u32(buf_of(b)) + vis_bytes, warp, lane, sm_base, S_base, p.f_off);
       __syncwarp();
       if (lane == 0) mbar_arrive(empty + b);    // this warp is done with the buffer
       if (tid == 0) {
@@ -299,15 +309,15 @@ __global__ void __launch_bounds__(THREADS, 1) k_fused(const FusedParams p) {
   }
 }
 
-template <int N, int NZ, int D = 1>
+template <int N, int NZ, int D = 1, bool CORR = false>
 static int launch_fused_n(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
   constexpr int THREADS = kFusedThreads;
   static std::atomic<uint64_t> attr{0};
-  const int rc = ensure_max_smem(k_fused<N, THREADS, NZ, D>, p, attr, "k_fused smem attribute");
+  const int rc = ensure_max_smem(k_fused<N, THREADS, NZ, D, CORR>, p, attr, "k_fused smem attribute");
   if (rc != BLINK_OK) return rc;
   const int blocks = std::min(fp.n_snap, p->sm_count);
   if (blocks <= 0) return BLINK_OK;
-  k_fused<N, THREADS, NZ, D><<<blocks, THREADS, p->fused_smem, st>>>(fp);
+  k_fused<N, THREADS, NZ, D, CORR><<<blocks, THREADS, fp.smem, st>>>(fp);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_fused launch");
   return BLINK_OK;
 }

@@ -67,13 +67,25 @@ __device__ __forceinline__ void load_idx(GroupIdx &gi, uint32_t blk) {
   for (int r = 0; r < kFusedLcap; ++r) asm volatile("ld.shared.s16 %0, [%1];" : "=r"(gi.e[r]) : "r"(blk + 64u * (r + 1)));
 }
 
-// lane l adds its L visibilities and folds the sum into its cell
-template <int L> __device__ __forceinline__ void fold_group(const GroupIdx &gi, uint32_t sm_base, uint32_t S_base) {
+// lane l adds its L visibilities and folds the sum into its cell.  CORR: every visibility is first
+// multiplied by its pre-gridding correction factor F (blink_correct.cu), which
+// arrived in the same buffer f_off bytes behind it -- the corrections "fused at load" of SURVEY 8(f) f2.
+template <int L, bool CORR>
+__device__ __forceinline__ void fold_group(const GroupIdx &gi, uint32_t sm_base, uint32_t S_base, uint32_t f_base) {
   float2 v[L], a;
 #pragma unroll
   for (int r = 0; r < L; ++r) {
-    asm volatile("{\n.reg .b32 t;\nand.b32 t, %2, 0x7FFF;\nmad.lo.u32 t, t, 8, %3;\nld.shared.v2.f32 {%0, %1}, [t];\n}"
-                 : "=f"(v[r].x), "=f"(v[r].y) : "r"(gi.e[r]), "r"(sm_base));
+    if constexpr (CORR) {
+      float2 x, f;
+      asm volatile("{\n.reg .b32 t, u;\nand.b32 t, %4, 0x7FFF;\nmad.lo.u32 u, t, 8, %6;\nmad.lo.u32 t, t, 8, %5;\n"
+                   "ld.shared.v2.f32 {%0, %1}, [t];\nld.shared.v2.f32 {%2, %3}, [u];\n}"
+                   : "=f"(x.x), "=f"(x.y), "=f"(f.x), "=f"(f.y) : "r"(gi.e[r]), "r"(sm_base), "r"(f_base));
+      v[r].x = x.x * f.x - x.y * f.y;
+      v[r].y = x.x * f.y + x.y * f.x;
+    } else {
+      asm volatile("{\n.reg .b32 t;\nand.b32 t, %2, 0x7FFF;\nmad.lo.u32 t, t, 8, %3;\nld.shared.v2.f32 {%0, %1}, [t];\n}"
+                   : "=f"(v[r].x), "=f"(v[r].y) : "r"(gi.e[r]), "r"(sm_base));
+    }
   }
   uint32_t sa;
   asm volatile("mad.lo.u32 %2, %3, 8, %4;\nld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(a.x), "=f"(a.y), "=r"(sa) : "r"(gi.j), "r"(S_base));
@@ -106,7 +118,10 @@ template <int L> __device__ __forceinline__ void fold_group(const GroupIdx &gi, 
 // One warp's share of a chunk: `tab` is the shared address of the chunk's gather table (it follows
 // the visibilities in the same buffer).  wd.x = offset of the warp's stream | number of groups
 // << 24, wd.y = L - 1 of each group, two bits apiece.
-__device__ __forceinline__ void consume_chunk(uint32_t tab, int warp, int lane, uint32_t sm_base, uint32_t S_base) {
+template <bool CORR = false>
+__device__ __forceinline__ void consume_chunk(uint32_t tab, int warp, int lane, uint32_t sm_base, uint32_t S_base,
+                                              uint32_t f_off = 0) {
+  const uint32_t f_base = sm_base + f_off;   // a visibility in slot s has its factor at f_base + 8 s
   const uint2 wd = lds_u2(tab + 8u * warp);
   uint32_t blk = tab + (wd.x & 0xFFFFFFu) + 2u * lane;
   uint32_t lseq = wd.y;
@@ -118,10 +133,10 @@ __device__ __forceinline__ void consume_chunk(uint32_t tab, int warp, int lane, 
     lseq >>= 2;
     blk += (L + 1) * 64;
     load_idx(nxt, blk);                    // past the last group: reads the bytes that follow, unused
-    if (L == 4) fold_group<4>(cur, sm_base, S_base);
-    else if (L == 3) fold_group<3>(cur, sm_base, S_base);
-    else if (L == 2) fold_group<2>(cur, sm_base, S_base);
-    else fold_group<1>(cur, sm_base, S_base);
+    if (L == 4) fold_group<4, CORR>(cur, sm_base, S_base, f_base);
+    else if (L == 3) fold_group<3, CORR>(cur, sm_base, S_base, f_base);
+    else if (L == 2) fold_group<2, CORR>(cur, sm_base, S_base, f_base);
+    else fold_group<1, CORR>(cur, sm_base, S_base, f_base);
   };
   while (n > 0) {
     step(ga, gb);
@@ -318,8 +333,10 @@ static void assign_cells(const HostGather &g, std::vector<int> &owner, std::vect
 
 // relative entries -> shared-memory slots of the buffer the chunk will land in (base_slot, in
 // 8-byte units); a padded entry reads the zero slot of a bank that the real entries of its
-// half-row leave free (zero slots: S[sink0 + b], S starting at slot s_slot0)
-static void finalize_chunk_table(std::vector<unsigned char> &b, uint32_t base_slot, uint32_t s_slot0, int sink0) {
+// half-row leave free
+// (zslot0: first of 16 consecutive always-zero slots a padded visibility entry may point at -- the sinks in
+// S, or, when correction factors ride along, 16 slots whose partners f_off behind them are finite too)
+static void finalize_chunk_table(std::vector<unsigned char> &b, uint32_t base_slot, uint32_t zslot0) {
   for (int w = 0; w < kFusedWarps; ++w) {
     uint32_t off, lseq;
     std::memcpy(&off, b.data() + 8 * w, 4);
@@ -343,7 +360,7 @@ static void finalize_chunk_table(std::vector<unsigned char> &b, uint32_t base_sl
           int free_bank = 0;
           while (free_bank < 15 && (used >> free_bank & 1u)) ++free_bank;
           for (int l = 0; l < 16; ++l)
-            if (e[l] == 0xFFFFu) e[l] = (uint16_t)(s_slot0 + sink0 + ((free_bank - (int)s_slot0) & 15));
+            if (e[l] == 0xFFFFu) e[l] = (uint16_t)(zslot0 + ((free_bank - (int)zslot0) & 15));
         }
       blk += (size_t)(L + 1) * 64;
     }

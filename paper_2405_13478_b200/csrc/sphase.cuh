@@ -31,7 +31,8 @@ template <int PF> struct PassRegs {
 
 template <int THREADS, int PF>
 __device__ __forceinline__ void pass_load(PassRegs<PF> &r, const float2 *__restrict__ vis,
-                                          const uint16_t *__restrict__ scat, int b0, int cnt, int tid) {
+                                          const uint16_t *__restrict__ scat, int b0, int cnt, int tid,
+                                          const float2 *__restrict__ corr = nullptr) {
 #pragma unroll
   for (int q = 0; q < PF; ++q) {
     const int i = q * THREADS + tid;
@@ -39,6 +40,16 @@ __device__ __forceinline__ void pass_load(PassRegs<PF> &r, const float2 *__restr
     if (i < cnt) {
       r.sc[q] = scat[b0 + i];
       r.v[q] = __ldcs(vis + b0 + i);               // streamed once: evict-first
+    }
+  }
+  if (corr != nullptr) {   // pre-gridding corrections fused at load: V * F[ch][bl] (blink_correct.cu), F from L2
+#pragma unroll
+    for (int q = 0; q < PF; ++q) {
+      const int i = q * THREADS + tid;
+      if (i < cnt) {
+        const float2 f = __ldg(corr + b0 + i), v = r.v[q];
+        r.v[q] = make_float2(v.x * f.x - v.y * f.y, v.x * f.y + v.y * f.x);
+      }
     }
   }
 }

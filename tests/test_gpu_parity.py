@@ -617,6 +617,61 @@ def test_corrections_match_oracle(torch_cuda, blink, name, n_t):
     plan.close()
 
 
+@pytest.mark.parametrize("name,options", [
+    ("tiny", {}), ("station", {}), ("station128", {}), ("station512", {}), ("mwa1", {}),
+    ("station", dict(grid_ring_min_snap=1)),          # blink_grid on the ring route (k_grid_ring<CORR>)
+    ("station128", dict(fused_route=-1)),             # blink_grid_image on the two-kernel route (k_cols_from_vis)
+    ("station_uniform_32", {}), ("mwa1_natural_64", {})])
+def test_corrections_fused_at_load(torch_cuda, blink, oracle, name, options):
+    """SURVEY 8(f) f2, fused: with blink_plan_apply_corrections(1), blink_grid and blink_grid_image grid
+    V * F without a separate pass.  Against the oracle chain corrections -> gridding -> imaging
+    (oracle/corrections.py applied in fp64, then the imaging oracle) at the usual grid and image bars,
+    on every route that loads visibilities; switching it off again restores the plain result bit for bit."""
+    torch = torch_cuda
+    from oracle import corrections as oc
+    w = _workload(name)
+    ant, gains, cables = _corr_inputs(w, 17)
+    l0, m0 = (0.2, -0.1) if w.pixscale > 1e-3 else (0.002, -0.001)
+    vis_h = w.vis()
+    vis = torch.from_numpy(vis_h).cuda()
+    plan = blink.Plan(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=options or None)
+    plain_uv = plan.grid(vis).clone()
+    plain_img = plan.grid_image(vis).clone()
+    with pytest.raises(blink.BlinkError):
+        plan.apply_corrections(True)                  # no table yet
+    plan.set_corrections(gains, cables, l0, m0)
+    path0 = plan.query_i32(blink.Q_FUSED_PATH)
+    plan.apply_corrections(True)
+    assert plan.query_i32(blink.Q_CORR_FUSED) == 1
+    F_ref = oc.correction_factors(ant, w.freq_hz, gains, cables, l0, m0)
+    vis_c = oc.apply_corrections(vis_h, F_ref).astype(np.complex64)
+    n_snap = w.n_t * w.n_ch
+    uv = torch.full((w.n_t, w.n_ch, w.n_pix, w.n_pix), float("nan"), dtype=torch.complex64, device="cuda")
+    plan.grid(vis, uv)
+    img = torch.full(uv.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(vis, img)
+    torch.cuda.synchronize()
+    assert torch.isfinite(uv.view(torch.float32)).all() and torch.isfinite(img).all()
+    sel = np.array(sorted({0, min(1, n_snap - 1), n_snap // 2, n_snap - 1}), np.int64)
+    ref = oracle.image_batch(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_c, sel, want_grids=True)
+    uvh = uv.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    imh = img.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        g_ref, i_ref = ref["grids"][q], ref["images"][q]
+        assert np.max(np.abs(uvh[q] - g_ref)) <= GRID_TOL * np.max(np.abs(g_ref)), f"grid snapshot {sel[q]}"
+        assert np.all(uvh[q][g_ref == 0] == 0)
+        assert np.max(np.abs(imh[q] - i_ref)) <= IMG_TOL * np.max(np.abs(i_ref)), f"image snapshot {sel[q]}"
+    # the same through the stand-alone pass: blink_correct, then the plain calls
+    plan.apply_corrections(False)
+    two = plan.grid_image(plan.correct(vis))
+    peak = two.abs().amax(dim=(-2, -1), keepdim=True)
+    assert ((img - two).abs() <= 1e-5 * peak).all()
+    assert torch.equal(plan.grid(vis).view(torch.float32), plain_uv.view(torch.float32))
+    assert torch.equal(plan.grid_image(vis), plain_img)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == path0
+    plan.close()
+
+
 def test_corrections_odd_table_and_unaligned_views(torch_cuda, blink):
     """Odd n_ch * n_bl and an 8-byte-aligned (not 16) buffer take the one-visibility kernel."""
     torch = torch_cuda
