@@ -401,6 +401,9 @@ def main():
     plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
     t_plan = time.perf_counter() - t_plan
     plan.reserve(w.n_t)
+    t_refresh = time.perf_counter()
+    plan.refresh(w.ant_enu_m)                    # a0 again + every table rebuilt and swapped in (f2: plan refresh)
+    t_refresh = time.perf_counter() - t_refresh
     vis = vis_h.cuda(non_blocking=True)
     shape = (w.n_t, w.n_ch, w.n_pix, w.n_pix)
     fused = args.path in ("fused", "auto")       # blink_grid_image is the fast public call
@@ -583,7 +586,7 @@ def main():
         "roofline_step": {"bound": "hbm", "achieved": step_gbs, "peak": peak, "unit": "GB/s",
                           "frac": step_gbs / peak, "algorithmic_bytes_per_snapshot": step_bytes},
         "side_bounds": side, "alu_peak": alu,
-        "plan_create_s": t_plan,
+        "plan_create_s": t_plan, "plan_refresh_s": t_refresh,
         "f2_corrections": corr, "cufft_reference": cufft,
         "f4_dynspec": dict(dyn, frac_of_hbm_peak=dyn["achieved_gbs"] / peak) if dyn else None,
         "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks,

@@ -141,6 +141,20 @@ int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m, int n_ant,
  * anything else on the same plan.
  */
 
+/*
+ * blink_plan_refresh -- step a0 again, for new antenna coordinates: the periodic plan refresh that
+ * time-dependent (u,v) need (a tracking array's projected baselines move
+ * with hour angle).  Same n_ant, frequencies, grid, weighting and options as at
+ * creation; runs the fp64 index kernel on the device and rebuilds every table (host cores, one channel
+ * per thread), then swaps them in, so afterwards the plan is indistinguishable from a new plan of the new
+ * coordinates (bit-exact indices, counts and images) while its scratch and host staging survive.
+ *   ant_enu_m  HOST [n_ant][3], the coordinates whose differences are the new baselines
+ * Synchronises the device (work queued on the old tables finishes first).  Drops the correction table
+ * (it depends on the geometry): call blink_plan_set_corrections / blink_plan_apply_corrections again.
+ * On error the plan is unchanged.
+ */
+int blink_plan_refresh(blink_plan *plan, const double *ant_enu_m, void *stream);
+
 /* frees the plan and its device memory; NULL is a no-op */
 int blink_plan_destroy(blink_plan *plan);
 

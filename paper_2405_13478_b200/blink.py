@@ -24,7 +24,7 @@ EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_pl
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
            "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct", "blink_dynspec",
            "blink_image", "blink_grid_validate", "blink_grid_image_host", "blink_plan_reserve_host",
-           "blink_plan_apply_corrections"]
+           "blink_plan_apply_corrections", "blink_plan_refresh"]
 TESTING_EXPORTS = ["blink_host_build_gather", "blink_host_fused_emulate", "blink_probe_fp32"]
 
 
@@ -83,6 +83,8 @@ def load() -> ctypes.CDLL:
     lib.blink_grid_image_host.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_plan_reserve_host.restype = ci
     lib.blink_plan_reserve_host.argtypes = [vp, ci]
+    lib.blink_plan_refresh.restype = ci
+    lib.blink_plan_refresh.argtypes = [vp, vp, vp]
     lib.blink_plan_destroy.restype = ci
     lib.blink_plan_destroy.argtypes = [vp]
     lib.blink_plan_query.restype = ci
@@ -207,6 +209,13 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+    def refresh(self, ant_enu_m, stream=None):
+        """blink_plan_refresh: new antenna coordinates, same everything else."""
+        ant = np.ascontiguousarray(ant_enu_m, np.float64)
+        if ant.shape != (self.n_ant, 3):
+            raise ValueError("ant_enu_m must be [n_ant, 3]")
+        _check(self._lib.blink_plan_refresh(self._h, ant.ctypes.data, _stream_ptr(stream)), "blink_plan_refresh")
 
     # ---- queries
     def _query(self, what, index, ctype, n=1):

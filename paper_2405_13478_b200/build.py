@@ -18,7 +18,7 @@ SOURCES = ["blink_plan.cu", "blink_grid.cu", "blink_image.cu", "blink_image_w.cu
 HEADERS = ["blink_internal.h", "fft_core.cuh", "sphase.cuh", "sgather.cuh", "wfft.cuh", "fused_kernel.cuh", os.path.join("..", "..", "include", "blink.h"),
            os.path.join("..", "..", "include", "blink_testing.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--expt-extended-lambda", "--expt-relaxed-constexpr"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "--expt-extended-lambda", "--expt-relaxed-constexpr"]
 OBJ_DIR = os.path.join(HERE, "build")
 
 
@@ -50,7 +50,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(res.stdout + res.stderr)
     if any(res.returncode != 0 for _, res in results):
         raise RuntimeError("nvcc failed building libblink.so")
-    link = subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] +
+    link = subprocess.run([nvcc, "-shared", "-Xcompiler", "-pthread", "-gencode", "arch=compute_100a,code=sm_100a"] +
                           [obj for obj, _ in results] + ["-o", LIB], capture_output=True, text=True)
     if link.returncode != 0:
         sys.stderr.write(link.stdout + link.stderr)

@@ -312,15 +312,17 @@ int grid_ring_layout(blink_plan *p, int corr, cudaStream_t st) {
       const size_t data_bytes = sizeof(float2) * (size_t)(C + zpad) * (corr ? 2 : 1);
       if (data_bytes > room) continue;
       tabs.assign((size_t)n_ch * n_chunk, AbstractTable());
-      bool ok = true;
+      std::atomic<bool> all_ok{true};
+      parallel_for(n_ch * n_chunk, [&](int i) {
+        if (!all_ok.load()) return;
+        const int ch = i / n_chunk, c = i % n_chunk;
+        bool ok = true;
+        build_chunk_table(p->gathers[ch], owner[ch], slot[ch], c * C, std::min(n_bl, (c + 1) * C), sink0, tabs[i], ok);
+        if (!ok) all_ok.store(false);
+      });
+      if (!all_ok.load()) continue;
       tab_stride = 0;
-      for (int ch = 0; ch < n_ch && ok; ++ch)
-        for (int c = 0; c < n_chunk && ok; ++c) {
-          AbstractTable &t = tabs[(size_t)ch * n_chunk + c];
-          build_chunk_table(p->gathers[ch], owner[ch], slot[ch], c * C, std::min(n_bl, (c + 1) * C), sink0, t, ok);
-          tab_stride = std::max(tab_stride, t.bytes.size());
-        }
-      if (!ok) continue;
+      for (const AbstractTable &t : tabs) tab_stride = std::max(tab_stride, t.bytes.size());
       buf_bytes = (data_bytes + tab_stride + 127) / 128 * 128;
       if (buf_bytes > room) continue;
       found = true;

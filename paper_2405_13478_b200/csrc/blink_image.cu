@@ -346,6 +346,7 @@ size_t scratch_need(const blink_plan *p, long long n_t, bool fused) {
 }
 
 int image_reserve(blink_plan *p, int n_t) {
+  p->reserved_n_t = std::max(p->reserved_n_t, n_t);
   const long long n_snap = std::max<long long>((long long)n_t * p->n_ch, 1);
   const size_t need = std::max(scratch_need(p, n_t, false), scratch_need(p, n_t, true));
   if (need <= p->scratch_bytes && (!p->warp_route || n_snap <= p->warp_snap_cap)) return BLINK_OK;

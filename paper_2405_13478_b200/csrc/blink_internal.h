@@ -4,8 +4,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <atomic>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/blink.h"
@@ -129,6 +131,7 @@ struct blink_plan {
   int wu = 0;                       // padded half-plane width
   float2 *d_scratch = nullptr;
   size_t scratch_bytes = 0;
+  int reserved_n_t = 0;             // largest n_t blink_plan_reserve has been asked for
   int image_path = 1;
   int chunk_snapshots = 0;
 
@@ -262,5 +265,29 @@ template <class K> inline int ensure_max_smem(K kern, const blink_plan *p, std::
   if (carveout) BLINK_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100), what);
   done.fetch_or(bit, std::memory_order_release);
   return BLINK_OK;
+}
+}  // namespace blink
+
+namespace blink {
+// plan-time host work is independent per channel (and per chunk): fn(i) for i in [0, n) on the host cores
+template <class F> inline void parallel_for(int n, F fn) {
+  const int hw = (int)std::thread::hardware_concurrency();
+  const int nt = std::min(n, std::max(1, std::min(hw, 32)));
+  if (nt <= 1) {
+    for (int i = 0; i < n; ++i) fn(i);
+    return;
+  }
+  std::atomic<int> next{0};
+  std::vector<std::thread> th;
+  th.reserve(nt);
+  for (int t = 0; t < nt; ++t)
+    th.emplace_back([&] {
+      for (;;) {
+        const int i = next.fetch_add(1);
+        if (i >= n) break;
+        fn(i);
+      }
+    });
+  for (auto &x : th) x.join();
 }
 }  // namespace blink

@@ -136,8 +136,9 @@ static void build_rank_tables(const std::vector<HostGather> &gathers, int n_ch, 
   t.cellrec.assign((size_t)n_ch * n_pass * ncm, 0);
   t.nact.assign((size_t)n_ch * n_pass, 0);
   std::vector<std::vector<uint16_t>> roffs((size_t)n_ch * n_pass);
-  int maxlen = 0;
-  for (int ch = 0; ch < n_ch; ++ch) {
+  std::vector<int> maxlen_ch(n_ch, 0);
+  parallel_for(n_ch, [&](int ch) {
+    int maxlen = 0;
     const HostGather &g = gathers[ch];
     uint16_t *sc = t.scat.data() + (size_t)ch * n_bl;
     for (int q = 0; q < n_pass; ++q) {
@@ -177,7 +178,9 @@ static void build_rank_tables(const std::vector<HostGather> &gathers, int n_ch, 
         }
       }
     }
-  }
+    maxlen_ch[ch] = maxlen;
+  });
+  const int maxlen = *std::max_element(maxlen_ch.begin(), maxlen_ch.end());
   t.roff_stride = ((maxlen + 1 + 3) / 4) * 4;   // rows stay 8-byte aligned for ushort4 reads
   t.roff.assign((size_t)n_ch * n_pass * t.roff_stride, 0);
   for (size_t i = 0; i < roffs.size(); ++i)
@@ -351,9 +354,10 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
   std::vector<int32_t> h_pband((size_t)n_ch * (p->n_bands + 1), 0);
   std::vector<HostGather> &gathers = p->gathers;
   gathers.assign(n_ch, HostGather());
-  for (int ch = 0; ch < n_ch; ++ch) {
+  std::vector<int> ch_rc(n_ch, BLINK_OK);
+  parallel_for(n_ch, [&](int ch) {
     HostGather &g = gathers[ch];
-    PLAN_TRY(build_gather_host(h_cell.data() + (size_t)ch * n_bl, n_bl, N, g));
+    if ((ch_rc[ch] = build_gather_host(h_cell.data() + (size_t)ch * n_bl, n_bl, N, g)) != BLINK_OK) return;
     ChannelInfo &ci = p->chinfo[ch];
     ci.n_kept = g.n_kept;
     ci.n_can = g.n_can;
@@ -397,10 +401,14 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
       h_pcell[(size_t)ch * 2 * n_bl + k] = pl[k].first;
       h_pcode[(size_t)ch * 2 * n_bl + k] = pl[k].second;
     }
+  });
+  for (int ch = 0; ch < n_ch; ++ch) {
+    PLAN_TRY(ch_rc[ch]);
+    const HostGather &g = gathers[ch];
     p->n_can_max = std::max(p->n_can_max, (int)g.n_can);
     for (int j = 0; j < g.n_can; ++j) p->seg_len_max = std::max(p->seg_len_max, g.seg_start[j + 1] - g.seg_start[j]);
-    p->kx_max_all = std::max(p->kx_max_all, kxm);
-    p->ky_max_all = std::max(p->ky_max_all, kym);
+    p->kx_max_all = std::max(p->kx_max_all, p->chinfo[ch].kx_max);
+    p->ky_max_all = std::max(p->ky_max_all, p->chinfo[ch].ky_max);
   }
   if (p->n_can_max > kPlaceMask) { plan_free(p); return BLINK_EUNSUPPORTED; }
 
@@ -590,6 +598,33 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
 extern "C" int blink_plan_destroy(blink_plan *plan) {
   plan_free(plan);
   return BLINK_OK;
+}
+
+// blink_plan_refresh: step a0 again for new antenna coordinates (a tracking array's projected baselines
+// move with hour angle), everything else as at creation.  The index kernel runs on the
+// device, the table packing on the host cores (one channel per thread); the new tables replace the old
+// ones once they are complete, the scratch and the host staging are kept.
+extern "C" int blink_plan_refresh(blink_plan *p, const double *ant_enu_m, void *stream) {
+  if (!p || !ant_enu_m) return BLINK_EINVAL;
+  int rc = check_device(p);
+  if (rc != BLINK_OK) return rc;
+  blink_plan *q = nullptr;
+  blink_options opt = p->opt;
+  rc = blink_plan_create_opts(&q, ant_enu_m, p->n_ant, p->h_freq.data(), p->n_ch, p->n_pix, p->pixscale, p->weighting,
+                              stream, opt.struct_size ? &opt : nullptr);
+  if (rc != BLINK_OK) return rc;
+  // kernels already queued still read the old tables
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) {
+    set_cuda_error(e, "blink_plan_refresh sync");
+    plan_free(q);
+    return BLINK_ECUDA;
+  }
+  std::swap(*p, *q);                       // p: the new tables; q: the old ones, about to be freed
+  std::swap(p->hp, q->hp);                 // the host staging depends on n_ch, n_bl, N only
+  const int reserved = q->reserved_n_t;
+  plan_free(q);
+  return reserved > 0 ? image_reserve(p, reserved) : BLINK_OK;   // scratch for the new bounding box
 }
 
 extern "C" int blink_plan_reserve(blink_plan *plan, int n_t) {

@@ -672,6 +672,47 @@ def test_corrections_fused_at_load(torch_cuda, blink, oracle, name, options):
     plan.close()
 
 
+@pytest.mark.parametrize("name", ["station128", "station", "mwa1"])
+def test_plan_refresh(torch_cuda, blink, oracle, name):
+    """blink_plan_refresh (time-dependent (u,v): the array seen from a new hour angle, here the layout
+    rotated and foreshortened): afterwards indices and counts are bit-exact against the oracle on the NEW
+    coordinates, and every call returns bit for bit what a plan created on them returns; scratch reserved
+    before the refresh still serves (hot calls with auto_reserve off)."""
+    torch = torch_cuda
+    w = _workload(name)
+    vis = torch.from_numpy(w.vis()).cuda()
+    a = np.deg2rad(7.5)
+    rot = np.array([[np.cos(a), -np.sin(a), 0.0], [0.93 * np.sin(a), 0.93 * np.cos(a), 0.0], [0.0, 0.0, 1.0]])
+    ant2 = np.asarray(w.ant_enu_m) @ rot.T
+    plan = _plan(blink, w)
+    plan.reserve(w.n_t)
+    before = plan.grid_image(vis).clone()
+    plan.refresh(ant2)
+    for ch in range(w.n_ch):
+        r = oracle.uv_cells(ant2, w.freq_hz[ch], w.n_pix, w.pixscale)
+        assert np.array_equal(plan.cell_idx(ch), r["cell"])
+        assert np.array_equal(plan.counts(ch), oracle.counts(r["cell"], r["cell_conj"], w.n_pix))
+        assert plan.n_dropped(ch) == r["n_dropped"]
+    fresh = blink.Plan(ant2, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == fresh.query_i32(blink.Q_FUSED_PATH)
+    uv = plan.grid(vis)
+    assert torch.equal(uv.view(torch.float32), fresh.grid(vis).view(torch.float32))
+    img = plan.grid_image(vis, auto_reserve=False)
+    assert torch.equal(img, fresh.grid_image(vis))
+    assert torch.equal(plan.image(uv, auto_reserve=False), fresh.image(uv))
+    assert not torch.equal(img, before)
+    n_snap = w.n_t * w.n_ch
+    sel = np.array([0, n_snap - 1], np.int64)
+    ref = oracle.image_batch(ant2, w.freq_hz, w.n_pix, w.pixscale, w.weighting, w.vis(), sel)
+    got = img.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        assert np.max(np.abs(got[q] - ref["images"][q])) <= IMG_TOL * np.max(np.abs(ref["images"][q]))
+    plan.refresh(w.ant_enu_m)                      # and back: the original images, bit for bit
+    assert torch.equal(plan.grid_image(vis, auto_reserve=False), before)
+    fresh.close()
+    plan.close()
+
+
 def test_corrections_odd_table_and_unaligned_views(torch_cuda, blink):
     """Odd n_ch * n_bl and an 8-byte-aligned (not 16) buffer take the one-visibility kernel."""
     torch = torch_cuda
