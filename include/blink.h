@@ -78,7 +78,8 @@ typedef enum blink_query {
   BLINK_Q_FUSED_PATH = 14,  /* out: int32  route of blink_grid_image: 1 = shared memory, 2 = warp-per-transform, 0 = two kernels */
   BLINK_Q_FUSED_CHUNK = 15, /* out: int32  snapshots per chunk of the two-kernel route */
   BLINK_Q_CORR = 16,        /* out: const float2* DEVICE [n_ch][n_bl] correction factors (NULL until set) */
-  BLINK_Q_CORR_FUSED = 17   /* out: int32  1 = blink_grid / blink_grid_image apply the factors at load */
+  BLINK_Q_CORR_FUSED = 17,  /* out: int32  1 = blink_grid / blink_grid_image apply the factors at load */
+  BLINK_Q_TENSOR_ROUTE = 18 /* out: int32  1 = the shared-memory route runs its transforms on the tensor cores (k_fused_tc) */
 } blink_query;
 
 typedef struct blink_plan blink_plan; /* opaque */

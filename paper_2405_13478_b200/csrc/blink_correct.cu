@@ -197,6 +197,7 @@ extern "C" int blink_plan_apply_corrections(blink_plan *p, int on, void *stream)
   if (on) {
     cudaStream_t st = (cudaStream_t)stream;
     if (p->fused_path == 1 && (rc = fused_layout(p, 1, st)) != BLINK_OK) return rc;
+    if (p->tc_route && (rc = fused_layout_tc(p, 1, st)) != BLINK_OK) return rc;
     if (p->ring_path == 1 && (rc = grid_ring_layout(p, 1, st)) != BLINK_OK) return rc;
   }
   p->corr_on = on;

@@ -34,7 +34,7 @@ int fused_setup(blink_plan *p) {
   return BLINK_OK;
 }
 
-static int upload_table(void **dst, const void *src, size_t bytes, cudaStream_t st, const char *what) {
+int upload_table(void **dst, const void *src, size_t bytes, cudaStream_t st, const char *what) {
   cudaError_t e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
   if (e != cudaSuccess) {
     set_cuda_error(e, what);
@@ -91,11 +91,17 @@ static bool fused_geom(const blink_plan *p, FusedGeom &g) {
 // chunk_vis + 16 with corr: the 16 extra slots of buffer 0 and their factor partners are zeroed once
 // by the kernel and never written again -- the "zero visibility" a padded table entry points at must
 // have a finite factor behind it.
-int fused_layout(blink_plan *p, int corr, cudaStream_t st) {
-  GatherLayout &L = p->fl[corr];
+static int fused_layout_impl(blink_plan *p, GatherLayout &L, int corr, bool tc, cudaStream_t st) {
   if (L.ok) return BLINK_OK;
   FusedGeom g;
   if (!fused_geom(p, g) || (int)p->gathers.size() != p->n_ch) return BLINK_OK;
+  if (tc) {
+    // k_fused_tc: the aliased region is its 64 KB operand region, followed by the 64 KB constant matrix;
+    // what is left holds up to two dedicated chunk buffers
+    if (p->n_pix != 256 || g.D != 1 || std::max(p->kx_max_all, p->ky_max_all) > 63) return BLINK_OK;
+    g.region = 65536;
+    g.region_al = 131072;
+  }
   const int n_bl = p->n_bl, n_ch = p->n_ch;
   const size_t limit = (size_t)p->max_smem_optin;
   const int zpad = corr ? 16 : 0;
@@ -103,9 +109,10 @@ int fused_layout(blink_plan *p, int corr, cudaStream_t st) {
   std::vector<std::vector<int>> owner(n_ch), slot(n_ch);
   for (int ch = 0; ch < n_ch; ++ch) assign_cells(p->gathers[ch], owner[ch], slot[ch]);
 
-  const int force_chunks = p->opt.tune[kTuneFusedChunks];
+  const int force_chunks = std::abs(p->opt.tune[kTuneFusedChunks]);
+  const bool two_buffers_ok = p->opt.tune[kTuneFusedChunks] < 0;   // (negative: also accept a ring of two buffers)
   std::vector<AbstractTable> tabs;
-  int n_chunk = 0, C = 0, nbuf = 0;
+  int n_chunk = 0, C = 0, nbuf = 0, nded = 1;
   size_t tab_stride = 0, buf_bytes = 0;
   bool found = false;
   for (n_chunk = std::max(1, force_chunks); n_chunk <= 64 && !found; ++n_chunk) {
@@ -128,10 +135,17 @@ int fused_layout(blink_plan *p, int corr, cudaStream_t st) {
     tab_stride = 0;
     for (const AbstractTable &t : tabs) tab_stride = std::max(tab_stride, t.bytes.size());
     buf_bytes = (data_bytes + tab_stride + 127) / 128 * 128;
-    nbuf = 1 + (int)std::min<size_t>(7, g.region / buf_bytes);
+    const size_t tail = g.s_bytes + 16 * 8 + 128 + 64;  // sums, mbarriers (<= 8 buffers) and the kernel's own words
+    if (g.region_al + buf_bytes + tail > limit) continue;
+    nded = tc ? (int)std::min<size_t>(2, (limit - g.region_al - tail) / buf_bytes) : 1;
+    nded = std::min(nded, n_chunk);
+    nbuf = nded + (int)std::min<size_t>(8 - nded, g.region / buf_bytes);
     nbuf = std::min(nbuf, n_chunk);
     if (nbuf < 2 && n_chunk > 1) continue;             // the ring needs a second buffer
-    const size_t total = g.region_al + buf_bytes + g.s_bytes + 16 * (size_t)nbuf + 8 + 64;
+    // (measured on the station, k_fused_tc: 6 chunks in a ring of two 0.424 ms, 9 chunks in a ring of three 0.471 ms:
+    // fewer, larger chunks mean fewer, fuller groups in phase S, which outweighs the deeper ring)
+    (void)two_buffers_ok;   // (two dedicated + one aliased keep the copies ahead of the sums)
+    const size_t total = g.region_al + (size_t)nded * buf_bytes + tail;
     if (total > limit || total > 0x7FFFu * 8u) continue;
     found = true;
     break;
@@ -143,10 +157,11 @@ int fused_layout(blink_plan *p, int corr, cudaStream_t st) {
   L.nbuf = nbuf;
   L.tab_stride = (int)tab_stride;
   L.buf_bytes = (uint32_t)buf_bytes;
+  L.nded = nded;
   L.off_first = (uint32_t)g.region_al;
-  L.off_S = (uint32_t)(g.region_al + buf_bytes);      // multiple of 128: slot s of S sits in bank s mod 16
-  L.off_bar = (uint32_t)(g.region_al + buf_bytes + g.s_bytes);
-  L.smem = g.region_al + buf_bytes + g.s_bytes + 16 * (size_t)nbuf + 8 + 16;
+  L.off_S = (uint32_t)(g.region_al + (size_t)nded * buf_bytes);      // multiple of 128: slot s of S sits in bank s mod 16
+  L.off_bar = (uint32_t)((L.off_S + g.s_bytes + 15) / 16 * 16);
+  L.smem = L.off_bar + 16 * (size_t)nbuf + 128;
   L.tab_off = (uint32_t)(sizeof(float2) * (size_t)(C + zpad));
   L.f_off = corr ? (uint32_t)(L.tab_off + tab_stride) : 0u;
 
@@ -159,7 +174,8 @@ int fused_layout(blink_plan *p, int corr, cudaStream_t st) {
       const size_t cp = (size_t)ch * n_chunk + c;
       std::vector<unsigned char> &b = tabs[cp].bytes;
       const int bi = c % nbuf;
-      const uint32_t base_slot = (uint32_t)((bi == 0 ? L.off_first : (uint32_t)(bi - 1) * L.buf_bytes) / 8);
+      const uint32_t base_slot =
+          (uint32_t)((bi < nded ? L.off_first + (uint32_t)bi * L.buf_bytes : (uint32_t)(bi - nded) * L.buf_bytes) / 8);
       finalize_chunk_table(b, base_slot, zslot0);
       std::memcpy(h_tab.data() + cp * tab_stride, b.data(), b.size());
       h_size[cp] = (uint32_t)b.size();
@@ -171,6 +187,9 @@ int fused_layout(blink_plan *p, int corr, cudaStream_t st) {
   L.ok = true;
   return BLINK_OK;
 }
+
+int fused_layout(blink_plan *p, int corr, cudaStream_t st) { return fused_layout_impl(p, p->fl[corr], corr, false, st); }
+int fused_layout_tc(blink_plan *p, int corr, cudaStream_t st) { return fused_layout_impl(p, p->tl[corr], corr, true, st); }
 
 // Lay out shared memory, build and upload the tables of the route (plain layout; the layout with
 // correction factors is built when blink_plan_apply_corrections first asks for it).
@@ -295,6 +314,7 @@ static int launch_fused_c(const blink_plan *p, const FusedParams &fp, cudaStream
 }
 
 static int launch_fused(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st) {
+  if (p->tc_route && p->tl[p->corr_on ? 1 : 0].ok) return launch_fused_tc(p, vis, n_t, img, st);
   const GatherLayout &L = p->fl[p->corr_on ? 1 : 0];
   FusedParams fp;
   fp.vis = vis; fp.img = img; fp.chinfo = p->d_chinfo;

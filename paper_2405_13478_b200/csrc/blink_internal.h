@@ -43,7 +43,8 @@ enum TuneSlot {
   kTuneImageRp = 4,       // two-pass imaging: row pairs per CTA (pass B)
   kTuneDirectMax = 5,     // two-kernel route: most cells per column for the direct-sum column transform, +1 (default 13)
   kTuneDynspecRoute = 6,  // blink_dynspec: 1 = register-load kernel even for aligned cubes
-  kTuneSpare = 7
+  kTuneTensor = 7         // 1 = the shared-memory route at N = 256 runs its transforms on the tensor cores (k_fused_tc);
+                          // default off: measured 0.422 ms against 0.403 ms for k_fused on the station
 };
 
 struct HostGather {    // cell-sorted tables of one channel (see blink_host_build_gather)
@@ -56,7 +57,7 @@ struct HostGather {    // cell-sorted tables of one channel (see blink_host_buil
 // (tab_off bytes behind the visibilities) and -- when the pre-gridding corrections are fused in --
 // its correction factors (f_off bytes behind the visibilities; 0 = none).
 struct GatherLayout {
-  int chunk_vis = 0, n_chunk = 0, nbuf = 0, tab_stride = 0;
+  int chunk_vis = 0, n_chunk = 0, nbuf = 0, tab_stride = 0, nded = 1;   // nded: dedicated (un-aliased) buffers
   uint32_t buf_bytes = 0, off_first = 0, off_S = 0, off_bar = 0, tab_off = 0, f_off = 0;
   size_t smem = 0;
   unsigned char *d_tab = nullptr;   // [n_ch][n_chunk][tab_stride]
@@ -162,6 +163,11 @@ struct blink_plan {
   int h_max = 0;                    // phase-H records per channel (padded with pos = 0xFFFF)
   int fused_threads = 512;
   blink::GatherLayout fl[2];        // [0] plain, [1] with correction factors; off_first = the dedicated buffer 0
+  // tensor-core form of the route (k_fused_tc, fused_tc_kernel.cuh): N = 256, bounding box inside |k| < 64
+  int tc_route = 0;                 // 1 = blink_grid_image takes k_fused_tc
+  blink::GatherLayout tl[2];        // its phase-S layouts ([0] plain, [1] with correction factors)
+  uint2 *d_tcref = nullptr;         // [n_ch][16][512] phase-H cell references
+  uint4 *d_cmat = nullptr;          // [4096] the constant cosine / sine matrix, bf16 hi | lo, operand layout
   uint2 *d_hrec = nullptr;          // [n_ch][h_max] {line position | j << 16 | flag << 30, weight}
   int fused_D = 1;                  // polyphase route: the image is fused_D x fused_D interleaved sub-images of n_pix / fused_D
   float2 *d_hw = nullptr;           // [n_ch][fused_D][h_max] complex phase-H weights of the sub-image rows
@@ -230,8 +236,14 @@ int grid_ring_layout(blink_plan *p, int corr, cudaStream_t st);
 int fused_setup(blink_plan *p);
 int fused_build(blink_plan *p, cudaStream_t st);
 int fused_layout(blink_plan *p, int corr, cudaStream_t st);
+int fused_layout_tc(blink_plan *p, int corr, cudaStream_t st);
+int fused_tc_build(blink_plan *p, cudaStream_t st);
+int launch_fused_tc(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);
+int upload_table(void **dst, const void *src, size_t bytes, cudaStream_t st, const char *what);
 // true when blink_grid_image takes the shared-memory kernel in the plan's current state
-inline bool fused_smem_route(const blink_plan *p) { return p->fused_path == 1 && p->fl[p->corr_on ? 1 : 0].ok; }
+inline bool fused_smem_route(const blink_plan *p) {
+  return p->fused_path == 1 && (p->fl[p->corr_on ? 1 : 0].ok || (p->tc_route && p->tl[p->corr_on ? 1 : 0].ok));
+}
 int fused_line_stride(int n_pix);
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);
 int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, float *img, cudaStream_t st);

@@ -204,9 +204,11 @@ static void plan_free(blink_plan *p) {
   cudaFree(p->d_cell); cudaFree(p->d_counts); cudaFree(p->d_chinfo); cudaFree(p->d_src);
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
   cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol); cudaFree(p->d_vrec); cudaFree(p->d_corr); cudaFree(p->d_tw32);
+  cudaFree(p->d_tcref); cudaFree(p->d_cmat);
   cudaFree(p->d_hrec); cudaFree(p->d_hw); cudaFree(p->d_pha); cudaFree(p->d_tw_sub); cudaFree(p->d_rplace);
   for (int c = 0; c < 2; ++c) {
     cudaFree(p->fl[c].d_tab); cudaFree(p->fl[c].d_size); cudaFree(p->rl[c].d_tab); cudaFree(p->rl[c].d_size);
+    cudaFree(p->tl[c].d_tab); cudaFree(p->tl[c].d_size);
   }
   delete p;
 }
@@ -547,6 +549,7 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
     p->warp_route = (p->opt.warp_route != -1 && warp_route_applies(p)) ? 1 : 0;
   }
   PLAN_TRY(fused_build(p, st));
+  PLAN_TRY(fused_tc_build(p, st));
   PLAN_TRY(grid_ring_build(p, st));
   if (weighting == BLINK_UNIFORM) {
     // canonical cells are exactly the occupied half-plane cells with ky > 0 or (ky == 0, kx >= 0);
@@ -683,6 +686,7 @@ extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *
     case BLINK_Q_FUSED_CHUNK: *(int32_t *)out = p->fused_chunk; break;
     case BLINK_Q_CORR: *(const void **)out = p->d_corr; break;
     case BLINK_Q_CORR_FUSED: *(int32_t *)out = p->corr_on; break;
+    case BLINK_Q_TENSOR_ROUTE: *(int32_t *)out = (fused_smem_route(p) && p->tc_route && p->tl[p->corr_on ? 1 : 0].ok) ? 1 : 0; break;
     default: return BLINK_EINVAL;
   }
   return BLINK_OK;

@@ -50,6 +50,7 @@ struct FusedParams {
   int n_bl, n_ch, n_snap, n_can_max, n_chunk, chunk_vis, nbuf, tab_stride, n_col, h_max;
   uint32_t buf_bytes, off_dedicated, off_S, off_bar;   // byte offsets into dynamic shared memory
   uint32_t tab_off, f_off, smem;                       // table / factors behind a buffer's visibilities; launch smem bytes
+  int chunk_shift;                                     // k_fused_tc: floor(8 * 65536 / n_chunk): (c * this) >> 16 = 8 c / n_chunk
 };
 
 

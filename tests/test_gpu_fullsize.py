@@ -18,9 +18,9 @@ def _plan(blink, w, **options):
     return blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=options or None)
 
 
-def _fullsize_grid_image(torch, blink, oracle, w, sel, expect_path):
+def _fullsize_grid_image(torch, blink, oracle, w, sel, expect_path, **options):
     vis = w.vis()
-    plan = _plan(blink, w)
+    plan = _plan(blink, w, **options)
     assert plan.query_i32(blink.Q_FUSED_PATH) == expect_path
     n_snap = w.n_t * w.n_ch
     img = torch.full((w.n_t, w.n_ch, w.n_pix, w.n_pix), float("nan"), dtype=torch.float32, device="cuda")
@@ -46,6 +46,14 @@ def test_full_size_station_grid_image(torch_cuda, blink, oracle):
     w = synth.config_station()
     n_snap = w.n_t * w.n_ch
     _fullsize_grid_image(torch_cuda, blink, oracle, w, [0, 147, 148, 149, 777, 1600, 3051, n_snap - 1], 1)
+
+
+def test_full_size_station_grid_image_tensor_cores(torch_cuda, blink, oracle):
+    """The same batch through k_fused_tc (tune[7] = 1): > 21 snapshots per CTA with the image of each held in
+    TMEM while the next one is gridded."""
+    w = synth.config_station()
+    n_snap = w.n_t * w.n_ch
+    _fullsize_grid_image(torch_cuda, blink, oracle, w, [0, 147, 148, 1600, n_snap - 149, n_snap - 1], 1, tune={7: 1})
 
 
 @pytest.mark.parametrize("n_pix,sel", [(128, [0, 148, 2222, 3999]), (256, [0, 148, 2222, 3999]),

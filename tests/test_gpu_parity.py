@@ -367,6 +367,50 @@ def test_polyphase_route_matches_two_kernel_route(torch_cuda, blink, oracle, n_p
     plan.close()
 
 
+@pytest.mark.parametrize("weighting,n_t", [(synth.NATURAL, 7), (synth.UNIFORM, 2)])
+def test_tensor_core_route(torch_cuda, blink, oracle, weighting, n_t):
+    """blink_grid_image at N = 256 with the transforms on the tensor cores (k_fused_tc, option tune[7] = 1:
+    band-limited DFT as bf16 hi/lo three-product GEMMs, tcgen05.mma with TMEM accumulators; the finished
+    image drains from TMEM during the next snapshot's gridding phase): more snapshots than CTAs (7 x 32 = 224),
+    every snapshot against the CUDA-core route at 1e-5 of the peak, sampled ones against the oracle at the
+    image bar; also with the correction factors fused into the load, and repeated calls."""
+    torch = torch_cuda
+    w = synth.config_station(n_t=n_t, n_ch=32)
+    w.weighting = weighting
+    vis_h = w.vis()
+    vis = torch.from_numpy(vis_h).cuda()
+    plan0 = _plan(blink, w)
+    assert plan0.query_i32(blink.Q_TENSOR_ROUTE) == 0
+    ref = plan0.grid_image(vis)
+    plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=dict(tune={7: 1}))
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 1 and plan.query_i32(blink.Q_TENSOR_ROUTE) == 1
+    img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    for _ in range(2):
+        plan.grid_image(vis, img)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img).all(), "image not fully overwritten"
+    peak = ref.abs().amax(dim=(-2, -1), keepdim=True)
+    assert ((img - ref).abs() <= 1e-5 * peak).all()
+    n_snap = w.n_t * w.n_ch
+    sel = np.array(sorted({0, 33, min(150, n_snap - 1), n_snap - 1}), np.int64)
+    orc = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_h, sel)
+    got = img.view(n_snap, 256, 256)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        pk = np.max(np.abs(orc["images"][q]))
+        assert np.max(np.abs(got[q] - orc["images"][q])) <= IMG_TOL * pk
+    # corrections fused at load on the same kernel
+    ant, gains, cables = _corr_inputs(w, 23)
+    for pl in (plan0, plan):
+        pl.set_corrections(gains, cables, 0.1, 0.05)
+        pl.apply_corrections(True)
+    assert plan.query_i32(blink.Q_TENSOR_ROUTE) == 1
+    c_ref, c_img = plan0.grid_image(vis), plan.grid_image(vis)
+    cpk = c_ref.abs().amax(dim=(-2, -1), keepdim=True)
+    assert ((c_img - c_ref).abs() <= 1e-5 * cpk).all()
+    plan0.close()
+    plan.close()
+
+
 def test_warp_route_ring_reuse(torch_cuda, blink, oracle):
     """blink_grid_image, warp-per-transform route (k_img1024), on more snapshots than its ring of U
     slots holds (here a ring of 3), so that pass A has to wait for pass B to release a slot: every
