@@ -380,8 +380,8 @@ extern "C" int blink_host_fused_emulate(const int32_t *cell, int n_bl, int n_pix
       std::memcpy(&wx, tab + 8 * w, 4);
       std::memcpy(&lseq, tab + 8 * w + 4, 4);
       size_t blk = wx & 0xFFFFFFu;
-      for (int n = (int)(wx >> 24); n > 0; --n, lseq >>= 2) {
-        const int L = (int)(lseq & 3u) + 1;
+      for (int gi = 0; gi < (int)(wx >> 24); ++gi) {
+        const int L = group_len(lseq, gi);
         const uint16_t *row = reinterpret_cast<const uint16_t *>(tab + blk);
         for (int lane = 0; lane < 32; ++lane) {
           float ax = 0.f, ay = 0.f;

@@ -61,10 +61,10 @@ struct GroupIdx {
   int e[kFusedLcap];     // sign-extended: conj (bit 15) lands in the sign bit
 };
 
-__device__ __forceinline__ void load_idx(GroupIdx &gi, uint32_t blk) {
+template <int ROWS> __device__ __forceinline__ void load_idx(GroupIdx &gi, uint32_t blk) {
   asm volatile("ld.shared.u16 %0, [%1];" : "=r"(gi.j) : "r"(blk));
 #pragma unroll
-  for (int r = 0; r < kFusedLcap; ++r) asm volatile("ld.shared.s16 %0, [%1];" : "=r"(gi.e[r]) : "r"(blk + 64u * (r + 1)));
+  for (int r = 0; r < ROWS; ++r) asm volatile("ld.shared.s16 %0, [%1];" : "=r"(gi.e[r]) : "r"(blk + 64u * (r + 1)));
 }
 
 // lane l adds its L visibilities and folds the sum into its cell.  CORR: every visibility is first
@@ -116,34 +116,44 @@ __device__ __forceinline__ void fold_group(const GroupIdx &gi, uint32_t sm_base,
 }
 
 // One warp's share of a chunk: `tab` is the shared address of the chunk's gather table (it follows
-// the visibilities in the same buffer).  wd.x = offset of the warp's stream | number of groups
-// << 24, wd.y = L - 1 of each group, two bits apiece.
+// the visibilities in the same buffer).  wd.x = offset of the warp's stream | number of groups << 24,
+// wd.y = how many of them have L = 4, 3, 2, 1 rows (one byte each, L = 4 in the low byte); the stream
+// holds them in that order, so each length class is a tight loop of its own with no per-group dispatch.
+template <int L, bool CORR>
+__device__ __forceinline__ void consume_class(int n, uint32_t &blk, GroupIdx &ga, GroupIdx &gb, uint32_t sm_base,
+                                              uint32_t S_base, uint32_t f_base) {
+  // ga holds the index set of the class's first group; on return it holds that of the next class's first
+  // group (rows beyond a group's own L are loaded too and ignored; past the last group of the stream the
+  // bytes that follow are read, unused)
+  while (n >= 2) {
+    blk += (L + 1) * 64;
+    load_idx<L>(gb, blk);
+    fold_group<L, CORR>(ga, sm_base, S_base, f_base);
+    blk += (L + 1) * 64;
+    load_idx<L>(ga, blk);
+    fold_group<L, CORR>(gb, sm_base, S_base, f_base);
+    n -= 2;
+  }
+  if (n) {
+    blk += (L + 1) * 64;
+    load_idx<L>(gb, blk);
+    fold_group<L, CORR>(ga, sm_base, S_base, f_base);
+    ga = gb;
+  }
+}
+
 template <bool CORR = false>
 __device__ __forceinline__ void consume_chunk(uint32_t tab, int warp, int lane, uint32_t sm_base, uint32_t S_base,
                                               uint32_t f_off = 0) {
   const uint32_t f_base = sm_base + f_off;   // a visibility in slot s has its factor at f_base + 8 s
   const uint2 wd = lds_u2(tab + 8u * warp);
   uint32_t blk = tab + (wd.x & 0xFFFFFFu) + 2u * lane;
-  uint32_t lseq = wd.y;
-  int n = wd.x >> 24;
   GroupIdx ga, gb;                         // two index sets, used alternately
-  load_idx(ga, blk);
-  auto step = [&](const GroupIdx &cur, GroupIdx &nxt) {
-    const int L = (lseq & 3u) + 1;
-    lseq >>= 2;
-    blk += (L + 1) * 64;
-    load_idx(nxt, blk);                    // past the last group: reads the bytes that follow, unused
-    if (L == 4) fold_group<4, CORR>(cur, sm_base, S_base, f_base);
-    else if (L == 3) fold_group<3, CORR>(cur, sm_base, S_base, f_base);
-    else if (L == 2) fold_group<2, CORR>(cur, sm_base, S_base, f_base);
-    else fold_group<1, CORR>(cur, sm_base, S_base, f_base);
-  };
-  while (n > 0) {
-    step(ga, gb);
-    if (--n == 0) break;
-    step(gb, ga);
-    --n;
-  }
+  load_idx<kFusedLcap>(ga, blk);
+  consume_class<4, CORR>((int)(wd.y & 0xFFu), blk, ga, gb, sm_base, S_base, f_base);
+  consume_class<3, CORR>((int)((wd.y >> 8) & 0xFFu), blk, ga, gb, sm_base, S_base, f_base);
+  consume_class<2, CORR>((int)((wd.y >> 16) & 0xFFu), blk, ga, gb, sm_base, S_base, f_base);
+  consume_class<1, CORR>((int)(wd.y >> 24), blk, ga, gb, sm_base, S_base, f_base);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -159,13 +169,23 @@ __device__ __forceinline__ void consume_chunk(uint32_t tab, int warp, int lane, 
 // different banks, and so should the 16 visibilities of every row -- so the shared-memory reads of
 // the inner loop are (nearly) conflict-free.  Pieces of one cell never share a group.  Table of one
 // (channel, chunk), all offsets in bytes from its start:
-//   [0, 128)                per warp: uint32 offset of its stream | number of groups << 24, uint32 with
-//                           L - 1 of each group (two bits apiece, first group in the low bits)
+//   [0, 128)                per warp: uint32 offset of its stream | number of groups << 24, uint32 with the
+//                           number of groups of L = 4, 3, 2, 1 rows (one byte each, L = 4 in the low byte)
 //   stream of a warp:       groups in descending L; per group: uint16 j[32]  slot of the cell sum in S
 //                             (empty lanes: the zero slot of a bank the half-warp does not use)
 //                           L rows of uint16 e[32]: slot | conj << 15, where slot is the visibility's
 //                             position in shared memory in 8-byte units (padding: a zero slot in a
 //                             bank the half-row does not use)
+// L of the gi-th group of a warp's stream, from the class counts of its header word
+static inline int group_len(uint32_t counts, int gi) {
+  int L = kFusedLcap;
+  for (; L > 1; --L, counts >>= 8) {
+    if (gi < (int)(counts & 0xFFu)) return L;
+    gi -= (int)(counts & 0xFFu);
+  }
+  return 1;
+}
+
 struct AbstractTable {           // entries still relative to the chunk: (bl - lo) | conj << 15, 0x7FFF = padding
   std::vector<unsigned char> bytes;
   long rows = 0, halfrow_wavefronts = 0, groups = 0, rmw_wavefronts = 0;   // statistics
@@ -264,8 +284,8 @@ static void build_chunk_table(const HostGather &g, const std::vector<int> &owner
     }
     std::stable_sort(groups.begin(), groups.end(), [](const PackGroup &a, const PackGroup &b) { return a.L > b.L; });
     if ((int)groups.size() > kFusedMaxGroups) { ok = false; return; }
-    uint32_t lseq = 0;
-    for (size_t gi = 0; gi < groups.size(); ++gi) lseq |= (uint32_t)(groups[gi].L - 1) << (2 * gi);
+    uint32_t lseq = 0;                     // groups per length class, L = 4 in the low byte (they are sorted by L)
+    for (size_t gi = 0; gi < groups.size(); ++gi) lseq += 1u << (8 * (kFusedLcap - groups[gi].L));
     const uint32_t off = (uint32_t)o.size() | ((uint32_t)groups.size() << 24);
     std::memcpy(o.data() + 8 * w, &off, 4);
     std::memcpy(o.data() + 8 * w + 4, &lseq, 4);
@@ -342,8 +362,8 @@ static void finalize_chunk_table(std::vector<unsigned char> &b, uint32_t base_sl
     std::memcpy(&off, b.data() + 8 * w, 4);
     std::memcpy(&lseq, b.data() + 8 * w + 4, 4);
     size_t blk = off & 0xFFFFFFu;
-    for (int gi = (int)(off >> 24); gi > 0; --gi, lseq >>= 2) {
-      const int L = (int)(lseq & 3u) + 1;
+    for (int gi = 0; gi < (int)(off >> 24); ++gi) {
+      const int L = group_len(lseq, gi);
       uint16_t *rows = reinterpret_cast<uint16_t *>(b.data() + blk);
       for (int r = 1; r <= L; ++r)
         for (int half = 0; half < 2; ++half) {
