@@ -79,7 +79,9 @@ typedef enum blink_query {
   BLINK_Q_FUSED_CHUNK = 15, /* out: int32  snapshots per chunk of the two-kernel route */
   BLINK_Q_CORR = 16,        /* out: const float2* DEVICE [n_ch][n_bl] correction factors (NULL until set) */
   BLINK_Q_CORR_FUSED = 17,  /* out: int32  1 = blink_grid / blink_grid_image apply the factors at load */
-  BLINK_Q_TENSOR_ROUTE = 18 /* out: int32  1 = the shared-memory route runs its transforms on the tensor cores (k_fused_tc) */
+  BLINK_Q_TENSOR_ROUTE = 18,/* out: int32  1 = the shared-memory route runs its transforms on the tensor cores (k_fused_tc) */
+  BLINK_Q_WARP_KERNEL = 19  /* out: int32  kernel behind BLINK_Q_FUSED_PATH 2: 2 = residue-class kernel (intermediate in shared
+                               memory, k_img1024r), 1 = ring kernel (intermediate in an L2-sized ring, k_img1024), 0 = neither */
 } blink_query;
 
 typedef struct blink_plan blink_plan; /* opaque */
@@ -94,7 +96,7 @@ typedef struct blink_options {
   int32_t struct_size;        /* sizeof(blink_options) of the caller's header */
   int32_t fused_route;        /* blink_grid_image shared-memory route (BLINK_Q_FUSED_PATH 1): 0 auto, -1 never */
   int32_t polyphase;          /* its polyphase form for N = 512 / 1024: 0 auto, -1 never */
-  int32_t warp_route;         /* warp-per-transform route at N = 1024 (BLINK_Q_FUSED_PATH 2): 0 auto, -1 never */
+  int32_t warp_route;         /* warp-per-transform route at N = 1024 (BLINK_Q_FUSED_PATH 2): 0 auto, -1 never, 2 = its ring kernel */
   int32_t warp_ring;          /* snapshots of intermediate U kept in flight by that route: 0 auto (32 MB), else >= 2 */
   int32_t grid_ring;          /* blink_grid ring route: 0 auto, -1 never */
   int32_t grid_ring_min_snap; /* fewest snapshots per call that take it: 0 auto (one per SM), else >= 1 */

@@ -18,7 +18,7 @@ NATURAL, UNIFORM = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ERESERVE = 0, -1, -2, -3, -4, -5
 (Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
  Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK, Q_CORR, Q_CORR_FUSED,
- Q_TENSOR_ROUTE) = range(19)
+ Q_TENSOR_ROUTE, Q_WARP_KERNEL) = range(20)
 
 # include/blink.h (the product ABI) and include/blink_testing.h (host-only test hooks)
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create", "blink_plan_create_opts",

@@ -339,6 +339,7 @@ int image_setup(blink_plan *p) {
 // completion counters per snapshot.
 size_t scratch_need(const blink_plan *p, long long n_t, bool fused) {
   if (fused && fused_smem_route(p)) return 0;
+  if (p->res_route) return 0;
   const long long n_snap = std::max<long long>(n_t * p->n_ch, 1);
   if (p->warp_route) return warp_route_scratch_bytes(p, n_snap);
   const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
@@ -382,6 +383,8 @@ static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2
   ip.snap_base = 0;
   ip.ch0 = ch0;
   ip.direct_max = p->opt.tune[kTuneDirectMax] > 0 ? std::min(32, p->opt.tune[kTuneDirectMax] - 1) : 12;
+  if (p->res_route)                         // residue-class kernel, intermediate in shared memory (blink_image_r.cu)
+    return launch_img1024r(p, ip, n_snap, st);
   if (p->warp_route)                        // persistent warp-per-transform kernel (blink_image_w.cu)
     return launch_img1024(p, ip, n_snap, st);
   switch (p->n_pix) {

@@ -153,6 +153,14 @@ struct blink_plan {
   int seg_len_max = 0;              // most baselines in any canonical cell of any channel
   int warp_ring = 0;                // slots of U in the warp route's ring
   long long warp_snap_cap = 0;      // snapshots per call the warp route's counters in scratch are sized for
+  // residue-class route at N = 1024 (blink_image_r.cu): the intermediate stays in shared memory, no scratch
+  int res_route = 0;                // 1 = blink_grid_image / blink_image take k_img1024r
+  int res_cap = 0;                  // padded cells per channel of its tables
+  uint4 *d_rrec = nullptr;          // [n_ch][res_cap] cell records in the kernel's per-warp, rank-major order
+  uint8_t *d_rca = nullptr;         // [n_ch][res_cap] iy >> 5 per cell
+  uint16_t *d_res = nullptr;        // [n_ch][res_cap] tile slot per entry (column, iy mod 32)
+  int32_t *d_rhdr = nullptr;        // [n_ch][17][20] per-warp headers
+  uint32_t *d_rmask = nullptr;      // [n_ch][512] non-empty bins per column
   // blink_grid, ring route (see grid_ring_build in blink_grid.cu): phase S as in k_fused
   int ring_path = 0;                // 1 = k_grid_ring available
   int ring_min_snap = 0;            // fewer snapshots per call take the band route
@@ -212,6 +220,10 @@ int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t s
 bool warp_route_applies(const blink_plan *p);
 size_t warp_route_scratch_bytes(const blink_plan *p, long long n_snap);
 size_t warp_route_ring_bytes(const blink_plan *p);
+// residue-class kernel at N = 1024 (blink_image_r.cu)
+int res_route_build(blink_plan *p, cudaStream_t st);
+void res_route_free(blink_plan *p);
+int launch_img1024r(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st);
 
 }  // namespace blink
 

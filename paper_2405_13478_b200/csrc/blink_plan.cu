@@ -205,6 +205,7 @@ static void plan_free(blink_plan *p) {
   cudaFree(p->d_seg); cudaFree(p->d_pcell); cudaFree(p->d_pcode); cudaFree(p->d_pband); cudaFree(p->d_scat); cudaFree(p->d_cellrec); cudaFree(p->d_roff); cudaFree(p->d_nact); cudaFree(p->d_wkey); cudaFree(p->d_wval); cudaFree(p->d_wcol);
   cudaFree(p->d_tw); cudaFree(p->d_scratch); cudaFree(p->d_vkey); cudaFree(p->d_vseg); cudaFree(p->d_vlen); cudaFree(p->d_vw); cudaFree(p->d_vcol); cudaFree(p->d_vrec); cudaFree(p->d_corr); cudaFree(p->d_tw32);
   cudaFree(p->d_tcref); cudaFree(p->d_cmat);
+  res_route_free(p);
   cudaFree(p->d_hrec); cudaFree(p->d_hw); cudaFree(p->d_pha); cudaFree(p->d_tw_sub); cudaFree(p->d_rplace);
   for (int c = 0; c < 2; ++c) {
     cudaFree(p->fl[c].d_tab); cudaFree(p->fl[c].d_size); cudaFree(p->rl[c].d_tab); cudaFree(p->rl[c].d_size);
@@ -263,7 +264,7 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
     if (opts->struct_size != (int32_t)sizeof(blink_options)) return BLINK_EINVAL;
     opt = *opts;
     auto route_ok = [](int32_t v) { return v == 0 || v == -1; };
-    if (!route_ok(opt.fused_route) || !route_ok(opt.polyphase) || !route_ok(opt.warp_route) || !route_ok(opt.grid_ring) ||
+    if (!route_ok(opt.fused_route) || !route_ok(opt.polyphase) || !(route_ok(opt.warp_route) || opt.warp_route == 2) || !route_ok(opt.grid_ring) ||
         opt.warp_ring < 0 || opt.warp_ring == 1 || opt.grid_ring_min_snap < 0 || opt.image_chunk_mb < 0)
       return BLINK_EINVAL;
   }
@@ -546,7 +547,8 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
     step(cudaMemcpyAsync(p->d_vcol, h_vcol.data(), sizeof(int32_t) * h_vcol.size(), cudaMemcpyHostToDevice, st));
     step(cudaStreamSynchronize(st));
     PLAN_CUDA(ce, "vis-route table upload");
-    p->warp_route = (p->opt.warp_route != -1 && warp_route_applies(p)) ? 1 : 0;
+    PLAN_TRY(res_route_build(p, st));
+    p->warp_route = (!p->res_route && p->opt.warp_route != -1 && warp_route_applies(p)) ? 1 : 0;
   }
   PLAN_TRY(fused_build(p, st));
   PLAN_TRY(fused_tc_build(p, st));
@@ -682,7 +684,8 @@ extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *
     case BLINK_Q_IMAGE_PATH: *(int32_t *)out = p->image_path; break;
     case BLINK_Q_SCRATCH_BYTES: *(int64_t *)out = (int64_t)p->scratch_bytes; break;
     case BLINK_Q_IMAGE_CHUNK: *(int32_t *)out = p->chunk_snapshots; break;
-    case BLINK_Q_FUSED_PATH: *(int32_t *)out = fused_smem_route(p) ? 1 : (p->warp_route ? 2 : 0); break;
+    case BLINK_Q_FUSED_PATH: *(int32_t *)out = fused_smem_route(p) ? 1 : ((p->warp_route || p->res_route) ? 2 : 0); break;
+    case BLINK_Q_WARP_KERNEL: *(int32_t *)out = p->res_route ? 2 : (p->warp_route ? 1 : 0); break;
     case BLINK_Q_FUSED_CHUNK: *(int32_t *)out = p->fused_chunk; break;
     case BLINK_Q_CORR: *(const void **)out = p->d_corr; break;
     case BLINK_Q_CORR_FUSED: *(int32_t *)out = p->corr_on; break;
