@@ -12,10 +12,14 @@
 // shared memory, where the row pass (two real image rows per 1024-point complex transform, one warp per
 // transform, wfft.cuh's 32 x 32 split) picks it up.  So per unit a CTA of 16 warps runs
 //
-//   S  bins:    warp w owns the 32 columns {32 ((w + b) mod 16) + b}; its lanes take the columns' non-empty
-//               bins ("entries", longest first, their cells laid out rank-major so lanes read consecutive
-//               slots) and store sum_j G_j w32^(a_j r) * w1024^(c r) into the tile; empty bins are never
-//               written: the plan's per-column bin mask says which to read.
+//   S  bins:    warp w owns the 32 columns {32 ((w + b) mod 16) + b}.  The columns' non-empty bins
+//               ("entries") are dealt to its lanes by the plan so that every lane has the same number of
+//               cells (longest entry first to the least loaded lane); a lane walks its own list, cell q of
+//               lane l at position 32 q + l (consecutive lanes read consecutive slots), adds
+//               G_j w32^(a_j r) and, at the last cell of an entry, stores the sum times w1024^(c r) into the
+//               tile.  Empty bins are never written: the plan's per-column bin mask says which to read.
+//               The image stores of the PREVIOUS unit (64 per lane, still in registers) are issued four
+//               per step inside this loop, so they do not arrive at the memory pipe as one burst.
 //   A  columns: lane = column; masked loads of its bins, dft32 in registers, and in place of the bins the
 //               row-pass operands Z = U[y] + i U[y + 512] (rows p) and conj U[y] + i conj U[y + 512]
 //               (rows 16 + p, the mirrored half kx < 0).  A column's 32 slots are private to its lane, so
@@ -48,22 +52,21 @@ constexpr int kRN = 1024;
 constexpr int kRW = 512;                        // columns of the tile (kx = 0 .. 511)
 constexpr int kRWarps = 16;
 constexpr int kRThreads = 32 * kRWarps;
-constexpr int kRHdr = 20;                       // ints per (channel, warp) header: cell base, entry base, E, nrank, n_1 .. n_15
-constexpr int kRHdrRows = kRWarps + 1;          // + one row {ncell, nent}
-constexpr int kRMaxRank = 16;                   // most cells in one bin
+constexpr int kRHdr = 4;                        // ints per (channel, warp) header: first position, first entry slot, steps, -
+constexpr int kRHdrRows = kRWarps + 1;          // + one row {positions, entry slots}
 constexpr size_t kROffTw = sizeof(cf32) * 32 * kRW;                 // tile first
 constexpr size_t kROffW32 = kROffTw + sizeof(cf32) * 1024;
 constexpr size_t kROffHdr = kROffW32 + sizeof(cf32) * 32;
 constexpr size_t kROffBar = kROffHdr + sizeof(int32_t) * kRHdrRows * kRHdr;
 constexpr size_t kROffCv = (kROffBar + 16 + 15) / 16 * 16;
-constexpr size_t kRBytesPerCell = sizeof(cf32) + sizeof(uint16_t) + sizeof(uint8_t);
+constexpr size_t kRBytesPerPos = sizeof(cf32) + sizeof(uint8_t);     // + 2 bytes per entry slot
 
 struct RParams {
   ImgParams ip;
-  int n_snap, cap;
-  const uint4 *rrec;        // [n_ch][cap] iy | flag << 10 | kx << 12 | len << 21, weight, source 0, source 1 / segment
-  const uint8_t *rca;       // [n_ch][cap] iy >> 5 of the cell at this position
-  const uint16_t *res;      // [n_ch][cap] tile slot c * 512 + kx of the entry
+  int n_snap, cap, ecap;
+  const uint4 *rrec;        // [n_ch][cap] iy | flag << 10 | kx << 12 | len << 21, weight, source 0, source 1 / segment (len 0 = padding)
+  const uint8_t *rca;       // [n_ch][cap] iy >> 5 of the cell at this position | 32 if it is the last of its entry
+  const uint16_t *res;      // [n_ch][ecap] tile slot c * 512 + kx of a lane's n-th entry at [32 n + lane] behind the warp's base
   const int32_t *rhdr;      // [n_ch][17][kRHdr]
   const uint32_t *rmask;    // [n_ch][512] non-empty bins of the column
   const float2 *uvsrc;      // blink_image: cell values from this uv grid; NULL = from the visibilities
@@ -91,7 +94,16 @@ __device__ __forceinline__ cf32 cell_from_vis(const uint4 r, const float2 v0, co
   return mk((ar + ar) * w, 0.f);
 }
 
-__global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
+// the image stores of one unit: t[n2] of lane n1 is pixel x = n1 + 32 n2 of rows y (real part) and y + 512 (imaginary part)
+struct ROut { float *r0, *r1; };
+template <int I> __device__ __forceinline__ void store4(const ROut &o, const cf32 *t) {      // stores 4 I .. 4 I + 3 of 64
+  __stcs(o.r0 + 32 * (2 * I), t[2 * I].x);
+  __stcs(o.r1 + 32 * (2 * I), t[2 * I].y);
+  __stcs(o.r0 + 32 * (2 * I + 1), t[2 * I + 1].x);
+  __stcs(o.r1 + 32 * (2 * I + 1), t[2 * I + 1].y);
+}
+
+template <bool DEFER> __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
   constexpr int N = kRN;
   const ImgParams &p = q.ip;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -100,9 +112,9 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
   cf32 *w32 = reinterpret_cast<cf32 *>(smem_raw + kROffW32);          // exp(2 pi i k / 32)
   int32_t *hdr = reinterpret_cast<int32_t *>(smem_raw + kROffHdr);
   uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + kROffBar); // [0] columns done, [1] exchange tiles free
-  cf32 *cv = reinterpret_cast<cf32 *>(smem_raw + kROffCv);            // cell values of the snapshot
-  uint16_t *es = reinterpret_cast<uint16_t *>(cv + q.cap);            // entry -> tile slot
-  uint8_t *ca = reinterpret_cast<uint8_t *>(es + q.cap);              // cell -> iy >> 5
+  cf32 *cv = reinterpret_cast<cf32 *>(smem_raw + kROffCv);            // cell values of the snapshot, by position
+  uint16_t *es = reinterpret_cast<uint16_t *>(cv + q.cap);            // entry slots -> tile slot
+  uint8_t *ca = reinterpret_cast<uint8_t *>(es + q.ecap);             // position -> iy >> 5 | last << 5
   const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
 
   for (int i = tid; i < 1024; i += kRThreads) twB[i] = __ldg(p.tw32 + i);
@@ -116,60 +128,69 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
   const int kcol = 32 * ((wv + lane) & 15) + lane;       // this lane's column in phases S / A
   uint32_t ph_a = 0, ph_b = 0, cmask = 0;
   int s_cur = -1;
+  cf32 t[32];
+  ROut out = {nullptr, nullptr};           // rows of the unit whose pixels are still in t[] (NULL: none)
   for (long long u = u0; u < u1; ++u) {
     const int s = (int)(u >> 5), r = (int)(u & 31);
     if (s != s_cur) {
       // ---------------------------------------------------------------- G: the snapshot's cell values
       // (every warp is past the columns barrier of the previous unit, so nobody reads the old ones)
+      if (out.r0 != nullptr) {
+#pragma unroll
+        for (int n2 = 0; n2 < 32; ++n2) {
+          __stcs(out.r0 + 32 * n2, t[n2].x);
+          __stcs(out.r1 + 32 * n2, t[n2].y);
+        }
+        out.r0 = nullptr;
+      }
       s_cur = s;
       const int ch = (s + p.ch0) % p.n_ch;
       const int32_t *gh = q.rhdr + (size_t)ch * kRHdrRows * kRHdr;
       for (int i = tid; i < kRHdrRows * kRHdr; i += kRThreads) hdr[i] = __ldg(gh + i);
       cmask = __ldg(q.rmask + (size_t)ch * kRW + kcol);
-      const int ncell = __ldg(gh + kRWarps * kRHdr), nent = __ldg(gh + kRWarps * kRHdr + 1);
+      const int npos = __ldg(gh + kRWarps * kRHdr), nes = __ldg(gh + kRWarps * kRHdr + 1);
       {
-        const uint4 *ge = reinterpret_cast<const uint4 *>(q.res + (size_t)ch * q.cap);
-        for (int i = tid; i < (nent + 7) / 8; i += kRThreads) reinterpret_cast<uint4 *>(es)[i] = __ldg(ge + i);
+        const uint4 *ge = reinterpret_cast<const uint4 *>(q.res + (size_t)ch * q.ecap);
+        for (int i = tid; i < (nes + 7) / 8; i += kRThreads) reinterpret_cast<uint4 *>(es)[i] = __ldg(ge + i);
         const uint4 *ga = reinterpret_cast<const uint4 *>(q.rca + (size_t)ch * q.cap);
-        for (int i = tid; i < (ncell + 15) / 16; i += kRThreads) reinterpret_cast<uint4 *>(ca)[i] = __ldg(ga + i);
+        for (int i = tid; i < (npos + 15) / 16; i += kRThreads) reinterpret_cast<uint4 *>(ca)[i] = __ldg(ga + i);
       }
       const uint4 *__restrict__ rec = q.rrec + (size_t)ch * q.cap;
       if (q.uvsrc != nullptr) {
         // blink_image: the plan's occupied cells with kx >= 0 straight from the uv grid (empty cells are
         // zero by contract and never read)
         const float2 *__restrict__ g = q.uvsrc + (size_t)(p.snap_base + s) * N * N;
-        for (int i = tid; i < ncell; i += kRThreads) {
+        for (int i = tid; i < npos; i += kRThreads) {
           const uint4 rr = __ldg(rec + i);
           const int iy = (int)(rr.x & 1023), flag = (rr.x >> 10) & 3, kx = (rr.x >> 12) & 511;
           const float w = __uint_as_float(rr.y);
-          const float2 v = __ldg(g + (size_t)iy * N + kx);
+          float2 v = make_float2(0.f, 0.f);
+          if (rr.x >> 21) v = __ldg(g + (size_t)iy * N + kx);
           cv[i] = mk(v.x * w, (flag == kPlaceDirect || flag == kPlaceConj) ? v.y * w : 0.f);
         }
       } else {
         const float2 *__restrict__ vis = p.vis + (size_t)(p.snap_base + s) * p.n_bl;
         const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
         const float2 *__restrict__ cf = p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr;
-        for (int i0 = tid; i0 < ncell; i0 += 4 * kRThreads) {       // four cells per thread in flight
-          uint4 rr[4];
-          float2 v0[4], v1[4];
+        for (int i0 = tid; i0 < npos; i0 += 8 * kRThreads) {       // eight cells per thread in flight
+          uint4 rr[8];
+          float2 v0[8], v1[8];
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
+          for (int j = 0; j < 8; ++j) {
             const int i = i0 + j * kRThreads;
-            rr[j] = i < ncell ? __ldg(rec + i) : make_uint4(0, 0, 0, 0);
+            rr[j] = i < npos ? __ldg(rec + i) : make_uint4(0, 0, 0, 0);
           }
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int i = i0 + j * kRThreads;
+          for (int j = 0; j < 8; ++j) {
+            const int len = (int)(rr[j].x >> 21);
             v0[j] = v1[j] = make_float2(0.f, 0.f);
-            if (i < ncell) {
-              v0[j] = ld_vis(vis, cf, rr[j].z >> 1);
-              if ((rr[j].x >> 21) == 2) v1[j] = ld_vis(vis, cf, rr[j].w >> 1);
-            }
+            if (len >= 1) v0[j] = ld_vis(vis, cf, rr[j].z >> 1);
+            if (len == 2) v1[j] = ld_vis(vis, cf, rr[j].w >> 1);
           }
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
+          for (int j = 0; j < 8; ++j) {
             const int i = i0 + j * kRThreads;
-            if (i < ncell) cv[i] = cell_from_vis(rr[j], v0[j], v1[j], vis, cf, src);
+            if (i < npos) cv[i] = (rr[j].x >> 21) ? cell_from_vis(rr[j], v0[j], v1[j], vis, cf, src) : mk(0.f, 0.f);
           }
         }
       }
@@ -179,27 +200,37 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
       mbar_wait(bars + 1, ph_b);
       ph_b ^= 1u;
     }
-    cf32 t[32];
     {
       // -------------------------------------------------------------- S: the bins of this warp's columns
       const int32_t *h = hdr + wv * kRHdr;
-      const int cbase = h[0], ebase = h[1], E = h[2], nrank = h[3];
+      const int L = h[2];
+      const cf32 *cvp = cv + h[0] + lane;
+      const uint8_t *cap_ = ca + h[0] + lane;
+      const uint16_t *esp = es + h[1] + lane;
       const cf32 *twr = twB + r * 32;                                 // w1024^(c r), c = 0 .. 31
-      for (int e = lane; e < E; e += 32) {
-        int qi = cbase + e;
-        cf32 acc = cmul(cv[qi], w32[((int)ca[qi] * r) & 31]);
-        int off = E;
-        for (int i = 1; i < nrank; ++i) {
-          const int ni = h[3 + i];
-          if (e >= ni) break;
-          qi = cbase + off + e;
-          const cf32 x = cmul(cv[qi], w32[((int)ca[qi] * r) & 31]);
-          acc = mk(acc.x + x.x, acc.y + x.y);
-          off += ni;
+      cf32 acc = mk(0.f, 0.f);
+      auto step = [&](int qq) {
+        const cf32 v = cvp[32 * qq];
+        const int m = cap_[32 * qq];
+        const cf32 w = w32[((m & 31) * r) & 31];
+        acc.x = fmaf(v.x, w.x, fmaf(-v.y, w.y, acc.x));
+        acc.y = fmaf(v.x, w.y, fmaf(v.y, w.x, acc.y));
+        if (m & 32) {                                                  // last cell of an entry
+          const int slot = *esp;
+          esp += 32;
+          Z[slot] = cmul(acc, twr[slot >> 9]);
+          acc = mk(0.f, 0.f);
         }
-        const int slot = es[ebase + e];
-        Z[slot] = cmul(acc, twr[slot >> 9]);
-      }
+      };
+      const bool have = DEFER && out.r0 != nullptr;
+      // sixteen steps with the 64 stores of the previous unit spread among them, then the rest
+#define BLINK_R_STEP(I)             \
+  if (I < L) step(I);               \
+  if (have) store4<I>(out, t);
+      BLINK_R_STEP(0) BLINK_R_STEP(1) BLINK_R_STEP(2) BLINK_R_STEP(3) BLINK_R_STEP(4) BLINK_R_STEP(5) BLINK_R_STEP(6) BLINK_R_STEP(7)
+      BLINK_R_STEP(8) BLINK_R_STEP(9) BLINK_R_STEP(10) BLINK_R_STEP(11) BLINK_R_STEP(12) BLINK_R_STEP(13) BLINK_R_STEP(14) BLINK_R_STEP(15)
+#undef BLINK_R_STEP
+      for (int qq = 16; qq < L; ++qq) step(qq);
       __syncwarp();
       // -------------------------------------------------------------- A: this lane's column, in place
       cf32 *zc = Z + kcol;
@@ -248,23 +279,40 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
       __syncwarp();
       if (lane == 0) mbar_arrive(bars + 1);
       dft32(t);
-      float *__restrict__ r0 = p.img + ((size_t)(p.snap_base + s) * N + 32 * wv + r) * N + lane;
-      float *__restrict__ r1 = r0 + (size_t)(N / 2) * N;
+      // the pixels stay in t[]: they are stored during phase S of the next unit (or below, after the last)
+      out.r0 = p.img + ((size_t)(p.snap_base + s) * N + 32 * wv + r) * N + lane;
+      out.r1 = out.r0 + (size_t)(N / 2) * N;
+      if constexpr (!DEFER) {
 #pragma unroll
-      for (int n2 = 0; n2 < 32; ++n2) {
-        __stcs(r0 + 32 * n2, t[n2].x);
-        __stcs(r1 + 32 * n2, t[n2].y);
+        for (int n2 = 0; n2 < 32; ++n2) {
+          __stcs(out.r0 + 32 * n2, t[n2].x);
+          __stcs(out.r1 + 32 * n2, t[n2].y);
+        }
+        out.r0 = nullptr;
       }
+    }
+  }
+  if (out.r0 != nullptr) {
+#pragma unroll
+    for (int n2 = 0; n2 < 32; ++n2) {
+      __stcs(out.r0 + 32 * n2, t[n2].x);
+      __stcs(out.r1 + 32 * n2, t[n2].y);
     }
   }
 }
 
 // ---- plan side ----------------------------------------------------------------------------------------
 struct RCell { int k, iy, seg, len, flag; float w; };
+struct RTables {
+  std::vector<uint4> rec;
+  std::vector<uint8_t> ca;
+  std::vector<uint16_t> es;
+  std::vector<int32_t> hdr;
+  std::vector<uint32_t> mask;
+};
 
-// the tables of one channel; false when a bin holds more than kRMaxRank cells
-static bool res_tables(const HostGather &g, int N, int weighting, float inv_norm, std::vector<uint4> &rec, std::vector<uint8_t> &ca,
-                       std::vector<uint16_t> &es, std::vector<int32_t> &hdr, std::vector<uint32_t> &mask) {
+// the tables of one channel
+static void res_tables(const HostGather &g, int N, int weighting, float inv_norm, RTables &o) {
   std::vector<RCell> cells;
   for (int j = 0; j < g.n_can; ++j) {
     const int c = g.can_cell[j], ix = c % N, iy = c / N;
@@ -276,48 +324,61 @@ static bool res_tables(const HostGather &g, int N, int weighting, float inv_norm
     if (kx >= 0) cells.push_back({kx, iy, g.seg_start[j], len, c == 0 ? kPlaceBoth : kPlaceDirect, w});
     if (kx <= 0 && c != 0) cells.push_back({-kx, (N - iy) % N, g.seg_start[j], len, kPlaceConj, w});
   }
-  // entries (column, bin) per owning warp
-  std::vector<std::map<int, std::vector<int>>> ent(kRWarps);   // slot -> cells, ascending iy
+  // entries (column, bin) per owning warp; the cells of an entry in ascending iy
+  std::vector<std::map<int, std::vector<int>>> ent(kRWarps);
   std::sort(cells.begin(), cells.end(), [](const RCell &a, const RCell &b) { return a.k != b.k ? a.k < b.k : a.iy < b.iy; });
-  mask.assign(kRW, 0u);
+  o.mask.assign(kRW, 0u);
   for (int i = 0; i < (int)cells.size(); ++i) {
     const int k = cells[i].k, c = cells[i].iy & 31;
-    const int w = ((k >> 5) - (k & 31)) & 15;
-    ent[w][c * kRW + k].push_back(i);
-    mask[k] |= 1u << c;
+    ent[((k >> 5) - (k & 31)) & 15][c * kRW + k].push_back(i);
+    o.mask[k] |= 1u << c;
   }
-  hdr.assign((size_t)kRHdrRows * kRHdr, 0);
-  rec.clear(); ca.clear(); es.clear();
+  o.hdr.assign((size_t)kRHdrRows * kRHdr, 0);
+  o.rec.clear(); o.ca.clear(); o.es.clear();
   for (int w = 0; w < kRWarps; ++w) {
+    // longest entry first to the lane with the fewest cells so far (ties: fewest entries, lowest lane)
     std::vector<std::pair<int, int>> order;      // (-len, slot)
     for (auto &kv : ent[w]) order.push_back({-(int)kv.second.size(), kv.first});
     std::sort(order.begin(), order.end());
-    const int E = (int)order.size(), nrank = E ? -order[0].first : 0;
-    if (nrank > kRMaxRank) return false;
-    int32_t *h = hdr.data() + (size_t)w * kRHdr;
-    h[0] = (int32_t)rec.size(); h[1] = (int32_t)es.size(); h[2] = E; h[3] = nrank;
-    for (auto &o : order) es.push_back((uint16_t)o.second);
-    for (int i = 0; i < nrank; ++i) {
-      int ni = 0;
-      for (auto &o : order) {
-        if (-o.first <= i) break;
-        const RCell &cl = cells[ent[w][o.second][i]];
-        uint32_t wbits;
-        memcpy(&wbits, &cl.w, 4);
-        rec.push_back(make_uint4((uint32_t)cl.iy | ((uint32_t)cl.flag << 10) | ((uint32_t)cl.k << 12) | ((uint32_t)cl.len << 21), wbits,
-                                 (uint32_t)g.src[cl.seg], cl.len == 2 ? (uint32_t)g.src[cl.seg + 1] : (uint32_t)cl.seg));
-        ca.push_back((uint8_t)(cl.iy >> 5));
-        ++ni;
+    std::vector<std::vector<int>> mine(32);      // slots of each lane's entries, in the order it walks them
+    int load[32] = {0};
+    for (auto &od : order) {
+      int best = 0;
+      for (int l = 1; l < 32; ++l)
+        if (load[l] < load[best] || (load[l] == load[best] && mine[l].size() < mine[best].size())) best = l;
+      mine[best].push_back(od.second);
+      load[best] += -od.first;
+    }
+    int L = 0, EL = 0;
+    for (int l = 0; l < 32; ++l) { L = std::max(L, load[l]); EL = std::max(EL, (int)mine[l].size()); }
+    int32_t *h = o.hdr.data() + (size_t)w * kRHdr;
+    h[0] = (int32_t)o.rec.size(); h[1] = (int32_t)o.es.size(); h[2] = L; h[3] = EL;
+    const size_t r0 = o.rec.size(), e0 = o.es.size();
+    o.rec.resize(r0 + (size_t)32 * L, make_uint4(0, 0, 0, 0));
+    o.ca.resize(r0 + (size_t)32 * L, 0);
+    o.es.resize(e0 + (size_t)32 * EL, 0);
+    for (int l = 0; l < 32; ++l) {
+      int qpos = 0;
+      for (size_t n = 0; n < mine[l].size(); ++n) {
+        const std::vector<int> &cl = ent[w][mine[l][n]];
+        o.es[e0 + 32 * n + l] = (uint16_t)mine[l][n];
+        for (size_t i = 0; i < cl.size(); ++i, ++qpos) {
+          const RCell &c = cells[cl[i]];
+          uint32_t wbits;
+          memcpy(&wbits, &c.w, 4);
+          o.rec[r0 + 32 * (size_t)qpos + l] =
+              make_uint4((uint32_t)c.iy | ((uint32_t)c.flag << 10) | ((uint32_t)c.k << 12) | ((uint32_t)c.len << 21), wbits,
+                         (uint32_t)g.src[c.seg], c.len == 2 ? (uint32_t)g.src[c.seg + 1] : (uint32_t)c.seg);
+          o.ca[r0 + 32 * (size_t)qpos + l] = (uint8_t)((c.iy >> 5) | (i + 1 == cl.size() ? 32 : 0));
+        }
       }
-      if (i >= 1) h[3 + i] = ni;
     }
   }
-  hdr[(size_t)kRWarps * kRHdr] = (int32_t)rec.size();
-  hdr[(size_t)kRWarps * kRHdr + 1] = (int32_t)es.size();
-  return true;
+  o.hdr[(size_t)kRWarps * kRHdr] = (int32_t)o.rec.size();
+  o.hdr[(size_t)kRWarps * kRHdr + 1] = (int32_t)o.es.size();
 }
 
-static size_t res_smem(int cap) { return kROffCv + (size_t)cap * kRBytesPerCell; }
+static size_t res_smem(int cap, int ecap) { return kROffCv + (size_t)cap * kRBytesPerPos + (size_t)ecap * sizeof(uint16_t); }
 
 void res_route_free(blink_plan *p) {
   cudaFree(p->d_rrec); cudaFree(p->d_rca); cudaFree(p->d_res); cudaFree(p->d_rhdr); cudaFree(p->d_rmask);
@@ -326,39 +387,31 @@ void res_route_free(blink_plan *p) {
 }
 
 // Residue-class route of blink_grid_image / blink_image at N = 1024: applies when every channel's occupied
-// half-plane cells (8 + 2 + 1 bytes each) fit in shared memory beside the 128 KB tile.
+// half-plane cells (9 bytes per position, 2 per entry slot) fit in shared memory beside the 128 KB tile.
 int res_route_build(blink_plan *p, cudaStream_t st) {
   p->res_route = 0;
   if (p->n_pix != kRN || p->opt.warp_route == -1 || p->opt.warp_route == 2) return BLINK_OK;
-  if (p->wu > kRW || p->seg_len_max > 2047 || p->max_smem_optin <= 0 || (size_t)p->max_smem_optin <= kROffCv) return BLINK_OK;
-  const int cap_max = (int)(((size_t)p->max_smem_optin - kROffCv) / kRBytesPerCell) / 16 * 16;
+  if (p->wu > kRW || p->seg_len_max > 2047 || p->max_smem_optin <= 0) return BLINK_OK;
   const int n_ch = p->n_ch;
-  std::vector<std::vector<uint4>> rec(n_ch);
-  std::vector<std::vector<uint8_t>> ca(n_ch);
-  std::vector<std::vector<uint16_t>> es(n_ch);
-  std::vector<std::vector<int32_t>> hdr(n_ch);
-  std::vector<std::vector<uint32_t>> mask(n_ch);
-  std::vector<int> ok(n_ch, 0);
-  parallel_for(n_ch, [&](int ch) {
-    ok[ch] = res_tables(p->gathers[ch], p->n_pix, p->weighting, p->chinfo[ch].inv_norm, rec[ch], ca[ch], es[ch], hdr[ch], mask[ch]) ? 1 : 0;
-  });
-  int cap = 16;
+  std::vector<RTables> tb(n_ch);
+  parallel_for(n_ch, [&](int ch) { res_tables(p->gathers[ch], p->n_pix, p->weighting, p->chinfo[ch].inv_norm, tb[ch]); });
+  int cap = 16, ecap = 16;
   for (int ch = 0; ch < n_ch; ++ch) {
-    if (!ok[ch]) return BLINK_OK;
-    cap = std::max(cap, ((int)rec[ch].size() + 15) / 16 * 16);
+    cap = std::max(cap, ((int)tb[ch].rec.size() + 15) / 16 * 16);
+    ecap = std::max(ecap, ((int)tb[ch].es.size() + 15) / 16 * 16);
   }
-  if (cap > cap_max) return BLINK_OK;
+  if (ecap > 0xFFFF || res_smem(cap, ecap) > (size_t)p->max_smem_optin) return BLINK_OK;
   std::vector<uint4> h_rec((size_t)n_ch * cap, make_uint4(0, 0, 0, 0));
   std::vector<uint8_t> h_ca((size_t)n_ch * cap, 0);
-  std::vector<uint16_t> h_es((size_t)n_ch * cap, 0);
+  std::vector<uint16_t> h_es((size_t)n_ch * ecap, 0);
   std::vector<int32_t> h_hdr((size_t)n_ch * kRHdrRows * kRHdr, 0);
   std::vector<uint32_t> h_mask((size_t)n_ch * kRW, 0u);
   for (int ch = 0; ch < n_ch; ++ch) {
-    std::copy(rec[ch].begin(), rec[ch].end(), h_rec.begin() + (size_t)ch * cap);
-    std::copy(ca[ch].begin(), ca[ch].end(), h_ca.begin() + (size_t)ch * cap);
-    std::copy(es[ch].begin(), es[ch].end(), h_es.begin() + (size_t)ch * cap);
-    std::copy(hdr[ch].begin(), hdr[ch].end(), h_hdr.begin() + (size_t)ch * kRHdrRows * kRHdr);
-    std::copy(mask[ch].begin(), mask[ch].end(), h_mask.begin() + (size_t)ch * kRW);
+    std::copy(tb[ch].rec.begin(), tb[ch].rec.end(), h_rec.begin() + (size_t)ch * cap);
+    std::copy(tb[ch].ca.begin(), tb[ch].ca.end(), h_ca.begin() + (size_t)ch * cap);
+    std::copy(tb[ch].es.begin(), tb[ch].es.end(), h_es.begin() + (size_t)ch * ecap);
+    std::copy(tb[ch].hdr.begin(), tb[ch].hdr.end(), h_hdr.begin() + (size_t)ch * kRHdrRows * kRHdr);
+    std::copy(tb[ch].mask.begin(), tb[ch].mask.end(), h_mask.begin() + (size_t)ch * kRW);
   }
   int rc;
   if ((rc = upload_table((void **)&p->d_rrec, h_rec.data(), sizeof(uint4) * h_rec.size(), st, "residue route records")) != BLINK_OK) return rc;
@@ -368,6 +421,7 @@ int res_route_build(blink_plan *p, cudaStream_t st) {
   if ((rc = upload_table((void **)&p->d_rmask, h_mask.data(), sizeof(uint32_t) * h_mask.size(), st, "residue route masks")) != BLINK_OK) return rc;
   BLINK_CUDA_TRY(cudaStreamSynchronize(st), "residue route upload");
   p->res_cap = cap;
+  p->res_ecap = ecap;
   p->res_route = 1;
   return BLINK_OK;
 }
@@ -377,18 +431,23 @@ int launch_img1024r(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t 
   RParams q;
   q.n_snap = n_snap;
   q.cap = p->res_cap;
+  q.ecap = p->res_ecap;
   q.rrec = p->d_rrec; q.rca = p->d_rca; q.res = p->d_res; q.rhdr = p->d_rhdr; q.rmask = p->d_rmask;
   q.uvsrc = ip.vis == nullptr ? ip.uv : nullptr;
   ip.snap_base = 0;
   q.ip = ip;
-  const size_t smem = res_smem(p->res_cap);
+  const size_t smem = res_smem(p->res_cap, p->res_ecap);
   static std::atomic<uint64_t> attr{0};
-  const int rc = ensure_max_smem(k_img1024r, p, attr, "k_img1024r smem attribute");
+  static std::atomic<uint64_t> attr1{0};
+  const bool defer = p->opt.tune[kTuneWarpCtasPerSm] == 2;
+  const int rc = defer ? ensure_max_smem(k_img1024r<true>, p, attr, "k_img1024r smem attribute")
+                       : ensure_max_smem(k_img1024r<false>, p, attr1, "k_img1024r smem attribute");
   if (rc != BLINK_OK) return rc;
   // one CTA per SM; fewer when there are fewer units than that
   const long long units = (long long)n_snap * 32;
   const int grid = (int)std::min<long long>(p->sm_count, units);
-  k_img1024r<<<grid, kRThreads, smem, st>>>(q);
+  if (defer) k_img1024r<true><<<grid, kRThreads, smem, st>>>(q);
+  else k_img1024r<false><<<grid, kRThreads, smem, st>>>(q);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_img1024r launch");
   return BLINK_OK;
 }
