@@ -155,11 +155,10 @@ struct blink_plan {
   long long warp_snap_cap = 0;      // snapshots per call the warp route's counters in scratch are sized for
   // residue-class route at N = 1024 (blink_image_r.cu): the intermediate stays in shared memory, no scratch
   int res_route = 0;                // 1 = blink_grid_image / blink_image take k_img1024r
-  int res_cap = 0, res_ecap = 0;    // padded positions / entry slots per channel of its tables
-  uint4 *d_rrec = nullptr;          // [n_ch][res_cap] cell records in the kernel's per-warp, rank-major order
-  uint8_t *d_rca = nullptr;         // [n_ch][res_cap] iy >> 5 per cell
-  uint16_t *d_res = nullptr;        // [n_ch][res_cap] tile slot per entry (column, iy mod 32)
-  int32_t *d_rhdr = nullptr;        // [n_ch][17][20] per-warp headers
+  int res_cap = 0;                  // positions per channel of its tables
+  uint4 *d_rrec = nullptr;          // [n_ch][res_cap] cell records, lane-interleaved lists per producer warp
+  uint32_t *d_rmeta = nullptr;      // [n_ch][res_cap] cell descriptors (iy, last-of-entry, tile slot)
+  int32_t *d_rhdr = nullptr;        // [n_ch][8][2] per-warp headers
   uint32_t *d_rmask = nullptr;      // [n_ch][512] non-empty bins per column
   // blink_grid, ring route (see grid_ring_build in blink_grid.cu): phase S as in k_fused
   int ring_path = 0;                // 1 = k_grid_ring available
