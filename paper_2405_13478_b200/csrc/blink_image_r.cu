@@ -55,10 +55,11 @@ constexpr int kRN = 1024;
 constexpr int kRW = 512;                        // columns of a tile (kx = 0 .. 511)
 constexpr int kRRows = 16;                      // rows of a tile = image rows per unit
 constexpr int kRUnits = kRN / kRRows;           // units (residue classes) per snapshot
-constexpr int kRProd = 8, kRCons = 8;           // producer / consumer warps
+constexpr int kRProd = 16, kRCons = 8;          // producer / consumer warps
 constexpr int kRThreads = 32 * (kRProd + kRCons);
-constexpr int kRLmax = 32;                      // most cells in a lane's list (descriptors live in registers)
-constexpr int kRHdr = 2;                        // ints per (channel, producer warp) header: first position, steps (multiple of 8)
+constexpr int kRLmax = 16;                      // most cells in a lane's list (descriptors live in registers)
+constexpr int kRHdr = 2;                        // ints per (channel, producer warp) header: first position, steps (multiple of 4)
+constexpr int kRRegsProd = 64, kRRegsCons = 112;// registers per thread after the role split: 16 x 32 x 64 + 8 x 32 x 112 = 768 x 80, the launch allocation
 constexpr size_t kRTile = sizeof(cf32) * kRRows * kRW;
 constexpr size_t kROffTw = 2 * kRTile;                              // the two tiles first
 constexpr size_t kROffNat = kROffTw + sizeof(cf32) * 1024;
@@ -69,7 +70,7 @@ struct RParams {
   ImgParams ip;
   int n_snap, cap;
   const uint4 *rrec;        // [n_ch][cap] iy | flag << 10 | kx << 12 | len << 21, weight, source 0, source 1 / segment (len 0 = padding)
-  const uint32_t *rmeta;    // [n_ch][cap] 8 iy | last-of-entry << 13 | tile slot (c * 512 + kx) << 14 (0 = padding)
+  const uint32_t *rmeta;    // [n_ch][cap] 8 iy | last-of-entry << 13 | 8 (tile slot c * 512 + kx) << 16 (0 = padding)
   const int32_t *rhdr;      // [n_ch][kRProd][kRHdr]
   const uint32_t *rmask;    // [n_ch][512] non-empty bins of the column (16 bits)
   const float2 *uvsrc;      // blink_image: cell values from this uv grid; NULL = from the visibilities
@@ -97,26 +98,27 @@ __device__ __forceinline__ cf32 cell_from_vis(const uint4 r, const float2 v0, co
   return mk((ar + ar) * w, 0.f);
 }
 
-// steps Q0 .. Q0 + 7 of a lane's list: acc += G w1024^(iy r); an entry's last cell stores the sum.
-// Loads first (values, then twiddles), then the chain, so the shared-memory latencies overlap.
+// steps Q0 .. Q0 + 3 of a lane's list: acc += G w1024^(iy r); an entry's last cell stores the sum.
+// Loads first (values, then twiddles), then the chain, so the shared-memory latencies overlap.  The
+// descriptor times r needs no masking first: its high fields only reach bits the table index drops.
 template <int Q0>
-__device__ __forceinline__ void bins8(const uint32_t (&meta)[kRLmax], const cf32 *__restrict__ cvp, const unsigned char *__restrict__ nat,
-                                      cf32 *__restrict__ zb, int r, cf32 &acc) {
-  cf32 v[8], w[8];
+__device__ __forceinline__ void bins4(const uint32_t (&meta)[kRLmax], const cf32 *__restrict__ cvp, const unsigned char *__restrict__ nat,
+                                      unsigned char *__restrict__ zb, int r, cf32 &acc) {
+  cf32 v[4], w[4];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) v[j] = cvp[32 * (Q0 + j)];
+  for (int j = 0; j < 4; ++j) v[j] = cvp[32 * (Q0 + j)];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) {
-    const uint32_t P = (meta[Q0 + j] & 0x1FFFu) * (uint32_t)r;        // 8 iy r
+  for (int j = 0; j < 4; ++j) {
+    const uint32_t P = meta[Q0 + j] * (uint32_t)r;                    // bits 3 .. 12: 8 (iy r mod 1024)
     w[j] = *reinterpret_cast<const cf32 *>(nat + ((P & 0x1FF8u) ^ ((P >> 4) & 0x78u)));
   }
 #pragma unroll
-  for (int j = 0; j < 8; ++j) {
+  for (int j = 0; j < 4; ++j) {
     acc.x = fmaf(v[j].x, w[j].x, fmaf(-v[j].y, w[j].y, acc.x));
     acc.y = fmaf(v[j].x, w[j].y, fmaf(v[j].y, w[j].x, acc.y));
     const uint32_t m = meta[Q0 + j];
     if (m & 0x2000u) {
-      zb[m >> 14] = acc;
+      *reinterpret_cast<cf32 *>(zb + (m >> 16)) = acc;
       acc = mk(0.f, 0.f);
     }
   }
@@ -145,9 +147,10 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
   const long long u0 = T * blockIdx.x / gridDim.x, u1 = T * (blockIdx.x + 1) / gridDim.x;
   if (wv < kRProd) {
     // =================================================================== producers
-    const int k0 = 32 * ((2 * wv + lane) & 15) + lane, k1 = 32 * ((2 * wv + 1 + lane) & 15) + lane;   // this lane's columns
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRRegsProd));
+    const int k0 = 32 * ((wv + lane) & 15) + lane;          // this lane's column
     uint32_t meta[kRLmax];
-    uint32_t cmask0 = 0, cmask1 = 0;
+    uint32_t cmask = 0;
     const cf32 *cvp = cv;
     int L = 0, s_cur = -1;
     long long n = 0;
@@ -160,8 +163,7 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
         const int32_t *gh = q.rhdr + ((size_t)ch * kRProd + wv) * kRHdr;
         const int base = __ldg(gh) + lane;
         L = __ldg(gh + 1);
-        cmask0 = __ldg(q.rmask + (size_t)ch * kRW + k0);
-        cmask1 = __ldg(q.rmask + (size_t)ch * kRW + k1);
+        cmask = __ldg(q.rmask + (size_t)ch * kRW + k0);
         cvp = cv + base;
         const uint32_t *__restrict__ gm = q.rmeta + (size_t)ch * q.cap + base;
 #pragma unroll
@@ -184,46 +186,44 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
           const float2 *__restrict__ vis = p.vis + (size_t)(p.snap_base + s) * p.n_bl;
           const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
           const float2 *__restrict__ cf = p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr;
-          for (int i0 = 0; i0 < L; i0 += 8) {            // eight cells in flight (L is a multiple of 8)
-            uint4 rr[8];
-            float2 v0[8], v1[8];
+          for (int i0 = 0; i0 < L; i0 += 4) {            // four cells in flight (L is a multiple of 4)
+            uint4 rr[4];
+            float2 v0[4], v1[4];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) rr[j] = __ldg(rec + 32 * (i0 + j));
+            for (int j = 0; j < 4; ++j) rr[j] = __ldg(rec + 32 * (i0 + j));
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
+            for (int j = 0; j < 4; ++j) {
               const int len = (int)(rr[j].x >> 21);
               v0[j] = v1[j] = make_float2(0.f, 0.f);
               if (len >= 1) v0[j] = ld_vis(vis, cf, rr[j].z >> 1);
               if (len == 2) v1[j] = ld_vis(vis, cf, rr[j].w >> 1);
             }
 #pragma unroll
-            for (int j = 0; j < 8; ++j)
+            for (int j = 0; j < 4; ++j)
               cvw[32 * (i0 + j)] = (rr[j].x >> 21) ? cell_from_vis(rr[j], v0[j], v1[j], vis, cf, src) : mk(0.f, 0.f);
           }
         }
       }
       const int buf = (int)(n & 1);
-      cf32 *zb = reinterpret_cast<cf32 *>(smem_raw + buf * kRTile);
+      unsigned char *zbytes = smem_raw + buf * kRTile;
       if (n >= 2) mbar_wait(bars + 2 + buf, (uint32_t)((n >> 1) - 1) & 1u);     // the consumers have left this tile
       // ---------------------------------------------------------------- S: the bins of this warp's columns
       {
         cf32 acc = mk(0.f, 0.f);
         const unsigned char *natb = reinterpret_cast<const unsigned char *>(nat);
-        if (L > 0) bins8<0>(meta, cvp, natb, zb, r, acc);
-        if (L > 8) bins8<8>(meta, cvp, natb, zb, r, acc);
-        if (L > 16) bins8<16>(meta, cvp, natb, zb, r, acc);
-        if (L > 24) bins8<24>(meta, cvp, natb, zb, r, acc);
+        if (L > 0) bins4<0>(meta, cvp, natb, zbytes, r, acc);
+        if (L > 4) bins4<4>(meta, cvp, natb, zbytes, r, acc);
+        if (L > 8) bins4<8>(meta, cvp, natb, zbytes, r, acc);
+        if (L > 12) bins4<12>(meta, cvp, natb, zbytes, r, acc);
       }
       __syncwarp();
-      // ---------------------------------------------------------------- A: this lane's two columns, in place
-#pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        cf32 *zc = zb + (j ? k1 : k0);
-        const uint32_t cm = j ? cmask1 : cmask0;
+      // ---------------------------------------------------------------- A: this lane's column, in place
+      {
+        cf32 *zc = reinterpret_cast<cf32 *>(zbytes) + k0;
         cf32 t[16];
-        if (__any_sync(0xffffffffu, cm != 0)) {
+        if (__any_sync(0xffffffffu, cmask != 0)) {
 #pragma unroll
-          for (int c = 0; c < 16; ++c) t[c] = ((cm >> c) & 1u) ? zc[c * kRW] : mk(0.f, 0.f);
+          for (int c = 0; c < 16; ++c) t[c] = ((cmask >> c) & 1u) ? zc[c * kRW] : mk(0.f, 0.f);
           dft16(t);                                                   // t[y'] = U[64 y' + r][k]
 #pragma unroll
           for (int pp = 0; pp < 8; ++pp) {
@@ -241,6 +241,7 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
     }
   } else {
     // =================================================================== consumers: row pair p
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRRegsCons));
     const int pr = wv - kRProd;
     long long n = 0;
     for (long long u = u0; u < u1; ++u, ++n) {
@@ -313,7 +314,7 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
   o.mask.assign(kRW, 0u);
   for (int i = 0; i < (int)cells.size(); ++i) {
     const int k = cells[i].k, c = cells[i].iy & (kRRows - 1);
-    ent[(((k >> 5) - (k & 31)) & 15) >> 1][c * kRW + k].push_back(i);     // column 32 a + b belongs to warp ((a - b) mod 16) / 2
+    ent[((k >> 5) - (k & 31)) & 15][c * kRW + k].push_back(i);     // column 32 a + b belongs to warp (a - b) mod 16
     o.mask[k] |= 1u << c;
   }
   o.hdr.assign((size_t)kRProd * kRHdr, 0);
@@ -348,7 +349,7 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
     }
     int L = 0;
     for (int l = 0; l < 32; ++l) L = std::max(L, load[l]);
-    L = (L + 7) / 8 * 8;
+    L = (L + 3) / 4 * 4;
     if (L > kRLmax) { o.ok = false; return; }
     o.hdr[(size_t)w * kRHdr] = (int32_t)o.rec.size();
     o.hdr[(size_t)w * kRHdr + 1] = L;
@@ -366,7 +367,7 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
           o.rec[r0 + 32 * (size_t)qpos + l] =
               make_uint4((uint32_t)c.iy | ((uint32_t)c.flag << 10) | ((uint32_t)c.k << 12) | ((uint32_t)c.len << 21), wbits,
                          (uint32_t)g.src[c.seg], c.len == 2 ? (uint32_t)g.src[c.seg + 1] : (uint32_t)c.seg);
-          o.meta[r0 + 32 * (size_t)qpos + l] = (uint32_t)(8 * c.iy) | (i + 1 == cl.size() ? 0x2000u : 0u) | ((uint32_t)mine[l][n] << 14);
+          o.meta[r0 + 32 * (size_t)qpos + l] = (uint32_t)(8 * c.iy) | (i + 1 == cl.size() ? 0x2000u : 0u) | ((uint32_t)(8 * mine[l][n]) << 16);
         }
       }
     }
