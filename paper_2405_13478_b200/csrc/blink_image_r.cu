@@ -62,15 +62,14 @@ constexpr int kRHdr = 2;                        // ints per (channel, producer w
 constexpr int kRRegsProd = 64, kRRegsCons = 112;// registers per thread after the role split: 16 x 32 x 64 + 8 x 32 x 112 = 768 x 80, the launch allocation
 constexpr size_t kRTile = sizeof(cf32) * kRRows * kRW;
 constexpr size_t kROffTw = 2 * kRTile;                              // the two tiles first
-constexpr size_t kROffNat = kROffTw + sizeof(cf32) * 1024;
-constexpr size_t kROffBar = kROffNat + sizeof(cf32) * 1024;
+constexpr size_t kROffBar = kROffTw + sizeof(cf32) * 1024;
 constexpr size_t kROffCv = kROffBar + 64;
 
 struct RParams {
   ImgParams ip;
   int n_snap, cap;
   const uint4 *rrec;        // [n_ch][cap] iy | flag << 10 | kx << 12 | len << 21, weight, source 0, source 1 / segment (len 0 = padding)
-  const uint32_t *rmeta;    // [n_ch][cap] 8 iy | last-of-entry << 13 | 8 (tile slot c * 512 + kx) << 16 (0 = padding)
+  const uint32_t *rmeta;    // [n_ch][cap] last-of-entry | 8 (tile slot c * 512 + kx) | iy << 22 (0 = padding)
   const int32_t *rhdr;      // [n_ch][kRProd][kRHdr]
   const uint32_t *rmask;    // [n_ch][512] non-empty bins of the column (16 bits)
   const float2 *uvsrc;      // blink_image: cell values from this uv grid; NULL = from the visibilities
@@ -98,27 +97,49 @@ __device__ __forceinline__ cf32 cell_from_vis(const uint4 r, const float2 v0, co
   return mk((ar + ar) * w, 0.f);
 }
 
+// wait of a warp that is ahead of the others: sleep between polls, so that the polling takes neither issue
+// slots nor the shared-memory pipe from the warps it is waiting for
+__device__ __forceinline__ void mbar_wait_idle(uint64_t *bar, uint32_t parity) {
+  for (;;) {
+    uint32_t done;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    if (done) break;
+    __nanosleep(100);
+  }
+}
+
 // steps Q0 .. Q0 + 3 of a lane's list: acc += G w1024^(iy r); an entry's last cell stores the sum.
-// Loads first (values, then twiddles), then the chain, so the shared-memory latencies overlap.  The
-// descriptor times r needs no masking first: its high fields only reach bits the table index drops.
+// The factor comes from the special-function unit, not from a table: shared-memory bandwidth is what
+// binds this kernel, and a 1024-entry table walked at stride iy r costs 5 wavefronts per step.  The
+// descriptor carries iy in its top 10 bits, so the 32-bit product with r IS the angle as a signed
+// binary fraction of a turn (mod 1 by overflow, in [-1/2, 1/2) where sin.approx / cos.approx are at
+// their best: absolute error 2^-21.4, against 2^-24 for the table -- the image is a sum of ~7e3 such
+// terms with unrelated errors, so this stays 1e2 below the 1e-4-of-peak bar; measured in DESIGN.md).
 template <int Q0>
-__device__ __forceinline__ void bins4(const uint32_t (&meta)[kRLmax], const cf32 *__restrict__ cvp, const unsigned char *__restrict__ nat,
-                                      unsigned char *__restrict__ zb, int r, cf32 &acc) {
+__device__ __forceinline__ void bins4(const uint32_t (&meta)[kRLmax], const cf32 *__restrict__ cvp, unsigned char *__restrict__ zb, int r,
+                                      cf32 &acc) {
   cf32 v[4], w[4];
 #pragma unroll
   for (int j = 0; j < 4; ++j) v[j] = cvp[32 * (Q0 + j)];
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
-    const uint32_t P = meta[Q0 + j] * (uint32_t)r;                    // bits 3 .. 12: 8 (iy r mod 1024)
-    w[j] = *reinterpret_cast<const cf32 *>(nat + ((P & 0x1FF8u) ^ ((P >> 4) & 0x78u)));
+    const int32_t P = (int32_t)((meta[Q0 + j] & 0xFFC00000u) * (uint32_t)r);      // turns * 2^32
+    const float ang = (float)P * 1.4629180792671596e-9f;                          // 2 pi / 2^32
+    w[j] = mk(__cosf(ang), __sinf(ang));
   }
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
     acc.x = fmaf(v[j].x, w[j].x, fmaf(-v[j].y, w[j].y, acc.x));
     acc.y = fmaf(v[j].x, w[j].y, fmaf(v[j].y, w[j].x, acc.y));
     const uint32_t m = meta[Q0 + j];
-    if (m & 0x2000u) {
-      *reinterpret_cast<cf32 *>(zb + (m >> 16)) = acc;
+    if (m & 1u) {
+      *reinterpret_cast<cf32 *>(zb + (m & 0xFFF8u)) = acc;
       acc = mk(0.f, 0.f);
     }
   }
@@ -129,14 +150,12 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
   const ImgParams &p = q.ip;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cf32 *twB = reinterpret_cast<cf32 *>(smem_raw + kROffTw);           // [n1][b] exp(2 pi i b n1 / 1024)
-  cf32 *nat = reinterpret_cast<cf32 *>(smem_raw + kROffNat);          // exp(2 pi i k / 1024) at [k ^ ((k >> 4) & 15)]
   uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + kROffBar); // full[2], empty[2]
   cf32 *cv = reinterpret_cast<cf32 *>(smem_raw + kROffCv);            // cell values of the snapshot, by position
   const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
 
   for (int i = tid; i < 1024; i += kRThreads) {
     twB[i] = __ldg(p.tw32 + i);
-    nat[i ^ ((i >> 4) & 15)] = __ldg(p.tw + i);     // swizzled: multiples of 2, 4, 8, 16 (even r) still spread over the banks
   }
   if (tid < 2) mbar_init(bars + tid, kRProd);
   else if (tid < 4) mbar_init(bars + tid, kRCons);
@@ -206,15 +225,14 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
       }
       const int buf = (int)(n & 1);
       unsigned char *zbytes = smem_raw + buf * kRTile;
-      if (n >= 2) mbar_wait(bars + 2 + buf, (uint32_t)((n >> 1) - 1) & 1u);     // the consumers have left this tile
+      if (n >= 2) mbar_wait_idle(bars + 2 + buf, (uint32_t)((n >> 1) - 1) & 1u);     // the consumers have left this tile
       // ---------------------------------------------------------------- S: the bins of this warp's columns
       {
         cf32 acc = mk(0.f, 0.f);
-        const unsigned char *natb = reinterpret_cast<const unsigned char *>(nat);
-        if (L > 0) bins4<0>(meta, cvp, natb, zbytes, r, acc);
-        if (L > 4) bins4<4>(meta, cvp, natb, zbytes, r, acc);
-        if (L > 8) bins4<8>(meta, cvp, natb, zbytes, r, acc);
-        if (L > 12) bins4<12>(meta, cvp, natb, zbytes, r, acc);
+        if (L > 0) bins4<0>(meta, cvp, zbytes, r, acc);
+        if (L > 4) bins4<4>(meta, cvp, zbytes, r, acc);
+        if (L > 8) bins4<8>(meta, cvp, zbytes, r, acc);
+        if (L > 12) bins4<12>(meta, cvp, zbytes, r, acc);
       }
       __syncwarp();
       // ---------------------------------------------------------------- A: this lane's column, in place
@@ -367,7 +385,7 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
           o.rec[r0 + 32 * (size_t)qpos + l] =
               make_uint4((uint32_t)c.iy | ((uint32_t)c.flag << 10) | ((uint32_t)c.k << 12) | ((uint32_t)c.len << 21), wbits,
                          (uint32_t)g.src[c.seg], c.len == 2 ? (uint32_t)g.src[c.seg + 1] : (uint32_t)c.seg);
-          o.meta[r0 + 32 * (size_t)qpos + l] = (uint32_t)(8 * c.iy) | (i + 1 == cl.size() ? 0x2000u : 0u) | ((uint32_t)(8 * mine[l][n]) << 16);
+          o.meta[r0 + 32 * (size_t)qpos + l] = ((uint32_t)c.iy << 22) | (i + 1 == cl.size() ? 1u : 0u) | (uint32_t)(8 * mine[l][n]);
         }
       }
     }
