@@ -57,8 +57,8 @@ constexpr int kRRows = 16;                      // rows of a tile = image rows p
 constexpr int kRUnits = kRN / kRRows;           // units (residue classes) per snapshot
 constexpr int kRProd = 16, kRCons = 8;          // producer / consumer warps
 constexpr int kRThreads = 32 * (kRProd + kRCons);
-constexpr int kRLmax = 16;                      // most cells in a lane's list (descriptors live in registers)
-constexpr int kRHdr = 2;                        // ints per (channel, producer warp) header: first position, steps (multiple of 4)
+constexpr int kRLmax = 16;                      // most cells in a lane's list
+constexpr int kRHdr = 2;                        // ints per (channel, producer warp) header: first position, steps
 constexpr int kRRegsProd = 64, kRRegsCons = 112;// registers per thread after the role split: 16 x 32 x 64 + 8 x 32 x 112 = 768 x 80, the launch allocation
 constexpr size_t kRTile = sizeof(cf32) * kRRows * kRW;
 constexpr size_t kROffTw = 2 * kRTile;                              // the two tiles first
@@ -122,14 +122,19 @@ __device__ __forceinline__ void mbar_wait_idle(uint64_t *bar, uint32_t parity) {
 // their best: absolute error 2^-21.4, against 2^-24 for the table -- the image is a sum of ~7e3 such
 // terms with unrelated errors, so this stays 1e2 below the 1e-4-of-peak bar; measured in DESIGN.md).
 template <int Q0>
-__device__ __forceinline__ void bins4(const uint32_t (&meta)[kRLmax], const cf32 *__restrict__ cvp, unsigned char *__restrict__ zb, int r,
-                                      cf32 &acc) {
+__device__ __forceinline__ void bins4(const uint32_t *__restrict__ mp, const cf32 *__restrict__ cvp, unsigned char *__restrict__ zb, int r,
+                                      int L, cf32 &acc) {
   cf32 v[4], w[4];
-#pragma unroll
-  for (int j = 0; j < 4; ++j) v[j] = cvp[32 * (Q0 + j)];
+  uint32_t m[4];
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
-    const int32_t P = (int32_t)((meta[Q0 + j] & 0xFFC00000u) * (uint32_t)r);      // turns * 2^32
+    const bool on = Q0 + j < L;                      // warp-uniform
+    m[j] = on ? mp[32 * (Q0 + j)] : 0u;
+    v[j] = on ? cvp[32 * (Q0 + j)] : mk(0.f, 0.f);
+  }
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int32_t P = (int32_t)((m[j] & 0xFFC00000u) * (uint32_t)r);              // turns * 2^32
     const float ang = (float)P * 1.4629180792671596e-9f;                          // 2 pi / 2^32
     w[j] = mk(__cosf(ang), __sinf(ang));
   }
@@ -137,9 +142,8 @@ __device__ __forceinline__ void bins4(const uint32_t (&meta)[kRLmax], const cf32
   for (int j = 0; j < 4; ++j) {
     acc.x = fmaf(v[j].x, w[j].x, fmaf(-v[j].y, w[j].y, acc.x));
     acc.y = fmaf(v[j].x, w[j].y, fmaf(v[j].y, w[j].x, acc.y));
-    const uint32_t m = meta[Q0 + j];
-    if (m & 1u) {
-      *reinterpret_cast<cf32 *>(zb + (m & 0xFFF8u)) = acc;
+    if (m[j] & 1u) {
+      *reinterpret_cast<cf32 *>(zb + (m[j] & 0xFFF8u)) = acc;
       acc = mk(0.f, 0.f);
     }
   }
@@ -152,6 +156,7 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
   cf32 *twB = reinterpret_cast<cf32 *>(smem_raw + kROffTw);           // [n1][b] exp(2 pi i b n1 / 1024)
   uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + kROffBar); // full[2], empty[2]
   cf32 *cv = reinterpret_cast<cf32 *>(smem_raw + kROffCv);            // cell values of the snapshot, by position
+  uint32_t *cmeta = reinterpret_cast<uint32_t *>(cv + q.cap);         // their descriptors (fixed per channel)
   const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
 
   for (int i = tid; i < 1024; i += kRThreads) {
@@ -168,9 +173,9 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
     // =================================================================== producers
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRRegsProd));
     const int k0 = 32 * ((wv + lane) & 15) + lane;          // this lane's column
-    uint32_t meta[kRLmax];
     uint32_t cmask = 0;
     const cf32 *cvp = cv;
+    uint32_t *mp = cmeta;
     int L = 0, s_cur = -1;
     long long n = 0;
     for (long long u = u0; u < u1; ++u, ++n) {
@@ -184,9 +189,9 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
         L = __ldg(gh + 1);
         cmask = __ldg(q.rmask + (size_t)ch * kRW + k0);
         cvp = cv + base;
+        mp = cmeta + base;
         const uint32_t *__restrict__ gm = q.rmeta + (size_t)ch * q.cap + base;
-#pragma unroll
-        for (int i = 0; i < kRLmax; ++i) meta[i] = i < L ? __ldg(gm + 32 * i) : 0u;
+        for (int i = 0; i < L; ++i) mp[32 * i] = __ldg(gm + 32 * i);
         const uint4 *__restrict__ rec = q.rrec + (size_t)ch * q.cap + base;
         cf32 *cvw = cv + base;
         if (q.uvsrc != nullptr) {
@@ -205,11 +210,11 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
           const float2 *__restrict__ vis = p.vis + (size_t)(p.snap_base + s) * p.n_bl;
           const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
           const float2 *__restrict__ cf = p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr;
-          for (int i0 = 0; i0 < L; i0 += 4) {            // four cells in flight (L is a multiple of 4)
+          for (int i0 = 0; i0 < L; i0 += 4) {            // four cells in flight
             uint4 rr[4];
             float2 v0[4], v1[4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) rr[j] = __ldg(rec + 32 * (i0 + j));
+            for (int j = 0; j < 4; ++j) rr[j] = i0 + j < L ? __ldg(rec + 32 * (i0 + j)) : make_uint4(0, 0, 0, 0);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               const int len = (int)(rr[j].x >> 21);
@@ -219,7 +224,7 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
             }
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-              cvw[32 * (i0 + j)] = (rr[j].x >> 21) ? cell_from_vis(rr[j], v0[j], v1[j], vis, cf, src) : mk(0.f, 0.f);
+              if (i0 + j < L) cvw[32 * (i0 + j)] = (rr[j].x >> 21) ? cell_from_vis(rr[j], v0[j], v1[j], vis, cf, src) : mk(0.f, 0.f);
           }
         }
       }
@@ -229,10 +234,10 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
       // ---------------------------------------------------------------- S: the bins of this warp's columns
       {
         cf32 acc = mk(0.f, 0.f);
-        if (L > 0) bins4<0>(meta, cvp, zbytes, r, acc);
-        if (L > 4) bins4<4>(meta, cvp, zbytes, r, acc);
-        if (L > 8) bins4<8>(meta, cvp, zbytes, r, acc);
-        if (L > 12) bins4<12>(meta, cvp, zbytes, r, acc);
+        if (L > 0) bins4<0>(mp, cvp, zbytes, r, L, acc);
+        if (L > 4) bins4<4>(mp, cvp, zbytes, r, L, acc);
+        if (L > 8) bins4<8>(mp, cvp, zbytes, r, L, acc);
+        if (L > 12) bins4<12>(mp, cvp, zbytes, r, L, acc);
       }
       __syncwarp();
       // ---------------------------------------------------------------- A: this lane's column, in place
@@ -305,10 +310,10 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
 
 // ---- plan side ----------------------------------------------------------------------------------------
 struct RCell { int k, iy, seg, len, flag; float w; };
-struct RTables {
-  std::vector<uint4> rec;
-  std::vector<uint32_t> meta;
-  std::vector<int32_t> hdr;
+struct RTables {                       // per producer warp: L steps, 32 L records / descriptors (lane-interleaved)
+  std::vector<uint4> rec[kRProd];
+  std::vector<uint32_t> meta[kRProd];
+  int L[kRProd] = {0};
   std::vector<uint32_t> mask;
   bool ok = true;
 };
@@ -335,8 +340,6 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
     ent[((k >> 5) - (k & 31)) & 15][c * kRW + k].push_back(i);     // column 32 a + b belongs to warp (a - b) mod 16
     o.mask[k] |= 1u << c;
   }
-  o.hdr.assign((size_t)kRProd * kRHdr, 0);
-  o.rec.clear(); o.meta.clear();
   for (int w = 0; w < kRProd; ++w) {
     // longest entry first to the lane with the fewest cells so far (ties: lowest lane)
     std::vector<std::pair<int, int>> order;      // (-len, slot)
@@ -367,13 +370,11 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
     }
     int L = 0;
     for (int l = 0; l < 32; ++l) L = std::max(L, load[l]);
-    L = (L + 3) / 4 * 4;
     if (L > kRLmax) { o.ok = false; return; }
-    o.hdr[(size_t)w * kRHdr] = (int32_t)o.rec.size();
-    o.hdr[(size_t)w * kRHdr + 1] = L;
-    const size_t r0 = o.rec.size();
-    o.rec.resize(r0 + (size_t)32 * L, make_uint4(0, 0, 0, 0));
-    o.meta.resize(r0 + (size_t)32 * L, 0u);
+    o.L[w] = L;
+    const size_t r0 = 0;
+    o.rec[w].assign((size_t)32 * L, make_uint4(0, 0, 0, 0));
+    o.meta[w].assign((size_t)32 * L, 0u);
     for (int l = 0; l < 32; ++l) {
       int qpos = 0;
       for (size_t n = 0; n < mine[l].size(); ++n) {
@@ -382,17 +383,17 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
           const RCell &c = cells[cl[i]];
           uint32_t wbits;
           memcpy(&wbits, &c.w, 4);
-          o.rec[r0 + 32 * (size_t)qpos + l] =
+          o.rec[w][r0 + 32 * (size_t)qpos + l] =
               make_uint4((uint32_t)c.iy | ((uint32_t)c.flag << 10) | ((uint32_t)c.k << 12) | ((uint32_t)c.len << 21), wbits,
                          (uint32_t)g.src[c.seg], c.len == 2 ? (uint32_t)g.src[c.seg + 1] : (uint32_t)c.seg);
-          o.meta[r0 + 32 * (size_t)qpos + l] = ((uint32_t)c.iy << 22) | (i + 1 == cl.size() ? 1u : 0u) | (uint32_t)(8 * mine[l][n]);
+          o.meta[w][r0 + 32 * (size_t)qpos + l] = ((uint32_t)c.iy << 22) | (i + 1 == cl.size() ? 1u : 0u) | (uint32_t)(8 * mine[l][n]);
         }
       }
     }
   }
 }
 
-static size_t res_smem(int cap) { return kROffCv + (size_t)cap * sizeof(cf32); }
+static size_t res_smem(int cap) { return kROffCv + (size_t)cap * (sizeof(cf32) + sizeof(uint32_t)); }
 
 void res_route_free(blink_plan *p) {
   cudaFree(p->d_rrec); cudaFree(p->d_rmeta); cudaFree(p->d_rhdr); cudaFree(p->d_rmask);
@@ -410,20 +411,29 @@ int res_route_build(blink_plan *p, cudaStream_t st) {
   const int n_ch = p->n_ch;
   std::vector<RTables> tb(n_ch);
   parallel_for(n_ch, [&](int ch) { res_tables(p->gathers[ch], p->n_pix, p->weighting, p->chinfo[ch].inv_norm, tb[ch]); });
-  int cap = 16;
-  for (int ch = 0; ch < n_ch; ++ch) {
+  // A warp's positions start at the same place for every channel (its longest list over the channels
+  // decides): its lanes rewrite their own values at a snapshot change while other warps still walk theirs.
+  int base[kRProd + 1] = {0};
+  for (int ch = 0; ch < n_ch; ++ch)
     if (!tb[ch].ok) return BLINK_OK;
-    cap = std::max(cap, (int)tb[ch].rec.size());
+  for (int w = 0; w < kRProd; ++w) {
+    int lmax = 0;
+    for (int ch = 0; ch < n_ch; ++ch) lmax = std::max(lmax, tb[ch].L[w]);
+    base[w + 1] = base[w] + 32 * lmax;
   }
+  const int cap = std::max(16, base[kRProd]);
   if (res_smem(cap) > (size_t)p->max_smem_optin) return BLINK_OK;
   std::vector<uint4> h_rec((size_t)n_ch * cap, make_uint4(0, 0, 0, 0));
   std::vector<uint32_t> h_meta((size_t)n_ch * cap, 0u);
   std::vector<int32_t> h_hdr((size_t)n_ch * kRProd * kRHdr, 0);
   std::vector<uint32_t> h_mask((size_t)n_ch * kRW, 0u);
   for (int ch = 0; ch < n_ch; ++ch) {
-    std::copy(tb[ch].rec.begin(), tb[ch].rec.end(), h_rec.begin() + (size_t)ch * cap);
-    std::copy(tb[ch].meta.begin(), tb[ch].meta.end(), h_meta.begin() + (size_t)ch * cap);
-    std::copy(tb[ch].hdr.begin(), tb[ch].hdr.end(), h_hdr.begin() + (size_t)ch * kRProd * kRHdr);
+    for (int w = 0; w < kRProd; ++w) {
+      std::copy(tb[ch].rec[w].begin(), tb[ch].rec[w].end(), h_rec.begin() + (size_t)ch * cap + base[w]);
+      std::copy(tb[ch].meta[w].begin(), tb[ch].meta[w].end(), h_meta.begin() + (size_t)ch * cap + base[w]);
+      h_hdr[((size_t)ch * kRProd + w) * kRHdr] = base[w];
+      h_hdr[((size_t)ch * kRProd + w) * kRHdr + 1] = tb[ch].L[w];
+    }
     std::copy(tb[ch].mask.begin(), tb[ch].mask.end(), h_mask.begin() + (size_t)ch * kRW);
   }
   int rc;
