@@ -10,26 +10,29 @@
 // i.e. the plan's occupied cells (7e3 of 5e5 for MWA Phase I) each times one unit-modulus factor, summed into
 // 16 bins per column, then ONE dense 16-point butterfly per column: a 16 x 512 complex tile = 64 KB of
 // shared memory, where the row pass (two real image rows per 1024-point complex transform, one warp per
-// transform, wfft.cuh's 32 x 32 split) picks it up.  A CTA of 16 warps is split by role over a ring of
-// two such tiles (full / empty mbarriers), so that the latency-bound table walk of one unit overlaps the
-// arithmetic of another on every scheduler:
+// transform, wfft.cuh's 32 x 32 split) picks it up.  A CTA of 24 warps is split by role over a ring of
+// two such tiles (full / empty mbarriers), so that the table walk of one unit overlaps the butterflies of
+// another on every scheduler; after the split the producers give registers to the consumers
+// (setmaxnreg: 16 x 32 x 64 + 8 x 32 x 112 = the 768 x 80 the CTA was launched with):
 //
-//   producers (warps 0-7), per unit:
-//   S  bins:    warp w owns the 64 columns {32 ((2 w + j + b) mod 16) + b}, j = 0, 1.  The columns'
-//               non-empty bins ("entries") are dealt to its lanes by the plan so that every lane has the same
-//               number of cells (longest entry first to the least loaded lane); a lane walks its own list --
-//               cell q of lane l at position 32 q + l, its value in shared memory, its 32-bit descriptor
-//               (iy, last-of-entry flag, tile slot) in a register for the whole snapshot -- adds
-//               G_j w1024^(iy_j r) and, at the last cell of an entry, stores the sum into the tile.  Empty
-//               bins are never written: the plan's per-column bin mask says which to read.
-//   A  columns: lane = column (two per lane); masked loads of its bins, dft16 in registers, and in place
-//               of the bins the row-pass operands Z = U[y] + i U[y + 512] (rows p) and conj U[y] + i conj
-//               U[y + 512] (rows 8 + p, the mirrored half kx < 0).  A column's 16 slots are private to its
-//               lane, so S and A of a warp are ordered by __syncwarp alone.
+//   producers (warps 0-15), per unit:
+//   S  bins:    warp w owns the 32 columns {32 ((w + b) mod 16) + b}.  The columns' non-empty bins
+//               ("entries") are dealt to its lanes by the plan so that every lane has the same number of
+//               cells (longest entry first to the least loaded lane, preferring a lane whose store lands in
+//               a free bank); a lane walks its own list -- cell q of lane l at position 32 q + l: value and
+//               32-bit descriptor (iy, last-of-entry flag, tile slot) in shared memory -- adds
+//               G_j w1024^(iy_j r) and, at the last cell of an entry, stores the sum into the tile.  The
+//               factor comes from the special-function unit, not from a table (see bins4).  Empty bins are
+//               never written: the plan's per-column bin mask says which to read.
+//   A  columns: lane = column; masked loads of its bins, dft16 in registers, and in place of the bins the
+//               row-pass operands Z = U[y] + i U[y + 512] (rows p) and conj U[y] + i conj U[y + 512]
+//               (rows 8 + p, the mirrored half kx < 0).  A column's 16 slots are private to its lane, so
+//               S and A of a warp are ordered by __syncwarp alone.
 //   G  (once per snapshot) every producer lane forms the values of ITS cells: the sum of the cell's
 //               visibilities in ascending baseline order x weight x fftshift sign / norm, exactly as in
-//               blink_image_w.cu.  Values and descriptors are lane-private: no barrier.
-//   consumers (warps 8-15), per unit:
+//               blink_image_w.cu.  Values and descriptors are lane-private and a warp's positions are the
+//               same for every channel, so a snapshot change needs no barrier.
+//   consumers (warps 16-23), per unit:
 //   B  rows:    warp p transforms row pair p: 32 loads per lane, dft32, twiddles, exchange through the warp's
 //               own two tile rows (XOR swizzle, conflict free), tile released, dft32, 64 coalesced streaming
 //               stores of 128 bytes.

@@ -47,7 +47,7 @@ def main():
     # (4): k_img1024, 6 snapshots through a ring of 2
     w = synth.config_mwa1(n_t=3, n_ch=2)
     vis = torch.from_numpy(w.vis()).cuda()
-    plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=dict(warp_ring=2))
+    plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=dict(warp_route=2, warp_ring=2))
     assert plan.query_i32(blink.Q_FUSED_PATH) == 2
     img = plan.grid_image(vis)
     img = plan.grid_image(vis)                      # twice: the kernel must leave its counters zero

@@ -256,12 +256,13 @@ def test_full_size_station_two_call_route(torch_cuda, blink, oracle):
 
 def test_full_size_mwa1_launch_configuration(torch_cuda, blink, oracle):
     """BASELINE.json configs[2] at FULL size (100 t x 24 ch x 8128 bl, 1024^2, uniform weighting) in
-    the launch configuration bench.py times (one blink_grid_image call, 2400 snapshots through the
-    ring of k_img1024); parity on sampled snapshots, every image checked to be fully written."""
+    the launch configuration bench.py times (one blink_grid_image call, 2400 snapshots = 153600 units
+    of k_img1024r over 148 CTAs); parity on sampled snapshots, every image checked to be fully written."""
     torch = torch_cuda
     w = synth.config_mwa1()
     vis = w.vis()
     plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_WARP_KERNEL) == 2
     plan.reserve(w.n_t)
     n_snap = w.n_t * w.n_ch
     img = torch.full((w.n_t, w.n_ch, w.n_pix, w.n_pix), float("nan"), dtype=torch.float32, device="cuda")
@@ -344,7 +345,7 @@ def test_polyphase_route_matches_two_kernel_route(torch_cuda, blink, oracle, n_p
     w.weighting = synth.UNIFORM
     vis_h = w.vis()
     vis = torch.from_numpy(vis_h).cuda()
-    plan0 = _plan(blink, w, polyphase=-1)
+    plan0 = _plan(blink, w, polyphase=-1, warp_route=-1)
     assert plan0.query_i32(blink.Q_FUSED_PATH) == 0
     ref = plan0.grid_image(vis)
     plan0.close()
@@ -427,8 +428,8 @@ def test_warp_route_ring_reuse(torch_cuda, blink, oracle):
     uv = plan0.grid(vis)
     img_lines = plan0.image(uv)             # blink_image on the line kernels (dense bounding-box read)
     plan0.close()
-    plan = _plan(blink, w, warp_ring=3)
-    assert plan.query_i32(blink.Q_FUSED_PATH) == 2
+    plan = _plan(blink, w, warp_route=2, warp_ring=3)      # 2 = the ring kernel (the default here is k_img1024r)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 2 and plan.query_i32(blink.Q_WARP_KERNEL) == 1
     img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
     for _ in range(3):                      # repeatedly: the kernel leaves its counters zero behind itself
         plan.grid_image(vis, img)
@@ -441,6 +442,50 @@ def test_warp_route_ring_reuse(torch_cuda, blink, oracle):
     img_uv = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
     plan.image(uv, img_uv)
     torch.cuda.synchronize()
+    assert torch.isfinite(img_uv).all()
+    assert ((img_uv - ref).abs() <= 1e-5 * peak).all()
+    n_snap = w.n_t * w.n_ch
+    sel = np.array([0, 10, n_snap - 1], np.int64)
+    orc = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_h, sel)
+    got = img.view(n_snap, w.n_pix, w.n_pix)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        pk = np.max(np.abs(orc["images"][q]))
+        assert np.max(np.abs(got[q] - orc["images"][q])) <= IMG_TOL * pk
+    plan.close()
+
+
+@pytest.mark.parametrize("weighting", ["uniform", "natural"])
+def test_residue_route(torch_cuda, blink, oracle, weighting):
+    """blink_grid_image and blink_image on the residue-class kernel (k_img1024r: producer / consumer warps
+    over a ring of two 16-row tiles in shared memory), with CTAs that start in the middle of a snapshot
+    and change snapshot -- and channel -- while other warps still walk the previous one's cells (7 x 3
+    snapshots x 64 units over 148 CTAs): every snapshot against the two-kernel route (same cell sums,
+    fp32 rounding apart) and bit-identical from call to call; sampled ones against the oracle at the
+    image bar."""
+    torch = torch_cuda
+    w = synth.config_mwa1(n_t=7, n_ch=3)
+    if weighting == "natural":
+        w.weighting = synth.NATURAL
+    vis_h = w.vis()
+    vis = torch.from_numpy(vis_h).cuda()
+    plan0 = _plan(blink, w, warp_route=-1)
+    assert plan0.query_i32(blink.Q_FUSED_PATH) == 0
+    ref = plan0.grid_image(vis)
+    uv = plan0.grid(vis)
+    plan0.close()
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 2 and plan.query_i32(blink.Q_WARP_KERNEL) == 2
+    assert plan.query_i64(blink.Q_SCRATCH_BYTES) == 0           # the intermediate never leaves the SM
+    img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(vis, img)
+    assert torch.isfinite(img).all()
+    peak = ref.abs().amax(dim=(-2, -1), keepdim=True)
+    assert ((img - ref).abs() <= 1e-5 * peak).all()
+    again = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(vis, again)
+    assert torch.equal(img, again)                              # f3: deterministic
+    img_uv = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.image(uv, img_uv)                                      # cell values read from the uv grid
     assert torch.isfinite(img_uv).all()
     assert ((img_uv - ref).abs() <= 1e-5 * peak).all()
     n_snap = w.n_t * w.n_ch
