@@ -257,7 +257,14 @@ def algorithmic_flops(w, plan, blink):
     fft = 5.0 * n * math.log2(n)
     grid = 2.0 * w.n_bl
     pass_b = (n / 2) * fft
-    if plan.query_i32(blink.Q_FUSED_PATH) == 2:
+    if plan.query_i32(blink.Q_FUSED_PATH) == 2 and plan.query_i32(blink.Q_WARP_KERNEL) == 2:
+        # residue-class kernel: 64 units per snapshot; per unit every occupied half-plane cell takes one complex
+        # multiply-add (8 flops; its unit-modulus factor comes from the special-function unit and is not counted),
+        # every one of the 512 tile columns a 16-point butterfly plus the two row-pass operands per row pair
+        half_cells = np.mean([plan.n_occ(c) for c in range(w.n_ch)]) / 2.0
+        pass_a = 64.0 * (half_cells * 8.0 + 512 * (5.0 * 16 * 4 + 4.0 * 16))
+        form = "sparse pass A (residue-class kernel)"
+    elif plan.query_i32(blink.Q_FUSED_PATH) == 2:
         half_cells = np.mean([plan.n_occ(c) for c in range(w.n_ch)]) / 2.0
         pass_a = half_cells * 8.0 * 32 + (kxm + 1) * (32 * 5.0 * 32 * 5 + 6.0 * n)
         form = "sparse pass A (warp route)"
@@ -332,7 +339,9 @@ def extra_workload(torch, blink, name, steps, stream, peak, peak_src, alu):
     roof, side = roofline_of(w, plan, blink, name, "fused", call_ms, ab["fused"], n_snap, peak, peak_src, alu)
     out = {"config": workload_config(w, name), "steps": steps, "ms_per_step": ms,
            "images_per_s": n_snap / (ms / 1e3), "mvis_per_s": n_snap * w.n_bl / (ms / 1e3) / 1e6,
-           "route": {1: "shared-memory (k_fused)", 2: "warp-per-transform (k_img1024)", 0: "two kernels"}[
+           "route": {1: "shared-memory (k_fused)", 0: "two kernels",
+                     2: {2: "residue-class kernel, intermediate in shared memory (k_img1024r)",
+                         1: "warp-per-transform ring kernel (k_img1024)"}.get(plan.query_i32(blink.Q_WARP_KERNEL), "?")}[
                plan.query_i32(blink.Q_FUSED_PATH)],
            "images_per_s_vs_sep_roofline": (n_snap / (ms / 1e3)) / (peak * 1e9 / ab["sep"]),
            "roofline": roof, "side_bounds": side}
