@@ -34,8 +34,8 @@
 //               same for every channel, so a snapshot change needs no barrier.
 //   consumers (warps 16-23), per unit:
 //   B  rows:    warp p transforms row pair p: 32 loads per lane, dft32, twiddles, exchange through the warp's
-//               own two tile rows (XOR swizzle, conflict free), tile released, dft32, 64 coalesced streaming
-//               stores of 128 bytes.
+//               own two tile rows (16-byte stores, 8-byte loads, XOR swizzle: conflict free), tile released,
+//               dft32, 64 coalesced streaming stores of 128 bytes.
 //
 // Units are dealt in contiguous runs, T = 64 n_snap units over the CTAs, so the CTAs finish together; no
 // scratch in HBM, no inter-CTA traffic, no cooperative launch.
@@ -289,14 +289,29 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
       dft32(t);
 #pragma unroll
       for (int n1 = 1; n1 < 32; ++n1) t[n1] = cmul(t[n1], twB[n1 * 32 + lane]);
-      // exchange through the warp's own two rows: element (b, n1) at row (b < 16 ? p : 8 + p), slot
-      // (b mod 16) * 32 + (n1 xor b): 8-byte stores by b and loads by n1 are both conflict-free
-      cf32 *th = zb + ((lane & 16) ? (8 + pr) * kRW : pr * kRW) + (lane & 15) * 32;
+      // exchange through the warp's own two rows (1024 slots, no room for padding): lane b writes its
+      // pairs (n1 = 2 j, 2 j + 1) as 16 bytes at pair slot j xor (b mod 16) of row segment b, lane n1
+      // reads element (b, n1) from pair slot (n1 / 2) xor (b mod 16): 16-byte stores (per quarter warp) and
+      // 8-byte loads (per half warp) are both conflict-free, and every address is one XOR from a lane constant
+      {
+        unsigned char *seg = reinterpret_cast<unsigned char *>(zb + ((lane & 16) ? (8 + pr) * kRW : pr * kRW)) + (lane & 15) * 256;
+        const uint32_t wx = (uint32_t)(lane & 15) << 4;
 #pragma unroll
-      for (int n1 = 0; n1 < 32; ++n1) th[n1 ^ lane] = t[n1];
+        for (int j = 0; j < 16; ++j)
+          *reinterpret_cast<float4 *>(seg + (wx ^ (uint32_t)(j << 4))) = make_float4(t[2 * j].x, t[2 * j].y, t[2 * j + 1].x, t[2 * j + 1].y);
+      }
       __syncwarp();
+      {
+        const unsigned char *row0 = reinterpret_cast<const unsigned char *>(zb + pr * kRW);
+        const unsigned char *row1 = reinterpret_cast<const unsigned char *>(zb + (8 + pr) * kRW);
+        const uint32_t rx = ((uint32_t)(lane >> 1) << 4) | ((uint32_t)(lane & 1) << 3);
 #pragma unroll
-      for (int b = 0; b < 32; ++b) t[b] = zb[(b < 16 ? pr * kRW : (8 + pr) * kRW) + (b & 15) * 32 + (lane ^ b)];
+        for (int b = 0; b < 16; ++b) {
+          const uint32_t o = (rx ^ (uint32_t)(b << 4)) + (uint32_t)(b * 256);
+          t[b] = *reinterpret_cast<const cf32 *>(row0 + o);
+          t[b + 16] = *reinterpret_cast<const cf32 *>(row1 + o);
+        }
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(bars + 2 + buf);
       dft32(t);
