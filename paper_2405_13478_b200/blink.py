@@ -26,7 +26,7 @@ EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_pl
            "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct", "blink_dynspec",
            "blink_image", "blink_grid_validate", "blink_grid_image_host", "blink_plan_reserve_host",
            "blink_plan_apply_corrections", "blink_plan_refresh"]
-TESTING_EXPORTS = ["blink_host_build_gather", "blink_host_fused_emulate", "blink_probe_fp32"]
+TESTING_EXPORTS = ["blink_host_build_gather", "blink_host_fused_emulate", "blink_host_residue_emulate", "blink_probe_fp32"]
 
 
 class Options(ctypes.Structure):
@@ -114,6 +114,8 @@ def load() -> ctypes.CDLL:
     lib.blink_host_build_gather.argtypes = [vp, ci, ci, vp, vp, vp, vp]
     lib.blink_host_fused_emulate.restype = ci
     lib.blink_host_fused_emulate.argtypes = [vp, ci, ci, ci, vp, vp, vp]
+    lib.blink_host_residue_emulate.restype = ci
+    lib.blink_host_residue_emulate.argtypes = [vp, ci, ci, vp, ci, vp, vp, vp]
     _lib = lib
     return lib
 
@@ -159,6 +161,27 @@ def host_fused_emulate(cell: np.ndarray, n_pix: int, chunk_vis: int, vis: np.nda
     if rc < 0:
         raise BlinkError(rc, "blink_host_fused_emulate")
     return dict(sums=sums[:stats[0]], n_can=int(stats[0]), groups=int(stats[1]), rows=int(stats[2]))
+
+
+def host_residue_emulate(cell: np.ndarray, weighting: int, vis: np.ndarray, units):
+    """blink_host_residue_emulate: the residue-class kernel (N = 1024) walked on the host (no GPU); returns the
+    image rows of the listed units as {row index: float32[1024]}."""
+    lib = load()
+    cell = np.ascontiguousarray(cell, np.int32)
+    vis = np.ascontiguousarray(vis, np.complex64)
+    units = np.ascontiguousarray(units, np.int32)
+    rows = np.zeros((len(units), 16, 1024), np.float32)
+    stats = np.zeros(3, np.int32)
+    rc = lib.blink_host_residue_emulate(cell.ctypes.data, cell.shape[0], int(weighting), vis.ctypes.data, len(units),
+                                        units.ctypes.data, rows.ctypes.data, stats.ctypes.data)
+    if rc < 0:
+        raise BlinkError(rc, "blink_host_residue_emulate")
+    out = {}
+    for i, r in enumerate(units):
+        for p in range(8):
+            out[64 * p + int(r)] = rows[i, p]
+            out[64 * p + int(r) + 512] = rows[i, 8 + p]
+    return dict(rows=out, positions=int(stats[0]), longest_list=int(stats[1]), n_can=int(stats[2]))
 
 
 def probe_fp32(op: int, iters: int, out, stream=None) -> int:

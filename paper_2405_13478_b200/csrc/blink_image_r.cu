@@ -44,6 +44,8 @@
 // + 4 N^2 (the image, written once) = SURVEY 8(d)'s B_fused.
 #include <algorithm>
 #include <array>
+#include <cmath>
+#include <complex>
 #include <cstring>
 #include <map>
 
@@ -487,3 +489,113 @@ int launch_img1024r(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t 
 }
 
 }  // namespace blink
+
+// Host model of k_img1024r for ONE channel and ONE snapshot (tests without a GPU): builds the tables
+// exactly as res_route_build does and walks them the way the kernel does -- phase G (cell values from
+// the records), phase S (lane lists -> bins; the tile starts as NaN, so a bin read that was never
+// written shows), phase A (masked bins -> 16-point column DFT -> row-pass operands in place), phase B
+// (operands of row pair p -> 1024-point DFT) -- in fp64 with direct DFT sums instead of the butterflies,
+// for the listed units.
+extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int weighting, const float *vis, int n_units,
+                                          const int32_t *units, float *rows, int32_t *stats) {
+  using namespace blink;
+  if (!cell || !vis || !rows || !units || n_bl < 1 || n_units < 0 || (weighting != BLINK_NATURAL && weighting != BLINK_UNIFORM))
+    return BLINK_EINVAL;
+  constexpr int N = kRN;
+  HostGather g;
+  int rc = build_gather_host(cell, n_bl, N, g);
+  if (rc != BLINK_OK) return rc;
+  long long wsum = 0, n_occ = 0;
+  for (int j = 0; j < g.n_can; ++j) {
+    wsum += 2LL * (g.seg_start[j + 1] - g.seg_start[j]);
+    n_occ += g.can_cell[j] == 0 ? 1 : 2;
+  }
+  const double norm = weighting == BLINK_NATURAL ? (double)wsum : (double)n_occ;
+  const float inv_norm = norm > 0.0 ? (float)(1.0 / norm) : 0.f;
+  RTables tb;
+  res_tables(g, N, weighting, inv_norm, tb);
+  if (!tb.ok) return BLINK_EUNSUPPORTED;
+  typedef std::complex<double> cd;
+  const double tau = 6.283185307179586476925286766559;
+  // phase G
+  std::vector<cd> cv[kRProd];
+  int lmax = 0, npos = 0;
+  for (int w = 0; w < kRProd; ++w) {
+    lmax = std::max(lmax, tb.L[w]);
+    npos += 32 * tb.L[w];
+    cv[w].assign((size_t)32 * tb.L[w], cd(0.0, 0.0));
+    for (size_t i = 0; i < cv[w].size(); ++i) {
+      const uint4 r = tb.rec[w][i];
+      const int flag = (r.x >> 10) & 3, len = (int)(r.x >> 21);
+      if (len == 0) continue;
+      float wt;
+      memcpy(&wt, &r.y, 4);
+      double ar = 0.0, ai = 0.0;
+      for (int q = 0; q < len; ++q) {
+        const int code = q == 0 ? (int)r.z : (len == 2 ? (int)r.w : g.src[(int)r.w + q]);
+        const int bl = code >> 1;
+        ar += vis[2 * bl];
+        ai += (code & 1) ? -(double)vis[2 * bl + 1] : (double)vis[2 * bl + 1];
+      }
+      if (flag == kPlaceDirect) cv[w][i] = cd(ar * wt, ai * wt);
+      else if (flag == kPlaceConj) cv[w][i] = cd(ar * wt, -ai * wt);
+      else cv[w][i] = cd(2.0 * ar * wt, 0.0);
+    }
+  }
+  if (stats) { stats[0] = npos; stats[1] = lmax; stats[2] = g.n_can; }
+  const double nan = std::nan("");
+  std::vector<cd> tile((size_t)kRRows * kRW), Z(N);
+  for (int iu = 0; iu < n_units; ++iu) {
+    const int r = units[iu];
+    if (r < 0 || r >= kRUnits) return BLINK_EINVAL;
+    std::fill(tile.begin(), tile.end(), cd(nan, nan));
+    // phase S
+    for (int w = 0; w < kRProd; ++w)
+      for (int l = 0; l < 32; ++l) {
+        cd acc(0.0, 0.0);
+        for (int q = 0; q < tb.L[w]; ++q) {
+          const uint32_t m = tb.meta[w][(size_t)32 * q + l];
+          const int32_t P = (int32_t)((m & 0xFFC00000u) * (uint32_t)r);
+          const double ang = (double)P * (tau / 4294967296.0);
+          acc += cv[w][(size_t)32 * q + l] * cd(cos(ang), sin(ang));
+          if (m & 1u) {
+            tile[(m & 0xFFF8u) >> 3] = acc;
+            acc = cd(0.0, 0.0);
+          }
+        }
+      }
+    // phase A, with the kernel's column ownership (warp w, lane b: column 32 ((w + b) mod 16) + b)
+    for (int w = 0; w < kRProd; ++w)
+      for (int b = 0; b < 32; ++b) {
+        const int k = 32 * ((w + b) & 15) + b;
+        cd t[kRRows], U[kRRows];
+        for (int c = 0; c < kRRows; ++c) t[c] = ((tb.mask[k] >> c) & 1u) ? tile[(size_t)c * kRW + k] : cd(0.0, 0.0);
+        for (int y1 = 0; y1 < kRRows; ++y1) {
+          cd a(0.0, 0.0);
+          for (int c = 0; c < kRRows; ++c) a += t[c] * std::polar(1.0, tau * (double)((c * y1) % kRRows) / kRRows);
+          U[y1] = a;
+        }
+        for (int pp = 0; pp < kRRows / 2; ++pp) {
+          const cd A = U[pp], B = U[pp + kRRows / 2];
+          tile[(size_t)pp * kRW + k] = A + cd(0.0, 1.0) * B;
+          tile[(size_t)(kRRows / 2 + pp) * kRW + k] = std::conj(A) + cd(0.0, 1.0) * std::conj(B);
+        }
+      }
+    // phase B
+    for (int pr = 0; pr < kRRows / 2; ++pr) {
+      for (int kk = 0; kk < N; ++kk) {
+        if (kk < kRW) Z[kk] = tile[(size_t)pr * kRW + kk];
+        else if (kk == kRW) Z[kk] = cd(0.0, 0.0);
+        else Z[kk] = tile[(size_t)(kRRows / 2 + pr) * kRW + (N - kk)];
+      }
+      float *r0 = rows + ((size_t)iu * kRRows + pr) * N, *r1 = rows + ((size_t)iu * kRRows + kRRows / 2 + pr) * N;
+      for (int x = 0; x < N; ++x) {
+        cd a(0.0, 0.0);
+        for (int kk = 0; kk < N; ++kk) a += Z[kk] * std::polar(1.0, tau * (double)((kk * x) % N) / N);
+        r0[x] = (float)a.real();      // image row 64 pr + r
+        r1[x] = (float)a.imag();      // image row 64 pr + r + 512
+      }
+    }
+  }
+  return BLINK_OK;
+}

@@ -112,6 +112,28 @@ def test_fused_gather_tables_on_host(blink, oracle, cfg, chunk):
     assert out["rows"] * 32 >= g["n_kept"] and out["groups"] * 32 >= g["n_can"]
 
 
+@pytest.mark.parametrize("weighting", ["uniform", "natural"])
+def test_residue_route_tables_on_host(blink, oracle, weighting):
+    """The residue-class kernel of blink_grid_image at N = 1024 (k_img1024r) walked on the host: its plan
+    tables (bins of the occupied half-plane cells dealt to lanes, last-of-bin flags, tile slots, per-column
+    bin masks) and its index algebra (y = 64 p + r, 16-point column pass over iy mod 16, operands
+    U[y] + i U[y + 512] and the mirrored half, row pair p) reproduce the oracle's image rows of the listed
+    residue classes -- on MWA-like cells, dropped baselines and the kx = 0 column included."""
+    w = synth.config_mwa1(n_t=1, n_ch=1)
+    wt = synth.UNIFORM if weighting == "uniform" else synth.NATURAL
+    r = oracle.uv_cells(w.ant_enu_m, w.freq_hz[0], w.n_pix, w.pixscale)
+    assert r["n_dropped"] > 0
+    vis = w.vis()
+    units = [0, 1, 37, 63]
+    out = blink.host_residue_emulate(r["cell"], wt, vis[0, 0], units)
+    assert out["longest_list"] <= 16 and out["positions"] % 32 == 0
+    ref = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, wt, vis, np.array([0], np.int64))["images"][0]
+    peak = np.max(np.abs(ref))
+    assert len(out["rows"]) == 16 * len(units)
+    for y, row in out["rows"].items():
+        assert np.max(np.abs(row - ref[y])) <= 2e-6 * peak, f"image row {y}"
+
+
 def test_fft_stage_algebra_on_host(tmp_path):
     exe = str(tmp_path / "host_fft_check")
     subprocess.run(["g++", "-O1", "-std=c++17", os.path.join(ROOT, "tests", "host_fft_check.cpp"),
