@@ -81,7 +81,9 @@ typedef enum blink_query {
   BLINK_Q_CORR_FUSED = 17,  /* out: int32  1 = blink_grid / blink_grid_image apply the factors at load */
   BLINK_Q_TENSOR_ROUTE = 18,/* out: int32  1 = the shared-memory route runs its transforms on the tensor cores (k_fused_tc) */
   BLINK_Q_WARP_KERNEL = 19  /* out: int32  kernel behind BLINK_Q_FUSED_PATH 2: 2 = residue-class kernel (intermediate in shared
-                               memory, k_img1024r), 1 = ring kernel (intermediate in an L2-sized ring, k_img1024), 0 = neither */
+                               memory, k_img1024r), 1 = ring kernel (intermediate in an L2-sized ring, k_img1024), 3 = BLINK_Q_FUSED_PATH is 0
+                               and the column pass of the two kernels is the residue-class kernel k_cols_res (N = 2048 / 4096,
+                               sparse half-plane), 0 = none of these */
 } blink_query;
 
 typedef struct blink_plan blink_plan; /* opaque */

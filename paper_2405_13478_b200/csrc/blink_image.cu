@@ -286,7 +286,10 @@ static int run_image_cfg(const blink_plan *p, ImgParams ip, int n_snap, cudaStre
   for (int base = 0; base < n_snap; base += chunk) {
     const int cs = std::min(chunk, n_snap - base);
     ip.snap_base = base;
-    if (from_vis) k_cols_from_vis<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
+    if (p->res_route == 2) {                // sparse half-plane at N = 2048 / 4096: column pass by residue class
+      rc = launch_cols_res(p, ip, cs, st);
+      if (rc != BLINK_OK) return rc;
+    } else if (from_vis) k_cols_from_vis<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
     else k_image_cols<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
     k_image_rows<N, RP><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
   }
@@ -339,7 +342,7 @@ int image_setup(blink_plan *p) {
 // completion counters per snapshot.
 size_t scratch_need(const blink_plan *p, long long n_t, bool fused) {
   if (fused && fused_smem_route(p)) return 0;
-  if (p->res_route) return 0;
+  if (p->res_route == 1) return 0;
   const long long n_snap = std::max<long long>(n_t * p->n_ch, 1);
   if (p->warp_route) return warp_route_scratch_bytes(p, n_snap);
   const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
@@ -383,7 +386,7 @@ static int launch_image_impl(const blink_plan *p, const float2 *uv, const float2
   ip.snap_base = 0;
   ip.ch0 = ch0;
   ip.direct_max = p->opt.tune[kTuneDirectMax] > 0 ? std::min(32, p->opt.tune[kTuneDirectMax] - 1) : 12;
-  if (p->res_route)                         // residue-class kernel, intermediate in shared memory (blink_image_r.cu)
+  if (p->res_route == 1)                    // residue-class kernel, intermediate in shared memory (blink_image_r.cu)
     return launch_img1024r(p, ip, n_snap, st);
   if (p->warp_route)                        // persistent warp-per-transform kernel (blink_image_w.cu)
     return launch_img1024(p, ip, n_snap, st);

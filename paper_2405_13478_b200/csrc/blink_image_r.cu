@@ -69,6 +69,10 @@ constexpr size_t kRTile = sizeof(cf32) * kRRows * kRW;
 constexpr size_t kROffTw = 2 * kRTile;                              // the two tiles first
 constexpr size_t kROffBar = kROffTw + sizeof(cf32) * 1024;
 constexpr size_t kROffCv = kROffBar + 64;
+// k_cols_res (N = 2048 / 4096, column pass only): two tiles of 8 rows x 1024 columns
+constexpr int kCW = 1024, kCRows = 8, kCLmax = 32, kCThreads = 32 * kRProd;
+constexpr size_t kCTile = sizeof(cf32) * kCRows * kCW;
+constexpr size_t kCOffCv = 2 * kCTile + 64;
 
 struct RParams {
   ImgParams ip;
@@ -76,14 +80,24 @@ struct RParams {
   const uint4 *rrec;        // [n_ch][cap] iy | flag << 10 | kx << 12 | len << 21, weight, source 0, source 1 / segment (len 0 = padding)
   const uint32_t *rmeta;    // [n_ch][cap] last-of-entry | 8 (tile slot c * 512 + kx) | iy << 22 (0 = padding)
   const int32_t *rhdr;      // [n_ch][kRProd][kRHdr]
-  const uint32_t *rmask;    // [n_ch][512] non-empty bins of the column (16 bits)
+  const uint32_t *rmask;    // [n_ch][tile columns] non-empty bins of the column
+  const int16_t *rcols;     // k_cols_res: [16][32][2] the two columns of every lane (the same for all channels)
   const float2 *uvsrc;      // blink_image: cell values from this uv grid; NULL = from the visibilities
 };
 
+// Packing of a cell record's first word for an N = 2^LOGN grid with 2^LOGW tile columns:
+// iy | flag << LOGN | kx << (LOGN + 2) | len << (LOGN + 2 + LOGW); the descriptor carries iy in its top LOGN bits
+template <int LOGN, int LOGW> struct RPack {
+  static constexpr int kFlagSh = LOGN, kKxSh = LOGN + 2, kLenSh = LOGN + 2 + LOGW;
+  static constexpr uint32_t kIyMask = (1u << LOGN) - 1u, kKxMask = (1u << LOGW) - 1u, kLenMax = (1u << (32 - kLenSh)) - 1u;
+  static constexpr uint32_t kAngleMask = ~0u << (32 - LOGN);
+};
+
 // value of one cell: weighted sum of its visibilities in ascending baseline order
+template <class PK>
 __device__ __forceinline__ cf32 cell_from_vis(const uint4 r, const float2 v0, const float2 v1, const float2 *__restrict__ vis,
                                               const float2 *__restrict__ cf, const int32_t *__restrict__ src) {
-  const int flag = (r.x >> 10) & 3, len = (int)(r.x >> 21);
+  const int flag = (r.x >> PK::kFlagSh) & 3, len = (int)(r.x >> PK::kLenSh);
   const float w = __uint_as_float(r.y);
   float ar = v0.x, ai = (r.z & 1) ? -v0.y : v0.y;
   if (len == 2) {
@@ -100,6 +114,47 @@ __device__ __forceinline__ cf32 cell_from_vis(const uint4 r, const float2 v0, co
   if (flag == kPlaceDirect) return mk(ar * w, ai * w);
   if (flag == kPlaceConj) return mk(ar * w, -ai * w);
   return mk((ar + ar) * w, 0.f);
+}
+
+// Phase G of a lane: descriptors and values of ITS L cells (positions base + 32 i) of snapshot s, channel ch
+template <class PK>
+__device__ __forceinline__ void cells_of_snapshot(const ImgParams &p, const float2 *__restrict__ uvsrc, const uint4 *__restrict__ rec,
+                                                  const uint32_t *__restrict__ gm, cf32 *__restrict__ cvw, uint32_t *__restrict__ mp,
+                                                  int L, int s, int ch, int n_pix) {
+  for (int i = 0; i < L; ++i) mp[32 * i] = __ldg(gm + 32 * i);
+  if (uvsrc != nullptr) {
+    // blink_image: the plan's occupied cells with kx >= 0 straight from the uv grid (empty cells are
+    // zero by contract and never read)
+    const float2 *__restrict__ g = uvsrc + (size_t)s * n_pix * n_pix;
+    for (int i = 0; i < L; ++i) {
+      const uint4 rr = __ldg(rec + 32 * i);
+      const int iy = (int)(rr.x & PK::kIyMask), flag = (rr.x >> PK::kFlagSh) & 3, kx = (rr.x >> PK::kKxSh) & PK::kKxMask;
+      const float w = __uint_as_float(rr.y);
+      float2 v = make_float2(0.f, 0.f);
+      if (rr.x >> PK::kLenSh) v = __ldg(g + (size_t)iy * n_pix + kx);
+      cvw[32 * i] = mk(v.x * w, (flag == kPlaceDirect || flag == kPlaceConj) ? v.y * w : 0.f);
+    }
+  } else {
+    const float2 *__restrict__ vis = p.vis + (size_t)s * p.n_bl;
+    const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
+    const float2 *__restrict__ cf = p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr;
+    for (int i0 = 0; i0 < L; i0 += 4) {            // four cells in flight
+      uint4 rr[4];
+      float2 v0[4], v1[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) rr[j] = i0 + j < L ? __ldg(rec + 32 * (i0 + j)) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int len = (int)(rr[j].x >> PK::kLenSh);
+        v0[j] = v1[j] = make_float2(0.f, 0.f);
+        if (len >= 1) v0[j] = ld_vis(vis, cf, rr[j].z >> 1);
+        if (len == 2) v1[j] = ld_vis(vis, cf, rr[j].w >> 1);
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (i0 + j < L) cvw[32 * (i0 + j)] = (rr[j].x >> PK::kLenSh) ? cell_from_vis<PK>(rr[j], v0[j], v1[j], vis, cf, src) : mk(0.f, 0.f);
+    }
+  }
 }
 
 // wait of a warp that is ahead of the others: sleep between polls, so that the polling takes neither issue
@@ -126,9 +181,9 @@ __device__ __forceinline__ void mbar_wait_idle(uint64_t *bar, uint32_t parity) {
 // binary fraction of a turn (mod 1 by overflow, in [-1/2, 1/2) where sin.approx / cos.approx are at
 // their best: absolute error 2^-21.4, against 2^-24 for the table -- the image is a sum of ~7e3 such
 // terms with unrelated errors, so this stays 1e2 below the 1e-4-of-peak bar; measured in DESIGN.md).
-template <int Q0>
-__device__ __forceinline__ void bins4(const uint32_t *__restrict__ mp, const cf32 *__restrict__ cvp, unsigned char *__restrict__ zb, int r,
-                                      int L, cf32 &acc) {
+template <class PK>
+__device__ __forceinline__ void bins4(const int Q0, const uint32_t *__restrict__ mp, const cf32 *__restrict__ cvp,
+                                      unsigned char *__restrict__ zb, int r, int L, cf32 &acc) {
   cf32 v[4], w[4];
   uint32_t m[4];
 #pragma unroll
@@ -139,7 +194,7 @@ __device__ __forceinline__ void bins4(const uint32_t *__restrict__ mp, const cf3
   }
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
-    const int32_t P = (int32_t)((m[j] & 0xFFC00000u) * (uint32_t)r);              // turns * 2^32
+    const int32_t P = (int32_t)((m[j] & PK::kAngleMask) * (uint32_t)r);           // turns * 2^32
     const float ang = (float)P * 1.4629180792671596e-9f;                          // 2 pi / 2^32
     w[j] = mk(__cosf(ang), __sinf(ang));
   }
@@ -156,6 +211,7 @@ __device__ __forceinline__ void bins4(const uint32_t *__restrict__ mp, const cf3
 
 __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
   constexpr int N = kRN;
+  using PK = RPack<10, 9>;
   const ImgParams &p = q.ip;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cf32 *twB = reinterpret_cast<cf32 *>(smem_raw + kROffTw);           // [n1][b] exp(2 pi i b n1 / 1024)
@@ -195,43 +251,8 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
         cmask = __ldg(q.rmask + (size_t)ch * kRW + k0);
         cvp = cv + base;
         mp = cmeta + base;
-        const uint32_t *__restrict__ gm = q.rmeta + (size_t)ch * q.cap + base;
-        for (int i = 0; i < L; ++i) mp[32 * i] = __ldg(gm + 32 * i);
-        const uint4 *__restrict__ rec = q.rrec + (size_t)ch * q.cap + base;
-        cf32 *cvw = cv + base;
-        if (q.uvsrc != nullptr) {
-          // blink_image: the plan's occupied cells with kx >= 0 straight from the uv grid (empty cells are
-          // zero by contract and never read)
-          const float2 *__restrict__ g = q.uvsrc + (size_t)(p.snap_base + s) * N * N;
-          for (int i = 0; i < L; ++i) {
-            const uint4 rr = __ldg(rec + 32 * i);
-            const int iy = (int)(rr.x & 1023), flag = (rr.x >> 10) & 3, kx = (rr.x >> 12) & 511;
-            const float w = __uint_as_float(rr.y);
-            float2 v = make_float2(0.f, 0.f);
-            if (rr.x >> 21) v = __ldg(g + (size_t)iy * N + kx);
-            cvw[32 * i] = mk(v.x * w, (flag == kPlaceDirect || flag == kPlaceConj) ? v.y * w : 0.f);
-          }
-        } else {
-          const float2 *__restrict__ vis = p.vis + (size_t)(p.snap_base + s) * p.n_bl;
-          const int32_t *__restrict__ src = p.src + (size_t)ch * p.n_bl;
-          const float2 *__restrict__ cf = p.corr ? p.corr + (size_t)ch * p.n_bl : nullptr;
-          for (int i0 = 0; i0 < L; i0 += 4) {            // four cells in flight
-            uint4 rr[4];
-            float2 v0[4], v1[4];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) rr[j] = i0 + j < L ? __ldg(rec + 32 * (i0 + j)) : make_uint4(0, 0, 0, 0);
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const int len = (int)(rr[j].x >> 21);
-              v0[j] = v1[j] = make_float2(0.f, 0.f);
-              if (len >= 1) v0[j] = ld_vis(vis, cf, rr[j].z >> 1);
-              if (len == 2) v1[j] = ld_vis(vis, cf, rr[j].w >> 1);
-            }
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-              if (i0 + j < L) cvw[32 * (i0 + j)] = (rr[j].x >> 21) ? cell_from_vis(rr[j], v0[j], v1[j], vis, cf, src) : mk(0.f, 0.f);
-          }
-        }
+        cells_of_snapshot<PK>(p, q.uvsrc, q.rrec + (size_t)ch * q.cap + base, q.rmeta + (size_t)ch * q.cap + base, cv + base, mp, L,
+                              p.snap_base + s, ch, N);
       }
       const int buf = (int)(n & 1);
       unsigned char *zbytes = smem_raw + buf * kRTile;
@@ -239,10 +260,10 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
       // ---------------------------------------------------------------- S: the bins of this warp's columns
       {
         cf32 acc = mk(0.f, 0.f);
-        if (L > 0) bins4<0>(mp, cvp, zbytes, r, L, acc);
-        if (L > 4) bins4<4>(mp, cvp, zbytes, r, L, acc);
-        if (L > 8) bins4<8>(mp, cvp, zbytes, r, L, acc);
-        if (L > 12) bins4<12>(mp, cvp, zbytes, r, L, acc);
+        if (L > 0) bins4<PK>(0, mp, cvp, zbytes, r, L, acc);
+        if (L > 4) bins4<PK>(4, mp, cvp, zbytes, r, L, acc);
+        if (L > 8) bins4<PK>(8, mp, cvp, zbytes, r, L, acc);
+        if (L > 12) bins4<PK>(12, mp, cvp, zbytes, r, L, acc);
       }
       __syncwarp();
       // ---------------------------------------------------------------- A: this lane's column, in place
@@ -328,6 +349,83 @@ __global__ void __launch_bounds__(kRThreads, 1) k_img1024r(const RParams q) {
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// k_cols_res: the column pass (steps a1-a3 and the first half of a4) of the two-kernel routes at N = 2048 /
+// 4096 for sparse half-planes at most 1024 columns wide (MWA Phase II: 7.5e3 occupied cells of 3.5e6), by
+// the same residue classes: y = (N / 8) y' + r, eight bins per column (iy mod 8), dft8, and the eight rows
+// U[(N / 8) y' + r][0 .. wu) of a unit leave the 8 x 1024 tile as bulk copies into the plan's U scratch,
+// where k_image_rows picks them up.  The direct sums of k_cols_from_vis cost N complex multiply-adds per
+// cell and column; here a cell costs N / 8 (one per unit) plus its column's butterflies.  One persistent CTA
+// of 16 warps per SM, every warp in phases S and A (two columns per lane, dealt by the plan so that the
+// warps carry the same number of cells), two tiles so that a unit's copies drain during the next unit.
+template <int LOGN>
+__global__ void __launch_bounds__(kCThreads, 1) k_cols_res(const RParams q) {
+  constexpr int N = 1 << LOGN, R = N / kCRows;
+  using PK = RPack<LOGN, 10>;
+  const ImgParams &p = q.ip;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  cf32 *cv = reinterpret_cast<cf32 *>(smem_raw + kCOffCv);            // cell values of the snapshot, by position
+  uint32_t *cmeta = reinterpret_cast<uint32_t *>(cv + q.cap);         // their descriptors (fixed per channel)
+  const int tid = threadIdx.x, lane = tid & 31, wv = tid >> 5;
+  const int k0 = __ldg(q.rcols + (wv * 32 + lane) * 2), k1 = __ldg(q.rcols + (wv * 32 + lane) * 2 + 1);
+  const long long T = (long long)q.n_snap * R;
+  const long long u0 = T * blockIdx.x / gridDim.x, u1 = T * (blockIdx.x + 1) / gridDim.x;
+  uint32_t cmask0 = 0, cmask1 = 0;
+  const cf32 *cvp = cv;
+  uint32_t *mp = cmeta;
+  int L = 0, s_cur = -1;
+  long long n = 0;
+  for (long long u = u0; u < u1; ++u, ++n) {
+    const int sl = (int)(u / R), r = (int)(u % R);
+    if (sl != s_cur) {
+      // ---------------------------------------------------------------- G: this lane's cells of the snapshot
+      s_cur = sl;
+      const int s = p.snap_base + sl, ch = (s + p.ch0) % p.n_ch;
+      const int32_t *gh = q.rhdr + ((size_t)ch * kRProd + wv) * kRHdr;
+      const int base = __ldg(gh) + lane;
+      L = __ldg(gh + 1);
+      cmask0 = __ldg(q.rmask + (size_t)ch * kCW + k0);
+      cmask1 = __ldg(q.rmask + (size_t)ch * kCW + k1);
+      cvp = cv + base;
+      mp = cmeta + base;
+      cells_of_snapshot<PK>(p, q.uvsrc, q.rrec + (size_t)ch * q.cap + base, q.rmeta + (size_t)ch * q.cap + base, cv + base, mp, L, s,
+                            ch, N);
+    }
+    const int buf = (int)(n & 1);
+    unsigned char *zb = smem_raw + buf * kCTile;
+    if (tid == 0 && n >= 2) bulk_wait_read<1>();       // the copies of the unit before last have read this tile
+    __syncthreads();
+    // ------------------------------------------------------------------ S: the bins of this warp's columns
+    {
+      cf32 acc = mk(0.f, 0.f);
+      for (int q0 = 0; q0 < L; q0 += 4) bins4<PK>(q0, mp, cvp, zb, r, L, acc);
+    }
+    __syncwarp();
+    // ------------------------------------------------------------------ A: this lane's two columns, in place
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      cf32 *zc = reinterpret_cast<cf32 *>(zb) + (j ? k1 : k0);
+      const uint32_t cm = j ? cmask1 : cmask0;
+      cf32 t[kCRows];
+#pragma unroll
+      for (int c = 0; c < kCRows; ++c) t[c] = ((cm >> c) & 1u) ? zc[c * kCW] : mk(0.f, 0.f);
+      if (cm != 0) dft8(t);                                           // t[y'] = U[(N / 8) y' + r][k]
+#pragma unroll
+      for (int c = 0; c < kCRows; ++c) zc[c * kCW] = t[c];
+    }
+    fence_async_smem();                                // the tile's generic writes before the copy engine reads it
+    __syncthreads();
+    if (tid == 0) {
+      float2 *__restrict__ U = p.U + ((size_t)sl * N + r) * p.wu;
+#pragma unroll
+      for (int y1 = 0; y1 < kCRows; ++y1)
+        bulk_store(U + (size_t)y1 * R * p.wu, reinterpret_cast<cf32 *>(zb) + y1 * kCW, (uint32_t)(p.wu * sizeof(cf32)));
+      bulk_commit();
+    }
+  }
+  if (tid == 0) bulk_wait_all();
+}
+
 // ---- plan side ----------------------------------------------------------------------------------------
 struct RCell { int k, iy, seg, len, flag; float w; };
 struct RTables {                       // per producer warp: L steps, 32 L records / descriptors (lane-interleaved)
@@ -338,9 +436,15 @@ struct RTables {                       // per producer warp: L steps, 32 L recor
   bool ok = true;
 };
 
-// the tables of one channel
-static void res_tables(const HostGather &g, int N, int weighting, float inv_norm, RTables &o) {
-  std::vector<RCell> cells;
+// geometry of a residue-class kernel's tables: N = 2^logn grid, 2^logw tile columns, `rows` bins per column
+// (= tile rows = rows of the column butterfly), longest lane list, and the producer warp that owns each column
+// (the lane is always kx mod 32, so that a warp's column accesses hit 32 different banks)
+struct RGeom {
+  int logn, logw, rows, lmax;
+  std::vector<int> owner;          // [2^logw] warp of column kx
+};
+
+static void half_plane_cells(const HostGather &g, int N, int weighting, float inv_norm, std::vector<RCell> &cells) {
   for (int j = 0; j < g.n_can; ++j) {
     const int c = g.can_cell[j], ix = c % N, iy = c / N;
     const int kx = ix < N / 2 ? ix : ix - N, ky = iy;
@@ -351,13 +455,20 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
     if (kx >= 0) cells.push_back({kx, iy, g.seg_start[j], len, c == 0 ? kPlaceBoth : kPlaceDirect, w});
     if (kx <= 0 && c != 0) cells.push_back({-kx, (N - iy) % N, g.seg_start[j], len, kPlaceConj, w});
   }
+  std::sort(cells.begin(), cells.end(), [](const RCell &a, const RCell &b) { return a.k != b.k ? a.k < b.k : a.iy < b.iy; });
+}
+
+// the tables of one channel
+static void res_tables(const HostGather &g, const RGeom &gm, int weighting, float inv_norm, RTables &o) {
+  const int N = 1 << gm.logn, W = 1 << gm.logw;
+  std::vector<RCell> cells;
+  half_plane_cells(g, N, weighting, inv_norm, cells);
   // entries (column, bin) per owning warp; the cells of an entry in ascending iy
   std::vector<std::map<int, std::vector<int>>> ent(kRProd);
-  std::sort(cells.begin(), cells.end(), [](const RCell &a, const RCell &b) { return a.k != b.k ? a.k < b.k : a.iy < b.iy; });
-  o.mask.assign(kRW, 0u);
+  o.mask.assign(W, 0u);
   for (int i = 0; i < (int)cells.size(); ++i) {
-    const int k = cells[i].k, c = cells[i].iy & (kRRows - 1);
-    ent[((k >> 5) - (k & 31)) & 15][c * kRW + k].push_back(i);     // column 32 a + b belongs to warp (a - b) mod 16
+    const int k = cells[i].k, c = cells[i].iy & (gm.rows - 1);
+    ent[gm.owner[k]][c * W + k].push_back(i);
     o.mask[k] |= 1u << c;
   }
   for (int w = 0; w < kRProd; ++w) {
@@ -390,7 +501,7 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
     }
     int L = 0;
     for (int l = 0; l < 32; ++l) L = std::max(L, load[l]);
-    if (L > kRLmax) { o.ok = false; return; }
+    if (L > gm.lmax) { o.ok = false; return; }
     o.L[w] = L;
     const size_t r0 = 0;
     o.rec[w].assign((size_t)32 * L, make_uint4(0, 0, 0, 0));
@@ -404,9 +515,10 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
           uint32_t wbits;
           memcpy(&wbits, &c.w, 4);
           o.rec[w][r0 + 32 * (size_t)qpos + l] =
-              make_uint4((uint32_t)c.iy | ((uint32_t)c.flag << 10) | ((uint32_t)c.k << 12) | ((uint32_t)c.len << 21), wbits,
+              make_uint4((uint32_t)c.iy | ((uint32_t)c.flag << gm.logn) | ((uint32_t)c.k << (gm.logn + 2)) |
+                             ((uint32_t)c.len << (gm.logn + 2 + gm.logw)), wbits,
                          (uint32_t)g.src[c.seg], c.len == 2 ? (uint32_t)g.src[c.seg + 1] : (uint32_t)c.seg);
-          o.meta[w][r0 + 32 * (size_t)qpos + l] = ((uint32_t)c.iy << 22) | (i + 1 == cl.size() ? 1u : 0u) | (uint32_t)(8 * mine[l][n]);
+          o.meta[w][r0 + 32 * (size_t)qpos + l] = ((uint32_t)c.iy << (32 - gm.logn)) | (i + 1 == cl.size() ? 1u : 0u) | (uint32_t)(8 * mine[l][n]);
         }
       }
     }
@@ -416,21 +528,68 @@ static void res_tables(const HostGather &g, int N, int weighting, float inv_norm
 static size_t res_smem(int cap) { return kROffCv + (size_t)cap * (sizeof(cf32) + sizeof(uint32_t)); }
 
 void res_route_free(blink_plan *p) {
-  cudaFree(p->d_rrec); cudaFree(p->d_rmeta); cudaFree(p->d_rhdr); cudaFree(p->d_rmask);
-  p->d_rrec = nullptr; p->d_rmeta = nullptr; p->d_rhdr = nullptr; p->d_rmask = nullptr;
+  cudaFree(p->d_rrec); cudaFree(p->d_rmeta); cudaFree(p->d_rhdr); cudaFree(p->d_rmask); cudaFree(p->d_rcols);
+  p->d_rrec = nullptr; p->d_rmeta = nullptr; p->d_rhdr = nullptr; p->d_rmask = nullptr; p->d_rcols = nullptr;
   p->res_route = 0;
 }
 
-// Residue-class route of blink_grid_image / blink_image at N = 1024: applies when every lane's list of
-// cells is at most kRLmax long (8192 occupied half-plane cells in all, dealt evenly) and the cell values
-// fit in shared memory beside the tiles.
+static size_t cols_smem(int cap) { return kCOffCv + (size_t)cap * (sizeof(cf32) + sizeof(uint32_t)); }
+
+// k_img1024r: column 32 a + b belongs to warp (a - b) mod 16
+static RGeom geom_1024() {
+  RGeom gm{10, 9, kRRows, kRLmax, std::vector<int>(kRW)};
+  for (int k = 0; k < kRW; ++k) gm.owner[k] = ((k >> 5) - (k & 31)) & 15;
+  return gm;
+}
+
+// k_cols_res: 1024 tile columns, two per lane.  For every b = kx mod 32 the 32 columns 32 a + b go, heaviest
+// first (occupied cells over all channels), to the warp with the fewest cells so far that still has a free
+// slot for this b -- the column density of a centrally condensed array falls by 10x from kx = 0 outwards.
+static RGeom geom_cols(const blink_plan *p, std::vector<int16_t> &cols) {
+  const int N = p->n_pix, logn = N == 2048 ? 11 : 12;
+  RGeom gm{logn, 10, kCRows, kCLmax, std::vector<int>(kCW, 0)};
+  std::vector<long long> wcol(kCW, 0);
+  for (const HostGather &g : p->gathers)
+    for (int j = 0; j < g.n_can; ++j) {
+      const int ix = g.can_cell[j] % N, kx = ix < N / 2 ? ix : ix - N;
+      if (std::abs(kx) < kCW) ++wcol[std::abs(kx)];
+    }
+  long long load[kRProd] = {0};
+  cols.assign((size_t)kRProd * 32 * 2, 0);
+  for (int b = 0; b < 32; ++b) {
+    int order[32], used[kRProd] = {0};
+    for (int a = 0; a < 32; ++a) order[a] = 32 * a + b;
+    std::sort(order, order + 32, [&](int x, int y) { return wcol[x] != wcol[y] ? wcol[x] > wcol[y] : x < y; });
+    for (int i = 0; i < 32; ++i) {
+      int best = -1;
+      for (int w = 0; w < kRProd; ++w)
+        if (used[w] < 2 && (best < 0 || load[w] < load[best])) best = w;
+      gm.owner[order[i]] = best;
+      cols[((size_t)best * 32 + b) * 2 + used[best]] = (int16_t)order[i];
+      ++used[best];
+      load[best] += wcol[order[i]];
+    }
+  }
+  return gm;
+}
+
+// Residue-class routes.  N = 1024 (res_route 1, k_img1024r: the whole of blink_grid_image / blink_image)
+// applies when every lane's list of cells is at most kRLmax long (8192 occupied half-plane cells in all,
+// dealt evenly) and the cell values fit in shared memory beside the tiles; N = 2048 / 4096 (res_route 2,
+// k_cols_res: the column pass of the two-kernel routes) when the half-plane is at most 1024 columns wide
+// and its cells fit beside the two 8 x 1024 tiles.
 int res_route_build(blink_plan *p, cudaStream_t st) {
   p->res_route = 0;
-  if (p->n_pix != kRN || p->opt.warp_route == -1 || p->opt.warp_route == 2) return BLINK_OK;
-  if (p->wu > kRW || p->seg_len_max > 2047 || p->max_smem_optin <= 0) return BLINK_OK;
+  if (p->opt.warp_route == -1 || p->opt.warp_route == 2 || p->max_smem_optin <= 0) return BLINK_OK;
+  const int N = p->n_pix, route = N == kRN ? 1 : ((N == 2048 || N == 4096) ? 2 : 0);
+  if (route == 0) return BLINK_OK;
+  std::vector<int16_t> h_cols;
+  const RGeom gm = route == 1 ? geom_1024() : geom_cols(p, h_cols);
+  const int W = 1 << gm.logw;
+  if (p->wu > W || p->seg_len_max > (int)((1u << (32 - (gm.logn + 2 + gm.logw))) - 1u)) return BLINK_OK;
   const int n_ch = p->n_ch;
   std::vector<RTables> tb(n_ch);
-  parallel_for(n_ch, [&](int ch) { res_tables(p->gathers[ch], p->n_pix, p->weighting, p->chinfo[ch].inv_norm, tb[ch]); });
+  parallel_for(n_ch, [&](int ch) { res_tables(p->gathers[ch], gm, p->weighting, p->chinfo[ch].inv_norm, tb[ch]); });
   // A warp's positions start at the same place for every channel (its longest list over the channels
   // decides): its lanes rewrite their own values at a snapshot change while other warps still walk theirs.
   int base[kRProd + 1] = {0};
@@ -442,11 +601,11 @@ int res_route_build(blink_plan *p, cudaStream_t st) {
     base[w + 1] = base[w] + 32 * lmax;
   }
   const int cap = std::max(16, base[kRProd]);
-  if (res_smem(cap) > (size_t)p->max_smem_optin) return BLINK_OK;
+  if ((route == 1 ? res_smem(cap) : cols_smem(cap)) > (size_t)p->max_smem_optin) return BLINK_OK;
   std::vector<uint4> h_rec((size_t)n_ch * cap, make_uint4(0, 0, 0, 0));
   std::vector<uint32_t> h_meta((size_t)n_ch * cap, 0u);
   std::vector<int32_t> h_hdr((size_t)n_ch * kRProd * kRHdr, 0);
-  std::vector<uint32_t> h_mask((size_t)n_ch * kRW, 0u);
+  std::vector<uint32_t> h_mask((size_t)n_ch * W, 0u);
   for (int ch = 0; ch < n_ch; ++ch) {
     for (int w = 0; w < kRProd; ++w) {
       std::copy(tb[ch].rec[w].begin(), tb[ch].rec[w].end(), h_rec.begin() + (size_t)ch * cap + base[w]);
@@ -454,16 +613,19 @@ int res_route_build(blink_plan *p, cudaStream_t st) {
       h_hdr[((size_t)ch * kRProd + w) * kRHdr] = base[w];
       h_hdr[((size_t)ch * kRProd + w) * kRHdr + 1] = tb[ch].L[w];
     }
-    std::copy(tb[ch].mask.begin(), tb[ch].mask.end(), h_mask.begin() + (size_t)ch * kRW);
+    std::copy(tb[ch].mask.begin(), tb[ch].mask.end(), h_mask.begin() + (size_t)ch * W);
   }
   int rc;
   if ((rc = upload_table((void **)&p->d_rrec, h_rec.data(), sizeof(uint4) * h_rec.size(), st, "residue route records")) != BLINK_OK) return rc;
   if ((rc = upload_table((void **)&p->d_rmeta, h_meta.data(), sizeof(uint32_t) * h_meta.size(), st, "residue route descriptors")) != BLINK_OK) return rc;
   if ((rc = upload_table((void **)&p->d_rhdr, h_hdr.data(), sizeof(int32_t) * h_hdr.size(), st, "residue route headers")) != BLINK_OK) return rc;
   if ((rc = upload_table((void **)&p->d_rmask, h_mask.data(), sizeof(uint32_t) * h_mask.size(), st, "residue route masks")) != BLINK_OK) return rc;
+  if (route == 2 &&
+      (rc = upload_table((void **)&p->d_rcols, h_cols.data(), sizeof(int16_t) * h_cols.size(), st, "residue route columns")) != BLINK_OK)
+    return rc;
   BLINK_CUDA_TRY(cudaStreamSynchronize(st), "residue route upload");
   p->res_cap = cap;
-  p->res_route = 1;
+  p->res_route = route;
   return BLINK_OK;
 }
 
@@ -472,7 +634,7 @@ int launch_img1024r(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t 
   RParams q;
   q.n_snap = n_snap;
   q.cap = p->res_cap;
-  q.rrec = p->d_rrec; q.rmeta = p->d_rmeta; q.rhdr = p->d_rhdr; q.rmask = p->d_rmask;
+  q.rrec = p->d_rrec; q.rmeta = p->d_rmeta; q.rhdr = p->d_rhdr; q.rmask = p->d_rmask; q.rcols = nullptr;
   q.uvsrc = ip.vis == nullptr ? ip.uv : nullptr;
   ip.snap_base = 0;
   q.ip = ip;
@@ -486,6 +648,29 @@ int launch_img1024r(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t 
   k_img1024r<<<grid, kRThreads, smem, st>>>(q);
   BLINK_CUDA_TRY(cudaGetLastError(), "k_img1024r launch");
   return BLINK_OK;
+}
+
+template <int LOGN> static int launch_cols_res_n(const blink_plan *p, const RParams &q, cudaStream_t st) {
+  static std::atomic<uint64_t> attr{0};
+  const int rc = ensure_max_smem(k_cols_res<LOGN>, p, attr, "k_cols_res smem attribute");
+  if (rc != BLINK_OK) return rc;
+  const long long units = (long long)q.n_snap * ((1 << LOGN) / kCRows);
+  const int grid = (int)std::min<long long>(p->sm_count, units);
+  k_cols_res<LOGN><<<grid, kCThreads, cols_smem(p->res_cap), st>>>(q);
+  BLINK_CUDA_TRY(cudaGetLastError(), "k_cols_res launch");
+  return BLINK_OK;
+}
+
+// pass A of a chunk of n_snap snapshots (ip.snap_base = the chunk's first) into the plan's U scratch
+int launch_cols_res(const blink_plan *p, const ImgParams &ip, int n_snap, cudaStream_t st) {
+  if (n_snap <= 0) return BLINK_OK;
+  RParams q;
+  q.n_snap = n_snap;
+  q.cap = p->res_cap;
+  q.rrec = p->d_rrec; q.rmeta = p->d_rmeta; q.rhdr = p->d_rhdr; q.rmask = p->d_rmask; q.rcols = p->d_rcols;
+  q.uvsrc = ip.vis == nullptr ? ip.uv : nullptr;
+  q.ip = ip;
+  return p->n_pix == 2048 ? launch_cols_res_n<11>(p, q, st) : launch_cols_res_n<12>(p, q, st);
 }
 
 }  // namespace blink
@@ -513,7 +698,7 @@ extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int wei
   const double norm = weighting == BLINK_NATURAL ? (double)wsum : (double)n_occ;
   const float inv_norm = norm > 0.0 ? (float)(1.0 / norm) : 0.f;
   RTables tb;
-  res_tables(g, N, weighting, inv_norm, tb);
+  res_tables(g, geom_1024(), weighting, inv_norm, tb);
   if (!tb.ok) return BLINK_EUNSUPPORTED;
   typedef std::complex<double> cd;
   const double tau = 6.283185307179586476925286766559;

@@ -154,7 +154,9 @@ struct blink_plan {
   int warp_ring = 0;                // slots of U in the warp route's ring
   long long warp_snap_cap = 0;      // snapshots per call the warp route's counters in scratch are sized for
   // residue-class route at N = 1024 (blink_image_r.cu): the intermediate stays in shared memory, no scratch
-  int res_route = 0;                // 1 = blink_grid_image / blink_image take k_img1024r
+  int res_route = 0;                // 1 = blink_grid_image / blink_image take k_img1024r (N = 1024); 2 = the column pass of the
+                                    // two-kernel routes is k_cols_res (N = 2048 / 4096)
+  int16_t *d_rcols = nullptr;       // [16][32][2] columns of every lane of k_cols_res
   int res_cap = 0;                  // positions per channel of its tables
   uint4 *d_rrec = nullptr;          // [n_ch][res_cap] cell records, lane-interleaved lists per producer warp
   uint32_t *d_rmeta = nullptr;      // [n_ch][res_cap] cell descriptors (iy, last-of-entry, tile slot)
@@ -223,6 +225,7 @@ size_t warp_route_ring_bytes(const blink_plan *p);
 int res_route_build(blink_plan *p, cudaStream_t st);
 void res_route_free(blink_plan *p);
 int launch_img1024r(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t st);
+int launch_cols_res(const blink_plan *p, const ImgParams &ip, int n_snap, cudaStream_t st);   // pass A of a chunk of n_snap snapshots
 
 }  // namespace blink
 

@@ -548,7 +548,7 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
     step(cudaStreamSynchronize(st));
     PLAN_CUDA(ce, "vis-route table upload");
     PLAN_TRY(res_route_build(p, st));
-    p->warp_route = (!p->res_route && p->opt.warp_route != -1 && warp_route_applies(p)) ? 1 : 0;
+    p->warp_route = (p->res_route != 1 && p->opt.warp_route != -1 && warp_route_applies(p)) ? 1 : 0;
   }
   PLAN_TRY(fused_build(p, st));
   PLAN_TRY(fused_tc_build(p, st));
@@ -684,8 +684,8 @@ extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *
     case BLINK_Q_IMAGE_PATH: *(int32_t *)out = p->image_path; break;
     case BLINK_Q_SCRATCH_BYTES: *(int64_t *)out = (int64_t)p->scratch_bytes; break;
     case BLINK_Q_IMAGE_CHUNK: *(int32_t *)out = p->chunk_snapshots; break;
-    case BLINK_Q_FUSED_PATH: *(int32_t *)out = fused_smem_route(p) ? 1 : ((p->warp_route || p->res_route) ? 2 : 0); break;
-    case BLINK_Q_WARP_KERNEL: *(int32_t *)out = p->res_route ? 2 : (p->warp_route ? 1 : 0); break;
+    case BLINK_Q_FUSED_PATH: *(int32_t *)out = fused_smem_route(p) ? 1 : ((p->warp_route || p->res_route == 1) ? 2 : 0); break;
+    case BLINK_Q_WARP_KERNEL: *(int32_t *)out = p->res_route == 1 ? 2 : (p->warp_route ? 1 : (p->res_route == 2 ? 3 : 0)); break;
     case BLINK_Q_FUSED_CHUNK: *(int32_t *)out = p->fused_chunk; break;
     case BLINK_Q_CORR: *(const void **)out = p->d_corr; break;
     case BLINK_Q_CORR_FUSED: *(int32_t *)out = p->corr_on; break;

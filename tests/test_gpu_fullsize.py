@@ -93,15 +93,15 @@ def _pixels(n, seed):
 
 
 def test_mwa2_4096_grid_image_sampled_pixels(torch_cuda, blink, oracle):
-    """BASELINE.json configs[3] (4096^2) through blink_grid_image (two-kernel route: column transforms
-    straight from the visibilities, k_cols_from_vis<4096> + k_image_rows<4096>), more snapshots than
-    one time step so the channel index wraps; every image fully written, every snapshot checked on
+    """BASELINE.json configs[3] (4096^2) through blink_grid_image (two-kernel route: column pass by
+    residue class straight from the visibilities, k_cols_res<12>, + k_image_rows<4096>), more snapshots
+    than one time step so the channel index wraps; every image fully written, every snapshot checked on
     sampled pixels."""
     torch = torch_cuda
     w = synth.config_mwa2(n_t=2, n_ch=3)
     vis = w.vis()
     plan = _plan(blink, w)
-    assert plan.query_i32(blink.Q_FUSED_PATH) == 0
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 0 and plan.query_i32(blink.Q_WARP_KERNEL) == 3
     n = w.n_pix
     img = torch.full((w.n_t, w.n_ch, n, n), float("nan"), dtype=torch.float32, device="cuda")
     plan.grid_image(torch.from_numpy(vis).cuda(), img)
@@ -124,6 +124,7 @@ def test_n2048_all_calls(torch_cuda, blink, oracle, weighting):
     w.n_pix, w.pixscale, w.weighting = 2048, 30.0 * synth.ARCSEC, weighting
     vis = w.vis()
     plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_WARP_KERNEL) == 3      # column pass: k_cols_res<11>
     n = w.n_pix
     for ch in range(w.n_ch):
         r = oracle.uv_cells(w.ant_enu_m, w.freq_hz[ch], n, w.pixscale)
@@ -144,4 +145,38 @@ def test_n2048_all_calls(torch_cuda, blink, oracle, weighting):
     for s in range(w.n_t * w.n_ch):
         _sampled_pixel_check(oracle, w, vis, s, imh[s], yx, uv=uvh[s])
         _sampled_pixel_check(oracle, w, vis, s, imh2[s], yx)
+    plan.close()
+
+
+@pytest.mark.parametrize("n_pix", [2048, 4096])
+def test_residue_column_pass_matches_line_kernels(torch_cuda, blink, n_pix):
+    """k_cols_res (column pass by residue class: cells of a snapshot in shared memory, units of 8 image rows,
+    rows leaving as bulk copies, CTAs that change snapshot and channel mid-run) against the line kernels
+    k_cols_from_vis / k_image_cols (option warp_route = -1) on EVERY pixel of every snapshot, for
+    blink_grid_image and for blink_image on blink_grid's uv grids; bit-identical from call to call."""
+    torch = torch_cuda
+    w = synth.config_mwa2(n_t=3, n_ch=2)
+    if n_pix == 2048:
+        w.n_pix, w.pixscale, w.weighting = 2048, 30.0 * synth.ARCSEC, synth.UNIFORM
+    v = torch.from_numpy(w.vis()).cuda()
+    plan0 = _plan(blink, w, warp_route=-1)
+    assert plan0.query_i32(blink.Q_WARP_KERNEL) == 0
+    ref = plan0.grid_image(v)
+    uv = plan0.grid(v)
+    ref_uv = plan0.image(uv)
+    plan0.close()
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_WARP_KERNEL) == 3
+    img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(v, img)
+    peak = ref.abs().amax(dim=(-2, -1), keepdim=True)
+    assert torch.isfinite(img).all()
+    assert ((img - ref).abs() <= 1e-5 * peak).all()
+    again = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(v, again)
+    assert torch.equal(img, again)
+    img_uv = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.image(uv, img_uv)
+    assert torch.isfinite(img_uv).all()
+    assert ((img_uv - ref_uv).abs() <= 1e-5 * peak).all()
     plan.close()
