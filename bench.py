@@ -268,6 +268,12 @@ def algorithmic_flops(w, plan, blink):
         half_cells = np.mean([plan.n_occ(c) for c in range(w.n_ch)]) / 2.0
         pass_a = half_cells * 8.0 * 32 + (kxm + 1) * (32 * 5.0 * 32 * 5 + 6.0 * n)
         form = "sparse pass A (warp route)"
+    elif plan.query_i32(blink.Q_WARP_KERNEL) == 3:
+        # k_cols_res (N = 2048 / 4096): N / 8 units per snapshot; per unit one complex multiply-add per occupied
+        # half-plane cell and an 8-point butterfly on each of the 1024 tile columns
+        half_cells = np.mean([plan.n_occ(c) for c in range(w.n_ch)]) / 2.0
+        pass_a = (n / 8.0) * (half_cells * 8.0 + 1024 * 5.0 * 8 * 3)
+        form = "sparse pass A (residue-class column pass)"
     else:
         pass_a = (kxm + 1) * fft
         form = "dense pruned pass A"
@@ -339,7 +345,8 @@ def extra_workload(torch, blink, name, steps, stream, peak, peak_src, alu):
     roof, side = roofline_of(w, plan, blink, name, "fused", call_ms, ab["fused"], n_snap, peak, peak_src, alu)
     out = {"config": workload_config(w, name), "steps": steps, "ms_per_step": ms,
            "images_per_s": n_snap / (ms / 1e3), "mvis_per_s": n_snap * w.n_bl / (ms / 1e3) / 1e6,
-           "route": {1: "shared-memory (k_fused)", 0: "two kernels",
+           "route": {1: "shared-memory (k_fused)",
+                     0: "two kernels" + (" (column pass k_cols_res)" if plan.query_i32(blink.Q_WARP_KERNEL) == 3 else ""),
                      2: {2: "residue-class kernel, intermediate in shared memory (k_img1024r)",
                          1: "warp-per-transform ring kernel (k_img1024)"}.get(plan.query_i32(blink.Q_WARP_KERNEL), "?")}[
                plan.query_i32(blink.Q_FUSED_PATH)],
