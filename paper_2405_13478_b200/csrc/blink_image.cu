@@ -33,20 +33,24 @@ template <int N> struct ImgCfg {
 template <int N, class Store>
 __device__ __forceinline__ void fft_tail(cf32 *v, int t, cf32 *line, const cf32 *__restrict__ tw, Store st) {
   using F = Fft<N>;
-  auto lds = [&](int idx) { return line[pad16(idx)]; };
-  auto sts = [&](int idx, cf32 x) { line[pad16(idx)] = x; };
+  // N >= 512: every stride is 1 or a multiple of 16, so the padded-line accesses take immediate offsets
+  constexpr bool kLine = N >= 512;
   F::template compute<0>(v, t, tw);
-  F::template store<0>(v, t, sts);
+  if constexpr (kLine) F::template store_line<0>(v, t, line);
+  else F::template store<0>(v, t, [&](int idx, cf32 x) { line[pad16(idx)] = x; });
   __syncthreads();
-  F::template load<1>(v, t, lds);
+  if constexpr (kLine) F::template load_line<1>(v, t, line);
+  else F::template load<1>(v, t, [&](int idx) { return line[pad16(idx)]; });
   F::template compute<1>(v, t, tw);
   if constexpr (F::NSTAGE == 2) {
     F::template store<1>(v, t, st);
   } else {
     __syncthreads();
-    F::template store<1>(v, t, sts);
+    if constexpr (kLine) F::template store_line<1>(v, t, line);
+    else F::template store<1>(v, t, [&](int idx, cf32 x) { line[pad16(idx)] = x; });
     __syncthreads();
-    F::template load<2>(v, t, lds);
+    if constexpr (kLine) F::template load_line<2>(v, t, line);
+    else F::template load<2>(v, t, [&](int idx) { return line[pad16(idx)]; });
     F::template compute<2>(v, t, tw);
     F::template store<2>(v, t, st);
   }

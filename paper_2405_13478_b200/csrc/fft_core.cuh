@@ -311,6 +311,34 @@ template <int N> struct Fft {
     }
   }
 
+  // Phases 1 and 3 against a pad16 line in shared memory, with the padding strength-reduced: the R
+  // accesses of a butterfly are a fixed stride apart in the PADDED line as well (strides that are
+  // multiples of 16 gain stride/16 pad slots; the unit stride of stage 0's store stays inside one block
+  // of 16), so a butterfly costs one address and R immediate offsets instead of R shift-add pairs.
+  template <int S> BLINK_HD static void load_line(cf32 *v, int t, const cf32 *line) {
+    constexpr int R = radix<S>();
+    static_assert((N / R) % 16 == 0, "input stride must be a multiple of the padding period");
+#pragma unroll
+    for (int b = 0; b < E / R; ++b) {
+      const cf32 *pb = line + pad16(t + b * T);
+#pragma unroll
+      for (int r = 0; r < R; ++r) v[b * R + r] = pb[r * (N / R + N / R / 16)];
+    }
+  }
+  template <int S> BLINK_HD static void store_line(const cf32 *v, int t, cf32 *line) {
+    constexpr int R = radix<S>();
+    constexpr int Ns = ns<S>();
+    static_assert(Ns == 1 || Ns % 16 == 0, "output stride must be 1 or a multiple of the padding period");
+#pragma unroll
+    for (int b = 0; b < E / R; ++b) {
+      const int j = t + b * T;
+      const int k = j & (Ns - 1);
+      cf32 *pb = line + pad16((j - k) * R + k);
+#pragma unroll
+      for (int r = 0; r < R; ++r) pb[r * (Ns + Ns / 16)] = v[b * R + r];
+    }
+  }
+
   // Phase 3 of stage S: out[(j/Ns) Ns R + k + r Ns] = v[b*R + r].  `st(idx, val)`.
   template <int S, class Store> BLINK_HD static void store(const cf32 *v, int t, Store st) {
     constexpr int R = radix<S>();
