@@ -30,12 +30,14 @@ template <int N> struct ImgCfg {
 };
 
 // run stages 1.. of the transform; stage 0's load is done by the caller
-template <int N, class Store>
+// BM: inputs r of the first-stage butterflies outside this mask are known to be zero (never read)
+template <int N, unsigned BM = 0xFFFFu, class Store>
 __device__ __forceinline__ void fft_tail(cf32 *v, int t, cf32 *line, const cf32 *__restrict__ tw, Store st) {
   using F = Fft<N>;
   // N >= 512: every stride is 1 or a multiple of 16, so the padded-line accesses take immediate offsets
   constexpr bool kLine = N >= 512;
-  F::template compute<0>(v, t, tw);
+  if constexpr (BM == 0xFFFFu) F::template compute<0>(v, t, tw);
+  else F::template compute0_pruned<BM>(v);
   if constexpr (kLine) F::template store_line<0>(v, t, line);
   else F::template store<0>(v, t, [&](int idx, cf32 x) { line[pad16(idx)] = x; });
   __syncthreads();
@@ -237,7 +239,10 @@ __global__ void __launch_bounds__(CT * (N / 16)) k_cols_from_vis(const ImgParams
   fft_tail<N>(v, t, line, p.tw, [&](int y, cf32 x) { U[(size_t)y * p.wu] = x; });
 }
 
-template <int N, int RP>
+// NZ < 8: the half-plane is narrower than NZ N / 16 columns, so of the 16 inputs of a first-stage butterfly
+// only r < NZ (direct half) and r >= 16 - NZ (mirrored half) can be non-zero: the others are neither loaded
+// nor added
+template <int N, int RP, int NZ = 8>
 __global__ void __launch_bounds__(RP * (N / 16)) k_image_rows(const ImgParams p) {
   using C = ImgCfg<N>;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -258,6 +263,7 @@ __global__ void __launch_bounds__(RP * (N / 16)) k_image_rows(const ImgParams p)
     float2 a[16], b[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
+      if (r >= NZ && r < 16 - NZ) continue;
       const int idx = t + r * C::T;
       const int k = r < 8 ? idx : N - idx;
       const bool ok = k <= kxm;
@@ -265,12 +271,14 @@ __global__ void __launch_bounds__(RP * (N / 16)) k_image_rows(const ImgParams p)
       b[r] = ok ? __ldg(U1 + k) : make_float2(0.f, 0.f);
     }
 #pragma unroll
-    for (int r = 0; r < 16; ++r)
+    for (int r = 0; r < 16; ++r) {
+      if (r >= NZ && r < 16 - NZ) continue;
       v[r] = r < 8 ? mk(a[r].x - b[r].y, a[r].y + b[r].x) : mk(a[r].x + b[r].y, b[r].x - a[r].y);
+    }
   }
   float *__restrict__ r0 = p.img + ((size_t)s * N + y0) * N;
   float *__restrict__ r1 = p.img + ((size_t)s * N + y1) * N;
-  fft_tail<N>(v, t, line, p.tw, [&](int x, cf32 z) { __stcs(r0 + x, z.x); __stcs(r1 + x, z.y); });
+  fft_tail<N, BandMask<NZ>::value>(v, t, line, p.tw, [&](int x, cf32 z) { __stcs(r0 + x, z.x); __stcs(r1 + x, z.y); });
 }
 
 template <int N, int CT, int RP>
@@ -283,6 +291,12 @@ static int run_image_cfg(const blink_plan *p, ImgParams ip, int n_snap, cudaStre
   int rc = ensure_max_smem(k_image_cols<N, CT>, p, attr_a, "k_image_cols smem attribute");
   if (rc == BLINK_OK) rc = ensure_max_smem(k_cols_from_vis<N, CT>, p, attr_v, "k_cols_from_vis smem attribute");
   if (rc == BLINK_OK) rc = ensure_max_smem(k_image_rows<N, RP>, p, attr_b, "k_image_rows smem attribute");
+  // a half-plane at most N / 4 columns wide: the row transforms' first stage pruned to 4 + 4 of 16 inputs
+  constexpr bool kNarrow = N >= 2048;
+  static std::atomic<uint64_t> attr_b4{0};
+  const bool narrow = kNarrow && p->kx_max_all < N / 4;
+  if constexpr (kNarrow)
+    if (rc == BLINK_OK && narrow) rc = ensure_max_smem(k_image_rows<N, RP, 4>, p, attr_b4, "k_image_rows smem attribute");
   if (rc != BLINK_OK) return rc;
   const size_t per_snap = sizeof(float2) * (size_t)N * p->wu;
   const int chunk = (int)std::min<size_t>((size_t)std::max(1, p->chunk_snapshots), p->scratch_bytes / per_snap);
@@ -295,7 +309,12 @@ static int run_image_cfg(const blink_plan *p, ImgParams ip, int n_snap, cudaStre
       if (rc != BLINK_OK) return rc;
     } else if (from_vis) k_cols_from_vis<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
     else k_image_cols<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
-    k_image_rows<N, RP><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
+    if constexpr (kNarrow) {
+      if (narrow) k_image_rows<N, RP, 4><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
+      else k_image_rows<N, RP><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
+    } else {
+      k_image_rows<N, RP><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
+    }
   }
   BLINK_CUDA_TRY(cudaGetLastError(), "k_image launch");
   return BLINK_OK;
