@@ -393,8 +393,7 @@ __global__ void __launch_bounds__(kCThreads, 1) k_cols_res(const RParams q) {
     }
     const int buf = (int)(n & 1);
     unsigned char *zb = smem_raw + buf * kCTile;
-    if (tid == 0 && n >= 2) bulk_wait_read<1>();       // the copies of the unit before last have read this tile
-    __syncthreads();
+    // (this tile was last read by the copies of unit n - 2: complete before the barrier of unit n - 1)
     // ------------------------------------------------------------------ S: the bins of this warp's columns
     {
       cf32 acc = mk(0.f, 0.f);
@@ -414,7 +413,8 @@ __global__ void __launch_bounds__(kCThreads, 1) k_cols_res(const RParams q) {
       for (int c = 0; c < kCRows; ++c) zc[c * kCW] = t[c];
     }
     fence_async_smem();                                // the tile's generic writes before the copy engine reads it
-    __syncthreads();
+    if (tid == 0 && n >= 1) bulk_wait_read<0>();       // the previous unit's copies have read the other tile: free for the next unit
+    __syncthreads();                                   // the one barrier of a unit
     if (tid == 0) {
       float2 *__restrict__ U = p.U + ((size_t)sl * N + r) * p.wu;
 #pragma unroll
