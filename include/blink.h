@@ -102,7 +102,7 @@ typedef struct blink_options {
   int32_t warp_ring;          /* snapshots of intermediate U kept in flight by that route: 0 auto (32 MB), else >= 2 */
   int32_t grid_ring;          /* blink_grid ring route: 0 auto, -1 never */
   int32_t grid_ring_min_snap; /* fewest snapshots per call that take it: 0 auto (one per SM), else >= 1 */
-  int32_t image_chunk_mb;     /* scratch budget (MiB) of the two-kernel imaging routes: 0 auto (512) */
+  int32_t image_chunk_mb;     /* scratch budget (MiB) of the two-kernel imaging routes: 0 auto (2048) */
   int32_t tune[8];            /* implementation tuning knobs, meaning private to this version (csrc/blink_internal.h) */
 } blink_options;
 

@@ -349,10 +349,10 @@ int image_setup(blink_plan *p) {
   p->img_ct = p->opt.tune[kTuneImageCt];
   p->img_rp = p->opt.tune[kTuneImageRp];
   p->image_path = 1;
-  // snapshots per launch pair.  The transforms are instruction-bound, not HBM-bound, so fewer and
-  // larger launches win over keeping U L2-resident (measured: 48 MB -> 11.1 ms, 400 MB -> 10.0 ms
-  // per 2400 MWA-I snapshots)
-  size_t budget = 512u << 20;
+  // snapshots per launch pair.  Fewer and larger launches win over keeping U L2-resident: every launch pair
+  // costs ~40 us of start-up and tail (measured per 480 MWA-II snapshots at 4096^2: 60 MB -> 19.2 ms,
+  // 512 MB -> 14.2 ms, 2 GB -> 12.3 ms, 8 GB -> 12.2 ms)
+  size_t budget = (size_t)2048 << 20;
   if (p->opt.image_chunk_mb > 0) budget = (size_t)p->opt.image_chunk_mb << 20;
   const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
   // a chunk's snapshots are the launch's gridDim.y: at most 65535
