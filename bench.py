@@ -372,7 +372,7 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "separate", "fused"],
                     help="separate = blink_grid + blink_image (uv grid in HBM); fused = blink_grid_image; "
                          "auto = fused")
-    ap.add_argument("--extra-workloads", default="mwa1,sweep512",
+    ap.add_argument("--extra-workloads", default="mwa1,mwa2,sweep512",
                     help="comma list of further workloads timed in the same process at N = 1 ('' = none)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
