@@ -586,7 +586,9 @@ int res_route_build(blink_plan *p, cudaStream_t st) {
   std::vector<int16_t> h_cols;
   const RGeom gm = route == 1 ? geom_1024() : geom_cols(p, h_cols);
   const int W = 1 << gm.logw;
-  if (p->wu > W || p->seg_len_max > (int)((1u << (32 - (gm.logn + 2 + gm.logw))) - 1u)) return BLINK_OK;
+  // wide, sparsely filled half-planes only: a compact array (a station imaged at 1024^2: 40 columns, 14 baselines
+  // per cell) is faster on the line kernels (measured 6.8 ms against 8.3 ms per 4000 snapshots)
+  if (p->wu < 256 || p->wu > W || p->seg_len_max > (int)((1u << (32 - (gm.logn + 2 + gm.logw))) - 1u)) return BLINK_OK;
   const int n_ch = p->n_ch;
   std::vector<RTables> tb(n_ch);
   parallel_for(n_ch, [&](int ch) { res_tables(p->gathers[ch], gm, p->weighting, p->chinfo[ch].inv_norm, tb[ch]); });
