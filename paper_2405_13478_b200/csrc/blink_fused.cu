@@ -10,9 +10,12 @@
 #include <cstdio>
 #include <cstring>
 
-// complex adds as scalar FADDs here: the packed FADD2 form (fft_core.cuh) measured 2 % slower on
-// k_fused<256> (station 0.419 -> 0.427 ms; 6 % faster on k_img1024, which keeps it)
-#define BLINK_SCALAR_COMPLEX
+// complex adds as packed fp32 pairs (fft_core.cuh, SASS FADD2) here too: pass B is issue-bound (42 % of
+// the kernel's instructions, a warp ready and another one issuing a third of the time), and the packed
+// form halves its adds -- station 0.403 -> 0.393 ms, sweep512 1.31 -> 1.25 ms.  (Round 1 measured the
+// opposite, 0.419 -> 0.427 ms, when phase S still dominated the kernel.)  Phase S adds packed as well
+// (sgather.cuh): 0.393 -> 0.392 ms.
+#define BLINK_PHASE_S_PACKED
 #include "blink_internal.h"
 #include "fft_core.cuh"
 #include "sgather.cuh"
@@ -25,8 +28,8 @@ using namespace blinkfft;
 
 int fused_line_stride(int n_pix) { return ((n_pix + n_pix / 16 + 15) / 16) * 16 + 1; }
 
-// N <= 128 is instantiated in blink_fused_small.cu (packed fp32 pairs in phase S and the butterflies)
-int launch_fused_small(const blink_plan *p, const FusedParams &fp, cudaStream_t st);
+// the polyphase instances with D = 4 live in blink_fused_d4.cu (scalar complex adds)
+int launch_fused_d4(const blink_plan *p, const FusedParams &fp, int nz, cudaStream_t st);
 
 int fused_setup(blink_plan *p) {
   p->fused_path = 0;
@@ -297,11 +300,11 @@ static int launch_fused_c(const blink_plan *p, const FusedParams &fp, cudaStream
   const int reach = std::max(p->kx_max_all, p->ky_max_all) + 1, T = n_sub / 16;
   const int nz = (reach + T - 1) / T;
   if (p->fused_D == 2) return nz <= 3 ? launch_fused_n<256, 3, 2, CORR>(p, fp, st) : launch_fused_n<256, 8, 2, CORR>(p, fp, st);
-  if (p->fused_D == 4) return nz <= 3 ? launch_fused_n<256, 3, 4, CORR>(p, fp, st) : launch_fused_n<256, 8, 4, CORR>(p, fp, st);
+  if (p->fused_D == 4) return launch_fused_d4(p, fp, nz, st);
   switch (p->n_pix) {
-    case 32:
-    case 64:
-    case 128: return launch_fused_small(p, fp, st);
+    case 32: return launch_fused_n<32, 8, 1, CORR>(p, fp, st);
+    case 64: return launch_fused_n<64, 8, 1, CORR>(p, fp, st);
+    case 128: return launch_fused_n<128, 8, 1, CORR>(p, fp, st);
     case 256:
       if constexpr (!CORR) {       // (with corrections: the two instances that cover every band limit)
         if (nz <= 2) return launch_fused_n<256, 2, 1, CORR>(p, fp, st);
