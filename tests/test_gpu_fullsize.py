@@ -180,3 +180,32 @@ def test_residue_column_pass_matches_line_kernels(torch_cuda, blink, n_pix):
     assert torch.isfinite(img_uv).all()
     assert ((img_uv - ref_uv).abs() <= 1e-5 * peak).all()
     plan.close()
+
+
+def test_corrections_fused_into_the_residue_column_pass(torch_cuda, blink):
+    """f2 fused at load on the 2048^2 route: k_cols_res multiplies every visibility by the plan's factor as its
+    lanes form their cells; against the stand-alone pass (blink_correct, then the plain call) on every pixel,
+    and switching it off again restores the plain images bit for bit."""
+    torch = torch_cuda
+    w = synth.config_mwa2(n_t=2, n_ch=2)
+    w.n_pix, w.pixscale = 2048, 30.0 * synth.ARCSEC
+    rng = np.random.default_rng(23)
+    n_ant = w.ant_enu_m.shape[0]
+    gains = rng.uniform(0.5, 2.0, (w.n_ch, n_ant)) * np.exp(1j * rng.uniform(-np.pi, np.pi, (w.n_ch, n_ant)))
+    cables = rng.uniform(0.0, 300.0, n_ant)
+    v = torch.from_numpy(w.vis()).cuda()
+    plan = _plan(blink, w)
+    assert plan.query_i32(blink.Q_WARP_KERNEL) == 3
+    plain = plan.grid_image(v).clone()
+    plan.set_corrections(gains, cables, 0.002, -0.001)
+    ref = plan.grid_image(plan.correct(v)).clone()
+    plan.apply_corrections(True)
+    img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(v, img)
+    assert torch.isfinite(img).all()
+    peak = ref.abs().amax(dim=(-2, -1), keepdim=True)
+    assert ((img - ref).abs() <= 1e-5 * peak).all()
+    assert not torch.equal(img, plain)
+    plan.apply_corrections(False)
+    assert torch.equal(plan.grid_image(v), plain)
+    plan.close()

@@ -710,6 +710,7 @@ def test_corrections_match_oracle(torch_cuda, blink, name, n_t):
     ("tiny", {}), ("station", {}), ("station128", {}), ("station512", {}), ("mwa1", {}),
     ("station", dict(grid_ring_min_snap=1)),          # blink_grid on the ring route (k_grid_ring<CORR>)
     ("station128", dict(fused_route=-1)),             # blink_grid_image on the two-kernel route (k_cols_from_vis)
+    ("mwa1", dict(warp_route=2)),                     # blink_grid_image on the ring kernel (k_img1024)
     ("station_uniform_32", {}), ("mwa1_natural_64", {})])
 def test_corrections_fused_at_load(torch_cuda, blink, oracle, name, options):
     """SURVEY 8(f) f2, fused: with blink_plan_apply_corrections(1), blink_grid and blink_grid_image grid
