@@ -46,21 +46,22 @@ int blink_host_fused_emulate(const int32_t *cell, int n_bl, int n_pix, int chunk
                              float *sums, int32_t *stats);
 
 /*
- * Host model of the residue-class kernel of blink_grid_image at N = 1024 (k_img1024r, csrc/blink_image_r.cu;
- * steps a1-a5) for ONE channel and ONE snapshot, exported so its plan tables and index
- * algebra are testable without a GPU: builds the tables as the plan does (bins of the occupied half-plane
- * cells dealt to the lanes of 16 producer warps) and walks them as the kernel does -- cell values, bins of
- * a unit (image rows y = 64 p + r and y + 512, p = 0..7), 16-point column transforms, row-pass operands,
- * 1024-point row transforms -- in fp64 with direct DFT sums in place of the butterflies.
- *   cell       HOST int32 [n_bl], -1 = dropped (cells of a 1024 x 1024 grid)
+ * Host model of the residue-class kernels (csrc/blink_image_r.cu; steps a1-a5) for ONE channel
+ * and ONE snapshot, exported so their plan tables and index algebra are testable without a GPU: builds the
+ * tables as the plan does (bins of the occupied half-plane cells dealt to the lanes of 16 warps; at N = 2048 /
+ * 4096 also the columns dealt to the warps) and walks them as the kernels do -- cell values, bins of a unit,
+ * column transforms, row transforms -- in fp64 with direct DFT sums in place of the butterflies.
+ *   n_pix = 1024: k_img1024r, a unit r in 0..63 = image rows 64 p + r (p = 0..7) and those + 512
+ *   n_pix = 2048 / 4096: k_cols_res, a unit r in 0..N/8-1 = image rows (N / 8) y' + r, y' = 0..7
+ *   cell       HOST int32 [n_bl], -1 = dropped (cells of an n_pix x n_pix grid)
  *   weighting  BLINK_NATURAL / BLINK_UNIFORM
  *   vis        HOST complex64 [n_bl] (interleaved floats)
- *   units      HOST int32 [n_units] residue classes r in 0 .. 63
- *   rows       HOST float32 [n_units][16][1024] out: image rows 64 p + r (p = 0..7), then 64 p + r + 512
+ *   units      HOST int32 [n_units]
+ *   rows       HOST float32 [n_units][16 or 8][n_pix] out: the unit's image rows in the order given above
  *   stats      HOST int32 [3] out (may be NULL): list positions, longest lane list, canonical cells
  * Returns 0, BLINK_EUNSUPPORTED when the cells do not fit the route, or a negative blink_status.
  */
-int blink_host_residue_emulate(const int32_t *cell, int n_bl, int weighting, const float *vis, int n_units,
+int blink_host_residue_emulate(const int32_t *cell, int n_bl, int n_pix, int weighting, const float *vis, int n_units,
                                const int32_t *units, float *rows, int32_t *stats);
 
 /*

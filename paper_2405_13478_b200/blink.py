@@ -115,7 +115,7 @@ def load() -> ctypes.CDLL:
     lib.blink_host_fused_emulate.restype = ci
     lib.blink_host_fused_emulate.argtypes = [vp, ci, ci, ci, vp, vp, vp]
     lib.blink_host_residue_emulate.restype = ci
-    lib.blink_host_residue_emulate.argtypes = [vp, ci, ci, vp, ci, vp, vp, vp]
+    lib.blink_host_residue_emulate.argtypes = [vp, ci, ci, ci, vp, ci, vp, vp, vp]
     _lib = lib
     return lib
 
@@ -163,24 +163,28 @@ def host_fused_emulate(cell: np.ndarray, n_pix: int, chunk_vis: int, vis: np.nda
     return dict(sums=sums[:stats[0]], n_can=int(stats[0]), groups=int(stats[1]), rows=int(stats[2]))
 
 
-def host_residue_emulate(cell: np.ndarray, weighting: int, vis: np.ndarray, units):
-    """blink_host_residue_emulate: the residue-class kernel (N = 1024) walked on the host (no GPU); returns the
-    image rows of the listed units as {row index: float32[1024]}."""
+def host_residue_emulate(cell: np.ndarray, n_pix: int, weighting: int, vis: np.ndarray, units):
+    """blink_host_residue_emulate: the residue-class kernels (N = 1024: k_img1024r; 2048 / 4096: k_cols_res +
+    plain row sums) walked on the host (no GPU); returns the image rows of the listed units as
+    {row index: float32[n_pix]}."""
     lib = load()
     cell = np.ascontiguousarray(cell, np.int32)
     vis = np.ascontiguousarray(vis, np.complex64)
     units = np.ascontiguousarray(units, np.int32)
-    rows = np.zeros((len(units), 16, 1024), np.float32)
+    per = 16 if n_pix == 1024 else 8
+    rows = np.zeros((len(units), per, n_pix), np.float32)
     stats = np.zeros(3, np.int32)
-    rc = lib.blink_host_residue_emulate(cell.ctypes.data, cell.shape[0], int(weighting), vis.ctypes.data, len(units),
-                                        units.ctypes.data, rows.ctypes.data, stats.ctypes.data)
+    rc = lib.blink_host_residue_emulate(cell.ctypes.data, cell.shape[0], int(n_pix), int(weighting), vis.ctypes.data,
+                                        len(units), units.ctypes.data, rows.ctypes.data, stats.ctypes.data)
     if rc < 0:
         raise BlinkError(rc, "blink_host_residue_emulate")
     out = {}
     for i, r in enumerate(units):
-        for p in range(8):
-            out[64 * p + int(r)] = rows[i, p]
-            out[64 * p + int(r) + 512] = rows[i, 8 + p]
+        for q in range(per):
+            if n_pix == 1024:
+                out[64 * (q % 8) + int(r) + (512 if q >= 8 else 0)] = rows[i, q]
+            else:
+                out[(n_pix // 8) * q + int(r)] = rows[i, q]
     return dict(rows=out, positions=int(stats[0]), longest_list=int(stats[1]), n_can=int(stats[2]))
 
 

@@ -545,11 +545,11 @@ static RGeom geom_1024() {
 // k_cols_res: 1024 tile columns, two per lane.  For every b = kx mod 32 the 32 columns 32 a + b go, heaviest
 // first (occupied cells over all channels), to the warp with the fewest cells so far that still has a free
 // slot for this b -- the column density of a centrally condensed array falls by 10x from kx = 0 outwards.
-static RGeom geom_cols(const blink_plan *p, std::vector<int16_t> &cols) {
-  const int N = p->n_pix, logn = N == 2048 ? 11 : 12;
+static RGeom geom_cols(const std::vector<HostGather> &gathers, int N, std::vector<int16_t> &cols) {
+  const int logn = N == 2048 ? 11 : 12;
   RGeom gm{logn, 10, kCRows, kCLmax, std::vector<int>(kCW, 0)};
   std::vector<long long> wcol(kCW, 0);
-  for (const HostGather &g : p->gathers)
+  for (const HostGather &g : gathers)
     for (int j = 0; j < g.n_can; ++j) {
       const int ix = g.can_cell[j] % N, kx = ix < N / 2 ? ix : ix - N;
       if (std::abs(kx) < kCW) ++wcol[std::abs(kx)];
@@ -584,7 +584,7 @@ int res_route_build(blink_plan *p, cudaStream_t st) {
   const int N = p->n_pix, route = N == kRN ? 1 : ((N == 2048 || N == 4096) ? 2 : 0);
   if (route == 0) return BLINK_OK;
   std::vector<int16_t> h_cols;
-  const RGeom gm = route == 1 ? geom_1024() : geom_cols(p, h_cols);
+  const RGeom gm = route == 1 ? geom_1024() : geom_cols(p->gathers, N, h_cols);
   const int W = 1 << gm.logw;
   // wide, sparsely filled half-planes only: a compact array (a station imaged at 1024^2: 40 columns, 14 baselines
   // per cell) is faster on the line kernels (measured 6.8 ms against 8.3 ms per 4000 snapshots)
@@ -677,18 +677,20 @@ int launch_cols_res(const blink_plan *p, const ImgParams &ip, int n_snap, cudaSt
 
 }  // namespace blink
 
-// Host model of k_img1024r for ONE channel and ONE snapshot (tests without a GPU): builds the tables
-// exactly as res_route_build does and walks them the way the kernel does -- phase G (cell values from
-// the records), phase S (lane lists -> bins; the tile starts as NaN, so a bin read that was never
-// written shows), phase A (masked bins -> 16-point column DFT -> row-pass operands in place), phase B
-// (operands of row pair p -> 1024-point DFT) -- in fp64 with direct DFT sums instead of the butterflies,
-// for the listed units.
-extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int weighting, const float *vis, int n_units,
+// Host model of the residue-class kernels for ONE channel and ONE snapshot (tests without a GPU): builds the
+// tables exactly as res_route_build does and walks them the way the kernels do -- phase G (cell values from
+// the records), phase S (lane lists -> bins; the tile starts as NaN, so a bin read that was never written
+// shows), phase A (masked bins -> column DFT; at N = 1024 also the row-pass operands in place) and the row
+// pass -- in fp64 with direct DFT sums instead of the butterflies, for the listed units.  N = 1024:
+// k_img1024r (16 rows per unit); N = 2048 / 4096: k_cols_res (8 rows per unit, columns dealt to warps by
+// cell count), followed by a plain Hermitian row sum in place of k_image_rows.
+extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int n_pix, int weighting, const float *vis, int n_units,
                                           const int32_t *units, float *rows, int32_t *stats) {
   using namespace blink;
   if (!cell || !vis || !rows || !units || n_bl < 1 || n_units < 0 || (weighting != BLINK_NATURAL && weighting != BLINK_UNIFORM))
     return BLINK_EINVAL;
-  constexpr int N = kRN;
+  if (n_pix != 1024 && n_pix != 2048 && n_pix != 4096) return BLINK_EUNSUPPORTED;
+  const int N = n_pix;
   HostGather g;
   int rc = build_gather_host(cell, n_bl, N, g);
   if (rc != BLINK_OK) return rc;
@@ -699,8 +701,11 @@ extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int wei
   }
   const double norm = weighting == BLINK_NATURAL ? (double)wsum : (double)n_occ;
   const float inv_norm = norm > 0.0 ? (float)(1.0 / norm) : 0.f;
+  std::vector<int16_t> cols;
+  const RGeom gm = N == kRN ? geom_1024() : geom_cols(std::vector<HostGather>{g}, N, cols);
+  const int W = 1 << gm.logw, ROWS = gm.rows, n_classes = N / ROWS, len_sh = gm.logn + 2 + gm.logw;
   RTables tb;
-  res_tables(g, geom_1024(), weighting, inv_norm, tb);
+  res_tables(g, gm, weighting, inv_norm, tb);
   if (!tb.ok) return BLINK_EUNSUPPORTED;
   typedef std::complex<double> cd;
   const double tau = 6.283185307179586476925286766559;
@@ -713,7 +718,7 @@ extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int wei
     cv[w].assign((size_t)32 * tb.L[w], cd(0.0, 0.0));
     for (size_t i = 0; i < cv[w].size(); ++i) {
       const uint4 r = tb.rec[w][i];
-      const int flag = (r.x >> 10) & 3, len = (int)(r.x >> 21);
+      const int flag = (r.x >> gm.logn) & 3, len = (int)(r.x >> len_sh);
       if (len == 0) continue;
       float wt;
       memcpy(&wt, &r.y, 4);
@@ -731,10 +736,14 @@ extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int wei
   }
   if (stats) { stats[0] = npos; stats[1] = lmax; stats[2] = g.n_can; }
   const double nan = std::nan("");
-  std::vector<cd> tile((size_t)kRRows * kRW), Z(N);
+  const uint32_t angle_mask = ~0u << (32 - gm.logn);
+  std::vector<cd> tile((size_t)ROWS * W), Z(N);
+  // the kernels' column ownership: k_img1024r warp w, lane b: column 32 ((w + b) mod 16) + b; k_cols_res: the dealt table
+  auto column_of = [&](int w, int b, int j) { return N == kRN ? 32 * ((w + b) & 15) + b : (int)cols[((size_t)w * 32 + b) * 2 + j]; };
+  const int cpl = N == kRN ? 1 : 2;
   for (int iu = 0; iu < n_units; ++iu) {
     const int r = units[iu];
-    if (r < 0 || r >= kRUnits) return BLINK_EINVAL;
+    if (r < 0 || r >= n_classes) return BLINK_EINVAL;
     std::fill(tile.begin(), tile.end(), cd(nan, nan));
     // phase S
     for (int w = 0; w < kRProd; ++w)
@@ -742,7 +751,7 @@ extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int wei
         cd acc(0.0, 0.0);
         for (int q = 0; q < tb.L[w]; ++q) {
           const uint32_t m = tb.meta[w][(size_t)32 * q + l];
-          const int32_t P = (int32_t)((m & 0xFFC00000u) * (uint32_t)r);
+          const int32_t P = (int32_t)((m & angle_mask) * (uint32_t)r);
           const double ang = (double)P * (tau / 4294967296.0);
           acc += cv[w][(size_t)32 * q + l] * cd(cos(ang), sin(ang));
           if (m & 1u) {
@@ -751,36 +760,56 @@ extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int wei
           }
         }
       }
-    // phase A, with the kernel's column ownership (warp w, lane b: column 32 ((w + b) mod 16) + b)
+    // phase A
     for (int w = 0; w < kRProd; ++w)
-      for (int b = 0; b < 32; ++b) {
-        const int k = 32 * ((w + b) & 15) + b;
-        cd t[kRRows], U[kRRows];
-        for (int c = 0; c < kRRows; ++c) t[c] = ((tb.mask[k] >> c) & 1u) ? tile[(size_t)c * kRW + k] : cd(0.0, 0.0);
-        for (int y1 = 0; y1 < kRRows; ++y1) {
+      for (int b = 0; b < 32; ++b)
+        for (int j = 0; j < cpl; ++j) {
+          const int k = column_of(w, b, j);
+          if ((k & 31) != b || gm.owner[k] != w) return BLINK_EINVAL;      // a lane's columns sit in its own bank
+          std::vector<cd> t(ROWS), U(ROWS);
+          for (int c = 0; c < ROWS; ++c) t[c] = ((tb.mask[k] >> c) & 1u) ? tile[(size_t)c * W + k] : cd(0.0, 0.0);
+          for (int y1 = 0; y1 < ROWS; ++y1) {
+            cd a(0.0, 0.0);
+            for (int c = 0; c < ROWS; ++c) a += t[c] * std::polar(1.0, tau * (double)((c * y1) % ROWS) / ROWS);
+            U[y1] = a;
+          }
+          if (N == kRN) {
+            for (int pp = 0; pp < ROWS / 2; ++pp) {
+              const cd A = U[pp], B = U[pp + ROWS / 2];
+              tile[(size_t)pp * W + k] = A + cd(0.0, 1.0) * B;
+              tile[(size_t)(ROWS / 2 + pp) * W + k] = std::conj(A) + cd(0.0, 1.0) * std::conj(B);
+            }
+          } else {
+            for (int y1 = 0; y1 < ROWS; ++y1) tile[(size_t)y1 * W + k] = U[y1];
+          }
+        }
+    if (N == kRN) {
+      // phase B of k_img1024r
+      for (int pr = 0; pr < ROWS / 2; ++pr) {
+        for (int kk = 0; kk < N; ++kk) {
+          if (kk < W) Z[kk] = tile[(size_t)pr * W + kk];
+          else if (kk == W) Z[kk] = cd(0.0, 0.0);
+          else Z[kk] = tile[(size_t)(ROWS / 2 + pr) * W + (N - kk)];
+        }
+        float *r0 = rows + ((size_t)iu * ROWS + pr) * N, *r1 = rows + ((size_t)iu * ROWS + ROWS / 2 + pr) * N;
+        for (int x = 0; x < N; ++x) {
           cd a(0.0, 0.0);
-          for (int c = 0; c < kRRows; ++c) a += t[c] * std::polar(1.0, tau * (double)((c * y1) % kRRows) / kRRows);
-          U[y1] = a;
-        }
-        for (int pp = 0; pp < kRRows / 2; ++pp) {
-          const cd A = U[pp], B = U[pp + kRRows / 2];
-          tile[(size_t)pp * kRW + k] = A + cd(0.0, 1.0) * B;
-          tile[(size_t)(kRRows / 2 + pp) * kRW + k] = std::conj(A) + cd(0.0, 1.0) * std::conj(B);
+          for (int kk = 0; kk < N; ++kk) a += Z[kk] * std::polar(1.0, tau * (double)((kk * x) % N) / N);
+          r0[x] = (float)a.real();      // image row 64 pr + r
+          r1[x] = (float)a.imag();      // image row 64 pr + r + 512
         }
       }
-    // phase B
-    for (int pr = 0; pr < kRRows / 2; ++pr) {
-      for (int kk = 0; kk < N; ++kk) {
-        if (kk < kRW) Z[kk] = tile[(size_t)pr * kRW + kk];
-        else if (kk == kRW) Z[kk] = cd(0.0, 0.0);
-        else Z[kk] = tile[(size_t)(kRRows / 2 + pr) * kRW + (N - kk)];
-      }
-      float *r0 = rows + ((size_t)iu * kRRows + pr) * N, *r1 = rows + ((size_t)iu * kRRows + kRRows / 2 + pr) * N;
-      for (int x = 0; x < N; ++x) {
-        cd a(0.0, 0.0);
-        for (int kk = 0; kk < N; ++kk) a += Z[kk] * std::polar(1.0, tau * (double)((kk * x) % N) / N);
-        r0[x] = (float)a.real();      // image row 64 pr + r
-        r1[x] = (float)a.imag();      // image row 64 pr + r + 512
+    } else {
+      // in place of k_image_rows: I[y][x] = Re U[y][0] + 2 Re sum_{kx > 0} U[y][kx] e^{2 pi i kx x / N}
+      std::vector<cd> ph(N);
+      for (int m = 0; m < N; ++m) ph[m] = std::polar(1.0, tau * (double)m / N);
+      for (int y1 = 0; y1 < ROWS; ++y1) {
+        float *ro = rows + ((size_t)iu * ROWS + y1) * N;       // image row (N / 8) y1 + r
+        for (int x = 0; x < N; ++x) {
+          double a = tile[(size_t)y1 * W].real();
+          for (int kk = 1; kk < W; ++kk) a += 2.0 * (tile[(size_t)y1 * W + kk] * ph[(int)(((long long)kk * x) % N)]).real();
+          ro[x] = (float)a;
+        }
       }
     }
   }

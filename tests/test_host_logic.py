@@ -125,13 +125,40 @@ def test_residue_route_tables_on_host(blink, oracle, weighting):
     assert r["n_dropped"] > 0
     vis = w.vis()
     units = [0, 1, 37, 63]
-    out = blink.host_residue_emulate(r["cell"], wt, vis[0, 0], units)
+    out = blink.host_residue_emulate(r["cell"], w.n_pix, wt, vis[0, 0], units)
     assert out["longest_list"] <= 16 and out["positions"] % 32 == 0
     ref = oracle.image_batch(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, wt, vis, np.array([0], np.int64))["images"][0]
     peak = np.max(np.abs(ref))
     assert len(out["rows"]) == 16 * len(units)
     for y, row in out["rows"].items():
         assert np.max(np.abs(row - ref[y])) <= 2e-6 * peak, f"image row {y}"
+
+
+@pytest.mark.parametrize("n_pix", [2048, 4096])
+def test_residue_column_pass_tables_on_host(blink, oracle, n_pix):
+    """k_cols_res (column pass by residue class at N = 2048 / 4096) walked on the host: tables generic in the
+    grid size (record and descriptor packing, eight bins per column), columns dealt to the warps by cell
+    count with every lane's columns in its own bank, units of eight rows y = (N / 8) y' + r -- against the
+    oracle's literal sums on sampled pixels of the unit's rows."""
+    w = synth.config_mwa2(n_t=1, n_ch=1)
+    if n_pix == 2048:
+        w.n_pix, w.pixscale, w.weighting = 2048, 30.0 * synth.ARCSEC, synth.UNIFORM
+    n = w.n_pix
+    r = oracle.uv_cells(w.ant_enu_m, w.freq_hz[0], n, w.pixscale)
+    vis = w.vis()
+    units = [0, n // 8 - 1, 77]
+    out = blink.host_residue_emulate(r["cell"], n, w.weighting, vis[0, 0], units)
+    assert out["positions"] % 32 == 0 and out["longest_list"] <= 32
+    g_ref, cnt = oracle.grid(r["cell"], r["cell_conj"], vis[0, 0], n)
+    gw, norm = oracle.weight(g_ref, cnt, w.weighting)
+    rng = np.random.default_rng(5)
+    ys = np.array(sorted(out["rows"].keys()))
+    assert len(ys) == 8 * len(units)
+    yx = np.stack([np.repeat(ys, 6), rng.integers(0, n, 6 * len(ys))], axis=1).astype(np.int32)
+    px = oracle.dft2_pixels(gw, norm, yx).real
+    got = np.array([out["rows"][int(y)][int(x)] for y, x in yx])
+    peak = max(np.max(np.abs(px)), abs(oracle.dft2_pixels(gw, norm, np.array([[n // 2, n // 2]], np.int32)).real[0]))
+    assert np.max(np.abs(got - px)) <= 5e-6 * peak
 
 
 def test_fft_stage_algebra_on_host(tmp_path):
