@@ -209,3 +209,51 @@ def test_corrections_fused_into_the_residue_column_pass(torch_cuda, blink):
     plan.apply_corrections(False)
     assert torch.equal(plan.grid_image(v), plain)
     plan.close()
+
+
+@pytest.mark.parametrize("seed", [11, 12])
+def test_residue_routes_on_random_arrays(torch_cuda, blink, seed):
+    """The residue-class kernels (k_img1024r, k_cols_res) against the line kernels (warp_route = -1) on every
+    pixel, for randomly drawn arrays: centrally condensed layouts of 24..128 antennas, some with a regular
+    sub-array (many baselines per cell), pixel scales that put the longest baselines at 0.6..4 times the grid
+    edge (dropped baselines), 1..3 channels and time steps, both weightings, N = 1024 / 2048 / 4096 -- through
+    blink_grid_image and blink_image.  Configurations the routes do not apply to compare the line kernels
+    with themselves."""
+    torch = torch_cuda
+    rng = np.random.default_rng(seed)
+    applied = 0
+    for _ in range(8):
+        n_pix = int(rng.choice([1024, 1024, 2048, 4096]))
+        n_ant = int(rng.integers(24, 129))
+        ext = float(rng.choice([300.0, 800.0, 1500.0, 3000.0]))
+        rad = np.minimum(rng.exponential(ext / 4, n_ant), ext)
+        phi = rng.uniform(0, 2 * np.pi, n_ant)
+        ant = np.stack([rad * np.cos(phi), rad * np.sin(phi), np.zeros(n_ant)], 1)
+        if rng.random() < 0.3:
+            ant[: n_ant // 4] = np.round(ant[: n_ant // 4] / 40.0) * 40.0
+        n_ch, n_t = int(rng.integers(1, 4)), int(rng.integers(1, 4))
+        f0 = float(rng.choice([120e6, 154e6, 200e6]))
+        freq = f0 + 1e4 * np.arange(n_ch)
+        frac = float(rng.choice([0.6, 0.9, 1.3, 2.5, 4.0]))
+        pixscale = frac * 0.5 / (2 * ext * f0 / 299792458.0)
+        weighting = int(rng.integers(0, 2))
+        n_bl = n_ant * (n_ant - 1) // 2
+        vis = (rng.standard_normal((n_t, n_ch, n_bl)) + 1j * rng.standard_normal((n_t, n_ch, n_bl))).astype(np.complex64)
+        v = torch.from_numpy(vis).cuda()
+        plan0 = blink.Plan(ant, freq, n_pix, pixscale, weighting, options=dict(warp_route=-1))
+        ref, uv = plan0.grid_image(v), plan0.grid(v)
+        ref_uv = plan0.image(uv)
+        plan0.close()
+        plan = blink.Plan(ant, freq, n_pix, pixscale, weighting)
+        applied += plan.query_i32(blink.Q_WARP_KERNEL) in (2, 3)
+        img = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+        plan.grid_image(v, img)
+        img_uv = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda")
+        plan.image(uv, img_uv)
+        plan.close()
+        peak = ref.abs().amax(dim=(-2, -1), keepdim=True).clamp_min(1e-30)
+        assert torch.isfinite(img).all() and torch.isfinite(img_uv).all()
+        assert ((img - ref).abs() <= 1e-5 * peak).all() and ((img_uv - ref_uv).abs() <= 1e-5 * peak).all()
+        del v, ref, uv, ref_uv, img, img_uv
+        torch.cuda.empty_cache()
+    assert applied >= 3
