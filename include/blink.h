@@ -274,20 +274,23 @@ int blink_dynspec(const blink_plan *plan, const void *images, int n_t, double al
  *     |k| < 128 (a compact array on a large image) as 2 x 2 / 4 x 4 interleaved 256^2 sub-images of
  *     the same cell sums (polyphase split of the inverse DFT: each sub-image is the 256^2 transform
  *     of the grid times a unit-modulus factor per cell);
- *   - warp-per-transform route (BLINK_Q_FUSED_PATH == 2; N = 1024 with a wide, sparsely filled
- *     half-plane, e.g. MWA): one cooperative launch in which one group of CTAs forms the column
- *     transforms as sparse sums straight from the visibilities and a second group runs the row
- *     transforms behind it; the intermediate U lives in a 32 MB ring of plan-owned scratch that
- *     stays in L2;
- *   - two-kernel route (BLINK_Q_FUSED_PATH == 0): the column transforms are fed straight from the visibilities through the
- *     plan's cell-sorted tables (each occupied cell sums its own baselines in ascending order), the
- *     row transforms follow; only the half-plane intermediate U passes through plan-owned scratch,
- *     in chunks of BLINK_Q_FUSED_CHUNK snapshots sized to stay L2-resident.
+ *   - residue-class route (BLINK_Q_FUSED_PATH == 2; N = 1024 with a wide, sparsely filled half-plane,
+ *     e.g. MWA; BLINK_Q_WARP_KERNEL says which kernel): one kernel; the image rows are dealt by y mod 64,
+ *     a class's 16 x 512 intermediate lives in shared memory between the warps that form it from the
+ *     plan's occupied cells and the warps that run the row transforms -- no scratch.  Planes with more
+ *     cells than fit the SM take the ring kernel instead: one cooperative launch, column-pass CTAs feeding
+ *     row-pass CTAs through a 32 MB ring of plan-owned scratch that stays in L2;
+ *   - two-kernel route (BLINK_Q_FUSED_PATH == 0): the column transforms are fed straight from the
+ *     visibilities through the plan's cell-sorted tables (each occupied cell sums its own baselines in
+ *     ascending order; at N = 2048 / 4096 with a sparse half-plane at most 1024 columns wide by residue
+ *     class as above), the row transforms follow; only the half-plane intermediate U passes through
+ *     plan-owned scratch, in chunks of BLINK_Q_FUSED_CHUNK snapshots (up to 2 GB).
  *   vis     DEVICE complex64 [n_t][n_ch][n_bl]; 16-byte aligned base (BLINK_EINVAL otherwise: the routes
  *           read it with bulk asynchronous copies)
  *   images  DEVICE float32   [n_t][n_ch][N][N]
- * Asynchronous on `stream`; no allocation, no host synchronisation.  The shared-memory route needs no
- * scratch; the other two need blink_plan_reserve(plan, n_t) beforehand (BLINK_ERESERVE otherwise).
+ * Asynchronous on `stream`; no allocation, no host synchronisation.  The shared-memory route and the
+ * residue-class kernel need no scratch; the others need blink_plan_reserve(plan, n_t) beforehand
+ * (BLINK_ERESERVE otherwise).
  */
 int blink_grid_image(const blink_plan *plan, const void *vis, int n_t, void *images, void *stream);
 
