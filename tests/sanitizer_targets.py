@@ -7,7 +7,9 @@
 CTAs, so every CTA of k_fused hands its chunk ring and its aliased line buffers from one snapshot to
 the next (also with the correction factors riding in the chunks); (3) blink_grid on the ring route;
 (4) blink_grid_image on the warp-per-transform route (k_img1024) with a ring of 2 slots of U for 6
-snapshots, so pass A waits on pass B through the global counters; (5) blink_dynspec.  Each result is
+snapshots, so pass A waits on pass B through the global counters; (5) blink_dynspec; (6) the residue-class
+kernels: k_img1024r (producer / consumer warps over a ring of two tiles, CTAs changing snapshot mid-run) and
+k_cols_res at 2048^2 (tiles leaving as bulk copies while the next unit is formed).  Each result is
 checked against the two-call route so a silent corruption would also fail here.  Not collected by
 pytest (no test_ prefix): the sanitizer slows these kernels 10-100 x."""
 import os
@@ -53,6 +55,21 @@ def main():
     img = plan.grid_image(vis)                      # twice: the kernel must leave its counters zero
     plan0 = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=dict(warp_route=-1))
     ref = plan0.grid_image(vis)
+    assert ((img - ref).abs() <= 1e-5 * ref.abs().amax(dim=(-2, -1), keepdim=True)).all()
+    # (6): k_img1024r on the same six snapshots (384 units over 148 CTAs), then k_cols_res at 2048^2
+    plan1 = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    assert plan1.query_i32(blink.Q_WARP_KERNEL) == 2
+    img = plan1.grid_image(vis)
+    assert ((img - ref).abs() <= 1e-5 * ref.abs().amax(dim=(-2, -1), keepdim=True)).all()
+    for pl in (plan, plan0, plan1):
+        pl.close()
+    w = synth.config_mwa2(n_t=1, n_ch=2)
+    w.n_pix, w.pixscale = 2048, 30.0 * synth.ARCSEC
+    vis = torch.from_numpy(w.vis()).cuda()
+    plan = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    assert plan.query_i32(blink.Q_WARP_KERNEL) == 3
+    plan0 = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=dict(warp_route=-1))
+    img, ref = plan.grid_image(vis), plan0.grid_image(vis)
     assert ((img - ref).abs() <= 1e-5 * ref.abs().amax(dim=(-2, -1), keepdim=True)).all()
     torch.cuda.synchronize()
     print("sanitizer targets ok")
