@@ -535,7 +535,7 @@ def main():
     if not args.no_e2e:
         img_h = torch.empty(shape, dtype=torch.float32).pin_memory()
         if fused:
-            plan.reserve_host(max(1, -(-w.n_t // 8)))
+            plan.reserve_host(0)                 # the plan's own chunk: about 32 MiB each way
 
             def e2e_step():
                 plan.grid_image_host(vis_h, img_h)

@@ -313,7 +313,8 @@ int blink_grid_image_host(blink_plan *plan, const void *vis_host, int n_t, void 
 
 /* allocates the staging of blink_grid_image_host for chunks of chunk_t time steps (three buffers of
  * chunk_t x (8 n_ch n_bl + 4 n_ch N^2) bytes, streams, events) and blink_grid_image's own scratch for such a
- * chunk; synchronises the device when it has to grow; never shrinks */
+ * chunk; synchronises the device when it has to grow; never shrinks.  chunk_t = 0: the plan picks the chunk
+ * (about 32 MiB each way) unless one is reserved already */
 int blink_plan_reserve_host(blink_plan *plan, int chunk_t);
 
 /*

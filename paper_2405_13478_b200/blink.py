@@ -417,15 +417,16 @@ class Plan:
         return images
 
     def reserve_host(self, chunk_t: int):
-        """blink_plan_reserve_host: staging of grid_image_host for chunks of chunk_t time steps."""
+        """blink_plan_reserve_host: staging of grid_image_host for chunks of chunk_t time steps (0: the plan
+        picks the chunk, about 32 MiB each way)."""
         _check(self._lib.blink_plan_reserve_host(self._h, int(chunk_t)), "blink_plan_reserve_host")
-        self._host_chunk_t = max(self._host_chunk_t, int(chunk_t))
+        self._host_chunk_t = max(self._host_chunk_t, int(chunk_t), 1)
         self._reserved_n_t = max(self._reserved_n_t, int(chunk_t))
 
     def grid_image_host(self, vis_h, images_h, stream=None):
         """blink_grid_image_host: vis_h complex64 CPU tensor [n_t, n_ch, n_bl] (pinned for overlap) ->
         images_h float32 CPU tensor [n_t, n_ch, N, N]; asynchronous on the stream (synchronise it before
-        reading images_h).  Without an earlier reserve_host the chunk is ~1/8 of the batch."""
+        reading images_h).  Without an earlier reserve_host the plan picks the chunk (reserve_host(0))."""
         import torch
         assert not vis_h.is_cuda and vis_h.dtype == torch.complex64 and vis_h.is_contiguous()
         n_t = vis_h.shape[0]
@@ -433,7 +434,7 @@ class Plan:
         assert not images_h.is_cuda and images_h.dtype == torch.float32 and images_h.is_contiguous()
         assert tuple(images_h.shape) == (n_t, self.n_ch, self.n_pix, self.n_pix)
         if self._host_chunk_t == 0:
-            self.reserve_host(max(1, -(-n_t // 8)))
+            self.reserve_host(0)
         _check(self._lib.blink_grid_image_host(self._h, vis_h.data_ptr(), n_t, images_h.data_ptr(),
                                                _stream_ptr(stream)), "blink_grid_image_host")
         return images_h

@@ -523,17 +523,19 @@ def test_grid_image_host_matches_device_path(torch_cuda, blink):
     torch.cuda.synchronize()
     assert torch.equal(img_p, ref)
     plan.close()
-    # a route that needs plan scratch (two kernels) behind the same call
-    w = synth.config_mwa1(n_t=3, n_ch=2)
-    vis_h = torch.from_numpy(w.vis()).pin_memory()
-    plan = _plan(blink, w)
-    ref = plan.grid_image(vis_h.cuda()).cpu()
-    img_h = torch.full(tuple(ref.shape), float("nan"), dtype=torch.float32).pin_memory()
-    plan.reserve_host(2)
-    plan.grid_image_host(vis_h, img_h)
-    torch.cuda.synchronize()
-    assert torch.equal(img_h, ref)
-    plan.close()
+    # the residue-class kernel, and a route that needs plan scratch (two kernels), behind the same call; the first
+    # with the chunk the plan picks itself (blink_plan_reserve_host(plan, 0): one time step here)
+    for options, chunk_t in ((dict(), 0), (dict(warp_route=-1), 2)):
+        w = synth.config_mwa1(n_t=3, n_ch=2)
+        vis_h = torch.from_numpy(w.vis()).pin_memory()
+        plan = _plan(blink, w, **options)
+        ref = plan.grid_image(vis_h.cuda()).cpu()
+        img_h = torch.full(tuple(ref.shape), float("nan"), dtype=torch.float32).pin_memory()
+        plan.reserve_host(chunk_t)
+        plan.grid_image_host(vis_h, img_h)
+        torch.cuda.synchronize()
+        assert torch.equal(img_h, ref)
+        plan.close()
 
 
 def test_boundary_contracts(torch_cuda, blink, oracle):
