@@ -49,8 +49,10 @@ typedef enum blink_status {
   BLINK_ENOMEM = -2, /* host or device allocation failed */
   BLINK_ECUDA = -3,  /* CUDA runtime error or no device (see blink_last_cuda_error) */
   BLINK_EUNSUPPORTED = -4, /* valid request outside what this build implements */
-  BLINK_ERESERVE = -5 /* the plan's device scratch is too small for this n_t: call blink_plan_reserve(plan, n_t)
-                         first (hot calls never allocate) */
+  BLINK_ERESERVE = -5, /* the plan's device scratch is too small for this n_t: call blink_plan_reserve(plan, n_t)
+                          first (hot calls never allocate) */
+  BLINK_ECAPACITY = -6 /* the request does not fit the fixed, built-in scratch of blink_image_static
+                          (BLINK_STATIC_SCRATCH_BYTES); nothing was launched */
 } blink_status;
 
 typedef enum blink_weighting {
@@ -202,6 +204,54 @@ int blink_grid(const blink_plan *plan, const void *vis, int n_t, void *uv_grid, 
  * larger one) beforehand, else BLINK_ERESERVE.
  */
 int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *images, void *stream);
+
+/*
+ * blink_image_static -- blink_image for callers that are not allowed to allocate device memory.
+ *
+ * Who that is.  blink_image keeps the intermediate U of its two passes in plan scratch, and that scratch
+ * only exists after blink_plan_reserve, which calls cudaMalloc (and, when it has to grow, synchronises the
+ * whole device and calls cudaFree).  Some users of an imager like this one cannot make that call at the
+ * point where they need images: a real-time ingest loop behind a correlator, where a device-wide stall
+ * from the allocator means dropped telescope data; a process that shares the GPU with a component (a
+ * correlator ring buffer, a framework's caching pool) which has already claimed the memory, so a later
+ * cudaMalloc may simply fail; code that runs under a "no driver allocation after start-up" rule.  For them
+ * this call images with an intermediate that was never allocated at run time: it lives in an array
+ * compiled into the library, BLINK_STATIC_SCRATCH_BYTES (32 MiB) of device memory that every GPU which
+ * loads libblink's imaging module holds until the process exits, whether or not this call is ever used.
+ *
+ * What it computes.  Exactly blink_image: same arguments, same layouts, same input contract on uv_grid,
+ * same arithmetic -- the two line kernels of blink_image (column pass, row pass) pointed at the built-in
+ * array instead of plan scratch, whatever route the plan would pick for blink_image itself.  For a plan
+ * whose blink_image runs the line kernels the images are bit-identical; for the other routes (N = 1024
+ * residue-class / ring kernels, N >= 2048 residue-class column pass) they agree to fp32 rounding order
+ * and both meet the oracle bar (1e-4 of the image peak).  The batch is cut into launch pairs of
+ * floor(BLINK_STATIC_SCRATCH_BYTES / (8 N wu)) snapshots, wu = the plan's half-plane width (kx_max over
+ * all channels + 1, rounded up to 16), so any n_t is accepted.
+ *
+ * The limit.  One snapshot's U (8 N wu bytes) must fit the array, else BLINK_ECAPACITY and nothing is
+ * launched; blink_last_cuda_error() then holds a sentence with both numbers.  Every plan with N <= 2048
+ * fits; at N = 4096 the half-plane may be at most 1024 columns wide (true of the MWA-shaped workloads).
+ *
+ * No allocation of any kind: no cudaMalloc / cudaFree / cudaMallocAsync, no host allocation, no library
+ * call that allocates.  The plan (an input, created at start-up) needs no blink_plan_reserve for it.
+ *
+ * First call on a device.  It looks up the array's device address (cudaGetSymbolAddress, with that device
+ * current -- the array's name is not a device pointer in host code) and raises the kernels' shared-memory
+ * limit; both are remembered per device.  Make that first call during set-up, and before any stream
+ * capture is begun; later calls only launch.
+ *
+ * Sharing.  There is ONE array per device, shared by every plan, thread and stream of the process, and it
+ * keeps whatever the last call left in it.  Nothing in it has to start at zero (the column pass writes
+ * every element of a chunk's U before the row pass reads it), so stale contents are harmless -- but two
+ * blink_image_static calls that overlap in time on the same GPU (different streams, or different threads
+ * on different streams) overwrite each other's intermediate and both results are garbage: issue all of
+ * them on one stream, or order the streams yourself.  blink_image and the other calls never touch the
+ * array and may overlap with it.
+ *
+ * Asynchronous on `stream`; no host synchronisation.  Errors as blink_image, plus BLINK_ECAPACITY.
+ */
+#define BLINK_STATIC_SCRATCH_BYTES (32u << 20)
+int blink_image_static(const blink_plan *plan, const void *uv_grid, int n_t, void *images, void *stream);
 
 /*
  * blink_plan_set_corrections -- the pre-gridding corrections of PAPER.md section 4.2 (:142-156):

@@ -15,7 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libblink.so")
 
 NATURAL, UNIFORM = 0, 1
-OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ERESERVE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ERESERVE, ECAPACITY = 0, -1, -2, -3, -4, -5, -6
+STATIC_SCRATCH_BYTES = 32 << 20     # BLINK_STATIC_SCRATCH_BYTES
 (Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
  Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK, Q_CORR, Q_CORR_FUSED,
  Q_TENSOR_ROUTE, Q_WARP_KERNEL) = range(20)
@@ -25,7 +26,7 @@ EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_pl
            "blink_plan_destroy", "blink_plan_query", "blink_plan_read", "blink_plan_reserve",
            "blink_grid", "blink_grid_image", "blink_plan_set_corrections", "blink_correct", "blink_dynspec",
            "blink_image", "blink_grid_validate", "blink_grid_image_host", "blink_plan_reserve_host",
-           "blink_plan_apply_corrections", "blink_plan_refresh"]
+           "blink_plan_apply_corrections", "blink_plan_refresh", "blink_image_static"]
 TESTING_EXPORTS = ["blink_host_build_gather", "blink_host_fused_emulate", "blink_host_residue_emulate", "blink_probe_fp32"]
 
 
@@ -98,6 +99,8 @@ def load() -> ctypes.CDLL:
     lib.blink_grid.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_image.restype = ci
     lib.blink_image.argtypes = [vp, vp, ci, vp, vp]
+    lib.blink_image_static.restype = ci
+    lib.blink_image_static.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_grid_image.restype = ci
     lib.blink_grid_image.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_plan_set_corrections.restype = ci
@@ -398,6 +401,24 @@ class Plan:
         self._ensure_reserved(n_t, auto_reserve)
         _check(self._lib.blink_image(self._h, uv_grid.data_ptr(), n_t, images.data_ptr(),
                                      _stream_ptr(stream)), "blink_image")
+        return images
+
+    def image_static(self, uv_grid, images, stream=None):
+        """blink_image_static: blink_image for a caller that must not allocate device memory (a real-time
+        loop that cannot take cudaMalloc's stall, a GPU whose memory is already spoken for).  The
+        intermediate of the two passes lives in a 32 MiB array built into libblink.so instead of plan
+        scratch, so no reserve() is needed and none is made; `images` is required because this wrapper
+        does not allocate either.  BlinkError with status ECAPACITY when one snapshot's intermediate
+        (8 N wu bytes) exceeds the array.  One array per GPU, shared by every plan: calls that overlap
+        on the device corrupt each other, keep them on one stream."""
+        import torch
+        assert uv_grid.is_cuda and uv_grid.dtype == torch.complex64 and uv_grid.is_contiguous()
+        n_t = uv_grid.shape[0]
+        assert tuple(uv_grid.shape[1:]) == (self.n_ch, self.n_pix, self.n_pix)
+        assert images.is_cuda and images.dtype == torch.float32 and images.is_contiguous()
+        assert tuple(images.shape) == (n_t, self.n_ch, self.n_pix, self.n_pix)
+        _check(self._lib.blink_image_static(self._h, uv_grid.data_ptr(), n_t, images.data_ptr(),
+                                            _stream_ptr(stream)), "blink_image_static")
         return images
 
     def grid_image(self, vis, images=None, stream=None, auto_reserve=True):

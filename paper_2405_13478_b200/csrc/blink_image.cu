@@ -15,6 +15,7 @@
 // U lives in a small plan-owned scratch (two-pass path) sized to stay L2-resident between the two
 // launches of a chunk of snapshots.
 #include <algorithm>
+#include <cstdio>
 
 #include "blink_internal.h"
 #include "fft_core.cuh"
@@ -434,7 +435,118 @@ int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, fl
   return launch_image_impl(p, nullptr, vis, n_snap, 0, img, st);
 }
 
+// ------------------------------------------------------------------------------------------
+// blink_image_static (blink.h): the line kernels above with their intermediate U in memory that nobody
+// allocates at run time.  For callers who may not enter the CUDA allocator when they need images (a
+// real-time loop that cannot afford cudaMalloc's device-wide stall, a GPU whose memory another component
+// already owns, a "no allocation after start-up" rule): the scratch is part of the library image.
+//
+// The array is a device object; in HOST code its name is only a handle the runtime maps to an address.
+// Passing `g_static_U` itself to a kernel would hand it a host-side pointer (a fault, or -- where the GPU
+// can reach host memory -- silent use of the wrong bytes), so the launcher asks the runtime for the real
+// device address once per device and passes that.
+static __device__ __align__(256) unsigned char g_static_U[BLINK_STATIC_SCRATCH_BYTES];
+
+constexpr int kStaticMaxDevices = 64;
+static std::atomic<float2 *> g_static_U_addr[kStaticMaxDevices];   // device address of g_static_U, per device ordinal
+
+// set-up, once per device, with that device current: cudaGetSymbolAddress resolves the symbol in the
+// CURRENT device's copy of the module.  Two threads racing here both get the same answer.
+static int static_scratch_addr(int device, float2 **out) {
+  if (device < 0 || device >= kStaticMaxDevices) return BLINK_EUNSUPPORTED;
+  float2 *a = g_static_U_addr[device].load(std::memory_order_acquire);
+  if (a == nullptr) {
+    void *ptr = nullptr;
+    BLINK_CUDA_TRY(cudaGetSymbolAddress(&ptr, g_static_U), "blink_image_static: cudaGetSymbolAddress(g_static_U)");
+    if (ptr == nullptr) return BLINK_ECUDA;
+    a = static_cast<float2 *>(ptr);
+    g_static_U_addr[device].store(a, std::memory_order_release);
+  }
+  *out = a;
+  return BLINK_OK;
+}
+
+template <int N, int CT, int RP>
+static int run_image_static_cfg(const blink_plan *p, ImgParams ip, int n_snap, int chunk, cudaStream_t st) {
+  using C = ImgCfg<N>;
+  const size_t smem_a = sizeof(cf32) * CT * C::LS, smem_b = sizeof(cf32) * RP * C::LS;
+  if (std::max(smem_a, smem_b) > (size_t)p->max_smem_optin) return BLINK_EUNSUPPORTED;
+  // per-device kernel attributes: part of the first call's set-up, like the address above
+  static std::atomic<uint64_t> attr_a{0}, attr_b{0}, attr_b4{0};
+  int rc = ensure_max_smem(k_image_cols<N, CT>, p, attr_a, "k_image_cols smem attribute");
+  if (rc == BLINK_OK) rc = ensure_max_smem(k_image_rows<N, RP>, p, attr_b, "k_image_rows smem attribute");
+  constexpr bool kNarrow = N >= 2048;
+  const bool narrow = kNarrow && p->kx_max_all < N / 4;
+  if constexpr (kNarrow)
+    if (rc == BLINK_OK && narrow) rc = ensure_max_smem(k_image_rows<N, RP, 4>, p, attr_b4, "k_image_rows smem attribute");
+  if (rc != BLINK_OK) return rc;
+  for (int base = 0; base < n_snap; base += chunk) {   // stream order keeps a pair's row pass ahead of the next column pass
+    const int cs = std::min(chunk, n_snap - base);
+    ip.snap_base = base;
+    k_image_cols<N, CT><<<dim3(p->wu / CT, cs), CT * C::T, smem_a, st>>>(ip);
+    if constexpr (kNarrow) {
+      if (narrow) k_image_rows<N, RP, 4><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
+      else k_image_rows<N, RP><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
+    } else {
+      k_image_rows<N, RP><<<dim3(N / 2 / RP, cs), RP * C::T, smem_b, st>>>(ip);
+    }
+  }
+  BLINK_CUDA_TRY(cudaGetLastError(), "blink_image_static launch");
+  return BLINK_OK;
+}
+
+// the default tile shapes of run_image_n (no tuning slots: this entry point has one configuration per N)
+template <int N> static int run_image_static_n(const blink_plan *p, const ImgParams &ip, int n_snap, int chunk, cudaStream_t st) {
+  using C = ImgCfg<N>;
+  if constexpr (N == 1024) return run_image_static_cfg<N, 8, 2>(p, ip, n_snap, chunk, st);
+  else if constexpr (N == 512) return run_image_static_cfg<N, 8, 8>(p, ip, n_snap, chunk, st);
+  else if constexpr (N <= 256) return run_image_static_cfg<N, 16, ((N / 2) < (256 / C::T) ? (N / 2) : (256 / C::T))>(p, ip, n_snap, chunk, st);
+  else return run_image_static_cfg<N, C::CT_MAX, (256 / C::T > 0 ? 256 / C::T : 1)>(p, ip, n_snap, chunk, st);
+}
+
+static int launch_image_static(const blink_plan *p, const float2 *uv, int n_snap, float *img, cudaStream_t st) {
+  const size_t per_snap = sizeof(float2) * (size_t)p->n_pix * p->wu;
+  if (per_snap > (size_t)BLINK_STATIC_SCRATCH_BYTES) {
+    char msg[200];
+    snprintf(msg, sizeof msg, "blink_image_static: one snapshot's intermediate is %zu bytes (8 x N = %d x wu = %d), "
+             "the built-in scratch holds %u", per_snap, p->n_pix, p->wu, (unsigned)BLINK_STATIC_SCRATCH_BYTES);
+    set_error_text(msg);
+    return BLINK_ECAPACITY;
+  }
+  float2 *U = nullptr;
+  int rc = static_scratch_addr(p->device, &U);
+  if (rc != BLINK_OK) return rc;
+  // a chunk's snapshots are the launch's gridDim.y: at most 65535
+  const int chunk = (int)std::min<size_t>(65535, (size_t)BLINK_STATIC_SCRATCH_BYTES / per_snap);
+  ImgParams ip = {};
+  ip.uv = uv; ip.img = img; ip.U = U; ip.chinfo = p->d_chinfo;
+  ip.wkey = p->d_wkey; ip.wval = p->d_wval; ip.wcol = p->d_wcol; ip.n_bl = p->n_bl;
+  ip.tw = p->d_tw; ip.n_ch = p->n_ch; ip.wu = p->wu; ip.uniform = p->weighting == BLINK_UNIFORM;
+  ip.snap_base = 0; ip.ch0 = 0;
+  switch (p->n_pix) {
+    case 32: return run_image_static_n<32>(p, ip, n_snap, chunk, st);
+    case 64: return run_image_static_n<64>(p, ip, n_snap, chunk, st);
+    case 128: return run_image_static_n<128>(p, ip, n_snap, chunk, st);
+    case 256: return run_image_static_n<256>(p, ip, n_snap, chunk, st);
+    case 512: return run_image_static_n<512>(p, ip, n_snap, chunk, st);
+    case 1024: return run_image_static_n<1024>(p, ip, n_snap, chunk, st);
+    case 2048: return run_image_static_n<2048>(p, ip, n_snap, chunk, st);
+    case 4096: return run_image_static_n<4096>(p, ip, n_snap, chunk, st);
+    default: return BLINK_EUNSUPPORTED;
+  }
+}
+
 }  // namespace blink
+
+extern "C" int blink_image_static(const blink_plan *plan, const void *uv_grid, int n_t, void *images, void *stream) {
+  if (!plan || n_t < 0) return BLINK_EINVAL;
+  if (n_t == 0) return BLINK_OK;
+  if (!uv_grid || !images) return BLINK_EINVAL;
+  if (((uintptr_t)uv_grid & 7) || ((uintptr_t)images & 3)) return BLINK_EINVAL;
+  int rc = check_device(plan);
+  if (rc != BLINK_OK) return rc;
+  return blink::launch_image_static(plan, (const float2 *)uv_grid, n_t * plan->n_ch, (float *)images, (cudaStream_t)stream);
+}
 
 extern "C" int blink_image(const blink_plan *plan, const void *uv_grid, int n_t, void *images, void *stream) {
   if (!plan || n_t < 0) return BLINK_EINVAL;

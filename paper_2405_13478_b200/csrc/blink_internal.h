@@ -232,6 +232,7 @@ int launch_cols_res(const blink_plan *p, const ImgParams &ip, int n_snap, cudaSt
 namespace blink {
 
 void set_cuda_error(cudaError_t e, const char *where);
+void set_error_text(const char *text);   // a non-CUDA explanation, read back through blink_last_cuda_error
 void host_pipe_free(blink_plan *p);
 int build_gather_host(const int32_t *cell, int n_bl, int n_pix, HostGather &out);
 

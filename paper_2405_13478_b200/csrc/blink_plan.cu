@@ -21,6 +21,8 @@ void set_cuda_error(cudaError_t e, const char *where) {
   cudaGetLastError();  // clear sticky-free errors
 }
 
+void set_error_text(const char *text) { g_cuda_err = text; }
+
 // ------------------------------------------------------------------------------------------
 // K0: one thread per (channel, baseline).  Operation order is part of the contract (blink.h
 // "Cell rule"): fp64, round-to-nearest intrinsics so that no FMA contraction can occur.
@@ -230,6 +232,7 @@ extern "C" const char *blink_strerror(int status) {
     case BLINK_ECUDA: return "CUDA error or no CUDA device";
     case BLINK_EUNSUPPORTED: return "not supported by this build";
     case BLINK_ERESERVE: return "plan scratch too small for this n_t: call blink_plan_reserve first";
+    case BLINK_ECAPACITY: return "one snapshot's intermediate exceeds the built-in scratch of blink_image_static";
     default: return "unknown status";
   }
 }
