@@ -394,6 +394,10 @@ int image_reserve(blink_plan *p, int n_t) {
     // the route's completion counters follow the ring; the kernel leaves them zero behind itself
     const size_t ring = warp_route_ring_bytes(p);
     BLINK_CUDA_TRY(cudaMemset(reinterpret_cast<unsigned char *>(p->d_scratch) + ring, 0, need - ring), "scratch counters");
+    // cudaMemset on device memory may return before the fill has run, and it runs on the legacy default
+    // stream: a k_img1024 launch on a non-blocking stream (the host pipe's, a torch side stream) is not
+    // ordered after it.  Reserve is allowed to synchronise; the hot call is not.
+    BLINK_CUDA_TRY(cudaDeviceSynchronize(), "scratch counters sync");
     p->warp_snap_cap = n_snap;
   }
   return BLINK_OK;

@@ -407,7 +407,15 @@ int launch_img1024(const blink_plan *p, ImgParams ip, int n_snap, cudaStream_t s
   if (rc != BLINK_OK) return rc;
   void *args[] = {(void *)&q};
   // cooperative: the item sequences are dealt statically, so every CTA of the grid must be resident
-  BLINK_CUDA_TRY(cudaLaunchCooperativeKernel((const void *)k_img1024, dim3(grid), dim3(kWThreads), args, smem, st), "k_img1024 launch");
+  const cudaError_t le = cudaLaunchCooperativeKernel((const void *)k_img1024, dim3(grid), dim3(kWThreads), args, smem, st);
+  if (le != cudaSuccess) {
+    // the kernel is the only thing that returns its counters to zero; after a launch that did not go
+    // through, put them back on this stream so the next call does not start from whatever they hold
+    set_cuda_error(le, "k_img1024 launch");
+    cudaMemsetAsync(cnt, 0, p->scratch_bytes - ring_bytes, st);
+    cudaGetLastError();
+    return BLINK_ECUDA;
+  }
   return BLINK_OK;
 }
 
