@@ -154,11 +154,21 @@ int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m, int n_ant,
  * with hour angle).  Same n_ant, frequencies, grid, weighting and options as at
  * creation; runs the fp64 index kernel on the device and rebuilds every table (host cores, one channel
  * per thread), then swaps them in, so afterwards the plan is indistinguishable from a new plan of the new
- * coordinates (bit-exact indices, counts and images) while its scratch and host staging survive.
+ * coordinates (bit-exact indices, counts and images), with scratch for the n_t reserved before and the
+ * host staging kept.
  *   ant_enu_m  HOST [n_ant][3], the coordinates whose differences are the new baselines
- * Synchronises the device (work queued on the old tables finishes first).  Drops the correction table
- * (it depends on the geometry): call blink_plan_set_corrections / blink_plan_apply_corrections again.
- * On error the plan is unchanged.
+ * Synchronises the device (work queued on the old tables finishes first).  Allocates: the new tables and
+ * the new scratch exist beside the old ones until the swap.  On error (BLINK_ENOMEM included) the plan is
+ * unchanged: nothing is swapped in unless everything, scratch included, could be built.
+ * Corrections: the factor table depends on the geometry and is dropped.  If the plan was applying it at
+ * load (blink_plan_apply_corrections on), blink_grid / blink_grid_image / blink_grid_image_host return
+ * BLINK_EINVAL after the refresh -- they do not quietly grid uncorrected data -- until the caller calls
+ * blink_plan_set_corrections + blink_plan_apply_corrections(plan, 1) again, or
+ * blink_plan_apply_corrections(plan, 0) to say that uncorrected is what it wants.
+ * Cost and cadence: the table packing runs on the host cores, about 0.13 s for the 256-antenna, 32-channel
+ * station plan (0.17 s to create it) -- meant for a refresh every few seconds of data or slower (a tracking
+ * array's cells move by a fraction of a cell per second), not once per batch: a 100-step station batch
+ * images in 0.4 ms.
  */
 int blink_plan_refresh(blink_plan *plan, const double *ant_enu_m, void *stream);
 

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libblink.so")
 SOURCES = ["blink_plan.cu", "blink_grid.cu", "blink_image.cu", "blink_image_w.cu", "blink_image_r.cu", "blink_fused.cu", "blink_fused_d4.cu", "blink_fused_tc.cu", "blink_correct.cu", "blink_dynspec.cu", "blink_probe.cu", "blink_host.cu"]
-HEADERS = ["blink_internal.h", "fft_core.cuh", "sphase.cuh", "sgather.cuh", "wfft.cuh", "fused_kernel.cuh", "fused_tc_kernel.cuh", os.path.join("..", "..", "include", "blink.h"),
+HEADERS = ["blink_internal.h", "parallel_for.h", "fft_core.cuh", "sphase.cuh", "sgather.cuh", "wfft.cuh", "fused_kernel.cuh", "fused_tc_kernel.cuh", os.path.join("..", "..", "include", "blink.h"),
            os.path.join("..", "..", "include", "blink_testing.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "--expt-extended-lambda", "--expt-relaxed-constexpr"]

@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(256) k_correct1(const float2 *__restrict__ in,
 }  // namespace blink
 
 extern "C" int blink_plan_set_corrections(blink_plan *p, const double *gains, const double *cable_len_m,
-                                          double l0, double m0, void *stream) {
+                                          double l0, double m0, void *stream) try {
   using namespace blink;
   if (!p) return BLINK_EINVAL;
   const double r2 = l0 * l0 + m0 * m0;
@@ -163,6 +163,11 @@ extern "C" int blink_plan_set_corrections(blink_plan *p, const double *gains, co
   }
   p->d_corr = d_F;
   return BLINK_OK;
+} catch (const std::bad_alloc &) {
+  return BLINK_ENOMEM;                      // host tables; the plan keeps the state it had
+} catch (...) {
+  blink::set_error_text("blink_plan_set_corrections: unexpected C++ exception");
+  return BLINK_ECUDA;
 }
 
 extern "C" int blink_correct(const blink_plan *p, const void *vis_in, int n_t, void *vis_out, void *stream) {
@@ -188,7 +193,7 @@ extern "C" int blink_correct(const blink_plan *p, const void *vis_in, int n_t, v
 // bulk-copy routes (the factors of a chunk ride in the same buffer as its visibilities and gather
 // table; their table layouts are built here, on first use), in registers on the others -- so no
 // separate 16-byte-per-visibility pass exists and the visibilities cross HBM once.
-extern "C" int blink_plan_apply_corrections(blink_plan *p, int on, void *stream) {
+extern "C" int blink_plan_apply_corrections(blink_plan *p, int on, void *stream) try {
   using namespace blink;
   if (!p || (on != 0 && on != 1)) return BLINK_EINVAL;
   int rc = check_device(p);
@@ -201,5 +206,11 @@ extern "C" int blink_plan_apply_corrections(blink_plan *p, int on, void *stream)
     if (p->ring_path == 1 && (rc = grid_ring_layout(p, 1, st)) != BLINK_OK) return rc;
   }
   p->corr_on = on;
+  p->corr_stale = 0;                  // the caller has said what it wants after a refresh
   return BLINK_OK;
+} catch (const std::bad_alloc &) {
+  return BLINK_ENOMEM;                      // host tables; the plan keeps the state it had
+} catch (...) {
+  blink::set_error_text("blink_plan_apply_corrections: unexpected C++ exception");
+  return BLINK_ECUDA;
 }

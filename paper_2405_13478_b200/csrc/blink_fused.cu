@@ -345,6 +345,7 @@ extern "C" int blink_grid_image(const blink_plan *plan, const void *vis, int n_t
   if (!vis || !images) return BLINK_EINVAL;
   if (((uintptr_t)vis & 15) || ((uintptr_t)images & 3)) return BLINK_EINVAL;
   int rc = check_device(plan);
+  if (rc == BLINK_OK) rc = check_corrections_current(plan);
   if (rc != BLINK_OK) return rc;
   if (blink::scratch_need(plan, n_t, true) > plan->scratch_bytes) return BLINK_ERESERVE;
   return blink::launch_grid_image(plan, (const float2 *)vis, n_t, (float *)images, (cudaStream_t)stream);

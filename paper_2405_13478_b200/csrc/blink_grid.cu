@@ -464,7 +464,8 @@ extern "C" int blink_grid(const blink_plan *plan, const void *vis, int n_t, void
   if (n_t == 0) return BLINK_OK;
   if (!vis || !uv_grid) return BLINK_EINVAL;
   if (((uintptr_t)vis & 7) || ((uintptr_t)uv_grid & 15)) return BLINK_EINVAL;
-  const int rc = check_device(plan);
+  int rc = check_device(plan);
+  if (rc == BLINK_OK) rc = check_corrections_current(plan);
   if (rc != BLINK_OK) return rc;
   return blink::launch_grid(plan, (const float2 *)vis, n_t * plan->n_ch, 0, (float2 *)uv_grid, (cudaStream_t)stream);
 }

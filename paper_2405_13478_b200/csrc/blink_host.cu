@@ -82,6 +82,7 @@ extern "C" int blink_grid_image_host(blink_plan *p, const void *vis_host, int n_
   if (n_t == 0) return BLINK_OK;
   if (!vis_host || !images_host) return BLINK_EINVAL;
   int rc = check_device(p);
+  if (rc == BLINK_OK) rc = check_corrections_current(p);
   if (rc != BLINK_OK) return rc;
   HostPipe &h = p->hp;
   if (h.chunk_t < 1) return BLINK_ERESERVE;

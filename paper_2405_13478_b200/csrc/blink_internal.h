@@ -90,6 +90,8 @@ struct blink_plan {
   std::vector<double> h_ant, h_freq;
   float2 *d_corr = nullptr;         // [n_ch][n_bl] correction factors F (blink_correct.cu), NULL until set
   int corr_on = 0;                  // 1 = blink_grid / blink_grid_image multiply by F as they load (blink_plan_apply_corrections)
+  int corr_stale = 0;               // 1 = the fused corrections were on when blink_plan_refresh dropped the table: the gridding
+                                    // calls refuse (BLINK_EINVAL) until blink_plan_apply_corrections is called again
   std::vector<blink::HostGather> gathers;   // per-channel cell-sorted tables, kept for lazily built layouts
 
   // per-channel facts (host)
@@ -265,6 +267,15 @@ int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, fl
 
 }  // namespace blink
 
+// gridding calls after a refresh that dropped active corrections: refuse rather than grid uncorrected data
+inline int check_corrections_current(const blink_plan *p) {
+  if (!p->corr_stale) return BLINK_OK;
+  blink::set_error_text("the plan applied corrections at load before blink_plan_refresh dropped their table: call "
+                        "blink_plan_set_corrections and blink_plan_apply_corrections(plan, 1) again, or "
+                        "blink_plan_apply_corrections(plan, 0) to grid uncorrected");
+  return BLINK_EINVAL;
+}
+
 // hot calls: the plan's device must be current
 inline int check_device(const blink_plan *p) {
   int d = -1;
@@ -295,26 +306,4 @@ template <class K> inline int ensure_max_smem(K kern, const blink_plan *p, std::
 }
 }  // namespace blink
 
-namespace blink {
-// plan-time host work is independent per channel (and per chunk): fn(i) for i in [0, n) on the host cores
-template <class F> inline void parallel_for(int n, F fn) {
-  const int hw = (int)std::thread::hardware_concurrency();
-  const int nt = std::min(n, std::max(1, std::min(hw, 32)));
-  if (nt <= 1) {
-    for (int i = 0; i < n; ++i) fn(i);
-    return;
-  }
-  std::atomic<int> next{0};
-  std::vector<std::thread> th;
-  th.reserve(nt);
-  for (int t = 0; t < nt; ++t)
-    th.emplace_back([&] {
-      for (;;) {
-        const int i = next.fetch_add(1);
-        if (i >= n) break;
-        fn(i);
-      }
-    });
-  for (auto &x : th) x.join();
-}
-}  // namespace blink
+#include "parallel_for.h"

@@ -261,7 +261,7 @@ extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int 
 
 extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m, int n_ant,
                                       const double *freq_hz, int n_ch, int n_pix, double pixscale,
-                                      int weighting, void *stream, const blink_options *opts) {
+                                      int weighting, void *stream, const blink_options *opts) try {
   blink_options opt = {};
   if (opts) {
     if (opts->struct_size != (int32_t)sizeof(blink_options)) return BLINK_EINVAL;
@@ -284,6 +284,13 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
   cudaStream_t st = (cudaStream_t)stream;
   blink_plan *p = new (std::nothrow) blink_plan();
   if (!p) return BLINK_ENOMEM;
+  // the half-built plan goes away on every early return below AND when a host table runs out of memory
+  // (std::bad_alloc unwinds through here to the handler at the end of this function)
+  struct Guard {
+    blink_plan *p;
+    void drop() { plan_free(p); p = nullptr; }
+    ~Guard() { if (p) plan_free(p); }
+  } guard{p};
   p->device = dev;
   p->opt = opt;
   p->n_ant = n_ant;
@@ -301,7 +308,7 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
   do {                        \
     int rc__ = (expr);        \
     if (rc__ != BLINK_OK) {   \
-      plan_free(p);           \
+      guard.drop();           \
       return rc__;            \
     }                         \
   } while (0)
@@ -310,7 +317,7 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
     cudaError_t e__ = (expr);               \
     if (e__ != cudaSuccess) {               \
       set_cuda_error(e__, where);           \
-      plan_free(p);                         \
+      guard.drop();                         \
       return BLINK_ECUDA;                   \
     }                                       \
   } while (0)
@@ -332,7 +339,7 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
   if ((rc = dev_alloc(&d_ant, (size_t)3 * n_ant)) || (rc = dev_alloc(&d_freq, (size_t)n_ch)) ||
       (rc = dev_alloc(&d_pi, (size_t)n_bl)) || (rc = dev_alloc(&d_pj, (size_t)n_bl))) {
     cudaFree(d_ant); cudaFree(d_freq); cudaFree(d_pi); cudaFree(d_pj);
-    plan_free(p);
+    guard.drop();
     return rc;
   }
   std::vector<int32_t> h_cell((size_t)n_ch * n_bl);
@@ -347,7 +354,7 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
                        cudaMemcpyDeviceToHost, st));
   step(cudaStreamSynchronize(st));
   cudaFree(d_ant); cudaFree(d_freq); cudaFree(d_pi); cudaFree(d_pj);
-  if (rc != BLINK_OK) { plan_free(p); return rc; }
+  if (rc != BLINK_OK) { guard.drop(); return rc; }
   PLAN_CUDA(ce, "plan upload / index kernel");
 
   // ---- host: per-channel facts, gather and placement tables -------------------------------
@@ -416,7 +423,7 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
     p->kx_max_all = std::max(p->kx_max_all, p->chinfo[ch].kx_max);
     p->ky_max_all = std::max(p->ky_max_all, p->chinfo[ch].ky_max);
   }
-  if (p->n_can_max > kPlaceMask) { plan_free(p); return BLINK_EUNSUPPORTED; }
+  if (p->n_can_max > kPlaceMask) { guard.drop(); return BLINK_EUNSUPPORTED; }
 
   // ---- gridder tables: rank-major stage slots, cells by descending per-pass length ------------
   {
@@ -432,9 +439,9 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
     if (p->n_pass < 1) p->n_pass = 1;
     p->grid_smem = sizeof(float2) * ((size_t)p->band_cells + (size_t)p->n_can_max +
                                      (size_t)p->stage_cap) + 64;
-    if (p->max_smem_optin > 0 && p->grid_smem > (size_t)p->max_smem_optin) { plan_free(p); return BLINK_EUNSUPPORTED; }
+    if (p->max_smem_optin > 0 && p->grid_smem > (size_t)p->max_smem_optin) { guard.drop(); return BLINK_EUNSUPPORTED; }
   }
-  if (p->n_can_max > 0xFFFF || p->stage_cap > 0x7FFF) { plan_free(p); return BLINK_EUNSUPPORTED; }
+  if (p->n_can_max > 0xFFFF || p->stage_cap > 0x7FFF) { guard.drop(); return BLINK_EUNSUPPORTED; }
   const int n_pass = p->n_pass, ncm = std::max(p->n_can_max, 1);
   RankTables rt;
   build_rank_tables(gathers, n_ch, n_bl, ncm, p->stage_cap, rt);
@@ -599,8 +606,14 @@ extern "C" int blink_plan_create_opts(blink_plan **out, const double *ant_enu_m,
   }
 #undef PLAN_TRY
 #undef PLAN_CUDA
+  guard.p = nullptr;
   *out = p;
   return BLINK_OK;
+} catch (const std::bad_alloc &) {
+  return BLINK_ENOMEM;                      // host memory for the plan tables; the guard has freed the plan
+} catch (...) {
+  blink::set_error_text("blink_plan_create: unexpected C++ exception");
+  return BLINK_ECUDA;
 }
 
 extern "C" int blink_plan_destroy(blink_plan *plan) {
@@ -611,7 +624,7 @@ extern "C" int blink_plan_destroy(blink_plan *plan) {
 // blink_plan_refresh: step a0 again for new antenna coordinates (a tracking array's projected baselines
 // move with hour angle), everything else as at creation.  The index kernel runs on the
 // device, the table packing on the host cores (one channel per thread); the new tables replace the old
-// ones once they are complete, the scratch and the host staging are kept.
+// ones once they are complete (its scratch included, sized as the old plan's was); the host staging is kept.
 extern "C" int blink_plan_refresh(blink_plan *p, const double *ant_enu_m, void *stream) {
   if (!p || !ant_enu_m) return BLINK_EINVAL;
   int rc = check_device(p);
@@ -621,6 +634,12 @@ extern "C" int blink_plan_refresh(blink_plan *p, const double *ant_enu_m, void *
   rc = blink_plan_create_opts(&q, ant_enu_m, p->n_ant, p->h_freq.data(), p->n_ch, p->n_pix, p->pixscale, p->weighting,
                               stream, opt.struct_size ? &opt : nullptr);
   if (rc != BLINK_OK) return rc;
+  // scratch for the new bounding box, while the old plan is still whole: a failure here (BLINK_ENOMEM for a
+  // wider half-plane) must leave the caller with the plan it had.  Both scratches exist until the swap.
+  if (p->reserved_n_t > 0 && (rc = image_reserve(q, p->reserved_n_t)) != BLINK_OK) {
+    plan_free(q);
+    return rc;
+  }
   // kernels already queued still read the old tables
   cudaError_t e = cudaDeviceSynchronize();
   if (e != cudaSuccess) {
@@ -630,9 +649,9 @@ extern "C" int blink_plan_refresh(blink_plan *p, const double *ant_enu_m, void *
   }
   std::swap(*p, *q);                       // p: the new tables; q: the old ones, about to be freed
   std::swap(p->hp, q->hp);                 // the host staging depends on n_ch, n_bl, N only
-  const int reserved = q->reserved_n_t;
+  p->corr_stale = (q->corr_on || q->corr_stale) ? 1 : 0;   // the factors went with the old geometry
   plan_free(q);
-  return reserved > 0 ? image_reserve(p, reserved) : BLINK_OK;   // scratch for the new bounding box
+  return BLINK_OK;
 }
 
 extern "C" int blink_plan_reserve(blink_plan *plan, int n_t) {

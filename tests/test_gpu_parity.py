@@ -805,6 +805,41 @@ def test_plan_refresh(torch_cuda, blink, oracle, name):
     plan.close()
 
 
+def test_refresh_with_corrections_fused_at_load_refuses_until_told(torch_cuda, blink):
+    """blink_plan_refresh drops the correction table; a plan that was applying it at load must not go on
+    gridding uncorrected data with BLINK_OK: the gridding calls return BLINK_EINVAL until the caller has
+    called apply_corrections again (on with a new table, or off)."""
+    torch = torch_cuda
+    w = _workload("station128")
+    vis = torch.from_numpy(w.vis()).cuda()
+    rng = np.random.default_rng(5)
+    cables = rng.uniform(0, 30, w.n_ant)
+    plan = _plan(blink, w)
+    plan.reserve(w.n_t)
+    plan.set_corrections(None, cables, 0.05, -0.02)
+    plan.apply_corrections(True)
+    corrected = plan.grid_image(vis).clone()
+    plan.refresh(w.ant_enu_m)
+    assert plan.query_i32(blink.Q_CORR_FUSED) == 0
+    for call in (lambda: plan.grid(vis), lambda: plan.grid_image(vis)):
+        with pytest.raises(blink.BlinkError) as ei:
+            call()
+        assert ei.value.status == blink.EINVAL and "blink_plan_refresh" in str(ei.value)
+    with pytest.raises(blink.BlinkError):            # on again needs a table first
+        plan.apply_corrections(True)
+    plan.set_corrections(None, cables, 0.05, -0.02)
+    with pytest.raises(blink.BlinkError):            # a table alone does not say the switch is wanted
+        plan.grid_image(vis)
+    plan.apply_corrections(True)
+    assert torch.equal(plan.grid_image(vis), corrected)
+    plan.refresh(w.ant_enu_m)
+    plan.apply_corrections(False)                    # "uncorrected is what I want"
+    plain = blink.Plan(w.ant_enu_m, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    assert torch.equal(plan.grid_image(vis), plain.grid_image(vis))
+    plain.close()
+    plan.close()
+
+
 def test_corrections_odd_table_and_unaligned_views(torch_cuda, blink):
     """Odd n_ch * n_bl and an 8-byte-aligned (not 16) buffer take the one-visibility kernel."""
     torch = torch_cuda

@@ -169,6 +169,16 @@ def test_fft_stage_algebra_on_host(tmp_path):
     assert out.returncode == 0 and out.stdout.strip().endswith("OK"), out.stdout
 
 
+def test_parallel_for_reports_a_throwing_worker(tmp_path):
+    """plan-time host loops (csrc/parallel_for.h): an exception in a worker must come back to the caller,
+    not end the process; every index runs once"""
+    exe = str(tmp_path / "host_parallel_check")
+    subprocess.run(["g++", "-O1", "-std=c++17", "-pthread", os.path.join(ROOT, "tests", "host_parallel_check.cpp"),
+                    "-o", exe], check=True)
+    out = subprocess.run([exe], capture_output=True, text=True)
+    assert out.returncode == 0 and out.stdout.strip().endswith("OK"), out.stdout + out.stderr
+
+
 def test_polyphase_identity_behind_the_large_image_route():
     """The identity k_fused<256, ..., D> rests on (blink_fused.cu): for a grid confined to |k| < N'/2,
     the D N' x D N' image is D x D interleaved N' x N' images of the same cells, each the N' transform
