@@ -82,10 +82,16 @@ typedef enum blink_query {
   BLINK_Q_CORR = 16,        /* out: const float2* DEVICE [n_ch][n_bl] correction factors (NULL until set) */
   BLINK_Q_CORR_FUSED = 17,  /* out: int32  1 = blink_grid / blink_grid_image apply the factors at load */
   BLINK_Q_TENSOR_ROUTE = 18,/* out: int32  1 = the shared-memory route runs its transforms on the tensor cores (k_fused_tc) */
-  BLINK_Q_WARP_KERNEL = 19  /* out: int32  kernel behind BLINK_Q_FUSED_PATH 2: 2 = residue-class kernel (intermediate in shared
+  BLINK_Q_WARP_KERNEL = 19, /* out: int32  kernel behind BLINK_Q_FUSED_PATH 2: 2 = residue-class kernel (intermediate in shared
                                memory, k_img1024r), 1 = ring kernel (intermediate in an L2-sized ring, k_img1024), 3 = BLINK_Q_FUSED_PATH is 0
                                and the column pass of the two kernels is the residue-class kernel k_cols_res (N = 2048 / 4096,
                                sparse half-plane), 0 = none of these */
+  BLINK_Q_FUSED_NZ = 20,    /* out: int32  which k_fused instance BLINK_Q_FUSED_PATH 1 runs in the plan's current state: its
+                               first transform stage reads NZ of the 8 N/16-cell blocks on either side of DC (2, 3, 4 or 8;
+                               8 = unpruned); 0 = not on that route, or on its tensor-core form.  For harnesses that must
+                               know which compiled instance they exercised */
+  BLINK_Q_FUSED_D = 21      /* out: int32  that route's polyphase factor: the image is D x D interleaved sub-images of
+                               N / D (1, 2 or 4); 0 = not on that route */
 } blink_query;
 
 typedef struct blink_plan blink_plan; /* opaque */

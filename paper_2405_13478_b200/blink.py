@@ -19,7 +19,7 @@ OK, EINVAL, ENOMEM, ECUDA, EUNSUPPORTED, ERESERVE, ECAPACITY = 0, -1, -2, -3, -4
 STATIC_SCRATCH_BYTES = 32 << 20     # BLINK_STATIC_SCRATCH_BYTES
 (Q_N_ANT, Q_N_BL, Q_N_CH, Q_N_PIX, Q_N_DROPPED, Q_WSUM, Q_N_OCC, Q_BBOX, Q_NORM, Q_CELL_IDX,
  Q_COUNTS, Q_IMAGE_PATH, Q_SCRATCH_BYTES, Q_IMAGE_CHUNK, Q_FUSED_PATH, Q_FUSED_CHUNK, Q_CORR, Q_CORR_FUSED,
- Q_TENSOR_ROUTE, Q_WARP_KERNEL) = range(20)
+ Q_TENSOR_ROUTE, Q_WARP_KERNEL, Q_FUSED_NZ, Q_FUSED_D) = range(22)
 
 # include/blink.h (the product ABI) and include/blink_testing.h (host-only test hooks)
 EXPORTS = ["blink_version", "blink_strerror", "blink_last_cuda_error", "blink_plan_create", "blink_plan_create_opts",

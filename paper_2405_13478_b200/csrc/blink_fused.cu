@@ -293,24 +293,37 @@ int fused_build(blink_plan *p, cudaStream_t st) {
   return BLINK_OK;
 }
 
-template <bool CORR>
-static int launch_fused_c(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
-  // band limit of the first transform stage, in units of N/16 cells
+// The NZ template argument of the k_fused instance the plan's current state selects (BLINK_Q_FUSED_NZ): the
+// first transform stage reads only the NZ N/16-cell blocks next to DC on either side.  N <= 128: always 8
+// (unpruned); sub-transforms of 256: 2, 3, 4 or 8 without corrections at D = 1, 3 or 8 otherwise.
+int fused_nz_instance(const blink_plan *p) {
   const int n_sub = p->n_pix / p->fused_D;
+  if (n_sub != 256) return 8;
+  // band limit of the first transform stage, in units of N/16 cells
   const int reach = std::max(p->kx_max_all, p->ky_max_all) + 1, T = n_sub / 16;
   const int nz = (reach + T - 1) / T;
-  if (p->fused_D == 2) return nz <= 3 ? launch_fused_n<256, 3, 2, CORR>(p, fp, st) : launch_fused_n<256, 8, 2, CORR>(p, fp, st);
+  if (p->fused_D == 1 && !p->corr_on) {   // (with corrections: the two instances that cover every band limit)
+    if (nz <= 2) return 2;
+    if (nz == 4) return 4;
+  }
+  return nz <= 3 ? 3 : 8;
+}
+
+template <bool CORR>
+static int launch_fused_c(const blink_plan *p, const FusedParams &fp, cudaStream_t st) {
+  const int nz = fused_nz_instance(p);
+  if (p->fused_D == 2) return nz == 3 ? launch_fused_n<256, 3, 2, CORR>(p, fp, st) : launch_fused_n<256, 8, 2, CORR>(p, fp, st);
   if (p->fused_D == 4) return launch_fused_d4(p, fp, nz, st);
   switch (p->n_pix) {
     case 32: return launch_fused_n<32, 8, 1, CORR>(p, fp, st);
     case 64: return launch_fused_n<64, 8, 1, CORR>(p, fp, st);
     case 128: return launch_fused_n<128, 8, 1, CORR>(p, fp, st);
     case 256:
-      if constexpr (!CORR) {       // (with corrections: the two instances that cover every band limit)
-        if (nz <= 2) return launch_fused_n<256, 2, 1, CORR>(p, fp, st);
-        if (nz > 3 && nz <= 4) return launch_fused_n<256, 4, 1, CORR>(p, fp, st);
+      if constexpr (!CORR) {
+        if (nz == 2) return launch_fused_n<256, 2, 1, CORR>(p, fp, st);
+        if (nz == 4) return launch_fused_n<256, 4, 1, CORR>(p, fp, st);
       }
-      if (nz <= 3) return launch_fused_n<256, 3, 1, CORR>(p, fp, st);
+      if (nz == 3) return launch_fused_n<256, 3, 1, CORR>(p, fp, st);
       return launch_fused_n<256, 8, 1, CORR>(p, fp, st);
     default: return BLINK_EUNSUPPORTED;
   }

@@ -262,6 +262,7 @@ inline bool fused_smem_route(const blink_plan *p) {
   return p->fused_path == 1 && (p->fl[p->corr_on ? 1 : 0].ok || (p->tc_route && p->tl[p->corr_on ? 1 : 0].ok));
 }
 int fused_line_stride(int n_pix);
+int fused_nz_instance(const blink_plan *p);
 int launch_grid_image(const blink_plan *p, const float2 *vis, int n_t, float *img, cudaStream_t st);
 int launch_image_from_vis(const blink_plan *p, const float2 *vis, int n_snap, float *img, cudaStream_t st);
 

@@ -712,6 +712,12 @@ extern "C" int blink_plan_query(const blink_plan *p, int what, int index, void *
     case BLINK_Q_CORR: *(const void **)out = p->d_corr; break;
     case BLINK_Q_CORR_FUSED: *(int32_t *)out = p->corr_on; break;
     case BLINK_Q_TENSOR_ROUTE: *(int32_t *)out = (fused_smem_route(p) && p->tc_route && p->tl[p->corr_on ? 1 : 0].ok) ? 1 : 0; break;
+    case BLINK_Q_FUSED_NZ: {
+      const bool tc = p->tc_route && p->tl[p->corr_on ? 1 : 0].ok;
+      *(int32_t *)out = (fused_smem_route(p) && !tc) ? fused_nz_instance(p) : 0;
+      break;
+    }
+    case BLINK_Q_FUSED_D: *(int32_t *)out = fused_smem_route(p) ? p->fused_D : 0; break;
     default: return BLINK_EINVAL;
   }
   return BLINK_OK;

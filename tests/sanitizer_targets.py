@@ -1,7 +1,9 @@
-"""Small invocations of the kernels whose synchronisation is the delicate part, for compute-sanitizer:
-
-    compute-sanitizer --tool memcheck  python tests/sanitizer_targets.py
-    compute-sanitizer --tool racecheck python tests/sanitizer_targets.py
+"""Small invocations of the kernels whose synchronisation is the delicate part: a plain stress-and-compare
+script (`python tests/sanitizer_targets.py` on a B200).  It was written as a compute-sanitizer target, but that
+tool is closed on this pool (profiles/r02_compute_sanitizer_unavailable.txt), so NO race checker stands behind
+these kernels: what this script and the -m gpu tests give is result comparison only -- every case below is
+checked against another route or the oracle, repeated calls must agree bit for bit, and outputs are
+NaN-prefilled so that a tile read before it was written shows.
 
 (1) __graft_entry__.smoke(); (2) blink_grid_image on the shared-memory route with more snapshots than
 CTAs, so every CTA of k_fused hands its chunk ring and its aliased line buffers from one snapshot to
@@ -11,7 +13,7 @@ snapshots, so pass A waits on pass B through the global counters; (5) blink_dyns
 kernels: k_img1024r (producer / consumer warps over a ring of two tiles, CTAs changing snapshot mid-run) and
 k_cols_res at 2048^2 (tiles leaving as bulk copies while the next unit is formed).  Each result is
 checked against the two-call route so a silent corruption would also fail here.  Not collected by
-pytest (no test_ prefix): the sanitizer slows these kernels 10-100 x."""
+pytest (no test_ prefix); the hand-over cases (2) are also -m gpu tests (test_every_fused_instance_against_oracle)."""
 import os
 import sys
 

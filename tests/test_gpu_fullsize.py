@@ -211,6 +211,85 @@ def test_corrections_fused_into_the_residue_column_pass(torch_cuda, blink):
     plan.close()
 
 
+@pytest.mark.parametrize("n_pix,chunk_mb", [(4096, 64), (4096, 100), (2048, 40)])
+def test_chunked_residue_column_pass(torch_cuda, blink, oracle, n_pix, chunk_mb):
+    """The launch configuration bench.py times for mwa2: the two-kernel route cut into SEVERAL launch pairs
+    (snap_base > 0 through k_cols_res + k_image_rows), forced on a small batch with blink_options.image_chunk_mb.
+    9 snapshots of 3 channels; 64 MiB / 40 MiB give chunks of 2 snapshots (the channel wraps inside a chunk and
+    across chunk boundaries), 100 MiB chunks of 3.  Through blink_grid_image AND blink_image, NaN-prefilled
+    images, every snapshot against the oracle on sampled pixels, and bit-equal to the same plan run with the
+    default 2 GB budget (one pair)."""
+    torch = torch_cuda
+    w = synth.config_mwa2(n_t=3, n_ch=3)
+    if n_pix == 2048:
+        w.n_pix, w.pixscale = 2048, 30.0 * synth.ARCSEC
+    vis = w.vis()
+    v = torch.from_numpy(vis).cuda()
+    n, n_snap = w.n_pix, w.n_t * w.n_ch
+    one = _plan(blink, w)
+    assert one.query_i32(blink.Q_WARP_KERNEL) == 3 and one.query_i32(blink.Q_FUSED_PATH) == 0
+    one.reserve(w.n_t)
+    assert one.query_i32(blink.Q_FUSED_CHUNK) >= n_snap and one.query_i32(blink.Q_IMAGE_CHUNK) >= n_snap
+    ref = one.grid_image(v)
+    uv = one.grid(v)
+    ref_uv = one.image(uv)
+    one.close()
+    plan = _plan(blink, w, image_chunk_mb=chunk_mb)
+    plan.reserve(w.n_t)
+    assert plan.query_i32(blink.Q_WARP_KERNEL) == 3 and plan.query_i32(blink.Q_FUSED_PATH) == 0
+    chunk = plan.query_i32(blink.Q_FUSED_CHUNK)
+    assert chunk == plan.query_i32(blink.Q_IMAGE_CHUNK)
+    assert 1 <= chunk and 3 * chunk <= n_snap, f"chunk {chunk}: fewer than 3 launch pairs"
+    if chunk_mb != 100:
+        assert chunk % w.n_ch != 0                   # the channel of a chunk's first snapshot differs chunk to chunk
+    img = torch.full((w.n_t, w.n_ch, n, n), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(v, img)
+    img_uv = torch.full((w.n_t, w.n_ch, n, n), float("nan"), dtype=torch.float32, device="cuda")
+    plan.image(uv, img_uv)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img).all() and torch.isfinite(img_uv).all(), "image not fully written"
+    assert torch.equal(img, ref), "chunking changed blink_grid_image's result"
+    assert torch.equal(img_uv, ref_uv), "chunking changed blink_image's result"
+    imh, imh_uv = img.cpu().numpy().reshape(-1, n, n), img_uv.cpu().numpy().reshape(-1, n, n)
+    yx = _pixels(n, 47)
+    for s in range(n_snap):
+        _sampled_pixel_check(oracle, w, vis, s, imh[s], yx)
+        _sampled_pixel_check(oracle, w, vis, s, imh_uv[s], yx)
+    plan.close()
+
+
+def test_corrections_fused_into_the_residue_column_pass_against_oracle(torch_cuda, blink, oracle):
+    """f2 fused at load on k_cols_res (2048^2), against the ORACLE chain (oracle/corrections.py in fp64 ->
+    gridding -> weighting -> literal sums on sampled pixels), in two launch pairs."""
+    torch = torch_cuda
+    from oracle import corrections as oc
+    w = synth.config_mwa2(n_t=2, n_ch=2)
+    w.n_pix, w.pixscale = 2048, 30.0 * synth.ARCSEC
+    rng = np.random.default_rng(29)
+    n_ant = w.ant_enu_m.shape[0]
+    gains = rng.uniform(0.5, 2.0, (w.n_ch, n_ant)) * np.exp(1j * rng.uniform(-np.pi, np.pi, (w.n_ch, n_ant)))
+    cables = rng.uniform(0.0, 300.0, n_ant)
+    l0, m0 = 0.002, -0.001
+    vis = w.vis()
+    plan = _plan(blink, w, image_chunk_mb=40)
+    plan.set_corrections(gains, cables, l0, m0)
+    plan.apply_corrections(True)
+    assert plan.query_i32(blink.Q_WARP_KERNEL) == 3 and plan.query_i32(blink.Q_CORR_FUSED) == 1
+    n = w.n_pix
+    img = torch.full((w.n_t, w.n_ch, n, n), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(torch.from_numpy(vis).cuda(), img)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img).all()
+    assert plan.query_i32(blink.Q_FUSED_CHUNK) < w.n_t * w.n_ch
+    F_ref = oc.correction_factors(w.ant_enu_m, w.freq_hz, gains, cables, l0, m0)
+    vis_c = oc.apply_corrections(vis, F_ref).astype(np.complex64)
+    imh = img.cpu().numpy().reshape(-1, n, n)
+    yx = _pixels(n, 53)
+    for s in range(w.n_t * w.n_ch):
+        _sampled_pixel_check(oracle, w, vis_c, s, imh[s], yx)
+    plan.close()
+
+
 @pytest.mark.parametrize("seed", [11, 12])
 def test_residue_routes_on_random_arrays(torch_cuda, blink, seed):
     """The residue-class kernels (k_img1024r, k_cols_res) against the line kernels (warp_route = -1) on every

@@ -412,6 +412,101 @@ def test_tensor_core_route(torch_cuda, blink, oracle, weighting, n_t):
     plan.close()
 
 
+# (East scale, North scale of the 38 m station disc, image side) -> the k_fused instance expected: (NZ, D) without
+# corrections, NZ with them.  All-sky pixels: a baseline of b metres lands 2 b / lambda cells from DC (lambda =
+# 1.87 m; the disc itself reaches 42), and the first stage of a 256-point transform reads NZ blocks of 16 cells on
+# either side of DC.  The band limit counts the longer axis, the shared memory the columns (East) only, so the
+# long-reach cases are discs stretched North and squeezed East: they still fit the SM.
+FUSED_INSTANCES = [
+    (0.7, 0.7, 256, (2, 1), 3),      # reach <= 32
+    (1.0, 1.0, 256, (3, 1), 3),      # the station layout
+    (0.7, 1.4, 256, (4, 1), 8),      # reach 49..64
+    (0.5, 2.2, 256, (8, 1), 8),      # reach > 64
+    (0.7, 1.4, 512, (8, 2), 8),      # polyphase 2 x 2 sub-images, unpruned first stage
+    (0.7, 1.4, 1024, (8, 4), 8),     # polyphase 4 x 4
+]
+
+
+@pytest.mark.parametrize("sx,sy,n_pix,plain_inst,corr_nz", FUSED_INSTANCES)
+def test_every_fused_instance_against_oracle(torch_cuda, blink, oracle, sx, sy, n_pix, plain_inst, corr_nz):
+    """Every compiled instance of the shared-memory kernel k_fused<256, ., NZ, D, CORR> (each has its own
+    compile-time pruned loads) runs under a test, and the test knows which one ran (BLINK_Q_FUSED_NZ / _D):
+    the station disc in four shapes at 256^2 (NZ = 2, 3, 4, 8), NZ = 8 at 512^2 (D = 2) and 1024^2 (D = 4), each plain
+    and with the corrections fused at load (CORR; oracle chain corrections -> gridding -> imaging).  300
+    snapshots over 148 persistent CTAs, so every CTA hands its buffers from one snapshot to the next; sampled
+    snapshots (first, last, around the hand-over) at the image bar."""
+    torch = torch_cuda
+    from oracle import corrections as oc
+    w = synth.config_station(n_t=100, n_ch=3, n_pix=n_pix)
+    w.ant_enu_m = w.ant_enu_m * np.array([sx, sy, 1.0])
+    vis_h = w.vis()
+    vis = torch.from_numpy(vis_h).cuda()
+    n_snap = w.n_t * w.n_ch
+    ant, gains, cables = _corr_inputs(w, 37)
+    plan = blink.Plan(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 1, "this layout was meant to fit the shared-memory route"
+    assert plan.query_i32(blink.Q_TENSOR_ROUTE) == 0
+    assert (plan.query_i32(blink.Q_FUSED_NZ), plan.query_i32(blink.Q_FUSED_D)) == plain_inst
+    sel = np.array(sorted({0, 1, 147, 148, 149, n_snap - 1}), np.int64)
+    if n_pix >= 512:
+        sel = np.array([0, 148, n_snap - 1], np.int64)
+    dsel = torch.from_numpy(sel).cuda()
+
+    def check(img, vis_ref, what):
+        assert bool(torch.isfinite(img.view(n_snap, -1).sum(dim=1)).all()), f"{what}: some image not fully written"
+        ref = oracle.image_batch(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_ref, sel)
+        got = img.view(n_snap, n_pix, n_pix)[dsel].cpu().numpy()
+        for q in range(len(sel)):
+            peak = np.max(np.abs(ref["images"][q]))
+            err = np.max(np.abs(got[q] - ref["images"][q]))
+            assert err <= IMG_TOL * peak, f"{what}, snapshot {sel[q]}: err {err:.3e} peak {peak:.3e}"
+
+    img = torch.full((w.n_t, w.n_ch, n_pix, n_pix), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(vis, img)
+    torch.cuda.synchronize()
+    check(img, vis_h, f"k_fused<256,.,{plain_inst[0]},{plain_inst[1]},0>")
+    l0, m0 = 0.2, -0.1
+    plan.set_corrections(gains, cables, l0, m0)
+    plan.apply_corrections(True)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 1 and plan.query_i32(blink.Q_CORR_FUSED) == 1
+    assert (plan.query_i32(blink.Q_FUSED_NZ), plan.query_i32(blink.Q_FUSED_D)) == (corr_nz, plain_inst[1])
+    img.fill_(float("nan"))
+    plan.grid_image(vis, img)
+    torch.cuda.synchronize()
+    F_ref = oc.correction_factors(ant, w.freq_hz, gains, cables, l0, m0)
+    check(img, oc.apply_corrections(vis_h, F_ref).astype(np.complex64), f"k_fused<256,.,{corr_nz},{plain_inst[1]},1>")
+    plan.close()
+
+
+def test_corrections_fused_into_the_tensor_core_kernel_against_oracle(torch_cuda, blink, oracle):
+    """f2 fused at load on k_fused_tc<true> against the ORACLE chain (the other test compares it with k_fused)."""
+    torch = torch_cuda
+    from oracle import corrections as oc
+    w = synth.config_station(n_t=4, n_ch=40)          # 160 snapshots: some CTAs image two
+    vis_h = w.vis()
+    ant, gains, cables = _corr_inputs(w, 41)
+    plan = blink.Plan(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=dict(tune={7: 1}))
+    l0, m0 = 0.1, 0.05
+    plan.set_corrections(gains, cables, l0, m0)
+    plan.apply_corrections(True)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 1 and plan.query_i32(blink.Q_TENSOR_ROUTE) == 1
+    assert plan.query_i32(blink.Q_FUSED_NZ) == 0
+    n_snap = w.n_t * w.n_ch
+    img = torch.full((w.n_t, w.n_ch, 256, 256), float("nan"), dtype=torch.float32, device="cuda")
+    plan.grid_image(torch.from_numpy(vis_h).cuda(), img)
+    torch.cuda.synchronize()
+    assert torch.isfinite(img).all()
+    F_ref = oc.correction_factors(ant, w.freq_hz, gains, cables, l0, m0)
+    vis_c = oc.apply_corrections(vis_h, F_ref).astype(np.complex64)
+    sel = np.array([0, 39, 40, 148, n_snap - 1], np.int64)
+    ref = oracle.image_batch(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_c, sel)
+    got = img.view(n_snap, 256, 256)[torch.from_numpy(sel).cuda()].cpu().numpy()
+    for q in range(len(sel)):
+        peak = np.max(np.abs(ref["images"][q]))
+        assert np.max(np.abs(got[q] - ref["images"][q])) <= IMG_TOL * peak, f"snapshot {sel[q]}"
+    plan.close()
+
+
 def test_warp_route_ring_reuse(torch_cuda, blink, oracle):
     """blink_grid_image, warp-per-transform route (k_img1024), on more snapshots than its ring of U
     slots holds (here a ring of 3), so that pass A has to wait for pass B to release a slot: every
