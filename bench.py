@@ -9,7 +9,9 @@ weight, inverse DFT, shift, normalise, real part) over one batch of synthetic vi
 resident in HBM, through the public call blink_grid_image (`--path separate`: blink_grid +
 blink_image with the uv grids in HBM).  Headline workload = BASELINE.json configs[1] (SKA-Low
 station, 100 t x 32 ch x 32640 bl, 256^2); at N = 1 the same process also times configs[2] (MWA
-Phase I, 1024^2) and configs[4] at 512^2 and reports them under "workloads".
+Phase I, 1024^2), configs[3] (MWA Phase II, 4096^2) and the whole configs[4] sweep (128^2 .. 1024^2),
+reports them under "workloads", and ends the line with a compact "summary" of every workload's
+[ms per step, fraction of the HBM roofline] so that a truncated log still carries them.
 """
 from __future__ import annotations
 
@@ -53,6 +55,18 @@ def algorithmic_bytes(w):
     return dict(grid=8 * w.n_bl + 8 * nn, image=12 * nn, sep=8 * w.n_bl + 20 * nn, fused=8 * w.n_bl + 4 * nn)
 
 
+def image_call_bytes(w, plan, blink):
+    """blink_image on the two-call path: what the call has to move is the 4 N^2 image plus the uv cells it
+    reads -- the routes read the plan's bounding box (line kernels) or only its occupied cells (residue-class
+    kernels), never the whole 8 N^2 grid; crediting 12 N^2 would put the call above the HBM peak."""
+    nn = w.n_pix * w.n_pix
+    if plan.query_i32(blink.Q_WARP_KERNEL) in (2, 3):
+        cells = float(np.mean([plan.n_occ(c) for c in range(w.n_ch)]))
+    else:
+        cells = float(np.mean([(2 * plan.bbox(c)[0] + 1) * (2 * plan.bbox(c)[1] + 1) for c in range(w.n_ch)]))
+    return 4 * nn + 8 * min(nn, cells)
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -64,23 +78,47 @@ def measured_peaks():
 _UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
 
 
-def ncu_traffic(workload: str, path: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch at the bench's own
-    size, from the newest committed `ncu --set full` summary profiles/r*_<workload>_<path>_fullsize_summary.txt
-    (written by `python -m paper_2405_13478_b200.ncu_summary`); None when there is none.  The file name
-    and its modification time go into the line: the capture is of the commit it was taken at."""
-    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{workload}_{path}_fullsize_summary.txt")))
+def kernel_sources_sha16():
+    """hash of the kernel sources (csrc/*), written into every ncu summary at capture time and compared here:
+    a summary taken before a kernel change says so in the line (`traffic_source.stale`)"""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2405_13478_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".h")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload: str, path: str, n_snap: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per STEP of the kernels behind the call, from the newest
+    round's committed `ncu --set full` summaries profiles/rNN_<workload>_<path>_fullsize[_<kernel>]_summary.txt
+    (written by `python -m paper_2405_13478_b200.ncu_summary`): one file per kernel of the step; a file whose
+    capture covered fewer snapshots than the step (one launch pair of the chunked route) carries a
+    `# snapshots_in_launch K` line and is scaled by n_snap / K.  None when there is none.  File names, times
+    and whether the kernel sources changed since the capture go into the line."""
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{workload}_{path}_fullsize*_summary.txt")))
     if not files:
         return None, None
-    f = files[-1]
-    tot = 0.0
-    for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
-        m = re.search(rf"^{re.escape(key)}\s+([0-9.,]+)\s+(\w+)", open(f).read(), re.M)
-        if not m or m.group(2) not in _UNIT:
-            return None, None
-        tot += float(m.group(1).replace(",", "")) * _UNIT[m.group(2)]
-    return int(tot), {"file": os.path.relpath(f, ROOT),
-                      "mtime": time.strftime("%Y-%m-%dT%H:%M:%SZ", time.gmtime(os.path.getmtime(f)))}
+    rnd = os.path.basename(files[-1]).split("_")[0]
+    files = [f for f in files if os.path.basename(f).startswith(rnd + "_")]
+    tot, src, sha = 0.0, [], kernel_sources_sha16()
+    for f in files:
+        txt = open(f).read()
+        scale = 1.0
+        m = re.search(r"^# snapshots_in_launch\s+(\d+)", txt, re.M)
+        if m:
+            scale = n_snap / float(m.group(1))
+        for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            m = re.search(rf"^{re.escape(key)}\s+([0-9.,]+)\s+(\w+)", txt, re.M)
+            if not m or m.group(2) not in _UNIT:
+                return None, None
+            tot += scale * float(m.group(1).replace(",", "")) * _UNIT[m.group(2)]
+        m = re.search(r"^# kernel_sources_sha16\s+(\w+)", txt, re.M)
+        src.append({"file": os.path.relpath(f, ROOT), "scaled_by": scale,
+                    "stale": (m.group(1) != sha) if m else "unknown (no source hash in the file)"})
+    return int(tot), src
 
 
 class ClockSampler:
@@ -309,12 +347,18 @@ def time_steps(torch, plan, vis, img, uv, steps, warmup, stream, barrier):
     total_ms = ev[0].elapsed_time(ev[3 * steps])
     grid_ms = float(np.mean([ev[3 * k].elapsed_time(ev[3 * k + 1]) for k in range(steps)]))
     image_ms = float(np.mean([ev[3 * k + 1].elapsed_time(ev[3 * k + 2]) for k in range(steps)]))
+    time_steps.per_step = [ev[3 * k].elapsed_time(ev[3 * k + 3]) for k in range(steps)]   # best and median
     return total_ms, grid_ms, image_ms
+
+
+def spread(per_step):
+    return {"best": float(np.min(per_step)), "median": float(np.median(per_step)), "worst": float(np.max(per_step)),
+            "n": len(per_step)}
 
 
 def roofline_of(w, plan, blink, name, path, ms_call, dom_bytes, n_snap, peak, peak_src, alu):
     achieved = dom_bytes * n_snap / (ms_call / 1e3) / 1e9
-    traffic, src = ncu_traffic(name, path)
+    traffic, src = ncu_traffic(name, path, n_snap)
     flops, form = algorithmic_flops(w, plan, blink)
     tf = flops * n_snap / (ms_call / 1e3) / 1e12
     t_hbm_us = dom_bytes / (peak * 1e9) * 1e6
@@ -327,6 +371,7 @@ def roofline_of(w, plan, blink, name, path, ms_call, dom_bytes, n_snap, peak, pe
                 "alu_us_per_snapshot_at_fma_peak": t_alu_us, "hbm_us_per_snapshot_at_peak": t_hbm_us,
                 "binding": "alu" if t_alu_us > t_hbm_us else "hbm"}
     return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "frac_is": "algorithmic bytes / CUDA-event time / measured copy peak (never the ncu traffic)",
             "traffic": traffic, "traffic_source": src, "peak_source": peak_src,
             "algorithmic_bytes_per_snapshot": dom_bytes, "atomics": "none (atomic-free design)"}, side
 
@@ -344,6 +389,7 @@ def extra_workload(torch, blink, name, steps, stream, peak, peak_src, alu):
     ab = algorithmic_bytes(w)
     roof, side = roofline_of(w, plan, blink, name, "fused", call_ms, ab["fused"], n_snap, peak, peak_src, alu)
     out = {"config": workload_config(w, name), "steps": steps, "ms_per_step": ms,
+           "ms_per_step_spread": spread(time_steps.per_step),
            "images_per_s": n_snap / (ms / 1e3), "mvis_per_s": n_snap * w.n_bl / (ms / 1e3) / 1e6,
            "route": {1: "shared-memory (k_fused)",
                      0: "two kernels" + (" (column pass k_cols_res)" if plan.query_i32(blink.Q_WARP_KERNEL) == 3 else ""),
@@ -372,7 +418,7 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "separate", "fused"],
                     help="separate = blink_grid + blink_image (uv grid in HBM); fused = blink_grid_image; "
                          "auto = fused")
-    ap.add_argument("--extra-workloads", default="mwa1,mwa2,sweep512",
+    ap.add_argument("--extra-workloads", default="mwa1,mwa2,sweep128,sweep256,sweep512,sweep1024",
                     help="comma list of further workloads timed in the same process at N = 1 ('' = none)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -439,6 +485,7 @@ def main():
         time.sleep(0.25)
     total_ms, grid_ms, image_ms = time_steps(torch, plan, vis, img, uv, args.steps, args.warmup, stream, barrier)
     clocks = sampler.stop() if rank == 0 else None
+    step_spread = spread(time_steps.per_step)
     total_ms = shard.max_over_ranks(total_ms, device="cuda")
     ms_per_step = total_ms / args.steps
     n_snap = w.n_snapshots
@@ -576,8 +623,9 @@ def main():
         calls = {"blink_grid_image": (grid_ms, ab["fused"])}
         step_bytes = ab["fused"]
     else:
-        calls = {"blink_grid": (grid_ms, ab["grid"]), "blink_image": (image_ms, ab["image"])}
-        step_bytes = ab["sep"]
+        ib = image_call_bytes(w, plan, blink)
+        calls = {"blink_grid": (grid_ms, ab["grid"]), "blink_image": (image_ms, ib)}
+        step_bytes = ab["grid"] + ib
     dom = max(calls, key=lambda k: calls[k][0])
     roof, side = roofline_of(w, plan, blink, args.workload, args.path, calls[dom][0], calls[dom][1], n_snap, peak,
                              peak_src, alu)
@@ -593,6 +641,7 @@ def main():
     out = {
         "metric": "dirty_images_per_s", "value": value, "unit": "images/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
+        "ms_per_step_spread": step_spread,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "mvis_per_s": value * w.n_bl / 1e6,
         "config": workload_config(w, args.workload),
@@ -620,6 +669,12 @@ def main():
                                                     peak_src, alu)
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(w, args)
+    # ---- last key, short: every workload's [ms per step, fraction of the HBM roofline on the one-call bytes]
+    # (north_star's targets are station and mwa1 >= 0.60; DESIGN.md section 7 says which are met)
+    sm = {args.workload: [round(ms_per_step, 4), round(out["roofline_step"]["frac"], 3)]}
+    for name, r in out.get("workloads", {}).items():
+        sm[name] = [round(r["ms_per_step"], 4), round(r["roofline"]["frac"], 3)]
+    out["summary"] = {"ms_per_step,frac_of_hbm_roofline": sm, "path": args.path}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()

@@ -50,6 +50,8 @@ class Options(ctypes.Structure):
                 setattr(self, k, int(v))
 
 _lib = None
+_tlib = None
+TESTING_LIB_PATH = os.path.join(_HERE, "libblink_testing.so")
 
 
 class BlinkError(RuntimeError):
@@ -111,6 +113,23 @@ def load() -> ctypes.CDLL:
     lib.blink_correct.argtypes = [vp, vp, ci, vp, vp]
     lib.blink_dynspec.restype = ci
     lib.blink_dynspec.argtypes = [vp, vp, ci, ctypes.c_double, vp, vp, vp]
+    _lib = lib
+    return lib
+
+
+def load_testing() -> ctypes.CDLL:
+    """dlopen libblink_testing.so: the test hooks of include/blink_testing.h (host models of the table walks,
+    the fp32 peak probe).  They are NOT in libblink.so -- the product library has no CPU model of anything."""
+    global _tlib
+    if _tlib is not None:
+        return _tlib
+    if not os.path.exists(TESTING_LIB_PATH):
+        raise ImportError(f"{TESTING_LIB_PATH} not found: run `python -m paper_2405_13478_b200.build`")
+    lib = ctypes.CDLL(TESTING_LIB_PATH)
+    vp, ci = ctypes.c_void_p, ctypes.c_int
+    lib.blink_strerror.restype = ctypes.c_char_p
+    lib.blink_strerror.argtypes = [ci]
+    lib.blink_last_cuda_error.restype = ctypes.c_char_p
     lib.blink_probe_fp32.restype = ci
     lib.blink_probe_fp32.argtypes = [ci, ci, vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_int64), vp]
     lib.blink_host_build_gather.restype = ci
@@ -119,7 +138,7 @@ def load() -> ctypes.CDLL:
     lib.blink_host_fused_emulate.argtypes = [vp, ci, ci, ci, vp, vp, vp]
     lib.blink_host_residue_emulate.restype = ci
     lib.blink_host_residue_emulate.argtypes = [vp, ci, ci, ci, vp, ci, vp, vp, vp]
-    _lib = lib
+    _tlib = lib
     return lib
 
 
@@ -136,7 +155,7 @@ def _stream_ptr(stream=None):
 
 def host_build_gather(cell: np.ndarray, n_pix: int):
     """blink_host_build_gather: cell-sorted gather tables of one channel (host logic, no GPU)."""
-    lib = load()
+    lib = load_testing()
     cell = np.ascontiguousarray(cell, np.int32)
     n_bl = cell.shape[0]
     n_can = ctypes.c_int32(0)
@@ -153,7 +172,7 @@ def host_build_gather(cell: np.ndarray, n_pix: int):
 
 def host_fused_emulate(cell: np.ndarray, n_pix: int, chunk_vis: int, vis: np.ndarray):
     """blink_host_fused_emulate: phase S of the shared-memory route walked on the host (no GPU)."""
-    lib = load()
+    lib = load_testing()
     cell = np.ascontiguousarray(cell, np.int32)
     vis = np.ascontiguousarray(vis, np.complex64)
     n_bl = cell.shape[0]
@@ -170,7 +189,7 @@ def host_residue_emulate(cell: np.ndarray, n_pix: int, weighting: int, vis: np.n
     """blink_host_residue_emulate: the residue-class kernels (N = 1024: k_img1024r; 2048 / 4096: k_cols_res +
     plain row sums) walked on the host (no GPU); returns the image rows of the listed units as
     {row index: float32[n_pix]}."""
-    lib = load()
+    lib = load_testing()
     cell = np.ascontiguousarray(cell, np.int32)
     vis = np.ascontiguousarray(vis, np.complex64)
     units = np.ascontiguousarray(units, np.int32)
@@ -194,7 +213,7 @@ def host_residue_emulate(cell: np.ndarray, n_pix: int, weighting: int, vis: np.n
 def probe_fp32(op: int, iters: int, out, stream=None) -> int:
     """blink_probe_fp32 (include/blink_testing.h): launches the fp32 peak probe on `out` (cuda float32
     scratch), returns the flops of the launch; the caller times it."""
-    lib = load()
+    lib = load_testing()
     flops = ctypes.c_int64(0)
     _check(lib.blink_probe_fp32(int(op), int(iters), out.data_ptr(), out.numel(), ctypes.byref(flops),
                                 _stream_ptr(stream)), "blink_probe_fp32")

@@ -1,4 +1,5 @@
-"""Build libblink.so (the C-ABI library, include/blink.h) for sm_100a, in-tree.
+"""Build libblink.so (the C-ABI library, include/blink.h) and libblink_testing.so (the same plus the test hooks of
+include/blink_testing.h) for sm_100a, in-tree.
 
     python -m paper_2405_13478_b200.build [--force]
 
@@ -23,11 +24,18 @@ OBJ_DIR = os.path.join(HERE, "build")
 
 
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not (os.path.exists(LIB) and os.path.exists(os.path.join(HERE, "libblink_testing.so"))):
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
+
+
+# translation units that also hold test hooks (include/blink_testing.h) behind BLINK_TESTING_HOOKS: compiled a
+# second time with the macro for libblink_testing.so -- the same library plus the host models and the fp32
+# probe.  libblink.so itself is the product ABI (include/blink.h) only: no CPU model of any kernel is in it.
+HOOK_SOURCES = ["blink_plan.cu", "blink_fused.cu", "blink_image_r.cu", "blink_probe.cu"]
+TESTING_LIB = os.path.join(HERE, "libblink_testing.so")
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -37,24 +45,30 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ_DIR, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
 
-    def compile_one(src):          # one translation unit -> object file (the units compile in parallel)
-        obj = os.path.join(OBJ_DIR, src.replace(".cu", ".o"))
-        cmd = [nvcc] + NVCC_FLAGS + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
-        return obj, subprocess.run(cmd, capture_output=True, text=True)
+    def compile_one(job):          # one translation unit -> object file (the units compile in parallel)
+        src, hooks = job
+        obj = os.path.join(OBJ_DIR, src.replace(".cu", ".hooks.o" if hooks else ".o"))
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-DBLINK_TESTING_HOOKS"] if hooks else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
+        return src, hooks, obj, subprocess.run(cmd, capture_output=True, text=True)
 
+    jobs = [(s, False) for s in SOURCES if s != "blink_probe.cu"] + [(s, True) for s in HOOK_SOURCES]
     from concurrent.futures import ThreadPoolExecutor
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        results = list(ex.map(compile_one, SOURCES))
-    for _, res in results:
+    with ThreadPoolExecutor(max_workers=len(jobs)) as ex:
+        results = list(ex.map(compile_one, jobs))
+    for *_, res in results:
         if verbose or res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)
-    if any(res.returncode != 0 for _, res in results):
+    if any(res.returncode != 0 for *_, res in results):
         raise RuntimeError("nvcc failed building libblink.so")
-    link = subprocess.run([nvcc, "-shared", "-Xcompiler", "-pthread", "-gencode", "arch=compute_100a,code=sm_100a"] +
-                          [obj for obj, _ in results] + ["-o", LIB], capture_output=True, text=True)
-    if link.returncode != 0:
-        sys.stderr.write(link.stdout + link.stderr)
-        raise RuntimeError("nvcc failed linking libblink.so")
+    product = [obj for _, hooks, obj, _ in results if not hooks]
+    testing = [obj for src, hooks, obj, _ in results if hooks] + \
+              [obj for src, hooks, obj, _ in results if not hooks and src not in HOOK_SOURCES]
+    for objs, lib in ((testing, TESTING_LIB), (product, LIB)):      # libblink.so last: _stale() looks at it
+        link = subprocess.run([nvcc, "-shared", "-Xcompiler", "-pthread", "-gencode", "arch=compute_100a,code=sm_100a"] +
+                              objs + ["-o", lib], capture_output=True, text=True)
+        if link.returncode != 0:
+            sys.stderr.write(link.stdout + link.stderr)
+            raise RuntimeError(f"nvcc failed linking {os.path.basename(lib)}")
     return LIB
 
 

@@ -364,6 +364,7 @@ extern "C" int blink_grid_image(const blink_plan *plan, const void *vis, int n_t
   return blink::launch_grid_image(plan, (const float2 *)vis, n_t, (float *)images, (cudaStream_t)stream);
 }
 
+#ifdef BLINK_TESTING_HOOKS   // libblink_testing.so only (build.py): libblink.so carries no host model and no probe
 // Host emulation of phase S of k_fused for ONE channel (tests without a GPU): builds the gather
 // tables exactly as fused_build does for chunks of chunk_vis baselines, then walks them the way a
 // warp does over a byte-for-byte model of shared memory.
@@ -425,3 +426,4 @@ extern "C" int blink_host_fused_emulate(const int32_t *cell, int n_bl, int n_pix
   if (stats) { stats[0] = g.n_can; stats[1] = (int32_t)groups; stats[2] = (int32_t)rows; }
   return BLINK_OK;
 }
+#endif  // BLINK_TESTING_HOOKS

@@ -677,6 +677,7 @@ int launch_cols_res(const blink_plan *p, const ImgParams &ip, int n_snap, cudaSt
 
 }  // namespace blink
 
+#ifdef BLINK_TESTING_HOOKS   // libblink_testing.so only (build.py): libblink.so carries no host model and no probe
 // Host model of the residue-class kernels for ONE channel and ONE snapshot (tests without a GPU): builds the
 // tables exactly as res_route_build does and walks them the way the kernels do -- phase G (cell values from
 // the records), phase S (lane lists -> bins; the tile starts as NaN, so a bin read that was never written
@@ -815,3 +816,4 @@ extern "C" int blink_host_residue_emulate(const int32_t *cell, int n_bl, int n_p
   }
   return BLINK_OK;
 }
+#endif  // BLINK_TESTING_HOOKS

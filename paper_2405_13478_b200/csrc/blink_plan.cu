@@ -239,6 +239,7 @@ extern "C" const char *blink_strerror(int status) {
 
 extern "C" const char *blink_last_cuda_error(void) { return g_cuda_err.c_str(); }
 
+#ifdef BLINK_TESTING_HOOKS   // libblink_testing.so only (build.py): libblink.so carries no host model and no probe
 extern "C" int blink_host_build_gather(const int32_t *cell, int n_bl, int n_pix, int32_t *n_can_out,
                                        int32_t *can_cell, int32_t *seg_start, int32_t *src) {
   if (!cell || n_bl < 0 || n_pix < 2 || (n_pix & 1) || !n_can_out || !can_cell || !seg_start || !src)
@@ -252,6 +253,7 @@ extern "C" int blink_host_build_gather(const int32_t *cell, int n_bl, int n_pix,
   std::copy(g.src.begin(), g.src.end(), src);
   return g.n_kept;
 }
+#endif  // BLINK_TESTING_HOOKS
 
 extern "C" int blink_plan_create(blink_plan **out, const double *ant_enu_m, int n_ant,
                                  const double *freq_hz, int n_ch, int n_pix, double pixscale,

@@ -2,6 +2,7 @@
 // the denominator of bench.py's ALU side bound.  Not on the hot path: a register-only kernel whose
 // threads run eight independent dependency chains of one instruction kind, so the fp32 pipe is the only
 // limit.  bench.py times the launch with CUDA events and divides *flops by the time.
+#ifdef BLINK_TESTING_HOOKS   // libblink_testing.so only (build.py): libblink.so carries no host model and no probe
 #include "blink_internal.h"
 
 namespace blink {
@@ -75,3 +76,4 @@ extern "C" int blink_probe_fp32(int op, int iters, void *out_dev, size_t out_flo
   *flops = (int64_t)blocks * 256 * (int64_t)iters * 64 * kFlopsPerOp[op];
   return BLINK_OK;
 }
+#endif  // BLINK_TESTING_HOOKS

@@ -1,11 +1,14 @@
 """Text summary of one kernel of an Nsight Compute report, for profiles/ (bench.py reads the DRAM
 traffic of its `roofline.traffic` from such a file).
 
-    python -m paper_2405_13478_b200.ncu_summary REPORT.ncu-rep [KERNEL_SUBSTRING] > profiles/NAME_summary.txt
+    python -m paper_2405_13478_b200.ncu_summary REPORT.ncu-rep [KERNEL_SUBSTRING [SNAPSHOTS_IN_LAUNCH]] > profiles/NAME_summary.txt
 
 Runs `ncu -i REPORT --page raw --csv`, takes the LAST launch whose kernel name contains the substring
 (default: the last launch in the report) and prints `metric  value  unit` lines for the metrics a
-roofline argument needs, then the warp-stall reasons sorted by weight."""
+roofline argument needs, then the warp-stall reasons sorted by weight.  Two comment lines go in front for
+bench.py: `# kernel_sources_sha16` (hash of csrc/ at capture time: bench.py flags a summary older than the
+kernels) and, when given, `# snapshots_in_launch` (a capture of ONE launch pair of a chunked route, to be scaled
+to the step).  A development tool, kept here because the files under profiles/ name it as their command."""
 from __future__ import annotations
 
 import csv
@@ -40,6 +43,12 @@ def main(argv):
         raise SystemExit(f"no launch matching {sub!r}")
     r = pick[-1]
     print(f"# {r[kcol]}  (launch {len(pick)} of {len(pick)} matching {sub!r}; report {rep})")
+    import os
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    from bench import kernel_sources_sha16
+    print(f"# kernel_sources_sha16 {kernel_sources_sha16()}")
+    if len(argv) > 3:
+        print(f"# snapshots_in_launch {int(argv[3])}")
     for name in WANT:
         if name in head:
             i = head.index(name)

@@ -25,15 +25,25 @@ def blink():
 
 
 def test_library_exports_every_declared_symbol(blink):
-    lib = blink.load()
+    """libblink.so exports exactly the product ABI of include/blink.h and none of the test hooks;
+    libblink_testing.so (same sources + BLINK_TESTING_HOOKS) exports both headers' names."""
+    lib, tlib = blink.load(), blink.load_testing()
+    declared = {}
     for header, names in (("blink.h", blink.EXPORTS), ("blink_testing.h", blink.TESTING_EXPORTS)):
         hdr = open(os.path.join(ROOT, "include", header)).read()
         hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-        declared = set(re.findall(r"\b(blink_[a-z0-9_]+)\s*\(", hdr))
-        assert declared, "no declarations parsed"
-        for name in declared:
-            assert hasattr(lib, name), f"{name} declared in {header} but not exported"
-        assert declared == set(names)
+        declared[header] = set(re.findall(r"\b(blink_[a-z0-9_]+)\s*\(", hdr))
+        assert declared[header], "no declarations parsed"
+        assert declared[header] == set(names)
+    for name in declared["blink.h"]:
+        assert hasattr(lib, name), f"{name} declared in blink.h but not exported by libblink.so"
+        assert hasattr(tlib, name), f"{name} missing from libblink_testing.so"
+    for name in declared["blink_testing.h"]:
+        assert hasattr(tlib, name), f"{name} declared in blink_testing.h but not exported by libblink_testing.so"
+        assert not hasattr(lib, name), f"test hook {name} is in the product library"
+    exported = subprocess.run(["nm", "-D", "--defined-only", blink.LIB_PATH], capture_output=True, text=True).stdout
+    c_names = {ln.split()[-1] for ln in exported.splitlines() if " T blink_" in ln}
+    assert c_names == declared["blink.h"], c_names ^ declared["blink.h"]
     assert lib.blink_version() == 200
     assert ctypes.sizeof(blink.Options) == 64          # blink_options: 8 + 8 int32
     assert lib.blink_strerror(-3).decode().startswith("CUDA")
