@@ -41,7 +41,7 @@
 extern "C" {
 #endif
 
-#define BLINK_VERSION 200 /* 0.2.0 */
+#define BLINK_VERSION 210 /* 0.2.1: + blink_image_static, BLINK_ECAPACITY, BLINK_Q_FUSED_NZ / _D; test hooks in libblink_testing.so */
 
 typedef enum blink_status {
   BLINK_OK = 0,

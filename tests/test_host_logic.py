@@ -44,7 +44,7 @@ def test_library_exports_every_declared_symbol(blink):
     exported = subprocess.run(["nm", "-D", "--defined-only", blink.LIB_PATH], capture_output=True, text=True).stdout
     c_names = {ln.split()[-1] for ln in exported.splitlines() if " T blink_" in ln}
     assert c_names == declared["blink.h"], c_names ^ declared["blink.h"]
-    assert lib.blink_version() == 200
+    assert lib.blink_version() == 210
     assert ctypes.sizeof(blink.Options) == 64          # blink_options: 8 + 8 int32
     assert lib.blink_strerror(-3).decode().startswith("CUDA")
 
@@ -237,3 +237,35 @@ def test_bench_reference_arm_runs_on_cpu_and_prints_the_contract_line():
     other = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "tiny",
                             "--steps", "1", "--warmup", "1"], capture_output=True, text=True, timeout=300, env=env)
     assert other.returncode == 0 and other.stdout.strip() == ""      # the other ranks exit 0 without work
+
+
+def test_bench_traffic_comes_from_summaries_of_the_current_kernels(tmp_path, monkeypatch):
+    """bench.py's `roofline.traffic` is read from committed ncu summaries: every workload of the default line
+    must resolve to files of the newest round, summed over the kernels of its step (mwa2: two kernels, one
+    launch pair scaled to the step), and a summary captured before a kernel change must be flagged -- the
+    committed ones must not be: after editing csrc/, re-capture (profiles/r03_README.md has the commands)."""
+    import bench
+    steps = {"station": 3200, "mwa1": 2400, "mwa2": 480, "sweep128": 4000, "sweep256": 4000, "sweep512": 4000,
+             "sweep1024": 4000}
+    for name, n_snap in steps.items():
+        w = bench.make_workload(name)
+        assert w.n_snapshots == n_snap
+        traffic, src = bench.ncu_traffic(name, "fused", n_snap)
+        assert traffic is not None and src, f"no committed full-size ncu summary for {name}"
+        alg = bench.algorithmic_bytes(w)["fused"] * n_snap
+        assert 0.9 * alg <= traffic <= 2.0 * alg, (name, traffic, alg)
+        for f in src:
+            assert f["stale"] is False, f"{f['file']} was captured before the last change under csrc/: re-capture it"
+    _, src = bench.ncu_traffic("mwa2", "fused", 480)
+    assert len(src) == 2 and all(abs(f["scaled_by"] - 480 / 75) < 1e-12 for f in src)
+    # the flag itself: a copy of a summary with another source hash reads as stale, one without a hash as unknown
+    prof = tmp_path / "profiles"
+    prof.mkdir()
+    txt = open(os.path.join(ROOT, src[0]["file"])).read()
+    (prof / "r09_x_fused_fullsize_summary.txt").write_text(re.sub(r"(# kernel_sources_sha16) \w+", r"\1 0123456789abcdef", txt))
+    (prof / "r09_y_fused_fullsize_summary.txt").write_text(re.sub(r"# kernel_sources_sha16 \w+\n", "", txt))
+    monkeypatch.setattr(bench, "ROOT", str(tmp_path))
+    monkeypatch.setattr(bench, "kernel_sources_sha16", lambda: "f" * 16)
+    assert bench.ncu_traffic("x", "fused", 75)[1][0]["stale"] is True
+    assert str(bench.ncu_traffic("y", "fused", 75)[1][0]["stale"]).startswith("unknown")
+    assert bench.ncu_traffic("z", "fused", 75) == (None, None)
