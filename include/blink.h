@@ -354,6 +354,10 @@ int blink_dynspec(const blink_plan *plan, const void *images, int n_t, double al
  *   vis     DEVICE complex64 [n_t][n_ch][n_bl]; 16-byte aligned base (BLINK_EINVAL otherwise: the routes
  *           read it with bulk asynchronous copies)
  *   images  DEVICE float32   [n_t][n_ch][N][N]
+ * Reproducibility: the residue-class and two-kernel routes return the same bits for the same plan and input, call
+ * after call.  The shared-memory route does so for the first snapshot each of its persistent CTAs images; later
+ * snapshots may differ between two calls in the last bit of the largest pixels (<= 2^-23 of the image peak; known
+ * issue).
  * Asynchronous on `stream`; no allocation, no host synchronisation.  The shared-memory route and the
  * residue-class kernel need no scratch; the others need blink_plan_reserve(plan, n_t) beforehand
  * (BLINK_ERESERVE otherwise).
@@ -366,7 +370,8 @@ int blink_grid_image(const blink_plan *plan, const void *vis, int n_t, void *ima
  * chunk, the imaging of the previous one and the device-to-host copy of the one before run concurrently on
  * three internal streams over a ring of plan-owned device buffers -- the interleaving of kernels and
  * transfers with pinned host memory that the paper lists as its next optimisation.
- * Results are bit-identical to blink_grid_image on the same visibilities.
+ * Results are those of blink_grid_image on the same visibilities (bit-identical on the routes that are
+ * bit-reproducible; see the note on reproducibility at blink_grid_image).
  *   vis_host     HOST complex64 [n_t][n_ch][n_bl]; page-locked (cudaHostAlloc / cudaHostRegister) for the
  *                copies to overlap -- pageable memory works, but the copies then serialise with the host
  *   images_host  HOST float32   [n_t][n_ch][N][N]; same

@@ -478,6 +478,55 @@ def test_every_fused_instance_against_oracle(torch_cuda, blink, oracle, sx, sy, 
     plan.close()
 
 
+def test_fused_handover_at_128_plain_corrected_and_ring_grid(torch_cuda, blink, oracle):
+    """180 snapshots of 128^2 over 148 persistent CTAs: every CTA of k_fused<128> hands its chunk ring and its
+    aliased line buffers from one snapshot to the next (plain, then with the correction factors riding in the
+    chunks), and blink_grid runs its ring route on the same batch.  Against the oracle on the snapshots around
+    the hand-over, against the two-call route on every pixel, twice (call-to-call agreement).  (These were the
+    shared-memory cases of the former stress script tests/sanitizer_targets.py; compute-sanitizer is closed on
+    this pool, so result comparison is the check there is.)"""
+    torch = torch_cuda
+    from oracle import corrections as oc
+    w = synth.config_station(n_t=60, n_ch=3, n_pix=128)
+    vis_h = w.vis()
+    vis = torch.from_numpy(vis_h).cuda()
+    n_snap = w.n_t * w.n_ch
+    ant, gains, cables = _corr_inputs(w, 43)
+    plan = blink.Plan(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting, options=dict(grid_ring_min_snap=1))
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 1 and plan.query_i32(blink.Q_FUSED_NZ) == 8
+    sel = np.array([0, 31, 147, 148, 149, n_snap - 1], np.int64)
+    dsel = torch.from_numpy(sel).cuda()
+
+    def run_and_check(vis_ref, what):
+        img = torch.full((w.n_t, w.n_ch, 128, 128), float("nan"), dtype=torch.float32, device="cuda")
+        plan.grid_image(vis, img)
+        again = torch.full_like(img, float("nan"))
+        plan.grid_image(vis, again)
+        two = plan.image(plan.grid(vis))                              # ring-route blink_grid + blink_image
+        torch.cuda.synchronize()
+        assert torch.isfinite(img).all(), what
+        # call to call: NOT asserted bit-identical.  Round 3 found that a few snapshots a CTA images after its
+        # first one differ between two calls in the last bit of the largest pixels (<= 2^-23 of the peak; DESIGN.md
+        # section 7 "Known issue"); anything beyond that level would be a corrupted buffer and fails here
+        pk = img.abs().amax(dim=(-2, -1), keepdim=True)
+        assert ((img - again).abs() <= 2.5e-7 * pk).all(), what
+        assert ((img - two).abs() <= 1e-5 * two.abs().amax(dim=(-2, -1), keepdim=True)).all(), what
+        ref = oracle.image_batch(ant, w.freq_hz, w.n_pix, w.pixscale, w.weighting, vis_ref, sel)
+        got = img.view(n_snap, 128, 128)[dsel].cpu().numpy()
+        for q in range(len(sel)):
+            peak = np.max(np.abs(ref["images"][q]))
+            assert np.max(np.abs(got[q] - ref["images"][q])) <= IMG_TOL * peak, f"{what}, snapshot {sel[q]}"
+
+    run_and_check(vis_h, "plain")
+    l0, m0 = 0.1, 0.2
+    plan.set_corrections(gains, cables, l0, m0)
+    plan.apply_corrections(True)
+    assert plan.query_i32(blink.Q_FUSED_PATH) == 1
+    F_ref = oc.correction_factors(ant, w.freq_hz, gains, cables, l0, m0)
+    run_and_check(oc.apply_corrections(vis_h, F_ref).astype(np.complex64), "corrections fused at load")
+    plan.close()
+
+
 def test_corrections_fused_into_the_tensor_core_kernel_against_oracle(torch_cuda, blink, oracle):
     """f2 fused at load on k_fused_tc<true> against the ORACLE chain (the other test compares it with k_fused)."""
     torch = torch_cuda
